@@ -1,0 +1,184 @@
+/* ws.h - C ABI of libwanstream: block-causal streaming attention over a paged per-session KV cache.
+ *
+ * The hot path of Wan-Streamer's streaming inference (arxiv 2606.25041): once per 160 ms streaming
+ * unit a newly arrived block of interleaved visual/audio/text tokens (PAPER.md:11 Abstract, :29 §1,
+ * :45 §2.1) is (1) committed to the session's full-history KV cache ("appends the received KV slice
+ * into its own full-history cache"; also :29, :31, :51, :59) and (2) attends
+ * block-causally to it: bidirectionally within its own block, causally to all earlier blocks
+ * (PAPER.md:11, :23 Fig. 1, :29, :38, :155; dependence structure of Eq. (1)).
+ * The paper gives no formula, sizes or dtype; the readings taken are listed in DESIGN.md §2.
+ *
+ * Conventions
+ *  - All functions return ws_status_t (WS_OK = 0). No exceptions, no abort(), nothing on stdout.
+ *    ws_last_error() returns a thread-local human-readable message for the last failure.
+ *  - "HOST" pointers are read before the call returns (the caller may reuse them immediately).
+ *    "DEVICE" pointers are CUDA device memory on `device`; they are CALLER-owned (the Python
+ *    harness allocates them as torch tensors) and only borrowed by the library.
+ *  - Calls enqueue their work on the given CUDA stream (a cudaStream_t passed as void*) and return
+ *    without synchronising.  All calls on one cache must use one stream (or be externally ordered).
+ *  - Arguments are validated BEFORE any state changes: on any error no session length, page table,
+ *    block boundary or free-list entry has changed (strong guarantee).
+ *  - One cache handle = one attention layer.  There is NO CPU fallback: without a CUDA device every
+ *    compute entry point fails with WS_ERR_CUDA (except under WS_FLAG_DRY_RUN, see below).
+ *
+ * Layouts (element = bf16 or fp32 according to `dtype`)
+ *  - K/V pools:   [num_pages][num_kv_heads][page_tokens][head_dim]   (one (page, head) slab is a
+ *                 dense page_tokens x head_dim matrix - TMA-addressable as a rank-4 tensor)
+ *  - k_new/v_new: [sum n][num_kv_heads][head_dim], token-major, contiguous
+ *  - q / out:     [sum n_q][num_q_heads][head_dim], token-major, contiguous
+ *  - lse:         [sum n_q][num_q_heads] fp32, natural log
+ *  - GQA: query head h reads KV head q_to_kv_head[h] (default h / (num_q_heads/num_kv_heads)).
+ */
+#ifndef WS_H_
+#define WS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  WS_OK = 0,
+  WS_ERR_INVALID_ARG = 1,        /* null pointer, bad size, duplicate session in one call, ...     */
+  WS_ERR_BAD_SESSION = 2,        /* session id not open                                            */
+  WS_ERR_OUT_OF_PAGES = 3,       /* free list (or per-session page/block capacity) exhausted       */
+  WS_ERR_UNSUPPORTED = 4,        /* shape/dtype combination no kernel covers                       */
+  WS_ERR_WORKSPACE_TOO_SMALL = 5,
+  WS_ERR_CUDA = 6                /* a CUDA call failed (message in ws_last_error())                */
+} ws_status_t;
+
+typedef enum { WS_BF16 = 0, WS_F32 = 1 } ws_dtype_t;
+
+enum {
+  /* Host metadata only: no CUDA call is ever made (pools/workspace may be NULL).  For testing the
+   * page allocator, scheduler and error paths on a machine without a GPU.  Compute is skipped.     */
+  WS_FLAG_DRY_RUN = 1u,
+  /* Debug: route bf16 attention through the generic SIMT kernel instead of the tcgen05 kernel.     */
+  WS_FLAG_FORCE_SIMT = 2u
+};
+
+typedef struct ws_cache ws_cache_t;   /* opaque; owns host metadata only */
+
+typedef struct {
+  int32_t dtype;                  /* ws_dtype_t                                                    */
+  int32_t num_q_heads;            /* Hq                                                            */
+  int32_t num_kv_heads;           /* Hkv, Hq % Hkv == 0                                            */
+  int32_t head_dim;               /* D: bf16 tensor-core path D = 128; generic path D <= 256, D%8==0 */
+  const int32_t* q_to_kv_head;    /* HOST [Hq] or NULL = grouped default                           */
+  int32_t page_tokens;            /* P: tokens per page (64 for the bf16 tensor-core path)         */
+  int32_t num_pages;              /* pages in each pool                                            */
+  int32_t max_sessions;           /* session slots                                                 */
+  int32_t max_pages_per_session;  /* device page-table row length                                  */
+  int32_t max_blocks_per_session; /* block-boundary capacity per session                           */
+  int32_t max_sessions_per_call;  /* upper bounds used to size the workspace                       */
+  int32_t max_q_tokens_per_call;
+  void*   k_pool;                 /* DEVICE, >= ws_pool_bytes() each                               */
+  void*   v_pool;
+  size_t  pool_bytes;
+  void*   workspace;              /* DEVICE scratch: page tables, per-call metadata, split partials */
+  size_t  workspace_bytes;        /* >= ws_workspace_bytes()                                       */
+  int32_t device;                 /* CUDA device ordinal                                           */
+  uint32_t flags;                 /* WS_FLAG_*                                                     */
+} ws_cache_config_t;
+
+/* Bytes each of k_pool / v_pool must hold: num_pages * Hkv * P * D * sizeof(element). */
+size_t ws_pool_bytes(const ws_cache_config_t* cfg);
+/* Bytes of DEVICE workspace the configuration needs (0 if cfg is invalid). */
+size_t ws_workspace_bytes(const ws_cache_config_t* cfg);
+
+/* Create a cache over caller-owned pools.  Does not touch pool contents.  The device page tables
+ * inside `workspace` are initialised on the legacy default stream and synchronised before return. */
+ws_status_t ws_cache_create(const ws_cache_config_t* cfg, ws_cache_t** out);
+/* Destroys host metadata; never frees caller memory.  Synchronises the device first. */
+ws_status_t ws_cache_destroy(ws_cache_t* cache);
+
+ws_status_t ws_session_open(ws_cache_t* cache, int32_t* session_out);
+/* Returns the session's pages to the free list. */
+ws_status_t ws_session_close(ws_cache_t* cache, int32_t session);
+/* Committed tokens, committed blocks, and a library-owned HOST view of the block ends
+ * e_1 < ... < e_B (valid until the next mutating call on this cache).  Any out-pointer may be NULL. */
+ws_status_t ws_session_info(const ws_cache_t* cache, int32_t session, int64_t* tokens,
+                            int32_t* blocks, const int64_t** block_ends);
+/* Roll a session back to its first `keep_blocks` committed blocks (pages beyond go back to the free
+ * list; cache contents of kept blocks are untouched).  Used to replay a streaming loop. */
+ws_status_t ws_session_truncate(ws_cache_t* cache, int32_t session, int32_t keep_blocks);
+/* Number of pages currently on the free list. */
+int32_t ws_free_pages(const ws_cache_t* cache);
+
+/* a2 - KV append / commit.  Appends ONE block per listed session:
+ *   Kc[L_s : L_s+n_s] <- k_new[cu[s] : cu[s+1]]  (same for V), bit-exact, then L_s += n_s and a block
+ *   boundary e = L_s is recorded.  n_s >= 1.
+ * session_ids: HOST [S] distinct open sessions; cu_new_tokens: HOST [S+1] prefix offsets (cu[0]=0);
+ * k_new, v_new: DEVICE [cu[S]][Hkv][D]; modality: HOST [cu[S]] tags 0=video 1=audio 2=text or NULL
+ * (stored as metadata only - it never changes the result, reading A4/A5). */
+ws_status_t ws_kv_append(ws_cache_t* cache, int32_t num_sessions, const int32_t* session_ids,
+                         const int32_t* cu_new_tokens, const void* k_new, const void* v_new,
+                         const uint8_t* modality, void* cuda_stream);
+
+/* a3 (+a4) - block-causal attention forward.  For each listed session the queries are the tokens of
+ * its LAST num_q_blocks[s] committed blocks (1 on the hot path: the block just appended).  A query
+ * row in block b sees keys j < e_b: its whole own block and every earlier block.
+ *   O[r,h,:] = sum_j softmax_j(scale * <Q[r,h,:], Kc[j,g(h),:]>) Vc[j,g(h),:],  LSE = log sum_j e^{s_j}
+ * session_ids: HOST [S]; num_q_blocks: HOST [S] or NULL (= 1 each); cu_q_tokens: HOST [S+1], where
+ * cu[s+1]-cu[s] must equal the token count of those blocks; q: DEVICE; out: DEVICE (same dtype as
+ * the cache); lse: DEVICE fp32 or NULL.  Long caches are split across CTAs and merged by a combine
+ * kernel using the workspace (a4). */
+ws_status_t ws_block_causal_attn_fwd(ws_cache_t* cache, int32_t num_sessions,
+                                     const int32_t* session_ids, const int32_t* num_q_blocks,
+                                     const int32_t* cu_q_tokens, const void* q, void* out,
+                                     float* lse, float scale, void* cuda_stream);
+
+/* One streaming-unit step with HOST buffers (the end-to-end path): copies q/k_new/v_new from host
+ * (pinned for async copies) into `staging` (DEVICE, >= ws_step_staging_bytes(n_total)), runs
+ * ws_kv_append then ws_block_causal_attn_fwd (one block per session, n_q = n_new), and copies the
+ * result back to out_host.  Returns after enqueueing; the caller synchronises the stream. */
+size_t ws_step_staging_bytes(const ws_cache_config_t* cfg, int32_t total_new_tokens);
+ws_status_t ws_stream_step_host(ws_cache_t* cache, int32_t num_sessions, const int32_t* session_ids,
+                                const int32_t* cu_new_tokens, const void* q_host,
+                                const void* k_new_host, const void* v_new_host, void* out_host,
+                                void* staging, size_t staging_bytes, float scale, void* cuda_stream);
+
+/* Read back logical tokens [start, start+count) of a session into contiguous [count][Hkv][D]
+ * DEVICE buffers (either may be NULL).  Test / snapshot utility. */
+ws_status_t ws_kv_gather(const ws_cache_t* cache, int32_t session, int64_t start, int64_t count,
+                         void* k_out, void* v_out, void* cuda_stream);
+
+/* ---- host-logic introspection (no device work; usable under WS_FLAG_DRY_RUN) ------------------ */
+/* Copies the session's physical page ids (HOST) into pages_out[0..cap); returns the count via n. */
+ws_status_t ws_session_pages(const ws_cache_t* cache, int32_t session, int32_t* pages_out,
+                             int32_t cap, int32_t* n);
+/* Deterministically permute the free list (Fisher-Yates, seed) so tests can check that results do
+ * not depend on the physical page assignment. */
+ws_status_t ws_debug_shuffle_free_pages(ws_cache_t* cache, uint64_t seed);
+/* Force the split-KV planner to cut every (session, KV head) group into at least `min_splits`
+ * pieces (0 = automatic).  For split-count invariance tests. */
+ws_status_t ws_debug_set_min_splits(ws_cache_t* cache, int32_t min_splits);
+
+/* Description of the last attention plan built on this cache (a1): CTAs launched, team size,
+ * number of (session,KV-head) groups, KV segments, split partial slots, combine items, and whether
+ * the tcgen05 kernel (1) or the generic SIMT kernel (0) was selected. */
+typedef struct {
+  int32_t num_ctas, team_size, num_groups, num_segments, num_partial_slots, num_combine_items;
+  int32_t used_tensor_core_kernel, total_kv_tiles;
+} ws_plan_info_t;
+ws_status_t ws_last_plan_info(const ws_cache_t* cache, ws_plan_info_t* out);
+/* Segment i of the last plan: group, session, kv_head, first query token, tile range [begin,end),
+ * team, partial slot base (-1 = writes the final output directly). */
+typedef struct {
+  int32_t group, session, kv_head, q_token0, tile_begin, tile_end, team, part_base;
+} ws_plan_segment_t;
+ws_status_t ws_last_plan_segment(const ws_cache_t* cache, int32_t i, ws_plan_segment_t* out);
+
+/* Number of kernels this library has launched on `cache` since creation (bench `gpu_launches`). */
+int64_t ws_launch_count(const ws_cache_t* cache);
+
+const char* ws_status_str(ws_status_t s);
+const char* ws_last_error(void);
+const char* ws_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WS_H_ */

@@ -1,0 +1,618 @@
+// api.cu - the C ABI declared in include/ws.h: argument validation, host metadata (a1), per-call
+// metadata staging, TMA descriptor creation and kernel launches.  No arithmetic of the method runs
+// on the host; there is no CPU fallback.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <memory>
+#include <string>
+#include <vector>
+
+#include "../../include/ws.h"
+#include "host_cache.h"
+#include "launch.h"
+#include "plan.h"
+#include "ws_internal.h"
+
+namespace {
+
+thread_local std::string g_err;
+
+ws_status_t fail(ws_status_t st, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return st;
+}
+
+#define WS_CUDA(expr)                                                                   \
+  do {                                                                                  \
+    cudaError_t e__ = (expr);                                                           \
+    if (e__ != cudaSuccess)                                                             \
+      return fail(WS_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(e__));        \
+  } while (0)
+
+constexpr int kRing = 8;            // per-call metadata slots in flight
+constexpr int kDefaultSms = 148;    // B200 (used for dry-run planning)
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+int eb_of(int32_t dtype) { return dtype == WS_BF16 ? 2 : 4; }
+
+bool config_valid(const ws_cache_config_t* c, const char** why) {
+  auto bad = [&](const char* w) { *why = w; return false; };
+  if (!c) return bad("cfg is NULL");
+  if (c->dtype != WS_BF16 && c->dtype != WS_F32) return bad("dtype");
+  if (c->num_q_heads < 1 || c->num_kv_heads < 1 || c->num_q_heads % c->num_kv_heads)
+    return bad("num_q_heads must be a positive multiple of num_kv_heads");
+  if (c->head_dim < 8 || c->head_dim > 256 || c->head_dim % 8) return bad("head_dim in [8,256], %8");
+  if (c->page_tokens < 1 || c->num_pages < 1) return bad("page_tokens / num_pages");
+  if (c->max_sessions < 1 || c->max_pages_per_session < 1 || c->max_blocks_per_session < 1)
+    return bad("max_sessions / max_pages_per_session / max_blocks_per_session");
+  if (c->max_sessions_per_call < 1 || c->max_q_tokens_per_call < 1)
+    return bad("max_sessions_per_call / max_q_tokens_per_call");
+  if ((int64_t)c->num_pages * c->num_kv_heads * c->page_tokens >= (1ll << 31))
+    return bad("pool has more than 2^31 (token, head) rows");
+  return true;
+}
+
+struct Layout {
+  size_t page_table, q_to_kv, meta, part_lse, part_o, total;
+  size_t meta_slot_bytes;
+  int32_t max_part_slots;
+};
+
+Layout make_layout(const ws_cache_config_t* c, int num_sms) {
+  Layout L{};
+  const int G = c->num_q_heads / c->num_kv_heads;
+  size_t off = 0;
+  L.page_table = off; off = align_up(off + (size_t)c->max_sessions * c->max_pages_per_session * 4, 256);
+  L.q_to_kv = off;    off = align_up(off + (size_t)c->num_q_heads * 4, 256);
+  const int64_t S = c->max_sessions_per_call, NQ = c->max_q_tokens_per_call;
+  int64_t groups = (int64_t)c->num_kv_heads * (2 * S + NQ * G / 2048 + 1);
+  int64_t words = 1024 + groups * 64 + 16 * (int64_t)num_sms + 2 * NQ + 8 * S +
+                  S * (NQ / c->page_tokens + 3) + NQ / c->page_tokens;
+  L.meta_slot_bytes = align_up((size_t)words * 4, 256);
+  L.meta = off;       off = align_up(off + L.meta_slot_bytes * kRing, 256);
+  L.max_part_slots = 4 * num_sms + 64;
+  L.part_lse = off;   off = align_up(off + (size_t)L.max_part_slots * ws::kPairRows * 4, 256);
+  L.part_o = off;     off = align_up(off + (size_t)L.max_part_slots * ws::kPairRows * c->head_dim * 4, 256);
+  L.total = off;
+  return L;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+struct ws_cache {
+  ws_cache_config_t cfg{};
+  std::vector<int32_t> q_to_kv;       // explicit map (empty = default)
+  bool default_map = true;
+  std::unique_ptr<ws::HostCache> host;
+  Layout lay{};
+  int num_sms = kDefaultSms;
+  bool dry = false;
+  bool tensor_path_ok = false;
+  // device views into the caller's workspace
+  int32_t* d_page_table = nullptr;
+  int32_t* d_q_to_kv = nullptr;
+  char* d_meta = nullptr;
+  float* d_part_lse = nullptr;
+  float* d_part_o = nullptr;
+  // pinned staging ring
+  char* h_meta = nullptr;
+  cudaEvent_t ev[kRing]{};
+  bool ev_pending[kRing]{};
+  int ring_pos = 0;
+  EncodeTiledFn encode = nullptr;
+  CUtensorMap tmap_k{}, tmap_v{};
+  int32_t min_splits = 0;
+  int64_t launches = 0;
+  ws::Plan last_plan;
+  bool last_tensor = false;
+};
+
+namespace {
+
+// Reserve the next metadata slot: returns host staging pointer; *dev gets the device address.
+ws_status_t next_slot(ws_cache* c, size_t bytes, char** host, char** dev) {
+  if (bytes > c->lay.meta_slot_bytes)
+    return fail(WS_ERR_WORKSPACE_TOO_SMALL, "per-call metadata (%zu B) exceeds the slot (%zu B)",
+                bytes, c->lay.meta_slot_bytes);
+  int i = c->ring_pos;
+  c->ring_pos = (c->ring_pos + 1) % kRing;
+  if (!c->dry && c->ev_pending[i]) {
+    WS_CUDA(cudaEventSynchronize(c->ev[i]));
+    c->ev_pending[i] = false;
+  }
+  *host = c->h_meta + (size_t)i * c->lay.meta_slot_bytes;
+  *dev = c->d_meta ? c->d_meta + (size_t)i * c->lay.meta_slot_bytes : nullptr;
+  return WS_OK;
+}
+
+ws_status_t upload_slot(ws_cache* c, const char* host, char* dev, size_t bytes, cudaStream_t st) {
+  if (c->dry) return WS_OK;
+  int i = (int)((host - c->h_meta) / c->lay.meta_slot_bytes);
+  WS_CUDA(cudaMemcpyAsync(dev, host, bytes, cudaMemcpyHostToDevice, st));
+  WS_CUDA(cudaEventRecord(c->ev[i], st));
+  c->ev_pending[i] = true;
+  return WS_OK;
+}
+
+ws_status_t encode_tmap(ws_cache* c, CUtensorMap* out, void* base, int rank, const cuuint64_t* dims,
+                        const cuuint64_t* strides_bytes, const cuuint32_t* box) {
+  cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  CUresult r = c->encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, base, dims,
+                         strides_bytes, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(WS_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+  return WS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t ws_pool_bytes(const ws_cache_config_t* cfg) {
+  const char* why;
+  if (!config_valid(cfg, &why)) return 0;
+  return (size_t)cfg->num_pages * cfg->num_kv_heads * cfg->page_tokens * cfg->head_dim *
+         eb_of(cfg->dtype);
+}
+
+size_t ws_workspace_bytes(const ws_cache_config_t* cfg) {
+  const char* why;
+  if (!config_valid(cfg, &why)) return 0;
+  int sms = kDefaultSms;
+  if (!(cfg->flags & WS_FLAG_DRY_RUN)) {
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, cfg->device) == cudaSuccess && v > 0)
+      sms = v;
+    else
+      (void)cudaGetLastError();
+  }
+  return make_layout(cfg, sms).total;
+}
+
+ws_status_t ws_cache_create(const ws_cache_config_t* cfg, ws_cache_t** out) {
+  const char* why = "";
+  if (!out) return fail(WS_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  if (!config_valid(cfg, &why)) return fail(WS_ERR_INVALID_ARG, "invalid config: %s", why);
+  std::unique_ptr<ws_cache> c(new ws_cache());
+  c->cfg = *cfg;
+  c->dry = (cfg->flags & WS_FLAG_DRY_RUN) != 0;
+  const int G = cfg->num_q_heads / cfg->num_kv_heads;
+  if (cfg->q_to_kv_head) {
+    c->q_to_kv.assign(cfg->q_to_kv_head, cfg->q_to_kv_head + cfg->num_q_heads);
+    for (int h = 0; h < cfg->num_q_heads; ++h) {
+      if (c->q_to_kv[h] < 0 || c->q_to_kv[h] >= cfg->num_kv_heads)
+        return fail(WS_ERR_INVALID_ARG, "q_to_kv_head[%d] out of range", h);
+      if (c->q_to_kv[h] != h / G) c->default_map = false;
+    }
+  }
+  c->cfg.q_to_kv_head = nullptr;
+  c->host.reset(new ws::HostCache(cfg->num_pages, cfg->page_tokens, cfg->max_sessions,
+                                  cfg->max_pages_per_session, cfg->max_blocks_per_session));
+  c->tensor_path_ok = cfg->dtype == WS_BF16 && cfg->head_dim == 128 && cfg->page_tokens == 64 &&
+                      c->default_map && (G == 1 || G == 2 || G == 4 || G == 8 || G == 16);
+  if (c->dry) {
+    c->lay = make_layout(cfg, kDefaultSms);
+    c->h_meta = (char*)malloc(c->lay.meta_slot_bytes * kRing);
+    if (!c->h_meta) return fail(WS_ERR_INVALID_ARG, "out of host memory");
+    *out = c.release();
+    return WS_OK;
+  }
+  if (!cfg->k_pool || !cfg->v_pool || !cfg->workspace)
+    return fail(WS_ERR_INVALID_ARG, "k_pool / v_pool / workspace must be device pointers");
+  if (cfg->pool_bytes < ws_pool_bytes(cfg))
+    return fail(WS_ERR_INVALID_ARG, "pool_bytes %zu < required %zu", cfg->pool_bytes, ws_pool_bytes(cfg));
+  WS_CUDA(cudaSetDevice(cfg->device));
+  int sms = 0;
+  WS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, cfg->device));
+  c->num_sms = sms;
+  c->lay = make_layout(cfg, sms);
+  if (cfg->workspace_bytes < c->lay.total)
+    return fail(WS_ERR_WORKSPACE_TOO_SMALL, "workspace_bytes %zu < required %zu",
+                cfg->workspace_bytes, c->lay.total);
+  char* ws_base = (char*)cfg->workspace;
+  if (((uintptr_t)ws_base & 255) || ((uintptr_t)cfg->k_pool & 255) || ((uintptr_t)cfg->v_pool & 255))
+    return fail(WS_ERR_INVALID_ARG, "pools and workspace must be 256-byte aligned");
+  c->d_page_table = (int32_t*)(ws_base + c->lay.page_table);
+  c->d_q_to_kv = (int32_t*)(ws_base + c->lay.q_to_kv);
+  c->d_meta = ws_base + c->lay.meta;
+  c->d_part_lse = (float*)(ws_base + c->lay.part_lse);
+  c->d_part_o = (float*)(ws_base + c->lay.part_o);
+  WS_CUDA(cudaMemset(c->d_page_table, 0, (size_t)cfg->max_sessions * cfg->max_pages_per_session * 4));
+  if (!c->default_map)
+    WS_CUDA(cudaMemcpy(c->d_q_to_kv, c->q_to_kv.data(), c->q_to_kv.size() * 4, cudaMemcpyHostToDevice));
+  WS_CUDA(cudaHostAlloc((void**)&c->h_meta, c->lay.meta_slot_bytes * kRing, cudaHostAllocDefault));
+  for (int i = 0; i < kRing; ++i) WS_CUDA(cudaEventCreateWithFlags(&c->ev[i], cudaEventDisableTiming));
+  if (c->tensor_path_ok) {
+    int major = 0;
+    WS_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, cfg->device));
+    if (major != 10) {
+      c->tensor_path_ok = false;      // tcgen05 kernel is sm_100a only; generic kernel still runs
+    } else {
+      void* fn = nullptr;
+      cudaDriverEntryPointQueryResult qres;
+      WS_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+      if (!fn || qres != cudaDriverEntryPointSuccess)
+        return fail(WS_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+      c->encode = (EncodeTiledFn)fn;
+      const cuuint64_t D = 128, P = 64, H = cfg->num_kv_heads, NP = cfg->num_pages;
+      cuuint64_t dims[4] = {D, P, H, NP};
+      cuuint64_t strides[3] = {D * 2, P * D * 2, H * P * D * 2};
+      cuuint32_t box[4] = {64, 64, 1, 1};
+      ws_status_t st = encode_tmap(c.get(), &c->tmap_k, cfg->k_pool, 4, dims, strides, box);
+      if (st != WS_OK) return st;
+      st = encode_tmap(c.get(), &c->tmap_v, cfg->v_pool, 4, dims, strides, box);
+      if (st != WS_OK) return st;
+      WS_CUDA(ws::sm100_attn_configure());
+    }
+  }
+  WS_CUDA(cudaDeviceSynchronize());
+  *out = c.release();
+  return WS_OK;
+}
+
+ws_status_t ws_cache_destroy(ws_cache_t* c) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  if (c->dry) {
+    free(c->h_meta);
+  } else {
+    (void)cudaDeviceSynchronize();
+    for (int i = 0; i < kRing; ++i)
+      if (c->ev[i]) (void)cudaEventDestroy(c->ev[i]);
+    if (c->h_meta) (void)cudaFreeHost(c->h_meta);
+  }
+  delete c;
+  return WS_OK;
+}
+
+ws_status_t ws_session_open(ws_cache_t* c, int32_t* session_out) {
+  if (!c || !session_out) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  int32_t s = c->host->open_session();
+  if (s < 0) return fail(WS_ERR_BAD_SESSION, "all %d session slots are open", c->cfg.max_sessions);
+  *session_out = s;
+  return WS_OK;
+}
+
+ws_status_t ws_session_close(ws_cache_t* c, int32_t session) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  if (!c->host->close_session(session)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", session);
+  return WS_OK;
+}
+
+ws_status_t ws_session_info(const ws_cache_t* c, int32_t session, int64_t* tokens, int32_t* blocks,
+                            const int64_t** block_ends) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  if (!c->host->is_open(session)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", session);
+  const ws::SessionState& st = c->host->session(session);
+  if (tokens) *tokens = st.tokens;
+  if (blocks) *blocks = (int32_t)st.block_ends.size();
+  if (block_ends) *block_ends = st.block_ends.data();
+  return WS_OK;
+}
+
+ws_status_t ws_session_truncate(ws_cache_t* c, int32_t session, int32_t keep_blocks) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  if (!c->host->is_open(session)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", session);
+  if (!c->host->truncate_blocks(session, keep_blocks))
+    return fail(WS_ERR_INVALID_ARG, "keep_blocks %d out of range", keep_blocks);
+  return WS_OK;
+}
+
+int32_t ws_free_pages(const ws_cache_t* c) { return c ? c->host->free_pages() : -1; }
+
+ws_status_t ws_session_pages(const ws_cache_t* c, int32_t session, int32_t* pages_out, int32_t cap,
+                             int32_t* n) {
+  if (!c || !n) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  if (!c->host->is_open(session)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", session);
+  const auto& pg = c->host->session(session).pages;
+  *n = (int32_t)pg.size();
+  for (int32_t i = 0; i < cap && i < *n && pages_out; ++i) pages_out[i] = pg[i];
+  return WS_OK;
+}
+
+ws_status_t ws_debug_shuffle_free_pages(ws_cache_t* c, uint64_t seed) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  c->host->shuffle_free(seed);
+  return WS_OK;
+}
+
+ws_status_t ws_debug_set_min_splits(ws_cache_t* c, int32_t min_splits) {
+  if (!c || min_splits < 0) return fail(WS_ERR_INVALID_ARG, "bad argument");
+  c->min_splits = min_splits;
+  return WS_OK;
+}
+
+// ------------------------------------------------------------------------------------ a2 append
+ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
+                         const int32_t* cu, const void* k_new, const void* v_new,
+                         const uint8_t* modality, void* cuda_stream) {
+  if (!c || !session_ids || !cu) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  if (S < 1 || S > c->cfg.max_sessions_per_call)
+    return fail(WS_ERR_INVALID_ARG, "num_sessions %d not in [1, %d]", S, c->cfg.max_sessions_per_call);
+  if (!c->dry && (!k_new || !v_new)) return fail(WS_ERR_INVALID_ARG, "k_new / v_new is NULL");
+  if (cu[0] != 0) return fail(WS_ERR_INVALID_ARG, "cu_new_tokens[0] must be 0");
+  const int32_t P = c->cfg.page_tokens;
+  int64_t extra_pages = 0;
+  for (int32_t s = 0; s < S; ++s) {
+    int32_t n = cu[s + 1] - cu[s];
+    if (n < 1) return fail(WS_ERR_INVALID_ARG, "session %d appends %d tokens (must be >= 1)", s, n);
+    int32_t id = session_ids[s];
+    if (!c->host->is_open(id)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", id);
+    for (int32_t t = 0; t < s; ++t)
+      if (session_ids[t] == id) return fail(WS_ERR_INVALID_ARG, "session %d listed twice", id);
+    if (!c->host->fits(id, n))
+      return fail(WS_ERR_OUT_OF_PAGES, "session %d exceeds its page-table or block capacity", id);
+    if (c->host->session(id).tokens + n >= (1ll << 31))
+      return fail(WS_ERR_UNSUPPORTED, "session %d would exceed 2^31 tokens", id);
+    extra_pages += c->host->pages_needed(id, c->host->session(id).tokens + n);
+  }
+  if (cu[S] > c->cfg.max_q_tokens_per_call)
+    return fail(WS_ERR_INVALID_ARG, "%d new tokens > max_q_tokens_per_call %d", cu[S],
+                c->cfg.max_q_tokens_per_call);
+  if (extra_pages > c->host->free_pages())
+    return fail(WS_ERR_OUT_OF_PAGES, "need %lld pages, %d free", (long long)extra_pages,
+                c->host->free_pages());
+  // metadata size check BEFORE mutating
+  size_t words = sizeof(ws::AppendMeta) / 4 + (size_t)S * sizeof(ws::AppendSession) / 4;
+  for (int32_t s = 0; s < S; ++s) words += (size_t)(cu[s + 1] - cu[s]) / P + 3;
+  if (words * 4 > c->lay.meta_slot_bytes)
+    return fail(WS_ERR_WORKSPACE_TOO_SMALL, "append metadata exceeds the slot");
+  char *h = nullptr, *d = nullptr;
+  ws_status_t st = next_slot(c, words * 4, &h, &d);
+  if (st != WS_OK) return st;
+
+  // ---- commit (no failure paths below except CUDA errors)
+  ws::AppendMeta hdr{S, cu[S], (int32_t)(sizeof(ws::AppendMeta) / 4),
+                     (int32_t)(sizeof(ws::AppendMeta) / 4 + S * sizeof(ws::AppendSession) / 4)};
+  int32_t* blob = (int32_t*)h;
+  ws::AppendSession* as = (ws::AppendSession*)(blob + hdr.off_sessions);
+  int32_t* pages = blob + hdr.off_pages;
+  int32_t npg = 0;
+  for (int32_t s = 0; s < S; ++s) {
+    int32_t id = session_ids[s], n = cu[s + 1] - cu[s];
+    int64_t len_old = c->host->session(id).tokens;
+    int32_t first = c->host->commit_block(id, n, modality ? modality + cu[s] : nullptr);
+    const ws::SessionState& ss = c->host->session(id);
+    as[s] = ws::AppendSession{id, (int32_t)len_old, cu[s], cu[s + 1], npg, {0, 0, 0}};
+    for (size_t i = first; i < ss.pages.size(); ++i) pages[npg++] = ss.pages[i];
+  }
+  memcpy(blob, &hdr, sizeof(hdr));
+  if (c->dry) return WS_OK;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  st = upload_slot(c, h, d, (size_t)(hdr.off_pages + npg) * 4, stream);
+  if (st != WS_OK) return st;
+  WS_CUDA(ws::launch_kv_append(k_new, v_new, c->cfg.k_pool, c->cfg.v_pool, c->d_page_table,
+                               (const int32_t*)d, cu[S], c->cfg.max_pages_per_session, P,
+                               c->cfg.num_kv_heads, c->cfg.head_dim, eb_of(c->cfg.dtype), c->num_sms,
+                               stream));
+  c->launches += 1;
+  return WS_OK;
+}
+
+// ------------------------------------------------------------------------------------ a3 + a4
+ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* session_ids,
+                                     const int32_t* num_q_blocks, const int32_t* cu, const void* q,
+                                     void* out, float* lse, float scale, void* cuda_stream) {
+  if (!c || !session_ids || !cu) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  if (S < 1 || S > c->cfg.max_sessions_per_call)
+    return fail(WS_ERR_INVALID_ARG, "num_sessions %d not in [1, %d]", S, c->cfg.max_sessions_per_call);
+  if (!c->dry && (!q || !out)) return fail(WS_ERR_INVALID_ARG, "q / out is NULL");
+  if (!(scale > 0.f) || !std::isfinite(scale)) return fail(WS_ERR_INVALID_ARG, "scale must be finite and > 0");
+  if (cu[0] != 0) return fail(WS_ERR_INVALID_ARG, "cu_q_tokens[0] must be 0");
+  std::vector<ws::PlanSession> ps(S);
+  std::vector<int32_t> vis_end, tok_slot;
+  bool any_multi = false;
+  for (int32_t s = 0; s < S; ++s) {
+    int32_t id = session_ids[s];
+    if (!c->host->is_open(id)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", id);
+    const ws::SessionState& ss = c->host->session(id);
+    int32_t m = num_q_blocks ? num_q_blocks[s] : 1;
+    int32_t B = (int32_t)ss.block_ends.size();
+    if (m < 1 || m > B)
+      return fail(WS_ERR_INVALID_ARG, "session %d: num_q_blocks %d not in [1, %d]", id, m, B);
+    int64_t q_start = (B - m) ? ss.block_ends[B - m - 1] : 0;
+    int64_t nq = ss.tokens - q_start;
+    if (cu[s + 1] - cu[s] != nq)
+      return fail(WS_ERR_INVALID_ARG, "session %d: cu gives %d query tokens, its last %d block(s) hold %lld",
+                  id, cu[s + 1] - cu[s], m, (long long)nq);
+    ps[s] = ws::PlanSession{id, cu[s], cu[s + 1], m > 1};
+    any_multi |= m > 1;
+    for (int32_t b = B - m; b < B; ++b) {
+      int64_t lo = b ? ss.block_ends[b - 1] : 0;
+      for (int64_t t = lo; t < ss.block_ends[b]; ++t) {
+        vis_end.push_back((int32_t)ss.block_ends[b]);
+        tok_slot.push_back(id);
+      }
+    }
+  }
+  const int32_t NQ = cu[S];
+  if (NQ > c->cfg.max_q_tokens_per_call)
+    return fail(WS_ERR_INVALID_ARG, "%d query tokens > max_q_tokens_per_call %d", NQ,
+                c->cfg.max_q_tokens_per_call);
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  const bool tensor = c->tensor_path_ok && !(c->cfg.flags & WS_FLAG_FORCE_SIMT);
+  c->last_tensor = tensor;
+  const int G = c->cfg.num_q_heads / c->cfg.num_kv_heads;
+  char *h = nullptr, *d = nullptr;
+
+  if (!tensor) {
+    if (c->dry && !c->tensor_path_ok) { c->last_plan = ws::Plan(); return WS_OK; }
+    if (!c->dry) {
+      size_t bytes = (size_t)NQ * 8;
+      ws_status_t st = next_slot(c, bytes, &h, &d);
+      if (st != WS_OK) return st;
+      memcpy(h, tok_slot.data(), (size_t)NQ * 4);
+      memcpy(h + (size_t)NQ * 4, vis_end.data(), (size_t)NQ * 4);
+      st = upload_slot(c, h, d, bytes, stream);
+      if (st != WS_OK) return st;
+      WS_CUDA(ws::launch_attn_simt(c->cfg.dtype, q, out, lse, c->cfg.k_pool, c->cfg.v_pool,
+                                   c->d_page_table, (const int32_t*)d,
+                                   c->default_map ? nullptr : c->d_q_to_kv, NQ,
+                                   c->cfg.max_pages_per_session, c->cfg.num_q_heads,
+                                   c->cfg.num_kv_heads, c->cfg.head_dim, c->cfg.page_tokens, scale,
+                                   stream));
+      c->launches += 1;
+      c->last_plan = ws::Plan();
+      return WS_OK;
+    }
+  }
+
+  ws::PlanConfig pc{c->cfg.num_kv_heads, G, c->num_sms, /*min_tiles=*/2, c->min_splits,
+                    c->lay.max_part_slots};
+  ws::Plan plan = ws::build_plan(pc, ps, vis_end);
+  if (!plan.ok)
+    return fail(WS_ERR_WORKSPACE_TOO_SMALL, "plan needs %d partial slots, workspace holds %d",
+                plan.num_part_slots, c->lay.max_part_slots);
+  std::vector<int32_t> blob = ws::serialise_plan(plan, vis_end, any_multi);
+  ws_status_t st = next_slot(c, blob.size() * 4, &h, &d);
+  if (st != WS_OK) return st;
+  memcpy(h, blob.data(), blob.size() * 4);
+  c->last_plan = std::move(plan);
+  if (c->dry) return WS_OK;
+  st = upload_slot(c, h, d, blob.size() * 4, stream);
+  if (st != WS_OK) return st;
+
+  ws::Sm100Launch L{};
+  L.p.q = q; L.p.out = out; L.p.lse = lse;
+  L.p.k_pool = c->cfg.k_pool; L.p.v_pool = c->cfg.v_pool;
+  L.p.page_table = c->d_page_table;
+  L.p.meta = (const int32_t*)d;
+  L.p.part_o = c->d_part_o; L.p.part_lse = c->d_part_lse;
+  L.p.max_pages_per_session = c->cfg.max_pages_per_session;
+  L.p.Hq = c->cfg.num_q_heads; L.p.Hkv = c->cfg.num_kv_heads; L.p.D = c->cfg.head_dim;
+  L.p.G = G; L.p.P = c->cfg.page_tokens; L.p.total_q_tokens = NQ; L.p.scale = scale;
+  L.tmap_k = c->tmap_k; L.tmap_v = c->tmap_v;
+  {
+    const cuuint64_t D = 128, Hq = c->cfg.num_q_heads;
+    cuuint64_t dims[3] = {D, Hq, (cuuint64_t)NQ};
+    cuuint64_t strides[2] = {D * 2, Hq * D * 2};
+    cuuint32_t box[3] = {64, (cuuint32_t)G, (cuuint32_t)(ws::kTileRows / G)};
+    st = encode_tmap(c, &L.tmap_q, const_cast<void*>(q), 3, dims, strides, box);
+    if (st != WS_OK) return st;
+  }
+  L.num_ctas = c->last_plan.num_teams * c->last_plan.team_size;
+  WS_CUDA(ws::launch_attn_sm100(L, stream));
+  c->launches += 1;
+  if (!c->last_plan.combine.empty()) {
+    WS_CUDA(ws::launch_combine(L.p, (int32_t)c->last_plan.combine.size(), c->last_plan.team_size, stream));
+    c->launches += 1;
+  }
+  return WS_OK;
+}
+
+size_t ws_step_staging_bytes(const ws_cache_config_t* cfg, int32_t n) {
+  const char* why;
+  if (!config_valid(cfg, &why) || n < 1) return 0;
+  size_t eb = eb_of(cfg->dtype), D = cfg->head_dim;
+  size_t qb = align_up((size_t)n * cfg->num_q_heads * D * eb, 256);
+  size_t kb = align_up((size_t)n * cfg->num_kv_heads * D * eb, 256);
+  return 2 * qb + 2 * kb;
+}
+
+ws_status_t ws_stream_step_host(ws_cache_t* c, int32_t S, const int32_t* session_ids,
+                                const int32_t* cu, const void* q_host, const void* k_host,
+                                const void* v_host, void* out_host, void* staging,
+                                size_t staging_bytes, float scale, void* cuda_stream) {
+  if (!c || !session_ids || !cu || !q_host || !k_host || !v_host || !out_host || !staging)
+    return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  if (c->dry) return fail(WS_ERR_CUDA, "ws_stream_step_host needs a CUDA device (dry-run cache)");
+  if (S < 1 || cu[0] != 0 || cu[S] < 1) return fail(WS_ERR_INVALID_ARG, "bad cu_new_tokens");
+  const int32_t n = cu[S];
+  if (staging_bytes < ws_step_staging_bytes(&c->cfg, n))
+    return fail(WS_ERR_WORKSPACE_TOO_SMALL, "staging_bytes %zu < required %zu", staging_bytes,
+                ws_step_staging_bytes(&c->cfg, n));
+  size_t eb = eb_of(c->cfg.dtype), D = c->cfg.head_dim;
+  size_t q_bytes = (size_t)n * c->cfg.num_q_heads * D * eb, kv_bytes = (size_t)n * c->cfg.num_kv_heads * D * eb;
+  size_t qb = align_up(q_bytes, 256), kb = align_up(kv_bytes, 256);
+  char* base = (char*)staging;
+  char *dq = base, *dout = base + qb, *dk = base + 2 * qb, *dv = base + 2 * qb + kb;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  WS_CUDA(cudaMemcpyAsync(dk, k_host, kv_bytes, cudaMemcpyHostToDevice, stream));
+  WS_CUDA(cudaMemcpyAsync(dv, v_host, kv_bytes, cudaMemcpyHostToDevice, stream));
+  WS_CUDA(cudaMemcpyAsync(dq, q_host, q_bytes, cudaMemcpyHostToDevice, stream));
+  ws_status_t st = ws_kv_append(c, S, session_ids, cu, dk, dv, nullptr, cuda_stream);
+  if (st != WS_OK) return st;
+  st = ws_block_causal_attn_fwd(c, S, session_ids, nullptr, cu, dq, dout, nullptr, scale, cuda_stream);
+  if (st != WS_OK) return st;
+  WS_CUDA(cudaMemcpyAsync(out_host, dout, q_bytes, cudaMemcpyDeviceToHost, stream));
+  return WS_OK;
+}
+
+ws_status_t ws_kv_gather(const ws_cache_t* c, int32_t session, int64_t start, int64_t count,
+                         void* k_out, void* v_out, void* cuda_stream) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  if (!c->host->is_open(session)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", session);
+  const ws::SessionState& ss = c->host->session(session);
+  if (start < 0 || count < 0 || start + count > ss.tokens)
+    return fail(WS_ERR_INVALID_ARG, "range [%lld, %lld) outside the %lld committed tokens",
+                (long long)start, (long long)(start + count), (long long)ss.tokens);
+  if (c->dry || count == 0) return WS_OK;
+  WS_CUDA(ws::launch_kv_gather(c->cfg.k_pool, c->cfg.v_pool, k_out, v_out,
+                               c->d_page_table + (int64_t)session * c->cfg.max_pages_per_session,
+                               start, count, c->cfg.page_tokens, c->cfg.num_kv_heads, c->cfg.head_dim,
+                               eb_of(c->cfg.dtype), c->num_sms, (cudaStream_t)cuda_stream));
+  const_cast<ws_cache*>(c)->launches += 1;
+  return WS_OK;
+}
+
+ws_status_t ws_last_plan_info(const ws_cache_t* c, ws_plan_info_t* out) {
+  if (!c || !out) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  const ws::Plan& p = c->last_plan;
+  out->num_ctas = p.num_teams * p.team_size;
+  out->team_size = p.team_size;
+  out->num_groups = (int32_t)p.groups.size();
+  out->num_segments = (int32_t)p.segments.size();
+  out->num_partial_slots = p.num_part_slots;
+  out->num_combine_items = (int32_t)p.combine.size();
+  out->used_tensor_core_kernel = c->last_tensor ? 1 : 0;
+  out->total_kv_tiles = p.total_tiles;
+  return WS_OK;
+}
+
+ws_status_t ws_last_plan_segment(const ws_cache_t* c, int32_t i, ws_plan_segment_t* out) {
+  if (!c || !out) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  const ws::Plan& p = c->last_plan;
+  if (i < 0 || i >= (int32_t)p.segments.size()) return fail(WS_ERR_INVALID_ARG, "segment %d out of range", i);
+  const ws::Segment& s = p.segments[i];
+  const ws::Group& g = p.groups[s.group];
+  *out = ws_plan_segment_t{s.group, g.slot, g.kv_head, g.q_token0, s.tile_begin, s.tile_end,
+                           p.seg_team[i], s.part_base};
+  return WS_OK;
+}
+
+int64_t ws_launch_count(const ws_cache_t* c) { return c ? c->launches : -1; }
+
+const char* ws_status_str(ws_status_t s) {
+  switch (s) {
+    case WS_OK: return "WS_OK";
+    case WS_ERR_INVALID_ARG: return "WS_ERR_INVALID_ARG";
+    case WS_ERR_BAD_SESSION: return "WS_ERR_BAD_SESSION";
+    case WS_ERR_OUT_OF_PAGES: return "WS_ERR_OUT_OF_PAGES";
+    case WS_ERR_UNSUPPORTED: return "WS_ERR_UNSUPPORTED";
+    case WS_ERR_WORKSPACE_TOO_SMALL: return "WS_ERR_WORKSPACE_TOO_SMALL";
+    case WS_ERR_CUDA: return "WS_ERR_CUDA";
+  }
+  return "WS_ERR_?";
+}
+
+const char* ws_last_error(void) { return g_err.c_str(); }
+const char* ws_version(void) { return "wanstream-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

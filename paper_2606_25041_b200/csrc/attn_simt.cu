@@ -1,0 +1,149 @@
+// attn_simt.cu - a3, generic CUDA-core kernel: block-causal attention of query tokens against a
+// paged cache, fp32 arithmetic throughout (exact expf), any D <= 256 (D % 8 == 0), any page size,
+// any q->kv head map, per-token visible end (multi-block queries).
+//
+// This is the kernel of the fp32 config (BASELINE configs[0]; tf32 tensor cores cannot meet 1e-5)
+// and the functional path for bf16 shapes the tcgen05 kernel does not cover; it also serves as an
+// on-GPU second opinion (WS_FLAG_FORCE_SIMT).  Definition followed: DESIGN.md §1 / PAPER.md:11, :29,
+// :47 Eq. (1): row r of block b sees keys j < e_b.
+//
+// One warp per (query token, q head).  Lane = key for the scores (online softmax, max/sum reduced
+// with warp shuffles), lane = output-dim slice for P.V.
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <math.h>
+
+#include "launch.h"
+
+namespace ws {
+
+template <typename T> struct Vec16;
+template <> struct Vec16<float> {
+  static constexpr int N = 4;
+  static __device__ __forceinline__ void load(const float* p, float* o) {
+    float4 v = *reinterpret_cast<const float4*>(p);
+    o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w;
+  }
+};
+template <> struct Vec16<__nv_bfloat16> {
+  static constexpr int N = 8;
+  static __device__ __forceinline__ void load(const __nv_bfloat16* p, float* o) {
+    uint4 v = *reinterpret_cast<const uint4*>(p);
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      o[2 * i] = __uint_as_float(w[i] << 16);
+      o[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+    }
+  }
+};
+
+__device__ __forceinline__ float to_f32(float x) { return x; }
+__device__ __forceinline__ float to_f32(__nv_bfloat16 x) { return __bfloat162float(x); }
+__device__ __forceinline__ void store_out(float* p, float x) { *p = x; }
+__device__ __forceinline__ void store_out(__nv_bfloat16* p, float x) { *p = __float2bfloat16_rn(x); }
+
+constexpr int kSimtWarps = 4;
+constexpr int kMaxD = 256;
+
+template <typename T>
+__global__ void __launch_bounds__(kSimtWarps * 32)
+attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict__ lse,
+                 const T* __restrict__ k_pool, const T* __restrict__ v_pool,
+                 const int32_t* __restrict__ page_table, const int32_t* __restrict__ tok_meta,
+                 const int32_t* __restrict__ q_to_kv, int32_t total_q_tokens, int32_t max_pages,
+                 int32_t Hq, int32_t Hkv, int32_t D, int32_t P, float scale) {
+  __shared__ float q_s[kSimtWarps][kMaxD];
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const int64_t w = (int64_t)blockIdx.x * kSimtWarps + wib;
+  if (w >= (int64_t)total_q_tokens * Hq) return;
+  const int32_t tok = (int32_t)(w / Hq), h = (int32_t)(w % Hq);
+  const int32_t g = q_to_kv ? q_to_kv[h] : h / (Hq / Hkv);
+  const int32_t slot = tok_meta[tok];
+  const int32_t vis = tok_meta[total_q_tokens + tok];
+  const int32_t* page_row = page_table + (int64_t)slot * max_pages;
+
+  const T* qrow = q + ((int64_t)tok * Hq + h) * D;
+  for (int d = lane; d < D; d += 32) q_s[wib][d] = to_f32(qrow[d]);
+  __syncwarp();
+
+  constexpr int VN = Vec16<T>::N;
+  float acc[kMaxD / 32];
+#pragma unroll
+  for (int i = 0; i < kMaxD / 32; ++i) acc[i] = 0.f;
+  float m = -INFINITY, l = 0.f;
+
+  for (int32_t base = 0; base < vis; base += 32) {
+    const int32_t j = base + lane;
+    const bool valid = j < vis;
+    float s = -INFINITY;
+    int32_t rowidx = 0;
+    if (valid) {
+      rowidx = (page_row[j / P] * Hkv + g) * P + (j % P);
+      const T* kp = k_pool + (int64_t)rowidx * D;
+      float a = 0.f;
+      for (int d = 0; d < D; d += VN) {
+        float kv[VN];
+        Vec16<T>::load(kp + d, kv);
+#pragma unroll
+        for (int e = 0; e < VN; ++e) a = fmaf(q_s[wib][d + e], kv[e], a);
+      }
+      s = a * scale;
+    }
+    float tmax = s;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
+    const float m_new = fmaxf(m, tmax);                 // finite: at least one key is valid
+    const float corr = expf(m - m_new);                 // m = -inf -> 0
+    const float p = valid ? expf(s - m_new) : 0.f;
+    float psum = p;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) psum += __shfl_xor_sync(0xffffffffu, psum, o);
+    l = l * corr + psum;
+#pragma unroll
+    for (int i = 0; i < kMaxD / 32; ++i) acc[i] *= corr;
+    const int nk = min(32, vis - base);
+    for (int kk = 0; kk < nk; ++kk) {
+      const float pk = __shfl_sync(0xffffffffu, p, kk);
+      const int32_t r = __shfl_sync(0xffffffffu, rowidx, kk);
+      const T* vp = v_pool + (int64_t)r * D;
+#pragma unroll
+      for (int i = 0; i < kMaxD / 32; ++i) {
+        int d = lane + 32 * i;
+        if (d < D) acc[i] = fmaf(pk, to_f32(vp[d]), acc[i]);
+      }
+    }
+    m = m_new;
+  }
+  const float inv = 1.f / l;
+  T* orow = out + ((int64_t)tok * Hq + h) * D;
+#pragma unroll
+  for (int i = 0; i < kMaxD / 32; ++i) {
+    int d = lane + 32 * i;
+    if (d < D) store_out(orow + d, acc[i] * inv);
+  }
+  if (lse && lane == 0) lse[(int64_t)tok * Hq + h] = m + logf(l);
+}
+
+cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse,
+                             const void* k_pool, const void* v_pool, const int32_t* page_table,
+                             const int32_t* tok_meta, const int32_t* q_to_kv, int32_t total_q_tokens,
+                             int32_t max_pages, int32_t Hq, int32_t Hkv, int32_t D, int32_t P,
+                             float scale, cudaStream_t stream) {
+  int64_t warps = (int64_t)total_q_tokens * Hq;
+  int32_t grid = (int32_t)((warps + kSimtWarps - 1) / kSimtWarps);
+  if (grid == 0) return cudaSuccess;
+  if (dtype == 1) {
+    attn_simt_kernel<float><<<grid, kSimtWarps * 32, 0, stream>>>(
+        (const float*)q, (float*)out, lse, (const float*)k_pool, (const float*)v_pool, page_table,
+        tok_meta, q_to_kv, total_q_tokens, max_pages, Hq, Hkv, D, P, scale);
+  } else {
+    attn_simt_kernel<__nv_bfloat16><<<grid, kSimtWarps * 32, 0, stream>>>(
+        (const __nv_bfloat16*)q, (__nv_bfloat16*)out, lse, (const __nv_bfloat16*)k_pool,
+        (const __nv_bfloat16*)v_pool, page_table, tok_meta, q_to_kv, total_q_tokens, max_pages, Hq,
+        Hkv, D, P, scale);
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace ws

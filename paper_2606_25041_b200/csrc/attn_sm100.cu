@@ -1,0 +1,409 @@
+// attn_sm100.cu - a3 on sm_100a: block-causal attention forward for bf16, D = 128, 64-token pages.
+//
+// Definition (DESIGN.md §1; PAPER.md:11, :23, :29 "block-causal attention", :47 Eq. (1)): a query
+// row in block b sees every key j < e_b.  On the hot path (the newest block attends) that is ALL
+// L + n keys, so every 128-key tile is "full" (no mask code runs) except the last one when
+// (L + n) % 128 != 0; multi-block queries add per-row visible ends (partial / skipped tiles).
+//
+// Mapping.  The G = Hq/Hkv query heads that share a KV head are packed with the tokens into the MMA
+// M dimension (row = token * G + head_in_group), so one K/V tile read serves all G heads.  A CTA
+// owns a PAIR of 128-row Q tiles (256 packed rows) of one (session, KV head) group and a contiguous
+// range of that group's KV tiles (a "segment" from the host planner, plan.cpp); it may process
+// several segments back to back.
+//
+// Pipeline (12 warps, 1 CTA / SM):
+//   warp 8  lane 0 : TMA producer - Q tiles (rank-3 map over [D, Hq, tokens]) and paged K/V tiles
+//                    (rank-4 map over [D, P, Hkv, pages]; the page id read from the device page
+//                    table is the outermost TMA coordinate) into a 5-slot ring of 32 KB buffers,
+//                    128B-swizzled, completion on mbarriers.
+//   warp 9  lane 0 : tcgen05.mma issuer - S_q = Q_q K^T (SS, M128 N128 K16 x 8) into TMEM, and
+//                    O_q += P_q V (A = P from TMEM, B = V from smem, MN-major) for q = 0, 1,
+//                    interleaved so the tensor pipe works on one Q tile while the softmax
+//                    warpgroup of the other is busy.  tcgen05.commit arrives on mbarriers.
+//   warps 0-3, 4-7 : softmax warpgroup for Q tile 0 / 1: tcgen05.ld of a whole S row per thread
+//                    (32x32b: thread = row, so max/sum need no cross-thread reduction), fp32 online
+//                    softmax in the log2 domain with lazy rescaling of O (only when the row max
+//                    grows by > 2^8), P rounded to bf16 and written back over S in TMEM, row sum
+//                    accumulated in fp32 from the unrounded p.  Epilogue: O / l -> bf16 out (+ LSE)
+//                    or fp32 partial + log2-LSE when the segment is one of several splits.
+//   warp 10        : TMEM allocation (512 columns: S0 S1 O0 O1) and release.
+//
+// Roofline: tensor-bound for G*n >= ~260 FLOP/B (configs 3-5), 4*D*rows*keys FLOPs per tile pair;
+// algorithmic bytes per tile = 2 x 128 x 128 x 2 B of K/V.  MUFU ex2 (16/clk/SM) is the co-limit.
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <math.h>
+
+#include "launch.h"
+#include "sm100_ptx.cuh"
+
+namespace ws {
+
+using namespace ptx;
+
+constexpr int kStages = 5;
+constexpr uint32_t kSlotBytes = kTileKeys * 128 * 2;       // one K or V tile: 128 keys x 128 dims bf16
+constexpr uint32_t kHalfBytes = kSlotBytes / 2;            // one 64-dim half: 128 rows x 128 B
+constexpr uint32_t kQTileBytes = kTileRows * 128 * 2;
+constexpr int kThreads = 384;
+constexpr uint32_t kTmemCols = 512;
+constexpr float kRescaleThreshold = 8.0f;                  // log2 units
+
+struct Barriers {
+  uint64_t q_full, q_empty;
+  uint64_t kv_full[kStages], kv_empty[kStages];
+  uint64_t s_full[2], p_full[2], o_full[2], o_empty[2];
+  uint32_t tmem_base;
+  uint32_t pad;
+};
+constexpr uint32_t kSmemBytes = 2 * kQTileBytes + kStages * kSlotBytes + sizeof(Barriers) + 1024;
+
+struct SegView {
+  Group g;
+  int32_t tile_begin, tile_end, part_base;
+};
+
+__device__ __forceinline__ bool load_segment(const int32_t* meta, const AttnMeta& hdr, int32_t si,
+                                             int32_t pair, SegView& v) {
+  const Segment s = reinterpret_cast<const Segment*>(meta + hdr.off_segments)[si];
+  v.g = reinterpret_cast<const Group*>(meta + hdr.off_groups)[s.group];
+  v.tile_begin = s.tile_begin; v.tile_end = s.tile_end; v.part_base = s.part_base;
+  return pair < v.g.npairs;
+}
+
+__global__ void __launch_bounds__(kThreads, 1)
+attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
+                  const __grid_constant__ CUtensorMap tmap_k,
+                  const __grid_constant__ CUtensorMap tmap_v, const AttnParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = smem_base;                           // 2 x 32 KB
+  const uint32_t sRing = smem_base + 2 * kQTileBytes;      // kStages x 32 KB
+  Barriers* bars = reinterpret_cast<Barriers*>(smem_raw + (smem_base - smem_u32(smem_raw)) +
+                                               2 * kQTileBytes + kStages * kSlotBytes);
+  const uint32_t bq_full = smem_u32(&bars->q_full), bq_empty = smem_u32(&bars->q_empty);
+  auto bkv_full = [&](int s) { return smem_u32(&bars->kv_full[s]); };
+  auto bkv_empty = [&](int s) { return smem_u32(&bars->kv_empty[s]); };
+  auto bs_full = [&](int q) { return smem_u32(&bars->s_full[q]); };
+  auto bp_full = [&](int q) { return smem_u32(&bars->p_full[q]); };
+  auto bo_full = [&](int q) { return smem_u32(&bars->o_full[q]); };
+  auto bo_empty = [&](int q) { return smem_u32(&bars->o_empty[q]); };
+
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+  const int lane = threadIdx.x & 31;
+  const AttnMeta hdr = *reinterpret_cast<const AttnMeta*>(p.meta);
+  const int32_t team = blockIdx.x / hdr.team_size;
+  const int32_t pair = blockIdx.x - team * hdr.team_size;
+  const int32_t* tsb = p.meta + hdr.off_team_seg_begin;
+  const int32_t seg_lo = tsb[team], seg_hi = tsb[team + 1];
+  const int32_t tok_per_pair = kPairRows / p.G;
+  const int32_t tok_per_tile = kTileRows / p.G;
+
+  if (warp == 8 && lane == 0) {
+    prefetch_tmap(&tmap_q); prefetch_tmap(&tmap_k); prefetch_tmap(&tmap_v);
+  }
+  if (warp == 9 && lane == 0) {
+    mbar_init(bq_full, 1); mbar_init(bq_empty, 1);
+    for (int s = 0; s < kStages; ++s) { mbar_init(bkv_full(s), 1); mbar_init(bkv_empty(s), 1); }
+    for (int q = 0; q < 2; ++q) {
+      mbar_init(bs_full(q), 1); mbar_init(bp_full(q), 128);
+      mbar_init(bo_full(q), 1); mbar_init(bo_empty(q), 128);
+    }
+    fence_mbar_init();
+  }
+  if (warp == 10) {
+    tmem_alloc<kTmemCols>(smem_u32(&bars->tmem_base));
+    tmem_relinquish();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = bars->tmem_base;
+
+  if (warp >= 8) {
+    setmaxnreg_dec<88>();
+    if (warp == 8 && lane == 0) {
+      // ===================================================== TMA producer
+      uint32_t ring_it = 0, q_it = 0;
+      for (int32_t si = seg_lo; si < seg_hi; ++si) {
+        SegView sv;
+        if (!load_segment(p.meta, hdr, si, pair, sv)) continue;
+        const int32_t* page_row = p.page_table + (int64_t)sv.g.slot * p.max_pages_per_session;
+        const int32_t last_page = (sv.g.kv_len - 1) / p.P;
+        int32_t pg0 = page_row[min(2 * sv.tile_begin, last_page)];
+        int32_t pg1 = page_row[min(2 * sv.tile_begin + 1, last_page)];
+        // Q pair
+        mbar_wait(bq_empty, (q_it & 1) ^ 1);
+        mbar_arrive_expect_tx(bq_full, 2 * kQTileBytes);
+        const int32_t tok0 = sv.g.q_token0 + pair * tok_per_pair;
+        for (int q = 0; q < 2; ++q)
+          for (int h = 0; h < 2; ++h)
+            tma_load_3d(sQ + q * kQTileBytes + h * kHalfBytes, &tmap_q, bq_full, h * 64,
+                        sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
+        ++q_it;
+        for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
+          const int32_t c0 = pg0, c1 = pg1;
+          if (j + 1 < sv.tile_end) {                        // prefetch next tile's page ids
+            pg0 = page_row[min(2 * j + 2, last_page)];
+            pg1 = page_row[min(2 * j + 3, last_page)];
+          }
+#pragma unroll
+          for (int kv = 0; kv < 2; ++kv) {
+            const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
+            const CUtensorMap* tm = kv == 0 ? &tmap_k : &tmap_v;
+            mbar_wait(bkv_empty(slot), par ^ 1);
+            mbar_arrive_expect_tx(bkv_full(slot), kSlotBytes);
+            const uint32_t dst = sRing + slot * kSlotBytes;
+            tma_load_4d(dst, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c0);
+            tma_load_4d(dst + kHalfBytes / 2, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c1);
+            tma_load_4d(dst + kHalfBytes, tm, bkv_full(slot), 64, 0, sv.g.kv_head, c0);
+            tma_load_4d(dst + kHalfBytes + kHalfBytes / 2, tm, bkv_full(slot), 64, 0,
+                        sv.g.kv_head, c1);
+            ++ring_it;
+          }
+        }
+      }
+    } else if (warp == 9 && lane == 0) {
+      // ===================================================== MMA issuer
+      constexpr uint32_t idesc_qk = make_idesc_bf16(128, 128, 0, 0);
+      constexpr uint32_t idesc_pv = make_idesc_bf16(128, 128, 0, 1);
+      uint32_t ring_it = 0, q_it = 0, tile_it = 0, seg_it = 0;
+      auto issue_S = [&](int q, uint32_t slot) {
+        const uint32_t a0 = sQ + q * kQTileBytes, b0 = sRing + slot * kSlotBytes;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+          const uint32_t off = (ks >> 2) * kHalfBytes + (ks & 3) * 32;
+          mma_ss(tmem_base + q * 128, make_smem_desc_sw128(a0 + off, 16, 1024),
+                 make_smem_desc_sw128(b0 + off, 16, 1024), idesc_qk, ks > 0);
+        }
+      };
+      auto issue_PV = [&](int q, uint32_t slot, bool accumulate) {
+        const uint32_t b0 = sRing + slot * kSlotBytes;
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks)
+          mma_ts(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8,
+                 make_smem_desc_sw128(b0 + ks * 2048, kHalfBytes, 1024), idesc_pv,
+                 (accumulate || ks > 0) ? 1u : 0u);
+      };
+      for (int32_t si = seg_lo; si < seg_hi; ++si) {
+        SegView sv;
+        if (!load_segment(p.meta, hdr, si, pair, sv)) continue;
+        const int32_t nt = sv.tile_end - sv.tile_begin;
+        mbar_wait(bq_full, q_it & 1);
+        {
+          const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
+          mbar_wait(bkv_full(slot), par);
+          tc_fence_after();
+          issue_S(0, slot); mma_commit(bs_full(0));
+          issue_S(1, slot); mma_commit(bs_full(1));
+          mma_commit(bkv_empty(slot));
+          if (nt == 1) mma_commit(bq_empty);
+          ++ring_it;
+        }
+        for (int32_t j = 0; j < nt; ++j) {
+          const uint32_t slot_v = ring_it % kStages, par_v = (ring_it / kStages) & 1;
+          ++ring_it;
+          const bool have_next = j + 1 < nt;
+          uint32_t slot_k = 0, par_k = 0;
+          if (have_next) { slot_k = ring_it % kStages; par_k = (ring_it / kStages) & 1; ++ring_it; }
+          mbar_wait(bkv_full(slot_v), par_v);
+          for (int q = 0; q < 2; ++q) {
+            mbar_wait(bp_full(q), tile_it & 1);
+            if (j == 0) mbar_wait(bo_empty(q), (seg_it & 1) ^ 1);
+            tc_fence_after();
+            issue_PV(q, slot_v, j > 0);
+            if (!have_next) mma_commit(bo_full(q));
+            if (have_next) {
+              if (q == 0) { mbar_wait(bkv_full(slot_k), par_k); tc_fence_after(); }
+              issue_S(q, slot_k);
+              mma_commit(bs_full(q));
+            }
+          }
+          mma_commit(bkv_empty(slot_v));
+          if (have_next) {
+            mma_commit(bkv_empty(slot_k));
+            if (j + 2 == nt) mma_commit(bq_empty);
+          }
+          ++tile_it;
+        }
+        ++q_it; ++seg_it;
+      }
+    }
+  } else {
+    // ======================================================= softmax warpgroups (warps 0-7)
+    setmaxnreg_inc<208>();
+    const int q = warp >> 2;
+    const uint32_t lane_base = (uint32_t)(warp & 3) * 32;
+    const int32_t row_in_tile = (int32_t)lane_base + lane;
+    const int32_t R = q * kTileRows + row_in_tile;           // packed row inside the pair
+    const uint32_t t_s = tmem_base + (lane_base << 16) + q * 128;
+    const uint32_t t_o = tmem_base + (lane_base << 16) + 256 + q * 128;
+    const float c = p.scale * 1.4426950408889634f;
+    uint32_t ring_it = 0, tile_it = 0, seg_it = 0;
+
+    for (int32_t si = seg_lo; si < seg_hi; ++si) {
+      SegView sv;
+      if (!load_segment(p.meta, hdr, si, pair, sv)) continue;
+      const int32_t nt = sv.tile_end - sv.tile_begin;
+      const int32_t tok = sv.g.q_token0 + pair * tok_per_pair + R / p.G;
+      const bool row_valid = tok < sv.g.q_token_end;
+      const int32_t head = sv.g.kv_head * p.G + R % p.G;
+      int32_t vis = sv.g.kv_len;
+      if (sv.g.vis_off >= 0 && row_valid) vis = (p.meta + hdr.off_vis)[sv.g.vis_off + (tok - sv.g.q_token0)];
+      float m_used = -INFINITY, l = 0.f;
+
+      for (int32_t j = 0; j < nt; ++j) {
+        const int32_t key0 = (sv.tile_begin + j) * kTileKeys;
+        // V(j) ring position: K(j) is 2j, V(j) is 2j+1 within the segment
+        const uint32_t v_it = ring_it + 2 * j + 1;
+        mbar_wait(bs_full(q), tile_it & 1);
+        tc_fence_after();
+        uint32_t sr[128];                                   // one whole S row (fp32 bits)
+        tmem_ld32(t_s + 0, sr + 0);
+        tmem_ld32(t_s + 32, sr + 32);
+        tmem_ld32(t_s + 64, sr + 64);
+        tmem_ld32(t_s + 96, sr + 96);
+        tmem_wait_ld();
+#define S_(i) __uint_as_float(sr[i])
+        const bool need_mask = __any_sync(0xffffffffu, key0 + kTileKeys > vis);
+        if (need_mask) {
+#pragma unroll
+          for (int i = 0; i < 128; ++i)
+            if (key0 + i >= vis) sr[i] = 0xff800000u;       // -inf
+        }
+        float mx0 = S_(0), mx1 = S_(1), mx2 = S_(2), mx3 = S_(3);
+#pragma unroll
+        for (int i = 4; i < 128; i += 4) {
+          mx0 = fmaxf(mx0, S_(i)); mx1 = fmaxf(mx1, S_(i + 1));
+          mx2 = fmaxf(mx2, S_(i + 2)); mx3 = fmaxf(mx3, S_(i + 3));
+        }
+        const float tm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;
+        const bool grow = tm > m_used + kRescaleThreshold;
+        if (j == 0) {
+          m_used = tm;
+        } else if (__any_sync(0xffffffffu, grow)) {
+          // lazy rescale of O and l (PV of the previous tile has completed: s_full was committed
+          // after it on the same in-order tensor pipe)
+          float alpha = 1.f;
+          if (grow) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
+#pragma unroll
+          for (int ch = 0; ch < 4; ++ch) {
+            uint32_t o[32];
+            tmem_ld32(t_o + ch * 32, o);
+            tmem_wait_ld();
+#pragma unroll
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+            tmem_st32(t_o + ch * 32, o);
+          }
+        }
+        const float m_c = (m_used == -INFINITY) ? 0.f : m_used;
+        float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+        uint32_t pk[64];
+#pragma unroll
+        for (int i = 0; i < 128; i += 4) {
+          const float p0 = ex2_approx(fmaf(S_(i), c, -m_c));
+          const float p1 = ex2_approx(fmaf(S_(i + 1), c, -m_c));
+          const float p2 = ex2_approx(fmaf(S_(i + 2), c, -m_c));
+          const float p3 = ex2_approx(fmaf(S_(i + 3), c, -m_c));
+          l0 += p0; l1 += p1; l2 += p2; l3 += p3;
+          pk[i / 2] = pack_bf16x2(p0, p1);
+          pk[i / 2 + 1] = pack_bf16x2(p2, p3);
+        }
+        l += (l0 + l1) + (l2 + l3);
+        tmem_st32(t_s + 0, pk);
+        tmem_st32(t_s + 32, pk + 32);
+        // last tile of the cache with a ragged end: zero the V rows beyond kv_len in smem so that
+        // 0 * (stale bits, possibly NaN) cannot reach O.  Done by warpgroup 0; the PV MMA of both
+        // Q tiles is issued after p_full[0].
+        if (q == 0 && key0 + kTileKeys > sv.g.kv_len) {
+          const uint32_t slot = v_it % kStages, par = (v_it / kStages) & 1;
+          mbar_wait(bkv_full(slot), par);
+          const int32_t r = (sv.g.kv_len - key0) + row_in_tile;
+          if (r < kTileKeys) {
+            const uint32_t base = sRing + slot * kSlotBytes + r * 128;
+#pragma unroll
+            for (int b = 0; b < 128; b += 16) {
+              asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(base + b), "r"(0u) : "memory");
+              asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(base + kHalfBytes + b), "r"(0u) : "memory");
+            }
+          }
+          fence_proxy_async_smem();
+        }
+        tmem_wait_st();
+        tc_fence_before();
+        mbar_arrive(bp_full(q));
+        ++tile_it;
+      }
+      ring_it += 2 * nt;
+
+      // ---------------------------------------------------- epilogue
+      mbar_wait(bo_full(q), seg_it & 1);
+      tc_fence_after();
+      const float inv_l = l > 0.f ? 1.f / l : 0.f;
+      const float lse2 = l > 0.f ? m_used + log2f(l) : -INFINITY;
+      if (sv.part_base < 0) {
+        __nv_bfloat16* orow = reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)tok * p.Hq + head) * p.D;
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+          uint32_t o[32];
+          tmem_ld32(t_o + ch * 32, o);
+          tmem_wait_ld();
+          if (row_valid) {
+#pragma unroll
+            for (int i = 0; i < 32; i += 8) {
+              uint4 w;
+              w.x = pack_bf16x2(__uint_as_float(o[i]) * inv_l, __uint_as_float(o[i + 1]) * inv_l);
+              w.y = pack_bf16x2(__uint_as_float(o[i + 2]) * inv_l, __uint_as_float(o[i + 3]) * inv_l);
+              w.z = pack_bf16x2(__uint_as_float(o[i + 4]) * inv_l, __uint_as_float(o[i + 5]) * inv_l);
+              w.w = pack_bf16x2(__uint_as_float(o[i + 6]) * inv_l, __uint_as_float(o[i + 7]) * inv_l);
+              *reinterpret_cast<uint4*>(orow + ch * 32 + i) = w;
+            }
+          }
+        }
+        if (row_valid && p.lse) p.lse[(int64_t)tok * p.Hq + head] = lse2 * 0.6931471805599453f;
+      } else {
+        const int64_t prow = (int64_t)(sv.part_base + pair) * kPairRows + R;
+        float* orow = p.part_o + prow * p.D;
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+          uint32_t o[32];
+          tmem_ld32(t_o + ch * 32, o);
+          tmem_wait_ld();
+          if (row_valid) {
+#pragma unroll
+            for (int i = 0; i < 32; i += 4) {
+              float4 w = make_float4(__uint_as_float(o[i]) * inv_l, __uint_as_float(o[i + 1]) * inv_l,
+                                     __uint_as_float(o[i + 2]) * inv_l, __uint_as_float(o[i + 3]) * inv_l);
+              *reinterpret_cast<float4*>(orow + ch * 32 + i) = w;
+            }
+          }
+        }
+        if (row_valid) p.part_lse[prow] = lse2;
+      }
+      tc_fence_before();
+      mbar_arrive(bo_empty(q));
+      ++seg_it;
+    }
+  }
+
+  __syncwarp();
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 10) {
+    tc_fence_after();
+    tmem_dealloc<kTmemCols>(tmem_base);
+  }
+}
+
+cudaError_t sm100_attn_configure() {
+  return cudaFuncSetAttribute(attn_sm100_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)kSmemBytes);
+}
+
+cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream) {
+  attn_sm100_kernel<<<l.num_ctas, kThreads, kSmemBytes, stream>>>(l.tmap_q, l.tmap_k, l.tmap_v, l.p);
+  return cudaGetLastError();
+}
+
+}  // namespace ws

@@ -1,0 +1,106 @@
+// kv_append.cu - a2: bit-exact paged KV append (commit) and its inverse (gather).
+// PAPER.md:83 "appends the received KV slice into its own full-history cache"; :29 "committed back
+// into the interaction history".  Pure data movement in 16-byte words: NaN payloads, -0 and
+// denormals are preserved.  HBM-bound; algorithmic bytes = 2 (read+write) x 2 (K,V) x n x Hkv x D x eb.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "launch.h"
+#include "ws_internal.h"
+
+namespace ws {
+
+// One thread moves one 16-byte chunk of K and the matching chunk of V.
+// chunks_per_token = Hkv * D * eb / 16; chunks_per_head = D * eb / 16.
+__global__ void __launch_bounds__(256)
+kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
+                 int4* __restrict__ k_pool, int4* __restrict__ v_pool,
+                 int32_t* __restrict__ page_table, const int32_t* __restrict__ meta,
+                 int32_t max_pages, int32_t P, int32_t Hkv, int32_t chunks_per_head) {
+  const AppendMeta hdr = *reinterpret_cast<const AppendMeta*>(meta);
+  const AppendSession* sess = reinterpret_cast<const AppendSession*>(meta + hdr.off_sessions);
+  const int32_t* pages = meta + hdr.off_pages;
+  const int32_t chunks_per_token = Hkv * chunks_per_head;
+  const int64_t total = (int64_t)hdr.total_tokens * chunks_per_token;
+
+  // Block 0 also publishes the page ids into the persistent device page table (idempotent).
+  if (blockIdx.x == 0) {
+    for (int32_t s = 0; s < hdr.num_sessions; ++s) {
+      const AppendSession a = sess[s];
+      int32_t first = a.len_old / P;
+      int32_t last = (a.len_old + (a.tok_end - a.tok_begin) + P - 1) / P;
+      for (int32_t i = first + threadIdx.x; i < last; i += blockDim.x)
+        page_table[(int64_t)a.slot * max_pages + i] = pages[a.page_off + (i - first)];
+    }
+  }
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+       idx += (int64_t)gridDim.x * blockDim.x) {
+    int32_t tok = (int32_t)(idx / chunks_per_token);
+    int32_t c = (int32_t)(idx - (int64_t)tok * chunks_per_token);
+    // session of this token: binary search over tok_end
+    int32_t lo = 0, hi = hdr.num_sessions - 1;
+    while (lo < hi) {
+      int32_t mid = (lo + hi) >> 1;
+      if (tok >= sess[mid].tok_end) lo = mid + 1; else hi = mid;
+    }
+    const AppendSession a = sess[lo];
+    int32_t pos = a.len_old + (tok - a.tok_begin);
+    int32_t page = pages[a.page_off + (pos / P - a.len_old / P)];
+    int32_t head = c / chunks_per_head;
+    int32_t off = c - head * chunks_per_head;
+    int64_t dst = (((int64_t)page * Hkv + head) * P + (pos % P)) * chunks_per_head + off;
+    k_pool[dst] = k_new[idx];
+    v_pool[dst] = v_new[idx];
+  }
+}
+
+__global__ void __launch_bounds__(256)
+kv_gather_kernel(const int4* __restrict__ k_pool, const int4* __restrict__ v_pool,
+                 int4* __restrict__ k_out, int4* __restrict__ v_out,
+                 const int32_t* __restrict__ page_row, int64_t start, int64_t count, int32_t P,
+                 int32_t Hkv, int32_t chunks_per_head) {
+  const int32_t chunks_per_token = Hkv * chunks_per_head;
+  const int64_t total = count * chunks_per_token;
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+       idx += (int64_t)gridDim.x * blockDim.x) {
+    int64_t tok = idx / chunks_per_token;
+    int32_t c = (int32_t)(idx - tok * chunks_per_token);
+    int64_t pos = start + tok;
+    int32_t page = page_row[pos / P];
+    int32_t head = c / chunks_per_head;
+    int32_t off = c - head * chunks_per_head;
+    int64_t src = (((int64_t)page * Hkv + head) * P + (pos % P)) * chunks_per_head + off;
+    if (k_out) k_out[idx] = k_pool[src];
+    if (v_out) v_out[idx] = v_pool[src];
+  }
+}
+
+cudaError_t launch_kv_append(const void* k_new, const void* v_new, void* k_pool, void* v_pool,
+                             int32_t* page_table, const int32_t* meta, int32_t total_tokens,
+                             int32_t max_pages, int32_t P, int32_t Hkv, int32_t D, int32_t eb,
+                             int32_t num_sms, cudaStream_t stream) {
+  int32_t cph = D * eb / 16;
+  int64_t total = (int64_t)total_tokens * Hkv * cph;
+  int64_t blocks = (total + 255) / 256;
+  int32_t grid = (int32_t)std::min<int64_t>(std::max<int64_t>(blocks, 1), (int64_t)num_sms * 8);
+  kv_append_kernel<<<grid, 256, 0, stream>>>((const int4*)k_new, (const int4*)v_new, (int4*)k_pool,
+                                             (int4*)v_pool, page_table, meta, max_pages, P, Hkv,
+                                             cph);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_kv_gather(const void* k_pool, const void* v_pool, void* k_out, void* v_out,
+                             const int32_t* page_row, int64_t start, int64_t count, int32_t P,
+                             int32_t Hkv, int32_t D, int32_t eb, int32_t num_sms,
+                             cudaStream_t stream) {
+  int32_t cph = D * eb / 16;
+  int64_t total = count * Hkv * cph;
+  int64_t blocks = (total + 255) / 256;
+  int32_t grid = (int32_t)std::min<int64_t>(std::max<int64_t>(blocks, 1), (int64_t)num_sms * 8);
+  kv_gather_kernel<<<grid, 256, 0, stream>>>((const int4*)k_pool, (const int4*)v_pool,
+                                             (int4*)k_out, (int4*)v_out, page_row, start, count, P,
+                                             Hkv, cph);
+  return cudaGetLastError();
+}
+
+}  // namespace ws

@@ -1,0 +1,41 @@
+// launch.h - host-callable launchers of the kernels (internal).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <algorithm>
+
+#include "ws_internal.h"
+
+namespace ws {
+
+cudaError_t launch_kv_append(const void* k_new, const void* v_new, void* k_pool, void* v_pool,
+                             int32_t* page_table, const int32_t* meta, int32_t total_tokens,
+                             int32_t max_pages, int32_t P, int32_t Hkv, int32_t D, int32_t eb,
+                             int32_t num_sms, cudaStream_t stream);
+cudaError_t launch_kv_gather(const void* k_pool, const void* v_pool, void* k_out, void* v_out,
+                             const int32_t* page_row, int64_t start, int64_t count, int32_t P,
+                             int32_t Hkv, int32_t D, int32_t eb, int32_t num_sms,
+                             cudaStream_t stream);
+
+// Generic SIMT attention (fp32 config; bf16 debug / unsupported-shape path).
+// tok_meta: [2][total_q_tokens] int32 = session slot, visible end per query token.
+cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse,
+                             const void* k_pool, const void* v_pool, const int32_t* page_table,
+                             const int32_t* tok_meta, const int32_t* q_to_kv, int32_t total_q_tokens,
+                             int32_t max_pages, int32_t Hq, int32_t Hkv, int32_t D, int32_t P,
+                             float scale, cudaStream_t stream);
+
+// sm_100a tcgen05 kernel (bf16, D = 128, P = 64).
+struct Sm100Launch {
+  AttnParams p;
+  CUtensorMap tmap_q, tmap_k, tmap_v;
+  int32_t num_ctas;
+};
+cudaError_t sm100_attn_configure();    // one-time cudaFuncSetAttribute
+cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream);
+cudaError_t launch_combine(const AttnParams& p, int32_t num_combine, int32_t team_size,
+                           cudaStream_t stream);
+
+}  // namespace ws

@@ -1,0 +1,133 @@
+// plan.cpp - see plan.h.
+//
+// Work decomposition.  A *group* is one (session, KV head, run of <= team_size row-tile pairs of
+// the session's packed query rows); every pair of a group streams the same K/V tiles.  The KV-tile
+// axes of all groups are concatenated into one flat axis of `total_tiles` tiles, which is cut into
+// `num_teams` equal ranges (stream-K style): team i owns flat tiles [i*T/n, (i+1)*T/n).  A team is
+// `team_size` CTAs launched with adjacent block ids; CTA p of the team processes pair p of whatever
+// group the team's range currently lies in, so the CTAs that share K/V tiles read them at the same
+// time and all but the first read hit in L2.  A range that covers only part of a group's tiles
+// yields a *partial* (normalised fp32 O + LSE) per pair; the combine kernel (a4) merges them.
+#include "plan.h"
+
+#include <algorithm>
+
+namespace ws {
+
+Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
+                const std::vector<int32_t>& vis_end) {
+  Plan plan;
+  const int32_t tok_per_pair = kPairRows / cfg.G;
+  int32_t max_pairs = 1;
+  for (const PlanSession& s : sessions) {
+    int32_t nq = s.q_end - s.q_begin;
+    max_pairs = std::max(max_pairs, (nq + tok_per_pair - 1) / tok_per_pair);
+  }
+  plan.team_size = std::min<int32_t>(kMaxTeam, max_pairs);
+  const int32_t Pt = plan.team_size;
+
+  std::vector<int32_t> group_tiles;
+  for (const PlanSession& s : sessions) {
+    int32_t nq = s.q_end - s.q_begin;
+    int32_t pairs = (nq + tok_per_pair - 1) / tok_per_pair;
+    for (int32_t h = 0; h < cfg.Hkv; ++h) {
+      for (int32_t b = 0; b < pairs; b += Pt) {
+        Group g{};
+        g.q_token0 = s.q_begin + b * tok_per_pair;
+        g.q_token_end = s.q_end;
+        g.kv_head = h;
+        g.slot = s.slot;
+        g.npairs = std::min(Pt, pairs - b);
+        int32_t last_tok = std::min(s.q_end, g.q_token0 + g.npairs * tok_per_pair) - 1;
+        g.kv_len = vis_end[last_tok];
+        g.vis_off = s.multi_block ? g.q_token0 : -1;
+        plan.groups.push_back(g);
+        int32_t nt = (g.kv_len + kTileKeys - 1) / kTileKeys;
+        group_tiles.push_back(nt);
+        plan.total_tiles += nt;
+      }
+    }
+  }
+  const int64_t T = plan.total_tiles;
+  int32_t teams_avail = std::max(1, cfg.num_sms / Pt);
+  int32_t min_tiles = std::max(1, cfg.min_tiles);
+  int32_t n_used = (int32_t)std::min<int64_t>(teams_avail, std::max<int64_t>(1, T / min_tiles));
+  plan.num_teams = n_used;
+
+  // walk the flat tile axis; cut at team boundaries (and at forced split boundaries)
+  int32_t team = 0;
+  int64_t flat = 0;
+  auto boundary = [&](int32_t i) { return (int64_t)i * T / n_used; };
+  for (size_t gi = 0; gi < plan.groups.size(); ++gi) {
+    int32_t nt = group_tiles[gi];
+    int32_t per = cfg.min_splits > 0 ? std::max(1, (nt + cfg.min_splits - 1) / cfg.min_splits) : nt;
+    int32_t t = 0;
+    while (t < nt) {
+      while (team + 1 < n_used && flat >= boundary(team + 1)) ++team;
+      int64_t room = (team + 1 < n_used) ? boundary(team + 1) - flat : (int64_t)nt - t;
+      int32_t take = (int32_t)std::min<int64_t>(room, nt - t);
+      take = std::min(take, per - (t % per));
+      Segment sg{(int32_t)gi, t, t + take, -1};
+      plan.segments.push_back(sg);
+      plan.seg_team.push_back(team);
+      t += take;
+      flat += take;
+    }
+  }
+  // partial slots: only groups cut into more than one segment need them
+  size_t i = 0;
+  while (i < plan.segments.size()) {
+    size_t j = i;
+    while (j < plan.segments.size() && plan.segments[j].group == plan.segments[i].group) ++j;
+    if (j - i > 1) {
+      const Group& g = plan.groups[plan.segments[i].group];
+      CombineItem c{plan.segments[i].group, plan.num_part_slots, (int32_t)(j - i), 0};
+      for (size_t k = i; k < j; ++k) {
+        plan.segments[k].part_base = plan.num_part_slots;
+        plan.num_part_slots += g.npairs;
+      }
+      plan.combine.push_back(c);
+    }
+    i = j;
+  }
+  plan.team_seg_begin.assign(n_used + 1, 0);
+  for (int32_t tm : plan.seg_team) plan.team_seg_begin[tm + 1]++;
+  for (int32_t k = 0; k < n_used; ++k) plan.team_seg_begin[k + 1] += plan.team_seg_begin[k];
+  plan.ok = plan.num_part_slots <= cfg.max_part_slots;
+  return plan;
+}
+
+std::vector<int32_t> serialise_plan(const Plan& plan, const std::vector<int32_t>& vis_end,
+                                    bool has_vis) {
+  static_assert(sizeof(Group) == 32 && sizeof(Segment) == 16 && sizeof(CombineItem) == 16 &&
+                sizeof(AttnMeta) == 48, "blob layout");
+  AttnMeta m{};
+  m.num_teams = plan.num_teams;
+  m.team_size = plan.team_size;
+  m.num_groups = (int32_t)plan.groups.size();
+  m.num_segments = (int32_t)plan.segments.size();
+  m.num_combine = (int32_t)plan.combine.size();
+  m.has_vis = has_vis ? 1 : 0;
+  int32_t off = sizeof(AttnMeta) / 4;
+  m.off_groups = off;            off += m.num_groups * (int32_t)(sizeof(Group) / 4);
+  m.off_team_seg_begin = off;    off += plan.num_teams + 1;
+  off = (off + 3) & ~3;
+  m.off_segments = off;          off += m.num_segments * (int32_t)(sizeof(Segment) / 4);
+  m.off_combine = off;           off += m.num_combine * (int32_t)(sizeof(CombineItem) / 4);
+  m.off_vis = off;               off += has_vis ? (int32_t)vis_end.size() : 0;
+  off = (off + 3) & ~3;
+  m.total_words = off;
+  std::vector<int32_t> blob(off, 0);
+  auto put = [&](int32_t at, const void* src, size_t bytes) {
+    if (bytes) std::copy((const char*)src, (const char*)src + bytes, (char*)(blob.data() + at));
+  };
+  put(0, &m, sizeof(m));
+  put(m.off_groups, plan.groups.data(), plan.groups.size() * sizeof(Group));
+  put(m.off_team_seg_begin, plan.team_seg_begin.data(), plan.team_seg_begin.size() * 4);
+  put(m.off_segments, plan.segments.data(), plan.segments.size() * sizeof(Segment));
+  put(m.off_combine, plan.combine.data(), plan.combine.size() * sizeof(CombineItem));
+  if (has_vis) put(m.off_vis, vis_end.data(), vis_end.size() * 4);
+  return blob;
+}
+
+}  // namespace ws

@@ -1,0 +1,45 @@
+// plan.h - a1: the ragged multi-session split-KV scheduler (host side, pure C++).
+// north_star: "a ragged multi-session scheduler that splits long caches across CTAs with a split-KV
+// combine kernel".  The paper itself is silent on scheduling (PAPER.md:83 only states the append).
+#pragma once
+#include <cstdint>
+#include <vector>
+
+#include "ws_internal.h"
+
+namespace ws {
+
+struct PlanSession {
+  int32_t slot;          // session slot (page-table row)
+  int32_t q_begin;       // first global query token of this session in the call
+  int32_t q_end;         // exclusive
+  bool multi_block;      // queries span more than one block (per-token visible ends differ)
+};
+
+struct PlanConfig {
+  int32_t Hkv, G;        // KV heads, q heads per KV head
+  int32_t num_sms;       // CTAs that can be resident at once (1 CTA / SM)
+  int32_t min_tiles;     // do not cut the work finer than this many KV tiles per segment
+  int32_t min_splits;    // debug: force at least this many segments per group (0 = automatic)
+  int32_t max_part_slots;
+};
+
+struct Plan {
+  int32_t team_size = 1, num_teams = 0, total_tiles = 0, num_part_slots = 0;
+  std::vector<Group> groups;
+  std::vector<int32_t> team_seg_begin;   // [num_teams + 1]
+  std::vector<Segment> segments;         // ordered by team, then by walk order
+  std::vector<int32_t> seg_team;         // team of each segment (introspection)
+  std::vector<CombineItem> combine;
+  bool ok = true;                        // false: partial slots exceed max_part_slots
+};
+
+// vis_end[t] for every global query token t (keys j < vis_end[t] are visible to token t).
+Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
+                const std::vector<int32_t>& vis_end);
+
+// Serialise into the device blob layout described by AttnMeta (ws_internal.h).
+std::vector<int32_t> serialise_plan(const Plan& plan, const std::vector<int32_t>& vis_end,
+                                    bool has_vis);
+
+}  // namespace ws

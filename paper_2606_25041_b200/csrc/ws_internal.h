@@ -1,0 +1,75 @@
+// ws_internal.h - structures shared by the host planner and the kernels (never exported).
+#pragma once
+#include <stdint.h>
+
+namespace ws {
+
+constexpr int kTileKeys = 128;    // keys per KV tile of the tensor-core kernel
+constexpr int kTileRows = 128;    // packed (token, q-head-in-group) rows per Q tile (UMMA M)
+constexpr int kPairRows = 256;    // one CTA processes a pair of Q tiles that share K/V tiles
+constexpr int kMaxTeam = 8;       // max row-tile pairs of one (session, KV head) group per team
+
+// One (session, KV head, sub-range of the session's query tokens): all of its row-tile pairs share
+// the same K/V stream, so the CTAs of one team walk the same KV tiles in lock-step (L2 reuse).
+struct Group {
+  int32_t q_token0;      // first global query token (row of q/out) covered by this group
+  int32_t q_token_end;   // end (exclusive) of the session's query tokens: rows beyond are not stored
+  int32_t kv_head;
+  int32_t slot;          // session slot = row of the device page table
+  int32_t kv_len;        // keys visible to the LAST row of the group (= max visible end)
+  int32_t npairs;        // row-tile pairs in this group (<= team size)
+  int32_t vis_off;       // >= 0: per-token visible ends at vis_end[vis_off + (token - q_token0)]
+  int32_t pad;
+};
+
+// A contiguous KV-tile range of one group, processed by one team (CTA p handles pair p).
+struct Segment {
+  int32_t group;
+  int32_t tile_begin;
+  int32_t tile_end;      // exclusive; tiles are kTileKeys keys
+  int32_t part_base;     // >= 0: partial slot of pair p is part_base + p; -1: write the final output
+};
+
+struct CombineItem {
+  int32_t group;
+  int32_t part_base;     // slot(i, p) = part_base + i * npairs + p
+  int32_t nparts;
+  int32_t pad;
+};
+
+// Header of the per-call metadata blob (all offsets in int32 words from the blob start).
+struct AttnMeta {
+  int32_t num_teams, team_size, num_groups, num_segments;
+  int32_t num_combine, has_vis, off_groups, off_team_seg_begin;
+  int32_t off_segments, off_combine, off_vis, total_words;
+};
+
+// Append metadata: per session in the call.
+struct AppendSession {
+  int32_t slot;          // page-table row
+  int32_t len_old;       // committed tokens before this append
+  int32_t tok_begin;     // cu[s]
+  int32_t tok_end;       // cu[s+1]
+  int32_t page_off;      // offset into the pages[] list of the blob: ids of the pages covering
+                         // logical page indices [len_old / P, ceil(len_new / P))
+  int32_t pad[3];
+};
+struct AppendMeta {
+  int32_t num_sessions, total_tokens, off_sessions, off_pages;
+};
+
+// Parameters common to the attention kernels.
+struct AttnParams {
+  const void* q; void* out; float* lse;
+  const void* k_pool; const void* v_pool;
+  const int32_t* page_table;   // [max_sessions][max_pages_per_session]
+  const int32_t* meta;         // AttnMeta blob (device)
+  float* part_o;               // [slots][kPairRows][D] fp32, normalised partial outputs
+  float* part_lse;             // [slots][kPairRows] fp32, log2-domain LSE (-inf = empty)
+  int32_t max_pages_per_session;
+  int32_t Hq, Hkv, D, G, P;
+  int32_t total_q_tokens;
+  float scale;
+};
+
+}  // namespace ws

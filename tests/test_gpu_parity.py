@@ -1,0 +1,369 @@
+"""GPU parity tests: the CUDA path (through the C ABI) vs the float64 oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): bf16 I/O max-abs <= 1e-2 and mean-abs <= 1e-3;
+fp32 config max-abs <= 1e-5; KV append bit-exact.  Because N(0,1) inputs at long caches make the
+outputs themselves tiny, the tests additionally gate on relative RMS error <= 1e-2,
+|dLSE| <= 1e-3 (bf16: scores rounded to fp32 from bf16 products) and closed-form / needle pins.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from synth_inputs import generate, spec_for_config, to_bf16
+from tests.gpu_harness import (compare, make_cache, preload_gpu, run_workload_gpu,
+                               run_workload_oracle, _torch_of, _numpy_of)
+
+pytestmark = pytest.mark.gpu
+
+BF16_TOL = dict(max_abs=1e-2, mean_abs=1e-3, rel_rms=1e-2, lse_max=1e-3)
+F32_TOL = dict(max_abs=1e-5, mean_abs=1e-5, rel_rms=1e-5, lse_max=1e-5)
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    import __graft_entry__ as entry
+    entry.build()
+
+
+def _assert_close(err, tol, label=""):
+    assert err["finite"], (label, err)
+    for k, v in tol.items():
+        assert err[k] <= v, (label, k, err)
+    assert err["kv_bit_exact"] in (True, None), (label, "kv append not bit exact")
+
+
+def _small(cfg, **kw):
+    return generate(spec_for_config(cfg, **kw))
+
+
+# ------------------------------------------------------------------ a2: append / gather
+def test_append_bit_exact_random_bits_and_canary():
+    """Random 16-bit patterns (NaN/Inf/denormal encodings) through ragged multi-session appends:
+    gather == concatenation, bit for bit; pages never handed out still hold the canary."""
+    import torch
+    from paper_2606_25041_b200 import WS_BF16, Cache
+    rng = np.random.default_rng(5)
+    Hkv, D, P = 4, 128, 64
+    canary = 0x7B7B
+    c = Cache(WS_BF16, 8, Hkv, D, P, num_pages=40, max_sessions=3, max_q_tokens_per_call=1024,
+              pool_fill=canary)
+    c.shuffle_free_pages(99)
+    ids = [c.session_open() for _ in range(3)]
+    logs = {i: ([], []) for i in ids}
+    plan = [([0], [37]), ([1, 2], [64, 1]), ([0, 1, 2], [91, 130, 200]), ([2], [63]), ([0, 2], [128, 5])]
+    dev = torch.device("cuda", 0)
+    for sess, ns in plan:
+        tot = sum(ns)
+        kb = rng.integers(0, 65536, size=(tot, Hkv, D), dtype=np.uint16)
+        vb = rng.integers(0, 65536, size=(tot, Hkv, D), dtype=np.uint16)
+        k = torch.from_numpy(kb.view(np.int16)).to(dev).view(torch.bfloat16)
+        v = torch.from_numpy(vb.view(np.int16)).to(dev).view(torch.bfloat16)
+        cu = np.concatenate([[0], np.cumsum(ns)])
+        c.kv_append([ids[s] for s in sess], cu, k, v)
+        for j, s in enumerate(sess):
+            logs[ids[s]][0].append(kb[cu[j]:cu[j + 1]]); logs[ids[s]][1].append(vb[cu[j]:cu[j + 1]])
+    used = set()
+    for i in ids:
+        tokens, blocks, ends = c.session_info(i)
+        kref = np.concatenate(logs[i][0]); vref = np.concatenate(logs[i][1])
+        assert tokens == len(kref) and ends[-1] == tokens
+        kg = torch.empty((tokens, Hkv, D), dtype=torch.bfloat16, device=dev); vg = torch.empty_like(kg)
+        c.kv_gather(i, 0, tokens, kg, vg)
+        torch.cuda.synchronize()
+        assert kg.view(torch.int16).cpu().numpy().view(np.uint16).tobytes() == kref.tobytes()
+        assert vg.view(torch.int16).cpu().numpy().view(np.uint16).tobytes() == vref.tobytes()
+        # partial gather in the middle
+        if tokens > 70:
+            kg2 = torch.empty((50, Hkv, D), dtype=torch.bfloat16, device=dev)
+            c.kv_gather(i, 20, 50, kg2, None)
+            torch.cuda.synchronize()
+            assert kg2.view(torch.int16).cpu().numpy().view(np.uint16).tobytes() == kref[20:70].tobytes()
+        used |= set(c.session_pages(i))
+    free = sorted(set(range(40)) - used)
+    assert len(free) == c.free_pages() and free
+    kp = c.k_pool.view(torch.int16).cpu().numpy().view(np.uint16)
+    vp = c.v_pool.view(torch.int16).cpu().numpy().view(np.uint16)
+    assert (kp[free] == canary).all() and (vp[free] == canary).all()
+
+
+# ------------------------------------------------------------------ config 1 (fp32, CUDA cores)
+def test_config1_tiny_fp32_incremental():
+    w = generate(spec_for_config(1))
+    got = run_workload_gpu(w)
+    assert not got["tensor"]
+    _assert_close(compare(got, run_workload_oracle(w), "f32"), F32_TOL, "cfg1")
+
+
+def test_config1_one_shot_equals_incremental_and_oracle():
+    """num_q_blocks = 3: the whole 48-token stream in one call (multi-block query)."""
+    import torch
+    from oracle.block_causal import OracleSession, attend
+    w = generate(spec_for_config(1))
+    si = w.sessions[0]
+    cache = make_cache(w, extra_q_tokens=48)
+    sid = cache.session_open()
+    dev = torch.device("cuda", 0)
+    sess = OracleSession(2, 64)
+    for t in range(3):
+        cache.kv_append([sid], [0, 16], _torch_of(si.k[t], dev), _torch_of(si.v[t], dev))
+        sess.append(si.k[t], si.v[t])
+    q = np.concatenate(si.q)
+    out = torch.empty((48, 2, 64), dtype=torch.float32, device=dev)
+    lse = torch.empty((48, 2), dtype=torch.float32, device=dev)
+    cache.block_causal_attn_fwd([sid], [0, 48], _torch_of(q, dev), out, w.spec.scale, lse=lse,
+                                num_q_blocks=[3])
+    torch.cuda.synchronize()
+    o_ref, l_ref = attend(sess, q, w.spec.scale, 3)
+    assert np.abs(out.cpu().numpy() - o_ref).max() <= 1e-5
+    assert np.abs(lse.cpu().numpy() - l_ref).max() <= 1e-5
+    inc = run_workload_gpu(w)
+    o_inc = np.concatenate([inc["out"][t][0] for t in range(3)])
+    assert np.abs(out.cpu().numpy() - o_inc).max() <= 2e-6
+
+
+def test_fp32_other_page_size_and_explicit_head_map():
+    import torch
+    from oracle.block_causal import OracleSession, attend
+    from paper_2606_25041_b200 import WS_F32, Cache
+    rng = np.random.default_rng(8)
+    Hq, Hkv, D = 4, 2, 40
+    mapping = [1, 0, 0, 1]
+    c = Cache(WS_F32, Hq, Hkv, D, 64, num_pages=8, max_sessions=1, q_to_kv_head=mapping)
+    sid = c.session_open()
+    dev = torch.device("cuda", 0)
+    sess = OracleSession(Hkv, D)
+    for n in (70, 33):
+        k = rng.standard_normal((n, Hkv, D), dtype=np.float32); v = rng.standard_normal((n, Hkv, D), dtype=np.float32)
+        c.kv_append([sid], [0, n], _torch_of(k, dev), _torch_of(v, dev)); sess.append(k, v)
+    q = rng.standard_normal((33, Hq, D), dtype=np.float32)
+    out = torch.empty((33, Hq, D), dtype=torch.float32, device=dev)
+    c.block_causal_attn_fwd([sid], [0, 33], _torch_of(q, dev), out, 0.2)
+    torch.cuda.synchronize()
+    o_ref, _ = attend(sess, q, 0.2, 1, q_to_kv=mapping)
+    assert np.abs(out.cpu().numpy() - o_ref).max() <= 1e-5
+
+
+# ------------------------------------------------------------------ bf16: generic kernel (second opinion)
+def test_bf16_generic_simt_kernel_small():
+    from paper_2606_25041_b200 import WS_FLAG_FORCE_SIMT
+    w = _small(2, cache_lens=(300,), num_q_heads=4, num_kv_heads=2, block_tokens=40,
+               modality_split=(30, 8, 2), steps=2)
+    got = run_workload_gpu(w, flags=WS_FLAG_FORCE_SIMT)
+    assert not got["tensor"]
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "simt bf16")
+
+
+# ------------------------------------------------------------------ bf16: tcgen05 kernel, small shapes
+SMALL_TC = [
+    # (label, overrides) - several KV tiles, ragged tails, empty cache, G in {1, 2, 4, 8}
+    ("mha_1tile_pair", dict(cache_lens=(128,), num_q_heads=2, num_kv_heads=2, block_tokens=128, modality_split=(96, 24, 8))),
+    ("empty_cache_ragged", dict(cache_lens=(0,), num_q_heads=4, num_kv_heads=1, block_tokens=72, modality_split=(54, 12, 6))),
+    ("gqa4_ragged_tail", dict(cache_lens=(1000,), num_q_heads=8, num_kv_heads=2, block_tokens=96, modality_split=(72, 18, 6), steps=2)),
+    ("gqa8_tail_le_64", dict(cache_lens=(531,), num_q_heads=8, num_kv_heads=1, block_tokens=40, modality_split=(30, 8, 2))),
+    ("gqa2_multi_pair", dict(cache_lens=(700,), num_q_heads=4, num_kv_heads=2, block_tokens=300, modality_split=(200, 80, 20))),
+    ("mha_aligned", dict(cache_lens=(2048,), num_q_heads=4, num_kv_heads=4, block_tokens=256)),
+]
+
+
+@pytest.mark.parametrize("label,ov", SMALL_TC, ids=[x[0] for x in SMALL_TC])
+def test_bf16_tensor_core_kernel_small(label, ov):
+    w = _small(2, **ov)
+    got = run_workload_gpu(w, pool_fill=0x7FC1)            # NaN canary in unused cache slots
+    assert got["tensor"]
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, label)
+
+
+@pytest.mark.parametrize("splits", [1, 2, 3, 7])
+def test_split_count_invariance(splits):
+    w = _small(3, cache_lens=(3000,), block_tokens=128, modality_split=(96, 24, 8))
+    got = run_workload_gpu(w, min_splits=splits)
+    assert got["tensor"]
+    if splits > 1:
+        assert got["plans"][-1]["num_combine_items"] > 0
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, f"splits={splits}")
+
+
+def test_page_assignment_independence():
+    w = _small(3, cache_lens=(1500,), block_tokens=64, modality_split=(48, 12, 4))
+    a = run_workload_gpu(w, gather=False)
+    b = run_workload_gpu(w, gather=False, shuffle_seed=4242)
+    np.testing.assert_array_equal(a["out"][0][0], b["out"][0][0])
+
+
+def test_ragged_multi_session_small_and_batched_equals_single():
+    w = _small(5, cache_len_range=(100, 1500), block_tokens=64, modality_split=(48, 12, 4))
+    got = run_workload_gpu(w)
+    ref = run_workload_oracle(w)
+    _assert_close(compare(got, ref, "bf16"), BF16_TOL, "ragged small")
+    # each session alone (same inputs) gives the same output within fp tolerance of the oracle
+    import dataclasses
+    for s in (0, 5):
+        solo = dataclasses.replace(w, spec=dataclasses.replace(w.spec, num_sessions=1),
+                                   cache_lens=[w.cache_lens[s]], sessions=[w.sessions[s]])
+        g1 = run_workload_gpu(solo, gather=False)
+        assert np.abs(g1["out"][0][0] - ref["out"][0][s]).max() <= 1e-2
+        assert np.abs(g1["out"][0][0] - got["out"][0][s]).max() <= 4e-3
+
+
+def test_multi_block_query_tensor_core():
+    """Three committed blocks queried in one call on the tcgen05 path (partial / skipped tiles)."""
+    import torch
+    from oracle.block_causal import OracleSession, attend
+    w = _small(2, cache_lens=(200,), num_q_heads=4, num_kv_heads=2, block_tokens=150,
+               modality_split=(100, 40, 10), steps=3)
+    si = w.sessions[0]
+    cache = make_cache(w, extra_q_tokens=450)
+    dev = torch.device("cuda", 0)
+    ids = preload_gpu(cache, w, [_torch_of(si.k_cache, dev)], [_torch_of(si.v_cache, dev)])
+    sess = OracleSession(2, 128); sess.append(si.k_cache, si.v_cache)
+    for t in range(3):
+        cache.kv_append(ids, [0, 150], _torch_of(si.k[t], dev), _torch_of(si.v[t], dev))
+        sess.append(si.k[t], si.v[t])
+    q = np.concatenate(si.q)
+    out = torch.empty((450, 4, 128), dtype=torch.bfloat16, device=dev)
+    lse = torch.empty((450, 4), dtype=torch.float32, device=dev)
+    cache.block_causal_attn_fwd(ids, [0, 450], _torch_of(q, dev), out, w.spec.scale, lse=lse, num_q_blocks=[3])
+    torch.cuda.synchronize()
+    assert cache.last_plan_info()["used_tensor_core_kernel"] == 1
+    o_ref, l_ref = attend(sess, q, w.spec.scale, 3)
+    d = out.float().cpu().numpy() - o_ref
+    assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3
+    assert np.abs(lse.cpu().numpy() - l_ref).max() <= 1e-3
+
+
+# ------------------------------------------------------------------ closed-form pins on the GPU
+def _run_custom_bf16(L, n, Hq, Hkv, kc, vc, q, kn, vn, scale, min_splits=0):
+    """single session, cache (kc, vc) then one block (kn, vn) with queries q; returns (O, LSE)."""
+    import torch
+    from paper_2606_25041_b200 import WS_BF16, Cache
+    P = 64
+    pages = (L + n + P - 1) // P + 2
+    c = Cache(WS_BF16, Hq, Hkv, 128, P, pages, max_sessions=1, max_q_tokens_per_call=max(n, 256))
+    if min_splits:
+        c.set_min_splits(min_splits)
+    sid = c.session_open()
+    dev = torch.device("cuda", 0)
+    pos = 0
+    while pos < L:
+        hi = min(L, pos + 256)
+        c.kv_append([sid], [0, hi - pos], _torch_of(kc[pos:hi], dev), _torch_of(vc[pos:hi], dev)); pos = hi
+    c.kv_append([sid], [0, n], _torch_of(kn, dev), _torch_of(vn, dev))
+    out = torch.empty((n, Hq, 128), dtype=torch.bfloat16, device=dev)
+    lse = torch.empty((n, Hq), dtype=torch.float32, device=dev)
+    c.block_causal_attn_fwd([sid], [0, n], _torch_of(q, dev), out, scale, lse=lse)
+    torch.cuda.synchronize()
+    assert c.last_plan_info()["used_tensor_core_kernel"] == 1
+    return out.float().cpu().numpy(), lse.cpu().numpy(), c.last_plan_segments()
+
+
+def test_needle_addressing_every_boundary():
+    """P3: q = u, K[j*] = 4u, all other K = 0, V rows distinct -> O == V[j*] exactly (bf16)."""
+    L, n, Hq, Hkv = 1000 + 37, 64, 4, 2
+    rng = np.random.default_rng(3)
+    u = rng.choice([-1.0, 1.0], size=128).astype(np.float32)
+    v_all = to_bf16(rng.standard_normal((L + n, Hkv, 128), dtype=np.float32))
+    q = to_bf16(np.tile(u, (n, Hq, 1)))
+    scale = 1.0 / math.sqrt(128)
+    _, _, segs = _run_custom_bf16(L, n, Hq, Hkv, to_bf16(np.zeros((L, Hkv, 128), np.float32)), v_all[:L], q,
+                                  to_bf16(np.zeros((n, Hkv, 128), np.float32)), v_all[L:], scale, min_splits=3)
+    cuts = sorted({s["tile_begin"] * 128 for s in segs} | {s["tile_end"] * 128 for s in segs})
+    targets = {0, 63, 64, 127, 128, L - 1, L, L + n - 1, L + n - 2}
+    for cpos in cuts:
+        targets |= {cpos - 1, cpos, cpos + 1}
+    for jstar in sorted(t for t in targets if 0 <= t < L + n):
+        k_all = np.zeros((L + n, Hkv, 128), np.float32)
+        k_all[jstar] = 4.0 * u
+        k_all = to_bf16(k_all)
+        o, lse, _ = _run_custom_bf16(L, n, Hq, Hkv, k_all[:L], v_all[:L], q, k_all[L:], v_all[L:], scale, min_splits=3)
+        want = v_all[jstar].astype(np.float32)                 # [Hkv, 128]
+        for h in range(Hq):
+            np.testing.assert_array_equal(o[:, h, :], np.tile(want[h // 2], (n, 1)), err_msg=f"j*={jstar}")
+
+
+def test_visible_count_lse_and_constant_v():
+    """P4: Q == 0 -> LSE = ln(#keys) (one dropped / duplicated key moves it by >= 1/N); P6: V == c -> O == c."""
+    L, n, Hq, Hkv = 4096 + 50, 256, 4, 4
+    rng = np.random.default_rng(4)
+    k_all = to_bf16(rng.standard_normal((L + n, Hkv, 128), dtype=np.float32))
+    v_all = to_bf16(np.full((L + n, Hkv, 128), 1.75, np.float32))
+    q0 = to_bf16(np.zeros((n, Hq, 128), np.float32))
+    o, lse, _ = _run_custom_bf16(L, n, Hq, Hkv, k_all[:L], v_all[:L], q0, k_all[L:], v_all[L:], 0.1)
+    assert np.abs(lse - math.log(L + n)).max() < 0.2 / (L + n)
+    np.testing.assert_array_equal(o, 1.75)
+    q = to_bf16(rng.standard_normal((n, Hq, 128), dtype=np.float32))
+    o, _, _ = _run_custom_bf16(L, n, Hq, Hkv, k_all[:L], v_all[:L], q, k_all[L:], v_all[L:], 0.1, min_splits=4)
+    np.testing.assert_allclose(o, 1.75, atol=1.75 * 2 ** -8)
+
+
+def test_large_scores_do_not_overflow():
+    """P5: scores of +-60 (x log2e) must not overflow or NaN; compared with the oracle."""
+    w = _small(5, num_sessions=2, cache_len_range=(500, 900), block_tokens=64, modality_split=(48, 12, 4),
+               outlier_frac=0.25, outlier_scale=8.0)
+    got = run_workload_gpu(w)
+    err = compare(got, run_workload_oracle(w), "bf16")
+    assert err["finite"] and err["max_abs"] <= 2e-2 and err["rel_rms"] <= 1e-2, err
+
+
+# ------------------------------------------------------------------ BASELINE configs at full size
+def _sample(n, Hq, k=24, seed=0):
+    rng = np.random.default_rng(seed)
+    rows = np.unique(np.concatenate([[0, n - 1], rng.integers(0, n, size=k)]))
+    heads = np.unique(np.concatenate([[0, Hq - 1], rng.integers(0, Hq, size=6)]))
+    return rows, heads
+
+
+def test_config2_full_size():
+    w = generate(spec_for_config(2))
+    got = run_workload_gpu(w)
+    assert got["tensor"]
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "cfg2")
+
+
+def test_config3_full_size_sampled():
+    w = generate(spec_for_config(3))
+    rows, heads = _sample(512, 32, seed=3)
+    got = run_workload_gpu(w)
+    ref = run_workload_oracle(w, rows=rows, heads=heads)
+    _assert_close(compare(got, ref, "bf16", rows=rows, heads=heads), BF16_TOL, "cfg3")
+
+
+def test_config4_long_session_20_steps_sampled():
+    w = generate(spec_for_config(4))
+    rows, heads = _sample(256, 32, k=12, seed=4)
+    got = run_workload_gpu(w)
+    assert got["tensor"] and got["plans"][0]["num_ctas"] == 148
+    ref = run_workload_oracle(w, rows=rows, heads=heads, steps=(0, 7, 19))
+    err = compare(got, ref, "bf16", rows=rows, heads=heads)
+    _assert_close(err, BF16_TOL, "cfg4")
+    # every step's output is finite and non-trivial
+    for t in range(20):
+        o = got["out"][t][0]
+        assert np.isfinite(o).all() and 0.003 < o.std() < 0.02
+
+
+def test_config5_ragged_multi_session_sampled():
+    w = generate(spec_for_config(5))
+    rows, heads = _sample(256, 32, k=12, seed=5)
+    got = run_workload_gpu(w)
+    ref = run_workload_oracle(w, rows=rows, heads=heads)
+    _assert_close(compare(got, ref, "bf16", rows=rows, heads=heads), BF16_TOL, "cfg5")
+
+
+def test_stream_step_host_end_to_end():
+    """ws_stream_step_host: pinned host buffers in, host result out, equals the device-pointer path."""
+    import torch
+    w = _small(3, cache_lens=(900,), block_tokens=128, modality_split=(96, 24, 8))
+    si = w.sessions[0]
+    dev = torch.device("cuda", 0)
+    cache = make_cache(w)
+    ids = preload_gpu(cache, w, [_torch_of(si.k_cache, dev)], [_torch_of(si.v_cache, dev)])
+    pin = lambda a: torch.from_numpy(a.view(np.uint16).copy()).view(torch.bfloat16).pin_memory()
+    qh, kh, vh = pin(si.q[0]), pin(si.k[0]), pin(si.v[0])
+    oh = torch.empty_like(qh).pin_memory()
+    staging = torch.empty(cache.step_staging_bytes(128), dtype=torch.uint8, device=dev)
+    cache.stream_step_host(ids, [0, 128], qh, kh, vh, oh, staging, w.spec.scale)
+    torch.cuda.synchronize()
+    ref = run_workload_oracle(w)
+    d = oh.float().numpy() - ref["out"][0][0]
+    assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3
