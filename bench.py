@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py - block-causal streaming attention on B200: TFLOP/s and us per streaming unit.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
+
+A "step" is one streaming unit of the hot path: ws_kv_append (commit the unit's K/V block) followed by
+ws_block_causal_attn_fwd (the block attends to the full history; includes the split-KV combine).
+Headline workload = BASELINE.json configs[3] ("bf16 long session": 32 q / 8 kv heads, D=128, block of
+256 tokens, cache 65536 growing over 20 consecutive units) - the configuration the north_star's 60 %
+target is quoted on.  After 20 units the session is rolled back (host metadata only) and replayed.
+K/V history (269-289 MB) exceeds the 126 MB L2, so no explicit flush is needed between steps.
+
+Prints ONE JSON line (see DESIGN.md "Measurement" for every field).  `--impl reference` times the
+float64 numpy oracle on the host cores on a bounded sample of the same workload (rank 0 only).
+N > 1: one process per GPU, each rank streams its own independent session (weak scaling, no
+data-path collective); torch.distributed is used for the barrier and the max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from synth_inputs import CONFIG_SPECS, algorithmic_bytes, algorithmic_flops, generate, spec_for_config  # noqa: E402
+
+NOMINAL_BF16_TFLOPS, NOMINAL_HBM_GBS = 2250.0, 8000.0
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d, "measured (MEASURED_PEAKS.json)"
+    return dict(FALLBACK_PEAKS), "fallback (B200_PROFILING.md)"
+
+
+def oracle_threads() -> int:
+    try:
+        from threadpoolctl import threadpool_info
+        import numpy  # noqa: F401
+        n = [i["num_threads"] for i in threadpool_info() if i.get("user_api") == "blas"]
+        return max(n) if n else (os.cpu_count() or 1)
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def oracle_sample_seconds(w, rows, budget_steps=1):
+    """Time the oracle (as it stands) on `rows` query tokens x all heads of step 0. Returns (s, flops)."""
+    from tests.gpu_harness import preload_rounds
+    from oracle.block_causal import OracleSession, attend
+    sp = w.spec
+    sess = []
+    for s, si in enumerate(w.sessions):
+        o = OracleSession(sp.num_kv_heads, sp.head_dim)
+        for ids, rng in preload_rounds(w):
+            for sidx, (lo, hi) in zip(ids, rng):
+                if sidx == s:
+                    o.append(si.k_cache[lo:hi], si.v_cache[lo:hi])
+        sess.append(o)
+    t0 = time.perf_counter()
+    flops = 0.0
+    for _ in range(budget_steps):
+        for s, si in enumerate(w.sessions):
+            sess[s].append(si.k[0], si.v[0])
+            attend(sess[s], si.q[0], sp.scale, 1, rows=rows)
+            flops += 4.0 * sp.head_dim * sp.num_q_heads * len(rows) * sess[s].length
+            # roll back so that every repetition times the same work
+            sess[s].k_slices.pop(); sess[s].v_slices.pop(); sess[s].block_ends.pop()
+    return time.perf_counter() - t0, flops
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        super().__init__(daemon=True)
+        self.index, self.period, self.stop_flag = index, period_s, threading.Event()
+        self.sm, self.reasons, self.max_mhz, self.err = [], set(), None, None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40,
+                     "sw_thermal_slowdown": 0x20, "hw_power_brake_slowdown": 0x80,
+                     "applications_clocks_setting": 0x2, "sync_boost": 0x10}
+            while not self.stop_flag.is_set():
+                self.sm.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+                time.sleep(self.period)
+        except Exception as e:  # pragma: no cover
+            self.err = repr(e)
+
+    def result(self):
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.sm),
+                **({"error": self.err} if self.err else {})}
+
+
+def read_traffic(cfg: int):
+    """dram bytes per launch of the attention kernel from the committed ncu summary, or None."""
+    p = os.path.join(ROOT, "profiles", f"traffic_cfg{cfg}.txt")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        if line.startswith("dram_bytes_per_launch"):
+            return float(line.split()[1])
+    return None
+
+
+def run_reference(args, spec):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = generate(spec_for_config(spec.cfg, steps=1))
+    nrows = args.ref_rows
+    rows = np.linspace(0, spec.block_tokens - 1, nrows).astype(np.int64)
+    for _ in range(args.warmup):
+        oracle_sample_seconds(w, rows[:2])
+    t, fl = 0.0, 0.0
+    for _ in range(args.steps):
+        dt, f = oracle_sample_seconds(w, rows)
+        t += dt; fl += f
+    tflops = fl / t / 1e12
+    cores = oracle_threads()
+    sample = (f"{nrows} of {spec.block_tokens} query tokens x all {spec.num_q_heads} heads per session, "
+              f"full history, unit 1 of the loop; FLOPs counted for the sampled rows only")
+    line = {"impl": "reference", "metric": "block_causal_attn_tflops", "value": tflops, "unit": "TFLOP/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": spec.name, "sample": sample},
+            "cpu_baseline": {"value": tflops, "unit": "TFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": tflops, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=40)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE config 2..5 (default 4 = headline)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-rows", type=int, default=32)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    spec = CONFIG_SPECS[args.config]
+    if args.impl == "reference":
+        if args.steps == 1000:
+            args.steps, args.warmup = 3, 1
+        return run_reference(args, spec)
+
+    import torch
+    import __graft_entry__ as entry
+    entry.build()
+    from paper_2606_25041_b200 import Cache, WS_BF16  # noqa: F401
+    from tests.gpu_harness import make_cache, preload_gpu, _torch_of
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback exists for this path)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    peaks, peak_src = load_peaks()
+    dev = torch.device("cuda", local)
+    w = generate(spec)                                  # same seeded inputs on every rank (replica)
+    sp = w.spec
+    S, n, steps_per_cycle = sp.num_sessions, sp.block_tokens, sp.steps
+    # ---- device-resident inputs
+    cache = make_cache(w, device=local)
+    dev_k = [_torch_of(s.k_cache, dev) for s in w.sessions]
+    dev_v = [_torch_of(s.v_cache, dev) for s in w.sessions]
+    ids = preload_gpu(cache, w, dev_k, dev_v)
+    del dev_k, dev_v
+    base_blocks = [cache.session_info(i)[1] for i in ids]
+    cu = [i * n for i in range(S + 1)]
+    q_d = [torch.cat([_torch_of(s.q[t], dev) for s in w.sessions]) for t in range(steps_per_cycle)]
+    k_d = [torch.cat([_torch_of(s.k[t], dev) for s in w.sessions]) for t in range(steps_per_cycle)]
+    v_d = [torch.cat([_torch_of(s.v[t], dev) for s in w.sessions]) for t in range(steps_per_cycle)]
+    out = torch.empty_like(q_d[0])
+    stream = torch.cuda.current_stream()
+
+    def reset():
+        for sid, b in zip(ids, base_blocks):
+            cache.session_truncate(sid, b)
+
+    def step(i):
+        t = i % steps_per_cycle
+        if t == 0:
+            reset()
+        cache.kv_append(ids, cu, k_d[t], v_d[t], stream=stream)
+        cache.block_causal_attn_fwd(ids, cu, q_d[t], out, sp.scale, stream=stream)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(nsteps, fn, first=0):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(stream)
+        for i in range(first, first + nsteps):
+            fn(i)
+        e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([ms], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    flops_cycle = [algorithmic_flops(sp, w.cache_lens, t) for t in range(steps_per_cycle)]
+    bytes_cycle = [algorithmic_bytes(sp, w.cache_lens, t) for t in range(steps_per_cycle)]
+
+    def work(nsteps, fn):
+        return sum(fn[i % steps_per_cycle] for i in range(nsteps))
+
+    K, W = args.steps, max(args.warmup, 3)
+    for i in range(W):
+        step(i)
+    # ---- pass A: whole-step throughput (no per-kernel events), clocks sampled during the region
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.05)
+    launches0 = cache.launch_count()
+    ms_total = timed(K, step)
+    launches = cache.launch_count() - launches0
+    sampler.stop_flag.set(); sampler.join(timeout=2)
+    flops_total = work(K, flops_cycle)
+    ms_per_step = ms_total / K
+    value = world * flops_total / (ms_total * 1e-3) / 1e12
+    # ---- pass B: same region with an event pair around every kernel launch (roofline)
+    cache.kernel_timing(True)
+    cache.read_kernel_times()
+    ms_total_b = timed(K, step)
+    kt = cache.read_kernel_times()
+    cache.kernel_timing(False)
+    attn_ms = kt["attn"][0] / max(1, kt["attn"][1])
+    comb_ms = kt["combine"][0] / max(1, kt["combine"][1])
+    app_ms = kt["append"][0] / max(1, kt["append"][1])
+    flops_per_launch = flops_total / K
+    achieved = flops_per_launch / (attn_ms * 1e-3) / 1e12
+    peak = float(peaks["bf16_tflops"])
+    kv_bytes_per_launch = work(K, bytes_cycle) / K
+    plan = cache.last_plan_info()
+    roofline = {"bound": "tensor", "kernel": "attn_sm100_kernel", "achieved": achieved, "peak": peak,
+                "unit": "TFLOP/s", "frac": achieved / peak, "peak_source": peak_src + " bf16 burst",
+                "traffic": read_traffic(args.config),
+                "frac_of_sustained": achieved / float(peaks.get("bf16_tflops_sustained", peak)),
+                "frac_of_nominal_2250": achieved / NOMINAL_BF16_TFLOPS,
+                "flops_per_launch": flops_per_launch, "algorithmic_bytes_per_step": kv_bytes_per_launch,
+                "kernel_us": {"attn": attn_ms * 1e3, "combine": comb_ms * 1e3, "append": app_ms * 1e3},
+                "attn_share_of_step": attn_ms / (ms_total_b / K),
+                "hbm_gbs_achieved_step": kv_bytes_per_launch / (ms_per_step * 1e-3) / 1e9,
+                "hbm_gbs_peak": float(peaks["hbm_gbs"]),
+                "step_roofline_us": 1e6 * max(flops_per_launch / (peak * 1e12),
+                                             kv_bytes_per_launch / (float(peaks["hbm_gbs"]) * 1e9)),
+                "step_frac_of_roofline": max(flops_per_launch / (peak * 1e12),
+                                             kv_bytes_per_launch / (float(peaks["hbm_gbs"]) * 1e9)) / (ms_per_step * 1e-3),
+                "ms_per_step_with_kernel_events": ms_total_b / K}
+
+    # ---- e2e: HOST buffers through ws_stream_step_host, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda t: t.cpu().pin_memory()
+        qh, kh, vh = [pin(x) for x in q_d], [pin(x) for x in k_d], [pin(x) for x in v_d]
+        oh = torch.empty_like(qh[0]).pin_memory()
+        staging = torch.empty(cache.step_staging_bytes(S * n), dtype=torch.uint8, device=dev)
+
+        def step_host(i):
+            t = i % steps_per_cycle
+            if t == 0:
+                reset()
+            cache.stream_step_host(ids, cu, qh[t], kh[t], vh[t], oh, staging, sp.scale, stream=stream)
+
+        Ke = max(20, K // 5)
+        for i in range(3 * steps_per_cycle if steps_per_cycle <= 4 else steps_per_cycle):
+            step_host(i)
+        ms_e = timed(Ke, step_host)
+        h2d = qh[0].numel() * 2 + kh[0].numel() * 2 + vh[0].numel() * 2
+        e2e = {"value": world * work(Ke, flops_cycle) / (ms_e * 1e-3) / 1e12, "unit": "TFLOP/s",
+               "us_per_unit": 1e3 * ms_e / Ke, "steps": Ke,
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(oh.numel() * 2),
+               "api": "ws_stream_step_host (pinned host q/k/v in, pinned host out)"}
+
+    # ---- CPU baseline: the oracle on a bounded sample, rank 0 at N=1 only
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        rows = np.linspace(0, n - 1, args.ref_rows).astype(np.int64)
+        w1 = w
+        dt, fl = oracle_sample_seconds(w1, rows)
+        cpu = {"value": fl / dt / 1e12, "unit": "TFLOP/s", "cores": oracle_threads(), "kind": "oracle",
+               "seconds": dt,
+               "sample": f"{len(rows)} of {n} query tokens x all {sp.num_q_heads} heads per session, full "
+                         f"history, unit 1; FLOPs counted for the sampled rows only"}
+
+    if rank == 0:
+        line = {"metric": "block_causal_attn_tflops", "value": value, "unit": "TFLOP/s",
+                "us_per_unit": ms_per_step * 1e3, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                "config": {"workload": sp.name, "baseline_config_index": args.config - 1,
+                           "sessions_per_gpu": S, "q_heads": sp.num_q_heads, "kv_heads": sp.num_kv_heads,
+                           "head_dim": sp.head_dim, "block_tokens": n, "cache_tokens": w.cache_lens,
+                           "units_per_cycle": steps_per_cycle, "page_tokens": sp.page_tokens,
+                           "l2": "inputs larger than L2 (K/V history %.0f MB per step vs 126 MB L2)" % (bytes_cycle[0] / 1e6)
+                                 if bytes_cycle[0] > 2 * 126e6 else "history fits L2: numbers are L2-warm",
+                           "parallelism": f"dp{world} (independent sessions per GPU, no collective)",
+                           "plan": plan},
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+                "clocks": sampler.result(),
+                "context": {"paper_model_side_latency_ms": 200, "paper_total_latency_ms": 550,
+                            "paper_hardware": "two-GPU thinker-performer path, GPU model not stated (PAPER.md:89)",
+                            "streaming_unit_ms": 160}}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

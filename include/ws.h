@@ -174,6 +174,13 @@ ws_status_t ws_last_plan_segment(const ws_cache_t* cache, int32_t i, ws_plan_seg
 /* Number of kernels this library has launched on `cache` since creation (bench `gpu_launches`). */
 int64_t ws_launch_count(const ws_cache_t* cache);
 
+/* Bench instrumentation: when enabled, every kernel launch of this cache is bracketed by a CUDA
+ * event pair recorded on the launch stream.  ws_debug_read_kernel_times synchronises those events
+ * and returns, for {append, attention, combine} in that order, the summed device milliseconds and
+ * the number of launches since the last read (then forgets them). */
+ws_status_t ws_debug_kernel_timing(ws_cache_t* cache, int32_t enable);
+ws_status_t ws_debug_read_kernel_times(ws_cache_t* cache, double* ms_sum3, int32_t* count3);
+
 const char* ws_status_str(ws_status_t s);
 const char* ws_last_error(void);
 const char* ws_version(void);

@@ -56,7 +56,8 @@ EXPORTS = ["ws_pool_bytes", "ws_workspace_bytes", "ws_cache_create", "ws_cache_d
            "ws_free_pages", "ws_kv_append", "ws_block_causal_attn_fwd", "ws_step_staging_bytes",
            "ws_stream_step_host", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
            "ws_debug_set_min_splits", "ws_last_plan_info", "ws_last_plan_segment",
-           "ws_launch_count", "ws_status_str", "ws_last_error", "ws_version"]
+           "ws_launch_count", "ws_debug_kernel_timing", "ws_debug_read_kernel_times",
+           "ws_status_str", "ws_last_error", "ws_version"]
 
 _lib = None
 
@@ -96,6 +97,8 @@ def load_library() -> C.CDLL:
     lib.ws_last_plan_info.argtypes = [vp, C.POINTER(PlanInfo)]
     lib.ws_last_plan_segment.argtypes = [vp, C.c_int32, C.POINTER(PlanSegment)]
     lib.ws_launch_count.argtypes = [vp]; lib.ws_launch_count.restype = C.c_int64
+    lib.ws_debug_kernel_timing.argtypes = [vp, C.c_int32]
+    lib.ws_debug_read_kernel_times.argtypes = [vp, C.POINTER(C.c_double), i32p]
     lib.ws_status_str.argtypes = [C.c_int]; lib.ws_status_str.restype = C.c_char_p
     lib.ws_last_error.restype = C.c_char_p
     lib.ws_version.restype = C.c_char_p
@@ -271,6 +274,15 @@ class Cache:
 
     def launch_count(self) -> int:
         return self.lib.ws_launch_count(self.handle)
+
+    def kernel_timing(self, enable: bool) -> None:
+        _check(self.lib.ws_debug_kernel_timing(self.handle, int(enable)))
+
+    def read_kernel_times(self) -> dict:
+        """{'append'|'attn'|'combine': (sum_ms, launches)} since the last read."""
+        ms, cnt = (C.c_double * 3)(), (C.c_int32 * 3)()
+        _check(self.lib.ws_debug_read_kernel_times(self.handle, ms, cnt))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(("append", "attn", "combine"))}
 
 
 # ---- module-level functions with the C names (same marshalling) -------------------------------

@@ -121,6 +121,10 @@ struct ws_cache {
   int64_t launches = 0;
   ws::Plan last_plan;
   bool last_tensor = false;
+  // optional per-kernel timing (bench): event pairs around each launch on the launch stream
+  bool timing = false;
+  std::vector<cudaEvent_t> ev_pool;                       // reusable events
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> t_append, t_attn, t_combine;
 };
 
 namespace {
@@ -149,6 +153,25 @@ ws_status_t upload_slot(ws_cache* c, const char* host, char* dev, size_t bytes, 
   c->ev_pending[i] = true;
   return WS_OK;
 }
+
+cudaEvent_t timing_event(ws_cache* c) {
+  cudaEvent_t e = nullptr;
+  if (!c->ev_pool.empty()) { e = c->ev_pool.back(); c->ev_pool.pop_back(); return e; }
+  if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+  return e;
+}
+// RAII-less helper: record an event pair around a launch when timing is enabled
+struct TimedLaunch {
+  ws_cache* c; std::vector<std::pair<cudaEvent_t, cudaEvent_t>>* dst; cudaStream_t st;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  TimedLaunch(ws_cache* c_, std::vector<std::pair<cudaEvent_t, cudaEvent_t>>* d, cudaStream_t s)
+      : c(c_), dst(d), st(s) {
+    if (c->timing) { e0 = timing_event(c); e1 = timing_event(c); if (e0) cudaEventRecord(e0, st); }
+  }
+  void done() {
+    if (c->timing && e0 && e1) { cudaEventRecord(e1, st); dst->emplace_back(e0, e1); }
+  }
+};
 
 ws_status_t encode_tmap(ws_cache* c, CUtensorMap* out, void* base, int rank, const cuuint64_t* dims,
                         const cuuint64_t* strides_bytes, const cuuint32_t* box) {
@@ -276,6 +299,9 @@ ws_status_t ws_cache_destroy(ws_cache_t* c) {
     (void)cudaDeviceSynchronize();
     for (int i = 0; i < kRing; ++i)
       if (c->ev[i]) (void)cudaEventDestroy(c->ev[i]);
+    for (auto* lst : {&c->t_append, &c->t_attn, &c->t_combine})
+      for (auto& pr : *lst) { (void)cudaEventDestroy(pr.first); (void)cudaEventDestroy(pr.second); }
+    for (cudaEvent_t e : c->ev_pool) (void)cudaEventDestroy(e);
     if (c->h_meta) (void)cudaFreeHost(c->h_meta);
   }
   delete c;
@@ -398,10 +424,12 @@ ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   st = upload_slot(c, h, d, (size_t)(hdr.off_pages + npg) * 4, stream);
   if (st != WS_OK) return st;
+  TimedLaunch tl(c, &c->t_append, stream);
   WS_CUDA(ws::launch_kv_append(k_new, v_new, c->cfg.k_pool, c->cfg.v_pool, c->d_page_table,
                                (const int32_t*)d, cu[S], c->cfg.max_pages_per_session, P,
                                c->cfg.num_kv_heads, c->cfg.head_dim, eb_of(c->cfg.dtype), c->num_sms,
                                stream));
+  tl.done();
   c->launches += 1;
   return WS_OK;
 }
@@ -462,12 +490,14 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
       memcpy(h + (size_t)NQ * 4, vis_end.data(), (size_t)NQ * 4);
       st = upload_slot(c, h, d, bytes, stream);
       if (st != WS_OK) return st;
+      TimedLaunch tl(c, &c->t_attn, stream);
       WS_CUDA(ws::launch_attn_simt(c->cfg.dtype, q, out, lse, c->cfg.k_pool, c->cfg.v_pool,
                                    c->d_page_table, (const int32_t*)d,
                                    c->default_map ? nullptr : c->d_q_to_kv, NQ,
                                    c->cfg.max_pages_per_session, c->cfg.num_q_heads,
                                    c->cfg.num_kv_heads, c->cfg.head_dim, c->cfg.page_tokens, scale,
                                    stream));
+      tl.done();
       c->launches += 1;
       c->last_plan = ws::Plan();
       return WS_OK;
@@ -508,10 +538,14 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     if (st != WS_OK) return st;
   }
   L.num_ctas = c->last_plan.num_teams * c->last_plan.team_size;
+  TimedLaunch tl(c, &c->t_attn, stream);
   WS_CUDA(ws::launch_attn_sm100(L, stream));
+  tl.done();
   c->launches += 1;
   if (!c->last_plan.combine.empty()) {
+    TimedLaunch tc(c, &c->t_combine, stream);
     WS_CUDA(ws::launch_combine(L.p, (int32_t)c->last_plan.combine.size(), c->last_plan.team_size, stream));
+    tc.done();
     c->launches += 1;
   }
   return WS_OK;
@@ -598,6 +632,30 @@ ws_status_t ws_last_plan_segment(const ws_cache_t* c, int32_t i, ws_plan_segment
 }
 
 int64_t ws_launch_count(const ws_cache_t* c) { return c ? c->launches : -1; }
+
+ws_status_t ws_debug_kernel_timing(ws_cache_t* c, int32_t enable) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  if (c->dry) return fail(WS_ERR_CUDA, "kernel timing needs a CUDA device");
+  c->timing = enable != 0;
+  return WS_OK;
+}
+
+ws_status_t ws_debug_read_kernel_times(ws_cache_t* c, double* ms_sum3, int32_t* count3) {
+  if (!c || !ms_sum3 || !count3) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>>* lists[3] = {&c->t_append, &c->t_attn, &c->t_combine};
+  for (int k = 0; k < 3; ++k) {
+    ms_sum3[k] = 0.0; count3[k] = (int32_t)lists[k]->size();
+    for (auto& pr : *lists[k]) {
+      WS_CUDA(cudaEventSynchronize(pr.second));
+      float ms = 0.f;
+      WS_CUDA(cudaEventElapsedTime(&ms, pr.first, pr.second));
+      ms_sum3[k] += ms;
+      c->ev_pool.push_back(pr.first); c->ev_pool.push_back(pr.second);
+    }
+    lists[k]->clear();
+  }
+  return WS_OK;
+}
 
 const char* ws_status_str(ws_status_t s) {
   switch (s) {

@@ -27,6 +27,7 @@ def _built():
 
 
 def _assert_close(err, tol, label=""):
+    print(f"[parity] {label}: " + " ".join(f"{k}={v:.3e}" if isinstance(v, float) else f"{k}={v}" for k, v in err.items()))
     assert err["finite"], (label, err)
     for k, v in tol.items():
         assert err[k] <= v, (label, k, err)
@@ -195,7 +196,10 @@ def test_ragged_multi_session_small_and_batched_equals_single():
     w = _small(5, cache_len_range=(100, 1500), block_tokens=64, modality_split=(48, 12, 4))
     got = run_workload_gpu(w)
     ref = run_workload_oracle(w)
-    _assert_close(compare(got, ref, "bf16"), BF16_TOL, "ragged small")
+    # short caches + x8 outlier channels concentrate the softmax, so |O| reaches ~4 and one bf16
+    # output ulp (2^-8 |O|) alone exceeds 1e-2: gate the error in excess of that ulp instead.
+    tol = dict(BF16_TOL); tol.pop("max_abs"); tol["max_excess"] = 5e-3
+    _assert_close(compare(got, ref, "bf16"), tol, "ragged small")
     # each session alone (same inputs) gives the same output within fp tolerance of the oracle
     import dataclasses
     for s in (0, 5):
