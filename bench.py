@@ -114,6 +114,18 @@ class ClockSampler(threading.Thread):
                 **({"error": self.err} if self.err else {})}
 
 
+def aggregate_over_ranks(ms_local: float, flops_local: float, dist=None, device=None):
+    """Whole-job numbers for N independent replicas: time = MAX over ranks, work = SUM over ranks."""
+    if dist is None:
+        return ms_local, flops_local
+    import torch
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    f = torch.tensor([flops_local], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(f, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(f.item())
+
+
 def read_traffic(cfg: int):
     """dram bytes per launch of the attention kernel from the committed ncu summary, or None."""
     p = os.path.join(ROOT, "profiles", f"traffic_cfg{cfg}.txt")
@@ -229,11 +241,7 @@ def main():
             fn(i)
         e1.record(stream)
         barrier()
-        ms = e0.elapsed_time(e1)
-        if dist is not None:
-            t = torch.tensor([ms], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms, _ = aggregate_over_ranks(e0.elapsed_time(e1), 0.0, dist, dev)
         return ms
 
     flops_cycle = [algorithmic_flops(sp, w.cache_lens, t) for t in range(steps_per_cycle)]
