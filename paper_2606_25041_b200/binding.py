@@ -14,7 +14,7 @@ from typing import Optional, Sequence
 import numpy as np
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_PKG, "libwanstream.so")
+LIB_PATH = os.environ.get("WS_LIB_PATH") or os.path.join(_PKG, "libwanstream.so")
 
 WS_BF16, WS_F32 = 0, 1
 WS_FLAG_DRY_RUN, WS_FLAG_FORCE_SIMT = 1, 2

@@ -34,6 +34,7 @@
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <math.h>
+#include <stdio.h>
 
 #include "launch.h"
 #include "sm100_ptx.cuh"
@@ -49,6 +50,20 @@ constexpr uint32_t kQTileBytes = kTileRows * 128 * 2;
 constexpr int kThreads = 384;
 constexpr uint32_t kTmemCols = 512;
 constexpr float kRescaleThreshold = 8.0f;                  // log2 units
+#ifndef WS_FAST_PATH
+#define WS_FAST_PATH 1
+#endif
+#ifndef WS_POLY_PER8
+#define WS_POLY_PER8 2
+#endif
+
+#ifdef WS_PROFILE
+#define PROF_DECL(n) long long prof_acc[n] = {0}; long long prof_t = clock64();
+#define PROF_MARK(i) { long long t_ = clock64(); prof_acc[i] += t_ - prof_t; prof_t = t_; }
+#else
+#define PROF_DECL(n)
+#define PROF_MARK(i)
+#endif
 
 struct Barriers {
   uint64_t q_full, q_empty;
@@ -70,6 +85,64 @@ __device__ __forceinline__ bool load_segment(const int32_t* meta, const AttnMeta
   v.g = reinterpret_cast<const Group*>(meta + hdr.off_groups)[s.group];
   v.tile_begin = s.tile_begin; v.tile_end = s.tile_end; v.part_base = s.part_base;
   return pair < v.g.npairs;
+}
+
+
+// 2^x for a PAIR of values on the FMA/ALU pipes (no MUFU): round-to-nearest split x = r + f with
+// f in [-0.5, 0.5], a degree-3 minimax polynomial for 2^f (max relative error 7.5e-5, well inside
+// one bf16 ulp of P) in packed f32x2 arithmetic, and an exponent-field add per element.  Used for
+// kPolyPairs of every 4 pairs to take load off the 16/clk/SM MUFU.
+__device__ __forceinline__ void ex2_poly2(uint64_t x2, float& p0, float& p1) {
+  float x0, x1;
+  unpack_f32x2(x2, x0, x1);
+  const uint64_t xc = pack_f32x2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
+  const uint64_t magic = pack_f32x2(12582912.f, 12582912.f);   // 1.5 * 2^23: integer part -> LSBs
+  const uint64_t t = add_f32x2(xc, magic);
+  const uint64_t f = sub_f32x2(xc, sub_f32x2(t, magic));
+  uint64_t p = fma_f32x2(f, pack_f32x2(0.055171459913253784f, 0.055171459913253784f),
+                         pack_f32x2(0.2426108568906784f, 0.2426108568906784f));
+  p = fma_f32x2(p, f, pack_f32x2(0.6932609677314758f, 0.6932609677314758f));
+  p = fma_f32x2(p, f, pack_f32x2(0.9999281167984009f, 0.9999281167984009f));
+  float t0, t1, q0, q1;
+  unpack_f32x2(t, t0, t1);
+  unpack_f32x2(p, q0, q1);
+  p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23));
+  p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
+}
+
+constexpr int kPolyPairs = WS_POLY_PER8 / 2;   // pairs out of every 4 that use the polynomial
+
+// One 32-column chunk of a softmax row: p = 2^(s*c - m), running sums, running max of s, bf16 pack.
+__device__ __forceinline__ void softmax_chunk(const uint32_t* sr, float c, float neg_mc,
+                                              uint64_t& l01, uint64_t& l23, float& mx0, float& mx1,
+                                              uint32_t* pk) {
+  const uint64_t c2 = pack_f32x2(c, c), nm2 = pack_f32x2(neg_mc, neg_mc);
+#pragma unroll
+  for (int i = 0; i < 32; i += 8) {
+    float pv[8];
+#pragma unroll
+    for (int e = 0; e < 8; e += 2) {
+      const float s0 = __uint_as_float(sr[i + e]), s1 = __uint_as_float(sr[i + e + 1]);
+      const uint64_t x2 = fma_f32x2(pack_f32x2(s0, s1), c2, nm2);
+      const int pr = e / 2;
+      const bool poly = kPolyPairs > 0 && (pr * kPolyPairs) / 4 != ((pr + 1) * kPolyPairs) / 4;
+      if (poly) {
+        ex2_poly2(x2, pv[e], pv[e + 1]);
+      } else {
+        float x0, x1;
+        unpack_f32x2(x2, x0, x1);
+        pv[e] = ex2_approx(x0); pv[e + 1] = ex2_approx(x1);
+      }
+    }
+    mx0 = fmaxf(mx0, fmaxf(__uint_as_float(sr[i]), __uint_as_float(sr[i + 1])));
+    mx1 = fmaxf(mx1, fmaxf(__uint_as_float(sr[i + 2]), __uint_as_float(sr[i + 3])));
+    mx0 = fmaxf(mx0, fmaxf(__uint_as_float(sr[i + 4]), __uint_as_float(sr[i + 5])));
+    mx1 = fmaxf(mx1, fmaxf(__uint_as_float(sr[i + 6]), __uint_as_float(sr[i + 7])));
+    l01 = add_f32x2(l01, add_f32x2(pack_f32x2(pv[0], pv[1]), pack_f32x2(pv[4], pv[5])));
+    l23 = add_f32x2(l23, add_f32x2(pack_f32x2(pv[2], pv[3]), pack_f32x2(pv[6], pv[7])));
+#pragma unroll
+    for (int e = 0; e < 8; e += 2) pk[(i + e) / 2] = pack_bf16x2(pv[e], pv[e + 1]);
+  }
 }
 
 __global__ void __launch_bounds__(kThreads, 1)
@@ -164,27 +237,32 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           }
         }
       }
-    } else if (warp == 9 && lane == 0) {
+    } else if (warp == 9) {
       // ===================================================== MMA issuer
+      // The whole warp runs the control flow convergently (all values stay warp-uniform, so the
+      // descriptors are built on the uniform datapath); one elected lane issues tcgen05.mma/commit.
+      const bool leader = elect_one();
       constexpr uint32_t idesc_qk = make_idesc_bf16(128, 128, 0, 0);
       constexpr uint32_t idesc_pv = make_idesc_bf16(128, 128, 0, 1);
+      const uint64_t desc_k = make_smem_desc_sw128(0, 16, 1024);          // K-major operands (Q, K)
+      const uint64_t desc_v = make_smem_desc_sw128(0, kHalfBytes, 1024);  // MN-major operand (V)
       uint32_t ring_it = 0, q_it = 0, tile_it = 0, seg_it = 0;
+      PROF_DECL(8)
       auto issue_S = [&](int q, uint32_t slot) {
-        const uint32_t a0 = sQ + q * kQTileBytes, b0 = sRing + slot * kSlotBytes;
+        const uint64_t da = desc_k + ((sQ + q * kQTileBytes) >> 4);
+        const uint64_t db = desc_k + ((sRing + slot * kSlotBytes) >> 4);
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {
-          const uint32_t off = (ks >> 2) * kHalfBytes + (ks & 3) * 32;
-          mma_ss(tmem_base + q * 128, make_smem_desc_sw128(a0 + off, 16, 1024),
-                 make_smem_desc_sw128(b0 + off, 16, 1024), idesc_qk, ks > 0);
+          const uint32_t off = ((ks >> 2) * kHalfBytes + (ks & 3) * 32) >> 4;
+          mma_ss(tmem_base + q * 128, da + off, db + off, idesc_qk, ks > 0);
         }
       };
       auto issue_PV = [&](int q, uint32_t slot, bool accumulate) {
-        const uint32_t b0 = sRing + slot * kSlotBytes;
+        const uint64_t db = desc_v + ((sRing + slot * kSlotBytes) >> 4);
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks)
-          mma_ts(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8,
-                 make_smem_desc_sw128(b0 + ks * 2048, kHalfBytes, 1024), idesc_pv,
-                 (accumulate || ks > 0) ? 1u : 0u);
+          mma_ts(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8, db + ks * (2048 >> 4),
+                 idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
       };
       for (int32_t si = seg_lo; si < seg_hi; ++si) {
         SegView sv;
@@ -195,10 +273,13 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
           mbar_wait(bkv_full(slot), par);
           tc_fence_after();
-          issue_S(0, slot); mma_commit(bs_full(0));
-          issue_S(1, slot); mma_commit(bs_full(1));
-          mma_commit(bkv_empty(slot));
-          if (nt == 1) mma_commit(bq_empty);
+          if (leader) {
+            issue_S(0, slot); mma_commit(bs_full(0));
+            issue_S(1, slot); mma_commit(bs_full(1));
+            mma_commit(bkv_empty(slot));
+            if (nt == 1) mma_commit(bq_empty);
+          }
+          __syncwarp();
           ++ring_it;
         }
         for (int32_t j = 0; j < nt; ++j) {
@@ -207,28 +288,47 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           const bool have_next = j + 1 < nt;
           uint32_t slot_k = 0, par_k = 0;
           if (have_next) { slot_k = ring_it % kStages; par_k = (ring_it / kStages) & 1; ++ring_it; }
+          PROF_MARK(0)
           mbar_wait(bkv_full(slot_v), par_v);
+          PROF_MARK(1)
+#pragma unroll
           for (int q = 0; q < 2; ++q) {
             mbar_wait(bp_full(q), tile_it & 1);
+            PROF_MARK(2 + q)
             if (j == 0) mbar_wait(bo_empty(q), (seg_it & 1) ^ 1);
             tc_fence_after();
-            issue_PV(q, slot_v, j > 0);
-            if (!have_next) mma_commit(bo_full(q));
+            if (leader) {
+              issue_PV(q, slot_v, j > 0);
+              if (!have_next) mma_commit(bo_full(q));
+            }
+            __syncwarp();
+            PROF_MARK(5)
             if (have_next) {
               if (q == 0) { mbar_wait(bkv_full(slot_k), par_k); tc_fence_after(); }
-              issue_S(q, slot_k);
-              mma_commit(bs_full(q));
+              PROF_MARK(4)
+              if (leader) {
+                issue_S(q, slot_k);
+                mma_commit(bs_full(q));
+              }
+              __syncwarp();
+              PROF_MARK(6)
             }
           }
-          mma_commit(bkv_empty(slot_v));
-          if (have_next) {
-            mma_commit(bkv_empty(slot_k));
-            if (j + 2 == nt) mma_commit(bq_empty);
+          if (leader) {
+            mma_commit(bkv_empty(slot_v));
+            if (have_next) {
+              mma_commit(bkv_empty(slot_k));
+              if (j + 2 == nt) mma_commit(bq_empty);
+            }
           }
+          __syncwarp();
           ++tile_it;
         }
         ++q_it; ++seg_it;
       }
+#ifdef WS_PROFILE
+      if (blockIdx.x == 5 && lane == 0) printf("MMA  misc %lld waitV %lld waitP0 %lld waitP1 %lld waitK %lld issuePV %lld issueS %lld tiles %u\n", prof_acc[0], prof_acc[1], prof_acc[2], prof_acc[3], prof_acc[4], prof_acc[5], prof_acc[6], tile_it);
+#endif
     }
   } else {
     // ======================================================= softmax warpgroups (warps 0-7)
@@ -241,6 +341,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t t_o = tmem_base + (lane_base << 16) + 256 + q * 128;
     const float c = p.scale * 1.4426950408889634f;
     uint32_t ring_it = 0, tile_it = 0, seg_it = 0;
+    PROF_DECL(8)
 
     for (int32_t si = seg_lo; si < seg_hi; ++si) {
       SegView sv;
@@ -257,60 +358,99 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         const int32_t key0 = (sv.tile_begin + j) * kTileKeys;
         // V(j) ring position: K(j) is 2j, V(j) is 2j+1 within the segment
         const uint32_t v_it = ring_it + 2 * j + 1;
+        PROF_MARK(0)
         mbar_wait(bs_full(q), tile_it & 1);
         tc_fence_after();
-        uint32_t sr[128];                                   // one whole S row (fp32 bits)
-        tmem_ld32(t_s + 0, sr + 0);
-        tmem_ld32(t_s + 32, sr + 32);
-        tmem_ld32(t_s + 64, sr + 64);
-        tmem_ld32(t_s + 96, sr + 96);
-        tmem_wait_ld();
-#define S_(i) __uint_as_float(sr[i])
+        PROF_MARK(1)
+        uint32_t pk[64];                                    // P row, packed bf16x2
         const bool need_mask = __any_sync(0xffffffffu, key0 + kTileKeys > vis);
-        if (need_mask) {
-#pragma unroll
-          for (int i = 0; i < 128; ++i)
-            if (key0 + i >= vis) sr[i] = 0xff800000u;       // -inf
-        }
-        float mx0 = S_(0), mx1 = S_(1), mx2 = S_(2), mx3 = S_(3);
-#pragma unroll
-        for (int i = 4; i < 128; i += 4) {
-          mx0 = fmaxf(mx0, S_(i)); mx1 = fmaxf(mx1, S_(i + 1));
-          mx2 = fmaxf(mx2, S_(i + 2)); mx3 = fmaxf(mx3, S_(i + 3));
-        }
-        const float tm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;
-        const bool grow = tm > m_used + kRescaleThreshold;
-        if (j == 0) {
-          m_used = tm;
-        } else if (__any_sync(0xffffffffu, grow)) {
-          // lazy rescale of O and l (PV of the previous tile has completed: s_full was committed
-          // after it on the same in-order tensor pipe)
-          float alpha = 1.f;
-          if (grow) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
-#pragma unroll
-          for (int ch = 0; ch < 4; ++ch) {
-            uint32_t o[32];
-            tmem_ld32(t_o + ch * 32, o);
-            tmem_wait_ld();
-#pragma unroll
-            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-            tmem_st32(t_o + ch * 32, o);
+        bool done = false;
+        if (WS_FAST_PATH && j > 0 && !need_mask) {
+          // ---- fast path (optimistic): exponentiate against the running reference m_used while
+          // the tile is still streaming out of TMEM in 32-column chunks; the tile max is tracked
+          // on the side and checked afterwards.  If any row's max outgrew m_used by more than the
+          // rescale threshold the results are discarded and the exact path below redoes the tile.
+          const float neg_mc = (m_used == -INFINITY) ? 0.f : -m_used;
+          uint64_t l01 = 0, l23 = 0;                        // packed fp32x2 partial row sums
+          float mx0 = -INFINITY, mx1 = -INFINITY;
+          uint32_t sa[32], sb[32];
+          tmem_ld32(t_s + 0, sa);
+          tmem_wait_ld();
+          tmem_ld32(t_s + 32, sb);
+          softmax_chunk(sa, c, neg_mc, l01, l23, mx0, mx1, pk + 0);
+          tmem_wait_ld();
+          tmem_ld32(t_s + 64, sa);
+          softmax_chunk(sb, c, neg_mc, l01, l23, mx0, mx1, pk + 16);
+          tmem_wait_ld();
+          tmem_ld32(t_s + 96, sb);
+          softmax_chunk(sa, c, neg_mc, l01, l23, mx0, mx1, pk + 32);
+          tmem_wait_ld();
+          softmax_chunk(sb, c, neg_mc, l01, l23, mx0, mx1, pk + 48);
+          const float tm = fmaxf(mx0, mx1) * c;
+          if (!__any_sync(0xffffffffu, tm > m_used + kRescaleThreshold)) {
+            float la, lb;
+            unpack_f32x2(add_f32x2(l01, l23), la, lb);
+            l += la + lb;
+            done = true;
           }
         }
-        const float m_c = (m_used == -INFINITY) ? 0.f : m_used;
-        float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
-        uint32_t pk[64];
+        if (!done) {
+          // ---- exact path: first tile of a segment, masked tiles, or a row max that grew
+          uint32_t sr[128];                                 // one whole S row (fp32 bits)
+          tmem_ld32(t_s + 0, sr + 0);
+          tmem_ld32(t_s + 32, sr + 32);
+          tmem_ld32(t_s + 64, sr + 64);
+          tmem_ld32(t_s + 96, sr + 96);
+          tmem_wait_ld();
+          PROF_MARK(2)
+#define S_(i) __uint_as_float(sr[i])
+          if (need_mask) {
 #pragma unroll
-        for (int i = 0; i < 128; i += 4) {
-          const float p0 = ex2_approx(fmaf(S_(i), c, -m_c));
-          const float p1 = ex2_approx(fmaf(S_(i + 1), c, -m_c));
-          const float p2 = ex2_approx(fmaf(S_(i + 2), c, -m_c));
-          const float p3 = ex2_approx(fmaf(S_(i + 3), c, -m_c));
-          l0 += p0; l1 += p1; l2 += p2; l3 += p3;
-          pk[i / 2] = pack_bf16x2(p0, p1);
-          pk[i / 2 + 1] = pack_bf16x2(p2, p3);
+            for (int i = 0; i < 128; ++i)
+              if (key0 + i >= vis) sr[i] = 0xff800000u;     // -inf
+          }
+          float mx0 = S_(0), mx1 = S_(1), mx2 = S_(2), mx3 = S_(3);
+#pragma unroll
+          for (int i = 4; i < 128; i += 4) {
+            mx0 = fmaxf(mx0, S_(i)); mx1 = fmaxf(mx1, S_(i + 1));
+            mx2 = fmaxf(mx2, S_(i + 2)); mx3 = fmaxf(mx3, S_(i + 3));
+          }
+          const float tm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;
+          const bool grow = tm > m_used + kRescaleThreshold;
+          if (j == 0) {
+            m_used = tm;
+          } else if (__any_sync(0xffffffffu, grow)) {
+            // lazy rescale of O and l (PV of the previous tile has completed: s_full was committed
+            // after it on the same in-order tensor pipe)
+            float alpha = 1.f;
+            if (grow) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
+#pragma unroll
+            for (int ch = 0; ch < 4; ++ch) {
+              uint32_t o[32];
+              tmem_ld32(t_o + ch * 32, o);
+              tmem_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+              tmem_st32(t_o + ch * 32, o);
+            }
+          }
+          const float m_c = (m_used == -INFINITY) ? 0.f : m_used;
+          float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+          PROF_MARK(3)
+#pragma unroll
+          for (int i = 0; i < 128; i += 4) {
+            const float p0 = ex2_approx(fmaf(S_(i), c, -m_c));
+            const float p1 = ex2_approx(fmaf(S_(i + 1), c, -m_c));
+            const float p2 = ex2_approx(fmaf(S_(i + 2), c, -m_c));
+            const float p3 = ex2_approx(fmaf(S_(i + 3), c, -m_c));
+            l0 += p0; l1 += p1; l2 += p2; l3 += p3;
+            pk[i / 2] = pack_bf16x2(p0, p1);
+            pk[i / 2 + 1] = pack_bf16x2(p2, p3);
+          }
+          l += (l0 + l1) + (l2 + l3);
+          PROF_MARK(4)
+#undef S_
         }
-        l += (l0 + l1) + (l2 + l3);
         tmem_st32(t_s + 0, pk);
         tmem_st32(t_s + 32, pk + 32);
         // last tile of the cache with a ragged end: zero the V rows beyond kv_len in smem so that
@@ -333,6 +473,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(bp_full(q));
+        PROF_MARK(5)
         ++tile_it;
       }
       ring_it += 2 * nt;
@@ -383,8 +524,12 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       }
       tc_fence_before();
       mbar_arrive(bo_empty(q));
+      PROF_MARK(6)
       ++seg_it;
     }
+#ifdef WS_PROFILE
+    if (blockIdx.x == 5 && lane == 0 && (warp & 3) == 0) printf("SMX%d other %lld waitS %lld ld %lld max %lld exp %lld store %lld epi %lld tiles %u\n", q, prof_acc[0], prof_acc[1], prof_acc[2], prof_acc[3], prof_acc[4], prof_acc[5], prof_acc[6], tile_it);
+#endif
   }
 
   __syncwarp();
