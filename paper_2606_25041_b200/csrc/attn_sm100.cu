@@ -50,6 +50,7 @@ constexpr uint32_t kQTileBytes = kTileRows * 128 * 2;
 constexpr int kThreads = 384;
 constexpr uint32_t kTmemCols = 512;
 constexpr float kRescaleThreshold = 8.0f;                  // log2 units
+constexpr float kFastSumLimit = 1024.0f;                   // fast path accepted while tile row sum < 2^10
 #ifndef WS_FAST_PATH
 #define WS_FAST_PATH 1
 #endif
@@ -68,7 +69,7 @@ constexpr float kRescaleThreshold = 8.0f;                  // log2 units
 struct Barriers {
   uint64_t q_full, q_empty;
   uint64_t kv_full[kStages], kv_empty[kStages];
-  uint64_t s_full[2], p_full[2], o_full[2], o_empty[2];
+  uint64_t s_full[2], p_full[2][2], pv_h0_done[2], o_full[2], o_empty[2];
   uint32_t tmem_base;
   uint32_t pad;
 };
@@ -114,8 +115,7 @@ constexpr int kPolyPairs = WS_POLY_PER8 / 2;   // pairs out of every 4 that use 
 
 // One 32-column chunk of a softmax row: p = 2^(s*c - m), running sums, running max of s, bf16 pack.
 __device__ __forceinline__ void softmax_chunk(const uint32_t* sr, float c, float neg_mc,
-                                              uint64_t& l01, uint64_t& l23, float& mx0, float& mx1,
-                                              uint32_t* pk) {
+                                              uint64_t& l01, uint64_t& l23, uint32_t* pk) {
   const uint64_t c2 = pack_f32x2(c, c), nm2 = pack_f32x2(neg_mc, neg_mc);
 #pragma unroll
   for (int i = 0; i < 32; i += 8) {
@@ -134,10 +134,6 @@ __device__ __forceinline__ void softmax_chunk(const uint32_t* sr, float c, float
         pv[e] = ex2_approx(x0); pv[e + 1] = ex2_approx(x1);
       }
     }
-    mx0 = fmaxf(mx0, fmaxf(__uint_as_float(sr[i]), __uint_as_float(sr[i + 1])));
-    mx1 = fmaxf(mx1, fmaxf(__uint_as_float(sr[i + 2]), __uint_as_float(sr[i + 3])));
-    mx0 = fmaxf(mx0, fmaxf(__uint_as_float(sr[i + 4]), __uint_as_float(sr[i + 5])));
-    mx1 = fmaxf(mx1, fmaxf(__uint_as_float(sr[i + 6]), __uint_as_float(sr[i + 7])));
     l01 = add_f32x2(l01, add_f32x2(pack_f32x2(pv[0], pv[1]), pack_f32x2(pv[4], pv[5])));
     l23 = add_f32x2(l23, add_f32x2(pack_f32x2(pv[2], pv[3]), pack_f32x2(pv[6], pv[7])));
 #pragma unroll
@@ -159,7 +155,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   auto bkv_full = [&](int s) { return smem_u32(&bars->kv_full[s]); };
   auto bkv_empty = [&](int s) { return smem_u32(&bars->kv_empty[s]); };
   auto bs_full = [&](int q) { return smem_u32(&bars->s_full[q]); };
-  auto bp_full = [&](int q) { return smem_u32(&bars->p_full[q]); };
+  auto bp_full = [&](int q, int half) { return smem_u32(&bars->p_full[q][half]); };
+  auto bpv_h0 = [&](int q) { return smem_u32(&bars->pv_h0_done[q]); };
   auto bo_full = [&](int q) { return smem_u32(&bars->o_full[q]); };
   auto bo_empty = [&](int q) { return smem_u32(&bars->o_empty[q]); };
 
@@ -172,6 +169,10 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   const int32_t seg_lo = tsb[team], seg_hi = tsb[team + 1];
   const int32_t tok_per_pair = kPairRows / p.G;
   const int32_t tok_per_tile = kTileRows / p.G;
+#ifdef WS_PROFILE
+  const long long prof_cta_t0 = clock64();
+  unsigned long long prof_g0; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(prof_g0));
+#endif
 
   if (warp == 8 && lane == 0) {
     prefetch_tmap(&tmap_q); prefetch_tmap(&tmap_k); prefetch_tmap(&tmap_v);
@@ -180,7 +181,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     mbar_init(bq_full, 1); mbar_init(bq_empty, 1);
     for (int s = 0; s < kStages; ++s) { mbar_init(bkv_full(s), 1); mbar_init(bkv_empty(s), 1); }
     for (int q = 0; q < 2; ++q) {
-      mbar_init(bs_full(q), 1); mbar_init(bp_full(q), 128);
+      mbar_init(bs_full(q), 1); mbar_init(bp_full(q, 0), 128); mbar_init(bp_full(q, 1), 128);
+      mbar_init(bpv_h0(q), 1);
       mbar_init(bo_full(q), 1); mbar_init(bo_empty(q), 128);
     }
     fence_mbar_init();
@@ -257,12 +259,15 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           mma_ss(tmem_base + q * 128, da + off, db + off, idesc_qk, ks > 0);
         }
       };
-      auto issue_PV = [&](int q, uint32_t slot, bool accumulate) {
+      // PV for one half of the tile's keys (k-steps 4*half .. 4*half+3)
+      auto issue_PV = [&](int q, uint32_t slot, int half, bool accumulate) {
         const uint64_t db = desc_v + ((sRing + slot * kSlotBytes) >> 4);
 #pragma unroll
-        for (int ks = 0; ks < 8; ++ks)
+        for (int k4 = 0; k4 < 4; ++k4) {
+          const int ks = half * 4 + k4;
           mma_ts(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8, db + ks * (2048 >> 4),
                  idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
+        }
       };
       for (int32_t si = seg_lo; si < seg_hi; ++si) {
         SegView sv;
@@ -293,12 +298,19 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           PROF_MARK(1)
 #pragma unroll
           for (int q = 0; q < 2; ++q) {
-            mbar_wait(bp_full(q), tile_it & 1);
+            mbar_wait(bp_full(q, 0), tile_it & 1);
             PROF_MARK(2 + q)
             if (j == 0) mbar_wait(bo_empty(q), (seg_it & 1) ^ 1);
             tc_fence_after();
             if (leader) {
-              issue_PV(q, slot_v, j > 0);
+              issue_PV(q, slot_v, 0, j > 0);
+              mma_commit(bpv_h0(q));
+            }
+            __syncwarp();
+            mbar_wait(bp_full(q, 1), tile_it & 1);
+            tc_fence_after();
+            if (leader) {
+              issue_PV(q, slot_v, 1, true);
               if (!have_next) mma_commit(bo_full(q));
             }
             __syncwarp();
@@ -365,37 +377,88 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         uint32_t pk[64];                                    // P row, packed bf16x2
         const bool need_mask = __any_sync(0xffffffffu, key0 + kTileKeys > vis);
         bool done = false;
-        if (WS_FAST_PATH && j > 0 && !need_mask) {
+        // (rows whose reference is still -inf, i.e. nothing visible so far, also take the exact path)
+        if (WS_FAST_PATH && j > 0 && !need_mask && !__any_sync(0xffffffffu, m_used == -INFINITY)) {
           // ---- fast path (optimistic): exponentiate against the running reference m_used while
-          // the tile is still streaming out of TMEM in 32-column chunks; the tile max is tracked
-          // on the side and checked afterwards.  If any row's max outgrew m_used by more than the
-          // rescale threshold the results are discarded and the exact path below redoes the tile.
-          const float neg_mc = (m_used == -INFINITY) ? 0.f : -m_used;
+          // the tile streams out of TMEM in 32-column chunks.  Each half (64 keys) is checked for
+          // scores that outgrew the reference - every p is <= the half's row sum, so a sum below
+          // kFastSumLimit proves none did (a NaN/inf sum fails the test) - and handed to the MMA
+          // warp as soon as it is written, so PV of the first half overlaps the second half.
+          const float neg_mc = -m_used;
           uint64_t l01 = 0, l23 = 0;                        // packed fp32x2 partial row sums
-          float mx0 = -INFINITY, mx1 = -INFINITY;
           uint32_t sa[32], sb[32];
           tmem_ld32(t_s + 0, sa);
           tmem_wait_ld();
           tmem_ld32(t_s + 32, sb);
-          softmax_chunk(sa, c, neg_mc, l01, l23, mx0, mx1, pk + 0);
+          softmax_chunk(sa, c, neg_mc, l01, l23, pk + 0);
           tmem_wait_ld();
           tmem_ld32(t_s + 64, sa);
-          softmax_chunk(sb, c, neg_mc, l01, l23, mx0, mx1, pk + 16);
-          tmem_wait_ld();
-          tmem_ld32(t_s + 96, sb);
-          softmax_chunk(sa, c, neg_mc, l01, l23, mx0, mx1, pk + 32);
-          tmem_wait_ld();
-          softmax_chunk(sb, c, neg_mc, l01, l23, mx0, mx1, pk + 48);
-          const float tm = fmaxf(mx0, mx1) * c;
-          if (!__any_sync(0xffffffffu, tm > m_used + kRescaleThreshold)) {
-            float la, lb;
+          softmax_chunk(sb, c, neg_mc, l01, l23, pk + 16);
+          float la, lb;
+          unpack_f32x2(add_f32x2(l01, l23), la, lb);
+          const float sum_a = la + lb;
+          if (!__any_sync(0xffffffffu, !(sum_a < kFastSumLimit))) {
+            tmem_st32(t_s + 0, pk);
+            tmem_wait_st();
+            tc_fence_before();
+            mbar_arrive(bp_full(q, 0));                     // first 64 keys of P handed off
+            tmem_wait_ld();
+            tmem_ld32(t_s + 96, sb);
+            l01 = 0; l23 = 0;
+            softmax_chunk(sa, c, neg_mc, l01, l23, pk + 32);
+            tmem_wait_ld();
+            softmax_chunk(sb, c, neg_mc, l01, l23, pk + 48);
             unpack_f32x2(add_f32x2(l01, l23), la, lb);
-            l += la + lb;
+            const float sum_b = la + lb;
+            l += sum_a;
+            if (!__any_sync(0xffffffffu, !(sum_b < kFastSumLimit))) {
+              l += sum_b;
+            } else {
+              // Rare: a score in the second half outgrew the reference after the first half was
+              // handed off.  Wait until PV of the first half has completed (O is then quiescent:
+              // the second-half PV needs our arrival), rescale O and l to the new reference and
+              // redo the second half exactly.
+              mbar_wait(bpv_h0(q), tile_it & 1);
+              tc_fence_after();
+              uint32_t sr[64];
+              tmem_ld32(t_s + 64, sr);
+              tmem_ld32(t_s + 96, sr + 32);
+              tmem_wait_ld();
+              float mx = __uint_as_float(sr[0]);
+#pragma unroll
+              for (int i = 1; i < 64; ++i) mx = fmaxf(mx, __uint_as_float(sr[i]));
+              const float tm = mx * c;
+              float alpha = 1.f;
+              if (tm > m_used + kRescaleThreshold) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
+#pragma unroll
+              for (int ch = 0; ch < 4; ++ch) {
+                uint32_t o[32];
+                tmem_ld32(t_o + ch * 32, o);
+                tmem_wait_ld();
+#pragma unroll
+                for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                tmem_st32(t_o + ch * 32, o);
+              }
+              float ls = 0.f;
+#pragma unroll
+              for (int i = 0; i < 64; i += 2) {
+                const float p0 = ex2_approx(fmaf(__uint_as_float(sr[i]), c, -m_used));
+                const float p1 = ex2_approx(fmaf(__uint_as_float(sr[i + 1]), c, -m_used));
+                ls += p0 + p1;
+                pk[32 + i / 2] = pack_bf16x2(p0, p1);
+              }
+              l += ls;
+            }
+            tmem_st32(t_s + 32, pk + 32);
+            tmem_wait_st();
+            tc_fence_before();
+            mbar_arrive(bp_full(q, 1));
             done = true;
           }
         }
         if (!done) {
-          // ---- exact path: first tile of a segment, masked tiles, or a row max that grew
+          // ---- exact path: first tile of a segment, masked tiles, or a first-half row max that
+          // outgrew the reference (nothing has been handed off yet in that case)
           uint32_t sr[128];                                 // one whole S row (fp32 bits)
           tmem_ld32(t_s + 0, sr + 0);
           tmem_ld32(t_s + 32, sr + 32);
@@ -450,29 +513,30 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           l += (l0 + l1) + (l2 + l3);
           PROF_MARK(4)
 #undef S_
-        }
-        tmem_st32(t_s + 0, pk);
-        tmem_st32(t_s + 32, pk + 32);
-        // last tile of the cache with a ragged end: zero the V rows beyond kv_len in smem so that
-        // 0 * (stale bits, possibly NaN) cannot reach O.  Done by warpgroup 0; the PV MMA of both
-        // Q tiles is issued after p_full[0].
-        if (q == 0 && key0 + kTileKeys > sv.g.kv_len) {
-          const uint32_t slot = v_it % kStages, par = (v_it / kStages) & 1;
-          mbar_wait(bkv_full(slot), par);
-          const int32_t r = (sv.g.kv_len - key0) + row_in_tile;
-          if (r < kTileKeys) {
-            const uint32_t base = sRing + slot * kSlotBytes + r * 128;
+          tmem_st32(t_s + 0, pk);
+          tmem_st32(t_s + 32, pk + 32);
+          // last tile of the cache with a ragged end: zero the V rows beyond kv_len in smem so that
+          // 0 * (stale bits, possibly NaN) cannot reach O.  Done by warpgroup 0; the PV MMAs of both
+          // Q tiles are issued after p_full[0][0].  (Such a tile always takes this exact path.)
+          if (q == 0 && key0 + kTileKeys > sv.g.kv_len) {
+            const uint32_t slot = v_it % kStages, par = (v_it / kStages) & 1;
+            mbar_wait(bkv_full(slot), par);
+            const int32_t r = (sv.g.kv_len - key0) + row_in_tile;
+            if (r < kTileKeys) {
+              const uint32_t base = sRing + slot * kSlotBytes + r * 128;
 #pragma unroll
-            for (int b = 0; b < 128; b += 16) {
-              asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(base + b), "r"(0u) : "memory");
-              asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(base + kHalfBytes + b), "r"(0u) : "memory");
+              for (int b = 0; b < 128; b += 16) {
+                asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(base + b), "r"(0u) : "memory");
+                asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(base + kHalfBytes + b), "r"(0u) : "memory");
+              }
             }
+            fence_proxy_async_smem();
           }
-          fence_proxy_async_smem();
+          tmem_wait_st();
+          tc_fence_before();
+          mbar_arrive(bp_full(q, 0));
+          mbar_arrive(bp_full(q, 1));
         }
-        tmem_wait_st();
-        tc_fence_before();
-        mbar_arrive(bp_full(q));
         PROF_MARK(5)
         ++tile_it;
       }
@@ -535,6 +599,14 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   __syncwarp();
   tc_fence_before();
   __syncthreads();
+#ifdef WS_PROFILE
+  if (threadIdx.x == 0) {
+    unsigned long long g1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(g1));
+    int tiles = 0; for (int si = seg_lo; si < seg_hi; ++si) { const Segment sg = reinterpret_cast<const Segment*>(p.meta + hdr.off_segments)[si]; tiles += sg.tile_end - sg.tile_begin; }
+    unsigned smid; asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
+    printf("CTA %d sm %u segs %d tiles %d cycles %lld t0 %llu t1 %llu\n", blockIdx.x, smid, seg_hi - seg_lo, tiles, clock64() - prof_cta_t0, prof_g0, g1);
+  }
+#endif
   if (warp == 10) {
     tc_fence_after();
     tmem_dealloc<kTmemCols>(tmem_base);

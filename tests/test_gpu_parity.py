@@ -309,6 +309,44 @@ def test_large_scores_do_not_overflow():
     assert err["finite"] and err["max_abs"] <= 2e-2 and err["rel_rms"] <= 1e-2, err
 
 
+@pytest.mark.parametrize("kind", ["ramp", "jump_second_half", "jump_first_half", "late_outlier"])
+def test_growing_scores_exercise_every_rescale_path(kind):
+    """Scores that keep outgrowing the running reference: ramps (every half tile rescales), a jump of
+    +230 (log2 units) inside the second / first half of a tile after that tile's other half was fine
+    (the optimistic fast path must recover, incl. the O rescale after an already handed-off half),
+    and a single huge late key.  Compared with the oracle; nothing may overflow."""
+    from oracle.block_causal import OracleSession, attend
+    L, n, Hq, Hkv = 1280, 128, 4, 2
+    rng = np.random.default_rng(17)
+    u = rng.choice([-1.0, 1.0], size=128).astype(np.float32)
+    N = L + n
+    amp = np.zeros(N, np.float32)
+    if kind == "ramp":
+        amp = np.arange(N, dtype=np.float32) * 0.25          # +16 per 64 keys (x1.44 in log2)
+    elif kind == "jump_second_half":
+        amp[128 * 3 + 100:] = 160.0                           # tile 3, key 100 (second half)
+    elif kind == "jump_first_half":
+        amp[128 * 5 + 20:] = 160.0                            # tile 5, key 20 (first half)
+    else:
+        amp[N - 3] = 90.0
+    scale = 1.0 / math.sqrt(128)
+    # score of key j = amp[j] (exactly: q = u, k_j = amp_j/(128*scale) * u), plus N(0,1)-ish noise keys
+    k_all = (amp[:, None, None] / (128.0 * scale)) * u[None, None, :] * np.ones((1, Hkv, 1), np.float32)
+    k_all = to_bf16(k_all + 0.05 * rng.standard_normal((N, Hkv, 128), dtype=np.float32))
+    v_all = to_bf16(rng.standard_normal((N, Hkv, 128), dtype=np.float32))
+    q = to_bf16(np.tile(u, (n, Hq, 1)) + 0.05 * rng.standard_normal((n, Hq, 128), dtype=np.float32))
+    for splits in (1, 2):
+        o, lse, _ = _run_custom_bf16(L, n, Hq, Hkv, k_all[:L], v_all[:L], q, k_all[L:], v_all[L:], scale,
+                                     min_splits=splits)
+        sess = OracleSession(Hkv, 128)
+        sess.append(k_all[:L], v_all[:L]); sess.append(k_all[L:], v_all[L:])
+        o_ref, l_ref = attend(sess, q, scale)
+        assert np.isfinite(o).all() and np.isfinite(lse).all(), kind
+        d = np.abs(o - o_ref)
+        assert (d - 2.0 ** -8 * np.abs(o_ref)).max() <= 6e-3, (kind, splits, d.max())
+        assert np.abs(lse - l_ref).max() <= 2e-3 * max(1.0, np.abs(l_ref).max() / 50), (kind, splits)
+
+
 # ------------------------------------------------------------------ BASELINE configs at full size
 def _sample(n, Hq, k=24, seed=0):
     rng = np.random.default_rng(seed)
