@@ -401,8 +401,15 @@ ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
   if (words * 4 > c->lay.meta_slot_bytes)
     return fail(WS_ERR_WORKSPACE_TOO_SMALL, "append metadata exceeds the slot");
   char *h = nullptr, *d = nullptr;
-  ws_status_t st = next_slot(c, words * 4, &h, &d);
-  if (st != WS_OK) return st;
+  ws::InlineAppendMeta inl{};
+  const bool inline_meta = words <= (size_t)ws::kInlineAppendWords;
+  ws_status_t st = WS_OK;
+  if (inline_meta) {
+    h = (char*)inl.w;
+  } else {
+    st = next_slot(c, words * 4, &h, &d);
+    if (st != WS_OK) return st;
+  }
 
   // ---- commit (no failure paths below except CUDA errors)
   ws::AppendMeta hdr{S, cu[S], (int32_t)(sizeof(ws::AppendMeta) / 4),
@@ -422,11 +429,13 @@ ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
   memcpy(blob, &hdr, sizeof(hdr));
   if (c->dry) return WS_OK;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
-  st = upload_slot(c, h, d, (size_t)(hdr.off_pages + npg) * 4, stream);
-  if (st != WS_OK) return st;
+  if (!inline_meta) {
+    st = upload_slot(c, h, d, (size_t)(hdr.off_pages + npg) * 4, stream);
+    if (st != WS_OK) return st;
+  }
   TimedLaunch tl(c, &c->t_append, stream);
   WS_CUDA(ws::launch_kv_append(k_new, v_new, c->cfg.k_pool, c->cfg.v_pool, c->d_page_table,
-                               (const int32_t*)d, cu[S], c->cfg.max_pages_per_session, P,
+                               inline_meta ? nullptr : (const int32_t*)d, inl, cu[S], c->cfg.max_pages_per_session, P,
                                c->cfg.num_kv_heads, c->cfg.head_dim, eb_of(c->cfg.dtype), c->num_sms,
                                stream));
   tl.done();
@@ -460,7 +469,7 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     if (cu[s + 1] - cu[s] != nq)
       return fail(WS_ERR_INVALID_ARG, "session %d: cu gives %d query tokens, its last %d block(s) hold %lld",
                   id, cu[s + 1] - cu[s], m, (long long)nq);
-    ps[s] = ws::PlanSession{id, cu[s], cu[s + 1], m > 1};
+    ps[s] = ws::PlanSession{id, cu[s], cu[s + 1], m > 1, (int32_t)ss.stable_tokens};
     any_multi |= m > 1;
     for (int32_t b = B - m; b < B; ++b) {
       int64_t lo = b ? ss.block_ends[b - 1] : 0;
@@ -504,22 +513,32 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     }
   }
 
-  ws::PlanConfig pc{c->cfg.num_kv_heads, G, c->num_sms, /*min_tiles=*/2, c->min_splits,
-                    c->lay.max_part_slots};
+  ws::PlanConfig pc{c->cfg.num_kv_heads, G, c->num_sms, /*min_tiles=*/2, /*seg_overhead_tiles=*/3.3f,
+                    c->min_splits, c->lay.max_part_slots};
   ws::Plan plan = ws::build_plan(pc, ps, vis_end);
   if (!plan.ok)
     return fail(WS_ERR_WORKSPACE_TOO_SMALL, "plan needs %d partial slots, workspace holds %d",
                 plan.num_part_slots, c->lay.max_part_slots);
   std::vector<int32_t> blob = ws::serialise_plan(plan, vis_end, any_multi);
-  ws_status_t st = next_slot(c, blob.size() * 4, &h, &d);
-  if (st != WS_OK) return st;
-  memcpy(h, blob.data(), blob.size() * 4);
+  const bool inline_meta = blob.size() <= (size_t)ws::kInlineAttnWords;
+  ws_status_t st = WS_OK;
+  if (!inline_meta) {
+    st = next_slot(c, blob.size() * 4, &h, &d);
+    if (st != WS_OK) return st;
+    memcpy(h, blob.data(), blob.size() * 4);
+  }
   c->last_plan = std::move(plan);
+  // every append launched before this kernel has completed once this kernel has (PDL chain, see
+  // attn_sm100.cu): the next call may read those tokens before its own griddepcontrol.wait
+  c->host->mark_all_stable();
   if (c->dry) return WS_OK;
-  st = upload_slot(c, h, d, blob.size() * 4, stream);
-  if (st != WS_OK) return st;
+  if (!inline_meta) {
+    st = upload_slot(c, h, d, blob.size() * 4, stream);
+    if (st != WS_OK) return st;
+  }
 
   ws::Sm100Launch L{};
+  if (inline_meta) { memcpy(L.inl.w, blob.data(), blob.size() * 4); d = nullptr; }
   L.p.q = q; L.p.out = out; L.p.lse = lse;
   L.p.k_pool = c->cfg.k_pool; L.p.v_pool = c->cfg.v_pool;
   L.p.page_table = c->d_page_table;
@@ -544,7 +563,7 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
   c->launches += 1;
   if (!c->last_plan.combine.empty()) {
     TimedLaunch tc(c, &c->t_combine, stream);
-    WS_CUDA(ws::launch_combine(L.p, (int32_t)c->last_plan.combine.size(), c->last_plan.team_size, stream));
+    WS_CUDA(ws::launch_combine(L.p, L.inl, (int32_t)c->last_plan.combine.size(), c->last_plan.team_size, stream));
     tc.done();
     c->launches += 1;
   }

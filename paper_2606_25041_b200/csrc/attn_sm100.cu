@@ -144,7 +144,10 @@ __device__ __forceinline__ void softmax_chunk(const uint32_t* sr, float c, float
 __global__ void __launch_bounds__(kThreads, 1)
 attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ CUtensorMap tmap_k,
-                  const __grid_constant__ CUtensorMap tmap_v, const AttnParams p) {
+                  const __grid_constant__ CUtensorMap tmap_v,
+                  const __grid_constant__ InlineAttnMeta inl, const AttnParams p_in) {
+  AttnParams p = p_in;
+  if (p.meta == nullptr) p.meta = inl.w;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem_base;                           // 2 x 32 KB
@@ -201,11 +204,14 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     if (warp == 8 && lane == 0) {
       // ===================================================== TMA producer
       uint32_t ring_it = 0, q_it = 0;
+      bool dep_waited = false;
       for (int32_t si = seg_lo; si < seg_hi; ++si) {
         SegView sv;
         if (!load_segment(p.meta, hdr, si, pair, sv)) continue;
         const int32_t* page_row = p.page_table + (int64_t)sv.g.slot * p.max_pages_per_session;
         const int32_t last_page = (sv.g.kv_len - 1) / p.P;
+        // tiles >= dep_tile may still be being written by the preceding append kernel (PDL)
+        if (!dep_waited && sv.tile_begin + 1 >= sv.g.dep_tile) { pdl_wait(); dep_waited = true; }
         int32_t pg0 = page_row[min(2 * sv.tile_begin, last_page)];
         int32_t pg1 = page_row[min(2 * sv.tile_begin + 1, last_page)];
         // Q pair
@@ -220,6 +226,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
           const int32_t c0 = pg0, c1 = pg1;
           if (j + 1 < sv.tile_end) {                        // prefetch next tile's page ids
+            if (!dep_waited && j + 2 >= sv.g.dep_tile) { pdl_wait(); dep_waited = true; }
             pg0 = page_row[min(2 * j + 2, last_page)];
             pg1 = page_row[min(2 * j + 3, last_page)];
           }
@@ -543,6 +550,9 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       ring_it += 2 * nt;
 
       // ---------------------------------------------------- epilogue
+      // first global write of this CTA: the predecessor grids (append; transitively the previous
+      // step's combine, which reads the partial buffers and writes `out`) must have completed
+      if (seg_it == 0) pdl_wait();
       mbar_wait(bo_full(q), seg_it & 1);
       tc_fence_after();
       const float inv_l = l > 0.f ? 1.f / l : 0.f;
@@ -597,6 +607,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   }
 
   __syncwarp();
+  pdl_launch_dependents();
   tc_fence_before();
   __syncthreads();
 #ifdef WS_PROFILE
@@ -604,7 +615,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     unsigned long long g1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(g1));
     int tiles = 0; for (int si = seg_lo; si < seg_hi; ++si) { const Segment sg = reinterpret_cast<const Segment*>(p.meta + hdr.off_segments)[si]; tiles += sg.tile_end - sg.tile_begin; }
     unsigned smid; asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
-    printf("CTA %d sm %u segs %d tiles %d cycles %lld t0 %llu t1 %llu\n", blockIdx.x, smid, seg_hi - seg_lo, tiles, clock64() - prof_cta_t0, prof_g0, g1);
+    if (blockIdx.x % 37 == 7) printf("CTA %d sm %u segs %d tiles %d cycles %lld t0 %llu t1 %llu\n", blockIdx.x, smid, seg_hi - seg_lo, tiles, clock64() - prof_cta_t0, prof_g0, g1);
   }
 #endif
   if (warp == 10) {
@@ -619,8 +630,8 @@ cudaError_t sm100_attn_configure() {
 }
 
 cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream) {
-  attn_sm100_kernel<<<l.num_ctas, kThreads, kSmemBytes, stream>>>(l.tmap_q, l.tmap_k, l.tmap_v, l.p);
-  return cudaGetLastError();
+  return launch_pdl(attn_sm100_kernel, dim3(l.num_ctas), dim3(kThreads), kSmemBytes, stream, l.tmap_q,
+                    l.tmap_k, l.tmap_v, l.inl, l.p);
 }
 
 }  // namespace ws

@@ -14,7 +14,10 @@ namespace ws {
 constexpr int kCombineRowsPerBlock = 8;   // one warp per packed row, D = 128 -> one float4 per lane
 
 __global__ void __launch_bounds__(kCombineRowsPerBlock * 32)
-combine_kernel(AttnParams p, int32_t team_size) {
+combine_kernel(AttnParams p, const __grid_constant__ InlineAttnMeta inl, int32_t team_size) {
+  pdl_wait();                      // partials of the attention kernel launched just before
+  pdl_launch_dependents();         // the next step's append does not depend on this kernel
+  if (p.meta == nullptr) p.meta = inl.w;
   const AttnMeta hdr = *reinterpret_cast<const AttnMeta*>(p.meta);
   const int32_t blocks_per_pair = kPairRows / kCombineRowsPerBlock;
   int32_t b = blockIdx.x;
@@ -59,12 +62,12 @@ combine_kernel(AttnParams p, int32_t team_size) {
     p.lse[(int64_t)tok * p.Hq + head] = (mx + log2f(wsum)) * 0.6931471805599453f;
 }
 
-cudaError_t launch_combine(const AttnParams& p, int32_t num_combine, int32_t team_size,
-                           cudaStream_t stream) {
+cudaError_t launch_combine(const AttnParams& p, const InlineAttnMeta& inl, int32_t num_combine,
+                           int32_t team_size, cudaStream_t stream) {
   if (num_combine == 0) return cudaSuccess;
   int32_t grid = num_combine * team_size * (kPairRows / kCombineRowsPerBlock);
-  combine_kernel<<<grid, kCombineRowsPerBlock * 32, 0, stream>>>(p, team_size);
-  return cudaGetLastError();
+  return launch_pdl(combine_kernel, dim3(grid), dim3(kCombineRowsPerBlock * 32), 0, stream, p, inl,
+                    team_size);
 }
 
 }  // namespace ws

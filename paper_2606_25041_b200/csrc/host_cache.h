@@ -12,6 +12,7 @@ namespace ws {
 struct SessionState {
   bool open = false;
   int64_t tokens = 0;
+  int64_t stable_tokens = 0;         // tokens whose append kernels are known complete (see api.cu)
   std::vector<int32_t> pages;        // physical page ids, logical page i -> pages[i]
   std::vector<int64_t> block_ends;   // e_1 < ... < e_B
   std::vector<uint8_t> modality;     // per committed token (optional metadata, may be shorter)
@@ -36,6 +37,7 @@ class HostCache {
   int32_t commit_block(int32_t s, int64_t n, const uint8_t* modality);
   bool truncate_blocks(int32_t s, int32_t keep_blocks);
 
+  void mark_all_stable() { for (auto& s : sess_) if (s.open) s.stable_tokens = s.tokens; }
   int32_t free_pages() const { return (int32_t)free_.size(); }
   void shuffle_free(uint64_t seed);
   int32_t page_tokens() const { return P_; }

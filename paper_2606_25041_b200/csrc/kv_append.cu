@@ -15,8 +15,13 @@ namespace ws {
 __global__ void __launch_bounds__(256)
 kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
                  int4* __restrict__ k_pool, int4* __restrict__ v_pool,
-                 int32_t* __restrict__ page_table, const int32_t* __restrict__ meta,
+                 int32_t* __restrict__ page_table, const int32_t* __restrict__ meta_g,
+                 const __grid_constant__ InlineAppendMeta inl,
                  int32_t max_pages, int32_t P, int32_t Hkv, int32_t chunks_per_head) {
+  // Nothing this kernel touches is produced by its stream predecessor (the previous step's combine
+  // writes only `out`), so the successor (this step's attention) may start its prologue right away.
+  pdl_launch_dependents();
+  const int32_t* meta = meta_g ? meta_g : inl.w;
   const AppendMeta hdr = *reinterpret_cast<const AppendMeta*>(meta);
   const AppendSession* sess = reinterpret_cast<const AppendSession*>(meta + hdr.off_sessions);
   const int32_t* pages = meta + hdr.off_pages;
@@ -52,6 +57,9 @@ kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
     k_pool[dst] = k_new[idx];
     v_pool[dst] = v_new[idx];
   }
+  // Completing only after the predecessor has completed keeps the dependency chain transitive: the
+  // attention kernel's griddepcontrol.wait on this grid then also covers everything before it.
+  pdl_wait();
 }
 
 __global__ void __launch_bounds__(256)
@@ -76,17 +84,16 @@ kv_gather_kernel(const int4* __restrict__ k_pool, const int4* __restrict__ v_poo
 }
 
 cudaError_t launch_kv_append(const void* k_new, const void* v_new, void* k_pool, void* v_pool,
-                             int32_t* page_table, const int32_t* meta, int32_t total_tokens,
-                             int32_t max_pages, int32_t P, int32_t Hkv, int32_t D, int32_t eb,
-                             int32_t num_sms, cudaStream_t stream) {
+                             int32_t* page_table, const int32_t* meta, const InlineAppendMeta& inl,
+                             int32_t total_tokens, int32_t max_pages, int32_t P, int32_t Hkv,
+                             int32_t D, int32_t eb, int32_t num_sms, cudaStream_t stream) {
   int32_t cph = D * eb / 16;
   int64_t total = (int64_t)total_tokens * Hkv * cph;
   int64_t blocks = (total + 255) / 256;
   int32_t grid = (int32_t)std::min<int64_t>(std::max<int64_t>(blocks, 1), (int64_t)num_sms * 8);
-  kv_append_kernel<<<grid, 256, 0, stream>>>((const int4*)k_new, (const int4*)v_new, (int4*)k_pool,
-                                             (int4*)v_pool, page_table, meta, max_pages, P, Hkv,
-                                             cph);
-  return cudaGetLastError();
+  return launch_pdl(kv_append_kernel, dim3(grid), dim3(256), 0, stream, (const int4*)k_new,
+                    (const int4*)v_new, (int4*)k_pool, (int4*)v_pool, page_table, meta, inl,
+                    max_pages, P, Hkv, cph);
 }
 
 cudaError_t launch_kv_gather(const void* k_pool, const void* v_pool, void* k_out, void* v_out,

@@ -5,13 +5,34 @@
 #include <stdint.h>
 
 #include <algorithm>
+#include <utility>
 
 #include "ws_internal.h"
 
 namespace ws {
 
+// PDL helpers: every kernel of the append -> attention -> combine chain is launched with
+// programmatic stream serialization; inside, griddepcontrol.wait guards the first access to data
+// the predecessor may still be writing and griddepcontrol.launch_dependents lets the successor start.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                       cudaStream_t stream, Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
+// meta == nullptr: the metadata blob is `inl` (passed in the kernel parameters)
 cudaError_t launch_kv_append(const void* k_new, const void* v_new, void* k_pool, void* v_pool,
-                             int32_t* page_table, const int32_t* meta, int32_t total_tokens,
+                             int32_t* page_table, const int32_t* meta, const InlineAppendMeta& inl,
+                             int32_t total_tokens,
                              int32_t max_pages, int32_t P, int32_t Hkv, int32_t D, int32_t eb,
                              int32_t num_sms, cudaStream_t stream);
 cudaError_t launch_kv_gather(const void* k_pool, const void* v_pool, void* k_out, void* v_out,
@@ -29,13 +50,14 @@ cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse
 
 // sm_100a tcgen05 kernel (bf16, D = 128, P = 64).
 struct Sm100Launch {
-  AttnParams p;
+  AttnParams p;                      // p.meta == nullptr: use `inl`
   CUtensorMap tmap_q, tmap_k, tmap_v;
+  InlineAttnMeta inl;
   int32_t num_ctas;
 };
 cudaError_t sm100_attn_configure();    // one-time cudaFuncSetAttribute
 cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream);
-cudaError_t launch_combine(const AttnParams& p, int32_t num_combine, int32_t team_size,
-                           cudaStream_t stream);
+cudaError_t launch_combine(const AttnParams& p, const InlineAttnMeta& inl, int32_t num_combine,
+                           int32_t team_size, cudaStream_t stream);
 
 }  // namespace ws

@@ -41,6 +41,7 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
         int32_t last_tok = std::min(s.q_end, g.q_token0 + g.npairs * tok_per_pair) - 1;
         g.kv_len = vis_end[last_tok];
         g.vis_off = s.multi_block ? g.q_token0 : -1;
+        g.dep_tile = s.stable_tokens / kTileKeys;
         plan.groups.push_back(g);
         int32_t nt = (g.kv_len + kTileKeys - 1) / kTileKeys;
         group_tiles.push_back(nt);
@@ -54,26 +55,33 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
   int32_t n_used = (int32_t)std::min<int64_t>(teams_avail, std::max<int64_t>(1, T / min_tiles));
   plan.num_teams = n_used;
 
-  // walk the flat tile axis; cut at team boundaries (and at forced split boundaries)
+  // Walk the flat tile axis; cut at team boundaries (and at forced split boundaries).  A team that
+  // continues into another group pays a fixed cost for the extra segment (Q reload, pipeline
+  // refill, epilogue), measured at ~3.3 KV tiles on B200: budgets are equalised in cost units.
+  const double ovh = cfg.seg_overhead_tiles;
+  const double total_cost = (double)T + ovh * std::max<double>(0.0, (double)plan.groups.size() - 1.0);
+  const double budget = total_cost / n_used;
   int32_t team = 0;
-  int64_t flat = 0;
-  auto boundary = [&](int32_t i) { return (int64_t)i * T / n_used; };
+  double used = 0.0;                 // cost consumed by the current team
   for (size_t gi = 0; gi < plan.groups.size(); ++gi) {
     int32_t nt = group_tiles[gi];
     int32_t per = cfg.min_splits > 0 ? std::max(1, (nt + cfg.min_splits - 1) / cfg.min_splits) : nt;
     int32_t t = 0;
     while (t < nt) {
-      while (team + 1 < n_used && flat >= boundary(team + 1)) ++team;
-      int64_t room = (team + 1 < n_used) ? boundary(team + 1) - flat : (int64_t)nt - t;
+      const bool last_team = team + 1 >= n_used;
+      const double seg_cost0 = (used > 0.0) ? ovh : 0.0;   // not the team's first segment
+      int64_t room = (int64_t)(budget - used - seg_cost0 + 0.5);
+      if (!last_team && room < 1) { ++team; used = 0.0; continue; }
+      if (last_team) room = nt - t;
       int32_t take = (int32_t)std::min<int64_t>(room, nt - t);
       take = std::min(take, per - (t % per));
-      Segment sg{(int32_t)gi, t, t + take, -1};
-      plan.segments.push_back(sg);
+      plan.segments.push_back(Segment{(int32_t)gi, t, t + take, -1});
       plan.seg_team.push_back(team);
+      used += seg_cost0 + take;
       t += take;
-      flat += take;
     }
   }
+  plan.num_teams = team + 1;
   // partial slots: only groups cut into more than one segment need them
   size_t i = 0;
   while (i < plan.segments.size()) {
@@ -90,9 +98,9 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
     }
     i = j;
   }
-  plan.team_seg_begin.assign(n_used + 1, 0);
+  plan.team_seg_begin.assign(plan.num_teams + 1, 0);
   for (int32_t tm : plan.seg_team) plan.team_seg_begin[tm + 1]++;
-  for (int32_t k = 0; k < n_used; ++k) plan.team_seg_begin[k + 1] += plan.team_seg_begin[k];
+  for (int32_t k = 0; k < plan.num_teams; ++k) plan.team_seg_begin[k + 1] += plan.team_seg_begin[k];
   plan.ok = plan.num_part_slots <= cfg.max_part_slots;
   return plan;
 }

@@ -14,12 +14,14 @@ struct PlanSession {
   int32_t q_begin;       // first global query token of this session in the call
   int32_t q_end;         // exclusive
   bool multi_block;      // queries span more than one block (per-token visible ends differ)
+  int32_t stable_tokens; // cache tokens that no in-flight predecessor kernel can still be writing
 };
 
 struct PlanConfig {
   int32_t Hkv, G;        // KV heads, q heads per KV head
   int32_t num_sms;       // CTAs that can be resident at once (1 CTA / SM)
   int32_t min_tiles;     // do not cut the work finer than this many KV tiles per segment
+  float seg_overhead_tiles;  // cost of starting one more segment in a team, in KV-tile units
   int32_t min_splits;    // debug: force at least this many segments per group (0 = automatic)
   int32_t max_part_slots;
 };

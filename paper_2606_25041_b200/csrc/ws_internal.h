@@ -11,6 +11,14 @@ constexpr int kMaxTeam = 8;       // max row-tile pairs of one (session, KV head
 
 // One (session, KV head, sub-range of the session's query tokens): all of its row-tile pairs share
 // the same K/V stream, so the CTAs of one team walk the same KV tiles in lock-step (L2 reuse).
+// Small per-call metadata travels in the kernel parameters instead of a host->device copy (keeps the
+// append -> attention -> combine chain free of stream operations between the kernels, which is what
+// lets programmatic dependent launch overlap them).  Larger blobs go through the workspace ring.
+constexpr int kInlineAttnWords = 800;     // 3200 B of the 4 KB kernel-parameter space
+constexpr int kInlineAppendWords = 120;
+struct InlineAttnMeta { int32_t w[kInlineAttnWords]; };
+struct InlineAppendMeta { int32_t w[kInlineAppendWords]; };
+
 struct Group {
   int32_t q_token0;      // first global query token (row of q/out) covered by this group
   int32_t q_token_end;   // end (exclusive) of the session's query tokens: rows beyond are not stored
@@ -19,7 +27,9 @@ struct Group {
   int32_t kv_len;        // keys visible to the LAST row of the group (= max visible end)
   int32_t npairs;        // row-tile pairs in this group (<= team size)
   int32_t vis_off;       // >= 0: per-token visible ends at vis_end[vis_off + (token - q_token0)]
-  int32_t pad;
+  int32_t dep_tile;      // KV tiles >= dep_tile (and their page-table entries) may have been written by
+                         // the kernel launched just before (the append of this step): the TMA producer
+                         // executes griddepcontrol.wait before touching them
 };
 
 // A contiguous KV-tile range of one group, processed by one team (CTA p handles pair p).
