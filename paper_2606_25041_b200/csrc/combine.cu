@@ -3,6 +3,9 @@
 //   m* = max_s LSE_s ; w_s = 2^(LSE_s - m*) ; O = sum_s w_s O_s / sum_s w_s ; LSE = m* + log2 sum_s w_s
 // (partials carry log2-domain LSEs; an empty range carries LSE = -inf and contributes w = 0).
 // HBM/L2-bound: reads nparts x 256 x (D+1) fp32 per (group, pair), writes bf16 O (+ fp32 LSE).
+// One warp per packed row: lane s loads the LSE of part s, the max and the weight sum are reduced
+// with warp shuffles, then the parts' O rows (one float4 per lane, D = 128) are accumulated with
+// four loads in flight per lane.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <math.h>
@@ -11,7 +14,7 @@
 
 namespace ws {
 
-constexpr int kCombineRowsPerBlock = 8;   // one warp per packed row, D = 128 -> one float4 per lane
+constexpr int kCombineRowsPerBlock = 8;
 
 __global__ void __launch_bounds__(kCombineRowsPerBlock * 32)
 combine_kernel(AttnParams p, const __grid_constant__ InlineAttnMeta inl, int32_t team_size) {
@@ -32,25 +35,49 @@ combine_kernel(AttnParams p, const __grid_constant__ InlineAttnMeta inl, int32_t
   const int32_t tok = g.q_token0 + pair * (kPairRows / p.G) + r / p.G;
   if (tok >= g.q_token_end) return;
   const int32_t head = g.kv_head * p.G + r % p.G;
+  const int64_t slot0 = ci.part_base + pair;            // slot(i) = slot0 + i * npairs
+  const int64_t stride = g.npairs;
 
-  float mx = -INFINITY;
-  for (int i = 0; i < ci.nparts; ++i) {
-    int64_t slot = ci.part_base + (int64_t)i * g.npairs + pair;
-    mx = fmaxf(mx, p.part_lse[slot * kPairRows + r]);
-  }
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-  float wsum = 0.f;
-  for (int i = 0; i < ci.nparts; ++i) {
-    int64_t slot = ci.part_base + (int64_t)i * g.npairs + pair;
-    float l2 = p.part_lse[slot * kPairRows + r];
-    if (l2 == -INFINITY) continue;
-    float w = exp2f(l2 - mx);
-    const float4 o = reinterpret_cast<const float4*>(p.part_o + (slot * kPairRows + r) * p.D)[lane];
-    acc.x = fmaf(w, o.x, acc.x); acc.y = fmaf(w, o.y, acc.y);
-    acc.z = fmaf(w, o.z, acc.z); acc.w = fmaf(w, o.w, acc.w);
-    wsum += w;
+  float mx_run = -INFINITY, wsum_run = 0.f;
+  // parts are processed in chunks of 32 (one LSE per lane); a chunk's results are merged into the
+  // running (max, sum, acc) with the usual rescale - almost always there is a single chunk
+  for (int32_t base = 0; base < ci.nparts; base += 32) {
+    const int32_t i = base + lane;
+    const float l2 = i < ci.nparts ? p.part_lse[(slot0 + i * stride) * kPairRows + r] : -INFINITY;
+    float mx = l2;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    const float mx_new = fmaxf(mx_run, mx);
+    if (mx_new == -INFINITY) continue;                  // nothing visible in these parts
+    const float w = l2 == -INFINITY ? 0.f : exp2f(l2 - mx_new);
+    float ws = w;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ws += __shfl_xor_sync(0xffffffffu, ws, o);
+    const float rescale = mx_run == -INFINITY ? 0.f : exp2f(mx_run - mx_new);
+    acc.x *= rescale; acc.y *= rescale; acc.z *= rescale; acc.w *= rescale;
+    wsum_run = wsum_run * rescale + ws;
+    mx_run = mx_new;
+    const int32_t cnt = min(32, ci.nparts - base);
+    for (int32_t k0 = 0; k0 < cnt; k0 += 4) {
+      float4 o[4];
+      float wk[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int32_t k = k0 + u;
+        wk[u] = __shfl_sync(0xffffffffu, w, k & 31);
+        if (k < cnt && wk[u] != 0.f)
+          o[u] = reinterpret_cast<const float4*>(p.part_o + ((slot0 + (base + k) * stride) * kPairRows + r) * p.D)[lane];
+        else { o[u] = make_float4(0.f, 0.f, 0.f, 0.f); wk[u] = 0.f; }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        acc.x = fmaf(wk[u], o[u].x, acc.x); acc.y = fmaf(wk[u], o[u].y, acc.y);
+        acc.z = fmaf(wk[u], o[u].z, acc.z); acc.w = fmaf(wk[u], o[u].w, acc.w);
+      }
+    }
   }
-  const float inv = 1.f / wsum;
+  const float inv = 1.f / wsum_run;
   __nv_bfloat162 lo = __floats2bfloat162_rn(acc.x * inv, acc.y * inv);
   __nv_bfloat162 hi = __floats2bfloat162_rn(acc.z * inv, acc.w * inv);
   uint2 packed;
@@ -59,7 +86,7 @@ combine_kernel(AttnParams p, const __grid_constant__ InlineAttnMeta inl, int32_t
   __nv_bfloat16* orow = reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)tok * p.Hq + head) * p.D;
   reinterpret_cast<uint2*>(orow)[lane] = packed;
   if (p.lse && lane == 0)
-    p.lse[(int64_t)tok * p.Hq + head] = (mx + log2f(wsum)) * 0.6931471805599453f;
+    p.lse[(int64_t)tok * p.Hq + head] = (mx_run + log2f(wsum_run)) * 0.6931471805599453f;
 }
 
 cudaError_t launch_combine(const AttnParams& p, const InlineAttnMeta& inl, int32_t num_combine,

@@ -185,6 +185,14 @@ def test_split_count_invariance(splits):
     _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, f"splits={splits}")
 
 
+def test_many_splits_combine_chunks():
+    """71 one-tile segments per group: the combine kernel merges more than 32 parts per row."""
+    w = _small(2, cache_lens=(9000,), num_q_heads=2, num_kv_heads=1, block_tokens=64, modality_split=(48, 12, 4))
+    got = run_workload_gpu(w, min_splits=71)
+    assert got["plans"][-1]["num_segments"] >= 71
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "71 splits")
+
+
 def test_page_assignment_independence():
     w = _small(3, cache_lens=(1500,), block_tokens=64, modality_split=(48, 12, 4))
     a = run_workload_gpu(w, gather=False)
