@@ -404,6 +404,37 @@ def test_config5_ragged_multi_session_sampled():
     _assert_close(compare(got, ref, "bf16", rows=rows, heads=heads), BF16_TOL, "cfg5")
 
 
+def test_outputs_stay_inside_their_buffers():
+    """compute-sanitizer is closed on this GPU pool, so out-of-bounds writes are caught with canaries:
+    `out`, `lse` and the workspace's neighbours are slices of larger canary-filled tensors; a ragged
+    3-session call with split partials must leave every guard element untouched and write every
+    element it owns (no NaN canary left inside)."""
+    import torch
+    w = _small(5, num_sessions=3, cache_len_range=(300, 2500), block_tokens=72, modality_split=(54, 12, 6))
+    dev = torch.device("cuda", 0)
+    cache = make_cache(w)
+    cache.set_min_splits(3)
+    ids = preload_gpu(cache, w, [_torch_of(s.k_cache, dev) for s in w.sessions],
+                      [_torch_of(s.v_cache, dev) for s in w.sessions])
+    n, S, Hq, D = 72, 3, 32, 128
+    q = torch.cat([_torch_of(s.q[0], dev) for s in w.sessions])
+    k = torch.cat([_torch_of(s.k[0], dev) for s in w.sessions])
+    v = torch.cat([_torch_of(s.v[0], dev) for s in w.sessions])
+    guard = 4096
+    big_out = torch.full((guard + S * n * Hq * D + guard,), float("nan"), dtype=torch.bfloat16, device=dev)
+    big_lse = torch.full((guard + S * n * Hq + guard,), float("nan"), dtype=torch.float32, device=dev)
+    out = big_out[guard:guard + S * n * Hq * D].view(S * n, Hq, D)
+    lse = big_lse[guard:guard + S * n * Hq].view(S * n, Hq)
+    cu = [0, n, 2 * n, 3 * n]
+    cache.kv_append(ids, cu, k, v)
+    cache.block_causal_attn_fwd(ids, cu, q, out, w.spec.scale, lse=lse)
+    torch.cuda.synchronize()
+    assert cache.last_plan_info()["num_combine_items"] > 0
+    assert torch.isnan(big_out[:guard]).all() and torch.isnan(big_out[-guard:]).all()
+    assert torch.isnan(big_lse[:guard]).all() and torch.isnan(big_lse[-guard:]).all()
+    assert torch.isfinite(out.float()).all() and torch.isfinite(lse).all()
+
+
 def test_stream_step_host_end_to_end():
     """ws_stream_step_host: pinned host buffers in, host result out, equals the device-pointer path."""
     import torch
