@@ -137,6 +137,55 @@ def read_traffic(cfg: int):
     return None
 
 
+def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, reset):
+    """NEXT-2: one solver step (append + attention + combine of an uncommitted block at the headline
+    shape) replayed from a CUDA graph.  NEXT-1: an 8192-token prompt (32 blocks of 256) prefilled in
+    one multi-block call."""
+    import math
+    import torch
+    from paper_2606_25041_b200 import WS_BF16, Cache
+    res = {}
+    # --- NEXT-2: CUDA-graph replay of one solver step
+    reset()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        cache.kv_append(ids, cu, k0, v0)
+        cache.block_causal_attn_fwd(ids, cu, q0, out, sp.scale)
+    reps = 200
+    for _ in range(5):
+        g.replay()
+    ms = timed(reps, lambda i: g.replay())
+    L = cache.session_info(ids[0])[0]
+    fl = 4.0 * sp.head_dim * sp.num_q_heads * sp.block_tokens * sum(cache.session_info(i)[0] for i in ids)
+    res["solver_step_cuda_graph"] = {"us_per_step": 1e3 * ms / reps, "tflops": fl / (ms / reps * 1e-3) / 1e12,
+                                     "kv_tokens": L, "replays": reps,
+                                     "what": "append + attention + combine of one uncommitted block, graph replay"}
+    reset()
+    # --- NEXT-1: multi-block prefill
+    Hq, Hkv, D, n, B = sp.num_q_heads, sp.num_kv_heads, sp.head_dim, 256, 32
+    T = n * B
+    c2 = Cache(WS_BF16, Hq, Hkv, D, 64, T // 64 + 4, max_sessions=1, max_q_tokens_per_call=T, device=dev.index or 0)
+    sid = c2.session_open()
+    gen = torch.Generator(device=dev); gen.manual_seed(2606)
+    mk = lambda h: torch.randn((T, h, D), device=dev, dtype=torch.float32, generator=gen).bfloat16()
+    q, k, v = mk(Hq), mk(Hkv), mk(Hkv)
+    for b in range(B):
+        c2.kv_append([sid], [0, n], k[b * n:(b + 1) * n], v[b * n:(b + 1) * n])
+    o2 = torch.empty_like(q)
+    call = lambda i: c2.block_causal_attn_fwd([sid], [0, T], q, o2, 1.0 / math.sqrt(D), num_q_blocks=[B])
+    for i in range(3):
+        call(i)
+    reps = 30
+    ms = timed(reps, call)
+    fl = 4.0 * D * Hq * sum(n * n * (b + 1) for b in range(B))
+    res["prefill_multi_block"] = {"tokens": T, "blocks": B, "us": 1e3 * ms / reps,
+                                  "tflops": fl / (ms / reps * 1e-3) / 1e12,
+                                  "what": "32 committed blocks of 256 tokens queried in one call (block-causal FLOPs)"}
+    c2.close()
+    return res
+
+
 def run_reference(args, spec):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -174,6 +223,7 @@ def main():
     ap.add_argument("--ref-rows", type=int, default=256, help="query tokens per session the oracle leg computes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-next", action="store_true", help="skip the NEXT-1 / NEXT-2 side measurements")
     args = ap.parse_args()
     spec = CONFIG_SPECS[args.config]
     if args.impl == "reference":
@@ -324,6 +374,11 @@ def main():
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(oh.numel() * 2),
                "api": "ws_stream_step_host (pinned host q/k/v in, pinned host out)"}
 
+    # ---- side measurements of the widened rows; not part of `value`
+    nxt = None
+    if not args.no_next and world == 1:
+        nxt = measure_next(cache, ids, base_blocks, sp, cu, q_d[0], k_d[0], v_d[0], out, dev, timed, reset)
+
     # ---- CPU baseline: the oracle on a bounded sample, rank 0 at N=1 only
     cpu = None
     if not args.no_cpu_baseline and world == 1:
@@ -349,6 +404,7 @@ def main():
                            "parallelism": f"dp{world} (independent sessions per GPU, no collective)",
                            "plan": plan},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+                "next": nxt,
                 "clocks": sampler.result(),
                 "context": {"paper_model_side_latency_ms": 200, "paper_total_latency_ms": 550,
                             "paper_hardware": "two-GPU thinker-performer path, GPU model not stated (PAPER.md:89)",

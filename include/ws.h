@@ -140,6 +140,15 @@ ws_status_t ws_stream_step_host(ws_cache_t* cache, int32_t num_sessions, const i
                                 const void* k_new_host, const void* v_new_host, void* out_host,
                                 void* staging, size_t staging_bytes, float scale, void* cuda_stream);
 
+/* NEXT-2 (solver-step mode): explicit Euler step of the flow-matching solver on a
+ * latent unit, z <- z + dtau * v  (Eq. (2): dz/dtau = eps - z_0 is the velocity the model
+ * predicts; dtau < 0 integrates from noise to data).  z, v: DEVICE, 16-byte aligned, `count` elements
+ * of `dtype` (ws_dtype_t); fp32 arithmetic, one rounding to the storage dtype.  An uncommitted noisy
+ * block is attended with ws_kv_append + ws_block_causal_attn_fwd + ws_session_truncate(keep) per
+ * solver step (stage / attend / roll back); the clean block is committed by the last append. */
+ws_status_t ws_fm_euler_update(int32_t dtype, void* z, const void* v, float dtau, int64_t count,
+                               void* cuda_stream);
+
 /* Read back logical tokens [start, start+count) of a session into contiguous [count][Hkv][D]
  * DEVICE buffers (either may be NULL).  Test / snapshot utility. */
 ws_status_t ws_kv_gather(const ws_cache_t* cache, int32_t session, int64_t start, int64_t count,

@@ -161,3 +161,13 @@ def attend_range(sess: OracleSession, q: np.ndarray, scale: float, key_lo: int, 
         out[:, h, :] = (P / Z) @ Vg
         lse[:, h] = (m + np.log(Z))[:, 0]
     return out, lse
+
+
+def fm_euler_update(z: np.ndarray, v: np.ndarray, dtau: float) -> np.ndarray:
+    """NEXT-2: one explicit Euler step of the flow-matching ODE, z <- z + dtau * v, in float64.
+
+    Eq. (2): z_tau = (1 - tau) z_0 + tau eps and dz/dtau = eps - z_0, so with the
+    exact velocity v = eps - z_0 a single step of size dtau = -tau from z_tau lands on z_0
+    (pinned by tests/test_oracle_pins.py::test_fm_euler_exact_velocity_recovers_clean_latent).
+    """
+    return np.asarray(z, dtype=np.float64) + float(dtau) * np.asarray(v, dtype=np.float64)

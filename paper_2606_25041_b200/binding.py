@@ -54,7 +54,7 @@ class PlanSegment(C.Structure):
 EXPORTS = ["ws_pool_bytes", "ws_workspace_bytes", "ws_cache_create", "ws_cache_destroy",
            "ws_session_open", "ws_session_close", "ws_session_info", "ws_session_truncate",
            "ws_free_pages", "ws_kv_append", "ws_block_causal_attn_fwd", "ws_step_staging_bytes",
-           "ws_stream_step_host", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
+           "ws_stream_step_host", "ws_fm_euler_update", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
            "ws_debug_set_min_splits", "ws_last_plan_info", "ws_last_plan_segment",
            "ws_launch_count", "ws_debug_kernel_timing", "ws_debug_read_kernel_times",
            "ws_status_str", "ws_last_error", "ws_version"]
@@ -90,6 +90,7 @@ def load_library() -> C.CDLL:
     lib.ws_step_staging_bytes.argtypes = [cfgp, C.c_int32]
     lib.ws_stream_step_host.argtypes = [vp, C.c_int32, i32p, i32p, vp, vp, vp, vp, vp, C.c_size_t,
                                         C.c_float, vp]
+    lib.ws_fm_euler_update.argtypes = [C.c_int32, vp, vp, C.c_float, C.c_int64, vp]
     lib.ws_kv_gather.argtypes = [vp, C.c_int32, C.c_int64, C.c_int64, vp, vp, vp]
     lib.ws_session_pages.argtypes = [vp, C.c_int32, i32p, C.c_int32, i32p]
     lib.ws_debug_shuffle_free_pages.argtypes = [vp, C.c_uint64]
@@ -303,6 +304,15 @@ def ws_stream_step_host(cache: Cache, session_ids, cu_new_tokens, q_host, k_host
                         staging, scale, stream=None):
     cache.stream_step_host(session_ids, cu_new_tokens, q_host, k_host, v_host, out_host, staging,
                            scale, stream)
+
+
+def ws_fm_euler_update(z, v, dtau: float, stream=None):
+    """z <- z + dtau * v in place (torch bf16 / fp32 tensors, same shape, contiguous)."""
+    import torch
+    if z.dtype != v.dtype or z.numel() != v.numel():
+        raise ValueError("z and v must have the same dtype and size")
+    dt = {torch.bfloat16: WS_BF16, torch.float32: WS_F32}[z.dtype]
+    _check(load_library().ws_fm_euler_update(dt, _ptr(z), _ptr(v), C.c_float(dtau), z.numel(), _stream_ptr(stream)))
 
 
 def ws_version() -> str:

@@ -22,7 +22,7 @@ TAG = os.environ.get("WS_BUILD_TAG", "")
 DEFS = os.environ.get("WS_BUILD_DEFS", "").split()
 OUT = os.path.join(PKG, f"libwanstream{'_' + TAG if TAG else ''}.so")
 OBJ = os.path.join(PKG, "build" + ("_" + TAG if TAG else ""))
-SOURCES = ["api.cu", "kv_append.cu", "attn_simt.cu", "attn_sm100.cu", "combine.cu",
+SOURCES = ["api.cu", "kv_append.cu", "attn_simt.cu", "attn_sm100.cu", "combine.cu", "fm_euler.cu",
            "host_cache.cpp", "plan.cpp"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

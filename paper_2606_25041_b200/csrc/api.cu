@@ -608,6 +608,16 @@ ws_status_t ws_stream_step_host(ws_cache_t* c, int32_t S, const int32_t* session
   return WS_OK;
 }
 
+ws_status_t ws_fm_euler_update(int32_t dtype, void* z, const void* v, float dtau, int64_t count,
+                               void* cuda_stream) {
+  if (dtype != WS_BF16 && dtype != WS_F32) return fail(WS_ERR_INVALID_ARG, "dtype");
+  if (count < 0 || (count > 0 && (!z || !v))) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  if (((uintptr_t)z & 15) || ((uintptr_t)v & 15)) return fail(WS_ERR_INVALID_ARG, "z / v must be 16-byte aligned");
+  if (!std::isfinite(dtau)) return fail(WS_ERR_INVALID_ARG, "dtau must be finite");
+  WS_CUDA(ws::launch_fm_euler(dtype, z, v, dtau, count, (cudaStream_t)cuda_stream));
+  return WS_OK;
+}
+
 ws_status_t ws_kv_gather(const ws_cache_t* c, int32_t session, int64_t start, int64_t count,
                          void* k_out, void* v_out, void* cuda_stream) {
   if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");

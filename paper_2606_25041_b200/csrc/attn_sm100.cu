@@ -80,14 +80,23 @@ struct SegView {
   int32_t tile_begin, tile_end, part_base;
 };
 
+// Loads segment `si` as seen by row-tile pair `pair`.  Returns false if this CTA has no rows in it
+// (pair >= npairs).  For multi-block queries the pair's own visible end clips the tile range: KV
+// tiles beyond the last key any of the pair's rows can see are skipped (block-lower-triangular
+// skipping at pair granularity); `v.tile_end <= v.tile_begin` then means "nothing to compute here".
 __device__ __forceinline__ bool load_segment(const int32_t* meta, const AttnMeta& hdr, int32_t si,
-                                             int32_t pair, SegView& v) {
+                                             int32_t pair, int32_t tok_per_pair, SegView& v) {
   const Segment s = reinterpret_cast<const Segment*>(meta + hdr.off_segments)[si];
   v.g = reinterpret_cast<const Group*>(meta + hdr.off_groups)[s.group];
   v.tile_begin = s.tile_begin; v.tile_end = s.tile_end; v.part_base = s.part_base;
-  return pair < v.g.npairs;
+  if (pair >= v.g.npairs) return false;
+  if (v.g.vis_off >= 0) {
+    const int32_t last_tok = min(v.g.q_token_end, v.g.q_token0 + (pair + 1) * tok_per_pair) - 1;
+    const int32_t pair_kv = (meta + hdr.off_vis)[v.g.vis_off + (last_tok - v.g.q_token0)];
+    v.tile_end = min(v.tile_end, (pair_kv + kTileKeys - 1) / kTileKeys);
+  }
+  return true;
 }
-
 
 // 2^x for a PAIR of values on the FMA/ALU pipes (no MUFU): round-to-nearest split x = r + f with
 // f in [-0.5, 0.5], a degree-3 minimax polynomial for 2^f (max relative error 7.5e-5, well inside
@@ -207,7 +216,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       bool dep_waited = false;
       for (int32_t si = seg_lo; si < seg_hi; ++si) {
         SegView sv;
-        if (!load_segment(p.meta, hdr, si, pair, sv)) continue;
+        if (!load_segment(p.meta, hdr, si, pair, tok_per_pair, sv)) continue;
+        if (sv.tile_end <= sv.tile_begin) continue;          // clipped away for this pair
         const int32_t* page_row = p.page_table + (int64_t)sv.g.slot * p.max_pages_per_session;
         const int32_t last_page = (sv.g.kv_len - 1) / p.P;
         // tiles >= dep_tile may still be being written by the preceding append kernel (PDL)
@@ -278,7 +288,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       };
       for (int32_t si = seg_lo; si < seg_hi; ++si) {
         SegView sv;
-        if (!load_segment(p.meta, hdr, si, pair, sv)) continue;
+        if (!load_segment(p.meta, hdr, si, pair, tok_per_pair, sv)) continue;
+        if (sv.tile_end <= sv.tile_begin) continue;          // clipped away for this pair
         const int32_t nt = sv.tile_end - sv.tile_begin;
         mbar_wait(bq_full, q_it & 1);
         {
@@ -360,14 +371,23 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t t_o = tmem_base + (lane_base << 16) + 256 + q * 128;
     const float c = p.scale * 1.4426950408889634f;
     uint32_t ring_it = 0, tile_it = 0, seg_it = 0;
+    bool pdl_done = false;
     PROF_DECL(8)
 
     for (int32_t si = seg_lo; si < seg_hi; ++si) {
       SegView sv;
-      if (!load_segment(p.meta, hdr, si, pair, sv)) continue;
+      if (!load_segment(p.meta, hdr, si, pair, tok_per_pair, sv)) continue;
       const int32_t nt = sv.tile_end - sv.tile_begin;
       const int32_t tok = sv.g.q_token0 + pair * tok_per_pair + R / p.G;
       const bool row_valid = tok < sv.g.q_token_end;
+      if (nt <= 0) {
+        // every tile of this segment lies beyond what the pair can see: publish an empty partial
+        // (the segment is one of several splits, otherwise it would start at tile 0)
+        if (!pdl_done) { pdl_wait(); pdl_done = true; }
+        if (row_valid && sv.part_base >= 0)
+          p.part_lse[(int64_t)(sv.part_base + pair) * kPairRows + R] = -INFINITY;
+        continue;
+      }
       const int32_t head = sv.g.kv_head * p.G + R % p.G;
       int32_t vis = sv.g.kv_len;
       if (sv.g.vis_off >= 0 && row_valid) vis = (p.meta + hdr.off_vis)[sv.g.vis_off + (tok - sv.g.q_token0)];
@@ -552,7 +572,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       // ---------------------------------------------------- epilogue
       // first global write of this CTA: the predecessor grids (append; transitively the previous
       // step's combine, which reads the partial buffers and writes `out`) must have completed
-      if (seg_it == 0) pdl_wait();
+      if (!pdl_done) { pdl_wait(); pdl_done = true; }
       mbar_wait(bo_full(q), seg_it & 1);
       tc_fence_after();
       const float inv_l = l > 0.f ? 1.f / l : 0.f;

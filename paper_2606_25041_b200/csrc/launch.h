@@ -42,6 +42,10 @@ cudaError_t launch_kv_gather(const void* k_pool, const void* v_pool, void* k_out
                              int32_t Hkv, int32_t D, int32_t eb, int32_t num_sms,
                              cudaStream_t stream);
 
+// NEXT-2: flow-matching Euler update z <- z + dtau * v (dtype 0 = bf16, 1 = fp32), 16-byte aligned.
+cudaError_t launch_fm_euler(int32_t dtype, void* z, const void* v, float dtau, int64_t count,
+                            cudaStream_t stream);
+
 // Generic SIMT attention (fp32 config; bf16 debug / unsupported-shape path).
 // tok_meta: [2][total_q_tokens] int32 = session slot, visible end per query token.
 cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse,

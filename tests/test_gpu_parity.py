@@ -248,6 +248,157 @@ def test_multi_block_query_tensor_core():
     assert np.abs(lse.cpu().numpy() - l_ref).max() <= 1e-3
 
 
+def _prefill_case(block_sizes, Hq, Hkv, seed, L0=0):
+    """one session: optional committed cache of L0 tokens, then `block_sizes` appended and queried in
+    ONE call (num_q_blocks = len(block_sizes)); returns (gpu O, gpu LSE, oracle O, oracle LSE)."""
+    import torch
+    from oracle.block_causal import OracleSession, attend
+    from paper_2606_25041_b200 import WS_BF16, Cache
+    rng = np.random.default_rng(seed)
+    T = sum(block_sizes)
+    mk = lambda *sh: to_bf16(rng.standard_normal(sh, dtype=np.float32))
+    k0, v0 = mk(L0, Hkv, 128), mk(L0, Hkv, 128)
+    q, k, v = mk(T, Hq, 128), mk(T, Hkv, 128), mk(T, Hkv, 128)
+    P = 64
+    c = Cache(WS_BF16, Hq, Hkv, 128, P, (L0 + T) // P + 4, max_sessions=1, max_q_tokens_per_call=max(T, 256))
+    sid = c.session_open()
+    dev = torch.device("cuda", 0)
+    sess = OracleSession(Hkv, 128)
+    pos = 0
+    while pos < L0:
+        hi = min(L0, pos + 256)
+        c.kv_append([sid], [0, hi - pos], _torch_of(k0[pos:hi], dev), _torch_of(v0[pos:hi], dev))
+        sess.append(k0[pos:hi], v0[pos:hi]); pos = hi
+    pos = 0
+    for b in block_sizes:
+        c.kv_append([sid], [0, b], _torch_of(k[pos:pos + b], dev), _torch_of(v[pos:pos + b], dev))
+        sess.append(k[pos:pos + b], v[pos:pos + b]); pos += b
+    out = torch.full((T, Hq, 128), float("nan"), dtype=torch.bfloat16, device=dev)
+    lse = torch.full((T, Hq), float("nan"), dtype=torch.float32, device=dev)
+    scale = 1.0 / math.sqrt(128)
+    c.block_causal_attn_fwd([sid], [0, T], _torch_of(q, dev), out, scale, lse=lse, num_q_blocks=[len(block_sizes)])
+    torch.cuda.synchronize()
+    assert c.last_plan_info()["used_tensor_core_kernel"] == 1
+    o_ref, l_ref = attend(sess, q, scale, len(block_sizes))
+    return out.float().cpu().numpy(), lse.cpu().numpy(), o_ref, l_ref
+
+
+@pytest.mark.parametrize("blocks,Hq,Hkv,L0", [
+    ([256] * 8, 8, 2, 0),                 # system prefill: 2048-token prompt in 8 units, empty cache
+    ([100, 37, 256, 1, 300], 4, 4, 500),  # ragged blocks (MHA), behind a committed cache
+    ([64] * 24, 16, 2, 0),                # G = 8, many short blocks: several blocks per Q-tile pair
+])
+def test_next1_multi_block_prefill(blocks, Hq, Hkv, L0):
+    """NEXT-1 (PAPER.md:75 system prefill; :69 training-format equivalence): many committed blocks
+    queried in one call on the tcgen05 path - block-lower-triangular skipping per Q-tile pair, per-row
+    masks inside partially visible tiles."""
+    o, lse, o_ref, l_ref = _prefill_case(blocks, Hq, Hkv, seed=sum(blocks) + Hq, L0=L0)
+    d = o - o_ref
+    assert np.isfinite(o).all() and np.isfinite(lse).all()
+    assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3
+    assert np.sqrt((d ** 2).mean() / (o_ref ** 2).mean()) <= 1e-2
+    assert np.abs(lse - l_ref).max() <= 1e-3
+
+
+# ------------------------------------------------------------------ NEXT-2: solver-step mode
+def test_next2_solver_steps_stage_attend_rollback():
+    """The performer's loop: per solver step an UNCOMMITTED noisy block attends to
+    the committed history + itself (append -> attend -> truncate), then the clean block is committed.
+    Every solver step must equal the oracle run on [history; that step's noisy block], and the final
+    history must hold only the clean block."""
+    import torch
+    from oracle.block_causal import OracleSession, attend, fm_euler_update
+    from paper_2606_25041_b200 import ws_fm_euler_update
+    w = _small(3, cache_lens=(1900,), block_tokens=128, modality_split=(96, 24, 8), steps=1)
+    si = w.sessions[0]
+    dev = torch.device("cuda", 0)
+    cache = make_cache(w)
+    ids = preload_gpu(cache, w, [_torch_of(si.k_cache, dev)], [_torch_of(si.v_cache, dev)])
+    base_blocks = cache.session_info(ids[0])[1]
+    hist = OracleSession(8, 128)
+    from tests.gpu_harness import preload_rounds
+    for _, rng_ in preload_rounds(w):
+        lo, hi = rng_[0]
+        hist.append(si.k_cache[lo:hi], si.v_cache[lo:hi])
+    rng = np.random.default_rng(77)
+    n, Hq, Hkv = 128, 32, 8
+    out = torch.empty((n, Hq, 128), dtype=torch.bfloat16, device=dev)
+    free0 = cache.free_pages()
+    for step in range(3):
+        qn, kn, vn = (to_bf16(rng.standard_normal(sh, dtype=np.float32)) for sh in ((n, Hq, 128), (n, Hkv, 128), (n, Hkv, 128)))
+        cache.kv_append(ids, [0, n], _torch_of(kn, dev), _torch_of(vn, dev))
+        cache.block_causal_attn_fwd(ids, [0, n], _torch_of(qn, dev), out, w.spec.scale)
+        torch.cuda.synchronize()
+        trial = OracleSession(8, 128)
+        trial.k_slices, trial.v_slices, trial.block_ends = list(hist.k_slices), list(hist.v_slices), list(hist.block_ends)
+        trial.append(kn, vn)
+        o_ref, _ = attend(trial, qn, w.spec.scale)
+        d = out.float().cpu().numpy() - o_ref
+        assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3, step
+        cache.session_truncate(ids[0], base_blocks)                 # roll the noisy block back
+        assert cache.session_info(ids[0])[0] == 1900 and cache.free_pages() == free0
+    # commit the clean block; the history now ends with it, bit for bit
+    cache.kv_append(ids, [0, n], _torch_of(si.k[0], dev), _torch_of(si.v[0], dev))
+    kg = torch.empty((n, Hkv, 128), dtype=torch.bfloat16, device=dev); vg = torch.empty_like(kg)
+    cache.kv_gather(ids[0], 1900, n, kg, vg)
+    torch.cuda.synchronize()
+    assert _numpy_of(kg).tobytes() == np.ascontiguousarray(si.k[0]).tobytes()
+    assert _numpy_of(vg).tobytes() == np.ascontiguousarray(si.v[0]).tobytes()
+    # Euler update of a latent unit (Eq. 2): fp32 and bf16, incl. a ragged tail
+    for dt, cnt in ((torch.float32, 4 * 1000 + 3), (torch.bfloat16, 8 * 777 + 5)):
+        z = torch.randn(cnt + 8, device=dev).to(dt)[:cnt + 8]
+        zz, vv = z[:cnt].clone(), torch.randn(cnt, device=dev).to(dt)
+        want = fm_euler_update(zz.float().cpu().numpy(), vv.float().cpu().numpy(), -0.125)
+        ws_fm_euler_update(zz, vv, -0.125)
+        torch.cuda.synchronize()
+        got = zz.float().cpu().numpy()
+        tol = 1e-6 if dt == torch.float32 else 2.0 ** -8
+        assert np.abs(got - want).max() <= tol * np.maximum(1.0, np.abs(want)).max()
+
+
+def test_next2_solver_step_is_cuda_graph_capturable():
+    """One solver step (append + attention + combine) captured once in a CUDA graph and replayed with
+    new buffer contents (PAPER.md:33, :85 name CUDA-graph capture): single-session metadata travels in
+    kernel parameters, so the captured sequence contains kernels only."""
+    import torch
+    from oracle.block_causal import OracleSession, attend
+    w = _small(3, cache_lens=(2500,), block_tokens=128, modality_split=(96, 24, 8), steps=1)
+    si = w.sessions[0]
+    dev = torch.device("cuda", 0)
+    cache = make_cache(w)
+    ids = preload_gpu(cache, w, [_torch_of(si.k_cache, dev)], [_torch_of(si.v_cache, dev)])
+    base_blocks = cache.session_info(ids[0])[1]
+    n, Hq, Hkv = 128, 32, 8
+    qb = torch.zeros((n, Hq, 128), dtype=torch.bfloat16, device=dev)
+    kb = torch.zeros((n, Hkv, 128), dtype=torch.bfloat16, device=dev); vb = torch.zeros_like(kb)
+    out = torch.zeros_like(qb)
+    # warm-up outside capture, then roll back
+    cache.kv_append(ids, [0, n], kb, vb); cache.block_causal_attn_fwd(ids, [0, n], qb, out, w.spec.scale)
+    cache.session_truncate(ids[0], base_blocks)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        cache.kv_append(ids, [0, n], kb, vb)
+        cache.block_causal_attn_fwd(ids, [0, n], qb, out, w.spec.scale)
+    hist = OracleSession(8, 128)
+    from tests.gpu_harness import preload_rounds
+    for _, rng_ in preload_rounds(w):
+        lo, hi = rng_[0]
+        hist.append(si.k_cache[lo:hi], si.v_cache[lo:hi])
+    rng = np.random.default_rng(78)
+    for step in range(3):
+        qn, kn, vn = (to_bf16(rng.standard_normal(sh, dtype=np.float32)) for sh in ((n, Hq, 128), (n, Hkv, 128), (n, Hkv, 128)))
+        qb.copy_(_torch_of(qn, dev)); kb.copy_(_torch_of(kn, dev)); vb.copy_(_torch_of(vn, dev))
+        g.replay()
+        torch.cuda.synchronize()
+        trial = OracleSession(8, 128)
+        trial.k_slices, trial.v_slices, trial.block_ends = list(hist.k_slices), list(hist.v_slices), list(hist.block_ends)
+        trial.append(kn, vn)
+        o_ref, _ = attend(trial, qn, w.spec.scale)
+        d = out.float().cpu().numpy() - o_ref
+        assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3, step
+
+
 # ------------------------------------------------------------------ closed-form pins on the GPU
 def _run_custom_bf16(L, n, Hq, Hkv, kc, vc, q, kn, vn, scale, min_splits=0):
     """single session, cache (kc, vc) then one block (kn, vn) with queries q; returns (O, LSE)."""

@@ -52,7 +52,7 @@ def test_two_rank_replicas_gloo():
         assert p.exitcode == 0
     (r0, t0, tiles0, ctas0, ms0, tot0), (r1, t1, tiles1, ctas1, ms1, tot1) = res
     assert (t0, t1) == (4096 + 256, 8192 + 256)                    # sessions are rank-private
-    assert tiles0 == 8 * 34 and tiles1 == 8 * 66 and ctas0 == ctas1 == 148
+    assert tiles0 == 8 * 34 and tiles1 == 8 * 66 and 128 <= ctas0 <= 148 and 128 <= ctas1 <= 148
     assert ms0 == ms1 == 20.0                                      # MAX over ranks
     want = 4.0 * 128 * 32 * 256 * (t0 + t1)
     assert tot0 == tot1 == pytest.approx(want)                     # SUM over ranks

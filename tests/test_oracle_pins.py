@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 import torch
 
-from oracle.block_causal import OracleSession, attend, attend_range, merge_partials
+from oracle.block_causal import OracleSession, attend, attend_range, fm_euler_update, merge_partials
 from oracle.brute_force import dense_block_causal
 from synth_inputs import generate, spec_for_config
 
@@ -331,3 +331,17 @@ def test_rows_subset_matches_full():
     o_s, l_s = attend(sess, q, 0.3, num_q_blocks=2, rows=[0, 11, 12, 20], heads=[3, 1])
     np.testing.assert_allclose(o_s, o[[0, 11, 12, 20]][:, [3, 1]], rtol=0, atol=1e-14)
     np.testing.assert_allclose(l_s, l[[0, 11, 12, 20]][:, [3, 1]], rtol=0, atol=1e-14)
+
+
+# ---------------------------------------------------------------- NEXT-2: flow-matching Euler step
+def test_fm_euler_exact_velocity_recovers_clean_latent():
+    """Eq. (2): z_tau = (1-tau) z0 + tau eps, velocity eps - z0.  One Euler step of size
+    -tau with the exact velocity returns z0; a step of +(1-tau) returns eps (closed form)."""
+    rng = np.random.default_rng(51)
+    z0, eps = rng.standard_normal((5, 7)), rng.standard_normal((5, 7))
+    for tau in (1.0, 0.6, 0.25):
+        zt = (1 - tau) * z0 + tau * eps
+        np.testing.assert_allclose(fm_euler_update(zt, eps - z0, -tau), z0, rtol=0, atol=1e-15)
+        np.testing.assert_allclose(fm_euler_update(zt, eps - z0, 1 - tau), eps, rtol=0, atol=1e-15)
+    # hand value: z = 2, v = 4, dtau = -0.25 -> 1
+    assert fm_euler_update(np.array([2.0]), np.array([4.0]), -0.25)[0] == 1.0
