@@ -370,7 +370,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t t_s = tmem_base + (lane_base << 16) + q * 128;
     const uint32_t t_o = tmem_base + (lane_base << 16) + 256 + q * 128;
     const float c = p.scale * 1.4426950408889634f;
-    uint32_t ring_it = 0, tile_it = 0, seg_it = 0;
+    uint32_t tile_it = 0, seg_it = 0;
     bool pdl_done = false;
     PROF_DECL(8)
 
@@ -395,8 +395,6 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 
       for (int32_t j = 0; j < nt; ++j) {
         const int32_t key0 = (sv.tile_begin + j) * kTileKeys;
-        // V(j) ring position: K(j) is 2j, V(j) is 2j+1 within the segment
-        const uint32_t v_it = ring_it + 2 * j + 1;
         PROF_MARK(0)
         mbar_wait(bs_full(q), tile_it & 1);
         tc_fence_after();
@@ -542,23 +540,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #undef S_
           tmem_st32(t_s + 0, pk);
           tmem_st32(t_s + 32, pk + 32);
-          // last tile of the cache with a ragged end: zero the V rows beyond kv_len in smem so that
-          // 0 * (stale bits, possibly NaN) cannot reach O.  Done by warpgroup 0; the PV MMAs of both
-          // Q tiles are issued after p_full[0][0].  (Such a tile always takes this exact path.)
-          if (q == 0 && key0 + kTileKeys > sv.g.kv_len) {
-            const uint32_t slot = v_it % kStages, par = (v_it / kStages) & 1;
-            mbar_wait(bkv_full(slot), par);
-            const int32_t r = (sv.g.kv_len - key0) + row_in_tile;
-            if (r < kTileKeys) {
-              const uint32_t base = sRing + slot * kSlotBytes + r * 128;
-#pragma unroll
-              for (int b = 0; b < 128; b += 16) {
-                asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(base + b), "r"(0u) : "memory");
-                asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(base + kHalfBytes + b), "r"(0u) : "memory");
-              }
-            }
-            fence_proxy_async_smem();
-          }
+          // (keys beyond the cache end in a ragged last tile: P is exactly 0 there and the append
+          // kernel keeps the unused tail of the last page zeroed, so 0 x V stays 0)
           tmem_wait_st();
           tc_fence_before();
           mbar_arrive(bp_full(q, 0));
@@ -567,8 +550,6 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         PROF_MARK(5)
         ++tile_it;
       }
-      ring_it += 2 * nt;
-
       // ---------------------------------------------------- epilogue
       // first global write of this CTA: the predecessor grids (append; transitively the previous
       // step's combine, which reads the partial buffers and writes `out`) must have completed

@@ -57,6 +57,29 @@ kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
     k_pool[dst] = k_new[idx];
     v_pool[dst] = v_new[idx];
   }
+  // Zero the unused tail of each session's last page: slots beyond the committed length are then
+  // always finite (zero), so the attention kernel may load whole pages and rely on P = 0 for the
+  // masked keys (0 x stale NaN bits would poison O).  At most P - 1 token rows per session.
+  {
+    const int4 zero = make_int4(0, 0, 0, 0);
+    for (int32_t s = 0; s < hdr.num_sessions; ++s) {
+      const AppendSession a = sess[s];
+      const int32_t len_new = a.len_old + (a.tok_end - a.tok_begin);
+      const int32_t tail = (P - len_new % P) % P;
+      if (tail == 0) continue;
+      const int32_t page = pages[a.page_off + ((len_new - 1) / P - a.len_old / P)];
+      const int64_t total_tail = (int64_t)tail * chunks_per_token;
+      for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total_tail;
+           idx += (int64_t)gridDim.x * blockDim.x) {
+        int32_t t = (int32_t)(idx / chunks_per_token);
+        int32_t c = (int32_t)(idx - (int64_t)t * chunks_per_token);
+        int32_t head = c / chunks_per_head, off = c - head * chunks_per_head;
+        int64_t dst = (((int64_t)page * Hkv + head) * P + (len_new % P + t)) * chunks_per_head + off;
+        k_pool[dst] = zero;
+        v_pool[dst] = zero;
+      }
+    }
+  }
   // Completing only after the predecessor has completed keeps the dependency chain transitive: the
   // attention kernel's griddepcontrol.wait on this grid then also covers everything before it.
   pdl_wait();
