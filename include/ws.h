@@ -56,7 +56,10 @@ enum {
    * page allocator, scheduler and error paths on a machine without a GPU.  Compute is skipped.     */
   WS_FLAG_DRY_RUN = 1u,
   /* Debug: route bf16 attention through the generic SIMT kernel instead of the tcgen05 kernel.     */
-  WS_FLAG_FORCE_SIMT = 2u
+  WS_FLAG_FORCE_SIMT = 2u,
+  /* Run the tcgen05 kernel on CTA pairs (cta_group::2, M = 256 per MMA, each CTA stages half of every
+   * K/V tile) when the plan's team size is even.  Correct but slower on B200. */
+  WS_FLAG_CTA_PAIRS = 4u
 };
 
 typedef struct ws_cache ws_cache_t;   /* opaque; owns host metadata only */
@@ -167,7 +170,7 @@ ws_status_t ws_debug_set_min_splits(ws_cache_t* cache, int32_t min_splits);
 
 /* Description of the last attention plan built on this cache (a1): CTAs launched, team size,
  * number of (session,KV-head) groups, KV segments, split partial slots, combine items, and whether
- * the tcgen05 kernel (1) or the generic SIMT kernel (0) was selected. */
+ * the tcgen05 kernel (1; 2 = on CTA pairs) or the generic SIMT kernel (0) was selected. */
 typedef struct {
   int32_t num_ctas, team_size, num_groups, num_segments, num_partial_slots, num_combine_items;
   int32_t used_tensor_core_kernel, total_kv_tiles;

@@ -121,6 +121,7 @@ struct ws_cache {
   int64_t launches = 0;
   ws::Plan last_plan;
   bool last_tensor = false;
+  int32_t last_cta_group = 1;
   // optional per-kernel timing (bench): event pairs around each launch on the launch stream
   bool timing = false;
   std::vector<cudaEvent_t> ev_pool;                       // reusable events
@@ -557,6 +558,11 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     if (st != WS_OK) return st;
   }
   L.num_ctas = c->last_plan.num_teams * c->last_plan.team_size;
+  // CTA pairs (tcgen05 cta_group::2) halve the shared-memory operand traffic but put two DSMEM
+  // round trips (remote P arrival, multicast S commit) on the S -> softmax -> PV chain that bounds
+  // this kernel: measured 309 us vs 224 us per config-4 unit.  Opt-in only.
+  L.cta_group = ((c->cfg.flags & WS_FLAG_CTA_PAIRS) && c->last_plan.team_size % 2 == 0) ? 2 : 1;
+  c->last_cta_group = L.cta_group;
   TimedLaunch tl(c, &c->t_attn, stream);
   WS_CUDA(ws::launch_attn_sm100(L, stream));
   tl.done();
@@ -644,7 +650,7 @@ ws_status_t ws_last_plan_info(const ws_cache_t* c, ws_plan_info_t* out) {
   out->num_segments = (int32_t)p.segments.size();
   out->num_partial_slots = p.num_part_slots;
   out->num_combine_items = (int32_t)p.combine.size();
-  out->used_tensor_core_kernel = c->last_tensor ? 1 : 0;
+  out->used_tensor_core_kernel = c->last_tensor ? c->last_cta_group : 0;
   out->total_kv_tiles = p.total_tiles;
   return WS_OK;
 }

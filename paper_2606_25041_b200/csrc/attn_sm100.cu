@@ -43,9 +43,16 @@ namespace ws {
 
 using namespace ptx;
 
-constexpr int kStages = 5;
-constexpr uint32_t kSlotBytes = kTileKeys * 128 * 2;       // one K or V tile: 128 keys x 128 dims bf16
-constexpr uint32_t kHalfBytes = kSlotBytes / 2;            // one 64-dim half: 128 rows x 128 B
+// kCG = 1: one CTA owns whole K/V tiles (32 KB slots, 5-slot ring).
+// kCG = 2: a CTA pair (cluster of 2, adjacent row-tile pairs of one team) runs M = 256 MMAs
+// (tcgen05 cta_group::2): each CTA stages only HALF of every K tile (64 keys) and V tile (64 dims),
+// halving shared-memory operand reads, TMA writes and L2 requests per FLOP (16 KB slots, 10-slot ring).
+template <int kCG> struct RingCfg;
+template <> struct RingCfg<1> { static constexpr int kStages = 5; static constexpr uint32_t kSlotBytes = 32768; };
+template <> struct RingCfg<2> { static constexpr int kStages = 10; static constexpr uint32_t kSlotBytes = 16384; };
+constexpr int kMaxStages = 10;
+constexpr uint32_t kRingBytes = 5 * 32768;                 // same footprint in both modes
+constexpr uint32_t kHalfBytes = 16384;                     // one 64-dim half of a 128-row tile: 128 rows x 128 B
 constexpr uint32_t kQTileBytes = kTileRows * 128 * 2;
 constexpr int kThreads = 384;
 constexpr uint32_t kTmemCols = 512;
@@ -68,12 +75,12 @@ constexpr float kFastSumLimit = 1024.0f;                   // fast path accepted
 
 struct Barriers {
   uint64_t q_full, q_empty;
-  uint64_t kv_full[kStages], kv_empty[kStages];
+  uint64_t kv_full[kMaxStages], kv_empty[kMaxStages];
   uint64_t s_full[2], p_full[2][2], pv_h0_done[2], o_full[2], o_empty[2];
   uint32_t tmem_base;
   uint32_t pad;
 };
-constexpr uint32_t kSmemBytes = 2 * kQTileBytes + kStages * kSlotBytes + sizeof(Barriers) + 1024;
+constexpr uint32_t kSmemBytes = 2 * kQTileBytes + kRingBytes + sizeof(Barriers) + 1024;
 
 struct SegView {
   Group g;
@@ -84,12 +91,15 @@ struct SegView {
 // (pair >= npairs).  For multi-block queries the pair's own visible end clips the tile range: KV
 // tiles beyond the last key any of the pair's rows can see are skipped (block-lower-triangular
 // skipping at pair granularity); `v.tile_end <= v.tile_begin` then means "nothing to compute here".
+template <int kClipPairMask>
 __device__ __forceinline__ bool load_segment(const int32_t* meta, const AttnMeta& hdr, int32_t si,
                                              int32_t pair, int32_t tok_per_pair, SegView& v) {
+  // `pair` is the LAST row-tile pair handled by this CTA group (the CTA's own pair for kCG = 1, the
+  // odd pair of the cluster for kCG = 2): both CTAs of a pair must walk the same tile range.
   const Segment s = reinterpret_cast<const Segment*>(meta + hdr.off_segments)[si];
   v.g = reinterpret_cast<const Group*>(meta + hdr.off_groups)[s.group];
   v.tile_begin = s.tile_begin; v.tile_end = s.tile_end; v.part_base = s.part_base;
-  if (pair >= v.g.npairs) return false;
+  if ((pair & ~(int32_t)(kClipPairMask)) >= v.g.npairs) return false;
   if (v.g.vis_off >= 0) {
     const int32_t last_tok = min(v.g.q_token_end, v.g.q_token0 + (pair + 1) * tok_per_pair) - 1;
     const int32_t pair_kv = (meta + hdr.off_vis)[v.g.vis_off + (last_tok - v.g.q_token0)];
@@ -150,6 +160,7 @@ __device__ __forceinline__ void softmax_chunk(const uint32_t* sr, float c, float
   }
 }
 
+template <int kCG>
 __global__ void __launch_bounds__(kThreads, 1)
 attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ CUtensorMap tmap_k,
@@ -160,9 +171,15 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem_base;                           // 2 x 32 KB
-  const uint32_t sRing = smem_base + 2 * kQTileBytes;      // kStages x 32 KB
+  constexpr int kStages = RingCfg<kCG>::kStages;
+  constexpr uint32_t kSlotBytes = RingCfg<kCG>::kSlotBytes;
+  const uint32_t sRing = smem_base + 2 * kQTileBytes;      // kStages x kSlotBytes
   Barriers* bars = reinterpret_cast<Barriers*>(smem_raw + (smem_base - smem_u32(smem_raw)) +
-                                               2 * kQTileBytes + kStages * kSlotBytes);
+                                               2 * kQTileBytes + kRingBytes);
+  // kCG = 2: rank of this CTA in its pair; the even CTA (leader) issues every MMA and owns the
+  // barriers that collect contributions of both CTAs (q_full, kv_full, p_full, o_empty)
+  const uint32_t cta_rank = kCG == 2 ? cluster_ctarank() : 0u;
+  const bool is_leader = cta_rank == 0;
   const uint32_t bq_full = smem_u32(&bars->q_full), bq_empty = smem_u32(&bars->q_empty);
   auto bkv_full = [&](int s) { return smem_u32(&bars->kv_full[s]); };
   auto bkv_empty = [&](int s) { return smem_u32(&bars->kv_empty[s]); };
@@ -177,6 +194,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   const AttnMeta hdr = *reinterpret_cast<const AttnMeta*>(p.meta);
   const int32_t team = blockIdx.x / hdr.team_size;
   const int32_t pair = blockIdx.x - team * hdr.team_size;
+  const int32_t clip_pair = kCG == 2 ? (pair | 1) : pair;  // see load_segment
   const int32_t* tsb = p.meta + hdr.off_team_seg_begin;
   const int32_t seg_lo = tsb[team], seg_hi = tsb[team + 1];
   const int32_t tok_per_pair = kPairRows / p.G;
@@ -193,18 +211,18 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     mbar_init(bq_full, 1); mbar_init(bq_empty, 1);
     for (int s = 0; s < kStages; ++s) { mbar_init(bkv_full(s), 1); mbar_init(bkv_empty(s), 1); }
     for (int q = 0; q < 2; ++q) {
-      mbar_init(bs_full(q), 1); mbar_init(bp_full(q, 0), 128); mbar_init(bp_full(q, 1), 128);
+      mbar_init(bs_full(q), 1); mbar_init(bp_full(q, 0), 128 * kCG); mbar_init(bp_full(q, 1), 128 * kCG);
       mbar_init(bpv_h0(q), 1);
-      mbar_init(bo_full(q), 1); mbar_init(bo_empty(q), 128);
+      mbar_init(bo_full(q), 1); mbar_init(bo_empty(q), 128 * kCG);
     }
     fence_mbar_init();
   }
   if (warp == 10) {
-    tmem_alloc<kTmemCols>(smem_u32(&bars->tmem_base));
-    tmem_relinquish();
+    if constexpr (kCG == 2) { tmem_alloc_2cta<kTmemCols>(smem_u32(&bars->tmem_base)); tmem_relinquish_2cta(); }
+    else { tmem_alloc<kTmemCols>(smem_u32(&bars->tmem_base)); tmem_relinquish(); }
   }
   tc_fence_before();
-  __syncthreads();
+  if constexpr (kCG == 2) cluster_sync_all(); else __syncthreads();   // peer barriers are initialised too
   tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
 
@@ -216,7 +234,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       bool dep_waited = false;
       for (int32_t si = seg_lo; si < seg_hi; ++si) {
         SegView sv;
-        if (!load_segment(p.meta, hdr, si, pair, tok_per_pair, sv)) continue;
+        if (!load_segment<kCG - 1>(p.meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
         if (sv.tile_end <= sv.tile_begin) continue;          // clipped away for this pair
         const int32_t* page_row = p.page_table + (int64_t)sv.g.slot * p.max_pages_per_session;
         const int32_t last_page = (sv.g.kv_len - 1) / p.P;
@@ -224,14 +242,19 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         if (!dep_waited && sv.tile_begin + 1 >= sv.g.dep_tile) { pdl_wait(); dep_waited = true; }
         int32_t pg0 = page_row[min(2 * sv.tile_begin, last_page)];
         int32_t pg1 = page_row[min(2 * sv.tile_begin + 1, last_page)];
-        // Q pair
+        // Q pair (own rows).  kCG = 2: the bytes of both CTAs are credited to the leader's q_full.
         mbar_wait(bq_empty, (q_it & 1) ^ 1);
-        mbar_arrive_expect_tx(bq_full, 2 * kQTileBytes);
+        if (is_leader) mbar_arrive_expect_tx(bq_full, kCG * 2 * kQTileBytes);
         const int32_t tok0 = sv.g.q_token0 + pair * tok_per_pair;
         for (int q = 0; q < 2; ++q)
-          for (int h = 0; h < 2; ++h)
-            tma_load_3d(sQ + q * kQTileBytes + h * kHalfBytes, &tmap_q, bq_full, h * 64,
-                        sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
+          for (int h = 0; h < 2; ++h) {
+            if constexpr (kCG == 2)
+              tma_load_3d_2cta(sQ + q * kQTileBytes + h * kHalfBytes, &tmap_q, bq_full, h * 64,
+                               sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
+            else
+              tma_load_3d(sQ + q * kQTileBytes + h * kHalfBytes, &tmap_q, bq_full, h * 64,
+                          sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
+          }
         ++q_it;
         for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
           const int32_t c0 = pg0, c1 = pg1;
@@ -245,24 +268,38 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
             const CUtensorMap* tm = kv == 0 ? &tmap_k : &tmap_v;
             mbar_wait(bkv_empty(slot), par ^ 1);
-            mbar_arrive_expect_tx(bkv_full(slot), kSlotBytes);
+            if (is_leader) mbar_arrive_expect_tx(bkv_full(slot), 32768);   // whole tile (both CTAs)
             const uint32_t dst = sRing + slot * kSlotBytes;
-            tma_load_4d(dst, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c0);
-            tma_load_4d(dst + kHalfBytes / 2, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c1);
-            tma_load_4d(dst + kHalfBytes, tm, bkv_full(slot), 64, 0, sv.g.kv_head, c0);
-            tma_load_4d(dst + kHalfBytes + kHalfBytes / 2, tm, bkv_full(slot), 64, 0,
-                        sv.g.kv_head, c1);
+            if constexpr (kCG == 2) {
+              if (kv == 0) {
+                // K: this CTA's 64 keys (page `cta_rank` of the tile), both 64-dim halves
+                const int32_t pg = cta_rank ? c1 : c0;
+                tma_load_4d_2cta(dst, tm, bkv_full(slot), 0, 0, sv.g.kv_head, pg);
+                tma_load_4d_2cta(dst + 8192, tm, bkv_full(slot), 64, 0, sv.g.kv_head, pg);
+              } else {
+                // V: all 128 keys, this CTA's 64 dims
+                tma_load_4d_2cta(dst, tm, bkv_full(slot), 64 * (int32_t)cta_rank, 0, sv.g.kv_head, c0);
+                tma_load_4d_2cta(dst + 8192, tm, bkv_full(slot), 64 * (int32_t)cta_rank, 0, sv.g.kv_head, c1);
+              }
+            } else {
+              tma_load_4d(dst, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c0);
+              tma_load_4d(dst + kHalfBytes / 2, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c1);
+              tma_load_4d(dst + kHalfBytes, tm, bkv_full(slot), 64, 0, sv.g.kv_head, c0);
+              tma_load_4d(dst + kHalfBytes + kHalfBytes / 2, tm, bkv_full(slot), 64, 0,
+                          sv.g.kv_head, c1);
+            }
             ++ring_it;
           }
         }
       }
-    } else if (warp == 9) {
-      // ===================================================== MMA issuer
+    } else if (warp == 9 && is_leader) {
+      // ===================================================== MMA issuer (kCG = 2: the even CTA only)
       // The whole warp runs the control flow convergently (all values stay warp-uniform, so the
       // descriptors are built on the uniform datapath); one elected lane issues tcgen05.mma/commit.
       const bool leader = elect_one();
-      constexpr uint32_t idesc_qk = make_idesc_bf16(128, 128, 0, 0);
-      constexpr uint32_t idesc_pv = make_idesc_bf16(128, 128, 0, 1);
+      constexpr uint32_t idesc_qk = make_idesc_bf16(128 * kCG, 128, 0, 0);
+      constexpr uint32_t idesc_pv = make_idesc_bf16(128 * kCG, 128, 0, 1);
+      auto commit = [&](uint32_t bar) { if constexpr (kCG == 2) mma_commit_2cta(bar); else mma_commit(bar); };
       const uint64_t desc_k = make_smem_desc_sw128(0, 16, 1024);          // K-major operands (Q, K)
       const uint64_t desc_v = make_smem_desc_sw128(0, kHalfBytes, 1024);  // MN-major operand (V)
       uint32_t ring_it = 0, q_it = 0, tile_it = 0, seg_it = 0;
@@ -272,8 +309,10 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         const uint64_t db = desc_k + ((sRing + slot * kSlotBytes) >> 4);
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {
-          const uint32_t off = ((ks >> 2) * kHalfBytes + (ks & 3) * 32) >> 4;
-          mma_ss(tmem_base + q * 128, da + off, db + off, idesc_qk, ks > 0);
+          const uint32_t offa = ((ks >> 2) * kHalfBytes + (ks & 3) * 32) >> 4;
+          const uint32_t offb = ((ks >> 2) * (kHalfBytes / kCG) + (ks & 3) * 32) >> 4;   // kCG = 2: 64-key halves
+          if constexpr (kCG == 2) mma_ss_2cta(tmem_base + q * 128, da + offa, db + offb, idesc_qk, ks > 0);
+          else mma_ss(tmem_base + q * 128, da + offa, db + offb, idesc_qk, ks > 0);
         }
       };
       // PV for one half of the tile's keys (k-steps 4*half .. 4*half+3)
@@ -282,13 +321,17 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #pragma unroll
         for (int k4 = 0; k4 < 4; ++k4) {
           const int ks = half * 4 + k4;
-          mma_ts(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8, db + ks * (2048 >> 4),
-                 idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
+          if constexpr (kCG == 2)
+            mma_ts_2cta(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8, db + ks * (2048 >> 4),
+                        idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
+          else
+            mma_ts(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8, db + ks * (2048 >> 4),
+                   idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
         }
       };
       for (int32_t si = seg_lo; si < seg_hi; ++si) {
         SegView sv;
-        if (!load_segment(p.meta, hdr, si, pair, tok_per_pair, sv)) continue;
+        if (!load_segment<kCG - 1>(p.meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
         if (sv.tile_end <= sv.tile_begin) continue;          // clipped away for this pair
         const int32_t nt = sv.tile_end - sv.tile_begin;
         mbar_wait(bq_full, q_it & 1);
@@ -297,10 +340,10 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           mbar_wait(bkv_full(slot), par);
           tc_fence_after();
           if (leader) {
-            issue_S(0, slot); mma_commit(bs_full(0));
-            issue_S(1, slot); mma_commit(bs_full(1));
-            mma_commit(bkv_empty(slot));
-            if (nt == 1) mma_commit(bq_empty);
+            issue_S(0, slot); commit(bs_full(0));
+            issue_S(1, slot); commit(bs_full(1));
+            commit(bkv_empty(slot));
+            if (nt == 1) commit(bq_empty);
           }
           __syncwarp();
           ++ring_it;
@@ -322,14 +365,14 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             tc_fence_after();
             if (leader) {
               issue_PV(q, slot_v, 0, j > 0);
-              mma_commit(bpv_h0(q));
+              commit(bpv_h0(q));
             }
             __syncwarp();
             mbar_wait(bp_full(q, 1), tile_it & 1);
             tc_fence_after();
             if (leader) {
               issue_PV(q, slot_v, 1, true);
-              if (!have_next) mma_commit(bo_full(q));
+              if (!have_next) commit(bo_full(q));
             }
             __syncwarp();
             PROF_MARK(5)
@@ -338,17 +381,17 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
               PROF_MARK(4)
               if (leader) {
                 issue_S(q, slot_k);
-                mma_commit(bs_full(q));
+                commit(bs_full(q));
               }
               __syncwarp();
               PROF_MARK(6)
             }
           }
           if (leader) {
-            mma_commit(bkv_empty(slot_v));
+            commit(bkv_empty(slot_v));
             if (have_next) {
-              mma_commit(bkv_empty(slot_k));
-              if (j + 2 == nt) mma_commit(bq_empty);
+              commit(bkv_empty(slot_k));
+              if (j + 2 == nt) commit(bq_empty);
             }
           }
           __syncwarp();
@@ -370,16 +413,20 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t t_s = tmem_base + (lane_base << 16) + q * 128;
     const uint32_t t_o = tmem_base + (lane_base << 16) + 256 + q * 128;
     const float c = p.scale * 1.4426950408889634f;
+    // p_full / o_empty live in the leader CTA (kCG = 2): arrive through the cluster address
+    auto arrive_leader = [&](uint32_t bar) {
+      if constexpr (kCG == 2) mbar_arrive_cluster(bar & kPeerBitMask); else mbar_arrive(bar);
+    };
     uint32_t tile_it = 0, seg_it = 0;
     bool pdl_done = false;
     PROF_DECL(8)
 
     for (int32_t si = seg_lo; si < seg_hi; ++si) {
       SegView sv;
-      if (!load_segment(p.meta, hdr, si, pair, tok_per_pair, sv)) continue;
+      if (!load_segment<kCG - 1>(p.meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
       const int32_t nt = sv.tile_end - sv.tile_begin;
       const int32_t tok = sv.g.q_token0 + pair * tok_per_pair + R / p.G;
-      const bool row_valid = tok < sv.g.q_token_end;
+      const bool row_valid = tok < sv.g.q_token_end && pair < sv.g.npairs;   // (kCG = 2: a ghost CTA computes but stores nothing)
       if (nt <= 0) {
         // every tile of this segment lies beyond what the pair can see: publish an empty partial
         // (the segment is one of several splits, otherwise it would start at tile 0)
@@ -426,7 +473,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             tmem_st32(t_s + 0, pk);
             tmem_wait_st();
             tc_fence_before();
-            mbar_arrive(bp_full(q, 0));                     // first 64 keys of P handed off
+            arrive_leader(bp_full(q, 0));                     // first 64 keys of P handed off
             tmem_wait_ld();
             tmem_ld32(t_s + 96, sb);
             l01 = 0; l23 = 0;
@@ -477,7 +524,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             tmem_st32(t_s + 32, pk + 32);
             tmem_wait_st();
             tc_fence_before();
-            mbar_arrive(bp_full(q, 1));
+            arrive_leader(bp_full(q, 1));
             done = true;
           }
         }
@@ -544,8 +591,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           // kernel keeps the unused tail of the last page zeroed, so 0 x V stays 0)
           tmem_wait_st();
           tc_fence_before();
-          mbar_arrive(bp_full(q, 0));
-          mbar_arrive(bp_full(q, 1));
+          arrive_leader(bp_full(q, 0));
+          arrive_leader(bp_full(q, 1));
         }
         PROF_MARK(5)
         ++tile_it;
@@ -598,7 +645,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         if (row_valid) p.part_lse[prow] = lse2;
       }
       tc_fence_before();
-      mbar_arrive(bo_empty(q));
+      arrive_leader(bo_empty(q));
       PROF_MARK(6)
       ++seg_it;
     }
@@ -610,7 +657,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   __syncwarp();
   pdl_launch_dependents();
   tc_fence_before();
-  __syncthreads();
+  if constexpr (kCG == 2) cluster_sync_all(); else __syncthreads();   // the leader's MMAs read the peer's smem / TMEM
 #ifdef WS_PROFILE
   if (threadIdx.x == 0) {
     unsigned long long g1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(g1));
@@ -621,18 +668,39 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #endif
   if (warp == 10) {
     tc_fence_after();
-    tmem_dealloc<kTmemCols>(tmem_base);
+    if constexpr (kCG == 2) tmem_dealloc_2cta<kTmemCols>(tmem_base); else tmem_dealloc<kTmemCols>(tmem_base);
   }
 }
 
 cudaError_t sm100_attn_configure() {
-  return cudaFuncSetAttribute(attn_sm100_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  cudaError_t e = cudaFuncSetAttribute(attn_sm100_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)kSmemBytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(attn_sm100_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               (int)kSmemBytes);
 }
 
 cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream) {
-  return launch_pdl(attn_sm100_kernel, dim3(l.num_ctas), dim3(kThreads), kSmemBytes, stream, l.tmap_q,
-                    l.tmap_k, l.tmap_v, l.inl, l.p);
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(l.num_ctas); cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = kSmemBytes; cfg.stream = stream;
+  cudaLaunchAttribute at[2];
+  int na = 0;
+  static const bool no_pdl = getenv("WS_NO_PDL") != nullptr;
+  if (!no_pdl) {
+    at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[na].val.programmaticStreamSerializationAllowed = 1;
+    ++na;
+  }
+  if (l.cta_group == 2) {
+    at[na].id = cudaLaunchAttributeClusterDimension;
+    at[na].val.clusterDim.x = 2; at[na].val.clusterDim.y = 1; at[na].val.clusterDim.z = 1;
+    ++na;
+    cfg.attrs = at; cfg.numAttrs = na;
+    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<2>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
+  }
+  cfg.attrs = at; cfg.numAttrs = na;
+  return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
 }
 
 }  // namespace ws

@@ -60,6 +60,7 @@ struct Sm100Launch {
   CUtensorMap tmap_q, tmap_k, tmap_v;
   InlineAttnMeta inl;
   int32_t num_ctas;
+  int32_t cta_group;                 // 1, or 2 (CTA pairs; needs an even team size)
 };
 cudaError_t sm100_attn_configure();    // one-time cudaFuncSetAttribute
 cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream);

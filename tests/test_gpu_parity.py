@@ -175,6 +175,27 @@ def test_bf16_tensor_core_kernel_small(label, ov):
     _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, label)
 
 
+@pytest.mark.parametrize("label,ov", [x for x in SMALL_TC if x[0] in ("gqa4_ragged_tail", "gqa8_tail_le_64", "mha_aligned")],
+                         ids=["gqa4_ragged_tail", "gqa8_tail_le_64", "mha_aligned"])
+def test_bf16_cta_pair_variant(label, ov):
+    """WS_FLAG_CTA_PAIRS: the same kernel on 2-CTA clusters (tcgen05 cta_group::2, each CTA stages half
+    of every K/V tile, cross-CTA barriers).  Opt-in; must match the oracle like the default path."""
+    from paper_2606_25041_b200 import WS_FLAG_CTA_PAIRS
+    w = _small(2, **ov)
+    got = run_workload_gpu(w, flags=WS_FLAG_CTA_PAIRS, pool_fill=0x7FC1)
+    even_team = got["plans"][-1]["team_size"] % 2 == 0
+    assert got["plans"][-1]["used_tensor_core_kernel"] == (2 if even_team else 1)
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, label + " (cta pairs)")
+
+
+def test_cta_pair_variant_config3_shape():
+    from paper_2606_25041_b200 import WS_FLAG_CTA_PAIRS
+    w = _small(3, cache_lens=(5000,), block_tokens=512)
+    got = run_workload_gpu(w, flags=WS_FLAG_CTA_PAIRS, min_splits=2)
+    assert got["plans"][-1]["used_tensor_core_kernel"] == 2 and got["plans"][-1]["team_size"] == 8
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "cfg3-like cta pairs")
+
+
 @pytest.mark.parametrize("splits", [1, 2, 3, 7])
 def test_split_count_invariance(splits):
     w = _small(3, cache_lens=(3000,), block_tokens=128, modality_split=(96, 24, 8))
