@@ -134,14 +134,19 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* cache, int32_t num_sessions,
                                      float* lse, float scale, void* cuda_stream);
 
 /* One streaming-unit step with HOST buffers (the end-to-end path): copies q/k_new/v_new from host
- * (pinned for async copies) into `staging` (DEVICE, >= ws_step_staging_bytes(n_total)), runs
- * ws_kv_append then ws_block_causal_attn_fwd (one block per session, n_q = n_new), and copies the
- * result back to out_host.  Returns after enqueueing; the caller synchronises the stream. */
+ * (pinned for async copies) into `staging` (DEVICE, >= ws_step_staging_bytes(n_total); two slots used
+ * alternately), runs ws_kv_append then ws_block_causal_attn_fwd (one block per session, n_q = n_new)
+ * on `cuda_stream`, and copies the result back to out_host.  Copy-in and copy-out run on two internal
+ * streams ordered by events, so consecutive steps overlap their copies with each other's kernels.
+ * Returns after enqueueing.  out_host (and the host input buffers) may be touched again once
+ * ws_stream_host_join(cache, stream) has been called and `stream` has been synchronised. */
 size_t ws_step_staging_bytes(const ws_cache_config_t* cfg, int32_t total_new_tokens);
 ws_status_t ws_stream_step_host(ws_cache_t* cache, int32_t num_sessions, const int32_t* session_ids,
                                 const int32_t* cu_new_tokens, const void* q_host,
                                 const void* k_new_host, const void* v_new_host, void* out_host,
                                 void* staging, size_t staging_bytes, float scale, void* cuda_stream);
+/* Makes `cuda_stream` wait for every copy-out issued by ws_stream_step_host on this cache so far. */
+ws_status_t ws_stream_host_join(ws_cache_t* cache, void* cuda_stream);
 
 /* NEXT-2 (solver-step mode): explicit Euler step of the flow-matching solver on a
  * latent unit, z <- z + dtau * v  (Eq. (2): dz/dtau = eps - z_0 is the velocity the model

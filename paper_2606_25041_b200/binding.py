@@ -54,7 +54,7 @@ class PlanSegment(C.Structure):
 EXPORTS = ["ws_pool_bytes", "ws_workspace_bytes", "ws_cache_create", "ws_cache_destroy",
            "ws_session_open", "ws_session_close", "ws_session_info", "ws_session_truncate",
            "ws_free_pages", "ws_kv_append", "ws_block_causal_attn_fwd", "ws_step_staging_bytes",
-           "ws_stream_step_host", "ws_fm_euler_update", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
+           "ws_stream_step_host", "ws_stream_host_join", "ws_fm_euler_update", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
            "ws_debug_set_min_splits", "ws_last_plan_info", "ws_last_plan_segment",
            "ws_launch_count", "ws_debug_kernel_timing", "ws_debug_read_kernel_times",
            "ws_status_str", "ws_last_error", "ws_version"]
@@ -90,6 +90,7 @@ def load_library() -> C.CDLL:
     lib.ws_step_staging_bytes.argtypes = [cfgp, C.c_int32]
     lib.ws_stream_step_host.argtypes = [vp, C.c_int32, i32p, i32p, vp, vp, vp, vp, vp, C.c_size_t,
                                         C.c_float, vp]
+    lib.ws_stream_host_join.argtypes = [vp, vp]
     lib.ws_fm_euler_update.argtypes = [C.c_int32, vp, vp, C.c_float, C.c_int64, vp]
     lib.ws_kv_gather.argtypes = [vp, C.c_int32, C.c_int64, C.c_int64, vp, vp, vp]
     lib.ws_session_pages.argtypes = [vp, C.c_int32, i32p, C.c_int32, i32p]
@@ -247,6 +248,9 @@ class Cache:
                                             _ptr(v_host), _ptr(out_host), _ptr(staging),
                                             staging.numel() * staging.element_size(),
                                             C.c_float(scale), _stream_ptr(stream)))
+
+    def stream_host_join(self, stream=None):
+        _check(self.lib.ws_stream_host_join(self.handle, _stream_ptr(stream)))
 
     def kv_gather(self, session: int, start: int, count: int, k_out, v_out, stream=None):
         _check(self.lib.ws_kv_gather(self.handle, session, start, count, _ptr(k_out), _ptr(v_out),

@@ -122,6 +122,11 @@ struct ws_cache {
   ws::Plan last_plan;
   bool last_tensor = false;
   int32_t last_cta_group = 1;
+  // ws_stream_step_host pipeline: copy streams + per-slot events (2 staging slots)
+  cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
+  cudaEvent_t ev_h2d[2]{}, ev_compute[2]{}, ev_d2h[2]{};
+  bool slot_used[2]{};
+  int64_t host_steps = 0;
   // optional per-kernel timing (bench): event pairs around each launch on the launch stream
   bool timing = false;
   std::vector<cudaEvent_t> ev_pool;                       // reusable events
@@ -303,6 +308,12 @@ ws_status_t ws_cache_destroy(ws_cache_t* c) {
     for (auto* lst : {&c->t_append, &c->t_attn, &c->t_combine})
       for (auto& pr : *lst) { (void)cudaEventDestroy(pr.first); (void)cudaEventDestroy(pr.second); }
     for (cudaEvent_t e : c->ev_pool) (void)cudaEventDestroy(e);
+    if (c->h2d_stream) {
+      for (int i = 0; i < 2; ++i) {
+        (void)cudaEventDestroy(c->ev_h2d[i]); (void)cudaEventDestroy(c->ev_compute[i]); (void)cudaEventDestroy(c->ev_d2h[i]);
+      }
+      (void)cudaStreamDestroy(c->h2d_stream); (void)cudaStreamDestroy(c->d2h_stream);
+    }
     if (c->h_meta) (void)cudaFreeHost(c->h_meta);
   }
   delete c;
@@ -582,7 +593,7 @@ size_t ws_step_staging_bytes(const ws_cache_config_t* cfg, int32_t n) {
   size_t eb = eb_of(cfg->dtype), D = cfg->head_dim;
   size_t qb = align_up((size_t)n * cfg->num_q_heads * D * eb, 256);
   size_t kb = align_up((size_t)n * cfg->num_kv_heads * D * eb, 256);
-  return 2 * qb + 2 * kb;
+  return 2 * (2 * qb + 2 * kb);          // two slots of {q, out, k_new, v_new}
 }
 
 ws_status_t ws_stream_step_host(ws_cache_t* c, int32_t S, const int32_t* session_ids,
@@ -597,20 +608,48 @@ ws_status_t ws_stream_step_host(ws_cache_t* c, int32_t S, const int32_t* session
   if (staging_bytes < ws_step_staging_bytes(&c->cfg, n))
     return fail(WS_ERR_WORKSPACE_TOO_SMALL, "staging_bytes %zu < required %zu", staging_bytes,
                 ws_step_staging_bytes(&c->cfg, n));
+  if (!c->h2d_stream) {
+    WS_CUDA(cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking));
+    WS_CUDA(cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+      WS_CUDA(cudaEventCreateWithFlags(&c->ev_h2d[i], cudaEventDisableTiming));
+      WS_CUDA(cudaEventCreateWithFlags(&c->ev_compute[i], cudaEventDisableTiming));
+      WS_CUDA(cudaEventCreateWithFlags(&c->ev_d2h[i], cudaEventDisableTiming));
+    }
+  }
   size_t eb = eb_of(c->cfg.dtype), D = c->cfg.head_dim;
   size_t q_bytes = (size_t)n * c->cfg.num_q_heads * D * eb, kv_bytes = (size_t)n * c->cfg.num_kv_heads * D * eb;
   size_t qb = align_up(q_bytes, 256), kb = align_up(kv_bytes, 256);
-  char* base = (char*)staging;
+  const int slot = (int)(c->host_steps & 1);
+  char* base = (char*)staging + (size_t)slot * (2 * qb + 2 * kb);
   char *dq = base, *dout = base + qb, *dk = base + 2 * qb, *dv = base + 2 * qb + kb;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
-  WS_CUDA(cudaMemcpyAsync(dk, k_host, kv_bytes, cudaMemcpyHostToDevice, stream));
-  WS_CUDA(cudaMemcpyAsync(dv, v_host, kv_bytes, cudaMemcpyHostToDevice, stream));
-  WS_CUDA(cudaMemcpyAsync(dq, q_host, q_bytes, cudaMemcpyHostToDevice, stream));
+  // copy-in on the H2D stream (after the slot's previous result has left the device), compute on the
+  // caller's stream, copy-out on the D2H stream: step t's copies overlap step t-1 / t+1's kernels
+  if (c->slot_used[slot]) WS_CUDA(cudaStreamWaitEvent(c->h2d_stream, c->ev_d2h[slot], 0));
+  WS_CUDA(cudaMemcpyAsync(dk, k_host, kv_bytes, cudaMemcpyHostToDevice, c->h2d_stream));
+  WS_CUDA(cudaMemcpyAsync(dv, v_host, kv_bytes, cudaMemcpyHostToDevice, c->h2d_stream));
+  WS_CUDA(cudaMemcpyAsync(dq, q_host, q_bytes, cudaMemcpyHostToDevice, c->h2d_stream));
+  WS_CUDA(cudaEventRecord(c->ev_h2d[slot], c->h2d_stream));
+  WS_CUDA(cudaStreamWaitEvent(stream, c->ev_h2d[slot], 0));
   ws_status_t st = ws_kv_append(c, S, session_ids, cu, dk, dv, nullptr, cuda_stream);
   if (st != WS_OK) return st;
   st = ws_block_causal_attn_fwd(c, S, session_ids, nullptr, cu, dq, dout, nullptr, scale, cuda_stream);
   if (st != WS_OK) return st;
-  WS_CUDA(cudaMemcpyAsync(out_host, dout, q_bytes, cudaMemcpyDeviceToHost, stream));
+  WS_CUDA(cudaEventRecord(c->ev_compute[slot], stream));
+  WS_CUDA(cudaStreamWaitEvent(c->d2h_stream, c->ev_compute[slot], 0));
+  WS_CUDA(cudaMemcpyAsync(out_host, dout, q_bytes, cudaMemcpyDeviceToHost, c->d2h_stream));
+  WS_CUDA(cudaEventRecord(c->ev_d2h[slot], c->d2h_stream));
+  c->slot_used[slot] = true;
+  c->host_steps += 1;
+  return WS_OK;
+}
+
+ws_status_t ws_stream_host_join(ws_cache_t* c, void* cuda_stream) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  if (c->dry) return WS_OK;
+  for (int i = 0; i < 2; ++i)
+    if (c->slot_used[i]) WS_CUDA(cudaStreamWaitEvent((cudaStream_t)cuda_stream, c->ev_d2h[i], 0));
   return WS_OK;
 }
 

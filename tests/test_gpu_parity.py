@@ -620,6 +620,7 @@ def test_stream_step_host_end_to_end():
     oh = torch.empty_like(qh).pin_memory()
     staging = torch.empty(cache.step_staging_bytes(128), dtype=torch.uint8, device=dev)
     cache.stream_step_host(ids, [0, 128], qh, kh, vh, oh, staging, w.spec.scale)
+    cache.stream_host_join()
     torch.cuda.synchronize()
     ref = run_workload_oracle(w)
     d = oh.float().numpy() - ref["out"][0][0]
