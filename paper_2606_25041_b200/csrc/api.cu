@@ -160,6 +160,17 @@ ws_status_t upload_slot(ws_cache* c, const char* host, char* dev, size_t bytes, 
   return WS_OK;
 }
 
+// Metadata that does not fit the kernel parameters travels through the pinned ring, whose slots are
+// recycled (and waited for with cudaEventSynchronize): that cannot be captured into a CUDA graph.
+ws_status_t refuse_if_capturing(cudaStream_t st, const char* what) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { (void)cudaGetLastError(); return WS_OK; }
+  if (cs != cudaStreamCaptureStatusNone)
+    return fail(WS_ERR_UNSUPPORTED, "%s exceeds the kernel-parameter tier; this call cannot be captured "
+                "into a CUDA graph (split the batch or query fewer tokens per call)", what);
+  return WS_OK;
+}
+
 cudaEvent_t timing_event(ws_cache* c) {
   cudaEvent_t e = nullptr;
   if (!c->ev_pool.empty()) { e = c->ev_pool.back(); c->ev_pool.pop_back(); return e; }
@@ -419,6 +430,10 @@ ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
   if (inline_meta) {
     h = (char*)inl.w;
   } else {
+    if (!c->dry) {
+      st = refuse_if_capturing((cudaStream_t)cuda_stream, "append metadata");
+      if (st != WS_OK) return st;
+    }
     st = next_slot(c, words * 4, &h, &d);
     if (st != WS_OK) return st;
   }
@@ -505,7 +520,9 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     if (c->dry && !c->tensor_path_ok) { c->last_plan = ws::Plan(); return WS_OK; }
     if (!c->dry) {
       size_t bytes = (size_t)NQ * 8;
-      ws_status_t st = next_slot(c, bytes, &h, &d);
+      ws_status_t st = refuse_if_capturing(stream, "generic-kernel metadata");
+      if (st != WS_OK) return st;
+      st = next_slot(c, bytes, &h, &d);
       if (st != WS_OK) return st;
       memcpy(h, tok_slot.data(), (size_t)NQ * 4);
       memcpy(h + (size_t)NQ * 4, vis_end.data(), (size_t)NQ * 4);
@@ -532,8 +549,12 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     return fail(WS_ERR_WORKSPACE_TOO_SMALL, "plan needs %d partial slots, workspace holds %d",
                 plan.num_part_slots, c->lay.max_part_slots);
   std::vector<int32_t> blob = ws::serialise_plan(plan, vis_end, any_multi);
-  const bool inline_meta = blob.size() <= (size_t)ws::kInlineAttnWords;
+  const bool inline_meta = blob.size() <= (size_t)ws::kInlineAttnWordsLarge;
   ws_status_t st = WS_OK;
+  if (!inline_meta && !c->dry) {
+    st = refuse_if_capturing(stream, "attention metadata");
+    if (st != WS_OK) return st;
+  }
   if (!inline_meta) {
     st = next_slot(c, blob.size() * 4, &h, &d);
     if (st != WS_OK) return st;
@@ -551,6 +572,7 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
 
   ws::Sm100Launch L{};
   if (inline_meta) { memcpy(L.inl.w, blob.data(), blob.size() * 4); d = nullptr; }
+  L.inl_words = inline_meta ? (int32_t)blob.size() : 0;
   L.p.q = q; L.p.out = out; L.p.lse = lse;
   L.p.k_pool = c->cfg.k_pool; L.p.v_pool = c->cfg.v_pool;
   L.p.page_table = c->d_page_table;
@@ -580,7 +602,7 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
   c->launches += 1;
   if (!c->last_plan.combine.empty()) {
     TimedLaunch tc(c, &c->t_combine, stream);
-    WS_CUDA(ws::launch_combine(L.p, L.inl, (int32_t)c->last_plan.combine.size(), c->last_plan.team_size, stream));
+    WS_CUDA(ws::launch_combine(L.p, L.inl, L.inl_words, (int32_t)c->last_plan.combine.size(), c->last_plan.team_size, stream));
     tc.done();
     c->launches += 1;
   }

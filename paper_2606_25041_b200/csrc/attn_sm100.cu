@@ -35,6 +35,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
+#include <string.h>
 
 #include "launch.h"
 #include "sm100_ptx.cuh"
@@ -160,12 +161,12 @@ __device__ __forceinline__ void softmax_chunk(const uint32_t* sr, float c, float
   }
 }
 
-template <int kCG>
+template <int kCG, int kInlW>
 __global__ void __launch_bounds__(kThreads, 1)
 attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ CUtensorMap tmap_k,
                   const __grid_constant__ CUtensorMap tmap_v,
-                  const __grid_constant__ InlineAttnMeta inl, const AttnParams p_in) {
+                  const __grid_constant__ InlineMeta<kInlW> inl, const AttnParams p_in) {
   AttnParams p = p_in;
   if (p.meta == nullptr) p.meta = inl.w;
   extern __shared__ uint8_t smem_raw[];
@@ -673,11 +674,15 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 }
 
 cudaError_t sm100_attn_configure() {
-  cudaError_t e = cudaFuncSetAttribute(attn_sm100_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)kSmemBytes);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(attn_sm100_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              (int)kSmemBytes);
+  const void* fns[4] = {(const void*)attn_sm100_kernel<1, kInlineAttnWords>,
+                        (const void*)attn_sm100_kernel<2, kInlineAttnWords>,
+                        (const void*)attn_sm100_kernel<1, kInlineAttnWordsLarge>,
+                        (const void*)attn_sm100_kernel<2, kInlineAttnWordsLarge>};
+  for (const void* f : fns) {
+    cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }
 
 cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream) {
@@ -696,11 +701,18 @@ cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream) {
     at[na].id = cudaLaunchAttributeClusterDimension;
     at[na].val.clusterDim.x = 2; at[na].val.clusterDim.y = 1; at[na].val.clusterDim.z = 1;
     ++na;
-    cfg.attrs = at; cfg.numAttrs = na;
-    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<2>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
   }
   cfg.attrs = at; cfg.numAttrs = na;
-  return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
+  if (l.inl_words <= kInlineAttnWords) {
+    InlineAttnMeta small;
+    memcpy(small.w, l.inl.w, sizeof(small.w));
+    if (l.cta_group == 2)
+      return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<2, kInlineAttnWords>, l.tmap_q, l.tmap_k, l.tmap_v, small, l.p);
+    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWords>, l.tmap_q, l.tmap_k, l.tmap_v, small, l.p);
+  }
+  if (l.cta_group == 2)
+    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<2, kInlineAttnWordsLarge>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
+  return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWordsLarge>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
 }
 
 }  // namespace ws

@@ -9,6 +9,7 @@
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <math.h>
+#include <string.h>
 
 #include "launch.h"
 
@@ -16,8 +17,9 @@ namespace ws {
 
 constexpr int kCombineRowsPerBlock = 8;
 
+template <int kInlW>
 __global__ void __launch_bounds__(kCombineRowsPerBlock * 32)
-combine_kernel(AttnParams p, const __grid_constant__ InlineAttnMeta inl, int32_t team_size) {
+combine_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int32_t team_size) {
   pdl_wait();                      // partials of the attention kernel launched just before
   pdl_launch_dependents();         // the next step's append does not depend on this kernel
   if (p.meta == nullptr) p.meta = inl.w;
@@ -89,12 +91,18 @@ combine_kernel(AttnParams p, const __grid_constant__ InlineAttnMeta inl, int32_t
     p.lse[(int64_t)tok * p.Hq + head] = (mx_run + log2f(wsum_run)) * 0.6931471805599453f;
 }
 
-cudaError_t launch_combine(const AttnParams& p, const InlineAttnMeta& inl, int32_t num_combine,
-                           int32_t team_size, cudaStream_t stream) {
+cudaError_t launch_combine(const AttnParams& p, const InlineAttnMetaLarge& inl, int32_t inl_words,
+                           int32_t num_combine, int32_t team_size, cudaStream_t stream) {
   if (num_combine == 0) return cudaSuccess;
   int32_t grid = num_combine * team_size * (kPairRows / kCombineRowsPerBlock);
-  return launch_pdl(combine_kernel, dim3(grid), dim3(kCombineRowsPerBlock * 32), 0, stream, p, inl,
-                    team_size);
+  if (inl_words <= kInlineAttnWords) {
+    InlineAttnMeta small;
+    memcpy(small.w, inl.w, sizeof(small.w));
+    return launch_pdl(combine_kernel<kInlineAttnWords>, dim3(grid), dim3(kCombineRowsPerBlock * 32), 0,
+                      stream, p, small, team_size);
+  }
+  return launch_pdl(combine_kernel<kInlineAttnWordsLarge>, dim3(grid), dim3(kCombineRowsPerBlock * 32),
+                    0, stream, p, inl, team_size);
 }
 
 }  // namespace ws

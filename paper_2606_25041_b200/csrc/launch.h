@@ -58,13 +58,14 @@ cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse
 struct Sm100Launch {
   AttnParams p;                      // p.meta == nullptr: use `inl`
   CUtensorMap tmap_q, tmap_k, tmap_v;
-  InlineAttnMeta inl;
+  InlineAttnMetaLarge inl;
+  int32_t inl_words;                 // words of `inl` in use (selects the small / large parameter tier)
   int32_t num_ctas;
   int32_t cta_group;                 // 1, or 2 (CTA pairs; needs an even team size)
 };
 cudaError_t sm100_attn_configure();    // one-time cudaFuncSetAttribute
 cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream);
-cudaError_t launch_combine(const AttnParams& p, const InlineAttnMeta& inl, int32_t num_combine,
-                           int32_t team_size, cudaStream_t stream);
+cudaError_t launch_combine(const AttnParams& p, const InlineAttnMetaLarge& inl, int32_t inl_words,
+                           int32_t num_combine, int32_t team_size, cudaStream_t stream);
 
 }  // namespace ws

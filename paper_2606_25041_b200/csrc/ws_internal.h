@@ -14,10 +14,17 @@ constexpr int kMaxTeam = 8;       // max row-tile pairs of one (session, KV head
 // Small per-call metadata travels in the kernel parameters instead of a host->device copy (keeps the
 // append -> attention -> combine chain free of stream operations between the kernels, which is what
 // lets programmatic dependent launch overlap them).  Larger blobs go through the workspace ring.
-constexpr int kInlineAttnWords = 800;     // 3200 B of the 4 KB kernel-parameter space
-constexpr int kInlineAppendWords = 120;
-struct InlineAttnMeta { int32_t w[kInlineAttnWords]; };
-struct InlineAppendMeta { int32_t w[kInlineAppendWords]; };
+// Two tiers for the attention blob: the small one keeps the launch of the common single-session step
+// light; the large one (CUDA >= 12.1 allows 32,764 B of kernel parameters on sm_70+) covers many-group
+// plans (MHA with 16+ heads, ragged multi-session batches) so that those steps, too, need no
+// host->device copy and stay CUDA-graph capturable.
+constexpr int kInlineAttnWords = 800;
+constexpr int kInlineAttnWordsLarge = 7000;
+constexpr int kInlineAppendWords = 960;
+template <int W> struct InlineMeta { int32_t w[W]; };
+using InlineAttnMeta = InlineMeta<kInlineAttnWords>;
+using InlineAttnMetaLarge = InlineMeta<kInlineAttnWordsLarge>;
+using InlineAppendMeta = InlineMeta<kInlineAppendWords>;
 
 struct Group {
   int32_t q_token0;      // first global query token (row of q/out) covered by this group

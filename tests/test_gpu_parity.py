@@ -420,6 +420,43 @@ def test_next2_solver_step_is_cuda_graph_capturable():
         assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3, step
 
 
+def test_graph_capture_ragged_multi_session_uses_large_parameter_tier():
+    """A ragged 8-session step (config-5 structure, scaled down) has too many groups / segments for
+    the small kernel-parameter tier; the large tier keeps it free of host->device copies, so the
+    whole append + attention + combine step is captured and replays correctly."""
+    import torch
+    w = _small(5, cache_lens=(700, 1300, 2081, 90, 1500, 333, 2600, 1024), steps=1)
+    dev = torch.device("cuda", 0)
+    cache = make_cache(w)
+    ids = preload_gpu(cache, w, [_torch_of(s.k_cache, dev) for s in w.sessions],
+                      [_torch_of(s.v_cache, dev) for s in w.sessions])
+    base = [cache.session_info(i)[1] for i in ids]
+    sp = w.spec
+    n, S = sp.block_tokens, sp.num_sessions
+    cu = [i * n for i in range(S + 1)]
+    q = torch.cat([_torch_of(s.q[0], dev) for s in w.sessions])
+    k = torch.cat([_torch_of(s.k[0], dev) for s in w.sessions])
+    v = torch.cat([_torch_of(s.v[0], dev) for s in w.sessions])
+    qb, kb, vb = torch.zeros_like(q), torch.zeros_like(k), torch.zeros_like(v)
+    out = torch.zeros_like(q)
+    cache.kv_append(ids, cu, kb, vb); cache.block_causal_attn_fwd(ids, cu, qb, out, sp.scale)
+    for sid, b in zip(ids, base):
+        cache.session_truncate(sid, b)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        cache.kv_append(ids, cu, kb, vb)
+        cache.block_causal_attn_fwd(ids, cu, qb, out, sp.scale)
+    qb.copy_(q); kb.copy_(k); vb.copy_(v)
+    g.replay()
+    torch.cuda.synchronize()
+    ref = run_workload_oracle(w)
+    o = out.float().cpu().numpy().astype(np.float64).reshape(S, n, sp.num_q_heads, sp.head_dim)
+    for s in range(S):
+        d = o[s] - ref["out"][0][s]
+        assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3, s
+
+
 # ------------------------------------------------------------------ closed-form pins on the GPU
 def _run_custom_bf16(L, n, Hq, Hkv, kc, vc, q, kn, vn, scale, min_splits=0):
     """single session, cache (kc, vc) then one block (kn, vn) with queries q; returns (O, LSE)."""
