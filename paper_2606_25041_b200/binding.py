@@ -55,7 +55,7 @@ EXPORTS = ["ws_pool_bytes", "ws_workspace_bytes", "ws_cache_create", "ws_cache_d
            "ws_session_open", "ws_session_close", "ws_session_info", "ws_session_truncate",
            "ws_free_pages", "ws_kv_append", "ws_block_causal_attn_fwd", "ws_step_staging_bytes",
            "ws_stream_step_host", "ws_stream_host_join", "ws_fm_euler_update", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
-           "ws_debug_set_min_splits", "ws_last_plan_info", "ws_last_plan_segment",
+           "ws_debug_set_min_splits", "ws_debug_set_decode_plan", "ws_last_plan_info", "ws_last_plan_segment",
            "ws_launch_count", "ws_debug_kernel_timing", "ws_debug_read_kernel_times",
            "ws_status_str", "ws_last_error", "ws_version"]
 
@@ -96,6 +96,7 @@ def load_library() -> C.CDLL:
     lib.ws_session_pages.argtypes = [vp, C.c_int32, i32p, C.c_int32, i32p]
     lib.ws_debug_shuffle_free_pages.argtypes = [vp, C.c_uint64]
     lib.ws_debug_set_min_splits.argtypes = [vp, C.c_int32]
+    lib.ws_debug_set_decode_plan.argtypes = [vp, C.c_int32]
     lib.ws_last_plan_info.argtypes = [vp, C.POINTER(PlanInfo)]
     lib.ws_last_plan_segment.argtypes = [vp, C.c_int32, C.POINTER(PlanSegment)]
     lib.ws_launch_count.argtypes = [vp]; lib.ws_launch_count.restype = C.c_int64
@@ -262,6 +263,9 @@ class Cache:
 
     def set_min_splits(self, n: int) -> None:
         _check(self.lib.ws_debug_set_min_splits(self.handle, n))
+
+    def set_decode_plan(self, enable: bool) -> None:
+        _check(self.lib.ws_debug_set_decode_plan(self.handle, int(enable)))
 
     def last_plan_info(self) -> dict:
         info = PlanInfo()

@@ -118,6 +118,7 @@ struct ws_cache {
   EncodeTiledFn encode = nullptr;
   CUtensorMap tmap_k{}, tmap_v{};
   int32_t min_splits = 0;
+  bool decode_plan_enabled = true;
   int64_t launches = 0;
   ws::Plan last_plan;
   bool last_tensor = false;
@@ -382,6 +383,12 @@ ws_status_t ws_debug_shuffle_free_pages(ws_cache_t* c, uint64_t seed) {
   return WS_OK;
 }
 
+ws_status_t ws_debug_set_decode_plan(ws_cache_t* c, int32_t enable) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  c->decode_plan_enabled = enable != 0;
+  return WS_OK;
+}
+
 ws_status_t ws_debug_set_min_splits(ws_cache_t* c, int32_t min_splits) {
   if (!c || min_splits < 0) return fail(WS_ERR_INVALID_ARG, "bad argument");
   c->min_splits = min_splits;
@@ -543,8 +550,12 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
   }
 
   ws::PlanConfig pc{c->cfg.num_kv_heads, G, c->num_sms, /*min_tiles=*/2, /*seg_overhead_tiles=*/3.3f,
-                    c->min_splits, c->lay.max_part_slots};
+                    c->min_splits, c->lay.max_part_slots, c->decode_plan_enabled};
   ws::Plan plan = ws::build_plan(pc, ps, vis_end);
+  if (!plan.ok && plan.alt) {           // too many (session, head) groups for two partials each
+    pc.allow_alt = false;
+    plan = ws::build_plan(pc, ps, vis_end);
+  }
   if (!plan.ok)
     return fail(WS_ERR_WORKSPACE_TOO_SMALL, "plan needs %d partial slots, workspace holds %d",
                 plan.num_part_slots, c->lay.max_part_slots);
@@ -561,6 +572,12 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     memcpy(h, blob.data(), blob.size() * 4);
   }
   c->last_plan = std::move(plan);
+  // CTA pairs (tcgen05 cta_group::2) halve the shared-memory operand traffic but put two DSMEM
+  // round trips (remote P arrival, multicast S commit) on the S -> softmax -> PV chain that bounds
+  // this kernel: measured 309 us vs 224 us per config-4 unit.  Opt-in only.
+  const int32_t cta_group = (!c->last_plan.alt && (c->cfg.flags & WS_FLAG_CTA_PAIRS) &&
+                             c->last_plan.team_size % 2 == 0) ? 2 : 1;
+  c->last_cta_group = c->last_plan.alt ? 3 : cta_group;
   // every append launched before this kernel has completed once this kernel has (PDL chain, see
   // attn_sm100.cu): the next call may read those tokens before its own griddepcontrol.wait
   c->host->mark_all_stable();
@@ -591,11 +608,8 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     if (st != WS_OK) return st;
   }
   L.num_ctas = c->last_plan.num_teams * c->last_plan.team_size;
-  // CTA pairs (tcgen05 cta_group::2) halve the shared-memory operand traffic but put two DSMEM
-  // round trips (remote P arrival, multicast S commit) on the S -> softmax -> PV chain that bounds
-  // this kernel: measured 309 us vs 224 us per config-4 unit.  Opt-in only.
-  L.cta_group = ((c->cfg.flags & WS_FLAG_CTA_PAIRS) && c->last_plan.team_size % 2 == 0) ? 2 : 1;
-  c->last_cta_group = L.cta_group;
+  L.cta_group = cta_group;
+  L.alt = c->last_plan.alt;
   TimedLaunch tl(c, &c->t_attn, stream);
   WS_CUDA(ws::launch_attn_sm100(L, stream));
   tl.done();

@@ -161,12 +161,15 @@ __device__ __forceinline__ void softmax_chunk(const uint32_t* sr, float c, float
   }
 }
 
-template <int kCG, int kInlW>
+// kAlt: decode plan (plan.h) - both accumulator sets use Q tile 0; set q processes the KV tiles of the
+// segment with (tile - tile_begin) % 2 == q and writes its own partial (slot part_base + q).
+template <int kCG, int kInlW, bool kAlt>
 __global__ void __launch_bounds__(kThreads, 1)
 attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ CUtensorMap tmap_k,
                   const __grid_constant__ CUtensorMap tmap_v,
                   const __grid_constant__ InlineMeta<kInlW> inl, const AttnParams p_in) {
+  static_assert(!(kAlt && kCG == 2), "the decode plan runs on single CTAs");
   AttnParams p = p_in;
   if (p.meta == nullptr) p.meta = inl.w;
   extern __shared__ uint8_t smem_raw[];
@@ -241,6 +244,35 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         const int32_t last_page = (sv.g.kv_len - 1) / p.P;
         // tiles >= dep_tile may still be being written by the preceding append kernel (PDL)
         if (!dep_waited && sv.tile_begin + 1 >= sv.g.dep_tile) { pdl_wait(); dep_waited = true; }
+        if constexpr (kAlt) {
+          // one Q tile serves both accumulator sets
+          mbar_wait(bq_empty, (q_it & 1) ^ 1);
+          mbar_arrive_expect_tx(bq_full, kQTileBytes);
+          for (int h = 0; h < 2; ++h)
+            tma_load_3d(sQ + h * kHalfBytes, &tmap_q, bq_full, h * 64, sv.g.kv_head * p.G, sv.g.q_token0);
+          ++q_it;
+          auto load_tile = [&](const CUtensorMap* tm, int32_t j) {
+            if (!dep_waited && j >= sv.g.dep_tile) { pdl_wait(); dep_waited = true; }
+            const int32_t c0 = page_row[min(2 * j, last_page)], c1 = page_row[min(2 * j + 1, last_page)];
+            const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
+            mbar_wait(bkv_empty(slot), par ^ 1);
+            mbar_arrive_expect_tx(bkv_full(slot), 32768);
+            const uint32_t dst = sRing + slot * kSlotBytes;
+            tma_load_4d(dst, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c0);
+            tma_load_4d(dst + kHalfBytes / 2, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c1);
+            tma_load_4d(dst + kHalfBytes, tm, bkv_full(slot), 64, 0, sv.g.kv_head, c0);
+            tma_load_4d(dst + kHalfBytes + kHalfBytes / 2, tm, bkv_full(slot), 64, 0, sv.g.kv_head, c1);
+            ++ring_it;
+          };
+          // consumption order of the MMA warp: K0 K1 | V0 K2 | V1 K3 | ...
+          load_tile(&tmap_k, sv.tile_begin);
+          if (sv.tile_begin + 1 < sv.tile_end) load_tile(&tmap_k, sv.tile_begin + 1);
+          for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
+            load_tile(&tmap_v, j);
+            if (j + 2 < sv.tile_end) load_tile(&tmap_k, j + 2);
+          }
+          continue;
+        }
         int32_t pg0 = page_row[min(2 * sv.tile_begin, last_page)];
         int32_t pg1 = page_row[min(2 * sv.tile_begin + 1, last_page)];
         // Q pair (own rows).  kCG = 2: the bytes of both CTAs are credited to the leader's q_full.
@@ -304,9 +336,10 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const uint64_t desc_k = make_smem_desc_sw128(0, 16, 1024);          // K-major operands (Q, K)
       const uint64_t desc_v = make_smem_desc_sw128(0, kHalfBytes, 1024);  // MN-major operand (V)
       uint32_t ring_it = 0, q_it = 0, tile_it = 0, seg_it = 0;
+      uint32_t alt_tiles0 = 0, alt_tiles1 = 0, alt_segs0 = 0, alt_segs1 = 0;   // kAlt: per accumulator set
       PROF_DECL(8)
       auto issue_S = [&](int q, uint32_t slot) {
-        const uint64_t da = desc_k + ((sQ + q * kQTileBytes) >> 4);
+        const uint64_t da = desc_k + ((sQ + (kAlt ? 0 : q) * kQTileBytes) >> 4);
         const uint64_t db = desc_k + ((sRing + slot * kSlotBytes) >> 4);
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {
@@ -336,6 +369,57 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         if (sv.tile_end <= sv.tile_begin) continue;          // clipped away for this pair
         const int32_t nt = sv.tile_end - sv.tile_begin;
         mbar_wait(bq_full, q_it & 1);
+        if constexpr (kAlt) {
+          // S_q <- Q K(tile q) for q = 0, 1; then per tile j (set q = j & 1): O_q += P V(j), S_q <- Q K(j+2)
+          for (int q = 0; q < 2 && q < nt; ++q) {
+            const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
+            mbar_wait(bkv_full(slot), par);
+            tc_fence_after();
+            if (leader) {
+              issue_S(q, slot); commit(bs_full(q)); commit(bkv_empty(slot));
+              if (q + 1 == nt || (q == 1 && nt == 2)) commit(bq_empty);
+            }
+            __syncwarp();
+            ++ring_it;
+          }
+          for (int32_t j = 0; j < nt; ++j) {
+            const int q = j & 1;
+            const uint32_t tq = q ? alt_tiles1 : alt_tiles0, sq = q ? alt_segs1 : alt_segs0;
+            const uint32_t slot_v = ring_it % kStages, par_v = (ring_it / kStages) & 1;
+            ++ring_it;
+            const bool have_next = j + 2 < nt;
+            uint32_t slot_k = 0, par_k = 0;
+            if (have_next) { slot_k = ring_it % kStages; par_k = (ring_it / kStages) & 1; ++ring_it; }
+            mbar_wait(bkv_full(slot_v), par_v);
+            mbar_wait(bp_full(q, 0), tq & 1);
+            if (j < 2) mbar_wait(bo_empty(q), (sq & 1) ^ 1);
+            tc_fence_after();
+            if (leader) { issue_PV(q, slot_v, 0, j >= 2); commit(bpv_h0(q)); }
+            __syncwarp();
+            mbar_wait(bp_full(q, 1), tq & 1);
+            tc_fence_after();
+            if (leader) {
+              issue_PV(q, slot_v, 1, true);
+              if (!have_next) commit(bo_full(q));
+              commit(bkv_empty(slot_v));
+            }
+            __syncwarp();
+            if (have_next) {
+              mbar_wait(bkv_full(slot_k), par_k);
+              tc_fence_after();
+              if (leader) {
+                issue_S(q, slot_k); commit(bs_full(q)); commit(bkv_empty(slot_k));
+                if (j + 3 == nt) commit(bq_empty);
+              }
+              __syncwarp();
+            }
+            if (q) ++alt_tiles1; else ++alt_tiles0;
+          }
+          ++alt_segs0;
+          if (nt > 1) ++alt_segs1;
+          ++q_it;
+          continue;
+        }
         {
           const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
           mbar_wait(bkv_full(slot), par);
@@ -410,7 +494,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const int q = warp >> 2;
     const uint32_t lane_base = (uint32_t)(warp & 3) * 32;
     const int32_t row_in_tile = (int32_t)lane_base + lane;
-    const int32_t R = q * kTileRows + row_in_tile;           // packed row inside the pair
+    const int32_t R = kAlt ? row_in_tile : q * kTileRows + row_in_tile;   // packed row inside the pair
     const uint32_t t_s = tmem_base + (lane_base << 16) + q * 128;
     const uint32_t t_o = tmem_base + (lane_base << 16) + 256 + q * 128;
     const float c = p.scale * 1.4426950408889634f;
@@ -418,22 +502,25 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     auto arrive_leader = [&](uint32_t bar) {
       if constexpr (kCG == 2) mbar_arrive_cluster(bar & kPeerBitMask); else mbar_arrive(bar);
     };
-    uint32_t tile_it = 0, seg_it = 0;
+    uint32_t tile_it = 0, seg_it = 0, alt_sync_it = 0;
     bool pdl_done = false;
     PROF_DECL(8)
 
     for (int32_t si = seg_lo; si < seg_hi; ++si) {
       SegView sv;
       if (!load_segment<kCG - 1>(p.meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
-      const int32_t nt = sv.tile_end - sv.tile_begin;
+      // kAlt: this warpgroup takes tiles tile_begin + q, + q + 2, ...
+      const int32_t nt = kAlt ? (sv.tile_end > sv.tile_begin ? (sv.tile_end - sv.tile_begin + 1 - q) / 2 : 0)
+                              : sv.tile_end - sv.tile_begin;
+      const int32_t part_slot = sv.part_base + pair;
       const int32_t tok = sv.g.q_token0 + pair * tok_per_pair + R / p.G;
       const bool row_valid = tok < sv.g.q_token_end && pair < sv.g.npairs;   // (kCG = 2: a ghost CTA computes but stores nothing)
-      if (nt <= 0) {
+      if (sv.tile_end <= sv.tile_begin) {
         // every tile of this segment lies beyond what the pair can see: publish an empty partial
         // (the segment is one of several splits, otherwise it would start at tile 0)
         if (!pdl_done) { pdl_wait(); pdl_done = true; }
-        if (row_valid && sv.part_base >= 0)
-          p.part_lse[(int64_t)(sv.part_base + pair) * kPairRows + R] = -INFINITY;
+        if (row_valid && sv.part_base >= 0 && (!kAlt || q == 0))
+          p.part_lse[(int64_t)part_slot * kPairRows + R] = -INFINITY;
         continue;
       }
       const int32_t head = sv.g.kv_head * p.G + R % p.G;
@@ -442,7 +529,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       float m_used = -INFINITY, l = 0.f;
 
       for (int32_t j = 0; j < nt; ++j) {
-        const int32_t key0 = (sv.tile_begin + j) * kTileKeys;
+        const int32_t key0 = (sv.tile_begin + (kAlt ? 2 * j + q : j)) * kTileKeys;
         PROF_MARK(0)
         mbar_wait(bs_full(q), tile_it & 1);
         tc_fence_after();
@@ -602,10 +689,46 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       // first global write of this CTA: the predecessor grids (append; transitively the previous
       // step's combine, which reads the partial buffers and writes `out`) must have completed
       if (!pdl_done) { pdl_wait(); pdl_done = true; }
-      mbar_wait(bo_full(q), seg_it & 1);
-      tc_fence_after();
-      const float inv_l = l > 0.f ? 1.f / l : 0.f;
-      const float lse2 = l > 0.f ? m_used + log2f(l) : -INFINITY;
+      if (nt > 0) {
+        mbar_wait(bo_full(q), seg_it & 1);
+        tc_fence_after();
+      }
+      float inv_l = l > 0.f ? 1.f / l : 0.f;                // coefficient of this set's accumulator
+      float lse2 = l > 0.f ? m_used + log2f(l) : -INFINITY;
+      float inv_l1 = 0.f;                                   // kAlt: coefficient of accumulator set 1
+      bool use1 = false;
+      if constexpr (kAlt) {
+        // The two accumulator sets hold attention over the even / odd KV tiles of the segment for the
+        // SAME rows: merge them here (LSE-weighted, exactly what the combine kernel does across
+        // segments) so the segment yields one result.  Set 1 hands (lse2, 1/l) to warpgroup 0 through
+        // the shared memory of the unused second Q tile (double-buffered by segment parity);
+        // warpgroup 0 reads O_1 straight from TMEM (same lanes) and releases it on set 1's behalf.
+        float2* xchg = reinterpret_cast<float2*>(smem_raw + (sQ - smem_u32(smem_raw)) + kQTileBytes) +
+                       (alt_sync_it & 1) * kTileRows;
+        ++alt_sync_it;
+        if (q == 1) {
+          xchg[row_in_tile] = make_float2(lse2, inv_l);
+          tc_fence_before();
+          asm volatile("bar.sync 1, 256;" ::: "memory");
+          if (nt > 0) ++seg_it;
+          continue;
+        }
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        tc_fence_after();                                   // set 1's PV completion was observed by warpgroup 1
+        const float2 peer = xchg[row_in_tile];
+        use1 = sv.tile_end - sv.tile_begin >= 2;            // set 1 processed at least one tile
+        const float mx = fmaxf(lse2, peer.x);
+        if (mx == -INFINITY) {
+          inv_l = 0.f;
+        } else {
+          const float w0 = ex2_approx(lse2 - mx), w1 = use1 ? ex2_approx(peer.x - mx) : 0.f;
+          const float inv_w = 1.f / (w0 + w1);
+          inv_l = w0 * inv_w * inv_l;
+          inv_l1 = w1 * inv_w * peer.y;
+          lse2 = mx + log2f(w0 + w1);
+        }
+      }
+      const float osc = kAlt ? 1.f : inv_l;                 // kAlt: already applied by the merge above
       if (sv.part_base < 0) {
         __nv_bfloat16* orow = reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)tok * p.Hq + head) * p.D;
 #pragma unroll
@@ -613,32 +736,58 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           uint32_t o[32];
           tmem_ld32(t_o + ch * 32, o);
           tmem_wait_ld();
+          if constexpr (kAlt) {
+            if (use1) {
+              uint32_t o1[32];
+              tmem_ld32(t_o + 128 + ch * 32, o1);
+              tmem_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 32; ++i)
+                o[i] = __float_as_uint(fmaf(__uint_as_float(o1[i]), inv_l1, __uint_as_float(o[i]) * inv_l));
+            } else {
+#pragma unroll
+              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * inv_l);
+            }
+          }
           if (row_valid) {
 #pragma unroll
             for (int i = 0; i < 32; i += 8) {
               uint4 w;
-              w.x = pack_bf16x2(__uint_as_float(o[i]) * inv_l, __uint_as_float(o[i + 1]) * inv_l);
-              w.y = pack_bf16x2(__uint_as_float(o[i + 2]) * inv_l, __uint_as_float(o[i + 3]) * inv_l);
-              w.z = pack_bf16x2(__uint_as_float(o[i + 4]) * inv_l, __uint_as_float(o[i + 5]) * inv_l);
-              w.w = pack_bf16x2(__uint_as_float(o[i + 6]) * inv_l, __uint_as_float(o[i + 7]) * inv_l);
+              w.x = pack_bf16x2(__uint_as_float(o[i]) * osc, __uint_as_float(o[i + 1]) * osc);
+              w.y = pack_bf16x2(__uint_as_float(o[i + 2]) * osc, __uint_as_float(o[i + 3]) * osc);
+              w.z = pack_bf16x2(__uint_as_float(o[i + 4]) * osc, __uint_as_float(o[i + 5]) * osc);
+              w.w = pack_bf16x2(__uint_as_float(o[i + 6]) * osc, __uint_as_float(o[i + 7]) * osc);
               *reinterpret_cast<uint4*>(orow + ch * 32 + i) = w;
             }
           }
         }
         if (row_valid && p.lse) p.lse[(int64_t)tok * p.Hq + head] = lse2 * 0.6931471805599453f;
       } else {
-        const int64_t prow = (int64_t)(sv.part_base + pair) * kPairRows + R;
+        const int64_t prow = (int64_t)part_slot * kPairRows + R;
         float* orow = p.part_o + prow * p.D;
 #pragma unroll
         for (int ch = 0; ch < 4; ++ch) {
           uint32_t o[32];
           tmem_ld32(t_o + ch * 32, o);
           tmem_wait_ld();
+          if constexpr (kAlt) {
+            if (use1) {
+              uint32_t o1[32];
+              tmem_ld32(t_o + 128 + ch * 32, o1);
+              tmem_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 32; ++i)
+                o[i] = __float_as_uint(fmaf(__uint_as_float(o1[i]), inv_l1, __uint_as_float(o[i]) * inv_l));
+            } else {
+#pragma unroll
+              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * inv_l);
+            }
+          }
           if (row_valid) {
 #pragma unroll
             for (int i = 0; i < 32; i += 4) {
-              float4 w = make_float4(__uint_as_float(o[i]) * inv_l, __uint_as_float(o[i + 1]) * inv_l,
-                                     __uint_as_float(o[i + 2]) * inv_l, __uint_as_float(o[i + 3]) * inv_l);
+              float4 w = make_float4(__uint_as_float(o[i]) * osc, __uint_as_float(o[i + 1]) * osc,
+                                     __uint_as_float(o[i + 2]) * osc, __uint_as_float(o[i + 3]) * osc);
               *reinterpret_cast<float4*>(orow + ch * 32 + i) = w;
             }
           }
@@ -647,6 +796,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       }
       tc_fence_before();
       arrive_leader(bo_empty(q));
+      if constexpr (kAlt) { if (use1) mbar_arrive(bo_empty(1)); }
       PROF_MARK(6)
       ++seg_it;
     }
@@ -674,10 +824,12 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 }
 
 cudaError_t sm100_attn_configure() {
-  const void* fns[4] = {(const void*)attn_sm100_kernel<1, kInlineAttnWords>,
-                        (const void*)attn_sm100_kernel<2, kInlineAttnWords>,
-                        (const void*)attn_sm100_kernel<1, kInlineAttnWordsLarge>,
-                        (const void*)attn_sm100_kernel<2, kInlineAttnWordsLarge>};
+  const void* fns[6] = {(const void*)attn_sm100_kernel<1, kInlineAttnWords, false>,
+                        (const void*)attn_sm100_kernel<2, kInlineAttnWords, false>,
+                        (const void*)attn_sm100_kernel<1, kInlineAttnWordsLarge, false>,
+                        (const void*)attn_sm100_kernel<2, kInlineAttnWordsLarge, false>,
+                        (const void*)attn_sm100_kernel<1, kInlineAttnWords, true>,
+                        (const void*)attn_sm100_kernel<1, kInlineAttnWordsLarge, true>};
   for (const void* f : fns) {
     cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
     if (e != cudaSuccess) return e;
@@ -697,7 +849,8 @@ cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream) {
     at[na].val.programmaticStreamSerializationAllowed = 1;
     ++na;
   }
-  if (l.cta_group == 2) {
+  const bool pairs = l.cta_group == 2 && !l.alt;
+  if (pairs) {
     at[na].id = cudaLaunchAttributeClusterDimension;
     at[na].val.clusterDim.x = 2; at[na].val.clusterDim.y = 1; at[na].val.clusterDim.z = 1;
     ++na;
@@ -706,13 +859,17 @@ cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream) {
   if (l.inl_words <= kInlineAttnWords) {
     InlineAttnMeta small;
     memcpy(small.w, l.inl.w, sizeof(small.w));
-    if (l.cta_group == 2)
-      return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<2, kInlineAttnWords>, l.tmap_q, l.tmap_k, l.tmap_v, small, l.p);
-    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWords>, l.tmap_q, l.tmap_k, l.tmap_v, small, l.p);
+    if (l.alt)
+      return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWords, true>, l.tmap_q, l.tmap_k, l.tmap_v, small, l.p);
+    if (pairs)
+      return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<2, kInlineAttnWords, false>, l.tmap_q, l.tmap_k, l.tmap_v, small, l.p);
+    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWords, false>, l.tmap_q, l.tmap_k, l.tmap_v, small, l.p);
   }
-  if (l.cta_group == 2)
-    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<2, kInlineAttnWordsLarge>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
-  return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWordsLarge>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
+  if (l.alt)
+    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWordsLarge, true>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
+  if (pairs)
+    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<2, kInlineAttnWordsLarge, false>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
+  return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWordsLarge, false>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
 }
 
 }  // namespace ws

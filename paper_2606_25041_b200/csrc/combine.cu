@@ -5,7 +5,7 @@
 // HBM/L2-bound: reads nparts x 256 x (D+1) fp32 per (group, pair), writes bf16 O (+ fp32 LSE).
 // One warp per packed row: lane s loads the LSE of part s, the max and the weight sum are reduced
 // with warp shuffles, then the parts' O rows (one float4 per lane, D = 128) are accumulated with
-// four loads in flight per lane.
+// kDepth loads in flight per lane.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <math.h>
@@ -17,7 +17,10 @@ namespace ws {
 
 constexpr int kCombineRowsPerBlock = 8;
 
-template <int kInlW>
+// kDepth = O-row loads in flight per lane: 4 keeps the kernel at 64 registers (8 blocks / SM) for
+// the large grids of the general plan; 8 serves the small grids of decode steps, where few warps
+// have work and memory-level parallelism has to come from each of them.
+template <int kInlW, int kDepth>
 __global__ void __launch_bounds__(kCombineRowsPerBlock * 32)
 combine_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int32_t team_size) {
   pdl_wait();                      // partials of the attention kernel launched just before
@@ -61,11 +64,11 @@ combine_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int3
     wsum_run = wsum_run * rescale + ws;
     mx_run = mx_new;
     const int32_t cnt = min(32, ci.nparts - base);
-    for (int32_t k0 = 0; k0 < cnt; k0 += 4) {
-      float4 o[4];
-      float wk[4];
+    for (int32_t k0 = 0; k0 < cnt; k0 += kDepth) {
+      float4 o[kDepth];
+      float wk[kDepth];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
+      for (int u = 0; u < kDepth; ++u) {
         const int32_t k = k0 + u;
         wk[u] = __shfl_sync(0xffffffffu, w, k & 31);
         if (k < cnt && wk[u] != 0.f)
@@ -73,7 +76,7 @@ combine_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int3
         else { o[u] = make_float4(0.f, 0.f, 0.f, 0.f); wk[u] = 0.f; }
       }
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
+      for (int u = 0; u < kDepth; ++u) {
         acc.x = fmaf(wk[u], o[u].x, acc.x); acc.y = fmaf(wk[u], o[u].y, acc.y);
         acc.z = fmaf(wk[u], o[u].z, acc.z); acc.w = fmaf(wk[u], o[u].w, acc.w);
       }
@@ -95,14 +98,16 @@ cudaError_t launch_combine(const AttnParams& p, const InlineAttnMetaLarge& inl, 
                            int32_t num_combine, int32_t team_size, cudaStream_t stream) {
   if (num_combine == 0) return cudaSuccess;
   int32_t grid = num_combine * team_size * (kPairRows / kCombineRowsPerBlock);
+  const dim3 g(grid), b(kCombineRowsPerBlock * 32);
+  const bool deep = grid <= 2 * 148;
   if (inl_words <= kInlineAttnWords) {
     InlineAttnMeta small;
     memcpy(small.w, inl.w, sizeof(small.w));
-    return launch_pdl(combine_kernel<kInlineAttnWords>, dim3(grid), dim3(kCombineRowsPerBlock * 32), 0,
-                      stream, p, small, team_size);
+    if (deep) return launch_pdl(combine_kernel<kInlineAttnWords, 8>, g, b, 0, stream, p, small, team_size);
+    return launch_pdl(combine_kernel<kInlineAttnWords, 4>, g, b, 0, stream, p, small, team_size);
   }
-  return launch_pdl(combine_kernel<kInlineAttnWordsLarge>, dim3(grid), dim3(kCombineRowsPerBlock * 32),
-                    0, stream, p, inl, team_size);
+  if (deep) return launch_pdl(combine_kernel<kInlineAttnWordsLarge, 8>, g, b, 0, stream, p, inl, team_size);
+  return launch_pdl(combine_kernel<kInlineAttnWordsLarge, 4>, g, b, 0, stream, p, inl, team_size);
 }
 
 }  // namespace ws

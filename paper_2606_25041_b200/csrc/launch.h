@@ -62,6 +62,7 @@ struct Sm100Launch {
   int32_t inl_words;                 // words of `inl` in use (selects the small / large parameter tier)
   int32_t num_ctas;
   int32_t cta_group;                 // 1, or 2 (CTA pairs; needs an even team size)
+  bool alt;                          // decode plan (plan.h): same Q tile, alternate KV tiles
 };
 cudaError_t sm100_attn_configure();    // one-time cudaFuncSetAttribute
 cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream);

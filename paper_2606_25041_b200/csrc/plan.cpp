@@ -25,6 +25,9 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
   }
   plan.team_size = std::min<int32_t>(kMaxTeam, max_pairs);
   const int32_t Pt = plan.team_size;
+  plan.alt = cfg.allow_alt;
+  for (const PlanSession& s : sessions)
+    if ((int64_t)(s.q_end - s.q_begin) * cfg.G > kTileRows) plan.alt = false;
 
   std::vector<int32_t> group_tiles;
   for (const PlanSession& s : sessions) {
@@ -108,7 +111,7 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
 std::vector<int32_t> serialise_plan(const Plan& plan, const std::vector<int32_t>& vis_end,
                                     bool has_vis) {
   static_assert(sizeof(Group) == 32 && sizeof(Segment) == 16 && sizeof(CombineItem) == 16 &&
-                sizeof(AttnMeta) == 48, "blob layout");
+                sizeof(AttnMeta) == 64, "blob layout");
   AttnMeta m{};
   m.num_teams = plan.num_teams;
   m.team_size = plan.team_size;
@@ -116,6 +119,7 @@ std::vector<int32_t> serialise_plan(const Plan& plan, const std::vector<int32_t>
   m.num_segments = (int32_t)plan.segments.size();
   m.num_combine = (int32_t)plan.combine.size();
   m.has_vis = has_vis ? 1 : 0;
+  m.alt = plan.alt ? 1 : 0;
   int32_t off = sizeof(AttnMeta) / 4;
   m.off_groups = off;            off += m.num_groups * (int32_t)(sizeof(Group) / 4);
   m.off_team_seg_begin = off;    off += plan.num_teams + 1;

@@ -24,9 +24,18 @@ struct PlanConfig {
   float seg_overhead_tiles;  // cost of starting one more segment in a team, in KV-tile units
   int32_t min_splits;    // debug: force at least this many segments per group (0 = automatic)
   int32_t max_part_slots;
+  bool allow_alt;        // permit the decode plan (below) when every session qualifies
 };
 
+// Decode plan ("alt", NEXT-4: n*G <= 128 packed rows per (session, KV head), e.g. token-causal text
+// decode).  Such a step is cache-read bound (n*G FLOP/B << ridge), so the CTA's two
+// S/O accumulator sets are not given two Q tiles but the SAME Q tile and ALTERNATE KV tiles: set 0
+// takes the even tiles of the segment, set 1 the odd ones, each with its own running max / sum.  The
+// tensor pipe and the two softmax warpgroups then consume K/V twice as fast per CTA (HBM-bound instead
+// of bound by the S -> softmax -> PV chain).  The two sets are merged inside the CTA at the end of the
+// segment (LSE-weighted), so a segment still yields one result and the plan is otherwise unchanged.
 struct Plan {
+  bool alt = false;
   int32_t team_size = 1, num_teams = 0, total_tiles = 0, num_part_slots = 0;
   std::vector<Group> groups;
   std::vector<int32_t> team_seg_begin;   // [num_teams + 1]

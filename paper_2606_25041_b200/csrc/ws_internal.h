@@ -18,7 +18,7 @@ constexpr int kMaxTeam = 8;       // max row-tile pairs of one (session, KV head
 // light; the large one (CUDA >= 12.1 allows 32,764 B of kernel parameters on sm_70+) covers many-group
 // plans (MHA with 16+ heads, ragged multi-session batches) so that those steps, too, need no
 // host->device copy and stay CUDA-graph capturable.
-constexpr int kInlineAttnWords = 800;
+constexpr int kInlineAttnWords = 1000;
 constexpr int kInlineAttnWordsLarge = 7000;
 constexpr int kInlineAppendWords = 960;
 template <int W> struct InlineMeta { int32_t w[W]; };
@@ -59,6 +59,8 @@ struct AttnMeta {
   int32_t num_teams, team_size, num_groups, num_segments;
   int32_t num_combine, has_vis, off_groups, off_team_seg_begin;
   int32_t off_segments, off_combine, off_vis, total_words;
+  int32_t alt;           // 1: decode plan (every group has <= kTileRows packed rows), see plan.h
+  int32_t pad[3];
 };
 
 // Append metadata: per session in the call.

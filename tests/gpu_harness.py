@@ -81,7 +81,8 @@ def preload_gpu(cache, w: Workload, dev_k: List, dev_v: List) -> List[int]:
 
 
 def run_workload_gpu(w: Workload, flags: int = 0, min_splits: int = 0, shuffle_seed: Optional[int] = None,
-                     want_lse: bool = True, gather: bool = True, pool_fill: Optional[int] = None) -> Dict:
+                     want_lse: bool = True, gather: bool = True, pool_fill: Optional[int] = None,
+                     decode_plan: Optional[bool] = None) -> Dict:
     import torch
     sp = w.spec
     dev = torch.device("cuda", 0)
@@ -90,6 +91,8 @@ def run_workload_gpu(w: Workload, flags: int = 0, min_splits: int = 0, shuffle_s
         cache.shuffle_free_pages(shuffle_seed)
     if min_splits:
         cache.set_min_splits(min_splits)
+    if decode_plan is not None:
+        cache.set_decode_plan(decode_plan)
     dev_k = [_torch_of(s.k_cache, dev) for s in w.sessions]
     dev_v = [_torch_of(s.v_cache, dev) for s in w.sessions]
     ids = preload_gpu(cache, w, dev_k, dev_v)

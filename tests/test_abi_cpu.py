@@ -116,7 +116,7 @@ def test_shuffled_free_list_is_a_permutation(pkg):
     assert sorted(pages) == list(range(32)) and pages != list(range(32))
 
 
-def _plan(pkg, lens, n, Hq=32, Hkv=8, min_splits=0, blocks=1):
+def _plan(pkg, lens, n, Hq=32, Hkv=8, min_splits=0, blocks=1, decode_plan=True):
     S = len(lens)
     P = 64
     pages = sum((L + n * blocks + P - 1) // P for L in lens) + 4
@@ -134,6 +134,7 @@ def _plan(pkg, lens, n, Hq=32, Hkv=8, min_splits=0, blocks=1):
         c.kv_append(ids, [i * n for i in range(S + 1)], None, None)
     if min_splits:
         c.set_min_splits(min_splits)
+    c.set_decode_plan(decode_plan)
     c.block_causal_attn_fwd(ids, [i * n * blocks for i in range(S + 1)], None, None, 0.1,
                             num_q_blocks=[blocks] * S)
     return c.last_plan_info(), c.last_plan_segments()
@@ -188,7 +189,7 @@ def test_planner_ragged_multi_session(pkg):
 
 
 def test_planner_small_and_forced_splits(pkg):
-    info, segs = _plan(pkg, [100], 16, Hq=8, Hkv=2)          # 1 tile per group: no split
+    info, segs = _plan(pkg, [100], 16, Hq=8, Hkv=2, decode_plan=False)   # 1 tile per group: no split
     _check_cover(info, segs, 2)
     assert info["num_combine_items"] == 0 and all(s["part_base"] == -1 for s in segs)
     info, segs = _plan(pkg, [1000], 64, Hq=8, Hkv=2, min_splits=3)
@@ -198,6 +199,24 @@ def test_planner_small_and_forced_splits(pkg):
     for s in segs:
         by_group.setdefault(s["group"], 0); by_group[s["group"]] += 1
     assert all(v >= 3 for v in by_group.values())
+
+
+def test_planner_decode_plan(pkg):
+    """NEXT-4: n*G <= 128 packed rows per (session, KV head) -> decode plan: one CTA per team; the
+    even / odd KV-tile accumulator sets are merged inside the CTA, so partial slots and combine items
+    follow the general rule (only groups cut into several segments)."""
+    for lens, n, Hq, Hkv in (([65536], 1, 32, 8), ([65536], 16, 32, 8), ([4096, 100, 9000], 32, 32, 8),
+                             ([5000], 128, 16, 16), ([70], 4, 8, 2)):
+        info, segs = _plan(pkg, lens, n, Hq=Hq, Hkv=Hkv)
+        assert info["used_tensor_core_kernel"] == 3 and info["team_size"] == 1, (lens, n, info)
+        tiles = Hkv * sum((L + n + 127) // 128 for L in lens)
+        _check_cover(info, segs, tiles)
+        assert info["num_ctas"] <= 148
+    # one row more than a Q tile holds -> general plan; and the switch forces it
+    info, _ = _plan(pkg, [4096], 33, Hq=32, Hkv=8)
+    assert info["used_tensor_core_kernel"] == 1
+    info, _ = _plan(pkg, [4096], 16, Hq=32, Hkv=8, decode_plan=False)
+    assert info["used_tensor_core_kernel"] == 1
 
 
 def test_planner_multi_block_queries(pkg):

@@ -269,7 +269,7 @@ def test_multi_block_query_tensor_core():
     assert np.abs(lse.cpu().numpy() - l_ref).max() <= 1e-3
 
 
-def _prefill_case(block_sizes, Hq, Hkv, seed, L0=0):
+def _prefill_case(block_sizes, Hq, Hkv, seed, L0=0, expect_kernel=1, min_splits=0):
     """one session: optional committed cache of L0 tokens, then `block_sizes` appended and queried in
     ONE call (num_q_blocks = len(block_sizes)); returns (gpu O, gpu LSE, oracle O, oracle LSE)."""
     import torch
@@ -282,6 +282,8 @@ def _prefill_case(block_sizes, Hq, Hkv, seed, L0=0):
     q, k, v = mk(T, Hq, 128), mk(T, Hkv, 128), mk(T, Hkv, 128)
     P = 64
     c = Cache(WS_BF16, Hq, Hkv, 128, P, (L0 + T) // P + 4, max_sessions=1, max_q_tokens_per_call=max(T, 256))
+    if min_splits:
+        c.set_min_splits(min_splits)
     sid = c.session_open()
     dev = torch.device("cuda", 0)
     sess = OracleSession(Hkv, 128)
@@ -299,7 +301,7 @@ def _prefill_case(block_sizes, Hq, Hkv, seed, L0=0):
     scale = 1.0 / math.sqrt(128)
     c.block_causal_attn_fwd([sid], [0, T], _torch_of(q, dev), out, scale, lse=lse, num_q_blocks=[len(block_sizes)])
     torch.cuda.synchronize()
-    assert c.last_plan_info()["used_tensor_core_kernel"] == 1
+    assert c.last_plan_info()["used_tensor_core_kernel"] == expect_kernel
     o_ref, l_ref = attend(sess, q, scale, len(block_sizes))
     return out.float().cpu().numpy(), lse.cpu().numpy(), o_ref, l_ref
 
@@ -319,6 +321,63 @@ def test_next1_multi_block_prefill(blocks, Hq, Hkv, L0):
     assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3
     assert np.sqrt((d ** 2).mean() / (o_ref ** 2).mean()) <= 1e-2
     assert np.abs(lse - l_ref).max() <= 1e-3
+
+
+# ------------------------------------------------------------------ NEXT-4: decode plan
+DECODE_CASES = [
+    # (label, overrides): n * G <= 128 packed rows -> decode plan (same Q tile, alternate KV tiles)
+    ("n1_gqa4", dict(cache_lens=(1000,), num_q_heads=32, num_kv_heads=8, block_tokens=1, modality_split=(0, 0, 1), steps=3)),
+    ("n4_gqa4_ragged", dict(cache_lens=(777,), num_q_heads=32, num_kv_heads=8, block_tokens=4, modality_split=(0, 0, 4), steps=2)),
+    ("n16_gqa4_long", dict(cache_lens=(20001,), num_q_heads=32, num_kv_heads=8, block_tokens=16, modality_split=(0, 0, 16), steps=3)),
+    ("n32_gqa4_full_tile", dict(cache_lens=(130,), num_q_heads=32, num_kv_heads=8, block_tokens=32, modality_split=(24, 6, 2))),
+    ("n16_gqa8_full_tile", dict(cache_lens=(531,), num_q_heads=8, num_kv_heads=1, block_tokens=16, modality_split=(12, 3, 1))),
+    ("n128_mha", dict(cache_lens=(2048,), num_q_heads=4, num_kv_heads=4, block_tokens=128, modality_split=(96, 24, 8))),
+    ("n3_empty_cache_single_tile", dict(cache_lens=(0,), num_q_heads=8, num_kv_heads=2, block_tokens=3, modality_split=(1, 1, 1), steps=2)),
+    ("n8_two_tiles", dict(cache_lens=(150,), num_q_heads=8, num_kv_heads=2, block_tokens=8, modality_split=(4, 3, 1))),
+]
+
+
+@pytest.mark.parametrize("label,ov", DECODE_CASES, ids=[x[0] for x in DECODE_CASES])
+def test_next4_decode_plan_matches_oracle(label, ov):
+    """NEXT-4 (PAPER.md:31, :77 token-causal text pass): few query rows per KV head, cache-read bound.
+    The scheduler picks the decode plan; results must match the oracle exactly as on the general plan,
+    and the general plan (forced) must agree too."""
+    w = _small(2, **ov)
+    ref = run_workload_oracle(w)
+    got = run_workload_gpu(w, pool_fill=0x7FC1)
+    assert all(pl["used_tensor_core_kernel"] == 3 for pl in got["plans"]), got["plans"]
+    _assert_close(compare(got, ref, "bf16"), BF16_TOL, label + " (decode plan)")
+    gen = run_workload_gpu(w, pool_fill=0x7FC1, decode_plan=False, gather=False)
+    assert all(pl["used_tensor_core_kernel"] == 1 for pl in gen["plans"])
+    _assert_close(compare(gen, ref, "bf16"), BF16_TOL, label + " (general plan)")
+
+
+@pytest.mark.parametrize("splits", [1, 2, 5, 40])
+def test_next4_decode_plan_split_count_invariance(splits):
+    w = _small(3, cache_lens=(6000,), block_tokens=16, modality_split=(12, 3, 1), steps=1)
+    got = run_workload_gpu(w, min_splits=splits, gather=False)
+    pl = got["plans"][-1]
+    assert pl["used_tensor_core_kernel"] == 3 and pl["num_segments"] >= 8 * min(splits, 20)
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, f"decode splits={splits}")
+
+
+@pytest.mark.parametrize("n,Hq,Hkv,L0,splits", [(16, 32, 8, 3000, 0), (9, 8, 2, 120, 0), (32, 4, 4, 1000, 3), (5, 16, 2, 0, 0)])
+def test_next4_token_causal_decode(n, Hq, Hkv, L0, splits):
+    """Token-causal decode = blocks of ONE token (reading A4): n tokens committed as n blocks
+    and queried in one call; row i sees the history plus tokens 0..i of the call."""
+    o, lse, o_ref, l_ref = _prefill_case([1] * n, Hq, Hkv, seed=100 + n, L0=L0, expect_kernel=3, min_splits=splits)
+    d = o - o_ref
+    assert np.isfinite(o).all() and np.isfinite(lse).all()
+    assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3
+    assert np.abs(lse - l_ref).max() <= 1e-3
+
+
+def test_next4_decode_ragged_multi_session():
+    w = _small(5, cache_lens=(700, 1300, 2081, 90, 1500, 333, 2600, 1024), block_tokens=8, modality_split=(4, 3, 1), steps=2)
+    got = run_workload_gpu(w)
+    assert all(pl["used_tensor_core_kernel"] == 3 for pl in got["plans"])
+    tol = dict(BF16_TOL); tol.pop("max_abs"); tol["max_excess"] = 8e-3
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), tol, "decode ragged multi-session")
 
 
 # ------------------------------------------------------------------ NEXT-2: solver-step mode
@@ -454,12 +513,15 @@ def test_graph_capture_ragged_multi_session_uses_large_parameter_tier():
     o = out.float().cpu().numpy().astype(np.float64).reshape(S, n, sp.num_q_heads, sp.head_dim)
     for s in range(S):
         d = o[s] - ref["out"][0][s]
-        assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3, s
+        # short caches + x8 outlier channels: |O| reaches ~4, gate the error in excess of the bf16
+        # output rounding (see test_ragged_multi_session_small_and_batched_equals_single)
+        assert (np.abs(d) - 2.0 ** -8 * np.abs(ref["out"][0][s])).max() <= 8e-3 and np.abs(d).mean() <= 1e-3, s
 
 
 # ------------------------------------------------------------------ closed-form pins on the GPU
-def _run_custom_bf16(L, n, Hq, Hkv, kc, vc, q, kn, vn, scale, min_splits=0):
-    """single session, cache (kc, vc) then one block (kn, vn) with queries q; returns (O, LSE)."""
+def _run_custom_bf16(L, n, Hq, Hkv, kc, vc, q, kn, vn, scale, min_splits=0, decode_plan=True):
+    """single session, cache (kc, vc) then one block (kn, vn) with queries q; returns (O, LSE).
+    decode_plan=False forces the general plan where the decode plan (n * G <= 128) would apply."""
     import torch
     from paper_2606_25041_b200 import WS_BF16, Cache
     P = 64
@@ -467,6 +529,7 @@ def _run_custom_bf16(L, n, Hq, Hkv, kc, vc, q, kn, vn, scale, min_splits=0):
     c = Cache(WS_BF16, Hq, Hkv, 128, P, pages, max_sessions=1, max_q_tokens_per_call=max(n, 256))
     if min_splits:
         c.set_min_splits(min_splits)
+    c.set_decode_plan(decode_plan)
     sid = c.session_open()
     dev = torch.device("cuda", 0)
     pos = 0
@@ -478,12 +541,14 @@ def _run_custom_bf16(L, n, Hq, Hkv, kc, vc, q, kn, vn, scale, min_splits=0):
     lse = torch.empty((n, Hq), dtype=torch.float32, device=dev)
     c.block_causal_attn_fwd([sid], [0, n], _torch_of(q, dev), out, scale, lse=lse)
     torch.cuda.synchronize()
-    assert c.last_plan_info()["used_tensor_core_kernel"] == 1
+    assert c.last_plan_info()["used_tensor_core_kernel"] == (3 if decode_plan and n * (Hq // Hkv) <= 128 else 1)
     return out.float().cpu().numpy(), lse.cpu().numpy(), c.last_plan_segments()
 
 
-def test_needle_addressing_every_boundary():
-    """P3: q = u, K[j*] = 4u, all other K = 0, V rows distinct -> O == V[j*] exactly (bf16)."""
+@pytest.mark.parametrize("decode_plan", [False, True], ids=["general_plan", "decode_plan"])
+def test_needle_addressing_every_boundary(decode_plan):
+    """P3: q = u, K[j*] = 4u, all other K = 0, V rows distinct -> O == V[j*] exactly (bf16).
+    n * G = 128 packed rows: run on the general plan (forced) and on the decode plan."""
     L, n, Hq, Hkv = 1000 + 37, 64, 4, 2
     rng = np.random.default_rng(3)
     u = rng.choice([-1.0, 1.0], size=128).astype(np.float32)
@@ -491,7 +556,8 @@ def test_needle_addressing_every_boundary():
     q = to_bf16(np.tile(u, (n, Hq, 1)))
     scale = 1.0 / math.sqrt(128)
     _, _, segs = _run_custom_bf16(L, n, Hq, Hkv, to_bf16(np.zeros((L, Hkv, 128), np.float32)), v_all[:L], q,
-                                  to_bf16(np.zeros((n, Hkv, 128), np.float32)), v_all[L:], scale, min_splits=3)
+                                  to_bf16(np.zeros((n, Hkv, 128), np.float32)), v_all[L:], scale, min_splits=3,
+                                  decode_plan=decode_plan)
     cuts = sorted({s["tile_begin"] * 128 for s in segs} | {s["tile_end"] * 128 for s in segs})
     targets = {0, 63, 64, 127, 128, L - 1, L, L + n - 1, L + n - 2}
     for cpos in cuts:
@@ -500,7 +566,8 @@ def test_needle_addressing_every_boundary():
         k_all = np.zeros((L + n, Hkv, 128), np.float32)
         k_all[jstar] = 4.0 * u
         k_all = to_bf16(k_all)
-        o, lse, _ = _run_custom_bf16(L, n, Hq, Hkv, k_all[:L], v_all[:L], q, k_all[L:], v_all[L:], scale, min_splits=3)
+        o, lse, _ = _run_custom_bf16(L, n, Hq, Hkv, k_all[:L], v_all[:L], q, k_all[L:], v_all[L:], scale, min_splits=3,
+                                     decode_plan=decode_plan)
         want = v_all[jstar].astype(np.float32)                 # [Hkv, 128]
         for h in range(Hq):
             np.testing.assert_array_equal(o[:, h, :], np.tile(want[h // 2], (n, 1)), err_msg=f"j*={jstar}")
@@ -530,14 +597,15 @@ def test_large_scores_do_not_overflow():
     assert err["finite"] and err["max_abs"] <= 2e-2 and err["rel_rms"] <= 1e-2, err
 
 
+@pytest.mark.parametrize("n", [128, 64], ids=["general_plan", "decode_plan"])
 @pytest.mark.parametrize("kind", ["ramp", "jump_second_half", "jump_first_half", "late_outlier"])
-def test_growing_scores_exercise_every_rescale_path(kind):
+def test_growing_scores_exercise_every_rescale_path(kind, n):
     """Scores that keep outgrowing the running reference: ramps (every half tile rescales), a jump of
     +230 (log2 units) inside the second / first half of a tile after that tile's other half was fine
     (the optimistic fast path must recover, incl. the O rescale after an already handed-off half),
     and a single huge late key.  Compared with the oracle; nothing may overflow."""
     from oracle.block_causal import OracleSession, attend
-    L, n, Hq, Hkv = 1280, 128, 4, 2
+    L, Hq, Hkv = 1280, 4, 2
     rng = np.random.default_rng(17)
     u = rng.choice([-1.0, 1.0], size=128).astype(np.float32)
     N = L + n
