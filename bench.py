@@ -157,6 +157,7 @@ def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, r
         g.replay()
     ms = timed(reps, lambda i: g.replay())
     L = cache.session_info(ids[0])[0]
+    w_cache_len = L - sp.block_tokens
     fl = 4.0 * sp.head_dim * sp.num_q_heads * sp.block_tokens * sum(cache.session_info(i)[0] for i in ids)
     res["solver_step_cuda_graph"] = {"us_per_step": 1e3 * ms / reps, "tflops": fl / (ms / reps * 1e-3) / 1e12,
                                      "kv_tokens": L, "replays": reps,
@@ -183,6 +184,40 @@ def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, r
                                   "tflops": fl / (ms / reps * 1e-3) / 1e12,
                                   "what": "32 committed blocks of 256 tokens queried in one call (block-causal FLOPs)"}
     c2.close()
+    # --- NEXT-4: decode steps (n * G <= 128 packed rows: cache-read bound, decode plan) on the headline
+    # session: n new tokens appended + attended against the 65,536-token history.  History (269 MB)
+    # exceeds L2, so every replay reads it from HBM.  Roofline = algorithmic bytes / measured HBM GB/s.
+    peaks, _ = load_peaks()
+    res["decode_step"] = []
+    for n_dec in ((1, 16) if len(ids) == 1 else ()):
+        reset()
+        kd, vd, qd = k0[:n_dec].contiguous(), v0[:n_dec].contiguous(), q0[:n_dec].contiguous()
+        od = torch.empty_like(qd)
+        cud = [0, n_dec]
+        cache.kv_append(ids, cud, kd, vd); cache.block_causal_attn_fwd(ids, cud, qd, od, sp.scale)
+        plan = cache.last_plan_info()
+        reset()
+        torch.cuda.synchronize()
+        gd = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(gd):
+            cache.kv_append(ids, cud, kd, vd)
+            cache.block_causal_attn_fwd(ids, cud, qd, od, sp.scale)
+        for _ in range(5):
+            gd.replay()
+        reps = 200
+        ms = timed(reps, lambda i: gd.replay())
+        reset()
+        Lk = w_cache_len + n_dec
+        eb = 2
+        byts = 2 * eb * sp.num_kv_heads * sp.head_dim * Lk + 2 * eb * sp.num_q_heads * sp.head_dim * n_dec \
+            + 4 * eb * sp.num_kv_heads * sp.head_dim * n_dec
+        us = 1e3 * ms / reps
+        res["decode_step"].append({
+            "new_tokens": n_dec, "kv_tokens": Lk, "us_per_step": us, "algorithmic_bytes": byts,
+            "hbm_gbs": byts / us / 1e3, "hbm_peak_gbs": float(peaks["hbm_gbs"]),
+            "frac_of_hbm_roofline": byts / us / 1e3 / float(peaks["hbm_gbs"]),
+            "kernel": plan["used_tensor_core_kernel"],
+            "what": "append + attention (decode plan) + combine, CUDA-graph replay, history read from HBM"})
     return res
 
 
