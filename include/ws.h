@@ -157,6 +157,62 @@ ws_status_t ws_stream_host_join(ws_cache_t* cache, void* cuda_stream);
 ws_status_t ws_fm_euler_update(int32_t dtype, void* z, const void* v, float dtau, int64_t count,
                                void* cuda_stream);
 
+/* ---- NEXT-3: replica link - the thinker -> performer KV-slice exchange ---------------------------
+ * PAPER.md:75 "After system prefill, the thinker broadcasts the initial KV cache to the performer";
+ * :77 / :31 the thinker produces "the current KV-cache slice" every unit; :83 the performer "appends the
+ * received KV slice into its own full-history cache"; :85 "KV-cache exchange".  Thinker and performer
+ * hold full REPLICAS of the cache (not shards).  B200-native form: the owner (thinker) links its cache
+ * to the replicas' pools mapped into its own address space (CUDA peer access in one process, or
+ * cudaIpcOpenMemHandle across processes - NVLink 5 / NVSwitch carries plain stores), and from then on
+ * the ONE kv_append kernel pass that commits a slice locally also stores it into every linked pool at
+ * the same physical page ids (one read of k_new/v_new, local + peer 16-byte stores, system-scope fence).
+ * No staging buffer, no separate send/recv, no second kernel on the replica's GPU.  The host-side
+ * commit (block boundary, page adoption) travels as a small int32 message over any transport
+ * (torch.distributed send/recv in the harness) and is applied by ws_replica_apply.
+ *
+ * Page ownership: a replica calls ws_replica_accept(owner_pages) once, before opening sessions: pages
+ * [0, owner_pages) are then handed out only by ws_replica_apply (the owner names them); the replica's
+ * own appends (solver-step staging, NEXT-2) draw from pages >= owner_pages, so an in-flight peer
+ * write can never land in a page the replica is using for something else.
+ *
+ * Ordering contract (the transport's job): a message may be applied - more precisely, work that reads
+ * the new tokens may be enqueued on the replica - only after the owner's append kernel has completed
+ * (stream synchronised before the send, or an interprocess event waited on by the replica's stream);
+ * and the owner must not append to a session while the replica still holds a staged (uncommitted)
+ * block of it whose first tokens share the session's last page. */
+typedef struct {
+  void*  k_pool;        /* replica's K pool as addressable from the OWNER's device                    */
+  void*  v_pool;
+  size_t pool_bytes;    /* each; must be >= ws_pool_bytes(owner cfg) (same Hkv, P, D, dtype assumed)  */
+} ws_peer_pools_t;
+enum { WS_MAX_PEERS = 4 };
+/* Owner side.  num_peers = 0 unlinks.  Does not touch the peers' memory. */
+ws_status_t ws_replica_link(ws_cache_t* owner, const ws_peer_pools_t* peers, int32_t num_peers);
+/* Replica side: reserve pages [0, owner_pages) for the owner.  No session may be open. */
+ws_status_t ws_replica_accept(ws_cache_t* replica, int32_t owner_pages);
+/* Owner side: serialise the commit of the LAST ws_kv_append call (or, for ws_replica_snapshot_message,
+ * the whole current state of one session: every block end and page id - the "initial KV cache" message
+ * after system prefill).  words: HOST int32[cap]; *n = words needed (WS_ERR_INVALID_ARG if cap < *n,
+ * with *n still set, so a NULL/0 query works). */
+ws_status_t ws_replica_commit_message(const ws_cache_t* owner, int32_t* words, int32_t cap, int32_t* n);
+ws_status_t ws_replica_snapshot_message(const ws_cache_t* owner, int32_t session, int32_t* words,
+                                        int32_t cap, int32_t* n);
+/* Owner side: copy every page of `session` into the linked pools at the same page ids (the data half
+ * of the initial broadcast; page-granular 16-byte copies, HBM read + NVLink write bound). */
+ws_status_t ws_replica_push_session(ws_cache_t* owner, int32_t session, void* cuda_stream);
+/* Replica side: validate a message against the replica's state (session at the stated length - or
+ * not yet open and starting from 0, then it is opened at the owner's id; named pages inside the
+ * accepted range and free; capacities) and, only if everything checks, adopt the pages, record the
+ * block boundaries and publish the page ids to the device page table (a small kernel on cuda_stream,
+ * CUDA-graph capturable).  The K/V bytes themselves were already stored by the owner's kernel. */
+ws_status_t ws_replica_apply(ws_cache_t* replica, const int32_t* words, int32_t n, void* cuda_stream);
+/* Interprocess mapping helpers (thin wrappers over cudaIpcGetMemHandle / cudaIpcOpenMemHandle that
+ * also handle pointers inside a larger allocation, e.g. a torch caching-allocator segment).
+ * handle: HOST 64 bytes.  ws_ipc_close takes the pointer ws_ipc_open returned. */
+ws_status_t ws_ipc_export(const void* device_ptr, uint8_t* handle64, uint64_t* offset);
+ws_status_t ws_ipc_open(const uint8_t* handle64, uint64_t offset, int32_t device, void** ptr_out);
+ws_status_t ws_ipc_close(void* ptr, uint64_t offset);
+
 /* Read back logical tokens [start, start+count) of a session into contiguous [count][Hkv][D]
  * DEVICE buffers (either may be NULL).  Test / snapshot utility. */
 ws_status_t ws_kv_gather(const ws_cache_t* cache, int32_t session, int64_t start, int64_t count,

@@ -51,7 +51,13 @@ class PlanSegment(C.Structure):
                                          "tile_end", "team", "part_base")]
 
 
-EXPORTS = ["ws_pool_bytes", "ws_workspace_bytes", "ws_cache_create", "ws_cache_destroy",
+class PeerPools(C.Structure):
+    _fields_ = [("k_pool", C.c_void_p), ("v_pool", C.c_void_p), ("pool_bytes", C.c_size_t)]
+
+
+EXPORTS = ["ws_replica_link", "ws_replica_accept", "ws_replica_commit_message",
+           "ws_replica_snapshot_message", "ws_replica_push_session", "ws_replica_apply",
+           "ws_ipc_export", "ws_ipc_open", "ws_ipc_close", "ws_pool_bytes", "ws_workspace_bytes", "ws_cache_create", "ws_cache_destroy",
            "ws_session_open", "ws_session_close", "ws_session_info", "ws_session_truncate",
            "ws_free_pages", "ws_kv_append", "ws_block_causal_attn_fwd", "ws_step_staging_bytes",
            "ws_stream_step_host", "ws_stream_host_join", "ws_fm_euler_update", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
@@ -93,6 +99,15 @@ def load_library() -> C.CDLL:
     lib.ws_stream_host_join.argtypes = [vp, vp]
     lib.ws_fm_euler_update.argtypes = [C.c_int32, vp, vp, C.c_float, C.c_int64, vp]
     lib.ws_kv_gather.argtypes = [vp, C.c_int32, C.c_int64, C.c_int64, vp, vp, vp]
+    lib.ws_replica_link.argtypes = [vp, C.POINTER(PeerPools), C.c_int32]
+    lib.ws_replica_accept.argtypes = [vp, C.c_int32]
+    lib.ws_replica_commit_message.argtypes = [vp, i32p, C.c_int32, i32p]
+    lib.ws_replica_snapshot_message.argtypes = [vp, C.c_int32, i32p, C.c_int32, i32p]
+    lib.ws_replica_push_session.argtypes = [vp, C.c_int32, vp]
+    lib.ws_replica_apply.argtypes = [vp, i32p, C.c_int32, vp]
+    lib.ws_ipc_export.argtypes = [vp, C.POINTER(C.c_uint8), C.POINTER(C.c_uint64)]
+    lib.ws_ipc_open.argtypes = [C.POINTER(C.c_uint8), C.c_uint64, C.c_int32, C.POINTER(vp)]
+    lib.ws_ipc_close.argtypes = [vp, C.c_uint64]
     lib.ws_session_pages.argtypes = [vp, C.c_int32, i32p, C.c_int32, i32p]
     lib.ws_debug_shuffle_free_pages.argtypes = [vp, C.c_uint64]
     lib.ws_debug_set_min_splits.argtypes = [vp, C.c_int32]
@@ -257,6 +272,47 @@ class Cache:
         _check(self.lib.ws_kv_gather(self.handle, session, start, count, _ptr(k_out), _ptr(v_out),
                                      _stream_ptr(stream)))
 
+    # ---- NEXT-3 replica link (thinker -> performer KV-slice exchange)
+    def pool_bytes(self) -> int:
+        return self.lib.ws_pool_bytes(C.byref(self.cfg))
+
+    def replica_link(self, peers) -> None:
+        """peers: list of Cache objects (same process) or (k_ptr, v_ptr, pool_bytes) tuples (mapped pools)."""
+        arr = (PeerPools * max(1, len(peers)))()
+        for i, pr in enumerate(peers):
+            if isinstance(pr, Cache):
+                if pr.dry:
+                    arr[i].k_pool, arr[i].v_pool, arr[i].pool_bytes = None, None, pr.pool_bytes()
+                else:
+                    arr[i].k_pool, arr[i].v_pool = pr.k_pool.data_ptr(), pr.v_pool.data_ptr()
+                    arr[i].pool_bytes = pr.k_pool.numel() * pr.k_pool.element_size()
+            else:
+                arr[i].k_pool, arr[i].v_pool, arr[i].pool_bytes = pr
+        _check(self.lib.ws_replica_link(self.handle, arr, len(peers)))
+
+    def replica_accept(self, owner_pages: int) -> None:
+        _check(self.lib.ws_replica_accept(self.handle, owner_pages))
+
+    def _message(self, fn, *args) -> np.ndarray:
+        n = C.c_int32()
+        fn(self.handle, *args, None, 0, C.byref(n))          # size query (fails with INVALID_ARG by design)
+        buf = (C.c_int32 * max(1, n.value))()
+        _check(fn(self.handle, *args, buf, n.value, C.byref(n)))
+        return np.frombuffer(buf, dtype=np.int32, count=n.value).copy()
+
+    def replica_commit_message(self) -> np.ndarray:
+        return self._message(self.lib.ws_replica_commit_message)
+
+    def replica_snapshot_message(self, session: int) -> np.ndarray:
+        return self._message(self.lib.ws_replica_snapshot_message, session)
+
+    def replica_push_session(self, session: int, stream=None) -> None:
+        _check(self.lib.ws_replica_push_session(self.handle, session, _stream_ptr(stream)))
+
+    def replica_apply(self, words, stream=None) -> None:
+        w = np.ascontiguousarray(np.asarray(words, dtype=np.int32))
+        _check(self.lib.ws_replica_apply(self.handle, _i32(w), len(w), _stream_ptr(stream)))
+
     # ---- introspection / debug
     def shuffle_free_pages(self, seed: int) -> None:
         _check(self.lib.ws_debug_shuffle_free_pages(self.handle, seed))
@@ -321,6 +377,24 @@ def ws_fm_euler_update(z, v, dtau: float, stream=None):
         raise ValueError("z and v must have the same dtype and size")
     dt = {torch.bfloat16: WS_BF16, torch.float32: WS_F32}[z.dtype]
     _check(load_library().ws_fm_euler_update(dt, _ptr(z), _ptr(v), C.c_float(dtau), z.numel(), _stream_ptr(stream)))
+
+
+def ws_ipc_export(tensor_or_ptr):
+    """(handle: bytes[64], offset) for a device pointer, to be opened in another process."""
+    h, off = (C.c_uint8 * 64)(), C.c_uint64()
+    _check(load_library().ws_ipc_export(_ptr(tensor_or_ptr), h, C.byref(off)))
+    return bytes(h), off.value
+
+
+def ws_ipc_open(handle: bytes, offset: int, device: int = 0) -> int:
+    out = C.c_void_p()
+    h = (C.c_uint8 * 64).from_buffer_copy(handle)
+    _check(load_library().ws_ipc_open(h, offset, device, C.byref(out)))
+    return out.value
+
+
+def ws_ipc_close(ptr: int, offset: int) -> None:
+    _check(load_library().ws_ipc_close(ptr, offset))
 
 
 def ws_version() -> str:

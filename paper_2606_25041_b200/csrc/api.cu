@@ -132,6 +132,9 @@ struct ws_cache {
   bool timing = false;
   std::vector<cudaEvent_t> ev_pool;                       // reusable events
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> t_append, t_attn, t_combine;
+  // NEXT-3 replica link
+  ws::PeerPools peers{};
+  std::vector<int32_t> last_commit;   // message describing the last ws_kv_append (ws_replica_commit_message)
 };
 
 namespace {
@@ -190,6 +193,26 @@ struct TimedLaunch {
     if (c->timing && e0 && e1) { cudaEventRecord(e1, st); dst->emplace_back(e0, e1); }
   }
 };
+
+// ---- NEXT-3 commit messages (include/ws.h): int32 words
+//   [0] magic  [1] version  [2] kind  [3] sessions  [4] total words  [5] P  [6] Hkv  [7] D  [8] dtype
+//   then per session: id, len_old, nblocks, npages, block_len[nblocks], page_id[npages]
+constexpr int32_t kMsgMagic = 0x57534b56, kMsgVersion = 1, kMsgCommit = 1, kMsgSnapshot = 2;
+constexpr int kMsgTotalWord = 4, kMsgHeaderWords = 9;
+void msg_begin(const ws_cache* c, std::vector<int32_t>& msg, int32_t kind, int32_t S) {
+  msg.clear();
+  msg.insert(msg.end(), {kMsgMagic, kMsgVersion, kind, S, 0, c->cfg.page_tokens, c->cfg.num_kv_heads,
+                         c->cfg.head_dim, c->cfg.dtype});
+}
+
+ws_status_t copy_message(const std::vector<int32_t>& msg, int32_t* words, int32_t cap, int32_t* n) {
+  if (!n) return fail(WS_ERR_INVALID_ARG, "n is NULL");
+  *n = (int32_t)msg.size();
+  if (msg.empty()) return fail(WS_ERR_INVALID_ARG, "no append has been made on this cache yet");
+  if (!words || cap < *n) return fail(WS_ERR_INVALID_ARG, "message needs %d words, cap is %d", *n, cap);
+  memcpy(words, msg.data(), msg.size() * 4);
+  return WS_OK;
+}
 
 ws_status_t encode_tmap(ws_cache* c, CUtensorMap* out, void* base, int rank, const cuuint64_t* dims,
                         const cuuint64_t* strides_bytes, const cuuint32_t* box) {
@@ -452,14 +475,20 @@ ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
   ws::AppendSession* as = (ws::AppendSession*)(blob + hdr.off_sessions);
   int32_t* pages = blob + hdr.off_pages;
   int32_t npg = 0;
+  std::vector<int32_t>& msg = c->last_commit;
+  msg_begin(c, msg, kMsgCommit, S);
   for (int32_t s = 0; s < S; ++s) {
     int32_t id = session_ids[s], n = cu[s + 1] - cu[s];
     int64_t len_old = c->host->session(id).tokens;
+    const size_t old_pages = c->host->session(id).pages.size();
     int32_t first = c->host->commit_block(id, n, modality ? modality + cu[s] : nullptr);
     const ws::SessionState& ss = c->host->session(id);
     as[s] = ws::AppendSession{id, (int32_t)len_old, cu[s], cu[s + 1], npg, {0, 0, 0}};
     for (size_t i = first; i < ss.pages.size(); ++i) pages[npg++] = ss.pages[i];
+    msg.insert(msg.end(), {id, (int32_t)len_old, 1, (int32_t)(ss.pages.size() - old_pages), n});
+    msg.insert(msg.end(), ss.pages.begin() + old_pages, ss.pages.end());
   }
+  msg[kMsgTotalWord] = (int32_t)msg.size();
   memcpy(blob, &hdr, sizeof(hdr));
   if (c->dry) return WS_OK;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
@@ -469,7 +498,7 @@ ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
   }
   TimedLaunch tl(c, &c->t_append, stream);
   WS_CUDA(ws::launch_kv_append(k_new, v_new, c->cfg.k_pool, c->cfg.v_pool, c->d_page_table,
-                               inline_meta ? nullptr : (const int32_t*)d, inl, cu[S], c->cfg.max_pages_per_session, P,
+                               inline_meta ? nullptr : (const int32_t*)d, inl, c->peers, cu[S], c->cfg.max_pages_per_session, P,
                                c->cfg.num_kv_heads, c->cfg.head_dim, eb_of(c->cfg.dtype), c->num_sms,
                                stream));
   tl.done();
@@ -696,6 +725,177 @@ ws_status_t ws_fm_euler_update(int32_t dtype, void* z, const void* v, float dtau
   if (((uintptr_t)z & 15) || ((uintptr_t)v & 15)) return fail(WS_ERR_INVALID_ARG, "z / v must be 16-byte aligned");
   if (!std::isfinite(dtau)) return fail(WS_ERR_INVALID_ARG, "dtau must be finite");
   WS_CUDA(ws::launch_fm_euler(dtype, z, v, dtau, count, (cudaStream_t)cuda_stream));
+  return WS_OK;
+}
+
+// ------------------------------------------------------------------------------------ NEXT-3
+ws_status_t ws_replica_link(ws_cache_t* c, const ws_peer_pools_t* peers, int32_t num_peers) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  if (num_peers < 0 || num_peers > WS_MAX_PEERS || (num_peers > 0 && !peers))
+    return fail(WS_ERR_INVALID_ARG, "num_peers %d not in [0, %d]", num_peers, (int)WS_MAX_PEERS);
+  ws::PeerPools pp{};
+  for (int32_t r = 0; r < num_peers; ++r) {
+    if (!c->dry) {
+      if (!peers[r].k_pool || !peers[r].v_pool) return fail(WS_ERR_INVALID_ARG, "peer %d: NULL pool", r);
+      if (((uintptr_t)peers[r].k_pool & 15) || ((uintptr_t)peers[r].v_pool & 15))
+        return fail(WS_ERR_INVALID_ARG, "peer %d: pools must be 16-byte aligned", r);
+      if (peers[r].k_pool == c->cfg.k_pool || peers[r].v_pool == c->cfg.v_pool)
+        return fail(WS_ERR_INVALID_ARG, "peer %d is the cache's own pool", r);
+    }
+    if (peers[r].pool_bytes < ws_pool_bytes(&c->cfg))
+      return fail(WS_ERR_INVALID_ARG, "peer %d: pool_bytes %zu < the owner's %zu", r, peers[r].pool_bytes,
+                  ws_pool_bytes(&c->cfg));
+    pp.k[r] = peers[r].k_pool; pp.v[r] = peers[r].v_pool;
+  }
+  pp.n = num_peers;
+  c->peers = pp;
+  return WS_OK;
+}
+
+ws_status_t ws_replica_accept(ws_cache_t* c, int32_t owner_pages) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  if (owner_pages < 0 || owner_pages > c->cfg.num_pages)
+    return fail(WS_ERR_INVALID_ARG, "owner_pages %d not in [0, %d]", owner_pages, c->cfg.num_pages);
+  if (!c->host->reserve_owner_pages(owner_pages))
+    return fail(WS_ERR_INVALID_ARG, "ws_replica_accept needs every session closed");
+  return WS_OK;
+}
+
+ws_status_t ws_replica_commit_message(const ws_cache_t* c, int32_t* words, int32_t cap, int32_t* n) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  return copy_message(c->last_commit, words, cap, n);
+}
+
+ws_status_t ws_replica_snapshot_message(const ws_cache_t* c, int32_t session, int32_t* words,
+                                        int32_t cap, int32_t* n) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  if (!c->host->is_open(session)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", session);
+  const ws::SessionState& ss = c->host->session(session);
+  if (ss.block_ends.empty()) return fail(WS_ERR_INVALID_ARG, "session %d has no committed block", session);
+  std::vector<int32_t> msg;
+  msg_begin(c, msg, kMsgSnapshot, 1);
+  msg.insert(msg.end(), {session, 0, (int32_t)ss.block_ends.size(), (int32_t)ss.pages.size()});
+  int64_t prev = 0;
+  for (int64_t e : ss.block_ends) { msg.push_back((int32_t)(e - prev)); prev = e; }
+  msg.insert(msg.end(), ss.pages.begin(), ss.pages.end());
+  msg[kMsgTotalWord] = (int32_t)msg.size();
+  return copy_message(msg, words, cap, n);
+}
+
+ws_status_t ws_replica_push_session(ws_cache_t* c, int32_t session, void* cuda_stream) {
+  if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  if (!c->host->is_open(session)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", session);
+  if (c->peers.n == 0) return fail(WS_ERR_INVALID_ARG, "no replica is linked (ws_replica_link)");
+  const ws::SessionState& ss = c->host->session(session);
+  if (c->dry || ss.pages.empty()) return WS_OK;
+  const int64_t page_bytes = (int64_t)c->cfg.num_kv_heads * c->cfg.page_tokens * c->cfg.head_dim * eb_of(c->cfg.dtype);
+  WS_CUDA(ws::launch_kv_push_pages(c->cfg.k_pool, c->cfg.v_pool, c->peers,
+                                   c->d_page_table + (int64_t)session * c->cfg.max_pages_per_session,
+                                   (int32_t)ss.pages.size(), page_bytes, c->num_sms, (cudaStream_t)cuda_stream));
+  c->launches += 1;
+  return WS_OK;
+}
+
+ws_status_t ws_replica_apply(ws_cache_t* c, const int32_t* w, int32_t n, void* cuda_stream) {
+  if (!c || !w) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  if (n < kMsgHeaderWords || w[0] != kMsgMagic) return fail(WS_ERR_INVALID_ARG, "not a commit message");
+  if (w[1] != kMsgVersion) return fail(WS_ERR_UNSUPPORTED, "message version %d (this library: %d)", w[1], kMsgVersion);
+  if (w[2] != kMsgCommit && w[2] != kMsgSnapshot) return fail(WS_ERR_INVALID_ARG, "unknown message kind %d", w[2]);
+  if (w[kMsgTotalWord] != n) return fail(WS_ERR_INVALID_ARG, "message says %d words, %d given", w[kMsgTotalWord], n);
+  if (w[5] != c->cfg.page_tokens || w[6] != c->cfg.num_kv_heads || w[7] != c->cfg.head_dim || w[8] != c->cfg.dtype)
+    return fail(WS_ERR_INVALID_ARG, "message geometry (P %d, Hkv %d, D %d, dtype %d) differs from this cache",
+                w[5], w[6], w[7], w[8]);
+  const int32_t S = w[3], P = c->cfg.page_tokens;
+  if (S < 1 || S > c->cfg.max_sessions) return fail(WS_ERR_INVALID_ARG, "message lists %d sessions", S);
+  // ---- pass 1: validate everything (no state changes)
+  struct Item { int32_t id, len_old, nblocks, npages; const int32_t* lens; const int32_t* pages; };
+  std::vector<Item> items;
+  std::vector<int32_t> seen_pages;
+  int32_t pos = kMsgHeaderWords;
+  for (int32_t s = 0; s < S; ++s) {
+    if (pos + 4 > n) return fail(WS_ERR_INVALID_ARG, "message truncated (session %d header)", s);
+    Item it{w[pos], w[pos + 1], w[pos + 2], w[pos + 3], nullptr, nullptr};
+    pos += 4;
+    if (it.nblocks < 1 || it.npages < 0 || it.len_old < 0 || (int64_t)pos + it.nblocks + it.npages > n)
+      return fail(WS_ERR_INVALID_ARG, "message truncated or malformed (session %d)", s);
+    it.lens = w + pos; it.pages = w + pos + it.nblocks;
+    pos += it.nblocks + it.npages;
+    if (it.id < 0 || it.id >= c->cfg.max_sessions) return fail(WS_ERR_BAD_SESSION, "session %d out of range", it.id);
+    for (const Item& o : items) if (o.id == it.id) return fail(WS_ERR_INVALID_ARG, "session %d listed twice", it.id);
+    int64_t have = 0, blocks = 0;
+    if (c->host->is_open(it.id)) {
+      have = c->host->session(it.id).tokens; blocks = (int64_t)c->host->session(it.id).block_ends.size();
+    }
+    if (have != it.len_old)
+      return fail(WS_ERR_INVALID_ARG, "session %d: replica holds %lld tokens, message continues from %d "
+                  "(a staged block must be rolled back first)", it.id, (long long)have, it.len_old);
+    int64_t total = it.len_old;
+    for (int32_t b = 0; b < it.nblocks; ++b) {
+      if (it.lens[b] < 1) return fail(WS_ERR_INVALID_ARG, "session %d: block of %d tokens", it.id, it.lens[b]);
+      total += it.lens[b];
+    }
+    if (total >= (1ll << 31)) return fail(WS_ERR_UNSUPPORTED, "session %d would exceed 2^31 tokens", it.id);
+    const int64_t need = (total + P - 1) / P, had = ((int64_t)it.len_old + P - 1) / P;
+    if (need - had != it.npages)
+      return fail(WS_ERR_INVALID_ARG, "session %d: %d pages named, %lld needed", it.id, it.npages, (long long)(need - had));
+    if (need > c->cfg.max_pages_per_session || blocks + it.nblocks > c->cfg.max_blocks_per_session)
+      return fail(WS_ERR_OUT_OF_PAGES, "session %d exceeds its page-table or block capacity", it.id);
+    for (int32_t i = 0; i < it.npages; ++i) {
+      if (!c->host->owner_page_free(it.pages[i]))
+        return fail(WS_ERR_OUT_OF_PAGES, "page %d is not a free owner page of this replica (ws_replica_accept: %d)",
+                    it.pages[i], c->host->owner_pages());
+      for (int32_t q : seen_pages) if (q == it.pages[i]) return fail(WS_ERR_INVALID_ARG, "page %d named twice", q);
+      seen_pages.push_back(it.pages[i]);
+    }
+    items.push_back(it);
+  }
+  if (pos != n) return fail(WS_ERR_INVALID_ARG, "message has %d trailing words", n - pos);
+  // ---- pass 2: adopt
+  for (const Item& it : items) {
+    if (!c->host->is_open(it.id)) c->host->open_session_at(it.id);
+    const int32_t first = (int32_t)c->host->session(it.id).pages.size();
+    c->host->adopt(it.id, it.lens, it.nblocks, it.pages, it.npages);
+    if (!c->dry && it.npages > 0) {
+      WS_CUDA(ws::launch_page_table_publish(c->d_page_table, it.pages, it.id, first, it.npages,
+                                            c->cfg.max_pages_per_session, (cudaStream_t)cuda_stream));
+      c->launches += (it.npages + ws::kInlineAppendWords - 1) / ws::kInlineAppendWords;
+    }
+  }
+  return WS_OK;
+}
+
+ws_status_t ws_ipc_export(const void* device_ptr, uint8_t* handle64, uint64_t* offset) {
+  if (!device_ptr || !handle64 || !offset) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  static_assert(sizeof(cudaIpcMemHandle_t) == 64, "handle size");
+  typedef CUresult (*RangeFn)(CUdeviceptr*, size_t*, CUdeviceptr);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  WS_CUDA(cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &qres));
+  if (!fn || qres != cudaDriverEntryPointSuccess) return fail(WS_ERR_CUDA, "cuMemGetAddressRange entry point not found");
+  CUdeviceptr base = 0; size_t size = 0;
+  CUresult r = ((RangeFn)fn)(&base, &size, (CUdeviceptr)(uintptr_t)device_ptr);
+  if (r != CUDA_SUCCESS) return fail(WS_ERR_CUDA, "cuMemGetAddressRange failed (%d)", (int)r);
+  cudaIpcMemHandle_t h;
+  WS_CUDA(cudaIpcGetMemHandle(&h, (void*)(uintptr_t)base));
+  memcpy(handle64, &h, 64);
+  *offset = (uint64_t)((uintptr_t)device_ptr - (uintptr_t)base);
+  return WS_OK;
+}
+
+ws_status_t ws_ipc_open(const uint8_t* handle64, uint64_t offset, int32_t device, void** ptr_out) {
+  if (!handle64 || !ptr_out) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  cudaIpcMemHandle_t h;
+  memcpy(&h, handle64, 64);
+  WS_CUDA(cudaSetDevice(device));
+  void* p = nullptr;
+  WS_CUDA(cudaIpcOpenMemHandle(&p, h, cudaIpcMemLazyEnablePeerAccess));
+  *ptr_out = (char*)p + offset;
+  return WS_OK;
+}
+
+ws_status_t ws_ipc_close(void* ptr, uint64_t offset) {
+  if (!ptr) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  WS_CUDA(cudaIpcCloseMemHandle((char*)ptr - offset));
   return WS_OK;
 }
 

@@ -28,7 +28,7 @@ int32_t HostCache::open_session() {
 bool HostCache::close_session(int32_t s) {
   if (!is_open(s)) return false;
   // return pages so that the lowest id is handed out first again
-  for (auto it = sess_[s].pages.rbegin(); it != sess_[s].pages.rend(); ++it) free_.push_back(*it);
+  for (auto it = sess_[s].pages.rbegin(); it != sess_[s].pages.rend(); ++it) release_page(*it);
   sess_[s] = SessionState();
   return true;
 }
@@ -70,11 +70,48 @@ bool HostCache::truncate_blocks(int32_t s, int32_t keep_blocks) {
   st.stable_tokens = std::min(st.stable_tokens, st.tokens);
   size_t keep_pages = (size_t)((st.tokens + P_ - 1) / P_);
   while (st.pages.size() > keep_pages) {
-    free_.push_back(st.pages.back());
+    release_page(st.pages.back());
     st.pages.pop_back();
   }
   if (st.modality.size() > (size_t)st.tokens) st.modality.resize((size_t)st.tokens);
   return true;
+}
+
+void HostCache::release_page(int32_t page) {
+  if (page < owner_pages_) owner_used_[page] = 0; else free_.push_back(page);
+}
+
+bool HostCache::reserve_owner_pages(int32_t owner_pages) {
+  const int32_t num_pages = (int32_t)free_.size();
+  for (const auto& s : sess_) if (s.open) return false;
+  // (no session open => every page is free, so free_.size() is the pool size)
+  int32_t total = num_pages + owner_pages_;
+  if (owner_pages < 0 || owner_pages > total) return false;
+  owner_pages_ = owner_pages;
+  owner_used_.assign((size_t)owner_pages, 0);
+  free_.clear();
+  for (int32_t i = total - 1; i >= owner_pages; --i) free_.push_back(i);
+  return true;
+}
+
+bool HostCache::open_session_at(int32_t s) {
+  if (s < 0 || s >= (int32_t)sess_.size() || sess_[s].open) return false;
+  sess_[s] = SessionState();
+  sess_[s].open = true;
+  return true;
+}
+
+void HostCache::adopt(int32_t s, const int32_t* block_lens, int32_t nblocks, const int32_t* pages,
+                      int32_t npages) {
+  SessionState& st = sess_[s];
+  for (int32_t i = 0; i < npages; ++i) {
+    owner_used_[pages[i]] = 1;
+    st.pages.push_back(pages[i]);
+  }
+  for (int32_t b = 0; b < nblocks; ++b) {
+    st.tokens += block_lens[b];
+    st.block_ends.push_back(st.tokens);
+  }
 }
 
 void HostCache::shuffle_free(uint64_t seed) {

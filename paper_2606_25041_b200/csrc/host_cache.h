@@ -37,15 +37,31 @@ class HostCache {
   int32_t commit_block(int32_t s, int64_t n, const uint8_t* modality);
   bool truncate_blocks(int32_t s, int32_t keep_blocks);
 
+  // ---- NEXT-3 replica side: pages [0, owner_pages) are handed out only by adopt()
+  // (the owner of the link names them); local appends draw from the rest.
+  bool reserve_owner_pages(int32_t owner_pages);   // false if a session is open or out of range
+  int32_t owner_pages() const { return owner_pages_; }
+  bool owner_page_free(int32_t page) const {
+    return page >= 0 && page < owner_pages_ && !owner_used_[page];
+  }
+  bool open_session_at(int32_t s);                 // open a specific slot (false if taken / invalid)
+  // Adopt `pages` (all owner_page_free) as the next logical pages of session s and commit the blocks
+  // whose lengths are given.  The caller has validated everything (strong guarantee lives in api.cu).
+  void adopt(int32_t s, const int32_t* block_lens, int32_t nblocks, const int32_t* pages, int32_t npages);
+
   void mark_all_stable() { for (auto& s : sess_) if (s.open) s.stable_tokens = s.tokens; }
   int32_t free_pages() const { return (int32_t)free_.size(); }
   void shuffle_free(uint64_t seed);
   int32_t page_tokens() const { return P_; }
   int32_t max_pages_per_session() const { return max_pages_; }
   int32_t max_sessions() const { return (int32_t)sess_.size(); }
+  int32_t max_blocks_per_session() const { return max_blocks_; }
 
  private:
+  void release_page(int32_t page);
   int32_t P_, max_pages_, max_blocks_;
+  int32_t owner_pages_ = 0;
+  std::vector<uint8_t> owner_used_;  // [owner_pages_]
   std::vector<SessionState> sess_;
   std::vector<int32_t> free_;        // stack: back() is handed out next
 };

@@ -16,7 +16,7 @@ __global__ void __launch_bounds__(256)
 kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
                  int4* __restrict__ k_pool, int4* __restrict__ v_pool,
                  int32_t* __restrict__ page_table, const int32_t* __restrict__ meta_g,
-                 const __grid_constant__ InlineAppendMeta inl,
+                 const __grid_constant__ InlineAppendMeta inl, const PeerPools peers,
                  int32_t max_pages, int32_t P, int32_t Hkv, int32_t chunks_per_head) {
   // Nothing this kernel touches is produced by its stream predecessor (the previous step's combine
   // writes only `out`), so the successor (this step's attention) may start its prologue right away.
@@ -54,8 +54,12 @@ kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
     int32_t head = c / chunks_per_head;
     int32_t off = c - head * chunks_per_head;
     int64_t dst = (((int64_t)page * Hkv + head) * P + (pos % P)) * chunks_per_head + off;
-    k_pool[dst] = k_new[idx];
-    v_pool[dst] = v_new[idx];
+    const int4 kx = k_new[idx], vx = v_new[idx];
+    k_pool[dst] = kx;
+    v_pool[dst] = vx;
+    // NEXT-3: the same slice goes to every linked replica pool at the same page id -
+    // plain stores through the peer mapping (NVLink), no second read of the slice.
+    for (int32_t r = 0; r < peers.n; ++r) { ((int4*)peers.k[r])[dst] = kx; ((int4*)peers.v[r])[dst] = vx; }
   }
   // Zero the unused tail of each session's last page: slots beyond the committed length are then
   // always finite (zero), so the attention kernel may load whole pages and rely on P = 0 for the
@@ -77,9 +81,12 @@ kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
         int64_t dst = (((int64_t)page * Hkv + head) * P + (len_new % P + t)) * chunks_per_head + off;
         k_pool[dst] = zero;
         v_pool[dst] = zero;
+        for (int32_t r = 0; r < peers.n; ++r) { ((int4*)peers.k[r])[dst] = zero; ((int4*)peers.v[r])[dst] = zero; }
       }
     }
   }
+  // Peer stores must be visible to the replica's GPU before the host learns this kernel completed.
+  if (peers.n > 0) __threadfence_system();
   // Completing only after the predecessor has completed keeps the dependency chain transitive: the
   // attention kernel's griddepcontrol.wait on this grid then also covers everything before it.
   pdl_wait();
@@ -106,16 +113,69 @@ kv_gather_kernel(const int4* __restrict__ k_pool, const int4* __restrict__ v_poo
   }
 }
 
+// NEXT-3 replica side: publish adopted page ids into the device page table (ws_replica_apply).
+// One launch covers one session: row `slot`, logical pages [first, first + n) <- ids[0..n).
+__global__ void __launch_bounds__(256)
+page_table_publish_kernel(int32_t* __restrict__ page_table, const __grid_constant__ InlineAppendMeta inl,
+                          int32_t slot, int32_t first, int32_t n, int32_t max_pages) {
+  for (int32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+    page_table[(int64_t)slot * max_pages + first + i] = inl.w[i];
+}
+
+// NEXT-3 owner side: the data half of the initial broadcast: every page of a session,
+// all KV heads (one page = Hkv * P * D * eb contiguous bytes), local pool -> linked pools.
+__global__ void __launch_bounds__(256)
+kv_push_pages_kernel(const int4* __restrict__ k_pool, const int4* __restrict__ v_pool,
+                     const PeerPools peers, const int32_t* __restrict__ page_row, int32_t npages,
+                     int32_t chunks_per_page) {
+  const int64_t total = (int64_t)npages * chunks_per_page;
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+       idx += (int64_t)gridDim.x * blockDim.x) {
+    const int32_t lp = (int32_t)(idx / chunks_per_page);
+    const int64_t off = (int64_t)page_row[lp] * chunks_per_page + (idx - (int64_t)lp * chunks_per_page);
+    const int4 kx = k_pool[off], vx = v_pool[off];
+    for (int32_t r = 0; r < peers.n; ++r) { ((int4*)peers.k[r])[off] = kx; ((int4*)peers.v[r])[off] = vx; }
+  }
+  __threadfence_system();
+}
+
+cudaError_t launch_page_table_publish(int32_t* page_table, const int32_t* ids, int32_t slot,
+                                      int32_t first, int32_t n, int32_t max_pages,
+                                      cudaStream_t stream) {
+  // chunks of at most kInlineAppendWords ids travel in the kernel parameters (capturable, no staging)
+  for (int32_t done = 0; done < n; done += kInlineAppendWords) {
+    const int32_t m = std::min(n - done, (int32_t)kInlineAppendWords);
+    InlineAppendMeta inl{};
+    for (int32_t i = 0; i < m; ++i) inl.w[i] = ids[done + i];
+    page_table_publish_kernel<<<(m + 255) / 256, 256, 0, stream>>>(page_table, inl, slot, first + done,
+                                                                    m, max_pages);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+cudaError_t launch_kv_push_pages(const void* k_pool, const void* v_pool, const PeerPools& peers,
+                                 const int32_t* page_row, int32_t npages, int64_t page_bytes,
+                                 int32_t num_sms, cudaStream_t stream) {
+  const int32_t cpp = (int32_t)(page_bytes / 16);
+  const int64_t total = (int64_t)npages * cpp;
+  const int32_t grid = (int32_t)std::min<int64_t>(std::max<int64_t>((total + 255) / 256, 1), (int64_t)num_sms * 16);
+  kv_push_pages_kernel<<<grid, 256, 0, stream>>>((const int4*)k_pool, (const int4*)v_pool, peers,
+                                                 page_row, npages, cpp);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_kv_append(const void* k_new, const void* v_new, void* k_pool, void* v_pool,
                              int32_t* page_table, const int32_t* meta, const InlineAppendMeta& inl,
-                             int32_t total_tokens, int32_t max_pages, int32_t P, int32_t Hkv,
+                             const PeerPools& peers, int32_t total_tokens, int32_t max_pages, int32_t P, int32_t Hkv,
                              int32_t D, int32_t eb, int32_t num_sms, cudaStream_t stream) {
   int32_t cph = D * eb / 16;
   int64_t total = (int64_t)total_tokens * Hkv * cph;
   int64_t blocks = (total + 255) / 256;
   int32_t grid = (int32_t)std::min<int64_t>(std::max<int64_t>(blocks, 1), (int64_t)num_sms * 8);
   return launch_pdl(kv_append_kernel, dim3(grid), dim3(256), 0, stream, (const int4*)k_new,
-                    (const int4*)v_new, (int4*)k_pool, (int4*)v_pool, page_table, meta, inl,
+                    (const int4*)v_new, (int4*)k_pool, (int4*)v_pool, page_table, meta, inl, peers,
                     max_pages, P, Hkv, cph);
 }
 

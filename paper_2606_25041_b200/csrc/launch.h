@@ -34,9 +34,15 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 // meta == nullptr: the metadata blob is `inl` (passed in the kernel parameters)
 cudaError_t launch_kv_append(const void* k_new, const void* v_new, void* k_pool, void* v_pool,
                              int32_t* page_table, const int32_t* meta, const InlineAppendMeta& inl,
-                             int32_t total_tokens,
+                             const PeerPools& peers, int32_t total_tokens,
                              int32_t max_pages, int32_t P, int32_t Hkv, int32_t D, int32_t eb,
                              int32_t num_sms, cudaStream_t stream);
+// NEXT-3 (replica link): see kv_append.cu
+cudaError_t launch_page_table_publish(int32_t* page_table, const int32_t* ids, int32_t slot,
+                                      int32_t first, int32_t n, int32_t max_pages, cudaStream_t stream);
+cudaError_t launch_kv_push_pages(const void* k_pool, const void* v_pool, const PeerPools& peers,
+                                 const int32_t* page_row, int32_t npages, int64_t page_bytes,
+                                 int32_t num_sms, cudaStream_t stream);
 cudaError_t launch_kv_gather(const void* k_pool, const void* v_pool, void* k_out, void* v_out,
                              const int32_t* page_row, int64_t start, int64_t count, int32_t P,
                              int32_t Hkv, int32_t D, int32_t eb, int32_t num_sms,

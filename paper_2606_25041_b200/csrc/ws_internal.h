@@ -77,6 +77,15 @@ struct AppendMeta {
   int32_t num_sessions, total_tokens, off_sessions, off_pages;
 };
 
+// NEXT-3: pools of the linked replicas as mapped on this device (16-byte words); n = 0: none.
+constexpr int kMaxPeers = 4;
+struct PeerPools {
+  void* k[kMaxPeers];
+  void* v[kMaxPeers];
+  int32_t n;
+  int32_t pad;
+};
+
 // Parameters common to the attention kernels.
 struct AttnParams {
   const void* q; void* out; float* lse;
