@@ -218,6 +218,52 @@ def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, r
             "frac_of_hbm_roofline": byts / us / 1e3 / float(peaks["hbm_gbs"]),
             "kernel": plan["used_tensor_core_kernel"],
             "what": "append + attention (decode plan) + combine, CUDA-graph replay, history read from HBM"})
+    # --- NEXT-3: replica link (thinker -> performer KV-slice exchange).  The box has ONE GPU, so the
+    # linked pool is a second pool on the same device: these numbers show the cost of the extra stores
+    # and of the page push at HBM speed; over NVLink 5 the peer stores run at <= 900 GB/s per direction.
+    if len(ids) == 1:
+        c = cache.cfg
+        rep = Cache(WS_BF16, Hq, Hkv, D, 64, c.num_pages, max_sessions=c.max_sessions,
+                    max_pages_per_session=c.max_pages_per_session, max_blocks_per_session=c.max_blocks_per_session,
+                    max_q_tokens_per_call=c.max_q_tokens_per_call, device=dev.index or 0)
+        rep.replica_accept(c.num_pages)
+
+        def append_only(i):
+            reset()
+            cache.kv_append(ids, cu, k0, v0)
+        reps = 200
+        for i in range(5):
+            append_only(i)
+        us_plain = 1e3 * timed(reps, append_only) / reps
+        cache.replica_link([rep])
+        for i in range(5):
+            append_only(i)
+        us_mirror = 1e3 * timed(reps, append_only) / reps
+        reset()
+        push = lambda i: cache.replica_push_session(ids[0])
+        for i in range(3):
+            push(i)
+        reps = 30
+        us_push = 1e3 * timed(reps, push) / reps
+        npages = len(cache.session_pages(ids[0]))
+        push_bytes = 2 * 2 * npages * Hkv * 64 * D * 2               # K and V, read + write
+        rep.replica_apply(cache.replica_snapshot_message(ids[0]))
+        kg = torch.empty((256, Hkv, D), dtype=torch.bfloat16, device=dev); vg = torch.empty_like(kg)
+        kr = torch.empty_like(kg); vr = torch.empty_like(kg)
+        L0 = cache.session_info(ids[0])[0]
+        cache.kv_gather(ids[0], L0 - 256, 256, kg, vg); rep.kv_gather(ids[0], L0 - 256, 256, kr, vr)
+        torch.cuda.synchronize()
+        res["replica_link"] = {
+            "slice_bytes": int(2 * k0.numel() * 2), "append_us": us_plain, "append_mirrored_us": us_mirror,
+            "push_session_us": us_push, "push_pages": npages, "push_bytes_read_plus_write": push_bytes,
+            "push_gbs": push_bytes / us_push / 1e3, "push_frac_of_hbm_copy_peak": push_bytes / us_push / 1e3 / float(peaks["hbm_gbs"]),
+            "replica_tail_bit_exact": bool(torch.equal(kg.view(torch.int16), kr.view(torch.int16))
+                                           and torch.equal(vg.view(torch.int16), vr.view(torch.int16))),
+            "what": "one mirrored ws_kv_append per unit (slice stored locally and into the linked pool in the "
+                    "same kernel pass) and ws_replica_push_session of the whole history (initial broadcast); "
+                    "the linked pool is on the SAME device (single-GPU box), not across NVLink"}
+        cache.replica_link([])
+        rep.close()
     return res
 
 
