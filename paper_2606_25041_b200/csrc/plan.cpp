@@ -62,27 +62,53 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
   // continues into another group pays a fixed cost for the extra segment (Q reload, pipeline
   // refill, epilogue), measured at ~3.3 KV tiles on B200: budgets are equalised in cost units.
   const double ovh = cfg.seg_overhead_tiles;
-  const double total_cost = (double)T + ovh * std::max<double>(0.0, (double)plan.groups.size() - 1.0);
-  const double budget = total_cost / n_used;
-  int32_t team = 0;
-  double used = 0.0;                 // cost consumed by the current team
-  for (size_t gi = 0; gi < plan.groups.size(); ++gi) {
-    int32_t nt = group_tiles[gi];
-    int32_t per = cfg.min_splits > 0 ? std::max(1, (nt + cfg.min_splits - 1) / cfg.min_splits) : nt;
-    int32_t t = 0;
-    while (t < nt) {
-      const bool last_team = team + 1 >= n_used;
-      const double seg_cost0 = (used > 0.0) ? ovh : 0.0;   // not the team's first segment
-      int64_t room = (int64_t)(budget - used - seg_cost0 + 0.5);
-      if (!last_team && room < 1) { ++team; used = 0.0; continue; }
-      if (last_team) room = nt - t;
-      int32_t take = (int32_t)std::min<int64_t>(room, nt - t);
-      take = std::min(take, per - (t % per));
-      plan.segments.push_back(Segment{(int32_t)gi, t, t + take, -1});
-      plan.seg_team.push_back(team);
-      used += seg_cost0 + take;
-      t += take;
+  // Greedy walk with a per-team budget B: a team takes tiles until its cost (tiles + ovh per extra
+  // segment) would exceed B; the last team takes whatever is left.  The smallest B for which the last
+  // team also stays within B minimises the maximum team cost - found by bisection.  (A fixed budget of
+  // total/teams leaves the last team with the sum of every team's rounding remainder: 63 tiles against
+  // an average of 7 on a 16-head MHA step; carrying the remainder forward instead overloads the teams
+  // that follow a group boundary.)
+  struct Cut { int32_t group, begin, end, team; };
+  std::vector<Cut> cuts;
+  auto walk = [&](double B, bool emit) -> double {
+    int32_t team = 0;
+    double used = 0.0, worst = 0.0;
+    if (emit) cuts.clear();
+    for (size_t gi = 0; gi < plan.groups.size(); ++gi) {
+      const int32_t nt = group_tiles[gi];
+      const int32_t per = cfg.min_splits > 0 ? std::max(1, (nt + cfg.min_splits - 1) / cfg.min_splits) : nt;
+      int32_t t = 0;
+      while (t < nt) {
+        const bool last_team = team + 1 >= n_used;
+        const double seg_cost0 = (used > 0.0) ? ovh : 0.0;   // not the team's first segment
+        int64_t room = (int64_t)(B - used - seg_cost0 + 1e-6);
+        if (!last_team && room < 1) { worst = std::max(worst, used); ++team; used = 0.0; continue; }
+        if (last_team) room = nt - t;
+        int32_t take = (int32_t)std::min<int64_t>(room, nt - t);
+        take = std::min(take, per - (t % per));
+        if (emit) cuts.push_back(Cut{(int32_t)gi, t, t + take, team});
+        used += seg_cost0 + take;
+        t += take;
+      }
     }
+    return std::max(worst, used);
+  };
+  const double total_cost = (double)T + ovh * std::max<double>(0.0, (double)plan.groups.size() - 1.0);
+  double lo = std::max(1.0, (double)T / n_used), hi = std::max(lo, total_cost);
+  if (walk(lo, false) <= lo + 1e-9) {
+    hi = lo;
+  } else {
+    for (int it = 0; it < 40 && hi - lo > 0.05; ++it) {
+      const double mid = 0.5 * (lo + hi);
+      if (walk(mid, false) <= mid + 1e-9) hi = mid; else lo = mid;
+    }
+  }
+  walk(hi, true);
+  int32_t team = 0;
+  for (const Cut& c : cuts) {
+    plan.segments.push_back(Segment{c.group, c.begin, c.end, -1});
+    plan.seg_team.push_back(c.team);
+    team = c.team;
   }
   plan.num_teams = team + 1;
   // partial slots: only groups cut into more than one segment need them

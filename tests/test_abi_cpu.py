@@ -185,7 +185,19 @@ def test_planner_ragged_multi_session(pkg):
     _check_cover(info, segs, tiles)
     assert info["num_groups"] == 64 and info["num_ctas"] == 148
     cost = _team_costs(segs)
-    assert cost[:-1].max() - cost[:-1].min() <= 2.0 and cost[-1] <= 1.02 * cost[:-1].max(), cost
+    # min-max budget: no team above the mean by more than a tile or so; a few teams that stop at a group
+    # boundary (cannot afford the next segment's start-up) stay below it
+    assert cost.max() <= cost.mean() + 2.0 and np.median(cost) >= cost.max() - 2.0, cost
+
+
+def test_planner_many_groups_last_team_not_overloaded(pkg):
+    """Regression: 16-head MHA, 66 tiles per group over 148 single-CTA teams.  Per-team rounding used to
+    leave the last team with the sum of every team's remainder (63 tiles against an average of 7)."""
+    info, segs = _plan(pkg, [8192], 256, Hq=16, Hkv=16)
+    _check_cover(info, segs, 16 * 66)
+    cost = _team_costs(segs)
+    assert info["team_size"] == 1 and 130 <= len(cost) <= 148
+    assert cost.max() <= 8.0 + 1e-6, cost            # 1056 tiles over 148 teams: 8 per team is the optimum
 
 
 def test_planner_small_and_forced_splits(pkg):

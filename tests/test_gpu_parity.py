@@ -236,7 +236,8 @@ def test_ragged_multi_session_small_and_batched_equals_single():
         solo = dataclasses.replace(w, spec=dataclasses.replace(w.spec, num_sessions=1),
                                    cache_lens=[w.cache_lens[s]], sessions=[w.sessions[s]])
         g1 = run_workload_gpu(solo, gather=False)
-        assert np.abs(g1["out"][0][0] - ref["out"][0][s]).max() <= 1e-2
+        d1 = np.abs(g1["out"][0][0] - ref["out"][0][s])
+        assert (d1 - np.abs(ref["out"][0][s]) * 2.0 ** -8).max() <= 8e-3 and d1.mean() <= 1e-3   # same gate as above
         # different split plans round P and O differently: both runs are within tolerance of the
         # oracle, so they are within twice the tolerance of each other (and much closer on average)
         a, b = g1["out"][0][0], got["out"][0][s]
