@@ -536,11 +536,9 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     any_multi |= m > 1;
     for (int32_t b = B - m; b < B; ++b) {
       int64_t lo = b ? ss.block_ends[b - 1] : 0;
-      for (int64_t t = lo; t < ss.block_ends[b]; ++t) {
-        vis_end.push_back((int32_t)ss.block_ends[b]);
-        tok_slot.push_back(id);
-      }
+      vis_end.insert(vis_end.end(), (size_t)(ss.block_ends[b] - lo), (int32_t)ss.block_ends[b]);
     }
+    tok_slot.insert(tok_slot.end(), (size_t)nq, id);
   }
   const int32_t NQ = cu[S];
   if (NQ > c->cfg.max_q_tokens_per_call)

@@ -30,6 +30,11 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
     if ((int64_t)(s.q_end - s.q_begin) * cfg.G > kTileRows) plan.alt = false;
 
   std::vector<int32_t> group_tiles;
+  {
+    size_t ng = 0;
+    for (const PlanSession& s : sessions) ng += (size_t)cfg.Hkv * (((s.q_end - s.q_begin + tok_per_pair - 1) / tok_per_pair + Pt - 1) / Pt);
+    plan.groups.reserve(ng); group_tiles.reserve(ng);
+  }
   for (const PlanSession& s : sessions) {
     int32_t nq = s.q_end - s.q_begin;
     int32_t pairs = (nq + tok_per_pair - 1) / tok_per_pair;
@@ -68,17 +73,27 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
   // total/teams leaves the last team with the sum of every team's rounding remainder: 63 tiles against
   // an average of 7 on a 16-head MHA step; carrying the remainder forward instead overloads the teams
   // that follow a group boundary.)
-  struct Cut { int32_t group, begin, end, team; };
-  std::vector<Cut> cuts;
   auto walk = [&](double B, bool emit) -> double {
     int32_t team = 0;
     double used = 0.0, worst = 0.0;
-    if (emit) cuts.clear();
+    if (emit) { plan.segments.clear(); plan.seg_team.clear(); }
     for (size_t gi = 0; gi < plan.groups.size(); ++gi) {
       const int32_t nt = group_tiles[gi];
       const int32_t per = cfg.min_splits > 0 ? std::max(1, (nt + cfg.min_splits - 1) / cfg.min_splits) : nt;
       int32_t t = 0;
       while (t < nt) {
+        if (!emit && used == 0.0 && per == nt) {
+          // fast-forward (feasibility walks only): every fresh team inside this group takes floor(B)
+          // tiles and then cannot afford another segment - skip them arithmetically
+          const int64_t full = (int64_t)(B + 1e-6);
+          const int64_t k = std::min<int64_t>((nt - t) / full, (int64_t)n_used - 1 - team);
+          if (full >= 1 && k > 0) {
+            worst = std::max(worst, (double)full);
+            team += (int32_t)k;
+            t += (int32_t)(k * full);
+            continue;
+          }
+        }
         const bool last_team = team + 1 >= n_used;
         const double seg_cost0 = (used > 0.0) ? ovh : 0.0;   // not the team's first segment
         int64_t room = (int64_t)(B - used - seg_cost0 + 1e-6);
@@ -86,30 +101,35 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
         if (last_team) room = nt - t;
         int32_t take = (int32_t)std::min<int64_t>(room, nt - t);
         take = std::min(take, per - (t % per));
-        if (emit) cuts.push_back(Cut{(int32_t)gi, t, t + take, team});
+        if (emit) {
+          plan.segments.push_back(Segment{(int32_t)gi, t, t + take, -1});
+          plan.seg_team.push_back(team);
+        }
         used += seg_cost0 + take;
         t += take;
       }
     }
     return std::max(worst, used);
   };
-  const double total_cost = (double)T + ovh * std::max<double>(0.0, (double)plan.groups.size() - 1.0);
-  double lo = std::max(1.0, (double)T / n_used), hi = std::max(lo, total_cost);
-  if (walk(lo, false) <= lo + 1e-9) {
-    hi = lo;
-  } else {
-    for (int it = 0; it < 40 && hi - lo > 0.05; ++it) {
+  // lo = T / teams is a lower bound of the optimum; grow the bracket geometrically until the walk fits,
+  // then bisect it to a quarter tile (5-8 walks in practice; this runs on the host once per call)
+  double lo = std::max(1.0, (double)T / n_used), hi = lo;
+  if (walk(lo, false) > lo + 1e-9) {
+    double step = 1.0;
+    for (;;) {
+      hi = lo + step;
+      if (walk(hi, false) <= hi + 1e-9) break;
+      lo = hi; step *= 2.0;
+    }
+    while (hi - lo > 0.25) {
       const double mid = 0.5 * (lo + hi);
       if (walk(mid, false) <= mid + 1e-9) hi = mid; else lo = mid;
     }
   }
+  plan.segments.reserve(plan.groups.size() + 2 * (size_t)n_used);
+  plan.seg_team.reserve(plan.groups.size() + 2 * (size_t)n_used);
   walk(hi, true);
-  int32_t team = 0;
-  for (const Cut& c : cuts) {
-    plan.segments.push_back(Segment{c.group, c.begin, c.end, -1});
-    plan.seg_team.push_back(c.team);
-    team = c.team;
-  }
+  const int32_t team = plan.seg_team.empty() ? 0 : plan.seg_team.back();
   plan.num_teams = team + 1;
   // partial slots: only groups cut into more than one segment need them
   size_t i = 0;
