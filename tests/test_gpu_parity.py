@@ -682,6 +682,61 @@ def test_config5_ragged_multi_session_sampled():
     _assert_close(compare(got, ref, "bf16", rows=rows, heads=heads), BF16_TOL, "cfg5")
 
 
+def test_maximum_size_one_million_token_session_sampled():
+    """Maximum sizes: one session with a 1,000,003-token committed history (mid-page end, 15,626 pages,
+    2 GB per pool, 7,815 KV tiles per head) - full-history streaming never evicts.
+    Inputs are seeded on the GPU (generating 2 G normals on the host would dominate the test) and read
+    back for the oracle, which checks sampled output elements; the cache tail is gathered bit for bit."""
+    import ml_dtypes
+    import torch
+    from oracle.block_causal import OracleSession, attend
+    from paper_2606_25041_b200 import WS_BF16, Cache
+    dev = torch.device("cuda", 0)
+    Hq, Hkv, D, P, L, n, blk = 32, 8, 128, 64, 1_000_003, 256, 8192
+    pages = (L + n + P - 1) // P + 3
+    cache = Cache(WS_BF16, Hq, Hkv, D, P, pages, max_sessions=1, max_blocks_per_session=256,
+                  max_q_tokens_per_call=blk)
+    s = cache.session_open()
+    gen = torch.Generator(device=dev); gen.manual_seed(2606_25041)
+    ora = OracleSession(Hkv, D)
+    to_np = lambda t: t.cpu().view(torch.int16).numpy().view(ml_dtypes.bfloat16)
+    pos = 0
+    while pos < L + n:
+        m = min(blk, L - pos) if pos < L else n
+        k = torch.randn((m, Hkv, D), device=dev, generator=gen).bfloat16()
+        v = torch.randn((m, Hkv, D), device=dev, generator=gen).bfloat16()
+        cache.kv_append([s], [0, m], k, v)
+        ora.append(to_np(k), to_np(v))
+        pos += m
+    assert cache.session_info(s)[0] == L + n and len(cache.session_pages(s)) == (L + n + P - 1) // P
+    q = torch.randn((n, Hq, D), device=dev, generator=gen).bfloat16()
+    out = torch.full((n, Hq, D), float("nan"), dtype=torch.bfloat16, device=dev)
+    lse = torch.full((n, Hq), float("nan"), dtype=torch.float32, device=dev)
+    cache.block_causal_attn_fwd([s], [0, n], q, out, 1.0 / math.sqrt(D), lse=lse)
+    torch.cuda.synchronize()
+    info = cache.last_plan_info()
+    assert info["used_tensor_core_kernel"] == 1 and info["num_ctas"] == 148
+    assert info["total_kv_tiles"] == Hkv * ((L + n + 127) // 128)
+    o = out.float().cpu().numpy().astype(np.float64)
+    assert np.isfinite(o).all() and np.isfinite(lse.cpu().numpy()).all()
+    rows, heads = np.array([0, 101, 255]), np.array([0, 3, 31])       # two KV groups
+    o_ref, l_ref = attend(ora, to_np(q), 1.0 / math.sqrt(D), rows=rows, heads=heads)
+    d = o[rows][:, heads] - o_ref
+    rel_rms = float(np.sqrt((d ** 2).mean() / (o_ref ** 2).mean()))
+    dl = np.abs(lse.cpu().numpy().astype(np.float64)[rows][:, heads] - l_ref).max()
+    print(f"[parity] 1M tokens: max_abs={np.abs(d).max():.3e} rel_rms={rel_rms:.3e} lse_max={dl:.3e}")
+    assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3 and rel_rms <= 1e-2 and dl <= 1e-3
+    # the end of the history (last preload block's mid-page tail + the new block), bit for bit
+    cnt = 700
+    kg = torch.empty((cnt, Hkv, D), dtype=torch.bfloat16, device=dev); vg = torch.empty_like(kg)
+    cache.kv_gather(s, L + n - cnt, cnt, kg, vg)
+    torch.cuda.synchronize()
+    kr, vr = ora.gather()
+    assert to_np(kg).tobytes() == np.ascontiguousarray(kr[-cnt:]).tobytes()
+    assert to_np(vg).tobytes() == np.ascontiguousarray(vr[-cnt:]).tobytes()
+    cache.close()
+
+
 def test_outputs_stay_inside_their_buffers():
     """compute-sanitizer is closed on this GPU pool, so out-of-bounds writes are caught with canaries:
     `out`, `lse` and the workspace's neighbours are slices of larger canary-filled tensors; a ragged
