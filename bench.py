@@ -505,6 +505,29 @@ def main():
     if not args.no_next and world == 1 and R == 1:
         nxt = measure_next(cache, ids, base_blocks, sp, cu, q_d[0], k_d[0], v_d[0], out, dev, timed, reset)
 
+    # ---- the same step without host work: one CUDA graph holding one step per cache, replayed
+    # (configs whose step is a single unit; the device-side cost of append -> attention -> combine)
+    if not args.no_next and world == 1 and steps_per_cycle == 1 and plan["used_tensor_core_kernel"]:
+        reset()
+        torch.cuda.synchronize()
+        gr = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(gr):
+            for r in range(R):
+                caches[r].kv_append(ids_of[r], cu, k_d[0], v_d[0])
+                caches[r].block_causal_attn_fwd(ids_of[r], cu, q_d[0], out, sp.scale)
+        for _ in range(5):
+            gr.replay()
+        reps = max(20, 400 // R)
+        ms_g = timed(reps, lambda i: gr.replay())
+        us_g = 1e3 * ms_g / (reps * R)
+        nxt = dict(nxt or {})
+        nxt["step_cuda_graph"] = {"us_per_unit": us_g, "tflops": flops_cycle[0] / (us_g * 1e-6) / 1e12,
+                                  "hbm_gbs": bytes_cycle[0] / (us_g * 1e-6) / 1e9,
+                                  "frac_of_step_roofline": roofline["step_roofline_us"] / us_g,
+                                  "what": "append + attention + combine of %d caches captured once, replayed: "
+                                          "no host planning or launch cost in the loop" % R}
+        reset()
+
     # ---- CPU baseline: the oracle on a bounded sample, rank 0 at N=1 only
     cpu = None
     if not args.no_cpu_baseline and world == 1:
