@@ -59,7 +59,13 @@ enum {
   WS_FLAG_FORCE_SIMT = 2u,
   /* Run the tcgen05 kernel on CTA pairs (cta_group::2, M = 256 per MMA, each CTA stages half of every
    * K/V tile) when the plan's team size is even.  Correct but slower on B200. */
-  WS_FLAG_CTA_PAIRS = 4u
+  WS_FLAG_CTA_PAIRS = 4u,
+  /* Run the split-KV combine (a4) as its own kernel after the attention kernel instead of inside it.
+   * By default the CTAs of the tcgen05 kernel merge the split partials themselves once every split of
+   * a (session, KV head) group has been published (per-group arrival counters in the workspace; the
+   * kernel is launched cooperatively so that all of its CTAs are co-resident while they wait on each
+   * other).  The separate kernel is kept for A/B measurements and is always used with CTA pairs.   */
+  WS_FLAG_SEPARATE_COMBINE = 8u
 };
 
 typedef struct ws_cache ws_cache_t;   /* opaque; owns host metadata only */

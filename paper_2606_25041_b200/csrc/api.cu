@@ -64,7 +64,7 @@ bool config_valid(const ws_cache_config_t* c, const char** why) {
 }
 
 struct Layout {
-  size_t page_table, q_to_kv, meta, part_lse, part_o, total;
+  size_t page_table, q_to_kv, meta, part_lse, part_o, merge_ctr, total;
   size_t meta_slot_bytes;
   int32_t max_part_slots;
 };
@@ -84,6 +84,7 @@ Layout make_layout(const ws_cache_config_t* c, int num_sms) {
   L.max_part_slots = 4 * num_sms + 64;
   L.part_lse = off;   off = align_up(off + (size_t)L.max_part_slots * ws::kPairRows * 4, 256);
   L.part_o = off;     off = align_up(off + (size_t)L.max_part_slots * ws::kPairRows * c->head_dim * 4, 256);
+  L.merge_ctr = off;  off = align_up(off + (size_t)L.max_part_slots * 2 * 4, 256);
   L.total = off;
   return L;
 }
@@ -110,6 +111,7 @@ struct ws_cache {
   char* d_meta = nullptr;
   float* d_part_lse = nullptr;
   float* d_part_o = nullptr;
+  int32_t* d_merge_ctr = nullptr;     // fused-combine counters (all zero between launches)
   // pinned staging ring
   char* h_meta = nullptr;
   cudaEvent_t ev[kRing]{};
@@ -299,6 +301,8 @@ ws_status_t ws_cache_create(const ws_cache_config_t* cfg, ws_cache_t** out) {
   c->d_meta = ws_base + c->lay.meta;
   c->d_part_lse = (float*)(ws_base + c->lay.part_lse);
   c->d_part_o = (float*)(ws_base + c->lay.part_o);
+  c->d_merge_ctr = (int32_t*)(ws_base + c->lay.merge_ctr);
+  WS_CUDA(cudaMemset(c->d_merge_ctr, 0, (size_t)c->lay.max_part_slots * 2 * 4));
   WS_CUDA(cudaMemset(c->d_page_table, 0, (size_t)cfg->max_sessions * cfg->max_pages_per_session * 4));
   if (!c->default_map)
     WS_CUDA(cudaMemcpy(c->d_q_to_kv, c->q_to_kv.data(), c->q_to_kv.size() * 4, cudaMemcpyHostToDevice));
@@ -622,6 +626,10 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
   L.p.page_table = c->d_page_table;
   L.p.meta = (const int32_t*)d;
   L.p.part_o = c->d_part_o; L.p.part_lse = c->d_part_lse;
+  const bool fused_combine = cta_group == 1 && !(c->cfg.flags & WS_FLAG_SEPARATE_COMBINE) &&
+                             !c->last_plan.combine.empty();
+  L.p.merge_ctr = fused_combine ? c->d_merge_ctr : nullptr;
+  L.p.max_part_slots = c->lay.max_part_slots;
   L.p.max_pages_per_session = c->cfg.max_pages_per_session;
   L.p.Hq = c->cfg.num_q_heads; L.p.Hkv = c->cfg.num_kv_heads; L.p.D = c->cfg.head_dim;
   L.p.G = G; L.p.P = c->cfg.page_tokens; L.p.total_q_tokens = NQ; L.p.scale = scale;
@@ -641,7 +649,7 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
   WS_CUDA(ws::launch_attn_sm100(L, stream));
   tl.done();
   c->launches += 1;
-  if (!c->last_plan.combine.empty()) {
+  if (!c->last_plan.combine.empty() && !fused_combine) {
     TimedLaunch tc(c, &c->t_combine, stream);
     WS_CUDA(ws::launch_combine(L.p, L.inl, L.inl_words, (int32_t)c->last_plan.combine.size(), c->last_plan.team_size, stream));
     tc.done();

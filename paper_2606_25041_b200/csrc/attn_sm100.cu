@@ -69,15 +69,33 @@ constexpr float kFastSumLimit = 1024.0f;                   // fast path accepted
 #ifdef WS_PROFILE
 #define PROF_DECL(n) long long prof_acc[n] = {0}; long long prof_t = clock64();
 #define PROF_MARK(i) { long long t_ = clock64(); prof_acc[i] += t_ - prof_t; prof_t = t_; }
+__device__ __forceinline__ unsigned long long prof_gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+__shared__ unsigned long long prof_stamps[24];
+#define PROF_STAMP(i) { if (prof_stamps[i] == 0) prof_stamps[i] = prof_gtime(); }
+#define PROF_CLK(i) { if (prof_stamps[i] == 0) prof_stamps[i] = clock64(); }
 #else
+#define PROF_STAMP(i) {}
+#define PROF_CLK(i) {}
 #define PROF_DECL(n)
 #define PROF_MARK(i)
 #endif
+
+// One merge duty of this CTA (fused combine): rows [r_lo, r_hi) of the (item, pair) whose partial slots
+// are slot0 + i * npairs, i < nparts.  Resolved from the metadata when the segment starts (off the
+// critical path) and parked in shared memory until the merge phase.
+struct MergeJob {
+  int32_t slot0, nparts, npairs, kv_head, tok0, r_lo, r_hi, pad;
+};
+constexpr int kMaxJobs = 4;
 
 struct Barriers {
   uint64_t q_full, q_empty;
   uint64_t kv_full[kMaxStages], kv_empty[kMaxStages];
   uint64_t s_full[2], p_full[2][2], pv_h0_done[2], o_full[2], o_empty[2];
+  uint64_t merge_full;
+  alignas(16) float lse_stage[kPairRows];
+  MergeJob jobs[kMaxJobs];
+  int32_t njobs, cur_slot0;          // staged epilogue: the pair's log2-LSEs on their way to part_lse
   uint32_t tmem_base;
   uint32_t pad;
 };
@@ -85,8 +103,9 @@ constexpr uint32_t kSmemBytes = 2 * kQTileBytes + kRingBytes + sizeof(Barriers) 
 
 struct SegView {
   Group g;
-  int32_t tile_begin, tile_end, part_base;
+  int32_t tile_begin, tile_end, part_base, group;
 };
+
 
 // Loads segment `si` as seen by row-tile pair `pair`.  Returns false if this CTA has no rows in it
 // (pair >= npairs).  For multi-block queries the pair's own visible end clips the tile range: KV
@@ -99,7 +118,7 @@ __device__ __forceinline__ bool load_segment(const int32_t* meta, const AttnMeta
   // odd pair of the cluster for kCG = 2): both CTAs of a pair must walk the same tile range.
   const Segment s = reinterpret_cast<const Segment*>(meta + hdr.off_segments)[si];
   v.g = reinterpret_cast<const Group*>(meta + hdr.off_groups)[s.group];
-  v.tile_begin = s.tile_begin; v.tile_end = s.tile_end; v.part_base = s.part_base;
+  v.tile_begin = s.tile_begin; v.tile_end = s.tile_end; v.part_base = s.part_base; v.group = s.group;
   if ((pair & ~(int32_t)(kClipPairMask)) >= v.g.npairs) return false;
   if (v.g.vis_off >= 0) {
     const int32_t last_tok = min(v.g.q_token_end, v.g.q_token0 + (pair + 1) * tok_per_pair) - 1;
@@ -161,6 +180,155 @@ __device__ __forceinline__ void softmax_chunk(const uint32_t* sr, float c, float
   }
 }
 
+
+// ---- fused split-KV combine (a4 inside the attention kernel; the paper is silent on this step) ----
+// A group whose KV range was cut into `nparts` segments yields nparts partials per row-tile pair, each
+// written by a different CTA.  Each of those CTAs also owns 1/nparts of the pair's rows: after it has
+// published ALL of its own partials it waits until the arrival counter of the (item, pair) shows that
+// every part is there and merges its rows (LSE-weighted, same arithmetic as combine_kernel).  The wait
+// cannot deadlock: a CTA signals before it waits, signalling depends on nothing but the CTA's own
+// progress, and the grid is launched cooperatively (all CTAs co-resident).
+__device__ __forceinline__ int32_t ld_acquire_gpu(const int32_t* p) {
+  int32_t v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+// volatile so that a batch of these stays in program order ahead of the mbarrier wait that follows it
+// (as plain loads the compiler sank each one to its first use: one exposed L2 latency per merged row)
+__device__ __forceinline__ float ld_cg_f32(const float* p) {
+  float v;
+  asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ int32_t ld_relaxed_gpu(const int32_t* p) {
+  int32_t v;
+  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void red_release_gpu_add(int32_t* p, int32_t v) {
+  asm volatile("red.release.gpu.global.add.s32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+
+// Partial-row storage format (private to the writers and the mergers): the 16-byte chunk c of packed row
+// r (4 of the row's 128 fp32) lives at chunk position c ^ (r & 7) of the row's 512 bytes.  The XOR makes
+// the thread-per-row shared-memory staging of the epilogue conflict-free (8 consecutive rows hit 8
+// different 16-byte bank groups) while a row stays one contiguous 512-byte run in global memory.
+__device__ __forceinline__ int part_chunk_pos(int c, int r) { return c ^ (r & 7); }
+
+// The 256 softmax threads (8 warps) merge packed rows [r_lo, r_hi) of one (item, pair).  The rows'
+// partials are contiguous per part ([slot][256 rows][128] fp32, [slot][256] LSEs), so each part is ONE
+// bulk copy of O rows into the (idle) K/V ring plus one of LSEs into the (idle) Q tiles; every copy of
+// the item is in flight at once and the merge itself reads shared memory only.  Warp w handles rows
+// w, w + 8, ...; lane = 16-byte chunk position of the row.  Every lane recomputes the row's weights
+// from the LSEs (broadcast shared-memory reads: no shuffles), kMR rows interleaved for ILP.
+constexpr int kMergeRowsCap = (int)(kRingBytes / 512);     // 320 rows of 512 B fit the ring
+constexpr int kMR = 4;
+__device__ __forceinline__ void merge_item(const AttnParams& p, const MergeJob& job,
+                                           uint32_t sRing, const uint8_t* ring, uint32_t sLse, const uint8_t* lse_s,
+                                           uint32_t bar, uint32_t& phase, int warp, int lane) {
+  const int32_t nparts = job.nparts, r_lo = job.r_lo, r_hi = job.r_hi, tok0 = job.tok0;
+  const int64_t slot0 = job.slot0, stride = job.npairs;
+  if (r_hi <= r_lo) return;
+  const int32_t rc = min(r_hi - r_lo, kMergeRowsCap / nparts);
+  const int32_t lse_stride = (rc + 8) & ~3;                 // floats per part in the LSE staging area
+  for (int32_t c0 = r_lo; c0 < r_hi; c0 += rc) {
+    const int32_t n = min(rc, r_hi - c0);
+    const int32_t c0a = c0 & ~3, nl = ((c0 + n + 3) & ~3) - c0a;   // 16-byte aligned LSE run covering [c0, c0 + n)
+    asm volatile("bar.sync 1, 256;" ::: "memory");          // ring idle: all MMAs of this CTA / the previous chunk done
+    if (warp == 0) {
+      fence_proxy_async_all();            // the parts were written through the generic proxy (other CTAs)
+      if (lane == 0) mbar_arrive_expect_tx(bar, (uint32_t)((n * 512 + nl * 4) * nparts));
+      __syncwarp();
+      for (int32_t part = lane; part < nparts; part += 32) {
+        bulk_load(sRing + (uint32_t)(part * rc) * 512u,
+                  p.part_o + ((slot0 + part * stride) * kPairRows + c0) * 128, (uint32_t)n * 512u, bar);
+        bulk_load(sLse + (uint32_t)(part * lse_stride) * 4u,
+                  p.part_lse + (slot0 + part * stride) * kPairRows + c0a, (uint32_t)nl * 4u, bar);
+      }
+    }
+    if (threadIdx.x == 0) PROF_STAMP(16)
+    mbar_wait(bar, phase);
+    if (threadIdx.x == 0) PROF_STAMP(17)
+    phase ^= 1u;
+    const float* lse_f = reinterpret_cast<const float*>(lse_s) + (c0 - c0a);
+    const float4* o_f = reinterpret_cast<const float4*>(ring) + lane;
+    for (int32_t lr0 = warp; lr0 < n; lr0 += 8 * kMR) {
+      float mx[kMR], ws[kMR];
+      float4 acc[kMR];
+      const float* lp[kMR];
+      const float4* op[kMR];
+#pragma unroll
+      for (int b = 0; b < kMR; ++b) {
+        const int32_t lr = min(lr0 + 8 * b, n - 1);         // (rows past the end repeat the last one; not stored)
+        lp[b] = lse_f + lr; op[b] = o_f + lr * 32;
+        mx[b] = -INFINITY; ws[b] = 0.f; acc[b] = make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+      if (nparts <= 8) {
+        // common case: every load of the batch is issued before the first use (unrolled over the parts)
+        float lv[kMR][8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+#pragma unroll
+          for (int b = 0; b < kMR; ++b) {
+            lv[b][k] = k < nparts ? lp[b][k * lse_stride] : -INFINITY;
+            mx[b] = fmaxf(mx[b], lv[b][k]);
+          }
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+          if (k < nparts) {
+#pragma unroll
+            for (int b = 0; b < kMR; ++b) {
+              const float w = lv[b][k] == -INFINITY ? 0.f : ex2_approx(lv[b][k] - mx[b]);
+              const float4 v = op[b][k * rc * 32];
+              ws[b] += w;
+              acc[b].x = fmaf(w, v.x, acc[b].x); acc[b].y = fmaf(w, v.y, acc[b].y);
+              acc[b].z = fmaf(w, v.z, acc[b].z); acc[b].w = fmaf(w, v.w, acc[b].w);
+            }
+          }
+      } else {
+        for (int32_t k = 0; k < nparts; ++k)
+#pragma unroll
+          for (int b = 0; b < kMR; ++b) mx[b] = fmaxf(mx[b], lp[b][k * lse_stride]);
+        for (int32_t k = 0; k < nparts; ++k) {
+#pragma unroll
+          for (int b = 0; b < kMR; ++b) {
+            const float lv = lp[b][k * lse_stride];
+            const float w = lv == -INFINITY ? 0.f : ex2_approx(lv - mx[b]);   // (mx = -inf only if every lv is)
+            const float4 v = op[b][k * rc * 32];
+            ws[b] += w;
+            acc[b].x = fmaf(w, v.x, acc[b].x); acc[b].y = fmaf(w, v.y, acc[b].y);
+            acc[b].z = fmaf(w, v.z, acc[b].z); acc[b].w = fmaf(w, v.w, acc[b].w);
+          }
+        }
+      }
+      // branch-free up to the stores, so that the kMR rows' address / normalisation chains interleave
+      uint2 packed[kMR];
+      uint2* dst[kMR];
+      float* ldst[kMR];
+      float lse_out[kMR];
+      const uint32_t G = (uint32_t)p.G;
+#pragma unroll
+      for (int b = 0; b < kMR; ++b) {
+        const uint32_t r = (uint32_t)(c0 + min(lr0 + 8 * b, n - 1));
+        const uint32_t dt = r / G, hh = r - dt * G;
+        const int64_t row = (int64_t)(tok0 + (int32_t)dt) * p.Hq + job.kv_head * p.G + (int32_t)hh;
+        const float inv = ws[b] > 0.f ? __fdividef(1.f, ws[b]) : 0.f;
+        packed[b].x = pack_bf16x2(acc[b].x * inv, acc[b].y * inv);
+        packed[b].y = pack_bf16x2(acc[b].z * inv, acc[b].w * inv);
+        dst[b] = reinterpret_cast<uint2*>(reinterpret_cast<__nv_bfloat16*>(p.out) + row * p.D) + part_chunk_pos(lane, (int)r);
+        ldst[b] = p.lse + row;
+        lse_out[b] = ws[b] > 0.f ? (mx[b] + __log2f(ws[b])) * 0.6931471805599453f : -INFINITY;
+      }
+#pragma unroll
+      for (int b = 0; b < kMR; ++b)
+        if (lr0 + 8 * b < n) {
+          *dst[b] = packed[b];                              // this lane holds logical chunk lane ^ (r & 7)
+          if (p.lse && lane == 0) *ldst[b] = lse_out[b];
+        }
+    }
+  }
+}
+
 // kAlt: decode plan (plan.h) - both accumulator sets use Q tile 0; set q processes the KV tiles of the
 // segment with (tile - tile_begin) % 2 == q and writes its own partial (slot part_base + q).
 template <int kCG, int kInlW, bool kAlt>
@@ -206,13 +374,15 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #ifdef WS_PROFILE
   const long long prof_cta_t0 = clock64();
   unsigned long long prof_g0; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(prof_g0));
+  if (threadIdx.x < 24) prof_stamps[threadIdx.x] = 0;
 #endif
 
   if (warp == 8 && lane == 0) {
     prefetch_tmap(&tmap_q); prefetch_tmap(&tmap_k); prefetch_tmap(&tmap_v);
   }
   if (warp == 9 && lane == 0) {
-    mbar_init(bq_full, 1); mbar_init(bq_empty, 1);
+    mbar_init(bq_full, 1); mbar_init(bq_empty, 1); mbar_init(smem_u32(&bars->merge_full), 1);
+    bars->njobs = 0;
     for (int s = 0; s < kStages; ++s) { mbar_init(bkv_full(s), 1); mbar_init(bkv_empty(s), 1); }
     for (int q = 0; q < 2; ++q) {
       mbar_init(bs_full(q), 1); mbar_init(bp_full(q, 0), 128 * kCG); mbar_init(bp_full(q, 1), 128 * kCG);
@@ -229,6 +399,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   if constexpr (kCG == 2) cluster_sync_all(); else __syncthreads();   // peer barriers are initialised too
   tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
+  if (threadIdx.x == 0) PROF_STAMP(0)
 
   if (warp >= 8) {
     setmaxnreg_dec<88>();
@@ -273,8 +444,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           }
           continue;
         }
-        int32_t pg0 = page_row[min(2 * sv.tile_begin, last_page)];
-        int32_t pg1 = page_row[min(2 * sv.tile_begin + 1, last_page)];
+        // (the page ids of the first tile are fetched while the Q loads are in flight)
         // Q pair (own rows).  kCG = 2: the bytes of both CTAs are credited to the leader's q_full.
         mbar_wait(bq_empty, (q_it & 1) ^ 1);
         if (is_leader) mbar_arrive_expect_tx(bq_full, kCG * 2 * kQTileBytes);
@@ -289,6 +459,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                           sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
           }
         ++q_it;
+        int32_t pg0 = page_row[min(2 * sv.tile_begin, last_page)];
+        int32_t pg1 = page_row[min(2 * sv.tile_begin + 1, last_page)];
         for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
           const int32_t c0 = pg0, c1 = pg1;
           if (j + 1 < sv.tile_end) {                        // prefetch next tile's page ids
@@ -424,6 +596,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
           mbar_wait(bkv_full(slot), par);
           tc_fence_after();
+          if (leader) PROF_STAMP(3)
           if (leader) {
             issue_S(0, slot); commit(bs_full(0));
             issue_S(1, slot); commit(bs_full(1));
@@ -505,6 +678,39 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     uint32_t tile_it = 0, seg_it = 0, alt_sync_it = 0;
     bool pdl_done = false;
     PROF_DECL(8)
+    const bool fused = kCG == 1 && p.merge_ctr != nullptr;
+    // publish this warpgroup's half of a partial: every thread's stores are fenced, the warpgroup
+    // meets on a named barrier, one thread bumps the arrival counter of the (item, pair) - keyed by
+    // the item's first partial slot, found from the group id (at most one combine item per group)
+    auto find_item = [&](int32_t group) {
+      const CombineItem* items = reinterpret_cast<const CombineItem*>(p.meta + hdr.off_combine);
+      int32_t k = 0;
+      while (k + 1 < hdr.num_combine && items[k].group != group) ++k;
+      return items[k];
+    };
+    auto publish = [&](bool fence_all) {
+      if (!fused) return;
+      // direct stores: every thread fences its own.  Staged path: the only writes are the bulk stores
+      // whose completion lane 0 of each warp has already waited for; the barrier below orders them
+      // before the (cumulative) release of the counter update.
+      if (fence_all) __threadfence();
+      if (threadIdx.x == 0) PROF_STAMP(14)
+      // one release per CTA and partial: both warpgroups meet (decode plan: warpgroup 0 alone)
+      if constexpr (kAlt) asm volatile("bar.sync 2, 128;" ::: "memory");
+      else asm volatile("bar.sync 3, 256;" ::: "memory");
+      if (threadIdx.x == 0) red_release_gpu_add(p.merge_ctr + bars->cur_slot0, 2);
+    };
+    // resolve the merge duty that comes with a partial segment (thread 0, while the first tile loads)
+    auto make_job = [&](const SegView& sv, MergeJob& job) {
+      const CombineItem ci = find_item(sv.group);
+      const int32_t part = (sv.part_base - ci.part_base) / sv.g.npairs;
+      job.slot0 = ci.part_base + pair; job.nparts = ci.nparts; job.npairs = sv.g.npairs; job.kv_head = sv.g.kv_head;
+      job.tok0 = sv.g.q_token0 + pair * tok_per_pair;
+      const int32_t nv = min(kAlt ? kTileRows : kPairRows, (min(sv.g.q_token_end, job.tok0 + tok_per_pair) - job.tok0) * p.G);
+      job.r_lo = (int32_t)((int64_t)part * nv / ci.nparts);
+      job.r_hi = (int32_t)((int64_t)(part + 1) * nv / ci.nparts);
+      job.pad = 0;
+    };
 
     for (int32_t si = seg_lo; si < seg_hi; ++si) {
       SegView sv;
@@ -513,6 +719,14 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const int32_t nt = kAlt ? (sv.tile_end > sv.tile_begin ? (sv.tile_end - sv.tile_begin + 1 - q) / 2 : 0)
                               : sv.tile_end - sv.tile_begin;
       const int32_t part_slot = sv.part_base + pair;
+      if (fused && sv.part_base >= 0 && threadIdx.x == 0) {
+        MergeJob job;
+        make_job(sv, job);
+        const int32_t j = bars->njobs;
+        if (j < kMaxJobs) bars->jobs[j] = job;
+        bars->njobs = j + 1;
+        bars->cur_slot0 = job.slot0;
+      }
       const int32_t tok = sv.g.q_token0 + pair * tok_per_pair + R / p.G;
       const bool row_valid = tok < sv.g.q_token_end && pair < sv.g.npairs;   // (kCG = 2: a ghost CTA computes but stores nothing)
       if (sv.tile_end <= sv.tile_begin) {
@@ -521,6 +735,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         if (!pdl_done) { pdl_wait(); pdl_done = true; }
         if (row_valid && sv.part_base >= 0 && (!kAlt || q == 0))
           p.part_lse[(int64_t)part_slot * kPairRows + R] = -INFINITY;
+        if (sv.part_base >= 0 && (!kAlt || q == 0)) publish(true);
         continue;
       }
       const int32_t head = sv.g.kv_head * p.G + R % p.G;
@@ -533,6 +748,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         PROF_MARK(0)
         mbar_wait(bs_full(q), tile_it & 1);
         tc_fence_after();
+        if (threadIdx.x == 0) PROF_STAMP(4)
         PROF_MARK(1)
         uint32_t pk[64];                                    // P row, packed bf16x2
         const bool need_mask = __any_sync(0xffffffffu, key0 + kTileKeys > vis);
@@ -688,11 +904,14 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       // ---------------------------------------------------- epilogue
       // first global write of this CTA: the predecessor grids (append; transitively the previous
       // step's combine, which reads the partial buffers and writes `out`) must have completed
+      if (threadIdx.x == 0) PROF_STAMP(5)
       if (!pdl_done) { pdl_wait(); pdl_done = true; }
+      if (threadIdx.x == 0) PROF_STAMP(6)
       if (nt > 0) {
         mbar_wait(bo_full(q), seg_it & 1);
         tc_fence_after();
       }
+      if (threadIdx.x == 0) PROF_STAMP(7)
       float inv_l = l > 0.f ? 1.f / l : 0.f;                // coefficient of this set's accumulator
       float lse2 = l > 0.f ? m_used + log2f(l) : -INFINITY;
       float inv_l1 = 0.f;                                   // kAlt: coefficient of accumulator set 1
@@ -729,6 +948,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         }
       }
       const float osc = kAlt ? 1.f : inv_l;                 // kAlt: already applied by the merge above
+      bool pub = false, pub_fence = false;
       if (sv.part_base < 0) {
         __nv_bfloat16* orow = reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)tok * p.Hq + head) * p.D;
 #pragma unroll
@@ -765,6 +985,12 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       } else {
         const int64_t prow = (int64_t)part_slot * kPairRows + R;
         float* orow = p.part_o + prow * p.D;
+        // Last segment of this CTA: nothing else will use the Q tiles (set 0: every S MMA has completed
+        // once o_full(0) fired) or the K/V ring (set 1 / decode plan: every MMA has completed), so the
+        // warp stages its 32 rows x 512 B there and writes them with ONE 16 KB bulk store; rows are
+        // contiguous in the partial buffer.  Otherwise: direct 16-byte stores (same chunk positions).
+        const bool staged = kCG == 1 && si + 1 == seg_hi;
+        const uint32_t stage = ((kAlt || q == 1) ? sRing : sQ) + (uint32_t)(warp & 3) * 16384u + (uint32_t)lane * 512u;
 #pragma unroll
         for (int ch = 0; ch < 4; ++ch) {
           uint32_t o[32];
@@ -782,24 +1008,83 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #pragma unroll
               for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * inv_l);
             }
-          }
-          if (row_valid) {
+          } else {
 #pragma unroll
-            for (int i = 0; i < 32; i += 4) {
-              float4 w = make_float4(__uint_as_float(o[i]) * osc, __uint_as_float(o[i + 1]) * osc,
-                                     __uint_as_float(o[i + 2]) * osc, __uint_as_float(o[i + 3]) * osc);
-              *reinterpret_cast<float4*>(orow + ch * 32 + i) = w;
-            }
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * osc);
+          }
+          if (staged) {
+#pragma unroll
+            for (int i = 0; i < 32; i += 4)
+              st_shared_v4(stage + (uint32_t)part_chunk_pos(ch * 8 + i / 4, lane) * 16u, o[i], o[i + 1], o[i + 2], o[i + 3]);
+          } else if (row_valid) {
+#pragma unroll
+            for (int i = 0; i < 32; i += 4)
+              *reinterpret_cast<uint4*>(orow + part_chunk_pos(ch * 8 + i / 4, R) * 4) = make_uint4(o[i], o[i + 1], o[i + 2], o[i + 3]);
           }
         }
-        if (row_valid) p.part_lse[prow] = lse2;
+        if (staged) {
+          bars->lse_stage[R] = lse2;
+          fence_proxy_async_smem();
+          __syncwarp();
+          if (threadIdx.x == 0) PROF_STAMP(13)
+          if (lane == 0) {
+            bulk_store(p.part_o + (prow - lane) * p.D, stage - (uint32_t)lane * 512u, 16384u);
+            bulk_store(p.part_lse + (prow - lane), smem_u32(&bars->lse_stage[R - lane]), 128u);
+            bulk_commit();
+            bulk_wait_all();
+          }
+          __syncwarp();
+        }
+        if (!staged && row_valid) p.part_lse[prow] = lse2;
+        pub = true; pub_fence = !staged;
       }
       tc_fence_before();
       arrive_leader(bo_empty(q));
       if constexpr (kAlt) { if (use1) mbar_arrive(bo_empty(1)); }
+      if (pub) publish(pub_fence);
+      if (threadIdx.x == 0) PROF_STAMP(8)
       PROF_MARK(6)
       ++seg_it;
     }
+    if (threadIdx.x == 0) PROF_STAMP(9)
+    if (fused && hdr.num_combine > 0) {
+      // ---------------------------------------------------- merge phase (a4)
+      uint32_t merge_phase = 0;
+      asm volatile("bar.sync 1, 256;" ::: "memory");        // jobs[] written by thread 0 are visible
+      const int32_t njobs = bars->njobs;
+      int32_t jn = 0;
+      for (int32_t si = seg_lo; si < seg_hi && jn < njobs; ++si) {
+        MergeJob job;
+        if (njobs <= kMaxJobs) {
+          job = bars->jobs[jn];
+        } else {
+          // more partial segments than parked jobs (many tiny groups per team): re-derive from the metadata
+          SegView sv;
+          if (!load_segment<kCG - 1>(p.meta, hdr, si, clip_pair, tok_per_pair, sv) || sv.part_base < 0) continue;
+          make_job(sv, job);
+        }
+        ++jn;
+        int32_t* ctr = p.merge_ctr + job.slot0;
+        if (warp == 0 && lane == 0) {       // the other warps meet this one on the barrier inside merge_item
+          // relaxed polls (an acquire load also invalidates L1 on every iteration), one acquire at the end
+          while (ld_relaxed_gpu(ctr) < 2 * job.nparts) {}
+          (void)ld_acquire_gpu(ctr);
+        }
+        __syncwarp();
+        if (threadIdx.x == 0) PROF_STAMP(11)
+        merge_item(p, job, sRing, smem_raw + (sRing - smem_u32(smem_raw)), sQ,
+                   smem_raw + (sQ - smem_u32(smem_raw)), smem_u32(&bars->merge_full), merge_phase, warp, lane);
+        __syncwarp();
+        if (threadIdx.x == 0) PROF_STAMP(12)
+        if (warp == 0 && lane == 0) {
+          // the last CTA to get here re-arms the counters for the next launch (every part has been
+          // published and every waiter has passed its wait by then)
+          int32_t* done = ctr + p.max_part_slots;
+          if (atomicAdd(done, 1) == job.nparts - 1) { *done = 0; *ctr = 0; }
+        }
+      }
+    }
+    if (threadIdx.x == 0) PROF_STAMP(10)
 #ifdef WS_PROFILE
     if (blockIdx.x == 5 && lane == 0 && (warp & 3) == 0) printf("SMX%d other %lld waitS %lld ld %lld max %lld exp %lld store %lld epi %lld tiles %u\n", q, prof_acc[0], prof_acc[1], prof_acc[2], prof_acc[3], prof_acc[4], prof_acc[5], prof_acc[6], tile_it);
 #endif
@@ -814,7 +1099,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     unsigned long long g1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(g1));
     int tiles = 0; for (int si = seg_lo; si < seg_hi; ++si) { const Segment sg = reinterpret_cast<const Segment*>(p.meta + hdr.off_segments)[si]; tiles += sg.tile_end - sg.tile_begin; }
     unsigned smid; asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
-    if (blockIdx.x % 37 == 7) printf("CTA %d sm %u segs %d tiles %d cycles %lld t0 %llu t1 %llu\n", blockIdx.x, smid, seg_hi - seg_lo, tiles, clock64() - prof_cta_t0, prof_g0, g1);
+    if (true) printf("CTA %d sm %u segs %d tiles %d cycles %lld t0 %llu dur %llu | setup %lld qissued %lld qfull %lld k0full %lld s0full %lld lasttile %lld pdlwait %lld ofull %lld stored %lld segsdone %lld merged %lld mwaited %lld mitem %lld staged0 %lld fenced0 %lld bar0 %lld staged3 %lld stored3 %lld stored4 %lld bar1 %lld epi0 %lld chdone %lld pfence %lld cpass1 %lld cpass2 %lld cepi %lld\n", blockIdx.x, smid, seg_hi - seg_lo, tiles, clock64() - prof_cta_t0, prof_g0, g1 - prof_g0,
+      (long long)(prof_stamps[0] - prof_g0), (long long)(prof_stamps[1] - prof_g0), (long long)(prof_stamps[2] - prof_g0), (long long)(prof_stamps[3] - prof_g0), (long long)(prof_stamps[4] - prof_g0), (long long)(prof_stamps[5] - prof_g0), (long long)(prof_stamps[6] - prof_g0), (long long)(prof_stamps[7] - prof_g0), (long long)(prof_stamps[8] - prof_g0), (long long)(prof_stamps[9] - prof_g0), (long long)(prof_stamps[10] - prof_g0), (long long)(prof_stamps[11] - prof_g0), (long long)(prof_stamps[12] - prof_g0), (long long)(prof_stamps[13] - prof_g0), (long long)(prof_stamps[14] - prof_g0), (long long)(prof_stamps[18] - prof_g0), (long long)(prof_stamps[15] - prof_g0), (long long)(prof_stamps[16] - prof_g0), (long long)(prof_stamps[17] - prof_g0), (long long)(prof_stamps[19] - prof_g0), 0ll, 0ll, 0ll, (long long)(prof_stamps[22] - prof_stamps[20]), (long long)(prof_stamps[21] - prof_stamps[20]), (long long)(prof_stamps[21] - prof_stamps[20]));
   }
 #endif
   if (warp == 10) {
@@ -841,8 +1127,14 @@ cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(l.num_ctas); cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = kSmemBytes; cfg.stream = stream;
-  cudaLaunchAttribute at[2];
+  cudaLaunchAttribute at[3];
   int na = 0;
+  if (l.p.merge_ctr != nullptr) {
+    // fused combine: CTAs wait on each other's partials, so the whole grid must be co-resident
+    at[na].id = cudaLaunchAttributeCooperative;
+    at[na].val.cooperative = 1;
+    ++na;
+  }
   static const bool no_pdl = getenv("WS_NO_PDL") != nullptr;
   if (!no_pdl) {
     at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;

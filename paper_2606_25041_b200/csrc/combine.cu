@@ -89,7 +89,7 @@ combine_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int3
   packed.x = *reinterpret_cast<uint32_t*>(&lo);
   packed.y = *reinterpret_cast<uint32_t*>(&hi);
   __nv_bfloat16* orow = reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)tok * p.Hq + head) * p.D;
-  reinterpret_cast<uint2*>(orow)[lane] = packed;
+  reinterpret_cast<uint2*>(orow)[lane ^ (r & 7)] = packed;   // partial rows store chunk c at position c ^ (r & 7) (attn_sm100.cu)
   if (p.lse && lane == 0)
     p.lse[(int64_t)tok * p.Hq + head] = (mx_run + log2f(wsum_run)) * 0.6931471805599453f;
 }

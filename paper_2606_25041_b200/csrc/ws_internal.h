@@ -98,6 +98,13 @@ struct AttnParams {
   int32_t Hq, Hkv, D, G, P;
   int32_t total_q_tokens;
   float scale;
+  // fused combine (a4 inside the attention kernel): arrival counters [max_part_slots] followed by
+  // completion counters [max_part_slots], indexed by the first partial slot of a (combine item, pair);
+  // all zero between launches (the last merging warp of an item resets them).  nullptr: the partials
+  // are merged by combine_kernel instead.
+  int32_t* merge_ctr;
+  int32_t max_part_slots;
+  int32_t pad_;
 };
 
 }  // namespace ws
