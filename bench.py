@@ -306,6 +306,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--warm-l2", action="store_true", help="replay one cache even if its history fits L2 (configs 2, 3)")
     ap.add_argument("--no-next", action="store_true", help="skip the NEXT-1 / NEXT-2 side measurements")
+    ap.add_argument("--fused-combine", action="store_true",
+                    help="A/B: merge the split-KV partials inside the attention kernel (WS_FLAG_FUSED_COMBINE)")
     args = ap.parse_args()
     spec = CONFIG_SPECS[args.config]
     if args.impl == "reference":
@@ -316,7 +318,7 @@ def main():
     import torch
     import __graft_entry__ as entry
     entry.build()
-    from paper_2606_25041_b200 import Cache, WS_BF16  # noqa: F401
+    from paper_2606_25041_b200 import Cache, WS_BF16, WS_FLAG_FUSED_COMBINE  # noqa: F401
     from tests.gpu_harness import make_cache, preload_gpu, _torch_of
 
     rank = int(os.environ.get("RANK", "0"))
@@ -346,7 +348,7 @@ def main():
     dev_v = [_torch_of(s.v_cache, dev) for s in w.sessions]
     caches, ids_of = [], []
     for _ in range(R):
-        c = make_cache(w, device=local)
+        c = make_cache(w, device=local, flags=WS_FLAG_FUSED_COMBINE if args.fused_combine else 0)
         caches.append(c)
         ids_of.append(preload_gpu(c, w, dev_k, dev_v))
     cache, ids = caches[0], ids_of[0]

@@ -60,12 +60,13 @@ enum {
   /* Run the tcgen05 kernel on CTA pairs (cta_group::2, M = 256 per MMA, each CTA stages half of every
    * K/V tile) when the plan's team size is even.  Correct but slower on B200. */
   WS_FLAG_CTA_PAIRS = 4u,
-  /* Run the split-KV combine (a4) as its own kernel after the attention kernel instead of inside it.
-   * By default the CTAs of the tcgen05 kernel merge the split partials themselves once every split of
-   * a (session, KV head) group has been published (per-group arrival counters in the workspace; the
-   * kernel is launched cooperatively so that all of its CTAs are co-resident while they wait on each
-   * other).  The separate kernel is kept for A/B measurements and is always used with CTA pairs.   */
-  WS_FLAG_SEPARATE_COMBINE = 8u
+  /* Merge the split-KV partials (a4) inside the attention kernel instead of in the combine kernel that
+   * follows it: every CTA publishes its partials (per-group arrival counters in the workspace), waits
+   * until all splits of its (session, KV head) group are there and merges its share of the rows; the
+   * kernel is then launched cooperatively so that all CTAs are co-resident while they wait on each
+   * other.  Correct and one launch fewer, but measured no faster than the separate kernel on B200
+   * (DESIGN.md section 8), so it is opt-in; never used together with CTA pairs.                     */
+  WS_FLAG_FUSED_COMBINE = 8u
 };
 
 typedef struct ws_cache ws_cache_t;   /* opaque; owns host metadata only */

@@ -17,7 +17,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("WS_LIB_PATH") or os.path.join(_PKG, "libwanstream.so")
 
 WS_BF16, WS_F32 = 0, 1
-WS_FLAG_DRY_RUN, WS_FLAG_FORCE_SIMT, WS_FLAG_CTA_PAIRS = 1, 2, 4
+WS_FLAG_DRY_RUN, WS_FLAG_FORCE_SIMT, WS_FLAG_CTA_PAIRS, WS_FLAG_FUSED_COMBINE = 1, 2, 4, 8
 STATUS_NAMES = ["WS_OK", "WS_ERR_INVALID_ARG", "WS_ERR_BAD_SESSION", "WS_ERR_OUT_OF_PAGES",
                 "WS_ERR_UNSUPPORTED", "WS_ERR_WORKSPACE_TOO_SMALL", "WS_ERR_CUDA"]
 

@@ -626,7 +626,7 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
   L.p.page_table = c->d_page_table;
   L.p.meta = (const int32_t*)d;
   L.p.part_o = c->d_part_o; L.p.part_lse = c->d_part_lse;
-  const bool fused_combine = cta_group == 1 && !(c->cfg.flags & WS_FLAG_SEPARATE_COMBINE) &&
+  const bool fused_combine = cta_group == 1 && (c->cfg.flags & WS_FLAG_FUSED_COMBINE) &&
                              !c->last_plan.combine.empty();
   L.p.merge_ctr = fused_combine ? c->d_merge_ctr : nullptr;
   L.p.max_part_slots = c->lay.max_part_slots;

@@ -70,12 +70,10 @@ constexpr float kFastSumLimit = 1024.0f;                   // fast path accepted
 #define PROF_DECL(n) long long prof_acc[n] = {0}; long long prof_t = clock64();
 #define PROF_MARK(i) { long long t_ = clock64(); prof_acc[i] += t_ - prof_t; prof_t = t_; }
 __device__ __forceinline__ unsigned long long prof_gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-__shared__ unsigned long long prof_stamps[24];
+__shared__ unsigned long long prof_stamps[16];
 #define PROF_STAMP(i) { if (prof_stamps[i] == 0) prof_stamps[i] = prof_gtime(); }
-#define PROF_CLK(i) { if (prof_stamps[i] == 0) prof_stamps[i] = clock64(); }
 #else
 #define PROF_STAMP(i) {}
-#define PROF_CLK(i) {}
 #define PROF_DECL(n)
 #define PROF_MARK(i)
 #endif
@@ -246,9 +244,9 @@ __device__ __forceinline__ void merge_item(const AttnParams& p, const MergeJob& 
                   p.part_lse + (slot0 + part * stride) * kPairRows + c0a, (uint32_t)nl * 4u, bar);
       }
     }
-    if (threadIdx.x == 0) PROF_STAMP(16)
+    if (threadIdx.x == 0) PROF_STAMP(14)
     mbar_wait(bar, phase);
-    if (threadIdx.x == 0) PROF_STAMP(17)
+    if (threadIdx.x == 0) PROF_STAMP(15)
     phase ^= 1u;
     const float* lse_f = reinterpret_cast<const float*>(lse_s) + (c0 - c0a);
     const float4* o_f = reinterpret_cast<const float4*>(ring) + lane;
@@ -374,7 +372,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #ifdef WS_PROFILE
   const long long prof_cta_t0 = clock64();
   unsigned long long prof_g0; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(prof_g0));
-  if (threadIdx.x < 24) prof_stamps[threadIdx.x] = 0;
+  if (threadIdx.x < 16) prof_stamps[threadIdx.x] = 0;
 #endif
 
   if (warp == 8 && lane == 0) {
@@ -461,6 +459,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         ++q_it;
         int32_t pg0 = page_row[min(2 * sv.tile_begin, last_page)];
         int32_t pg1 = page_row[min(2 * sv.tile_begin + 1, last_page)];
+        PROF_STAMP(1)
         for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
           const int32_t c0 = pg0, c1 = pg1;
           if (j + 1 < sv.tile_end) {                        // prefetch next tile's page ids
@@ -541,6 +540,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         if (sv.tile_end <= sv.tile_begin) continue;          // clipped away for this pair
         const int32_t nt = sv.tile_end - sv.tile_begin;
         mbar_wait(bq_full, q_it & 1);
+        if (leader) PROF_STAMP(2)
         if constexpr (kAlt) {
           // S_q <- Q K(tile q) for q = 0, 1; then per tile j (set q = j & 1): O_q += P V(j), S_q <- Q K(j+2)
           for (int q = 0; q < 2 && q < nt; ++q) {
@@ -694,7 +694,6 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       // whose completion lane 0 of each warp has already waited for; the barrier below orders them
       // before the (cumulative) release of the counter update.
       if (fence_all) __threadfence();
-      if (threadIdx.x == 0) PROF_STAMP(14)
       // one release per CTA and partial: both warpgroups meet (decode plan: warpgroup 0 alone)
       if constexpr (kAlt) asm volatile("bar.sync 2, 128;" ::: "memory");
       else asm volatile("bar.sync 3, 256;" ::: "memory");
@@ -989,7 +988,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         // once o_full(0) fired) or the K/V ring (set 1 / decode plan: every MMA has completed), so the
         // warp stages its 32 rows x 512 B there and writes them with ONE 16 KB bulk store; rows are
         // contiguous in the partial buffer.  Otherwise: direct 16-byte stores (same chunk positions).
-        const bool staged = kCG == 1 && si + 1 == seg_hi;
+        const bool staged = kCG == 1 && si + 1 == seg_hi && __all_sync(0xffffffffu, row_valid);   // (few valid rows, e.g. decode steps: store just those)
         const uint32_t stage = ((kAlt || q == 1) ? sRing : sQ) + (uint32_t)(warp & 3) * 16384u + (uint32_t)lane * 512u;
 #pragma unroll
         for (int ch = 0; ch < 4; ++ch) {
@@ -1099,8 +1098,14 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     unsigned long long g1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(g1));
     int tiles = 0; for (int si = seg_lo; si < seg_hi; ++si) { const Segment sg = reinterpret_cast<const Segment*>(p.meta + hdr.off_segments)[si]; tiles += sg.tile_end - sg.tile_begin; }
     unsigned smid; asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
-    if (true) printf("CTA %d sm %u segs %d tiles %d cycles %lld t0 %llu dur %llu | setup %lld qissued %lld qfull %lld k0full %lld s0full %lld lasttile %lld pdlwait %lld ofull %lld stored %lld segsdone %lld merged %lld mwaited %lld mitem %lld staged0 %lld fenced0 %lld bar0 %lld staged3 %lld stored3 %lld stored4 %lld bar1 %lld epi0 %lld chdone %lld pfence %lld cpass1 %lld cpass2 %lld cepi %lld\n", blockIdx.x, smid, seg_hi - seg_lo, tiles, clock64() - prof_cta_t0, prof_g0, g1 - prof_g0,
-      (long long)(prof_stamps[0] - prof_g0), (long long)(prof_stamps[1] - prof_g0), (long long)(prof_stamps[2] - prof_g0), (long long)(prof_stamps[3] - prof_g0), (long long)(prof_stamps[4] - prof_g0), (long long)(prof_stamps[5] - prof_g0), (long long)(prof_stamps[6] - prof_g0), (long long)(prof_stamps[7] - prof_g0), (long long)(prof_stamps[8] - prof_g0), (long long)(prof_stamps[9] - prof_g0), (long long)(prof_stamps[10] - prof_g0), (long long)(prof_stamps[11] - prof_g0), (long long)(prof_stamps[12] - prof_g0), (long long)(prof_stamps[13] - prof_g0), (long long)(prof_stamps[14] - prof_g0), (long long)(prof_stamps[18] - prof_g0), (long long)(prof_stamps[15] - prof_g0), (long long)(prof_stamps[16] - prof_g0), (long long)(prof_stamps[17] - prof_g0), (long long)(prof_stamps[19] - prof_g0), 0ll, 0ll, 0ll, (long long)(prof_stamps[22] - prof_stamps[20]), (long long)(prof_stamps[21] - prof_stamps[20]), (long long)(prof_stamps[21] - prof_stamps[20]));
+    // one line per CTA: ns since the CTA started (globaltimer) at which thread 0 / the producer / the MMA warp
+    // passed each point (first segment / first merge job only)
+    static const char* names[16] = {"setup", "qissued", "qfull", "k0full", "s0full", "lasttile", "pdlwait", "ofull",
+                                    "stored", "segsdone", "merged", "mwaited", "mitem", "staged", "missued", "mloaded"};
+    printf("CTA %d sm %u segs %d tiles %d cycles %lld t0 %llu dur %llu |", blockIdx.x, smid, seg_hi - seg_lo, tiles,
+           clock64() - prof_cta_t0, prof_g0, g1 - prof_g0);
+    for (int i = 0; i < 16; ++i) printf(" %s %lld", names[i], prof_stamps[i] ? (long long)(prof_stamps[i] - prof_g0) : -1ll);
+    printf("\n");
   }
 #endif
   if (warp == 10) {

@@ -196,7 +196,7 @@ def test_cta_pair_variant_config3_shape():
     _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "cfg3-like cta pairs")
 
 
-@pytest.mark.parametrize("splits", [1, 2, 3, 7])
+@pytest.mark.parametrize("splits", [1, 2, 3, 7, 12])
 def test_split_count_invariance(splits):
     w = _small(3, cache_lens=(3000,), block_tokens=128, modality_split=(96, 24, 8))
     got = run_workload_gpu(w, min_splits=splits)
@@ -212,6 +212,50 @@ def test_many_splits_combine_chunks():
     got = run_workload_gpu(w, min_splits=71)
     assert got["plans"][-1]["num_segments"] >= 71
     _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "71 splits")
+
+
+@pytest.mark.parametrize("splits", [2, 3, 12, 71])
+def test_fused_combine(splits):
+    """WS_FLAG_FUSED_COMBINE: the partials are merged inside the attention kernel (arrival counters,
+    cooperative launch) instead of by combine_kernel; both read the same partial-row format and must
+    match the oracle.  Two steps on one cache: the counters re-arm themselves between launches."""
+    from paper_2606_25041_b200 import WS_FLAG_FUSED_COMBINE
+    w = _small(2, cache_lens=(9000,), num_q_heads=4, num_kv_heads=2, block_tokens=96, modality_split=(72, 18, 6), steps=2)
+    fused = run_workload_gpu(w, flags=WS_FLAG_FUSED_COMBINE, min_splits=splits, gather=False)
+    sep = run_workload_gpu(w, min_splits=splits, gather=False)
+    assert sep["plans"][-1]["num_combine_items"] > 0
+    ref = run_workload_oracle(w)
+    _assert_close(compare(sep, ref, "bf16"), BF16_TOL, f"separate combine, splits={splits}")
+    _assert_close(compare(fused, ref, "bf16"), BF16_TOL, f"fused combine, splits={splits}")
+    # same partials, same merge arithmetic up to the exponential used for the weights
+    for t in range(2):
+        assert np.abs(sep["out"][t][0] - fused["out"][t][0]).max() <= 2.0 ** -7 * np.abs(ref["out"][t][0]).max()
+
+
+def test_fused_combine_many_partial_segments_per_cta():
+    """Every group cut into one-tile segments (158 parts per row, > 32) and ~4.3 tiles per CTA: CTAs own more
+    partial segments than merge jobs can be parked in shared memory (overflow path re-derives them), the
+    part count exceeds one warp's lanes, and the merge stages its rows through the ring in several chunks."""
+    w = _small(3, cache_lens=(20000,), num_q_heads=8, num_kv_heads=4, block_tokens=128, modality_split=(96, 24, 8), steps=2)
+    from paper_2606_25041_b200 import WS_FLAG_FUSED_COMBINE
+    got = run_workload_gpu(w, flags=WS_FLAG_FUSED_COMBINE, min_splits=200, gather=False)
+    for plan in got["plans"]:
+        assert plan["num_segments"] >= 4 * 158 and plan["num_segments"] > 4 * plan["num_ctas"]
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "one-tile segments")
+
+
+def test_fused_combine_decode_plan_and_ragged_batch():
+    """WS_FLAG_FUSED_COMBINE on the decode plan (few valid rows per partial: direct stores, warpgroup 0 alone
+    publishes) and on a ragged multi-session batch (teams that walk several groups)."""
+    from paper_2606_25041_b200 import WS_FLAG_FUSED_COMBINE
+    w = _small(3, cache_lens=(6000,), block_tokens=16, modality_split=(12, 3, 1), steps=2)
+    got = run_workload_gpu(w, flags=WS_FLAG_FUSED_COMBINE, min_splits=5, gather=False)
+    assert got["plans"][-1]["used_tensor_core_kernel"] == 3 and got["plans"][-1]["num_combine_items"] > 0
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "fused combine, decode plan")
+    w = _small(5, cache_len_range=(100, 1500), block_tokens=64, modality_split=(48, 12, 4))
+    got = run_workload_gpu(w, flags=WS_FLAG_FUSED_COMBINE, gather=False)
+    tol = dict(BF16_TOL); tol.pop("max_abs"); tol["max_excess"] = 8e-3     # see the ragged test below
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), tol, "fused combine, ragged batch")
 
 
 def test_page_assignment_independence():
