@@ -329,6 +329,7 @@ ws_status_t ws_cache_create(const ws_cache_config_t* cfg, ws_cache_t** out) {
       st = encode_tmap(c.get(), &c->tmap_v, cfg->v_pool, 4, dims, strides, box);
       if (st != WS_OK) return st;
       WS_CUDA(ws::sm100_attn_configure());
+      WS_CUDA(ws::combine_configure());
     }
   }
   WS_CUDA(cudaDeviceSynchronize());
@@ -651,7 +652,9 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
   c->launches += 1;
   if (!c->last_plan.combine.empty() && !fused_combine) {
     TimedLaunch tc(c, &c->t_combine, stream);
-    WS_CUDA(ws::launch_combine(L.p, L.inl, L.inl_words, (int32_t)c->last_plan.combine.size(), c->last_plan.team_size, stream));
+    int32_t max_parts = 1;
+    for (const ws::CombineItem& ci : c->last_plan.combine) max_parts = std::max(max_parts, ci.nparts);
+    WS_CUDA(ws::launch_combine(L.p, L.inl, L.inl_words, (int32_t)c->last_plan.combine.size(), c->last_plan.team_size, max_parts, stream));
     tc.done();
     c->launches += 1;
   }

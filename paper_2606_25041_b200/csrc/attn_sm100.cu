@@ -39,6 +39,7 @@
 
 #include "launch.h"
 #include "sm100_ptx.cuh"
+#include "merge.cuh"
 
 namespace ws {
 
@@ -78,12 +79,6 @@ __shared__ unsigned long long prof_stamps[16];
 #define PROF_MARK(i)
 #endif
 
-// One merge duty of this CTA (fused combine): rows [r_lo, r_hi) of the (item, pair) whose partial slots
-// are slot0 + i * npairs, i < nparts.  Resolved from the metadata when the segment starts (off the
-// critical path) and parked in shared memory until the merge phase.
-struct MergeJob {
-  int32_t slot0, nparts, npairs, kv_head, tok0, r_lo, r_hi, pad;
-};
 constexpr int kMaxJobs = 4;
 
 struct Barriers {
@@ -109,18 +104,18 @@ struct SegView {
 // (pair >= npairs).  For multi-block queries the pair's own visible end clips the tile range: KV
 // tiles beyond the last key any of the pair's rows can see are skipped (block-lower-triangular
 // skipping at pair granularity); `v.tile_end <= v.tile_begin` then means "nothing to compute here".
-template <int kClipPairMask>
-__device__ __forceinline__ bool load_segment(const int32_t* meta, const AttnMeta& hdr, int32_t si,
+template <int kClipPairMask, int W>
+__device__ __forceinline__ bool load_segment(const MetaView<W>& meta, const AttnMeta& hdr, int32_t si,
                                              int32_t pair, int32_t tok_per_pair, SegView& v) {
   // `pair` is the LAST row-tile pair handled by this CTA group (the CTA's own pair for kCG = 1, the
   // odd pair of the cluster for kCG = 2): both CTAs of a pair must walk the same tile range.
-  const Segment s = reinterpret_cast<const Segment*>(meta + hdr.off_segments)[si];
-  v.g = reinterpret_cast<const Group*>(meta + hdr.off_groups)[s.group];
+  const Segment s = meta.template load<Segment>(hdr.off_segments + si * (int32_t)(sizeof(Segment) / 4));
+  v.g = meta.template load<Group>(hdr.off_groups + s.group * (int32_t)(sizeof(Group) / 4));
   v.tile_begin = s.tile_begin; v.tile_end = s.tile_end; v.part_base = s.part_base; v.group = s.group;
   if ((pair & ~(int32_t)(kClipPairMask)) >= v.g.npairs) return false;
   if (v.g.vis_off >= 0) {
     const int32_t last_tok = min(v.g.q_token_end, v.g.q_token0 + (pair + 1) * tok_per_pair) - 1;
-    const int32_t pair_kv = (meta + hdr.off_vis)[v.g.vis_off + (last_tok - v.g.q_token0)];
+    const int32_t pair_kv = meta[hdr.off_vis + v.g.vis_off + (last_tok - v.g.q_token0)];
     v.tile_end = min(v.tile_end, (pair_kv + kTileKeys - 1) / kTileKeys);
   }
   return true;
@@ -207,126 +202,6 @@ __device__ __forceinline__ void red_release_gpu_add(int32_t* p, int32_t v) {
   asm volatile("red.release.gpu.global.add.s32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
 }
 
-// Partial-row storage format (private to the writers and the mergers): the 16-byte chunk c of packed row
-// r (4 of the row's 128 fp32) lives at chunk position c ^ (r & 7) of the row's 512 bytes.  The XOR makes
-// the thread-per-row shared-memory staging of the epilogue conflict-free (8 consecutive rows hit 8
-// different 16-byte bank groups) while a row stays one contiguous 512-byte run in global memory.
-__device__ __forceinline__ int part_chunk_pos(int c, int r) { return c ^ (r & 7); }
-
-// The 256 softmax threads (8 warps) merge packed rows [r_lo, r_hi) of one (item, pair).  The rows'
-// partials are contiguous per part ([slot][256 rows][128] fp32, [slot][256] LSEs), so each part is ONE
-// bulk copy of O rows into the (idle) K/V ring plus one of LSEs into the (idle) Q tiles; every copy of
-// the item is in flight at once and the merge itself reads shared memory only.  Warp w handles rows
-// w, w + 8, ...; lane = 16-byte chunk position of the row.  Every lane recomputes the row's weights
-// from the LSEs (broadcast shared-memory reads: no shuffles), kMR rows interleaved for ILP.
-constexpr int kMergeRowsCap = (int)(kRingBytes / 512);     // 320 rows of 512 B fit the ring
-constexpr int kMR = 4;
-__device__ __forceinline__ void merge_item(const AttnParams& p, const MergeJob& job,
-                                           uint32_t sRing, const uint8_t* ring, uint32_t sLse, const uint8_t* lse_s,
-                                           uint32_t bar, uint32_t& phase, int warp, int lane) {
-  const int32_t nparts = job.nparts, r_lo = job.r_lo, r_hi = job.r_hi, tok0 = job.tok0;
-  const int64_t slot0 = job.slot0, stride = job.npairs;
-  if (r_hi <= r_lo) return;
-  const int32_t rc = min(r_hi - r_lo, kMergeRowsCap / nparts);
-  const int32_t lse_stride = (rc + 8) & ~3;                 // floats per part in the LSE staging area
-  for (int32_t c0 = r_lo; c0 < r_hi; c0 += rc) {
-    const int32_t n = min(rc, r_hi - c0);
-    const int32_t c0a = c0 & ~3, nl = ((c0 + n + 3) & ~3) - c0a;   // 16-byte aligned LSE run covering [c0, c0 + n)
-    asm volatile("bar.sync 1, 256;" ::: "memory");          // ring idle: all MMAs of this CTA / the previous chunk done
-    if (warp == 0) {
-      fence_proxy_async_all();            // the parts were written through the generic proxy (other CTAs)
-      if (lane == 0) mbar_arrive_expect_tx(bar, (uint32_t)((n * 512 + nl * 4) * nparts));
-      __syncwarp();
-      for (int32_t part = lane; part < nparts; part += 32) {
-        bulk_load(sRing + (uint32_t)(part * rc) * 512u,
-                  p.part_o + ((slot0 + part * stride) * kPairRows + c0) * 128, (uint32_t)n * 512u, bar);
-        bulk_load(sLse + (uint32_t)(part * lse_stride) * 4u,
-                  p.part_lse + (slot0 + part * stride) * kPairRows + c0a, (uint32_t)nl * 4u, bar);
-      }
-    }
-    if (threadIdx.x == 0) PROF_STAMP(14)
-    mbar_wait(bar, phase);
-    if (threadIdx.x == 0) PROF_STAMP(15)
-    phase ^= 1u;
-    const float* lse_f = reinterpret_cast<const float*>(lse_s) + (c0 - c0a);
-    const float4* o_f = reinterpret_cast<const float4*>(ring) + lane;
-    for (int32_t lr0 = warp; lr0 < n; lr0 += 8 * kMR) {
-      float mx[kMR], ws[kMR];
-      float4 acc[kMR];
-      const float* lp[kMR];
-      const float4* op[kMR];
-#pragma unroll
-      for (int b = 0; b < kMR; ++b) {
-        const int32_t lr = min(lr0 + 8 * b, n - 1);         // (rows past the end repeat the last one; not stored)
-        lp[b] = lse_f + lr; op[b] = o_f + lr * 32;
-        mx[b] = -INFINITY; ws[b] = 0.f; acc[b] = make_float4(0.f, 0.f, 0.f, 0.f);
-      }
-      if (nparts <= 8) {
-        // common case: every load of the batch is issued before the first use (unrolled over the parts)
-        float lv[kMR][8];
-#pragma unroll
-        for (int k = 0; k < 8; ++k)
-#pragma unroll
-          for (int b = 0; b < kMR; ++b) {
-            lv[b][k] = k < nparts ? lp[b][k * lse_stride] : -INFINITY;
-            mx[b] = fmaxf(mx[b], lv[b][k]);
-          }
-#pragma unroll
-        for (int k = 0; k < 8; ++k)
-          if (k < nparts) {
-#pragma unroll
-            for (int b = 0; b < kMR; ++b) {
-              const float w = lv[b][k] == -INFINITY ? 0.f : ex2_approx(lv[b][k] - mx[b]);
-              const float4 v = op[b][k * rc * 32];
-              ws[b] += w;
-              acc[b].x = fmaf(w, v.x, acc[b].x); acc[b].y = fmaf(w, v.y, acc[b].y);
-              acc[b].z = fmaf(w, v.z, acc[b].z); acc[b].w = fmaf(w, v.w, acc[b].w);
-            }
-          }
-      } else {
-        for (int32_t k = 0; k < nparts; ++k)
-#pragma unroll
-          for (int b = 0; b < kMR; ++b) mx[b] = fmaxf(mx[b], lp[b][k * lse_stride]);
-        for (int32_t k = 0; k < nparts; ++k) {
-#pragma unroll
-          for (int b = 0; b < kMR; ++b) {
-            const float lv = lp[b][k * lse_stride];
-            const float w = lv == -INFINITY ? 0.f : ex2_approx(lv - mx[b]);   // (mx = -inf only if every lv is)
-            const float4 v = op[b][k * rc * 32];
-            ws[b] += w;
-            acc[b].x = fmaf(w, v.x, acc[b].x); acc[b].y = fmaf(w, v.y, acc[b].y);
-            acc[b].z = fmaf(w, v.z, acc[b].z); acc[b].w = fmaf(w, v.w, acc[b].w);
-          }
-        }
-      }
-      // branch-free up to the stores, so that the kMR rows' address / normalisation chains interleave
-      uint2 packed[kMR];
-      uint2* dst[kMR];
-      float* ldst[kMR];
-      float lse_out[kMR];
-      const uint32_t G = (uint32_t)p.G;
-#pragma unroll
-      for (int b = 0; b < kMR; ++b) {
-        const uint32_t r = (uint32_t)(c0 + min(lr0 + 8 * b, n - 1));
-        const uint32_t dt = r / G, hh = r - dt * G;
-        const int64_t row = (int64_t)(tok0 + (int32_t)dt) * p.Hq + job.kv_head * p.G + (int32_t)hh;
-        const float inv = ws[b] > 0.f ? __fdividef(1.f, ws[b]) : 0.f;
-        packed[b].x = pack_bf16x2(acc[b].x * inv, acc[b].y * inv);
-        packed[b].y = pack_bf16x2(acc[b].z * inv, acc[b].w * inv);
-        dst[b] = reinterpret_cast<uint2*>(reinterpret_cast<__nv_bfloat16*>(p.out) + row * p.D) + part_chunk_pos(lane, (int)r);
-        ldst[b] = p.lse + row;
-        lse_out[b] = ws[b] > 0.f ? (mx[b] + __log2f(ws[b])) * 0.6931471805599453f : -INFINITY;
-      }
-#pragma unroll
-      for (int b = 0; b < kMR; ++b)
-        if (lr0 + 8 * b < n) {
-          *dst[b] = packed[b];                              // this lane holds logical chunk lane ^ (r & 7)
-          if (p.lse && lane == 0) *ldst[b] = lse_out[b];
-        }
-    }
-  }
-}
-
 // kAlt: decode plan (plan.h) - both accumulator sets use Q tile 0; set q processes the KV tiles of the
 // segment with (tile - tile_begin) % 2 == q and writes its own partial (slot part_base + q).
 template <int kCG, int kInlW, bool kAlt>
@@ -337,7 +212,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ InlineMeta<kInlW> inl, const AttnParams p_in) {
   static_assert(!(kAlt && kCG == 2), "the decode plan runs on single CTAs");
   AttnParams p = p_in;
-  if (p.meta == nullptr) p.meta = inl.w;
+  const MetaView<kInlW> meta{p.meta, inl};
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem_base;                           // 2 x 32 KB
@@ -361,12 +236,11 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
   const int lane = threadIdx.x & 31;
-  const AttnMeta hdr = *reinterpret_cast<const AttnMeta*>(p.meta);
+  const AttnMeta hdr = meta.template load<AttnMeta>(0);
   const int32_t team = blockIdx.x / hdr.team_size;
   const int32_t pair = blockIdx.x - team * hdr.team_size;
   const int32_t clip_pair = kCG == 2 ? (pair | 1) : pair;  // see load_segment
-  const int32_t* tsb = p.meta + hdr.off_team_seg_begin;
-  const int32_t seg_lo = tsb[team], seg_hi = tsb[team + 1];
+  const int32_t seg_lo = meta[hdr.off_team_seg_begin + team], seg_hi = meta[hdr.off_team_seg_begin + team + 1];
   const int32_t tok_per_pair = kPairRows / p.G;
   const int32_t tok_per_tile = kTileRows / p.G;
 #ifdef WS_PROFILE
@@ -407,7 +281,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       bool dep_waited = false;
       for (int32_t si = seg_lo; si < seg_hi; ++si) {
         SegView sv;
-        if (!load_segment<kCG - 1>(p.meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
+        if (!load_segment<kCG - 1>(meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
         if (sv.tile_end <= sv.tile_begin) continue;          // clipped away for this pair
         const int32_t* page_row = p.page_table + (int64_t)sv.g.slot * p.max_pages_per_session;
         const int32_t last_page = (sv.g.kv_len - 1) / p.P;
@@ -536,7 +410,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       };
       for (int32_t si = seg_lo; si < seg_hi; ++si) {
         SegView sv;
-        if (!load_segment<kCG - 1>(p.meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
+        if (!load_segment<kCG - 1>(meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
         if (sv.tile_end <= sv.tile_begin) continue;          // clipped away for this pair
         const int32_t nt = sv.tile_end - sv.tile_begin;
         mbar_wait(bq_full, q_it & 1);
@@ -683,10 +557,9 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     // meets on a named barrier, one thread bumps the arrival counter of the (item, pair) - keyed by
     // the item's first partial slot, found from the group id (at most one combine item per group)
     auto find_item = [&](int32_t group) {
-      const CombineItem* items = reinterpret_cast<const CombineItem*>(p.meta + hdr.off_combine);
       int32_t k = 0;
-      while (k + 1 < hdr.num_combine && items[k].group != group) ++k;
-      return items[k];
+      while (k + 1 < hdr.num_combine && meta[hdr.off_combine + k * (int32_t)(sizeof(CombineItem) / 4)] != group) ++k;
+      return meta.template load<CombineItem>(hdr.off_combine + k * (int32_t)(sizeof(CombineItem) / 4));
     };
     auto publish = [&](bool fence_all) {
       if (!fused) return;
@@ -713,7 +586,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 
     for (int32_t si = seg_lo; si < seg_hi; ++si) {
       SegView sv;
-      if (!load_segment<kCG - 1>(p.meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
+      if (!load_segment<kCG - 1>(meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
       // kAlt: this warpgroup takes tiles tile_begin + q, + q + 2, ...
       const int32_t nt = kAlt ? (sv.tile_end > sv.tile_begin ? (sv.tile_end - sv.tile_begin + 1 - q) / 2 : 0)
                               : sv.tile_end - sv.tile_begin;
@@ -739,7 +612,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       }
       const int32_t head = sv.g.kv_head * p.G + R % p.G;
       int32_t vis = sv.g.kv_len;
-      if (sv.g.vis_off >= 0 && row_valid) vis = (p.meta + hdr.off_vis)[sv.g.vis_off + (tok - sv.g.q_token0)];
+      if (sv.g.vis_off >= 0 && row_valid) vis = meta[hdr.off_vis + sv.g.vis_off + (tok - sv.g.q_token0)];
       float m_used = -INFINITY, l = 0.f;
 
       for (int32_t j = 0; j < nt; ++j) {
@@ -1059,7 +932,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         } else {
           // more partial segments than parked jobs (many tiny groups per team): re-derive from the metadata
           SegView sv;
-          if (!load_segment<kCG - 1>(p.meta, hdr, si, clip_pair, tok_per_pair, sv) || sv.part_base < 0) continue;
+          if (!load_segment<kCG - 1>(meta, hdr, si, clip_pair, tok_per_pair, sv) || sv.part_base < 0) continue;
           make_job(sv, job);
         }
         ++jn;
@@ -1071,7 +944,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         }
         __syncwarp();
         if (threadIdx.x == 0) PROF_STAMP(11)
-        merge_item(p, job, sRing, smem_raw + (sRing - smem_u32(smem_raw)), sQ,
+        merge_item(p, job, (int32_t)(kRingBytes / 512), sRing, smem_raw + (sRing - smem_u32(smem_raw)), sQ,
                    smem_raw + (sQ - smem_u32(smem_raw)), smem_u32(&bars->merge_full), merge_phase, warp, lane);
         __syncwarp();
         if (threadIdx.x == 0) PROF_STAMP(12)
@@ -1096,7 +969,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #ifdef WS_PROFILE
   if (threadIdx.x == 0) {
     unsigned long long g1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(g1));
-    int tiles = 0; for (int si = seg_lo; si < seg_hi; ++si) { const Segment sg = reinterpret_cast<const Segment*>(p.meta + hdr.off_segments)[si]; tiles += sg.tile_end - sg.tile_begin; }
+    int tiles = 0; for (int si = seg_lo; si < seg_hi; ++si) { const Segment sg = meta.template load<Segment>(hdr.off_segments + si * 4); tiles += sg.tile_end - sg.tile_begin; }
     unsigned smid; asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
     // one line per CTA: ns since the CTA started (globaltimer) at which thread 0 / the producer / the MMA warp
     // passed each point (first segment / first merge job only)

@@ -1,20 +1,29 @@
-// combine.cu - a4: split-KV combine.  The paper is silent on this step; north_star names it.
-// Attention over a disjoint union of key ranges is the LSE-weighted mean of the per-range results:
-//   m* = max_s LSE_s ; w_s = 2^(LSE_s - m*) ; O = sum_s w_s O_s / sum_s w_s ; LSE = m* + log2 sum_s w_s
-// (partials carry log2-domain LSEs; an empty range carries LSE = -inf and contributes w = 0).
-// HBM/L2-bound: reads nparts x 256 x (D+1) fp32 per (group, pair), writes bf16 O (+ fp32 LSE).
-// One warp per packed row: lane s loads the LSE of part s, the max and the weight sum are reduced
-// with warp shuffles, then the parts' O rows (one float4 per lane, D = 128) are accumulated with
-// kDepth loads in flight per lane.
+// combine.cu - a4: split-KV combine as its own kernel (the default; WS_FLAG_FUSED_COMBINE moves the same
+// merge into the attention kernel).  The paper is silent on this step; north_star names it.
+// Attention over a disjoint union of key ranges is the LSE-weighted mean of the per-range results (merge.cuh).
+// HBM/L2-bound: reads nparts x rows x (D+1) fp32 per (group, pair), writes bf16 O (+ fp32 LSE).
+//
+// One 256-thread block merges up to 32 packed rows of one (combine item, row-tile pair).  The rows of
+// one part are contiguous in the partial buffer ([slot][256 rows][128] fp32), so the block fetches each
+// part with ONE bulk copy (cp.async.bulk, completion on an mbarrier) into shared memory - every byte the
+// block needs is in flight at once, a single exposed L2/HBM latency - and then merges from shared memory
+// (merge_item, shared with the fused path).  The earlier one-warp-per-row version paid two dependent
+// global latencies per row (LSEs, then O rows): 11-15 us per config-4 step against ~2.5 us of L2 traffic.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <math.h>
 #include <string.h>
 
 #include "launch.h"
+#include "merge.cuh"
 
 namespace ws {
 
+// ---- row-per-warp variant: few rows with many parts each (decode steps, heavily split short steps) ----
+// One warp per packed row: lane s loads the LSE of part s, the max and the weight sum are reduced with warp
+// shuffles, then the parts' O rows (one float4 per lane, D = 128) are accumulated with kDepth loads in flight
+// per lane.  Two dependent global latencies per row, but thousands of independent warps: better than the
+// staged kernel below when a block would stage only a handful of rows.
 constexpr int kCombineRowsPerBlock = 8;
 
 // kDepth = O-row loads in flight per lane: 4 keeps the kernel at 64 registers (8 blocks / SM) for
@@ -22,18 +31,18 @@ constexpr int kCombineRowsPerBlock = 8;
 // have work and memory-level parallelism has to come from each of them.
 template <int kInlW, int kDepth>
 __global__ void __launch_bounds__(kCombineRowsPerBlock * 32)
-combine_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int32_t team_size) {
+combine_rows_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int32_t team_size) {
   pdl_wait();                      // partials of the attention kernel launched just before
   pdl_launch_dependents();         // the next step's append does not depend on this kernel
-  if (p.meta == nullptr) p.meta = inl.w;
-  const AttnMeta hdr = *reinterpret_cast<const AttnMeta*>(p.meta);
+  const MetaView<kInlW> meta{p.meta, inl};
+  const AttnMeta hdr = meta.template load<AttnMeta>(0);
   const int32_t blocks_per_pair = kPairRows / kCombineRowsPerBlock;
   int32_t b = blockIdx.x;
   const int32_t rchunk = b % blocks_per_pair; b /= blocks_per_pair;
   const int32_t pair = b % team_size;
   const int32_t item = b / team_size;
-  const CombineItem ci = reinterpret_cast<const CombineItem*>(p.meta + hdr.off_combine)[item];
-  const Group g = reinterpret_cast<const Group*>(p.meta + hdr.off_groups)[ci.group];
+  const CombineItem ci = meta.template load<CombineItem>(hdr.off_combine + item * (int32_t)(sizeof(CombineItem) / 4));
+  const Group g = meta.template load<Group>(hdr.off_groups + ci.group * (int32_t)(sizeof(Group) / 4));
   if (pair >= g.npairs) return;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const int32_t r = rchunk * kCombineRowsPerBlock + wib;
@@ -94,20 +103,80 @@ combine_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int3
     p.lse[(int64_t)tok * p.Hq + head] = (mx_run + log2f(wsum_run)) * 0.6931471805599453f;
 }
 
+
+// ---- staged variant ----
+constexpr int kCombineRowsMax = 32;                    // rows per block (fewer when a row has many parts)
+constexpr int kCombineRowsCap = 192;                   // staged rows x parts per chunk: 96 KB -> 2 blocks / SM
+constexpr uint32_t kCombineLseBytes = 8192;            // nparts x (rows + 8) fp32, nparts <= 148
+constexpr uint32_t kCombineSmem = kCombineRowsCap * 512 + kCombineLseBytes + 1024;
+
+template <int kInlW>
+__global__ void __launch_bounds__(256)
+combine_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int32_t team_size, int32_t rows_pb) {
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ uint64_t bar;
+  const uint32_t sO = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint8_t* o_s = smem_raw + (sO - smem_u32(smem_raw));
+  const uint32_t sLse = sO + kCombineRowsCap * 512;
+  const MetaView<kInlW> meta{p.meta, inl};
+  const AttnMeta hdr = meta.template load<AttnMeta>(0);
+  const int32_t chunks = (kPairRows + rows_pb - 1) / rows_pb;
+  int32_t b = blockIdx.x;
+  const int32_t rchunk = b % chunks; b /= chunks;
+  const int32_t pair = b % team_size;
+  const int32_t item = b / team_size;
+  const CombineItem ci = meta.template load<CombineItem>(hdr.off_combine + item * (int32_t)(sizeof(CombineItem) / 4));
+  const Group g = meta.template load<Group>(hdr.off_groups + ci.group * (int32_t)(sizeof(Group) / 4));
+  MergeJob job;
+  job.slot0 = ci.part_base + pair; job.nparts = ci.nparts; job.npairs = g.npairs; job.kv_head = g.kv_head;
+  job.tok0 = g.q_token0 + pair * (kPairRows / p.G);
+  const int32_t nv = min(hdr.alt ? kTileRows : kPairRows, (min(g.q_token_end, job.tok0 + kPairRows / p.G) - job.tok0) * p.G);
+  job.r_lo = rchunk * rows_pb; job.r_hi = min(nv, job.r_lo + rows_pb); job.pad = 0;
+  const bool active = pair < g.npairs && job.r_lo < job.r_hi;     // block-uniform
+  if (threadIdx.x == 0) { mbar_init(smem_u32(&bar), 1); fence_mbar_init(); }
+  __syncthreads();
+  pdl_wait();                      // partials of the attention kernel launched just before
+  pdl_launch_dependents();         // the next step's append does not depend on this kernel
+  if (!active) return;
+  uint32_t phase = 0;
+  // the LSE area holds nparts x ((rows + 8) & ~3) floats: shrink the chunk for very many parts
+  const int32_t lse_cap = (int32_t)(kCombineLseBytes / 4) / ci.nparts - 8;
+  merge_item(p, job, min(kCombineRowsCap, max(1, lse_cap) * ci.nparts), sO, o_s, sLse,
+             smem_raw + (sLse - smem_u32(smem_raw)), smem_u32(&bar), phase, (int)(threadIdx.x >> 5), (int)(threadIdx.x & 31));
+}
+
+cudaError_t combine_configure() {
+  cudaError_t e = cudaFuncSetAttribute((const void*)combine_kernel<kInlineAttnWords>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCombineSmem);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute((const void*)combine_kernel<kInlineAttnWordsLarge>,
+                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kCombineSmem);
+}
+
 cudaError_t launch_combine(const AttnParams& p, const InlineAttnMetaLarge& inl, int32_t inl_words,
-                           int32_t num_combine, int32_t team_size, cudaStream_t stream) {
+                           int32_t num_combine, int32_t team_size, int32_t max_parts, cudaStream_t stream) {
   if (num_combine == 0) return cudaSuccess;
-  int32_t grid = num_combine * team_size * (kPairRows / kCombineRowsPerBlock);
-  const dim3 g(grid), b(kCombineRowsPerBlock * 32);
-  const bool deep = grid <= 2 * 148;
-  if (inl_words <= kInlineAttnWords) {
-    InlineAttnMeta small;
-    memcpy(small.w, inl.w, sizeof(small.w));
-    if (deep) return launch_pdl(combine_kernel<kInlineAttnWords, 8>, g, b, 0, stream, p, small, team_size);
-    return launch_pdl(combine_kernel<kInlineAttnWords, 4>, g, b, 0, stream, p, small, team_size);
+  const bool small_tier = inl_words <= kInlineAttnWords;
+  InlineAttnMeta small;
+  if (small_tier) memcpy(small.w, inl.w, sizeof(small.w));
+  if (max_parts > 8) {
+    // many parts per row: a staged block would hold only a few rows - one warp per row instead
+    const int32_t grid = num_combine * team_size * (kPairRows / kCombineRowsPerBlock);
+    const dim3 g(grid), b(kCombineRowsPerBlock * 32);
+    const bool deep = grid <= 2 * 148;
+    if (small_tier) {
+      if (deep) return launch_pdl(combine_rows_kernel<kInlineAttnWords, 8>, g, b, 0, stream, p, small, team_size);
+      return launch_pdl(combine_rows_kernel<kInlineAttnWords, 4>, g, b, 0, stream, p, small, team_size);
+    }
+    if (deep) return launch_pdl(combine_rows_kernel<kInlineAttnWordsLarge, 8>, g, b, 0, stream, p, inl, team_size);
+    return launch_pdl(combine_rows_kernel<kInlineAttnWordsLarge, 4>, g, b, 0, stream, p, inl, team_size);
   }
-  if (deep) return launch_pdl(combine_kernel<kInlineAttnWordsLarge, 8>, g, b, 0, stream, p, inl, team_size);
-  return launch_pdl(combine_kernel<kInlineAttnWordsLarge, 4>, g, b, 0, stream, p, inl, team_size);
+  // rows per block: as many as fit the staging area in one piece for the item with the most parts
+  const int32_t rows_pb = std::max(1, std::min(kCombineRowsMax, kCombineRowsCap / std::max(1, max_parts)));
+  const int32_t grid = num_combine * team_size * ((kPairRows + rows_pb - 1) / rows_pb);
+  const dim3 g(grid), b(256);
+  if (small_tier) return launch_pdl(combine_kernel<kInlineAttnWords>, g, b, kCombineSmem, stream, p, small, team_size, rows_pb);
+  return launch_pdl(combine_kernel<kInlineAttnWordsLarge>, g, b, kCombineSmem, stream, p, inl, team_size, rows_pb);
 }
 
 }  // namespace ws

@@ -21,21 +21,23 @@ kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
   // Nothing this kernel touches is produced by its stream predecessor (the previous step's combine
   // writes only `out`), so the successor (this step's attention) may start its prologue right away.
   pdl_launch_dependents();
-  const int32_t* meta = meta_g ? meta_g : inl.w;
-  const AppendMeta hdr = *reinterpret_cast<const AppendMeta*>(meta);
-  const AppendSession* sess = reinterpret_cast<const AppendSession*>(meta + hdr.off_sessions);
-  const int32_t* pages = meta + hdr.off_pages;
+  const MetaView<kInlineAppendWords> meta{meta_g, inl};    // (constant-bank reads when the blob is inline)
+  const AppendMeta hdr = meta.load<AppendMeta>(0);
+  constexpr int32_t kSessWords = (int32_t)(sizeof(AppendSession) / 4);
+  auto sess = [&](int32_t s) { return meta.load<AppendSession>(hdr.off_sessions + s * kSessWords); };
+  auto sess_tok_end = [&](int32_t s) { return meta[hdr.off_sessions + s * kSessWords + 3]; };
+  auto pages = [&](int32_t i) { return meta[hdr.off_pages + i]; };
   const int32_t chunks_per_token = Hkv * chunks_per_head;
   const int64_t total = (int64_t)hdr.total_tokens * chunks_per_token;
 
   // Block 0 also publishes the page ids into the persistent device page table (idempotent).
   if (blockIdx.x == 0) {
     for (int32_t s = 0; s < hdr.num_sessions; ++s) {
-      const AppendSession a = sess[s];
+      const AppendSession a = sess(s);
       int32_t first = a.len_old / P;
       int32_t last = (a.len_old + (a.tok_end - a.tok_begin) + P - 1) / P;
       for (int32_t i = first + threadIdx.x; i < last; i += blockDim.x)
-        page_table[(int64_t)a.slot * max_pages + i] = pages[a.page_off + (i - first)];
+        page_table[(int64_t)a.slot * max_pages + i] = pages(a.page_off + (i - first));
     }
   }
   for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
@@ -46,11 +48,11 @@ kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
     int32_t lo = 0, hi = hdr.num_sessions - 1;
     while (lo < hi) {
       int32_t mid = (lo + hi) >> 1;
-      if (tok >= sess[mid].tok_end) lo = mid + 1; else hi = mid;
+      if (tok >= sess_tok_end(mid)) lo = mid + 1; else hi = mid;
     }
-    const AppendSession a = sess[lo];
+    const AppendSession a = sess(lo);
     int32_t pos = a.len_old + (tok - a.tok_begin);
-    int32_t page = pages[a.page_off + (pos / P - a.len_old / P)];
+    int32_t page = pages(a.page_off + (pos / P - a.len_old / P));
     int32_t head = c / chunks_per_head;
     int32_t off = c - head * chunks_per_head;
     int64_t dst = (((int64_t)page * Hkv + head) * P + (pos % P)) * chunks_per_head + off;
@@ -67,11 +69,11 @@ kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
   {
     const int4 zero = make_int4(0, 0, 0, 0);
     for (int32_t s = 0; s < hdr.num_sessions; ++s) {
-      const AppendSession a = sess[s];
+      const AppendSession a = sess(s);
       const int32_t len_new = a.len_old + (a.tok_end - a.tok_begin);
       const int32_t tail = (P - len_new % P) % P;
       if (tail == 0) continue;
-      const int32_t page = pages[a.page_off + ((len_new - 1) / P - a.len_old / P)];
+      const int32_t page = pages(a.page_off + ((len_new - 1) / P - a.len_old / P));
       const int64_t total_tail = (int64_t)tail * chunks_per_token;
       for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total_tail;
            idx += (int64_t)gridDim.x * blockDim.x) {
@@ -172,7 +174,10 @@ cudaError_t launch_kv_append(const void* k_new, const void* v_new, void* k_pool,
                              int32_t D, int32_t eb, int32_t num_sms, cudaStream_t stream) {
   int32_t cph = D * eb / 16;
   int64_t total = (int64_t)total_tokens * Hkv * cph;
-  int64_t blocks = (total + 255) / 256;
+  // (a short append still zeroes up to P - 1 token rows of the last page: size the grid for that too -
+  // a one-token decode append ran 11.8 us as a single block)
+  int64_t work = std::max<int64_t>(total, (int64_t)(P - 1) * Hkv * cph);
+  int64_t blocks = (work + 255) / 256;
   int32_t grid = (int32_t)std::min<int64_t>(std::max<int64_t>(blocks, 1), (int64_t)num_sms * 8);
   return launch_pdl(kv_append_kernel, dim3(grid), dim3(256), 0, stream, (const int4*)k_new,
                     (const int4*)v_new, (int4*)k_pool, (int4*)v_pool, page_table, meta, inl, peers,

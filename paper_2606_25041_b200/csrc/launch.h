@@ -72,7 +72,8 @@ struct Sm100Launch {
 };
 cudaError_t sm100_attn_configure();    // one-time cudaFuncSetAttribute
 cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream);
+cudaError_t combine_configure();        // one-time cudaFuncSetAttribute
 cudaError_t launch_combine(const AttnParams& p, const InlineAttnMetaLarge& inl, int32_t inl_words,
-                           int32_t num_combine, int32_t team_size, cudaStream_t stream);
+                           int32_t num_combine, int32_t team_size, int32_t max_parts, cudaStream_t stream);
 
 }  // namespace ws
