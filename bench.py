@@ -504,7 +504,7 @@ def main():
 
     # ---- side measurements of the widened rows; not part of `value`
     nxt = None
-    if not args.no_next and world == 1 and R == 1:
+    if not args.no_next and world == 1 and R == 1 and plan["used_tensor_core_kernel"]:
         nxt = measure_next(cache, ids, base_blocks, sp, cu, q_d[0], k_d[0], v_d[0], out, dev, timed, reset)
 
     # ---- the same step without host work: one CUDA graph holding one step per cache, replayed
