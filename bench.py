@@ -53,29 +53,49 @@ def oracle_threads() -> int:
         return os.cpu_count() or 1
 
 
-def oracle_sample_seconds(w, rows, budget_steps=1):
-    """Time the oracle (as it stands) on `rows` query tokens x all heads of step 0. Returns (s, flops)."""
-    from tests.gpu_harness import preload_rounds
-    from oracle.block_causal import OracleSession, attend
-    sp = w.spec
-    sess = []
-    for s, si in enumerate(w.sessions):
-        o = OracleSession(sp.num_kv_heads, sp.head_dim)
-        for ids, rng in preload_rounds(w):
-            for sidx, (lo, hi) in zip(ids, rng):
-                if sidx == s:
-                    o.append(si.k_cache[lo:hi], si.v_cache[lo:hi])
-        sess.append(o)
-    t0 = time.perf_counter()
-    flops = 0.0
-    for _ in range(budget_steps):
+class OracleSampler:
+    """The oracle (as it stands) on a sample of query tokens of unit 1: sessions are built once (untimed),
+    every step() commits the unit's K/V, attends `rows` query tokens x all heads and rolls the commit back,
+    so that every repetition times the same work."""
+
+    def __init__(self, w, kv_heads=None):
+        """kv_heads: sample only the first `kv_heads` KV heads (with their query heads); heads are independent."""
+        from tests.gpu_harness import preload_rounds
+        from oracle.block_causal import OracleSession
+        self.w, sp = w, w.spec
+        self.nh = sp.num_kv_heads if kv_heads is None else kv_heads
+        self.nq = self.nh * (sp.num_q_heads // sp.num_kv_heads)
+        self.sess = []
         for s, si in enumerate(w.sessions):
-            sess[s].append(si.k[0], si.v[0])
-            attend(sess[s], si.q[0], sp.scale, 1, rows=rows)
-            flops += 4.0 * sp.head_dim * sp.num_q_heads * len(rows) * sess[s].length
-            # roll back so that every repetition times the same work
-            sess[s].k_slices.pop(); sess[s].v_slices.pop(); sess[s].block_ends.pop()
-    return time.perf_counter() - t0, flops
+            o = OracleSession(self.nh, sp.head_dim)
+            for ids, rng in preload_rounds(w):
+                for sidx, (lo, hi) in zip(ids, rng):
+                    if sidx == s:
+                        o.append(si.k_cache[lo:hi, :self.nh], si.v_cache[lo:hi, :self.nh])
+            self.sess.append(o)
+
+    def step(self, rows):
+        """Returns (seconds, flops of the sampled rows)."""
+        from oracle.block_causal import attend
+        sp = self.w.spec
+        t0 = time.perf_counter()
+        flops = 0.0
+        for s, si in enumerate(self.w.sessions):
+            self.sess[s].append(si.k[0][:, :self.nh], si.v[0][:, :self.nh])
+            attend(self.sess[s], si.q[0][:, :self.nq], sp.scale, 1, rows=rows)
+            flops += 4.0 * sp.head_dim * self.nq * len(rows) * self.sess[s].length
+            self.sess[s].k_slices.pop(); self.sess[s].v_slices.pop(); self.sess[s].block_ends.pop()
+        return time.perf_counter() - t0, flops
+
+
+def oracle_sample_seconds(w, rows, budget_steps=1):
+    """Time the oracle on `rows` query tokens x all heads of step 0. Returns (s, flops)."""
+    smp = OracleSampler(w)
+    t, fl = 0.0, 0.0
+    for _ in range(budget_steps):
+        dt, f = smp.step(rows)
+        t += dt; fl += f
+    return t, fl
 
 
 class ClockSampler(threading.Thread):
@@ -268,22 +288,38 @@ def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, r
 
 
 def run_reference(args, spec):
+    """Reference arm = the oracle on the host cores (tier rules): exactly --steps timed steps after --warmup
+    untimed ones; each step attends a bounded sample of the unit's query tokens (all heads, full history),
+    sized from a calibration step so that the whole run stays within ~2.5 minutes."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     w = generate(spec_for_config(spec.cfg, steps=1))
-    nrows = args.ref_rows
-    rows = np.linspace(0, spec.block_tokens - 1, nrows).astype(np.int64)
+    n, total = spec.block_tokens, args.steps + args.warmup
+    budget_s = 150.0
+    # calibration on one KV head: a step costs a fixed part per head (the oracle widens the whole history
+    # to float64 on every call) plus a part per sampled row
+    cal = OracleSampler(w, kv_heads=1)
+    cal.step(np.array([0], dtype=np.int64))
+    t1 = min(cal.step(np.array([n // 2], dtype=np.int64))[0] for _ in range(2))
+    t9 = cal.step(np.linspace(0, n - 1, 9).astype(np.int64))[0]
+    per_row = max((t9 - t1) / 8.0, 1e-7)
+    fixed = max(t1 - per_row, 1e-6)
+    nh = int(max(1, min(spec.num_kv_heads, budget_s / (total * (fixed + per_row)))))
+    nrows = int(max(1, min(args.ref_rows, n, (budget_s / (total * nh) - fixed) / per_row)))
+    smp = cal if nh == 1 else OracleSampler(w, kv_heads=nh)
+    rows = np.unique(np.linspace(0, n - 1, nrows).astype(np.int64))
     for _ in range(args.warmup):
-        oracle_sample_seconds(w, rows[:2])
+        smp.step(rows)
     t, fl = 0.0, 0.0
     for _ in range(args.steps):
-        dt, f = oracle_sample_seconds(w, rows)
+        dt, f = smp.step(rows)
         t += dt; fl += f
     tflops = fl / t / 1e12
     cores = oracle_threads()
-    sample = (f"{nrows} of {spec.block_tokens} query tokens x all {spec.num_q_heads} heads per session, "
-              f"full history, unit 1 of the loop; FLOPs counted for the sampled rows only")
+    sample = (f"{len(rows)} of {n} query tokens x {smp.nq} of {spec.num_q_heads} query heads ({smp.nh} of "
+              f"{spec.num_kv_heads} KV heads) per session per step, full history, unit 1 of the loop; "
+              f"FLOPs counted for the sampled rows and heads only")
     line = {"impl": "reference", "metric": "block_causal_attn_tflops", "value": tflops, "unit": "TFLOP/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -311,8 +347,6 @@ def main():
     args = ap.parse_args()
     spec = CONFIG_SPECS[args.config]
     if args.impl == "reference":
-        if args.steps == 1000:
-            args.steps, args.warmup = 3, 1
         return run_reference(args, spec)
 
     import torch
