@@ -11,6 +11,7 @@
 #include <cstring>
 #include <memory>
 #include <string>
+#include <mutex>
 #include <vector>
 
 #include "../../include/ws.h"
@@ -93,6 +94,33 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// Process-wide plan cache (see ws_block_causal_attn_fwd): a handful of entries, least recently used out.
+struct PlanCacheEntry {
+  std::vector<int32_t> key;
+  ws::Plan plan;
+  std::vector<int32_t> blob;
+  uint64_t stamp = 0;
+};
+std::mutex g_plan_mu;
+std::vector<PlanCacheEntry> g_plan_cache;
+uint64_t g_plan_clock = 0;
+constexpr size_t kPlanCacheEntries = 16;
+
+bool plan_cache_lookup(const std::vector<int32_t>& key, ws::Plan* plan, std::vector<int32_t>* blob) {
+  std::lock_guard<std::mutex> lk(g_plan_mu);
+  for (PlanCacheEntry& e : g_plan_cache)
+    if (e.key == key) { e.stamp = ++g_plan_clock; *plan = e.plan; *blob = e.blob; return true; }
+  return false;
+}
+
+void plan_cache_insert(const std::vector<int32_t>& key, const ws::Plan& plan, const std::vector<int32_t>& blob) {
+  std::lock_guard<std::mutex> lk(g_plan_mu);
+  PlanCacheEntry* slot = nullptr;
+  if (g_plan_cache.size() < kPlanCacheEntries) { g_plan_cache.emplace_back(); slot = &g_plan_cache.back(); }
+  else { slot = &g_plan_cache[0]; for (PlanCacheEntry& e : g_plan_cache) if (e.stamp < slot->stamp) slot = &e; }
+  slot->key = key; slot->plan = plan; slot->blob = blob; slot->stamp = ++g_plan_clock;
+}
 
 }  // namespace
 
@@ -583,15 +611,32 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
 
   ws::PlanConfig pc{c->cfg.num_kv_heads, G, c->num_sms, /*min_tiles=*/2, /*seg_overhead_tiles=*/3.3f,
                     c->min_splits, c->lay.max_part_slots, c->decode_plan_enabled};
-  ws::Plan plan = ws::build_plan(pc, ps, vis_end);
-  if (!plan.ok && plan.alt) {           // too many (session, head) groups for two partials each
-    pc.allow_alt = false;
-    plan = ws::build_plan(pc, ps, vis_end);
+  // The plan is a pure function of the head geometry and the sessions' (query range, cache length): the
+  // layers of one model step (one cache handle each, same sessions, same lengths) all need the same one,
+  // so single-block steps look it up in a small process-wide cache before planning (~6-15 us of host work).
+  ws::Plan plan;
+  std::vector<int32_t> blob;
+  std::vector<int32_t> key;
+  bool cached = false;
+  if (!any_multi) {
+    key.reserve(8 + 5 * (size_t)S);
+    key.insert(key.end(), {pc.Hkv, pc.G, pc.num_sms, pc.min_splits, pc.max_part_slots, (int32_t)pc.allow_alt, S});
+    for (int32_t s = 0; s < S; ++s)
+      key.insert(key.end(), {ps[s].slot, ps[s].q_begin, ps[s].q_end, vis_end[ps[s].q_begin], ps[s].stable_tokens});
+    cached = plan_cache_lookup(key, &plan, &blob);
   }
-  if (!plan.ok)
-    return fail(WS_ERR_WORKSPACE_TOO_SMALL, "plan needs %d partial slots, workspace holds %d",
-                plan.num_part_slots, c->lay.max_part_slots);
-  std::vector<int32_t> blob = ws::serialise_plan(plan, vis_end, any_multi);
+  if (!cached) {
+    plan = ws::build_plan(pc, ps, vis_end);
+    if (!plan.ok && plan.alt) {           // too many (session, head) groups for two partials each
+      pc.allow_alt = false;
+      plan = ws::build_plan(pc, ps, vis_end);
+    }
+    if (!plan.ok)
+      return fail(WS_ERR_WORKSPACE_TOO_SMALL, "plan needs %d partial slots, workspace holds %d",
+                  plan.num_part_slots, c->lay.max_part_slots);
+    blob = ws::serialise_plan(plan, vis_end, any_multi);
+    if (!any_multi) plan_cache_insert(key, plan, blob);
+  }
   const bool inline_meta = blob.size() <= (size_t)ws::kInlineAttnWordsLarge;
   ws_status_t st = WS_OK;
   if (!inline_meta && !c->dry) {
