@@ -235,3 +235,20 @@ def test_planner_multi_block_queries(pkg):
     info, segs = _plan(pkg, [300], 200, Hq=4, Hkv=4, blocks=3)   # 600 query tokens, G=1 -> 3 pairs
     assert info["team_size"] == 3
     _check_cover(info, segs, 4 * ((300 + 600 + 127) // 128))
+
+
+def test_plan_cache_is_transparent(pkg):
+    """Single-block steps look their plan up in a process-wide cache keyed by geometry + per-session (slot,
+    query range, cache length): two handles ('layers') with the same sessions get the same plan, a changed
+    length or split setting gets its own, and a repeated call returns exactly what planning returned."""
+    lens, n = [5000, 777], 64
+    a_info, a_segs = _plan(pkg, lens, n)
+    b_info, b_segs = _plan(pkg, lens, n)              # second handle, same shape: served from the cache
+    assert a_info == b_info and a_segs == b_segs
+    _check_cover(b_info, b_segs, sum((L + n + 127) // 128 for L in lens) * 8)
+    c_info, c_segs = _plan(pkg, [5000 + 128, 777], n)
+    assert c_info["total_kv_tiles"] == a_info["total_kv_tiles"] + 8 and c_segs != a_segs
+    d_info, d_segs = _plan(pkg, lens, n, min_splits=3)
+    assert d_info["num_segments"] >= 3 * d_info["num_groups"] > a_info["num_groups"]
+    e_info, e_segs = _plan(pkg, lens, n)              # the unforced plan is still what the cache returns
+    assert e_info == a_info and e_segs == a_segs
