@@ -249,8 +249,24 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   if (threadIdx.x < 16) prof_stamps[threadIdx.x] = 0;
 #endif
 
+  // The TMA producer resolves its first segment (and, when that segment starts in tokens no in-flight
+  // append can still be writing, the page ids of its first tile) while the other warps allocate TMEM and
+  // initialise the barriers: takes the metadata and page-table latencies off the path to the first MMA.
+  SegView sv_first;
+  int32_t si_first = seg_hi, pre_pg0 = 0, pre_pg1 = 0;
+  bool pre_pages = false;
   if (warp == 8 && lane == 0) {
     prefetch_tmap(&tmap_q); prefetch_tmap(&tmap_k); prefetch_tmap(&tmap_v);
+    for (si_first = seg_lo; si_first < seg_hi; ++si_first)
+      if (load_segment<kCG - 1>(meta, hdr, si_first, clip_pair, tok_per_pair, sv_first) &&
+          sv_first.tile_end > sv_first.tile_begin) break;
+    if (!kAlt && si_first < seg_hi && sv_first.tile_begin + 1 < sv_first.g.dep_tile) {
+      const int32_t* page_row = p.page_table + (int64_t)sv_first.g.slot * p.max_pages_per_session;
+      const int32_t last_page = (sv_first.g.kv_len - 1) / p.P;
+      pre_pg0 = page_row[min(2 * sv_first.tile_begin, last_page)];
+      pre_pg1 = page_row[min(2 * sv_first.tile_begin + 1, last_page)];
+      pre_pages = true;
+    }
   }
   if (warp == 9 && lane == 0) {
     mbar_init(bq_full, 1); mbar_init(bq_empty, 1); mbar_init(smem_u32(&bars->merge_full), 1);
@@ -279,10 +295,14 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       // ===================================================== TMA producer
       uint32_t ring_it = 0, q_it = 0;
       bool dep_waited = false;
-      for (int32_t si = seg_lo; si < seg_hi; ++si) {
+      for (int32_t si = si_first; si < seg_hi; ++si) {
         SegView sv;
-        if (!load_segment<kCG - 1>(meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
-        if (sv.tile_end <= sv.tile_begin) continue;          // clipped away for this pair
+        if (si == si_first) {
+          sv = sv_first;
+        } else {
+          if (!load_segment<kCG - 1>(meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
+          if (sv.tile_end <= sv.tile_begin) continue;        // clipped away for this pair
+        }
         const int32_t* page_row = p.page_table + (int64_t)sv.g.slot * p.max_pages_per_session;
         const int32_t last_page = (sv.g.kv_len - 1) / p.P;
         // tiles >= dep_tile may still be being written by the preceding append kernel (PDL)
@@ -331,8 +351,13 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                           sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
           }
         ++q_it;
-        int32_t pg0 = page_row[min(2 * sv.tile_begin, last_page)];
-        int32_t pg1 = page_row[min(2 * sv.tile_begin + 1, last_page)];
+        int32_t pg0, pg1;
+        if (si == si_first && pre_pages) {
+          pg0 = pre_pg0; pg1 = pre_pg1;
+        } else {
+          pg0 = page_row[min(2 * sv.tile_begin, last_page)];
+          pg1 = page_row[min(2 * sv.tile_begin + 1, last_page)];
+        }
         PROF_STAMP(1)
         for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
           const int32_t c0 = pg0, c1 = pg1;
