@@ -124,7 +124,7 @@ __device__ __forceinline__ bool load_segment(const MetaView<W>& meta, const Attn
 // 2^x for a PAIR of values on the FMA/ALU pipes (no MUFU): round-to-nearest split x = r + f with
 // f in [-0.5, 0.5], a degree-3 minimax polynomial for 2^f (max relative error 7.5e-5, well inside
 // one bf16 ulp of P) in packed f32x2 arithmetic, and an exponent-field add per element.  Used for
-// kPolyPairs of every 4 pairs to take load off the 16/clk/SM MUFU.
+// WS_POLY_PER8 of every 8 exponentials (default 2 = 25 %) to take load off the 16/clk/SM MUFU.
 __device__ __forceinline__ void ex2_poly2(uint64_t x2, float& p0, float& p1) {
   float x0, x1;
   unpack_f32x2(x2, x0, x1);
@@ -143,7 +143,6 @@ __device__ __forceinline__ void ex2_poly2(uint64_t x2, float& p0, float& p1) {
   p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
 }
 
-constexpr int kPolyPairs = WS_POLY_PER8 / 2;   // pairs out of every 4 that use the polynomial
 
 // One 32-column chunk of a softmax row: p = 2^(s*c - m), running sums, running max of s, bf16 pack.
 __device__ __forceinline__ void softmax_chunk(const uint32_t* sr, float c, float neg_mc,
@@ -157,7 +156,11 @@ __device__ __forceinline__ void softmax_chunk(const uint32_t* sr, float c, float
       const float s0 = __uint_as_float(sr[i + e]), s1 = __uint_as_float(sr[i + e + 1]);
       const uint64_t x2 = fma_f32x2(pack_f32x2(s0, s1), c2, nm2);
       const int pr = e / 2;
-      const bool poly = kPolyPairs > 0 && (pr * kPolyPairs) / 4 != ((pr + 1) * kPolyPairs) / 4;
+      // WS_POLY_PER8 polynomial exponentials per 8 elements, i.e. PER8 / 2 pairs per group of 4 pairs; an
+      // odd PER8 alternates between rounding down and up from one group to the next
+      constexpr int kPolyEven = WS_POLY_PER8 / 2, kPolyOdd = (WS_POLY_PER8 + 1) / 2;
+      const int kp = ((i / 8) & 1) ? kPolyOdd : kPolyEven;
+      const bool poly = kp > 0 && (pr * kp) / 4 != ((pr + 1) * kp) / 4;
       if (poly) {
         ex2_poly2(x2, pv[e], pv[e + 1]);
       } else {
