@@ -481,16 +481,19 @@ def test_next2_solver_steps_stage_attend_rollback():
         assert np.abs(got - want).max() <= tol * np.maximum(1.0, np.abs(want)).max()
 
 
-def test_next2_solver_step_is_cuda_graph_capturable():
+@pytest.mark.parametrize("fused", [False, True], ids=["combine_kernel", "fused_combine"])
+def test_next2_solver_step_is_cuda_graph_capturable(fused):
     """One solver step (append + attention + combine) captured once in a CUDA graph and replayed with
     new buffer contents (PAPER.md:33, :85 name CUDA-graph capture): single-session metadata travels in
-    kernel parameters, so the captured sequence contains kernels only."""
+    kernel parameters, so the captured sequence contains kernels only.  With WS_FLAG_FUSED_COMBINE the
+    attention node is a cooperative launch whose arrival counters re-arm themselves between replays."""
     import torch
     from oracle.block_causal import OracleSession, attend
+    from paper_2606_25041_b200 import WS_FLAG_FUSED_COMBINE
     w = _small(3, cache_lens=(2500,), block_tokens=128, modality_split=(96, 24, 8), steps=1)
     si = w.sessions[0]
     dev = torch.device("cuda", 0)
-    cache = make_cache(w)
+    cache = make_cache(w, flags=WS_FLAG_FUSED_COMBINE if fused else 0)
     ids = preload_gpu(cache, w, [_torch_of(si.k_cache, dev)], [_torch_of(si.v_cache, dev)])
     base_blocks = cache.session_info(ids[0])[1]
     n, Hq, Hkv = 128, 32, 8
@@ -505,6 +508,7 @@ def test_next2_solver_step_is_cuda_graph_capturable():
     with torch.cuda.graph(g):
         cache.kv_append(ids, [0, n], kb, vb)
         cache.block_causal_attn_fwd(ids, [0, n], qb, out, w.spec.scale)
+    assert cache.last_plan_info()["num_combine_items"] > 0      # the step does split its KV ranges
     hist = OracleSession(8, 128)
     from tests.gpu_harness import preload_rounds
     for _, rng_ in preload_rounds(w):
