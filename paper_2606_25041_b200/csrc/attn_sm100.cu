@@ -59,12 +59,16 @@ constexpr uint32_t kQTileBytes = kTileRows * 128 * 2;
 constexpr int kThreads = 384;
 constexpr uint32_t kTmemCols = 512;
 constexpr float kRescaleThreshold = 8.0f;                  // log2 units
+constexpr int kFirstPieceSteps = 6;                         // P is handed to the MMA warp as keys 0-95, then 96-127
 constexpr float kFastSumLimit = 1024.0f;                   // fast path accepted while tile row sum < 2^10
 #ifndef WS_FAST_PATH
 #define WS_FAST_PATH 1
 #endif
 #ifndef WS_POLY_PER8
 #define WS_POLY_PER8 2
+#endif
+#ifndef WS_DUAL_ISSUER
+#define WS_DUAL_ISSUER 0
 #endif
 
 #ifdef WS_PROFILE
@@ -239,6 +243,13 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
   const int lane = threadIdx.x & 31;
+  // Compile-time experiment (-DWS_DUAL_ISSUER=1, general plan on single CTAs): one tcgen05.mma issuer warp
+  // PER Q tile (warps 9 and 11) instead of one warp walking q = 0, 1 in turn, so that a wait for one
+  // set's P never delays the other set's MMAs.  The two chains only share read-only K/V tiles; each ring
+  // slot / the Q pair is then released by two commits.  Correct, and no faster (235 vs 233 us per config-4
+  // unit): the tensor pipe's idle ~20 % is the time in which BOTH sets are in their softmax, not issuer
+  // head-of-line blocking.  Off by default.
+  constexpr bool kDual = kCG == 1 && !kAlt && WS_DUAL_ISSUER;
   const AttnMeta hdr = meta.template load<AttnMeta>(0);
   const int32_t team = blockIdx.x / hdr.team_size;
   const int32_t pair = blockIdx.x - team * hdr.team_size;
@@ -272,9 +283,9 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     }
   }
   if (warp == 9 && lane == 0) {
-    mbar_init(bq_full, 1); mbar_init(bq_empty, 1); mbar_init(smem_u32(&bars->merge_full), 1);
+    mbar_init(bq_full, 1); mbar_init(bq_empty, kDual ? 2 : 1); mbar_init(smem_u32(&bars->merge_full), 1);
     bars->njobs = 0;
-    for (int s = 0; s < kStages; ++s) { mbar_init(bkv_full(s), 1); mbar_init(bkv_empty(s), 1); }
+    for (int s = 0; s < kStages; ++s) { mbar_init(bkv_full(s), 1); mbar_init(bkv_empty(s), kDual ? 2 : 1); }
     for (int q = 0; q < 2; ++q) {
       mbar_init(bs_full(q), 1); mbar_init(bp_full(q, 0), 128 * kCG); mbar_init(bp_full(q, 1), 128 * kCG);
       mbar_init(bpv_h0(q), 1);
@@ -398,7 +409,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           }
         }
       }
-    } else if (warp == 9 && is_leader) {
+    } else if ((warp == 9 || (kDual && warp == 11)) && is_leader) {
       // ===================================================== MMA issuer (kCG = 2: the even CTA only)
       // The whole warp runs the control flow convergently (all values stay warp-uniform, so the
       // descriptors are built on the uniform datapath); one elected lane issues tcgen05.mma/commit.
@@ -410,6 +421,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const uint64_t desc_v = make_smem_desc_sw128(0, kHalfBytes, 1024);  // MN-major operand (V)
       uint32_t ring_it = 0, q_it = 0, tile_it = 0, seg_it = 0;
       uint32_t alt_tiles0 = 0, alt_tiles1 = 0, alt_segs0 = 0, alt_segs1 = 0;   // kAlt: per accumulator set
+      const int q_lo = kDual ? (warp == 9 ? 0 : 1) : 0, q_hi = kDual ? q_lo : 1;   // Q tiles this warp issues for
       PROF_DECL(8)
       auto issue_S = [&](int q, uint32_t slot) {
         const uint64_t da = desc_k + ((sQ + (kAlt ? 0 : q) * kQTileBytes) >> 4);
@@ -422,12 +434,12 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           else mma_ss(tmem_base + q * 128, da + offa, db + offb, idesc_qk, ks > 0);
         }
       };
-      // PV for one half of the tile's keys (k-steps 4*half .. 4*half+3)
+      // PV for one of the two pieces in which the softmax hands P over (k-steps of 16 keys)
       auto issue_PV = [&](int q, uint32_t slot, int half, bool accumulate) {
         const uint64_t db = desc_v + ((sRing + slot * kSlotBytes) >> 4);
 #pragma unroll
-        for (int k4 = 0; k4 < 4; ++k4) {
-          const int ks = half * 4 + k4;
+        for (int ks = 0; ks < 8; ++ks) {
+          if ((ks < kFirstPieceSteps) != (half == 0)) continue;   // piece 0: keys 0-95, piece 1: keys 96-127
           if constexpr (kCG == 2)
             mma_ts_2cta(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8, db + ks * (2048 >> 4),
                         idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
@@ -500,8 +512,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           tc_fence_after();
           if (leader) PROF_STAMP(3)
           if (leader) {
-            issue_S(0, slot); commit(bs_full(0));
-            issue_S(1, slot); commit(bs_full(1));
+            for (int q = q_lo; q <= q_hi; ++q) { issue_S(q, slot); commit(bs_full(q)); }
             commit(bkv_empty(slot));
             if (nt == 1) commit(bq_empty);
           }
@@ -517,10 +528,9 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           PROF_MARK(0)
           mbar_wait(bkv_full(slot_v), par_v);
           PROF_MARK(1)
-#pragma unroll
-          for (int q = 0; q < 2; ++q) {
+          for (int q = q_lo; q <= q_hi; ++q) {
             mbar_wait(bp_full(q, 0), tile_it & 1);
-            PROF_MARK(2 + q)
+            PROF_MARK(2 + (q & 1))
             if (j == 0) mbar_wait(bo_empty(q), (seg_it & 1) ^ 1);
             tc_fence_after();
             if (leader) {
@@ -537,7 +547,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             __syncwarp();
             PROF_MARK(5)
             if (have_next) {
-              if (q == 0) { mbar_wait(bkv_full(slot_k), par_k); tc_fence_after(); }
+              if (q == q_lo) { mbar_wait(bkv_full(slot_k), par_k); tc_fence_after(); }
               PROF_MARK(4)
               if (leader) {
                 issue_S(q, slot_k);
@@ -656,10 +666,13 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         // (rows whose reference is still -inf, i.e. nothing visible so far, also take the exact path)
         if (WS_FAST_PATH && j > 0 && !need_mask && !__any_sync(0xffffffffu, m_used == -INFINITY)) {
           // ---- fast path (optimistic): exponentiate against the running reference m_used while
-          // the tile streams out of TMEM in 32-column chunks.  Each half (64 keys) is checked for
-          // scores that outgrew the reference - every p is <= the half's row sum, so a sum below
-          // kFastSumLimit proves none did (a NaN/inf sum fails the test) - and handed to the MMA
-          // warp as soon as it is written, so PV of the first half overlaps the second half.
+          // the tile streams out of TMEM in 32-column chunks.  Each piece (keys 0-95, keys 96-127) is
+          // checked for scores that outgrew the reference - every p is <= the piece's row sum, so a sum
+          // below kFastSumLimit proves none did (a NaN/inf sum fails the test) - and handed to the MMA
+          // warp as soon as it is written: PV of the first piece (384 tensor cycles) overlaps the softmax
+          // of the last 32 keys, and only 128 cycles of PV remain on the S -> softmax -> PV -> S chain.
+          // (Measured the same as a 64/64 split, 233 us per config-4 unit: the softmax time of the two
+          // sets, which share each sub-partition's MUFU / issue slots, stretches by what the chain saves.)
           const float neg_mc = -m_used;
           uint64_t l01 = 0, l23 = 0;                        // packed fp32x2 partial row sums
           uint32_t sa[32], sb[32];
@@ -670,19 +683,20 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           tmem_wait_ld();
           tmem_ld32(t_s + 64, sa);
           softmax_chunk(sb, c, neg_mc, l01, l23, pk + 16);
+          tmem_wait_ld();
+          tmem_ld32(t_s + 96, sb);
+          softmax_chunk(sa, c, neg_mc, l01, l23, pk + 32);
           float la, lb;
           unpack_f32x2(add_f32x2(l01, l23), la, lb);
           const float sum_a = la + lb;
           if (!__any_sync(0xffffffffu, !(sum_a < kFastSumLimit))) {
             tmem_st32(t_s + 0, pk);
+            tmem_st16(t_s + 32, pk + 32);
             tmem_wait_st();
             tc_fence_before();
-            arrive_leader(bp_full(q, 0));                     // first 64 keys of P handed off
+            arrive_leader(bp_full(q, 0));                     // first 96 keys of P handed off
             tmem_wait_ld();
-            tmem_ld32(t_s + 96, sb);
             l01 = 0; l23 = 0;
-            softmax_chunk(sa, c, neg_mc, l01, l23, pk + 32);
-            tmem_wait_ld();
             softmax_chunk(sb, c, neg_mc, l01, l23, pk + 48);
             unpack_f32x2(add_f32x2(l01, l23), la, lb);
             const float sum_b = la + lb;
@@ -690,19 +704,18 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             if (!__any_sync(0xffffffffu, !(sum_b < kFastSumLimit))) {
               l += sum_b;
             } else {
-              // Rare: a score in the second half outgrew the reference after the first half was
-              // handed off.  Wait until PV of the first half has completed (O is then quiescent:
-              // the second-half PV needs our arrival), rescale O and l to the new reference and
-              // redo the second half exactly.
+              // Rare: a score among the last 32 keys outgrew the reference after the first piece was
+              // handed off.  Wait until PV of the first piece has completed (O is then quiescent:
+              // the PV of the last piece needs our arrival), rescale O and l to the new reference and
+              // redo the last 32 keys exactly.
               mbar_wait(bpv_h0(q), tile_it & 1);
               tc_fence_after();
-              uint32_t sr[64];
-              tmem_ld32(t_s + 64, sr);
-              tmem_ld32(t_s + 96, sr + 32);
+              uint32_t sr[32];
+              tmem_ld32(t_s + 96, sr);
               tmem_wait_ld();
               float mx = __uint_as_float(sr[0]);
 #pragma unroll
-              for (int i = 1; i < 64; ++i) mx = fmaxf(mx, __uint_as_float(sr[i]));
+              for (int i = 1; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sr[i]));
               const float tm = mx * c;
               float alpha = 1.f;
               if (tm > m_used + kRescaleThreshold) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
@@ -717,15 +730,15 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
               }
               float ls = 0.f;
 #pragma unroll
-              for (int i = 0; i < 64; i += 2) {
+              for (int i = 0; i < 32; i += 2) {
                 const float p0 = ex2_approx(fmaf(__uint_as_float(sr[i]), c, -m_used));
                 const float p1 = ex2_approx(fmaf(__uint_as_float(sr[i + 1]), c, -m_used));
                 ls += p0 + p1;
-                pk[32 + i / 2] = pack_bf16x2(p0, p1);
+                pk[48 + i / 2] = pack_bf16x2(p0, p1);
               }
               l += ls;
             }
-            tmem_st32(t_s + 32, pk + 32);
+            tmem_st16(t_s + 48, pk + 48);
             tmem_wait_st();
             tc_fence_before();
             arrive_leader(bp_full(q, 1));
@@ -891,6 +904,13 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         // contiguous in the partial buffer.  Otherwise: direct 16-byte stores (same chunk positions).
         const bool staged = kCG == 1 && si + 1 == seg_hi && __all_sync(0xffffffffu, row_valid);   // (few valid rows, e.g. decode steps: store just those)
         const uint32_t stage = ((kAlt || q == 1) ? sRing : sQ) + (uint32_t)(warp & 3) * 16384u + (uint32_t)lane * 512u;
+        if (kDual && si + 1 == seg_hi) {
+          // Two issuer warps: o_full(q) only covers the MMAs of this set's issuer, but set 0 stages over BOTH
+          // Q tiles (set 1's last S MMA may still be reading the second) and set 1 over ring slots (set 0's
+          // last PV may still be reading V).  Both warpgroups meet here, each after its own o_full: every
+          // MMA of the CTA has then completed.  (Last segment only; the sets run within a tile of each other.)
+          asm volatile("bar.sync 4, 256;" ::: "memory");
+        }
 #pragma unroll
         for (int ch = 0; ch < 4; ++ch) {
           uint32_t o[32];
