@@ -355,6 +355,8 @@ def _prefill_case(block_sizes, Hq, Hkv, seed, L0=0, expect_kernel=1, min_splits=
     ([256] * 8, 8, 2, 0),                 # system prefill: 2048-token prompt in 8 units, empty cache
     ([100, 37, 256, 1, 300], 4, 4, 500),  # ragged blocks (MHA), behind a committed cache
     ([64] * 24, 16, 2, 0),                # G = 8, many short blocks: several blocks per Q-tile pair
+    ([256] * 29 + [200], 4, 2, 0),        # 7624-token prompt: the metadata blob (one visible end per token)
+                                          # exceeds both kernel-parameter tiers -> pinned ring + device blob
 ])
 def test_next1_multi_block_prefill(blocks, Hq, Hkv, L0):
     """NEXT-1 (PAPER.md:75 system prefill; :69 training-format equivalence): many committed blocks
