@@ -88,6 +88,33 @@ def test_append_bit_exact_random_bits_and_canary():
     assert (kp[free] == canary).all() and (vp[free] == canary).all()
 
 
+def test_append_large_block_metadata_through_device_blob():
+    """One 70,001-token block (1094 new pages): the append descriptor exceeds the kernel-parameter tier and
+    travels through the pinned ring into the workspace; the kernel reads it from the device blob.  Bit-exact
+    gather, ragged last page, then a second (inline) append behind it."""
+    import torch
+    from paper_2606_25041_b200 import WS_BF16, Cache
+    rng = np.random.default_rng(17)
+    Hkv, D, P, n1, n2 = 1, 128, 64, 70001, 77
+    c = Cache(WS_BF16, 2, Hkv, D, P, num_pages=(n1 + n2) // P + 3, max_sessions=1, max_q_tokens_per_call=n1)
+    sid = c.session_open()
+    dev = torch.device("cuda", 0)
+    ref_k, ref_v = [], []
+    for n in (n1, n2):
+        kb = rng.integers(0, 65536, size=(n, Hkv, D), dtype=np.uint16)
+        vb = rng.integers(0, 65536, size=(n, Hkv, D), dtype=np.uint16)
+        c.kv_append([sid], [0, n], torch.from_numpy(kb.view(np.int16)).to(dev).view(torch.bfloat16),
+                    torch.from_numpy(vb.view(np.int16)).to(dev).view(torch.bfloat16))
+        ref_k.append(kb); ref_v.append(vb)
+    tokens, blocks, ends = c.session_info(sid)
+    assert tokens == n1 + n2 and blocks == 2 and list(ends) == [n1, n1 + n2]
+    kg = torch.empty((tokens, Hkv, D), dtype=torch.bfloat16, device=dev); vg = torch.empty_like(kg)
+    c.kv_gather(sid, 0, tokens, kg, vg)
+    torch.cuda.synchronize()
+    assert kg.view(torch.int16).cpu().numpy().view(np.uint16).tobytes() == np.concatenate(ref_k).tobytes()
+    assert vg.view(torch.int16).cpu().numpy().view(np.uint16).tobytes() == np.concatenate(ref_v).tobytes()
+
+
 # ------------------------------------------------------------------ config 1 (fp32, CUDA cores)
 def test_config1_tiny_fp32_incremental():
     w = generate(spec_for_config(1))
