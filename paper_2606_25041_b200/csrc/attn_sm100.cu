@@ -1020,13 +1020,15 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     int tiles = 0; for (int si = seg_lo; si < seg_hi; ++si) { const Segment sg = meta.template load<Segment>(hdr.off_segments + si * 4); tiles += sg.tile_end - sg.tile_begin; }
     unsigned smid; asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
     // one line per CTA: ns since the CTA started (globaltimer) at which thread 0 / the producer / the MMA warp
-    // passed each point (first segment / first merge job only)
-    static const char* names[16] = {"setup", "qissued", "qfull", "k0full", "s0full", "lasttile", "pdlwait", "ofull",
-                                    "stored", "segsdone", "merged", "mwaited", "mitem", "staged", "missued", "mloaded"};
-    printf("CTA %d sm %u segs %d tiles %d cycles %lld t0 %llu dur %llu |", blockIdx.x, smid, seg_hi - seg_lo, tiles,
-           clock64() - prof_cta_t0, prof_g0, g1 - prof_g0);
-    for (int i = 0; i < 16; ++i) printf(" %s %lld", names[i], prof_stamps[i] ? (long long)(prof_stamps[i] - prof_g0) : -1ll);
-    printf("\n");
+    // passed each point (first segment / first merge job only; -1 = never).  A single printf: lines of
+    // different CTAs must not interleave.
+#define PS_(i) (prof_stamps[i] ? (long long)(prof_stamps[i] - prof_g0) : -1ll)
+    printf("CTA %d sm %u segs %d tiles %d cycles %lld t0 %llu dur %llu | setup %lld qissued %lld qfull %lld k0full %lld "
+           "s0full %lld lasttile %lld pdlwait %lld ofull %lld stored %lld segsdone %lld merged %lld mwaited %lld mitem %lld "
+           "staged %lld missued %lld mloaded %lld\n", blockIdx.x, smid, seg_hi - seg_lo, tiles, clock64() - prof_cta_t0,
+           prof_g0, g1 - prof_g0, PS_(0), PS_(1), PS_(2), PS_(3), PS_(4), PS_(5), PS_(6), PS_(7), PS_(8), PS_(9), PS_(10),
+           PS_(11), PS_(12), PS_(13), PS_(14), PS_(15));
+#undef PS_
   }
 #endif
   if (warp == 10) {
