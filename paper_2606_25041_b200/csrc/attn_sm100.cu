@@ -274,7 +274,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     for (si_first = seg_lo; si_first < seg_hi; ++si_first)
       if (load_segment<kCG - 1>(meta, hdr, si_first, clip_pair, tok_per_pair, sv_first) &&
           sv_first.tile_end > sv_first.tile_begin) break;
-    if (!kAlt && si_first < seg_hi && sv_first.tile_begin + 1 < sv_first.g.dep_tile) {
+    if (si_first < seg_hi && sv_first.tile_begin + 1 < sv_first.g.dep_tile) {
       const int32_t* page_row = p.page_table + (int64_t)sv_first.g.slot * p.max_pages_per_session;
       const int32_t last_page = (sv_first.g.kv_len - 1) / p.P;
       pre_pg0 = page_row[min(2 * sv_first.tile_begin, last_page)];
@@ -330,7 +330,9 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           ++q_it;
           auto load_tile = [&](const CUtensorMap* tm, int32_t j) {
             if (!dep_waited && j >= sv.g.dep_tile) { pdl_wait(); dep_waited = true; }
-            const int32_t c0 = page_row[min(2 * j, last_page)], c1 = page_row[min(2 * j + 1, last_page)];
+            const bool pre = si == si_first && pre_pages && j == sv.tile_begin;   // ids fetched during set-up
+            const int32_t c0 = pre ? pre_pg0 : page_row[min(2 * j, last_page)];
+            const int32_t c1 = pre ? pre_pg1 : page_row[min(2 * j + 1, last_page)];
             const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
             mbar_wait(bkv_empty(slot), par ^ 1);
             mbar_arrive_expect_tx(bkv_full(slot), 32768);
