@@ -673,8 +673,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           // below kFastSumLimit proves none did (a NaN/inf sum fails the test) - and handed to the MMA
           // warp as soon as it is written: PV of the first piece (384 tensor cycles) overlaps the softmax
           // of the last 32 keys, and only 128 cycles of PV remain on the S -> softmax -> PV -> S chain.
-          // (Measured the same as a 64/64 split, 233 us per config-4 unit: the softmax time of the two
-          // sets, which share each sub-partition's MUFU / issue slots, stretches by what the chain saves.)
+          // (ncu: 2541 instead of 2611 cycles per tile pair with a 64/64 split; the power-capped live time
+          // per config-4 unit did not move.)
           const float neg_mc = -m_used;
           uint64_t l01 = 0, l23 = 0;                        // packed fp32x2 partial row sums
           uint32_t sa[32], sb[32];
