@@ -105,6 +105,10 @@ combine_rows_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl,
 
 
 // ---- staged variant ----
+#ifndef WS_STAGED_MAX_PARTS
+#define WS_STAGED_MAX_PARTS 8
+#endif
+constexpr int kStagedMaxParts = WS_STAGED_MAX_PARTS;   // more parts per row than this: row-per-warp variant
 constexpr int kCombineRowsMax = 32;                    // rows per block (fewer when a row has many parts)
 constexpr int kCombineRowsCap = 192;                   // staged rows x parts per chunk: 96 KB -> 2 blocks / SM
 constexpr uint32_t kCombineLseBytes = 8192;            // nparts x (rows + 8) fp32, nparts <= 148
@@ -159,7 +163,7 @@ cudaError_t launch_combine(const AttnParams& p, const InlineAttnMetaLarge& inl, 
   const bool small_tier = inl_words <= kInlineAttnWords;
   InlineAttnMeta small;
   if (small_tier) memcpy(small.w, inl.w, sizeof(small.w));
-  if (max_parts > 8) {
+  if (max_parts > kStagedMaxParts) {
     // many parts per row: a staged block would hold only a few rows - one warp per row instead
     const int32_t grid = num_combine * team_size * (kPairRows / kCombineRowsPerBlock);
     const dim3 g(grid), b(kCombineRowsPerBlock * 32);
