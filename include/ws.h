@@ -140,6 +140,15 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* cache, int32_t num_sessions,
                                      const int32_t* cu_q_tokens, const void* q, void* out,
                                      float* lse, float scale, void* cuda_stream);
 
+/* One streaming-unit step with DEVICE buffers in a single call: ws_kv_append(k_new, v_new) followed by
+ * ws_block_causal_attn_fwd of the block just committed (one block per session, n_q = n_new; PAPER.md:83
+ * "appends the received KV slice", then the unit attends).  Same kernels and results as the two calls;
+ * saves one trip through the caller's binding per step.  If the attention part fails (e.g.
+ * WS_ERR_WORKSPACE_TOO_SMALL) the append has already been committed: ws_session_truncate rolls it back. */
+ws_status_t ws_stream_step(ws_cache_t* cache, int32_t num_sessions, const int32_t* session_ids,
+                           const int32_t* cu_new_tokens, const void* q, const void* k_new,
+                           const void* v_new, void* out, float* lse, float scale, void* cuda_stream);
+
 /* One streaming-unit step with HOST buffers (the end-to-end path): copies q/k_new/v_new from host
  * (pinned for async copies) into `staging` (DEVICE, >= ws_step_staging_bytes(n_total); two slots used
  * alternately), runs ws_kv_append then ws_block_causal_attn_fwd (one block per session, n_q = n_new)

@@ -60,7 +60,7 @@ EXPORTS = ["ws_replica_link", "ws_replica_accept", "ws_replica_commit_message",
            "ws_ipc_export", "ws_ipc_open", "ws_ipc_close", "ws_pool_bytes", "ws_workspace_bytes", "ws_cache_create", "ws_cache_destroy",
            "ws_session_open", "ws_session_close", "ws_session_info", "ws_session_truncate",
            "ws_free_pages", "ws_kv_append", "ws_block_causal_attn_fwd", "ws_step_staging_bytes",
-           "ws_stream_step_host", "ws_stream_host_join", "ws_fm_euler_update", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
+           "ws_stream_step", "ws_stream_step_host", "ws_stream_host_join", "ws_fm_euler_update", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
            "ws_debug_set_min_splits", "ws_debug_set_decode_plan", "ws_last_plan_info", "ws_last_plan_segment",
            "ws_launch_count", "ws_debug_kernel_timing", "ws_debug_read_kernel_times",
            "ws_status_str", "ws_last_error", "ws_version"]
@@ -94,6 +94,7 @@ def load_library() -> C.CDLL:
                                              C.c_float, vp]
     lib.ws_step_staging_bytes.restype = C.c_size_t
     lib.ws_step_staging_bytes.argtypes = [cfgp, C.c_int32]
+    lib.ws_stream_step.argtypes = [vp, C.c_int32, i32p, i32p, vp, vp, vp, vp, vp, C.c_float, vp]
     lib.ws_stream_step_host.argtypes = [vp, C.c_int32, i32p, i32p, vp, vp, vp, vp, vp, C.c_size_t,
                                         C.c_float, vp]
     lib.ws_stream_host_join.argtypes = [vp, vp]
@@ -259,6 +260,12 @@ class Cache:
                                                  nqb, _i32(cu_q_tokens), _ptr(q), _ptr(out),
                                                  _ptr(lse), C.c_float(scale), _stream_ptr(stream)))
 
+    def stream_step(self, session_ids, cu_new_tokens, q, k_new, v_new, out, scale: float, lse=None, stream=None):
+        """ws_kv_append + ws_block_causal_attn_fwd of the block just committed, one call (device buffers)."""
+        _check(self.lib.ws_stream_step(self.handle, len(session_ids), _i32(session_ids), _i32(cu_new_tokens),
+                                       _ptr(q), _ptr(k_new), _ptr(v_new), _ptr(out), _ptr(lse),
+                                       C.c_float(scale), _stream_ptr(stream)))
+
     def step_staging_bytes(self, total_new_tokens: int) -> int:
         return self.lib.ws_step_staging_bytes(C.byref(self.cfg), total_new_tokens)
 
@@ -367,6 +374,10 @@ def ws_block_causal_attn_fwd(cache: Cache, session_ids, cu_q_tokens, q, out, sca
 
 def ws_kv_gather(cache: Cache, session, start, count, k_out, v_out, stream=None):
     cache.kv_gather(session, start, count, k_out, v_out, stream)
+
+
+def ws_stream_step(cache: Cache, session_ids, cu_new_tokens, q, k_new, v_new, out, scale, lse=None, stream=None):
+    cache.stream_step(session_ids, cu_new_tokens, q, k_new, v_new, out, scale, lse=lse, stream=stream)
 
 
 def ws_stream_step_host(cache: Cache, session_ids, cu_new_tokens, q_host, k_host, v_host, out_host,

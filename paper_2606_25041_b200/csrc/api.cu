@@ -706,6 +706,20 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
   return WS_OK;
 }
 
+ws_status_t ws_stream_step(ws_cache_t* c, int32_t S, const int32_t* session_ids, const int32_t* cu,
+                           const void* q, const void* k_new, const void* v_new, void* out, float* lse,
+                           float scale, void* cuda_stream) {
+  // validate what only the second half would reject BEFORE the append commits anything
+  if (!c || !session_ids || !cu) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  if (!c->dry && (!q || !out)) return fail(WS_ERR_INVALID_ARG, "q / out is NULL");
+  if (!(scale > 0.f) || !std::isfinite(scale)) return fail(WS_ERR_INVALID_ARG, "scale must be finite and > 0");
+  if (S >= 1 && S <= c->cfg.max_sessions_per_call && cu[S] > c->cfg.max_q_tokens_per_call)
+    return fail(WS_ERR_INVALID_ARG, "%d query tokens > max_q_tokens_per_call %d", cu[S], c->cfg.max_q_tokens_per_call);
+  ws_status_t st = ws_kv_append(c, S, session_ids, cu, k_new, v_new, nullptr, cuda_stream);
+  if (st != WS_OK) return st;
+  return ws_block_causal_attn_fwd(c, S, session_ids, nullptr, cu, q, out, lse, scale, cuda_stream);
+}
+
 size_t ws_step_staging_bytes(const ws_cache_config_t* cfg, int32_t n) {
   const char* why;
   if (!config_valid(cfg, &why) || n < 1) return 0;

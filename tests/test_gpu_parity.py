@@ -863,3 +863,37 @@ def test_stream_step_host_end_to_end():
     ref = run_workload_oracle(w)
     d = oh.float().numpy() - ref["out"][0][0]
     assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3
+
+
+def test_stream_step_single_call_equals_two_calls():
+    """ws_stream_step (append + attend in one call, device buffers): bit-identical to ws_kv_append followed by
+    ws_block_causal_attn_fwd on a twin cache, matches the oracle, and rejects what the attention half would
+    reject before anything is committed."""
+    import torch
+    from paper_2606_25041_b200 import WsError
+    w = _small(5, cache_len_range=(100, 1500), block_tokens=64, modality_split=(48, 12, 4), steps=2)
+    S, n, sp = w.spec.num_sessions, 64, w.spec
+    dev = torch.device("cuda", 0)
+    dk = [_torch_of(s.k_cache, dev) for s in w.sessions]; dv = [_torch_of(s.v_cache, dev) for s in w.sessions]
+    a, b = make_cache(w), make_cache(w)
+    ids_a, ids_b = preload_gpu(a, w, dk, dv), preload_gpu(b, w, dk, dv)
+    cu = [i * n for i in range(S + 1)]
+    ref = run_workload_oracle(w)
+    for t in range(2):
+        q = torch.cat([_torch_of(s.q[t], dev) for s in w.sessions])
+        k = torch.cat([_torch_of(s.k[t], dev) for s in w.sessions])
+        v = torch.cat([_torch_of(s.v[t], dev) for s in w.sessions])
+        oa = torch.full((S * n, sp.num_q_heads, 128), float("nan"), dtype=torch.bfloat16, device=dev); ob = oa.clone()
+        la = torch.full((S * n, sp.num_q_heads), float("nan"), dtype=torch.float32, device=dev); lb = la.clone()
+        a.stream_step(ids_a, cu, q, k, v, oa, sp.scale, lse=la)
+        b.kv_append(ids_b, cu, k, v); b.block_causal_attn_fwd(ids_b, cu, q, ob, sp.scale, lse=lb)
+        torch.cuda.synchronize()
+        assert torch.equal(oa.view(torch.int16), ob.view(torch.int16)) and torch.equal(la, lb)
+        o = oa.float().cpu().numpy().reshape(S, n, sp.num_q_heads, 128)
+        for s in range(S):
+            d = np.abs(o[s] - ref["out"][t][s])
+            assert (d - np.abs(ref["out"][t][s]) * 2.0 ** -8).max() <= 8e-3 and d.mean() <= 1e-3
+    tokens_before = a.session_info(ids_a[0])[0]
+    with pytest.raises(WsError):
+        a.stream_step(ids_a, cu, q, k, v, oa, -1.0)          # bad scale: nothing may be committed
+    assert a.session_info(ids_a[0])[0] == tokens_before
