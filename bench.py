@@ -4,7 +4,8 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
 
 A "step" is one streaming unit of the hot path: ws_kv_append (commit the unit's K/V block) followed by
-ws_block_causal_attn_fwd (the block attends to the full history; includes the split-KV combine).
+ws_block_causal_attn_fwd (the block attends to the full history; includes the split-KV combine), issued through
+ws_stream_step (the two in one C call: same kernels, one trip through the binding).
 Headline workload = BASELINE.json configs[3] ("bf16 long session": 32 q / 8 kv heads, D=128, block of
 256 tokens, cache 65536 growing over 20 consecutive units) - the configuration the north_star's 60 %
 target is quoted on.  After 20 units the session is rolled back (host metadata only) and replayed.
@@ -404,8 +405,8 @@ def main():
         r, t = i % R, (i // R) % steps_per_cycle
         if t == 0:
             reset(r)
-        caches[r].kv_append(ids_of[r], cu, k_d[t], v_d[t], stream=stream)
-        caches[r].block_causal_attn_fwd(ids_of[r], cu, q_d[t], out, sp.scale, stream=stream)
+        # ws_stream_step = ws_kv_append + ws_block_causal_attn_fwd of the block just committed, one C call
+        caches[r].stream_step(ids_of[r], cu, q_d[t], k_d[t], v_d[t], out, sp.scale, stream=stream)
 
     def barrier():
         if dist is not None:
