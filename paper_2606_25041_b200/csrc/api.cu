@@ -587,17 +587,26 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     if (c->dry && !c->tensor_path_ok) { c->last_plan = ws::Plan(); return WS_OK; }
     if (!c->dry) {
       size_t bytes = (size_t)NQ * 8;
-      ws_status_t st = refuse_if_capturing(stream, "generic-kernel metadata");
-      if (st != WS_OK) return st;
-      st = next_slot(c, bytes, &h, &d);
-      if (st != WS_OK) return st;
-      memcpy(h, tok_slot.data(), (size_t)NQ * 4);
-      memcpy(h + (size_t)NQ * 4, vis_end.data(), (size_t)NQ * 4);
-      st = upload_slot(c, h, d, bytes, stream);
-      if (st != WS_OK) return st;
+      ws::InlineAppendMeta inl;
+      ws_status_t st = WS_OK;
+      if (2 * (size_t)NQ <= (size_t)ws::kInlineAppendWords) {
+        // small call (the fp32 config: 16 tokens): the metadata rides in the kernel parameters
+        memcpy(inl.w, tok_slot.data(), (size_t)NQ * 4);
+        memcpy(inl.w + NQ, vis_end.data(), (size_t)NQ * 4);
+        d = nullptr;
+      } else {
+        st = refuse_if_capturing(stream, "generic-kernel metadata");
+        if (st != WS_OK) return st;
+        st = next_slot(c, bytes, &h, &d);
+        if (st != WS_OK) return st;
+        memcpy(h, tok_slot.data(), (size_t)NQ * 4);
+        memcpy(h + (size_t)NQ * 4, vis_end.data(), (size_t)NQ * 4);
+        st = upload_slot(c, h, d, bytes, stream);
+        if (st != WS_OK) return st;
+      }
       TimedLaunch tl(c, &c->t_attn, stream);
       WS_CUDA(ws::launch_attn_simt(c->cfg.dtype, q, out, lse, c->cfg.k_pool, c->cfg.v_pool,
-                                   c->d_page_table, (const int32_t*)d,
+                                   c->d_page_table, (const int32_t*)d, inl,
                                    c->default_map ? nullptr : c->d_q_to_kv, NQ,
                                    c->cfg.max_pages_per_session, c->cfg.num_q_heads,
                                    c->cfg.num_kv_heads, c->cfg.head_dim, c->cfg.page_tokens, scale,

@@ -51,16 +51,20 @@ __global__ void __launch_bounds__(kSimtWarps * 32)
 attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict__ lse,
                  const T* __restrict__ k_pool, const T* __restrict__ v_pool,
                  const int32_t* __restrict__ page_table, const int32_t* __restrict__ tok_meta,
+                 const __grid_constant__ InlineAppendMeta inl,
                  const int32_t* __restrict__ q_to_kv, int32_t total_q_tokens, int32_t max_pages,
                  int32_t Hq, int32_t Hkv, int32_t D, int32_t P, float scale) {
+  // per-token (session slot, visible end): device blob, or - small calls - the kernel parameter itself
+  // (constant-bank reads; no host->device copy in the chain, so the call is CUDA-graph capturable)
+  const MetaView<kInlineAppendWords> meta{tok_meta, inl};
   __shared__ float q_s[kSimtWarps][kMaxD];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const int64_t w = (int64_t)blockIdx.x * kSimtWarps + wib;
   if (w >= (int64_t)total_q_tokens * Hq) return;
   const int32_t tok = (int32_t)(w / Hq), h = (int32_t)(w % Hq);
   const int32_t g = q_to_kv ? q_to_kv[h] : h / (Hq / Hkv);
-  const int32_t slot = tok_meta[tok];
-  const int32_t vis = tok_meta[total_q_tokens + tok];
+  const int32_t slot = meta[tok];
+  const int32_t vis = meta[total_q_tokens + tok];
   const int32_t* page_row = page_table + (int64_t)slot * max_pages;
 
   const T* qrow = q + ((int64_t)tok * Hq + h) * D;
@@ -127,20 +131,20 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
 
 cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse,
                              const void* k_pool, const void* v_pool, const int32_t* page_table,
-                             const int32_t* tok_meta, const int32_t* q_to_kv, int32_t total_q_tokens,
-                             int32_t max_pages, int32_t Hq, int32_t Hkv, int32_t D, int32_t P,
-                             float scale, cudaStream_t stream) {
+                             const int32_t* tok_meta, const InlineAppendMeta& inl, const int32_t* q_to_kv,
+                             int32_t total_q_tokens, int32_t max_pages, int32_t Hq, int32_t Hkv, int32_t D,
+                             int32_t P, float scale, cudaStream_t stream) {
   int64_t warps = (int64_t)total_q_tokens * Hq;
   int32_t grid = (int32_t)((warps + kSimtWarps - 1) / kSimtWarps);
   if (grid == 0) return cudaSuccess;
   if (dtype == 1) {
     attn_simt_kernel<float><<<grid, kSimtWarps * 32, 0, stream>>>(
         (const float*)q, (float*)out, lse, (const float*)k_pool, (const float*)v_pool, page_table,
-        tok_meta, q_to_kv, total_q_tokens, max_pages, Hq, Hkv, D, P, scale);
+        tok_meta, inl, q_to_kv, total_q_tokens, max_pages, Hq, Hkv, D, P, scale);
   } else {
     attn_simt_kernel<__nv_bfloat16><<<grid, kSimtWarps * 32, 0, stream>>>(
         (const __nv_bfloat16*)q, (__nv_bfloat16*)out, lse, (const __nv_bfloat16*)k_pool,
-        (const __nv_bfloat16*)v_pool, page_table, tok_meta, q_to_kv, total_q_tokens, max_pages, Hq,
+        (const __nv_bfloat16*)v_pool, page_table, tok_meta, inl, q_to_kv, total_q_tokens, max_pages, Hq,
         Hkv, D, P, scale);
   }
   return cudaGetLastError();

@@ -897,3 +897,35 @@ def test_stream_step_single_call_equals_two_calls():
     with pytest.raises(WsError):
         a.stream_step(ids_a, cu, q, k, v, oa, -1.0)          # bad scale: nothing may be committed
     assert a.session_info(ids_a[0])[0] == tokens_before
+
+
+def test_fp32_generic_kernel_step_is_cuda_graph_capturable():
+    """Small calls of the generic (fp32 / CUDA-core) kernel carry their per-token metadata in the kernel
+    parameters: the tiny fp32 config's unit (append + attend) can be captured and replayed."""
+    import torch
+    from oracle.block_causal import OracleSession, attend
+    w = generate(spec_for_config(1))
+    si = w.sessions[0]
+    dev = torch.device("cuda", 0)
+    cache = make_cache(w)
+    sid = cache.session_open()
+    n = 16
+    kb = torch.zeros((n, 2, 64), dtype=torch.float32, device=dev); vb = torch.zeros_like(kb)
+    qb = torch.zeros((n, 2, 64), dtype=torch.float32, device=dev); out = torch.zeros_like(qb)
+    cache.kv_append([sid], [0, n], _torch_of(si.k[0], dev), _torch_of(si.v[0], dev))      # unit 1 committed
+    base = cache.session_info(sid)[1]
+    cache.stream_step([sid], [0, n], qb, kb, vb, out, w.spec.scale)                       # warm-up, rolled back
+    cache.session_truncate(sid, base)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        cache.stream_step([sid], [0, n], qb, kb, vb, out, w.spec.scale)
+    assert cache.last_plan_info()["used_tensor_core_kernel"] == 0
+    for t in (1, 2):                                   # the same captured step serves as unit 2, then (new data) again
+        qb.copy_(_torch_of(si.q[t], dev)); kb.copy_(_torch_of(si.k[t], dev)); vb.copy_(_torch_of(si.v[t], dev))
+        g.replay()
+        torch.cuda.synchronize()
+        sess = OracleSession(2, 64)
+        sess.append(si.k[0], si.v[0]); sess.append(si.k[t], si.v[t])
+        o_ref, _ = attend(sess, si.q[t], w.spec.scale)
+        assert np.abs(out.cpu().numpy() - o_ref).max() <= 1e-5
