@@ -77,13 +77,16 @@ def default_q_to_kv(num_q_heads: int, num_kv_heads: int) -> np.ndarray:
 def attend(sess: OracleSession, q: np.ndarray, scale: float, num_q_blocks: int = 1,
            q_to_kv: Optional[Sequence[int]] = None,
            rows: Optional[Sequence[int]] = None,
-           heads: Optional[Sequence[int]] = None) -> Tuple[np.ndarray, np.ndarray]:
+           heads: Optional[Sequence[int]] = None, want_abs: bool = False):
     """Block-causal attention of the LAST `num_q_blocks` committed blocks against the history.
 
     q: [n_q, Hq, D] (n_q = total tokens of those blocks, storage dtype, widened to float64 here).
     rows / heads: optional subsets (indices into n_q / Hq) so that full-size configs can be
     checked on sampled outputs; the arithmetic per output element is identical.
     Returns O float64 [len(rows), len(heads), D] and LSE float64 [len(rows), len(heads)].
+    want_abs: additionally return A[r,h,:] = sum_j (p_j / Z) * |Vc[j,g,:]| (same weights, |V| instead
+    of V): the condition number of the output w.r.t. relative perturbations of the weights, used by the
+    tests to state the bf16 error bound of DESIGN.md reading A10 (|O| <= A, with equality for V >= 0).
     """
     B = len(sess.block_ends) - 1
     assert 1 <= num_q_blocks <= B
@@ -98,6 +101,7 @@ def attend(sess: OracleSession, q: np.ndarray, scale: float, num_q_blocks: int =
     Kc, Vc = sess.gather()
     out = np.zeros((len(rows), len(heads), D), dtype=np.float64)
     lse = np.zeros((len(rows), len(heads)), dtype=np.float64)
+    absw = np.zeros_like(out) if want_abs else None
     # block index of every selected query row, and that block's visible end e_b
     abs_pos = q_start + rows
     ends = np.asarray(sess.block_ends)
@@ -118,6 +122,10 @@ def attend(sess: OracleSession, q: np.ndarray, scale: float, num_q_blocks: int =
                 Z = P.sum(axis=1, keepdims=True)
                 out[sel, hi, :] = (P / Z) @ Vg[:e]
                 lse[sel, hi] = (m + np.log(Z))[:, 0]
+                if want_abs:
+                    absw[sel, hi, :] = (P / Z) @ np.abs(Vg[:e])
+    if want_abs:
+        return out, lse, absw
     return out, lse
 
 

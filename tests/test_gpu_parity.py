@@ -1,9 +1,14 @@
 """GPU parity tests: the CUDA path (through the C ABI) vs the float64 oracle on the same seeded inputs.
 
-Tolerances (BASELINE.json north_star): bf16 I/O max-abs <= 1e-2 and mean-abs <= 1e-3;
-fp32 config max-abs <= 1e-5; KV append bit-exact.  Because N(0,1) inputs at long caches make the
-outputs themselves tiny, the tests additionally gate on relative RMS error <= 1e-2,
-|dLSE| <= 1e-3 (bf16: scores rounded to fp32 from bf16 products) and closed-form / needle pins.
+Tolerances (BASELINE.json north_star; DESIGN.md §2 readings A10 / A18, §6): bf16 I/O max-abs <= 1e-2 and
+mean-abs <= 1e-3 over ALL output elements of a config; fp32 config max-abs <= 1e-5; KV append bit-exact.
+Because N(0,1) inputs at long caches make the outputs themselves tiny, the tests
+additionally gate on relative RMS error <= 1e-2, |dLSE| <= 1e-4 and closed-form / needle pins, and on the
+element-wise bound that follows from the arithmetic (gpu_harness.bf16_error_bound, `bound_viol <= 0`):
+    |O_gpu - O_ref| <= half a bf16 ulp of the output + 1.05 * 2^-8 * sum_j w_j |v_j|.
+Where max|O_ref| >= 1 (short caches with x8 outlier channels concentrate the softmax; |O| reaches ~4) the
+bf16 rounding of the output alone is up to 2^-7 = 7.8e-3 and the contractual max-abs 1e-2 stops being
+meaningful: those cases (BF16_TOL_BIG_O) gate on the derived bound, mean-abs and rel-RMS instead.
 """
 import math
 
@@ -11,12 +16,13 @@ import numpy as np
 import pytest
 
 from synth_inputs import generate, spec_for_config, to_bf16
-from tests.gpu_harness import (compare, make_cache, preload_gpu, run_workload_gpu,
+from tests.gpu_harness import (bf16_error_bound, compare, make_cache, preload_gpu, run_workload_gpu,
                                run_workload_oracle, _torch_of, _numpy_of)
 
 pytestmark = pytest.mark.gpu
 
-BF16_TOL = dict(max_abs=1e-2, mean_abs=1e-3, rel_rms=1e-2, lse_max=1e-3)
+BF16_TOL = dict(max_abs=1e-2, mean_abs=1e-3, rel_rms=1e-2, lse_max=1e-4, bound_viol=0.0)
+BF16_TOL_BIG_O = {k: v for k, v in BF16_TOL.items() if k != "max_abs"}
 F32_TOL = dict(max_abs=1e-5, mean_abs=1e-5, rel_rms=1e-5, lse_max=1e-5)
 
 
@@ -30,7 +36,7 @@ def _assert_close(err, tol, label=""):
     print(f"[parity] {label}: " + " ".join(f"{k}={v:.3e}" if isinstance(v, float) else f"{k}={v}" for k, v in err.items()))
     assert err["finite"], (label, err)
     for k, v in tol.items():
-        assert err[k] <= v, (label, k, err)
+        assert err[k] <= v, (label, k, err)                 # (a NaN - metric not computed - fails too)
     assert err["kv_bit_exact"] in (True, None), (label, "kv append not bit exact")
 
 
@@ -281,8 +287,7 @@ def test_fused_combine_decode_plan_and_ragged_batch():
     _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "fused combine, decode plan")
     w = _small(5, cache_len_range=(100, 1500), block_tokens=64, modality_split=(48, 12, 4))
     got = run_workload_gpu(w, flags=WS_FLAG_FUSED_COMBINE, gather=False)
-    tol = dict(BF16_TOL); tol.pop("max_abs"); tol["max_excess"] = 8e-3     # see the ragged test below
-    _assert_close(compare(got, run_workload_oracle(w), "bf16"), tol, "fused combine, ragged batch")
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL_BIG_O, "fused combine, ragged batch")
 
 
 def test_page_assignment_independence():
@@ -297,10 +302,9 @@ def test_ragged_multi_session_small_and_batched_equals_single():
     got = run_workload_gpu(w)
     ref = run_workload_oracle(w)
     # short caches + x8 outlier channels concentrate the softmax, so |O| reaches ~4 and the bf16
-    # rounding of the output alone (up to 2^-7 = 7.8e-3 for |O| in [2,4)) approaches 1e-2: gate the
-    # error in excess of 2^-8 |O| instead (what is left is the bf16 rounding of P at |O| ~ 4).
-    tol = dict(BF16_TOL); tol.pop("max_abs"); tol["max_excess"] = 8e-3
-    _assert_close(compare(got, ref, "bf16"), tol, "ragged small")
+    # rounding of the output alone (up to 2^-7 = 7.8e-3 for |O| in [2,4)) approaches 1e-2: the gate is
+    # the derived element-wise bound (module docstring), not the flat max-abs.
+    _assert_close(compare(got, ref, "bf16"), BF16_TOL_BIG_O, "ragged small")
     # each session alone (same inputs) gives the same output within fp tolerance of the oracle
     import dataclasses
     for s in (0, 5):
@@ -308,7 +312,7 @@ def test_ragged_multi_session_small_and_batched_equals_single():
                                    cache_lens=[w.cache_lens[s]], sessions=[w.sessions[s]])
         g1 = run_workload_gpu(solo, gather=False)
         d1 = np.abs(g1["out"][0][0] - ref["out"][0][s])
-        assert (d1 - np.abs(ref["out"][0][s]) * 2.0 ** -8).max() <= 8e-3 and d1.mean() <= 1e-3   # same gate as above
+        assert (d1 <= bf16_error_bound(ref["out"][0][s], g1["out"][0][0], ref["abs"][0][s])).all() and d1.mean() <= 1e-3
         # different split plans round P and O differently: both runs are within tolerance of the
         # oracle, so they are within twice the tolerance of each other (and much closer on average)
         a, b = g1["out"][0][0], got["out"][0][s]
@@ -338,7 +342,7 @@ def test_multi_block_query_tensor_core():
     o_ref, l_ref = attend(sess, q, w.spec.scale, 3)
     d = out.float().cpu().numpy() - o_ref
     assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3
-    assert np.abs(lse.cpu().numpy() - l_ref).max() <= 1e-3
+    assert np.abs(lse.cpu().numpy() - l_ref).max() <= 1e-4
 
 
 def _prefill_case(block_sizes, Hq, Hkv, seed, L0=0, expect_kernel=1, min_splits=0):
@@ -394,7 +398,7 @@ def test_next1_multi_block_prefill(blocks, Hq, Hkv, L0):
     assert np.isfinite(o).all() and np.isfinite(lse).all()
     assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3
     assert np.sqrt((d ** 2).mean() / (o_ref ** 2).mean()) <= 1e-2
-    assert np.abs(lse - l_ref).max() <= 1e-3
+    assert np.abs(lse - l_ref).max() <= 1e-4
 
 
 # ------------------------------------------------------------------ NEXT-4: decode plan
@@ -443,15 +447,14 @@ def test_next4_token_causal_decode(n, Hq, Hkv, L0, splits):
     d = o - o_ref
     assert np.isfinite(o).all() and np.isfinite(lse).all()
     assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3
-    assert np.abs(lse - l_ref).max() <= 1e-3
+    assert np.abs(lse - l_ref).max() <= 1e-4
 
 
 def test_next4_decode_ragged_multi_session():
     w = _small(5, cache_lens=(700, 1300, 2081, 90, 1500, 333, 2600, 1024), block_tokens=8, modality_split=(4, 3, 1), steps=2)
     got = run_workload_gpu(w)
     assert all(pl["used_tensor_core_kernel"] == 3 for pl in got["plans"])
-    tol = dict(BF16_TOL); tol.pop("max_abs"); tol["max_excess"] = 8e-3
-    _assert_close(compare(got, run_workload_oracle(w), "bf16"), tol, "decode ragged multi-session")
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL_BIG_O, "decode ragged multi-session")
 
 
 # ------------------------------------------------------------------ NEXT-2: solver-step mode
@@ -591,9 +594,9 @@ def test_graph_capture_ragged_multi_session_uses_large_parameter_tier():
     o = out.float().cpu().numpy().astype(np.float64).reshape(S, n, sp.num_q_heads, sp.head_dim)
     for s in range(S):
         d = o[s] - ref["out"][0][s]
-        # short caches + x8 outlier channels: |O| reaches ~4, gate the error in excess of the bf16
-        # output rounding (see test_ragged_multi_session_small_and_batched_equals_single)
-        assert (np.abs(d) - 2.0 ** -8 * np.abs(ref["out"][0][s])).max() <= 8e-3 and np.abs(d).mean() <= 1e-3, s
+        # short caches + x8 outlier channels: |O| reaches ~4: derived bound instead of the flat max-abs
+        # (see test_ragged_multi_session_small_and_batched_equals_single)
+        assert (np.abs(d) <= bf16_error_bound(ref["out"][0][s], o[s], ref["abs"][0][s])).all() and np.abs(d).mean() <= 1e-3, s
 
 
 # ------------------------------------------------------------------ closed-form pins on the GPU
@@ -671,8 +674,7 @@ def test_large_scores_do_not_overflow():
     w = _small(5, num_sessions=2, cache_len_range=(500, 900), block_tokens=64, modality_split=(48, 12, 4),
                outlier_frac=0.25, outlier_scale=8.0)
     got = run_workload_gpu(w)
-    err = compare(got, run_workload_oracle(w), "bf16")
-    assert err["finite"] and err["max_abs"] <= 2e-2 and err["rel_rms"] <= 1e-2, err
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL_BIG_O, "large scores")
 
 
 @pytest.mark.parametrize("n", [128, 64], ids=["general_plan", "decode_plan"])
@@ -707,10 +709,10 @@ def test_growing_scores_exercise_every_rescale_path(kind, n):
                                      min_splits=splits)
         sess = OracleSession(Hkv, 128)
         sess.append(k_all[:L], v_all[:L]); sess.append(k_all[L:], v_all[L:])
-        o_ref, l_ref = attend(sess, q, scale)
+        o_ref, l_ref, a_ref = attend(sess, q, scale, want_abs=True)
         assert np.isfinite(o).all() and np.isfinite(lse).all(), kind
         d = np.abs(o - o_ref)
-        assert (d - 2.0 ** -8 * np.abs(o_ref)).max() <= 6e-3, (kind, splits, d.max())
+        assert (d <= bf16_error_bound(o_ref, o, a_ref)).all(), (kind, splits, (d - bf16_error_bound(o_ref, o, a_ref)).max())
         assert np.abs(lse - l_ref).max() <= 2e-3 * max(1.0, np.abs(l_ref).max() / 50), (kind, splits)
 
 
@@ -729,34 +731,39 @@ def test_config2_full_size():
     _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "cfg2")
 
 
-def test_config3_full_size_sampled():
+def test_config3_full_size_every_element():
+    """Every output element (512 tokens x 32 heads x 128) against the oracle (reading A18)."""
     w = generate(spec_for_config(3))
-    rows, heads = _sample(512, 32, seed=3)
     got = run_workload_gpu(w)
-    ref = run_workload_oracle(w, rows=rows, heads=heads)
-    _assert_close(compare(got, ref, "bf16", rows=rows, heads=heads), BF16_TOL, "cfg3")
+    assert got["tensor"]
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "cfg3 (all elements)")
 
 
-def test_config4_long_session_20_steps_sampled():
+def test_config4_long_session_20_steps():
+    """Units 1 and 20 (cache 65,536 and 70,400 tokens): every output element; the 18 units in between:
+    sampled rows x heads (the float64 oracle needs ~5 s per full unit on the test box)."""
     w = generate(spec_for_config(4))
-    rows, heads = _sample(256, 32, k=12, seed=4)
     got = run_workload_gpu(w)
     assert got["tensor"] and got["plans"][0]["num_ctas"] == 148
-    ref = run_workload_oracle(w, rows=rows, heads=heads, steps=(0, 7, 19))
-    err = compare(got, ref, "bf16", rows=rows, heads=heads)
-    _assert_close(err, BF16_TOL, "cfg4")
+    full = run_workload_oracle(w, steps=(0, 19))
+    _assert_close(compare(got, full, "bf16"), BF16_TOL, "cfg4 units 1 and 20 (all elements)")
+    rows, heads = _sample(256, 32, k=12, seed=4)
+    part = run_workload_oracle(w, rows=rows, heads=heads, steps=range(1, 19))
+    err = compare(got, part, "bf16", rows=rows, heads=heads)
+    err["kv_bit_exact"] = None                                    # (checked by the first comparison)
+    _assert_close(err, BF16_TOL, "cfg4 units 2-19 (sampled)")
     # every step's output is finite and non-trivial
     for t in range(20):
         o = got["out"][t][0]
         assert np.isfinite(o).all() and 0.003 < o.std() < 0.02
 
 
-def test_config5_ragged_multi_session_sampled():
+def test_config5_ragged_multi_session_every_element():
+    """All 8 sessions x 256 tokens x 32 heads x 128 against the oracle (reading A18)."""
     w = generate(spec_for_config(5))
-    rows, heads = _sample(256, 32, k=12, seed=5)
     got = run_workload_gpu(w)
-    ref = run_workload_oracle(w, rows=rows, heads=heads)
-    _assert_close(compare(got, ref, "bf16", rows=rows, heads=heads), BF16_TOL, "cfg5")
+    assert got["tensor"]
+    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "cfg5 (all elements)")
 
 
 def test_maximum_size_one_million_token_session_sampled():
@@ -802,7 +809,7 @@ def test_maximum_size_one_million_token_session_sampled():
     rel_rms = float(np.sqrt((d ** 2).mean() / (o_ref ** 2).mean()))
     dl = np.abs(lse.cpu().numpy().astype(np.float64)[rows][:, heads] - l_ref).max()
     print(f"[parity] 1M tokens: max_abs={np.abs(d).max():.3e} rel_rms={rel_rms:.3e} lse_max={dl:.3e}")
-    assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3 and rel_rms <= 1e-2 and dl <= 1e-3
+    assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3 and rel_rms <= 1e-2 and dl <= 1e-4
     # the end of the history (last preload block's mid-page tail + the new block), bit for bit
     cnt = 700
     kg = torch.empty((cnt, Hkv, D), dtype=torch.bfloat16, device=dev); vg = torch.empty_like(kg)
@@ -892,7 +899,7 @@ def test_stream_step_single_call_equals_two_calls():
         o = oa.float().cpu().numpy().reshape(S, n, sp.num_q_heads, 128)
         for s in range(S):
             d = np.abs(o[s] - ref["out"][t][s])
-            assert (d - np.abs(ref["out"][t][s]) * 2.0 ** -8).max() <= 8e-3 and d.mean() <= 1e-3
+            assert (d <= bf16_error_bound(ref["out"][t][s], o[s], ref["abs"][t][s])).all() and d.mean() <= 1e-3
     tokens_before = a.session_info(ids_a[0])[0]
     with pytest.raises(WsError):
         a.stream_step(ids_a, cu, q, k, v, oa, -1.0)          # bad scale: nothing may be committed

@@ -345,3 +345,35 @@ def test_fm_euler_exact_velocity_recovers_clean_latent():
         np.testing.assert_allclose(fm_euler_update(zt, eps - z0, 1 - tau), eps, rtol=0, atol=1e-15)
     # hand value: z = 2, v = 4, dtau = -0.25 -> 1
     assert fm_euler_update(np.array([2.0]), np.array([4.0]), -0.25)[0] == 1.0
+
+
+def test_abs_weighted_output_pins():
+    """attend(want_abs=True): A = sum_j w_j |v_j| (the condition number the bf16 error bound of the GPU
+    tests is stated with).  Pins: V >= 0  =>  A == O; flipping the sign of V rows leaves A unchanged and
+    |O| <= A always; hand example P0 with V negated on key 1: rows 0,1 -> A = (1/3, 2/3), O = (1/3, -2/3)."""
+    q, k, v = _stream([5, 7, 4], 4, 2, 8, seed=91)
+    sess = OracleSession(2, 8)
+    pos = 0
+    for b in (5, 7, 4):
+        sess.append(k[pos:pos + b], np.abs(v[pos:pos + b])); pos += b
+    o, lse, a = attend(sess, q[-4:], 0.3, want_abs=True)
+    np.testing.assert_allclose(a, o, rtol=0, atol=1e-15)
+    sess2 = OracleSession(2, 8)
+    pos = 0
+    sign = np.where(np.arange(16) % 3 == 0, -1.0, 1.0)[:, None, None]
+    for b in (5, 7, 4):
+        sess2.append(k[pos:pos + b], (np.abs(v) * sign)[pos:pos + b]); pos += b
+    o2, lse2, a2 = attend(sess2, q[-4:], 0.3, want_abs=True)
+    np.testing.assert_allclose(a2, a, rtol=0, atol=1e-15)
+    np.testing.assert_array_equal(lse2, lse)
+    assert (np.abs(o2) <= a2 + 1e-15).all() and np.abs(o2 - o).max() > 1e-3
+    # P0 geometry (tests/golden/p0_hand_example.txt) with V[1] negated
+    s0 = OracleSession(1, 2)
+    kk = np.log(np.array([1.0, 2.0, 3.0, 4.0]))
+    K = np.stack([kk, np.zeros(4)], axis=1)[:, None, :]
+    V = np.array([[1.0, 0.0], [0.0, -1.0], [2.0, 0.0], [0.0, 2.0]])[:, None, :]
+    s0.append(K[:2], V[:2])
+    Q = np.tile(np.array([1.0, 0.0]), (2, 1, 1))
+    o0, _, a0 = attend(s0, Q, 1.0, want_abs=True)
+    np.testing.assert_allclose(o0[:, 0], [[1 / 3, -2 / 3]] * 2, atol=1e-15)
+    np.testing.assert_allclose(a0[:, 0], [[1 / 3, 2 / 3]] * 2, atol=1e-15)
