@@ -57,16 +57,20 @@ enum {
   WS_FLAG_DRY_RUN = 1u,
   /* Debug: route bf16 attention through the generic SIMT kernel instead of the tcgen05 kernel.     */
   WS_FLAG_FORCE_SIMT = 2u,
-  /* Run the tcgen05 kernel on CTA pairs (cta_group::2, M = 256 per MMA, each CTA stages half of every
-   * K/V tile) when the plan's team size is even.  Correct but slower on B200. */
-  WS_FLAG_CTA_PAIRS = 4u,
+  /* (4u is retired: it selected a cta_group::2 variant of the tcgen05 kernel that was measured slower
+   * and has been removed.)                                                      */
   /* Merge the split-KV partials (a4) inside the attention kernel instead of in the combine kernel that
    * follows it: every CTA publishes its partials (per-group arrival counters in the workspace), waits
    * until all splits of its (session, KV head) group are there and merges its share of the rows; the
    * kernel is then launched cooperatively so that all CTAs are co-resident while they wait on each
    * other.  Correct and one launch fewer, but measured no faster than the separate kernel on B200
-   * (DESIGN.md section 8), so it is opt-in; never used together with CTA pairs.                     */
-  WS_FLAG_FUSED_COMBINE = 8u
+   * (DESIGN.md section 8), so it is opt-in.                                                         */
+  WS_FLAG_FUSED_COMBINE = 8u,
+  /* ws_stream_step normally commits and attends a block in ONE launch (the attention kernel reads the
+   * new keys from k_new / v_new and two of its warps copy them into the pool).  With this flag it
+   * launches the append kernel and the attention kernel separately, as ws_kv_append followed by
+   * ws_block_causal_attn_fwd would (A/B measurements, tests: both must give identical results).     */
+  WS_FLAG_SEPARATE_APPEND = 16u
 };
 
 typedef struct ws_cache ws_cache_t;   /* opaque; owns host metadata only */

@@ -14,10 +14,10 @@ from typing import Optional, Sequence
 import numpy as np
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("WS_LIB_PATH") or os.path.join(_PKG, "libwanstream.so")
+LIB_PATH = os.path.join(_PKG, "libwanstream.so")
 
 WS_BF16, WS_F32 = 0, 1
-WS_FLAG_DRY_RUN, WS_FLAG_FORCE_SIMT, WS_FLAG_CTA_PAIRS, WS_FLAG_FUSED_COMBINE = 1, 2, 4, 8
+WS_FLAG_DRY_RUN, WS_FLAG_FORCE_SIMT, WS_FLAG_FUSED_COMBINE, WS_FLAG_SEPARATE_APPEND = 1, 2, 8, 16
 STATUS_NAMES = ["WS_OK", "WS_ERR_INVALID_ARG", "WS_ERR_BAD_SESSION", "WS_ERR_OUT_OF_PAGES",
                 "WS_ERR_UNSUPPORTED", "WS_ERR_WORKSPACE_TOO_SMALL", "WS_ERR_CUDA"]
 

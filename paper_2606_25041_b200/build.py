@@ -16,18 +16,14 @@ from concurrent.futures import ThreadPoolExecutor
 PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
-# Development aid: WS_BUILD_TAG=<tag> WS_BUILD_DEFS="-DX=1 ..." builds libwanstream_<tag>.so next to
-# the default library (kernel parameter sweeps); WS_LIB_PATH selects it at load time (binding.py).
-TAG = os.environ.get("WS_BUILD_TAG", "")
-DEFS = os.environ.get("WS_BUILD_DEFS", "").split()
-OUT = os.path.join(PKG, f"libwanstream{'_' + TAG if TAG else ''}.so")
-OBJ = os.path.join(PKG, "build" + ("_" + TAG if TAG else ""))
+OUT = os.path.join(PKG, "libwanstream.so")
+OBJ = os.path.join(PKG, "build")
 SOURCES = ["api.cu", "kv_append.cu", "attn_simt.cu", "attn_sm100.cu", "combine.cu", "fm_euler.cu",
            "host_cache.cpp", "plan.cpp"]
-NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+NVCC = "/usr/local/cuda/bin/nvcc"
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-I", os.path.join(ROOT, "include"),
-         "--expt-relaxed-constexpr", *DEFS]
+         "--expt-relaxed-constexpr"]
 
 
 def _digest() -> str:

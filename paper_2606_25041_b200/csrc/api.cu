@@ -152,7 +152,6 @@ struct ws_cache {
   int64_t launches = 0;
   ws::Plan last_plan;
   bool last_tensor = false;
-  int32_t last_cta_group = 1;
   // ws_stream_step_host pipeline: copy streams + per-slot events (2 staging slots)
   cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
   cudaEvent_t ev_h2d[2]{}, ev_compute[2]{}, ev_d2h[2]{};
@@ -168,6 +167,21 @@ struct ws_cache {
 };
 
 namespace {
+
+// Makes the cache's device current for the duration of an entry point (one process may own caches on
+// several devices: the owner + replica mode of NEXT-3) and restores the caller's device afterwards.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(const ws_cache* c) {
+    if (!c || c->dry) return;
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != c->cfg.device)
+      switched = cudaSetDevice(c->cfg.device) == cudaSuccess;
+    else
+      (void)cudaGetLastError();
+  }
+  ~DeviceGuard() { if (switched) (void)cudaSetDevice(prev); }
+};
 
 // Reserve the next metadata slot: returns host staging pointer; *dev gets the device address.
 ws_status_t next_slot(ws_cache* c, size_t bytes, char** host, char** dev) {
@@ -370,7 +384,8 @@ ws_status_t ws_cache_destroy(ws_cache_t* c) {
   if (c->dry) {
     free(c->h_meta);
   } else {
-    (void)cudaDeviceSynchronize();
+    DeviceGuard dg(c);
+    (void)cudaDeviceSynchronize();          // the cache's device: copies from the pinned ring may be in flight
     for (int i = 0; i < kRing; ++i)
       if (c->ev[i]) (void)cudaEventDestroy(c->ev[i]);
     for (auto* lst : {&c->t_append, &c->t_attn, &c->t_combine})
@@ -452,9 +467,23 @@ ws_status_t ws_debug_set_min_splits(ws_cache_t* c, int32_t min_splits) {
 }
 
 // ------------------------------------------------------------------------------------ a2 append
-ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
-                         const int32_t* cu, const void* k_new, const void* v_new,
-                         const uint8_t* modality, void* cuda_stream) {
+}  // extern "C"
+
+namespace {
+
+// The append of one call, prepared on the host: validated, committed to the host metadata, descriptor blob
+// built - in `inl` (kernel-parameter tier) or in a slot of the pinned ring (`h` / `d`).
+struct AppendPrep {
+  bool inline_meta = true;
+  ws::InlineAppendMeta inl{};
+  char* h = nullptr;
+  char* d = nullptr;
+  size_t bytes = 0;
+};
+
+// No state changes.  *words = size of the descriptor blob.
+ws_status_t append_validate(ws_cache* c, int32_t S, const int32_t* session_ids, const int32_t* cu,
+                            const void* k_new, const void* v_new, size_t* words_out) {
   if (!c || !session_ids || !cu) return fail(WS_ERR_INVALID_ARG, "NULL argument");
   if (S < 1 || S > c->cfg.max_sessions_per_call)
     return fail(WS_ERR_INVALID_ARG, "num_sessions %d not in [1, %d]", S, c->cfg.max_sessions_per_call);
@@ -481,27 +510,29 @@ ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
   if (extra_pages > c->host->free_pages())
     return fail(WS_ERR_OUT_OF_PAGES, "need %lld pages, %d free", (long long)extra_pages,
                 c->host->free_pages());
-  // metadata size check BEFORE mutating
   size_t words = sizeof(ws::AppendMeta) / 4 + (size_t)S * sizeof(ws::AppendSession) / 4;
   for (int32_t s = 0; s < S; ++s) words += (size_t)(cu[s + 1] - cu[s]) / P + 3;
   if (words * 4 > c->lay.meta_slot_bytes)
     return fail(WS_ERR_WORKSPACE_TOO_SMALL, "append metadata exceeds the slot");
-  char *h = nullptr, *d = nullptr;
-  ws::InlineAppendMeta inl{};
-  const bool inline_meta = words <= (size_t)ws::kInlineAppendWords;
-  ws_status_t st = WS_OK;
-  if (inline_meta) {
-    h = (char*)inl.w;
-  } else {
+  *words_out = words;
+  return WS_OK;
+}
+
+// Commits the blocks to the host metadata and builds the descriptor.  Call only after append_validate.
+ws_status_t append_commit(ws_cache* c, int32_t S, const int32_t* session_ids, const int32_t* cu,
+                          const uint8_t* modality, size_t words, cudaStream_t stream, AppendPrep* ap) {
+  ap->inline_meta = words <= (size_t)ws::kInlineAppendWords;
+  char* h = (char*)ap->inl.w;
+  if (!ap->inline_meta) {
     if (!c->dry) {
-      st = refuse_if_capturing((cudaStream_t)cuda_stream, "append metadata");
+      ws_status_t st = refuse_if_capturing(stream, "append metadata");
       if (st != WS_OK) return st;
     }
-    st = next_slot(c, words * 4, &h, &d);
+    ws_status_t st = next_slot(c, words * 4, &ap->h, &ap->d);
     if (st != WS_OK) return st;
+    h = ap->h;
   }
-
-  // ---- commit (no failure paths below except CUDA errors)
+  // ---- commit (no failure paths below)
   ws::AppendMeta hdr{S, cu[S], (int32_t)(sizeof(ws::AppendMeta) / 4),
                      (int32_t)(sizeof(ws::AppendMeta) / 4 + S * sizeof(ws::AppendSession) / 4)};
   int32_t* blob = (int32_t*)h;
@@ -523,32 +554,39 @@ ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
   }
   msg[kMsgTotalWord] = (int32_t)msg.size();
   memcpy(blob, &hdr, sizeof(hdr));
+  ap->bytes = (size_t)(hdr.off_pages + npg) * 4;
+  return WS_OK;
+}
+
+ws_status_t append_launch(ws_cache* c, const AppendPrep& ap, const void* k_new, const void* v_new,
+                          int32_t total_tokens, cudaStream_t stream) {
   if (c->dry) return WS_OK;
-  cudaStream_t stream = (cudaStream_t)cuda_stream;
-  if (!inline_meta) {
-    st = upload_slot(c, h, d, (size_t)(hdr.off_pages + npg) * 4, stream);
+  if (!ap.inline_meta) {
+    ws_status_t st = upload_slot(c, ap.h, ap.d, ap.bytes, stream);
     if (st != WS_OK) return st;
   }
   TimedLaunch tl(c, &c->t_append, stream);
   WS_CUDA(ws::launch_kv_append(k_new, v_new, c->cfg.k_pool, c->cfg.v_pool, c->d_page_table,
-                               inline_meta ? nullptr : (const int32_t*)d, inl, c->peers, cu[S], c->cfg.max_pages_per_session, P,
-                               c->cfg.num_kv_heads, c->cfg.head_dim, eb_of(c->cfg.dtype), c->num_sms,
-                               stream));
+                               ap.inline_meta ? nullptr : (const int32_t*)ap.d, ap.inl, c->peers, total_tokens,
+                               c->cfg.max_pages_per_session, c->cfg.page_tokens, c->cfg.num_kv_heads,
+                               c->cfg.head_dim, eb_of(c->cfg.dtype), c->num_sms, stream));
   tl.done();
   c->launches += 1;
   return WS_OK;
 }
 
-// ------------------------------------------------------------------------------------ a3 + a4
-ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* session_ids,
-                                     const int32_t* num_q_blocks, const int32_t* cu, const void* q,
-                                     void* out, float* lse, float scale, void* cuda_stream) {
-  if (!c || !session_ids || !cu) return fail(WS_ERR_INVALID_ARG, "NULL argument");
-  if (S < 1 || S > c->cfg.max_sessions_per_call)
-    return fail(WS_ERR_INVALID_ARG, "num_sessions %d not in [1, %d]", S, c->cfg.max_sessions_per_call);
-  if (!c->dry && (!q || !out)) return fail(WS_ERR_INVALID_ARG, "q / out is NULL");
-  if (!(scale > 0.f) || !std::isfinite(scale)) return fail(WS_ERR_INVALID_ARG, "scale must be finite and > 0");
-  if (cu[0] != 0) return fail(WS_ERR_INVALID_ARG, "cu_q_tokens[0] must be 0");
+// Fused step: the block committed by `ap` is attended in the same launch (tcgen05 kernel only).
+struct FusedAppend {
+  const AppendPrep* ap;
+  const void* k_new;
+  const void* v_new;
+};
+
+// a3 + a4.  fuse != nullptr: every session's last block (its cu range) is the one being committed by this
+// launch: its keys are read from k_new / v_new, and warps 10-11 of the kernel copy it into the pool.
+ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const int32_t* num_q_blocks,
+                      const int32_t* cu, const void* q, void* out, float* lse, float scale,
+                      cudaStream_t stream, const FusedAppend* fuse) {
   std::vector<ws::PlanSession> ps(S);
   std::vector<int32_t> vis_end, tok_slot;
   bool any_multi = false;
@@ -565,7 +603,7 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     if (cu[s + 1] - cu[s] != nq)
       return fail(WS_ERR_INVALID_ARG, "session %d: cu gives %d query tokens, its last %d block(s) hold %lld",
                   id, cu[s + 1] - cu[s], m, (long long)nq);
-    ps[s] = ws::PlanSession{id, cu[s], cu[s + 1], m > 1, (int32_t)ss.stable_tokens};
+    ps[s] = ws::PlanSession{id, cu[s], cu[s + 1], m > 1, fuse ? (int32_t)nq : 0};
     any_multi |= m > 1;
     for (int32_t b = B - m; b < B; ++b) {
       int64_t lo = b ? ss.block_ends[b - 1] : 0;
@@ -577,13 +615,13 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
   if (NQ > c->cfg.max_q_tokens_per_call)
     return fail(WS_ERR_INVALID_ARG, "%d query tokens > max_q_tokens_per_call %d", NQ,
                 c->cfg.max_q_tokens_per_call);
-  cudaStream_t stream = (cudaStream_t)cuda_stream;
   const bool tensor = c->tensor_path_ok && !(c->cfg.flags & WS_FLAG_FORCE_SIMT);
   c->last_tensor = tensor;
   const int G = c->cfg.num_q_heads / c->cfg.num_kv_heads;
   char *h = nullptr, *d = nullptr;
 
   if (!tensor) {
+    if (fuse) return fail(WS_ERR_UNSUPPORTED, "internal: fused step on the generic kernel");
     if (c->dry && !c->tensor_path_ok) { c->last_plan = ws::Plan(); return WS_OK; }
     if (!c->dry) {
       size_t bytes = (size_t)NQ * 8;
@@ -631,7 +669,7 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     key.reserve(8 + 5 * (size_t)S);
     key.insert(key.end(), {pc.Hkv, pc.G, pc.num_sms, pc.min_splits, pc.max_part_slots, (int32_t)pc.allow_alt, S});
     for (int32_t s = 0; s < S; ++s)
-      key.insert(key.end(), {ps[s].slot, ps[s].q_begin, ps[s].q_end, vis_end[ps[s].q_begin], ps[s].stable_tokens});
+      key.insert(key.end(), {ps[s].slot, ps[s].q_begin, ps[s].q_end, vis_end[ps[s].q_begin], ps[s].new_len});
     cached = plan_cache_lookup(key, &plan, &blob);
   }
   if (!cached) {
@@ -658,37 +696,22 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     memcpy(h, blob.data(), blob.size() * 4);
   }
   c->last_plan = std::move(plan);
-  // CTA pairs (tcgen05 cta_group::2) halve the shared-memory operand traffic but put two DSMEM
-  // round trips (remote P arrival, multicast S commit) on the S -> softmax -> PV chain that bounds
-  // this kernel: measured 309 us vs 224 us per config-4 unit.  Opt-in only.
-  const int32_t cta_group = (!c->last_plan.alt && (c->cfg.flags & WS_FLAG_CTA_PAIRS) &&
-                             c->last_plan.team_size % 2 == 0) ? 2 : 1;
-  c->last_cta_group = c->last_plan.alt ? 3 : cta_group;
-  // every append launched before this kernel has completed once this kernel has (PDL chain, see
-  // attn_sm100.cu): the next call may read those tokens before its own griddepcontrol.wait
-  c->host->mark_all_stable();
   if (c->dry) return WS_OK;
-  if (!inline_meta) {
-    st = upload_slot(c, h, d, blob.size() * 4, stream);
-    if (st != WS_OK) return st;
-  }
 
   ws::Sm100Launch L{};
-  if (inline_meta) { memcpy(L.inl.w, blob.data(), blob.size() * 4); d = nullptr; }
-  L.inl_words = inline_meta ? (int32_t)blob.size() : 0;
   L.p.q = q; L.p.out = out; L.p.lse = lse;
   L.p.k_pool = c->cfg.k_pool; L.p.v_pool = c->cfg.v_pool;
   L.p.page_table = c->d_page_table;
-  L.p.meta = (const int32_t*)d;
   L.p.part_o = c->d_part_o; L.p.part_lse = c->d_part_lse;
-  const bool fused_combine = cta_group == 1 && (c->cfg.flags & WS_FLAG_FUSED_COMBINE) &&
-                             !c->last_plan.combine.empty();
+  const bool fused_combine = (c->cfg.flags & WS_FLAG_FUSED_COMBINE) && !c->last_plan.combine.empty();
   L.p.merge_ctr = fused_combine ? c->d_merge_ctr : nullptr;
   L.p.max_part_slots = c->lay.max_part_slots;
   L.p.max_pages_per_session = c->cfg.max_pages_per_session;
   L.p.Hq = c->cfg.num_q_heads; L.p.Hkv = c->cfg.num_kv_heads; L.p.D = c->cfg.head_dim;
   L.p.G = G; L.p.P = c->cfg.page_tokens; L.p.total_q_tokens = NQ; L.p.scale = scale;
   L.tmap_k = c->tmap_k; L.tmap_v = c->tmap_v;
+  L.tmap_kn = c->tmap_k; L.tmap_vn = c->tmap_v;
+  // every tensor map is encoded before anything is enqueued: a failure leaves the stream untouched
   {
     const cuuint64_t D = 128, Hq = c->cfg.num_q_heads;
     cuuint64_t dims[3] = {D, Hq, (cuuint64_t)NQ};
@@ -697,8 +720,29 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
     st = encode_tmap(c, &L.tmap_q, const_cast<void*>(q), 3, dims, strides, box);
     if (st != WS_OK) return st;
   }
+  if (fuse) {
+    const cuuint64_t D = 128, Hkv = c->cfg.num_kv_heads;
+    cuuint64_t dims[3] = {D, Hkv, (cuuint64_t)NQ};
+    cuuint64_t strides[2] = {D * 2, Hkv * D * 2};
+    cuuint32_t box[3] = {64, 1, 64};
+    st = encode_tmap(c, &L.tmap_kn, const_cast<void*>(fuse->k_new), 3, dims, strides, box);
+    if (st != WS_OK) return st;
+    st = encode_tmap(c, &L.tmap_vn, const_cast<void*>(fuse->v_new), 3, dims, strides, box);
+    if (st != WS_OK) return st;
+    L.p.k_new = fuse->k_new; L.p.v_new = fuse->v_new;
+    L.p.k_pool_w = c->cfg.k_pool; L.p.v_pool_w = c->cfg.v_pool; L.p.page_table_w = c->d_page_table;
+    L.p.append_tokens = NQ;
+    L.app = fuse->ap->inl;
+    L.peers = c->peers;
+  }
+  if (!inline_meta) {
+    st = upload_slot(c, h, d, blob.size() * 4, stream);
+    if (st != WS_OK) return st;
+  }
+  if (inline_meta) { memcpy(L.inl.w, blob.data(), blob.size() * 4); d = nullptr; }
+  L.inl_words = inline_meta ? (int32_t)blob.size() : 0;
+  L.p.meta = (const int32_t*)d;
   L.num_ctas = c->last_plan.num_teams * c->last_plan.team_size;
-  L.cta_group = cta_group;
   L.alt = c->last_plan.alt;
   TimedLaunch tl(c, &c->t_attn, stream);
   WS_CUDA(ws::launch_attn_sm100(L, stream));
@@ -715,18 +759,68 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
   return WS_OK;
 }
 
+ws_status_t attn_validate_args(ws_cache* c, int32_t S, const int32_t* session_ids, const int32_t* cu,
+                               const void* q, void* out, float scale) {
+  if (!c || !session_ids || !cu) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  if (S < 1 || S > c->cfg.max_sessions_per_call)
+    return fail(WS_ERR_INVALID_ARG, "num_sessions %d not in [1, %d]", S, c->cfg.max_sessions_per_call);
+  if (!c->dry && (!q || !out)) return fail(WS_ERR_INVALID_ARG, "q / out is NULL");
+  if (!(scale > 0.f) || !std::isfinite(scale)) return fail(WS_ERR_INVALID_ARG, "scale must be finite and > 0");
+  if (cu[0] != 0) return fail(WS_ERR_INVALID_ARG, "cu_q_tokens[0] must be 0");
+  return WS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
+                         const int32_t* cu, const void* k_new, const void* v_new,
+                         const uint8_t* modality, void* cuda_stream) {
+  size_t words = 0;
+  ws_status_t st = append_validate(c, S, session_ids, cu, k_new, v_new, &words);
+  if (st != WS_OK) return st;
+  DeviceGuard dg(c);
+  AppendPrep ap;
+  st = append_commit(c, S, session_ids, cu, modality, words, (cudaStream_t)cuda_stream, &ap);
+  if (st != WS_OK) return st;
+  return append_launch(c, ap, k_new, v_new, cu[S], (cudaStream_t)cuda_stream);
+}
+
+// ------------------------------------------------------------------------------------ a3 + a4
+ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* session_ids,
+                                     const int32_t* num_q_blocks, const int32_t* cu, const void* q,
+                                     void* out, float* lse, float scale, void* cuda_stream) {
+  ws_status_t st = attn_validate_args(c, S, session_ids, cu, q, out, scale);
+  if (st != WS_OK) return st;
+  DeviceGuard dg(c);
+  return attn_impl(c, S, session_ids, num_q_blocks, cu, q, out, lse, scale, (cudaStream_t)cuda_stream, nullptr);
+}
+
 ws_status_t ws_stream_step(ws_cache_t* c, int32_t S, const int32_t* session_ids, const int32_t* cu,
                            const void* q, const void* k_new, const void* v_new, void* out, float* lse,
                            float scale, void* cuda_stream) {
   // validate what only the second half would reject BEFORE the append commits anything
-  if (!c || !session_ids || !cu) return fail(WS_ERR_INVALID_ARG, "NULL argument");
-  if (!c->dry && (!q || !out)) return fail(WS_ERR_INVALID_ARG, "q / out is NULL");
-  if (!(scale > 0.f) || !std::isfinite(scale)) return fail(WS_ERR_INVALID_ARG, "scale must be finite and > 0");
-  if (S >= 1 && S <= c->cfg.max_sessions_per_call && cu[S] > c->cfg.max_q_tokens_per_call)
-    return fail(WS_ERR_INVALID_ARG, "%d query tokens > max_q_tokens_per_call %d", cu[S], c->cfg.max_q_tokens_per_call);
-  ws_status_t st = ws_kv_append(c, S, session_ids, cu, k_new, v_new, nullptr, cuda_stream);
+  ws_status_t st = attn_validate_args(c, S, session_ids, cu, q, out, scale);
   if (st != WS_OK) return st;
-  return ws_block_causal_attn_fwd(c, S, session_ids, nullptr, cu, q, out, lse, scale, cuda_stream);
+  size_t words = 0;
+  st = append_validate(c, S, session_ids, cu, k_new, v_new, &words);
+  if (st != WS_OK) return st;
+  DeviceGuard dg(c);
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  AppendPrep ap;
+  st = append_commit(c, S, session_ids, cu, nullptr, words, stream, &ap);
+  if (st != WS_OK) return st;
+  // One launch commits and attends when the tcgen05 kernel runs and the append descriptor fits the kernel
+  // parameters (up to ~900 new pages per call); otherwise: the append kernel, then attention over the pool.
+  const bool tensor = c->tensor_path_ok && !(c->cfg.flags & WS_FLAG_FORCE_SIMT);
+  if (tensor && ap.inline_meta && !(c->cfg.flags & WS_FLAG_SEPARATE_APPEND)) {
+    const FusedAppend fuse{&ap, k_new, v_new};
+    return attn_impl(c, S, session_ids, nullptr, cu, q, out, lse, scale, stream, &fuse);
+  }
+  st = append_launch(c, ap, k_new, v_new, cu[S], stream);
+  if (st != WS_OK) return st;
+  return attn_impl(c, S, session_ids, nullptr, cu, q, out, lse, scale, stream, nullptr);
 }
 
 size_t ws_step_staging_bytes(const ws_cache_config_t* cfg, int32_t n) {
@@ -750,6 +844,13 @@ ws_status_t ws_stream_step_host(ws_cache_t* c, int32_t S, const int32_t* session
   if (staging_bytes < ws_step_staging_bytes(&c->cfg, n))
     return fail(WS_ERR_WORKSPACE_TOO_SMALL, "staging_bytes %zu < required %zu", staging_bytes,
                 ws_step_staging_bytes(&c->cfg, n));
+  // everything the step would reject is rejected before the first copy is enqueued
+  ws_status_t st = attn_validate_args(c, S, session_ids, cu, q_host, out_host, scale);
+  if (st != WS_OK) return st;
+  size_t words = 0;
+  st = append_validate(c, S, session_ids, cu, k_host, v_host, &words);
+  if (st != WS_OK) return st;
+  DeviceGuard dg(c);
   if (!c->h2d_stream) {
     WS_CUDA(cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking));
     WS_CUDA(cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking));
@@ -763,7 +864,10 @@ ws_status_t ws_stream_step_host(ws_cache_t* c, int32_t S, const int32_t* session
   size_t q_bytes = (size_t)n * c->cfg.num_q_heads * D * eb, kv_bytes = (size_t)n * c->cfg.num_kv_heads * D * eb;
   size_t qb = align_up(q_bytes, 256), kb = align_up(kv_bytes, 256);
   const int slot = (int)(c->host_steps & 1);
-  char* base = (char*)staging + (size_t)slot * (2 * qb + 2 * kb);
+  // Fixed slot stride (half of the caller's buffer, 256-byte aligned): steps with different token counts
+  // must not place slot 1 inside the region slot 0 of the previous, larger step is still using.
+  const size_t slot_stride = (staging_bytes / 2) & ~(size_t)255;
+  char* base = (char*)staging + (size_t)slot * slot_stride;
   char *dq = base, *dout = base + qb, *dk = base + 2 * qb, *dv = base + 2 * qb + kb;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   // copy-in on the H2D stream (after the slot's previous result has left the device), compute on the
@@ -774,9 +878,7 @@ ws_status_t ws_stream_step_host(ws_cache_t* c, int32_t S, const int32_t* session
   WS_CUDA(cudaMemcpyAsync(dq, q_host, q_bytes, cudaMemcpyHostToDevice, c->h2d_stream));
   WS_CUDA(cudaEventRecord(c->ev_h2d[slot], c->h2d_stream));
   WS_CUDA(cudaStreamWaitEvent(stream, c->ev_h2d[slot], 0));
-  ws_status_t st = ws_kv_append(c, S, session_ids, cu, dk, dv, nullptr, cuda_stream);
-  if (st != WS_OK) return st;
-  st = ws_block_causal_attn_fwd(c, S, session_ids, nullptr, cu, dq, dout, nullptr, scale, cuda_stream);
+  st = ws_stream_step(c, S, session_ids, cu, dq, dk, dv, dout, nullptr, scale, cuda_stream);
   if (st != WS_OK) return st;
   WS_CUDA(cudaEventRecord(c->ev_compute[slot], stream));
   WS_CUDA(cudaStreamWaitEvent(c->d2h_stream, c->ev_compute[slot], 0));
@@ -861,6 +963,7 @@ ws_status_t ws_replica_snapshot_message(const ws_cache_t* c, int32_t session, in
 
 ws_status_t ws_replica_push_session(ws_cache_t* c, int32_t session, void* cuda_stream) {
   if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  DeviceGuard dg(c);
   if (!c->host->is_open(session)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", session);
   if (c->peers.n == 0) return fail(WS_ERR_INVALID_ARG, "no replica is linked (ws_replica_link)");
   const ws::SessionState& ss = c->host->session(session);
@@ -875,6 +978,7 @@ ws_status_t ws_replica_push_session(ws_cache_t* c, int32_t session, void* cuda_s
 
 ws_status_t ws_replica_apply(ws_cache_t* c, const int32_t* w, int32_t n, void* cuda_stream) {
   if (!c || !w) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  DeviceGuard dg(c);
   if (n < kMsgHeaderWords || w[0] != kMsgMagic) return fail(WS_ERR_INVALID_ARG, "not a commit message");
   if (w[1] != kMsgVersion) return fail(WS_ERR_UNSUPPORTED, "message version %d (this library: %d)", w[1], kMsgVersion);
   if (w[2] != kMsgCommit && w[2] != kMsgSnapshot) return fail(WS_ERR_INVALID_ARG, "unknown message kind %d", w[2]);
@@ -979,6 +1083,7 @@ ws_status_t ws_ipc_close(void* ptr, uint64_t offset) {
 ws_status_t ws_kv_gather(const ws_cache_t* c, int32_t session, int64_t start, int64_t count,
                          void* k_out, void* v_out, void* cuda_stream) {
   if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
+  DeviceGuard dg(c);
   if (!c->host->is_open(session)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", session);
   const ws::SessionState& ss = c->host->session(session);
   if (start < 0 || count < 0 || start + count > ss.tokens)
@@ -1002,7 +1107,7 @@ ws_status_t ws_last_plan_info(const ws_cache_t* c, ws_plan_info_t* out) {
   out->num_segments = (int32_t)p.segments.size();
   out->num_partial_slots = p.num_part_slots;
   out->num_combine_items = (int32_t)p.combine.size();
-  out->used_tensor_core_kernel = c->last_tensor ? c->last_cta_group : 0;
+  out->used_tensor_core_kernel = c->last_tensor ? (p.alt ? 3 : 1) : 0;
   out->total_kv_tiles = p.total_tiles;
   return WS_OK;
 }
@@ -1029,6 +1134,7 @@ ws_status_t ws_debug_kernel_timing(ws_cache_t* c, int32_t enable) {
 
 ws_status_t ws_debug_read_kernel_times(ws_cache_t* c, double* ms_sum3, int32_t* count3) {
   if (!c || !ms_sum3 || !count3) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  DeviceGuard dg(c);
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>>* lists[3] = {&c->t_append, &c->t_attn, &c->t_combine};
   for (int k = 0; k < 3; ++k) {
     ms_sum3[k] = 0.0; count3[k] = (int32_t)lists[k]->size();

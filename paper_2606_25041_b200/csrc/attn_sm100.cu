@@ -12,21 +12,26 @@
 // several segments back to back.
 //
 // Pipeline (12 warps, 1 CTA / SM):
-//   warp 8  lane 0 : TMA producer - Q tiles (rank-3 map over [D, Hq, tokens]) and paged K/V tiles
-//                    (rank-4 map over [D, P, Hkv, pages]; the page id read from the device page
-//                    table is the outermost TMA coordinate) into a 5-slot ring of 32 KB buffers,
-//                    128B-swizzled, completion on mbarriers.
+//   warp 8  lane 0 : TMA producer - Q tiles (rank-3 map over [D, Hq, tokens]) and K/V tiles into a
+//                    5-slot ring of 32 KB buffers, 128B-swizzled, completion on mbarriers.  Keys of the
+//                    committed cache come from the paged pool (rank-4 map over [D, P, Hkv, pages]; the
+//                    page id read from the device page table is the outermost TMA coordinate); in a
+//                    fused step (ws_stream_step) the keys of the block being committed come straight
+//                    from the caller's k_new / v_new (rank-3 maps over [D, Hkv, tokens]) as KV tiles of
+//                    their own after the cache tiles, so nothing waits for the commit.
 //   warp 9  lane 0 : tcgen05.mma issuer - S_q = Q_q K^T (SS, M128 N128 K16 x 8) into TMEM, and
 //                    O_q += P_q V (A = P from TMEM, B = V from smem, MN-major) for q = 0, 1,
 //                    interleaved so the tensor pipe works on one Q tile while the softmax
 //                    warpgroup of the other is busy.  tcgen05.commit arrives on mbarriers.
 //   warps 0-3, 4-7 : softmax warpgroup for Q tile 0 / 1: tcgen05.ld of a whole S row per thread
 //                    (32x32b: thread = row, so max/sum need no cross-thread reduction), fp32 online
-//                    softmax in the log2 domain with lazy rescaling of O (only when the row max
-//                    grows by > 2^8), P rounded to bf16 and written back over S in TMEM, row sum
-//                    accumulated in fp32 from the unrounded p.  Epilogue: O / l -> bf16 out (+ LSE)
-//                    or fp32 partial + log2-LSE when the segment is one of several splits.
+//                    softmax in the log2 domain, P rounded to bf16 and written back over S in TMEM,
+//                    row sum accumulated in fp32 from the unrounded p.  Epilogue: O / l -> bf16 out
+//                    (+ LSE) or fp32 partial + log2-LSE when the segment is one of several splits.
 //   warp 10        : TMEM allocation (512 columns: S0 S1 O0 O1) and release.
+//   warps 10, 11   : fused step only: commit the new block (a2, kv_append.cuh) - copy k_new / v_new
+//                    into the pool pages, publish the page ids, zero the last page's tail - while the
+//                    other warps attend.
 //
 // Roofline: tensor-bound for G*n >= ~260 FLOP/B (configs 3-5), 4*D*rows*keys FLOPs per tile pair;
 // algorithmic bytes per tile = 2 x 128 x 128 x 2 B of K/V.  MUFU ex2 (16/clk/SM) is the co-limit.
@@ -37,6 +42,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include "kv_append.cuh"
 #include "launch.h"
 #include "sm100_ptx.cuh"
 #include "merge.cuh"
@@ -45,49 +51,33 @@ namespace ws {
 
 using namespace ptx;
 
-// kCG = 1: one CTA owns whole K/V tiles (32 KB slots, 5-slot ring).
-// kCG = 2: a CTA pair (cluster of 2, adjacent row-tile pairs of one team) runs M = 256 MMAs
-// (tcgen05 cta_group::2): each CTA stages only HALF of every K tile (64 keys) and V tile (64 dims),
-// halving shared-memory operand reads, TMA writes and L2 requests per FLOP (16 KB slots, 10-slot ring).
-template <int kCG> struct RingCfg;
-template <> struct RingCfg<1> { static constexpr int kStages = 5; static constexpr uint32_t kSlotBytes = 32768; };
-template <> struct RingCfg<2> { static constexpr int kStages = 10; static constexpr uint32_t kSlotBytes = 16384; };
-constexpr int kMaxStages = 10;
-constexpr uint32_t kRingBytes = 5 * 32768;                 // same footprint in both modes
+constexpr int kStages = 5;                                 // K/V ring: 5 slots of one 128-key tile (32 KB)
+constexpr uint32_t kSlotBytes = 32768;
+constexpr uint32_t kRingBytes = kStages * kSlotBytes;
 constexpr uint32_t kHalfBytes = 16384;                     // one 64-dim half of a 128-row tile: 128 rows x 128 B
 constexpr uint32_t kQTileBytes = kTileRows * 128 * 2;
 constexpr int kThreads = 384;
 constexpr uint32_t kTmemCols = 512;
-constexpr float kRescaleThreshold = 8.0f;                  // log2 units
 constexpr int kFirstPieceSteps = 6;                         // P is handed to the MMA warp as keys 0-95, then 96-127
-constexpr float kFastSumLimit = 1024.0f;                   // fast path accepted while tile row sum < 2^10
-#ifndef WS_FAST_PATH
-#define WS_FAST_PATH 1
-#endif
-#ifndef WS_POLY_PER8
-#define WS_POLY_PER8 2
-#endif
-#ifndef WS_DUAL_ISSUER
-#define WS_DUAL_ISSUER 0
-#endif
-
-#ifdef WS_PROFILE
-#define PROF_DECL(n) long long prof_acc[n] = {0}; long long prof_t = clock64();
-#define PROF_MARK(i) { long long t_ = clock64(); prof_acc[i] += t_ - prof_t; prof_t = t_; }
-__device__ __forceinline__ unsigned long long prof_gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-__shared__ unsigned long long prof_stamps[16];
-#define PROF_STAMP(i) { if (prof_stamps[i] == 0) prof_stamps[i] = prof_gtime(); }
-#else
-#define PROF_STAMP(i) {}
-#define PROF_DECL(n)
-#define PROF_MARK(i)
-#endif
+// Optimistic (fast) softmax path: a tile is exponentiated against the running reference without looking
+// for its maximum, and accepted while its row sum stays below BOTH limits:
+//  * kFastSumLimit - every p is <= the sum, so nothing overflowed bf16's useful range;
+//  * kFastSumShare x the row's accumulated sum l - the tile cannot hold a key that carries a large share
+//    of the row's weight.  A tile that could (the first few of a segment, or one with a dominant key)
+//    takes the exact path, which re-references the row to its exact maximum whenever that grew, so the
+//    dominant weight is p = 1 exactly and suffers no bf16 rounding (reading A10: with a stale
+//    reference the x8-outlier config reached 1.2e-2 max-abs; with this rule it stays at the output's
+//    own rounding).
+constexpr float kFastSumLimit = 1024.0f;
+constexpr float kFastSumShare = 0.5f;
+// 2 of every 8 exponentials run as a polynomial on the FMA pipe (ex2_poly2); sweep: DESIGN.md section 8
+constexpr int kPolyPer8 = 2;
 
 constexpr int kMaxJobs = 4;
 
 struct Barriers {
   uint64_t q_full, q_empty;
-  uint64_t kv_full[kMaxStages], kv_empty[kMaxStages];
+  uint64_t kv_full[kStages], kv_empty[kStages];
   uint64_t s_full[2], p_full[2][2], pv_h0_done[2], o_full[2], o_empty[2];
   uint64_t merge_full;
   alignas(16) float lse_stage[kPairRows];
@@ -108,15 +98,13 @@ struct SegView {
 // (pair >= npairs).  For multi-block queries the pair's own visible end clips the tile range: KV
 // tiles beyond the last key any of the pair's rows can see are skipped (block-lower-triangular
 // skipping at pair granularity); `v.tile_end <= v.tile_begin` then means "nothing to compute here".
-template <int kClipPairMask, int W>
+template <int W>
 __device__ __forceinline__ bool load_segment(const MetaView<W>& meta, const AttnMeta& hdr, int32_t si,
                                              int32_t pair, int32_t tok_per_pair, SegView& v) {
-  // `pair` is the LAST row-tile pair handled by this CTA group (the CTA's own pair for kCG = 1, the
-  // odd pair of the cluster for kCG = 2): both CTAs of a pair must walk the same tile range.
   const Segment s = meta.template load<Segment>(hdr.off_segments + si * (int32_t)(sizeof(Segment) / 4));
   v.g = meta.template load<Group>(hdr.off_groups + s.group * (int32_t)(sizeof(Group) / 4));
   v.tile_begin = s.tile_begin; v.tile_end = s.tile_end; v.part_base = s.part_base; v.group = s.group;
-  if ((pair & ~(int32_t)(kClipPairMask)) >= v.g.npairs) return false;
+  if (pair >= v.g.npairs) return false;
   if (v.g.vis_off >= 0) {
     const int32_t last_tok = min(v.g.q_token_end, v.g.q_token0 + (pair + 1) * tok_per_pair) - 1;
     const int32_t pair_kv = meta[hdr.off_vis + v.g.vis_off + (last_tok - v.g.q_token0)];
@@ -128,7 +116,7 @@ __device__ __forceinline__ bool load_segment(const MetaView<W>& meta, const Attn
 // 2^x for a PAIR of values on the FMA/ALU pipes (no MUFU): round-to-nearest split x = r + f with
 // f in [-0.5, 0.5], a degree-3 minimax polynomial for 2^f (max relative error 7.5e-5, well inside
 // one bf16 ulp of P) in packed f32x2 arithmetic, and an exponent-field add per element.  Used for
-// WS_POLY_PER8 of every 8 exponentials (default 2 = 25 %) to take load off the 16/clk/SM MUFU.
+// kPolyPer8 of every 8 exponentials (2 = 25 %) to take load off the 16/clk/SM MUFU.
 __device__ __forceinline__ void ex2_poly2(uint64_t x2, float& p0, float& p1) {
   float x0, x1;
   unpack_f32x2(x2, x0, x1);
@@ -160,9 +148,9 @@ __device__ __forceinline__ void softmax_chunk(const uint32_t* sr, float c, float
       const float s0 = __uint_as_float(sr[i + e]), s1 = __uint_as_float(sr[i + e + 1]);
       const uint64_t x2 = fma_f32x2(pack_f32x2(s0, s1), c2, nm2);
       const int pr = e / 2;
-      // WS_POLY_PER8 polynomial exponentials per 8 elements, i.e. PER8 / 2 pairs per group of 4 pairs; an
-      // odd PER8 alternates between rounding down and up from one group to the next
-      constexpr int kPolyEven = WS_POLY_PER8 / 2, kPolyOdd = (WS_POLY_PER8 + 1) / 2;
+      // kPolyPer8 polynomial exponentials per 8 elements, i.e. kPolyPer8 / 2 pairs per group of 4 pairs; an
+      // odd count alternates between rounding down and up from one group to the next
+      constexpr int kPolyEven = kPolyPer8 / 2, kPolyOdd = (kPolyPer8 + 1) / 2;
       const int kp = ((i / 8) & 1) ? kPolyOdd : kPolyEven;
       const bool poly = kp > 0 && (pr * kp) / 4 != ((pr + 1) * kp) / 4;
       if (poly) {
@@ -211,27 +199,29 @@ __device__ __forceinline__ void red_release_gpu_add(int32_t* p, int32_t v) {
 
 // kAlt: decode plan (plan.h) - both accumulator sets use Q tile 0; set q processes the KV tiles of the
 // segment with (tile - tile_begin) % 2 == q and writes its own partial (slot part_base + q).
-template <int kCG, int kInlW, bool kAlt>
+//
+// Programmatic dependent launch (protocol: launch.h).  Thread 0 lets the successor's CTAs be scheduled as
+// soon as this CTA is set up; the TMA producer executes griddepcontrol.wait before its first load (q,
+// k_new, v_new may come from the caller's kernel just before; pool pages and page-table entries from an
+// append just before), the append warps before their first store, and every softmax thread before its
+// first global write (out / partials may still be read or written by the previous step's kernels).
+template <int kInlW, bool kAlt>
 __global__ void __launch_bounds__(kThreads, 1)
 attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ CUtensorMap tmap_k,
                   const __grid_constant__ CUtensorMap tmap_v,
-                  const __grid_constant__ InlineMeta<kInlW> inl, const AttnParams p_in) {
-  static_assert(!(kAlt && kCG == 2), "the decode plan runs on single CTAs");
+                  const __grid_constant__ CUtensorMap tmap_kn,
+                  const __grid_constant__ CUtensorMap tmap_vn,
+                  const __grid_constant__ InlineMeta<kInlW> inl,
+                  const __grid_constant__ InlineAppendMeta app, const PeerPools peers, const AttnParams p_in) {
   AttnParams p = p_in;
   const MetaView<kInlW> meta{p.meta, inl};
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem_base;                           // 2 x 32 KB
-  constexpr int kStages = RingCfg<kCG>::kStages;
-  constexpr uint32_t kSlotBytes = RingCfg<kCG>::kSlotBytes;
   const uint32_t sRing = smem_base + 2 * kQTileBytes;      // kStages x kSlotBytes
   Barriers* bars = reinterpret_cast<Barriers*>(smem_raw + (smem_base - smem_u32(smem_raw)) +
                                                2 * kQTileBytes + kRingBytes);
-  // kCG = 2: rank of this CTA in its pair; the even CTA (leader) issues every MMA and owns the
-  // barriers that collect contributions of both CTAs (q_full, kv_full, p_full, o_empty)
-  const uint32_t cta_rank = kCG == 2 ? cluster_ctarank() : 0u;
-  const bool is_leader = cta_rank == 0;
   const uint32_t bq_full = smem_u32(&bars->q_full), bq_empty = smem_u32(&bars->q_empty);
   auto bkv_full = [&](int s) { return smem_u32(&bars->kv_full[s]); };
   auto bkv_empty = [&](int s) { return smem_u32(&bars->kv_empty[s]); };
@@ -243,84 +233,92 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
   const int lane = threadIdx.x & 31;
-  // Compile-time experiment (-DWS_DUAL_ISSUER=1, general plan on single CTAs): one tcgen05.mma issuer warp
-  // PER Q tile (warps 9 and 11) instead of one warp walking q = 0, 1 in turn, so that a wait for one
-  // set's P never delays the other set's MMAs.  The two chains only share read-only K/V tiles; each ring
-  // slot / the Q pair is then released by two commits.  Correct, and no faster (235 vs 233 us per config-4
-  // unit): the tensor pipe's idle ~20 % is the time in which BOTH sets are in their softmax, not issuer
-  // head-of-line blocking.  Off by default.
-  constexpr bool kDual = kCG == 1 && !kAlt && WS_DUAL_ISSUER;
   const AttnMeta hdr = meta.template load<AttnMeta>(0);
   const int32_t team = blockIdx.x / hdr.team_size;
   const int32_t pair = blockIdx.x - team * hdr.team_size;
-  const int32_t clip_pair = kCG == 2 ? (pair | 1) : pair;  // see load_segment
   const int32_t seg_lo = meta[hdr.off_team_seg_begin + team], seg_hi = meta[hdr.off_team_seg_begin + team + 1];
   const int32_t tok_per_pair = kPairRows / p.G;
   const int32_t tok_per_tile = kTileRows / p.G;
-#ifdef WS_PROFILE
-  const long long prof_cta_t0 = clock64();
-  unsigned long long prof_g0; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(prof_g0));
-  if (threadIdx.x < 16) prof_stamps[threadIdx.x] = 0;
-#endif
 
-  // The TMA producer resolves its first segment (and, when that segment starts in tokens no in-flight
-  // append can still be writing, the page ids of its first tile) while the other warps allocate TMEM and
-  // initialise the barriers: takes the metadata and page-table latencies off the path to the first MMA.
+  // The TMA producer resolves its first segment and the page ids of its first tile while the other warps
+  // allocate TMEM and initialise the barriers: takes the metadata and page-table latencies off the path to
+  // the first MMA.
   SegView sv_first;
   int32_t si_first = seg_hi, pre_pg0 = 0, pre_pg1 = 0;
-  bool pre_pages = false;
   if (warp == 8 && lane == 0) {
     prefetch_tmap(&tmap_q); prefetch_tmap(&tmap_k); prefetch_tmap(&tmap_v);
+    if (p.append_tokens > 0) { prefetch_tmap(&tmap_kn); prefetch_tmap(&tmap_vn); }
+    pdl_wait();
     for (si_first = seg_lo; si_first < seg_hi; ++si_first)
-      if (load_segment<kCG - 1>(meta, hdr, si_first, clip_pair, tok_per_pair, sv_first) &&
+      if (load_segment(meta, hdr, si_first, pair, tok_per_pair, sv_first) &&
           sv_first.tile_end > sv_first.tile_begin) break;
-    if (si_first < seg_hi && sv_first.tile_begin + 1 < sv_first.g.dep_tile) {
+    if (si_first < seg_hi && sv_first.tile_begin * kTileKeys < sv_first.g.cache_len) {
       const int32_t* page_row = p.page_table + (int64_t)sv_first.g.slot * p.max_pages_per_session;
-      const int32_t last_page = (sv_first.g.kv_len - 1) / p.P;
+      const int32_t last_page = (sv_first.g.cache_len - 1) / p.P;
       pre_pg0 = page_row[min(2 * sv_first.tile_begin, last_page)];
       pre_pg1 = page_row[min(2 * sv_first.tile_begin + 1, last_page)];
-      pre_pages = true;
     }
   }
   if (warp == 9 && lane == 0) {
-    mbar_init(bq_full, 1); mbar_init(bq_empty, kDual ? 2 : 1); mbar_init(smem_u32(&bars->merge_full), 1);
+    mbar_init(bq_full, 1); mbar_init(bq_empty, 1); mbar_init(smem_u32(&bars->merge_full), 1);
     bars->njobs = 0;
-    for (int s = 0; s < kStages; ++s) { mbar_init(bkv_full(s), 1); mbar_init(bkv_empty(s), kDual ? 2 : 1); }
+    for (int s = 0; s < kStages; ++s) { mbar_init(bkv_full(s), 1); mbar_init(bkv_empty(s), 1); }
     for (int q = 0; q < 2; ++q) {
-      mbar_init(bs_full(q), 1); mbar_init(bp_full(q, 0), 128 * kCG); mbar_init(bp_full(q, 1), 128 * kCG);
+      mbar_init(bs_full(q), 1); mbar_init(bp_full(q, 0), 128); mbar_init(bp_full(q, 1), 128);
       mbar_init(bpv_h0(q), 1);
-      mbar_init(bo_full(q), 1); mbar_init(bo_empty(q), 128 * kCG);
+      mbar_init(bo_full(q), 1); mbar_init(bo_empty(q), 128);
     }
     fence_mbar_init();
   }
-  if (warp == 10) {
-    if constexpr (kCG == 2) { tmem_alloc_2cta<kTmemCols>(smem_u32(&bars->tmem_base)); tmem_relinquish_2cta(); }
-    else { tmem_alloc<kTmemCols>(smem_u32(&bars->tmem_base)); tmem_relinquish(); }
-  }
+  if (warp == 10) { tmem_alloc<kTmemCols>(smem_u32(&bars->tmem_base)); tmem_relinquish(); }
   tc_fence_before();
-  if constexpr (kCG == 2) cluster_sync_all(); else __syncthreads();   // peer barriers are initialised too
+  __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
-  if (threadIdx.x == 0) PROF_STAMP(0)
+  if (threadIdx.x == 0) pdl_launch_dependents();
 
   if (warp >= 8) {
     setmaxnreg_dec<88>();
     if (warp == 8 && lane == 0) {
       // ===================================================== TMA producer
       uint32_t ring_it = 0, q_it = 0;
-      bool dep_waited = false;
       for (int32_t si = si_first; si < seg_hi; ++si) {
         SegView sv;
         if (si == si_first) {
           sv = sv_first;
         } else {
-          if (!load_segment<kCG - 1>(meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
+          if (!load_segment(meta, hdr, si, pair, tok_per_pair, sv)) continue;
           if (sv.tile_end <= sv.tile_begin) continue;        // clipped away for this pair
         }
         const int32_t* page_row = p.page_table + (int64_t)sv.g.slot * p.max_pages_per_session;
-        const int32_t last_page = (sv.g.kv_len - 1) / p.P;
-        // tiles >= dep_tile may still be being written by the preceding append kernel (PDL)
-        if (!dep_waited && sv.tile_begin + 1 >= sv.g.dep_tile) { pdl_wait(); dep_waited = true; }
+        const int32_t last_page = (sv.g.cache_len - 1) / p.P;
+        const int32_t Tc = (sv.g.cache_len + kTileKeys - 1) / kTileKeys;   // tiles >= Tc: the block being committed
+        // one 128-key K or V tile -> the next ring slot: 64-key x 64-dim boxes at offsets 0 (keys 0-63,
+        // dims 0-63), 8 KB (keys 64-127), 16 KB and 24 KB (dims 64-127)
+        auto load_tile = [&](bool is_v, int32_t j, int32_t c0, int32_t c1) {
+          const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
+          mbar_wait(bkv_empty(slot), par ^ 1);
+          mbar_arrive_expect_tx(bkv_full(slot), kSlotBytes);
+          const uint32_t dst = sRing + slot * kSlotBytes;
+          if (j < Tc) {
+            const CUtensorMap* tm = is_v ? &tmap_v : &tmap_k;
+            tma_load_4d(dst, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c0);
+            tma_load_4d(dst + kHalfBytes / 2, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c1);
+            tma_load_4d(dst + kHalfBytes, tm, bkv_full(slot), 64, 0, sv.g.kv_head, c0);
+            tma_load_4d(dst + kHalfBytes + kHalfBytes / 2, tm, bkv_full(slot), 64, 0, sv.g.kv_head, c1);
+          } else {
+            // rows past the end of k_new / v_new are zero-filled by TMA; rows of the next session's
+            // block (batched calls) are finite data; both are masked by the softmax
+            const CUtensorMap* tm = is_v ? &tmap_vn : &tmap_kn;
+            const int32_t tok = sv.g.new_tok0 + (j - Tc) * kTileKeys;
+            tma_load_3d(dst, tm, bkv_full(slot), 0, sv.g.kv_head, tok);
+            tma_load_3d(dst + kHalfBytes / 2, tm, bkv_full(slot), 0, sv.g.kv_head, tok + 64);
+            tma_load_3d(dst + kHalfBytes, tm, bkv_full(slot), 64, sv.g.kv_head, tok);
+            tma_load_3d(dst + kHalfBytes + kHalfBytes / 2, tm, bkv_full(slot), 64, sv.g.kv_head, tok + 64);
+          }
+          ++ring_it;
+        };
+        auto page_of = [&](int32_t logical) { return logical <= 2 * Tc - 1 ? page_row[min(logical, last_page)] : 0; };
         if constexpr (kAlt) {
           // one Q tile serves both accumulator sets
           mbar_wait(bq_empty, (q_it & 1) ^ 1);
@@ -328,112 +326,59 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           for (int h = 0; h < 2; ++h)
             tma_load_3d(sQ + h * kHalfBytes, &tmap_q, bq_full, h * 64, sv.g.kv_head * p.G, sv.g.q_token0);
           ++q_it;
-          auto load_tile = [&](const CUtensorMap* tm, int32_t j) {
-            if (!dep_waited && j >= sv.g.dep_tile) { pdl_wait(); dep_waited = true; }
-            const bool pre = si == si_first && pre_pages && j == sv.tile_begin;   // ids fetched during set-up
-            const int32_t c0 = pre ? pre_pg0 : page_row[min(2 * j, last_page)];
-            const int32_t c1 = pre ? pre_pg1 : page_row[min(2 * j + 1, last_page)];
-            const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
-            mbar_wait(bkv_empty(slot), par ^ 1);
-            mbar_arrive_expect_tx(bkv_full(slot), 32768);
-            const uint32_t dst = sRing + slot * kSlotBytes;
-            tma_load_4d(dst, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c0);
-            tma_load_4d(dst + kHalfBytes / 2, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c1);
-            tma_load_4d(dst + kHalfBytes, tm, bkv_full(slot), 64, 0, sv.g.kv_head, c0);
-            tma_load_4d(dst + kHalfBytes + kHalfBytes / 2, tm, bkv_full(slot), 64, 0, sv.g.kv_head, c1);
-            ++ring_it;
+          auto load_alt = [&](bool is_v, int32_t j) {
+            const bool pre = si == si_first && j == sv.tile_begin;   // ids fetched during set-up
+            load_tile(is_v, j, pre ? pre_pg0 : page_of(2 * j), pre ? pre_pg1 : page_of(2 * j + 1));
           };
           // consumption order of the MMA warp: K0 K1 | V0 K2 | V1 K3 | ...
-          load_tile(&tmap_k, sv.tile_begin);
-          if (sv.tile_begin + 1 < sv.tile_end) load_tile(&tmap_k, sv.tile_begin + 1);
+          load_alt(false, sv.tile_begin);
+          if (sv.tile_begin + 1 < sv.tile_end) load_alt(false, sv.tile_begin + 1);
           for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
-            load_tile(&tmap_v, j);
-            if (j + 2 < sv.tile_end) load_tile(&tmap_k, j + 2);
+            load_alt(true, j);
+            if (j + 2 < sv.tile_end) load_alt(false, j + 2);
           }
           continue;
         }
-        // (the page ids of the first tile are fetched while the Q loads are in flight)
-        // Q pair (own rows).  kCG = 2: the bytes of both CTAs are credited to the leader's q_full.
+        // Q pair (own rows); the page ids of the first tile are fetched while the Q loads are in flight
         mbar_wait(bq_empty, (q_it & 1) ^ 1);
-        if (is_leader) mbar_arrive_expect_tx(bq_full, kCG * 2 * kQTileBytes);
+        mbar_arrive_expect_tx(bq_full, 2 * kQTileBytes);
         const int32_t tok0 = sv.g.q_token0 + pair * tok_per_pair;
         for (int q = 0; q < 2; ++q)
-          for (int h = 0; h < 2; ++h) {
-            if constexpr (kCG == 2)
-              tma_load_3d_2cta(sQ + q * kQTileBytes + h * kHalfBytes, &tmap_q, bq_full, h * 64,
-                               sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
-            else
-              tma_load_3d(sQ + q * kQTileBytes + h * kHalfBytes, &tmap_q, bq_full, h * 64,
-                          sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
-          }
+          for (int h = 0; h < 2; ++h)
+            tma_load_3d(sQ + q * kQTileBytes + h * kHalfBytes, &tmap_q, bq_full, h * 64,
+                        sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
         ++q_it;
         int32_t pg0, pg1;
-        if (si == si_first && pre_pages) {
+        if (si == si_first) {
           pg0 = pre_pg0; pg1 = pre_pg1;
         } else {
-          pg0 = page_row[min(2 * sv.tile_begin, last_page)];
-          pg1 = page_row[min(2 * sv.tile_begin + 1, last_page)];
+          pg0 = page_of(2 * sv.tile_begin); pg1 = page_of(2 * sv.tile_begin + 1);
         }
-        PROF_STAMP(1)
         for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
           const int32_t c0 = pg0, c1 = pg1;
-          if (j + 1 < sv.tile_end) {                        // prefetch next tile's page ids
-            if (!dep_waited && j + 2 >= sv.g.dep_tile) { pdl_wait(); dep_waited = true; }
-            pg0 = page_row[min(2 * j + 2, last_page)];
-            pg1 = page_row[min(2 * j + 3, last_page)];
-          }
-#pragma unroll
-          for (int kv = 0; kv < 2; ++kv) {
-            const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
-            const CUtensorMap* tm = kv == 0 ? &tmap_k : &tmap_v;
-            mbar_wait(bkv_empty(slot), par ^ 1);
-            if (is_leader) mbar_arrive_expect_tx(bkv_full(slot), 32768);   // whole tile (both CTAs)
-            const uint32_t dst = sRing + slot * kSlotBytes;
-            if constexpr (kCG == 2) {
-              if (kv == 0) {
-                // K: this CTA's 64 keys (page `cta_rank` of the tile), both 64-dim halves
-                const int32_t pg = cta_rank ? c1 : c0;
-                tma_load_4d_2cta(dst, tm, bkv_full(slot), 0, 0, sv.g.kv_head, pg);
-                tma_load_4d_2cta(dst + 8192, tm, bkv_full(slot), 64, 0, sv.g.kv_head, pg);
-              } else {
-                // V: all 128 keys, this CTA's 64 dims
-                tma_load_4d_2cta(dst, tm, bkv_full(slot), 64 * (int32_t)cta_rank, 0, sv.g.kv_head, c0);
-                tma_load_4d_2cta(dst + 8192, tm, bkv_full(slot), 64 * (int32_t)cta_rank, 0, sv.g.kv_head, c1);
-              }
-            } else {
-              tma_load_4d(dst, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c0);
-              tma_load_4d(dst + kHalfBytes / 2, tm, bkv_full(slot), 0, 0, sv.g.kv_head, c1);
-              tma_load_4d(dst + kHalfBytes, tm, bkv_full(slot), 64, 0, sv.g.kv_head, c0);
-              tma_load_4d(dst + kHalfBytes + kHalfBytes / 2, tm, bkv_full(slot), 64, 0,
-                          sv.g.kv_head, c1);
-            }
-            ++ring_it;
-          }
+          if (j + 1 < sv.tile_end) { pg0 = page_of(2 * j + 2); pg1 = page_of(2 * j + 3); }   // next tile's ids
+          load_tile(false, j, c0, c1);
+          load_tile(true, j, c0, c1);
         }
       }
-    } else if ((warp == 9 || (kDual && warp == 11)) && is_leader) {
-      // ===================================================== MMA issuer (kCG = 2: the even CTA only)
+    } else if (warp == 9) {
+      // ===================================================== MMA issuer
       // The whole warp runs the control flow convergently (all values stay warp-uniform, so the
       // descriptors are built on the uniform datapath); one elected lane issues tcgen05.mma/commit.
       const bool leader = elect_one();
-      constexpr uint32_t idesc_qk = make_idesc_bf16(128 * kCG, 128, 0, 0);
-      constexpr uint32_t idesc_pv = make_idesc_bf16(128 * kCG, 128, 0, 1);
-      auto commit = [&](uint32_t bar) { if constexpr (kCG == 2) mma_commit_2cta(bar); else mma_commit(bar); };
+      constexpr uint32_t idesc_qk = make_idesc_bf16(128, 128, 0, 0);
+      constexpr uint32_t idesc_pv = make_idesc_bf16(128, 128, 0, 1);
       const uint64_t desc_k = make_smem_desc_sw128(0, 16, 1024);          // K-major operands (Q, K)
       const uint64_t desc_v = make_smem_desc_sw128(0, kHalfBytes, 1024);  // MN-major operand (V)
       uint32_t ring_it = 0, q_it = 0, tile_it = 0, seg_it = 0;
       uint32_t alt_tiles0 = 0, alt_tiles1 = 0, alt_segs0 = 0, alt_segs1 = 0;   // kAlt: per accumulator set
-      const int q_lo = kDual ? (warp == 9 ? 0 : 1) : 0, q_hi = kDual ? q_lo : 1;   // Q tiles this warp issues for
-      PROF_DECL(8)
       auto issue_S = [&](int q, uint32_t slot) {
         const uint64_t da = desc_k + ((sQ + (kAlt ? 0 : q) * kQTileBytes) >> 4);
         const uint64_t db = desc_k + ((sRing + slot * kSlotBytes) >> 4);
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {
-          const uint32_t offa = ((ks >> 2) * kHalfBytes + (ks & 3) * 32) >> 4;
-          const uint32_t offb = ((ks >> 2) * (kHalfBytes / kCG) + (ks & 3) * 32) >> 4;   // kCG = 2: 64-key halves
-          if constexpr (kCG == 2) mma_ss_2cta(tmem_base + q * 128, da + offa, db + offb, idesc_qk, ks > 0);
-          else mma_ss(tmem_base + q * 128, da + offa, db + offb, idesc_qk, ks > 0);
+          const uint32_t off = ((ks >> 2) * kHalfBytes + (ks & 3) * 32) >> 4;
+          mma_ss(tmem_base + q * 128, da + off, db + off, idesc_qk, ks > 0);
         }
       };
       // PV for one of the two pieces in which the softmax hands P over (k-steps of 16 keys)
@@ -442,21 +387,16 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {
           if ((ks < kFirstPieceSteps) != (half == 0)) continue;   // piece 0: keys 0-95, piece 1: keys 96-127
-          if constexpr (kCG == 2)
-            mma_ts_2cta(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8, db + ks * (2048 >> 4),
-                        idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
-          else
-            mma_ts(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8, db + ks * (2048 >> 4),
-                   idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
+          mma_ts(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8, db + ks * (2048 >> 4),
+                 idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
         }
       };
       for (int32_t si = seg_lo; si < seg_hi; ++si) {
         SegView sv;
-        if (!load_segment<kCG - 1>(meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
+        if (!load_segment(meta, hdr, si, pair, tok_per_pair, sv)) continue;
         if (sv.tile_end <= sv.tile_begin) continue;          // clipped away for this pair
         const int32_t nt = sv.tile_end - sv.tile_begin;
         mbar_wait(bq_full, q_it & 1);
-        if (leader) PROF_STAMP(2)
         if constexpr (kAlt) {
           // S_q <- Q K(tile q) for q = 0, 1; then per tile j (set q = j & 1): O_q += P V(j), S_q <- Q K(j+2)
           for (int q = 0; q < 2 && q < nt; ++q) {
@@ -464,8 +404,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             mbar_wait(bkv_full(slot), par);
             tc_fence_after();
             if (leader) {
-              issue_S(q, slot); commit(bs_full(q)); commit(bkv_empty(slot));
-              if (q + 1 == nt || (q == 1 && nt == 2)) commit(bq_empty);
+              issue_S(q, slot); mma_commit(bs_full(q)); mma_commit(bkv_empty(slot));
+              if (q + 1 == nt || (q == 1 && nt == 2)) mma_commit(bq_empty);
             }
             __syncwarp();
             ++ring_it;
@@ -482,22 +422,22 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             mbar_wait(bp_full(q, 0), tq & 1);
             if (j < 2) mbar_wait(bo_empty(q), (sq & 1) ^ 1);
             tc_fence_after();
-            if (leader) { issue_PV(q, slot_v, 0, j >= 2); commit(bpv_h0(q)); }
+            if (leader) { issue_PV(q, slot_v, 0, j >= 2); mma_commit(bpv_h0(q)); }
             __syncwarp();
             mbar_wait(bp_full(q, 1), tq & 1);
             tc_fence_after();
             if (leader) {
               issue_PV(q, slot_v, 1, true);
-              if (!have_next) commit(bo_full(q));
-              commit(bkv_empty(slot_v));
+              if (!have_next) mma_commit(bo_full(q));
+              mma_commit(bkv_empty(slot_v));
             }
             __syncwarp();
             if (have_next) {
               mbar_wait(bkv_full(slot_k), par_k);
               tc_fence_after();
               if (leader) {
-                issue_S(q, slot_k); commit(bs_full(q)); commit(bkv_empty(slot_k));
-                if (j + 3 == nt) commit(bq_empty);
+                issue_S(q, slot_k); mma_commit(bs_full(q)); mma_commit(bkv_empty(slot_k));
+                if (j + 3 == nt) mma_commit(bq_empty);
               }
               __syncwarp();
             }
@@ -512,11 +452,10 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
           mbar_wait(bkv_full(slot), par);
           tc_fence_after();
-          if (leader) PROF_STAMP(3)
           if (leader) {
-            for (int q = q_lo; q <= q_hi; ++q) { issue_S(q, slot); commit(bs_full(q)); }
-            commit(bkv_empty(slot));
-            if (nt == 1) commit(bq_empty);
+            for (int q = 0; q < 2; ++q) { issue_S(q, slot); mma_commit(bs_full(q)); }
+            mma_commit(bkv_empty(slot));
+            if (nt == 1) mma_commit(bq_empty);
           }
           __syncwarp();
           ++ring_it;
@@ -527,43 +466,37 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           const bool have_next = j + 1 < nt;
           uint32_t slot_k = 0, par_k = 0;
           if (have_next) { slot_k = ring_it % kStages; par_k = (ring_it / kStages) & 1; ++ring_it; }
-          PROF_MARK(0)
           mbar_wait(bkv_full(slot_v), par_v);
-          PROF_MARK(1)
-          for (int q = q_lo; q <= q_hi; ++q) {
+          for (int q = 0; q < 2; ++q) {
             mbar_wait(bp_full(q, 0), tile_it & 1);
-            PROF_MARK(2 + (q & 1))
             if (j == 0) mbar_wait(bo_empty(q), (seg_it & 1) ^ 1);
             tc_fence_after();
             if (leader) {
               issue_PV(q, slot_v, 0, j > 0);
-              commit(bpv_h0(q));
+              mma_commit(bpv_h0(q));
             }
             __syncwarp();
             mbar_wait(bp_full(q, 1), tile_it & 1);
             tc_fence_after();
             if (leader) {
               issue_PV(q, slot_v, 1, true);
-              if (!have_next) commit(bo_full(q));
+              if (!have_next) mma_commit(bo_full(q));
             }
             __syncwarp();
-            PROF_MARK(5)
             if (have_next) {
-              if (q == q_lo) { mbar_wait(bkv_full(slot_k), par_k); tc_fence_after(); }
-              PROF_MARK(4)
+              if (q == 0) { mbar_wait(bkv_full(slot_k), par_k); tc_fence_after(); }
               if (leader) {
                 issue_S(q, slot_k);
-                commit(bs_full(q));
+                mma_commit(bs_full(q));
               }
               __syncwarp();
-              PROF_MARK(6)
             }
           }
           if (leader) {
-            commit(bkv_empty(slot_v));
+            mma_commit(bkv_empty(slot_v));
             if (have_next) {
-              commit(bkv_empty(slot_k));
-              if (j + 2 == nt) commit(bq_empty);
+              mma_commit(bkv_empty(slot_k));
+              if (j + 2 == nt) mma_commit(bq_empty);
             }
           }
           __syncwarp();
@@ -571,9 +504,20 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         }
         ++q_it; ++seg_it;
       }
-#ifdef WS_PROFILE
-      if (blockIdx.x == 5 && lane == 0) printf("MMA  misc %lld waitV %lld waitP0 %lld waitP1 %lld waitK %lld issuePV %lld issueS %lld tiles %u\n", prof_acc[0], prof_acc[1], prof_acc[2], prof_acc[3], prof_acc[4], prof_acc[5], prof_acc[6], tile_it);
-#endif
+    }
+    if (warp >= 10 && p.append_tokens > 0) {
+      // ===================================================== a2 inside the fused step (kv_append.cuh)
+      // The pool rows and page-table entries written here are not read by this launch (its KV tiles over
+      // the new block come from k_new / v_new); at most the masked tail of a session's last cache page is
+      // overwritten while a tile holding it is in flight, which changes nothing: those keys carry P = 0
+      // and the bytes are finite before and after.
+      pdl_wait();
+      const AppendGeom geom{reinterpret_cast<const int4*>(p.k_new), reinterpret_cast<const int4*>(p.v_new),
+                            reinterpret_cast<int4*>(p.k_pool_w), reinterpret_cast<int4*>(p.v_pool_w),
+                            p.page_table_w, p.max_pages_per_session, p.P, p.Hkv, p.D * 2 / 16};
+      const MetaView<kInlineAppendWords> ameta{nullptr, app};
+      append_work(ameta, geom, peers, ((int64_t)blockIdx.x * 2 + (warp - 10)) * 32 + lane, (int64_t)gridDim.x * 64,
+                  (blockIdx.x == 0 && warp == 10) ? lane : -1, 32);
     }
   } else {
     // ======================================================= softmax warpgroups (warps 0-7)
@@ -585,14 +529,9 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t t_s = tmem_base + (lane_base << 16) + q * 128;
     const uint32_t t_o = tmem_base + (lane_base << 16) + 256 + q * 128;
     const float c = p.scale * 1.4426950408889634f;
-    // p_full / o_empty live in the leader CTA (kCG = 2): arrive through the cluster address
-    auto arrive_leader = [&](uint32_t bar) {
-      if constexpr (kCG == 2) mbar_arrive_cluster(bar & kPeerBitMask); else mbar_arrive(bar);
-    };
     uint32_t tile_it = 0, seg_it = 0, alt_sync_it = 0;
     bool pdl_done = false;
-    PROF_DECL(8)
-    const bool fused = kCG == 1 && p.merge_ctr != nullptr;
+    const bool fused = p.merge_ctr != nullptr;
     // publish this warpgroup's half of a partial: every thread's stores are fenced, the warpgroup
     // meets on a named barrier, one thread bumps the arrival counter of the (item, pair) - keyed by
     // the item's first partial slot, found from the group id (at most one combine item per group)
@@ -626,7 +565,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 
     for (int32_t si = seg_lo; si < seg_hi; ++si) {
       SegView sv;
-      if (!load_segment<kCG - 1>(meta, hdr, si, clip_pair, tok_per_pair, sv)) continue;
+      if (!load_segment(meta, hdr, si, pair, tok_per_pair, sv)) continue;
       // kAlt: this warpgroup takes tiles tile_begin + q, + q + 2, ...
       const int32_t nt = kAlt ? (sv.tile_end > sv.tile_begin ? (sv.tile_end - sv.tile_begin + 1 - q) / 2 : 0)
                               : sv.tile_end - sv.tile_begin;
@@ -640,7 +579,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         bars->cur_slot0 = job.slot0;
       }
       const int32_t tok = sv.g.q_token0 + pair * tok_per_pair + R / p.G;
-      const bool row_valid = tok < sv.g.q_token_end && pair < sv.g.npairs;   // (kCG = 2: a ghost CTA computes but stores nothing)
+      const bool row_valid = tok < sv.g.q_token_end;
       if (sv.tile_end <= sv.tile_begin) {
         // every tile of this segment lies beyond what the pair can see: publish an empty partial
         // (the segment is one of several splits, otherwise it would start at tile 0)
@@ -653,29 +592,31 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const int32_t head = sv.g.kv_head * p.G + R % p.G;
       int32_t vis = sv.g.kv_len;
       if (sv.g.vis_off >= 0 && row_valid) vis = meta[hdr.off_vis + sv.g.vis_off + (tok - sv.g.q_token0)];
+      // keys of tile t: [key0, key0 + 128) of the pool part (t < Tc, ends at cache_len) or of the block
+      // being committed (t >= Tc, starts at cache_len, ends at kv_len); a row sees keys below vis
+      const int32_t Tc = (sv.g.cache_len + kTileKeys - 1) / kTileKeys;
+      const int32_t vis_cache = min(vis, sv.g.cache_len);
       float m_used = -INFINITY, l = 0.f;
 
       for (int32_t j = 0; j < nt; ++j) {
-        const int32_t key0 = (sv.tile_begin + (kAlt ? 2 * j + q : j)) * kTileKeys;
-        PROF_MARK(0)
+        const int32_t t = sv.tile_begin + (kAlt ? 2 * j + q : j);
+        const int32_t key0 = t < Tc ? t * kTileKeys : sv.g.cache_len + (t - Tc) * kTileKeys;
+        const int32_t lim = t < Tc ? vis_cache : vis;        // keys >= lim of this tile are masked
         mbar_wait(bs_full(q), tile_it & 1);
         tc_fence_after();
-        if (threadIdx.x == 0) PROF_STAMP(4)
-        PROF_MARK(1)
         uint32_t pk[64];                                    // P row, packed bf16x2
-        const bool need_mask = __any_sync(0xffffffffu, key0 + kTileKeys > vis);
+        const bool need_mask = __any_sync(0xffffffffu, key0 + kTileKeys > lim);
         bool done = false;
         // (rows whose reference is still -inf, i.e. nothing visible so far, also take the exact path)
-        if (WS_FAST_PATH && j > 0 && !need_mask && !__any_sync(0xffffffffu, m_used == -INFINITY)) {
+        if (j > 0 && !need_mask && !__any_sync(0xffffffffu, m_used == -INFINITY)) {
           // ---- fast path (optimistic): exponentiate against the running reference m_used while
           // the tile streams out of TMEM in 32-column chunks.  Each piece (keys 0-95, keys 96-127) is
-          // checked for scores that outgrew the reference - every p is <= the piece's row sum, so a sum
-          // below kFastSumLimit proves none did (a NaN/inf sum fails the test) - and handed to the MMA
-          // warp as soon as it is written: PV of the first piece (384 tensor cycles) overlaps the softmax
-          // of the last 32 keys, and only 128 cycles of PV remain on the S -> softmax -> PV -> S chain.
-          // (ncu: 2541 instead of 2611 cycles per tile pair with a 64/64 split; the power-capped live time
-          // per config-4 unit did not move.)
+          // checked against the two limits described at kFastSumLimit / kFastSumShare (a NaN/inf sum
+          // fails the test) and handed to the MMA warp as soon as it is written: PV of the first piece
+          // (384 tensor cycles) overlaps the softmax of the last 32 keys, and only 128 cycles of PV
+          // remain on the S -> softmax -> PV -> S chain.
           const float neg_mc = -m_used;
+          const float sum_lim = fminf(kFastSumLimit, kFastSumShare * l);
           uint64_t l01 = 0, l23 = 0;                        // packed fp32x2 partial row sums
           uint32_t sa[32], sb[32];
           tmem_ld32(t_s + 0, sa);
@@ -691,25 +632,25 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           float la, lb;
           unpack_f32x2(add_f32x2(l01, l23), la, lb);
           const float sum_a = la + lb;
-          if (!__any_sync(0xffffffffu, !(sum_a < kFastSumLimit))) {
+          if (!__any_sync(0xffffffffu, !(sum_a < sum_lim))) {
             tmem_st32(t_s + 0, pk);
             tmem_st16(t_s + 32, pk + 32);
             tmem_wait_st();
             tc_fence_before();
-            arrive_leader(bp_full(q, 0));                     // first 96 keys of P handed off
+            mbar_arrive(bp_full(q, 0));                     // first 96 keys of P handed off
             tmem_wait_ld();
             l01 = 0; l23 = 0;
             softmax_chunk(sb, c, neg_mc, l01, l23, pk + 48);
             unpack_f32x2(add_f32x2(l01, l23), la, lb);
             const float sum_b = la + lb;
             l += sum_a;
-            if (!__any_sync(0xffffffffu, !(sum_b < kFastSumLimit))) {
+            if (!__any_sync(0xffffffffu, !(sum_b < sum_lim))) {
               l += sum_b;
             } else {
-              // Rare: a score among the last 32 keys outgrew the reference after the first piece was
-              // handed off.  Wait until PV of the first piece has completed (O is then quiescent:
-              // the PV of the last piece needs our arrival), rescale O and l to the new reference and
-              // redo the last 32 keys exactly.
+              // Rare: the last 32 keys fail the test after the first piece was handed off.  Wait until
+              // PV of the first piece has completed (O is then quiescent: the PV of the last piece needs
+              // our arrival), re-reference O and l to the exact maximum if it grew and redo the last 32
+              // keys exactly.
               mbar_wait(bpv_h0(q), tile_it & 1);
               tc_fence_after();
               uint32_t sr[32];
@@ -720,7 +661,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
               for (int i = 1; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sr[i]));
               const float tm = mx * c;
               float alpha = 1.f;
-              if (tm > m_used + kRescaleThreshold) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
+              if (tm > m_used) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
 #pragma unroll
               for (int ch = 0; ch < 4; ++ch) {
                 uint32_t o[32];
@@ -743,25 +684,24 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             tmem_st16(t_s + 48, pk + 48);
             tmem_wait_st();
             tc_fence_before();
-            arrive_leader(bp_full(q, 1));
+            mbar_arrive(bp_full(q, 1));
             done = true;
           }
         }
         if (!done) {
-          // ---- exact path: first tile of a segment, masked tiles, or a first-half row max that
-          // outgrew the reference (nothing has been handed off yet in that case)
+          // ---- exact path: first tile of a segment, masked tiles, tiles that may carry a large share of
+          // the row's weight (nothing has been handed off yet in that case)
           uint32_t sr[128];                                 // one whole S row (fp32 bits)
           tmem_ld32(t_s + 0, sr + 0);
           tmem_ld32(t_s + 32, sr + 32);
           tmem_ld32(t_s + 64, sr + 64);
           tmem_ld32(t_s + 96, sr + 96);
           tmem_wait_ld();
-          PROF_MARK(2)
 #define S_(i) __uint_as_float(sr[i])
           if (need_mask) {
 #pragma unroll
             for (int i = 0; i < 128; ++i)
-              if (key0 + i >= vis) sr[i] = 0xff800000u;     // -inf
+              if (key0 + i >= lim) sr[i] = 0xff800000u;     // -inf
           }
           float mx0 = S_(0), mx1 = S_(1), mx2 = S_(2), mx3 = S_(3);
 #pragma unroll
@@ -770,12 +710,14 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             mx2 = fmaxf(mx2, S_(i + 2)); mx3 = fmaxf(mx3, S_(i + 3));
           }
           const float tm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;
-          const bool grow = tm > m_used + kRescaleThreshold;
+          // the reference follows the exact running maximum on this path: the row's largest weight so
+          // far is then p = 1, exactly representable in bf16
+          const bool grow = tm > m_used;
           if (j == 0) {
             m_used = tm;
           } else if (__any_sync(0xffffffffu, grow)) {
-            // lazy rescale of O and l (PV of the previous tile has completed: s_full was committed
-            // after it on the same in-order tensor pipe)
+            // rescale O and l (PV of the previous tile has completed: s_full was committed after it on
+            // the same in-order tensor pipe)
             float alpha = 1.f;
             if (grow) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
 #pragma unroll
@@ -790,7 +732,6 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           }
           const float m_c = (m_used == -INFINITY) ? 0.f : m_used;
           float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
-          PROF_MARK(3)
 #pragma unroll
           for (int i = 0; i < 128; i += 4) {
             const float p0 = ex2_approx(fmaf(S_(i), c, -m_c));
@@ -802,31 +743,27 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             pk[i / 2 + 1] = pack_bf16x2(p2, p3);
           }
           l += (l0 + l1) + (l2 + l3);
-          PROF_MARK(4)
 #undef S_
           tmem_st32(t_s + 0, pk);
           tmem_st32(t_s + 32, pk + 32);
-          // (keys beyond the cache end in a ragged last tile: P is exactly 0 there and the append
-          // kernel keeps the unused tail of the last page zeroed, so 0 x V stays 0)
+          // (masked keys: P is exactly 0 there and the bytes behind them are finite - the append keeps the
+          // unused tail of a session's last page zeroed, rows past the end of k_new are zero-filled - so
+          // 0 x V stays 0)
           tmem_wait_st();
           tc_fence_before();
-          arrive_leader(bp_full(q, 0));
-          arrive_leader(bp_full(q, 1));
+          mbar_arrive(bp_full(q, 0));
+          mbar_arrive(bp_full(q, 1));
         }
-        PROF_MARK(5)
         ++tile_it;
       }
       // ---------------------------------------------------- epilogue
       // first global write of this CTA: the predecessor grids (append; transitively the previous
       // step's combine, which reads the partial buffers and writes `out`) must have completed
-      if (threadIdx.x == 0) PROF_STAMP(5)
       if (!pdl_done) { pdl_wait(); pdl_done = true; }
-      if (threadIdx.x == 0) PROF_STAMP(6)
       if (nt > 0) {
         mbar_wait(bo_full(q), seg_it & 1);
         tc_fence_after();
       }
-      if (threadIdx.x == 0) PROF_STAMP(7)
       float inv_l = l > 0.f ? 1.f / l : 0.f;                // coefficient of this set's accumulator
       float lse2 = l > 0.f ? m_used + log2f(l) : -INFINITY;
       float inv_l1 = 0.f;                                   // kAlt: coefficient of accumulator set 1
@@ -904,15 +841,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         // once o_full(0) fired) or the K/V ring (set 1 / decode plan: every MMA has completed), so the
         // warp stages its 32 rows x 512 B there and writes them with ONE 16 KB bulk store; rows are
         // contiguous in the partial buffer.  Otherwise: direct 16-byte stores (same chunk positions).
-        const bool staged = kCG == 1 && si + 1 == seg_hi && __all_sync(0xffffffffu, row_valid);   // (few valid rows, e.g. decode steps: store just those)
+        const bool staged = si + 1 == seg_hi && __all_sync(0xffffffffu, row_valid);   // (few valid rows, e.g. decode steps: store just those)
         const uint32_t stage = ((kAlt || q == 1) ? sRing : sQ) + (uint32_t)(warp & 3) * 16384u + (uint32_t)lane * 512u;
-        if (kDual && si + 1 == seg_hi) {
-          // Two issuer warps: o_full(q) only covers the MMAs of this set's issuer, but set 0 stages over BOTH
-          // Q tiles (set 1's last S MMA may still be reading the second) and set 1 over ring slots (set 0's
-          // last PV may still be reading V).  Both warpgroups meet here, each after its own o_full: every
-          // MMA of the CTA has then completed.  (Last segment only; the sets run within a tile of each other.)
-          asm volatile("bar.sync 4, 256;" ::: "memory");
-        }
 #pragma unroll
         for (int ch = 0; ch < 4; ++ch) {
           uint32_t o[32];
@@ -948,7 +878,6 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           bars->lse_stage[R] = lse2;
           fence_proxy_async_smem();
           __syncwarp();
-          if (threadIdx.x == 0) PROF_STAMP(13)
           if (lane == 0) {
             bulk_store(p.part_o + (prow - lane) * p.D, stage - (uint32_t)lane * 512u, 16384u);
             bulk_store(p.part_lse + (prow - lane), smem_u32(&bars->lse_stage[R - lane]), 128u);
@@ -961,14 +890,11 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         pub = true; pub_fence = !staged;
       }
       tc_fence_before();
-      arrive_leader(bo_empty(q));
+      mbar_arrive(bo_empty(q));
       if constexpr (kAlt) { if (use1) mbar_arrive(bo_empty(1)); }
       if (pub) publish(pub_fence);
-      if (threadIdx.x == 0) PROF_STAMP(8)
-      PROF_MARK(6)
       ++seg_it;
     }
-    if (threadIdx.x == 0) PROF_STAMP(9)
     if (fused && hdr.num_combine > 0) {
       // ---------------------------------------------------- merge phase (a4)
       uint32_t merge_phase = 0;
@@ -982,7 +908,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         } else {
           // more partial segments than parked jobs (many tiny groups per team): re-derive from the metadata
           SegView sv;
-          if (!load_segment<kCG - 1>(meta, hdr, si, clip_pair, tok_per_pair, sv) || sv.part_base < 0) continue;
+          if (!load_segment(meta, hdr, si, pair, tok_per_pair, sv) || sv.part_base < 0) continue;
           make_job(sv, job);
         }
         ++jn;
@@ -993,11 +919,9 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           (void)ld_acquire_gpu(ctr);
         }
         __syncwarp();
-        if (threadIdx.x == 0) PROF_STAMP(11)
         merge_item(p, job, (int32_t)(kRingBytes / 512), sRing, smem_raw + (sRing - smem_u32(smem_raw)), sQ,
                    smem_raw + (sQ - smem_u32(smem_raw)), smem_u32(&bars->merge_full), merge_phase, warp, lane);
         __syncwarp();
-        if (threadIdx.x == 0) PROF_STAMP(12)
         if (warp == 0 && lane == 0) {
           // the last CTA to get here re-arms the counters for the next launch (every part has been
           // published and every waiter has passed its wait by then)
@@ -1006,46 +930,21 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         }
       }
     }
-    if (threadIdx.x == 0) PROF_STAMP(10)
-#ifdef WS_PROFILE
-    if (blockIdx.x == 5 && lane == 0 && (warp & 3) == 0) printf("SMX%d other %lld waitS %lld ld %lld max %lld exp %lld store %lld epi %lld tiles %u\n", q, prof_acc[0], prof_acc[1], prof_acc[2], prof_acc[3], prof_acc[4], prof_acc[5], prof_acc[6], tile_it);
-#endif
   }
 
-  __syncwarp();
-  pdl_launch_dependents();
   tc_fence_before();
-  if constexpr (kCG == 2) cluster_sync_all(); else __syncthreads();   // the leader's MMAs read the peer's smem / TMEM
-#ifdef WS_PROFILE
-  if (threadIdx.x == 0) {
-    unsigned long long g1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(g1));
-    int tiles = 0; for (int si = seg_lo; si < seg_hi; ++si) { const Segment sg = meta.template load<Segment>(hdr.off_segments + si * 4); tiles += sg.tile_end - sg.tile_begin; }
-    unsigned smid; asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
-    // one line per CTA: ns since the CTA started (globaltimer) at which thread 0 / the producer / the MMA warp
-    // passed each point (first segment / first merge job only; -1 = never).  A single printf: lines of
-    // different CTAs must not interleave.
-#define PS_(i) (prof_stamps[i] ? (long long)(prof_stamps[i] - prof_g0) : -1ll)
-    printf("CTA %d sm %u segs %d tiles %d cycles %lld t0 %llu dur %llu | setup %lld qissued %lld qfull %lld k0full %lld "
-           "s0full %lld lasttile %lld pdlwait %lld ofull %lld stored %lld segsdone %lld merged %lld mwaited %lld mitem %lld "
-           "staged %lld missued %lld mloaded %lld\n", blockIdx.x, smid, seg_hi - seg_lo, tiles, clock64() - prof_cta_t0,
-           prof_g0, g1 - prof_g0, PS_(0), PS_(1), PS_(2), PS_(3), PS_(4), PS_(5), PS_(6), PS_(7), PS_(8), PS_(9), PS_(10),
-           PS_(11), PS_(12), PS_(13), PS_(14), PS_(15));
-#undef PS_
-  }
-#endif
+  __syncthreads();
   if (warp == 10) {
     tc_fence_after();
-    if constexpr (kCG == 2) tmem_dealloc_2cta<kTmemCols>(tmem_base); else tmem_dealloc<kTmemCols>(tmem_base);
+    tmem_dealloc<kTmemCols>(tmem_base);
   }
 }
 
 cudaError_t sm100_attn_configure() {
-  const void* fns[6] = {(const void*)attn_sm100_kernel<1, kInlineAttnWords, false>,
-                        (const void*)attn_sm100_kernel<2, kInlineAttnWords, false>,
-                        (const void*)attn_sm100_kernel<1, kInlineAttnWordsLarge, false>,
-                        (const void*)attn_sm100_kernel<2, kInlineAttnWordsLarge, false>,
-                        (const void*)attn_sm100_kernel<1, kInlineAttnWords, true>,
-                        (const void*)attn_sm100_kernel<1, kInlineAttnWordsLarge, true>};
+  const void* fns[4] = {(const void*)attn_sm100_kernel<kInlineAttnWords, false>,
+                        (const void*)attn_sm100_kernel<kInlineAttnWordsLarge, false>,
+                        (const void*)attn_sm100_kernel<kInlineAttnWords, true>,
+                        (const void*)attn_sm100_kernel<kInlineAttnWordsLarge, true>};
   for (const void* f : fns) {
     cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
     if (e != cudaSuccess) return e;
@@ -1057,7 +956,7 @@ cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3(l.num_ctas); cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = kSmemBytes; cfg.stream = stream;
-  cudaLaunchAttribute at[3];
+  cudaLaunchAttribute at[2];
   int na = 0;
   if (l.p.merge_ctr != nullptr) {
     // fused combine: CTAs wait on each other's partials, so the whole grid must be co-resident
@@ -1065,33 +964,24 @@ cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream) {
     at[na].val.cooperative = 1;
     ++na;
   }
-  static const bool no_pdl = getenv("WS_NO_PDL") != nullptr;
-  if (!no_pdl) {
-    at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[na].val.programmaticStreamSerializationAllowed = 1;
-    ++na;
-  }
-  const bool pairs = l.cta_group == 2 && !l.alt;
-  if (pairs) {
-    at[na].id = cudaLaunchAttributeClusterDimension;
-    at[na].val.clusterDim.x = 2; at[na].val.clusterDim.y = 1; at[na].val.clusterDim.z = 1;
-    ++na;
-  }
+  at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[na].val.programmaticStreamSerializationAllowed = 1;
+  ++na;
   cfg.attrs = at; cfg.numAttrs = na;
   if (l.inl_words <= kInlineAttnWords) {
     InlineAttnMeta small;
     memcpy(small.w, l.inl.w, sizeof(small.w));
     if (l.alt)
-      return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWords, true>, l.tmap_q, l.tmap_k, l.tmap_v, small, l.p);
-    if (pairs)
-      return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<2, kInlineAttnWords, false>, l.tmap_q, l.tmap_k, l.tmap_v, small, l.p);
-    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWords, false>, l.tmap_q, l.tmap_k, l.tmap_v, small, l.p);
+      return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<kInlineAttnWords, true>, l.tmap_q, l.tmap_k, l.tmap_v,
+                                l.tmap_kn, l.tmap_vn, small, l.app, l.peers, l.p);
+    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<kInlineAttnWords, false>, l.tmap_q, l.tmap_k, l.tmap_v,
+                              l.tmap_kn, l.tmap_vn, small, l.app, l.peers, l.p);
   }
   if (l.alt)
-    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWordsLarge, true>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
-  if (pairs)
-    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<2, kInlineAttnWordsLarge, false>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
-  return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<1, kInlineAttnWordsLarge, false>, l.tmap_q, l.tmap_k, l.tmap_v, l.inl, l.p);
+    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<kInlineAttnWordsLarge, true>, l.tmap_q, l.tmap_k, l.tmap_v,
+                              l.tmap_kn, l.tmap_vn, l.inl, l.app, l.peers, l.p);
+  return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<kInlineAttnWordsLarge, false>, l.tmap_q, l.tmap_k, l.tmap_v,
+                            l.tmap_kn, l.tmap_vn, l.inl, l.app, l.peers, l.p);
 }
 
 }  // namespace ws

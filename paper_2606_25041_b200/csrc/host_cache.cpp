@@ -67,7 +67,6 @@ bool HostCache::truncate_blocks(int32_t s, int32_t keep_blocks) {
   if (keep_blocks < 0 || keep_blocks > (int32_t)st.block_ends.size()) return false;
   st.block_ends.resize(keep_blocks);
   st.tokens = keep_blocks ? st.block_ends.back() : 0;
-  st.stable_tokens = std::min(st.stable_tokens, st.tokens);
   size_t keep_pages = (size_t)((st.tokens + P_ - 1) / P_);
   while (st.pages.size() > keep_pages) {
     release_page(st.pages.back());

@@ -12,7 +12,6 @@ namespace ws {
 struct SessionState {
   bool open = false;
   int64_t tokens = 0;
-  int64_t stable_tokens = 0;         // tokens whose append kernels are known complete (see api.cu)
   std::vector<int32_t> pages;        // physical page ids, logical page i -> pages[i]
   std::vector<int64_t> block_ends;   // e_1 < ... < e_B
   std::vector<uint8_t> modality;     // per committed token (optional metadata, may be shorter)
@@ -49,7 +48,6 @@ class HostCache {
   // whose lengths are given.  The caller has validated everything (strong guarantee lives in api.cu).
   void adopt(int32_t s, const int32_t* block_lens, int32_t nblocks, const int32_t* pages, int32_t npages);
 
-  void mark_all_stable() { for (auto& s : sess_) if (s.open) s.stable_tokens = s.tokens; }
   int32_t free_pages() const { return (int32_t)free_.size(); }
   void shuffle_free(uint64_t seed);
   int32_t page_tokens() const { return P_; }

@@ -5,93 +5,33 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "kv_append.cuh"
 #include "launch.h"
 #include "ws_internal.h"
 
 namespace ws {
 
-// One thread moves one 16-byte chunk of K and the matching chunk of V.
-// chunks_per_token = Hkv * D * eb / 16; chunks_per_head = D * eb / 16.
+// ws_kv_append's own launch: one thread per 16-byte chunk of K (and the matching chunk of V), device code
+// in kv_append.cuh.  chunks_per_token = Hkv * D * eb / 16; chunks_per_head = D * eb / 16.
+//
+// Programmatic dependent launch (launch.h): the kernel may start while its stream predecessor is still
+// running, so it waits for that grid (griddepcontrol.wait: complete and flushed) BEFORE its first access -
+// k_new / v_new may have been produced by the predecessor, and the pool rows / page-table entries it
+// writes may still be being read by it (an attention kernel over a session that was rolled back and is
+// re-appended at the same positions).  Only then does it let its own successor start early; the successor's
+// own wait covers this grid.
 __global__ void __launch_bounds__(256)
 kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
                  int4* __restrict__ k_pool, int4* __restrict__ v_pool,
                  int32_t* __restrict__ page_table, const int32_t* __restrict__ meta_g,
                  const __grid_constant__ InlineAppendMeta inl, const PeerPools peers,
                  int32_t max_pages, int32_t P, int32_t Hkv, int32_t chunks_per_head) {
-  // Nothing this kernel touches is produced by its stream predecessor (the previous step's combine
-  // writes only `out`), so the successor (this step's attention) may start its prologue right away.
+  pdl_wait();
   pdl_launch_dependents();
   const MetaView<kInlineAppendWords> meta{meta_g, inl};    // (constant-bank reads when the blob is inline)
-  const AppendMeta hdr = meta.load<AppendMeta>(0);
-  constexpr int32_t kSessWords = (int32_t)(sizeof(AppendSession) / 4);
-  auto sess = [&](int32_t s) { return meta.load<AppendSession>(hdr.off_sessions + s * kSessWords); };
-  auto sess_tok_end = [&](int32_t s) { return meta[hdr.off_sessions + s * kSessWords + 3]; };
-  auto pages = [&](int32_t i) { return meta[hdr.off_pages + i]; };
-  const int32_t chunks_per_token = Hkv * chunks_per_head;
-  const int64_t total = (int64_t)hdr.total_tokens * chunks_per_token;
-
-  // Block 0 also publishes the page ids into the persistent device page table (idempotent).
-  if (blockIdx.x == 0) {
-    for (int32_t s = 0; s < hdr.num_sessions; ++s) {
-      const AppendSession a = sess(s);
-      int32_t first = a.len_old / P;
-      int32_t last = (a.len_old + (a.tok_end - a.tok_begin) + P - 1) / P;
-      for (int32_t i = first + threadIdx.x; i < last; i += blockDim.x)
-        page_table[(int64_t)a.slot * max_pages + i] = pages(a.page_off + (i - first));
-    }
-  }
-  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
-       idx += (int64_t)gridDim.x * blockDim.x) {
-    int32_t tok = (int32_t)(idx / chunks_per_token);
-    int32_t c = (int32_t)(idx - (int64_t)tok * chunks_per_token);
-    // session of this token: binary search over tok_end
-    int32_t lo = 0, hi = hdr.num_sessions - 1;
-    while (lo < hi) {
-      int32_t mid = (lo + hi) >> 1;
-      if (tok >= sess_tok_end(mid)) lo = mid + 1; else hi = mid;
-    }
-    const AppendSession a = sess(lo);
-    int32_t pos = a.len_old + (tok - a.tok_begin);
-    int32_t page = pages(a.page_off + (pos / P - a.len_old / P));
-    int32_t head = c / chunks_per_head;
-    int32_t off = c - head * chunks_per_head;
-    int64_t dst = (((int64_t)page * Hkv + head) * P + (pos % P)) * chunks_per_head + off;
-    const int4 kx = k_new[idx], vx = v_new[idx];
-    k_pool[dst] = kx;
-    v_pool[dst] = vx;
-    // NEXT-3: the same slice goes to every linked replica pool at the same page id -
-    // plain stores through the peer mapping (NVLink), no second read of the slice.
-    for (int32_t r = 0; r < peers.n; ++r) { ((int4*)peers.k[r])[dst] = kx; ((int4*)peers.v[r])[dst] = vx; }
-  }
-  // Zero the unused tail of each session's last page: slots beyond the committed length are then
-  // always finite (zero), so the attention kernel may load whole pages and rely on P = 0 for the
-  // masked keys (0 x stale NaN bits would poison O).  At most P - 1 token rows per session.
-  {
-    const int4 zero = make_int4(0, 0, 0, 0);
-    for (int32_t s = 0; s < hdr.num_sessions; ++s) {
-      const AppendSession a = sess(s);
-      const int32_t len_new = a.len_old + (a.tok_end - a.tok_begin);
-      const int32_t tail = (P - len_new % P) % P;
-      if (tail == 0) continue;
-      const int32_t page = pages(a.page_off + ((len_new - 1) / P - a.len_old / P));
-      const int64_t total_tail = (int64_t)tail * chunks_per_token;
-      for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total_tail;
-           idx += (int64_t)gridDim.x * blockDim.x) {
-        int32_t t = (int32_t)(idx / chunks_per_token);
-        int32_t c = (int32_t)(idx - (int64_t)t * chunks_per_token);
-        int32_t head = c / chunks_per_head, off = c - head * chunks_per_head;
-        int64_t dst = (((int64_t)page * Hkv + head) * P + (len_new % P + t)) * chunks_per_head + off;
-        k_pool[dst] = zero;
-        v_pool[dst] = zero;
-        for (int32_t r = 0; r < peers.n; ++r) { ((int4*)peers.k[r])[dst] = zero; ((int4*)peers.v[r])[dst] = zero; }
-      }
-    }
-  }
-  // Peer stores must be visible to the replica's GPU before the host learns this kernel completed.
-  if (peers.n > 0) __threadfence_system();
-  // Completing only after the predecessor has completed keeps the dependency chain transitive: the
-  // attention kernel's griddepcontrol.wait on this grid then also covers everything before it.
-  pdl_wait();
+  const AppendGeom g{k_new, v_new, k_pool, v_pool, page_table, max_pages, P, Hkv, chunks_per_head};
+  append_work(meta, g, peers, (int64_t)blockIdx.x * blockDim.x + threadIdx.x, (int64_t)gridDim.x * blockDim.x,
+              blockIdx.x == 0 ? (int32_t)threadIdx.x : -1, (int32_t)blockDim.x);
 }
 
 __global__ void __launch_bounds__(256)

@@ -5,16 +5,19 @@
 #include <stdint.h>
 
 #include <algorithm>
-#include <cstdlib>
 #include <utility>
 
 #include "ws_internal.h"
 
 namespace ws {
 
-// PDL helpers: every kernel of the append -> attention -> combine chain is launched with
-// programmatic stream serialization; inside, griddepcontrol.wait guards the first access to data
-// the predecessor may still be writing and griddepcontrol.launch_dependents lets the successor start.
+// PDL helpers: every kernel of the (append ->) attention -> combine chain is launched with programmatic
+// stream serialization.  Protocol: a kernel executes griddepcontrol.wait before its
+// first access to anything its stream predecessor may have written or may still be reading - caller-
+// produced inputs included, the predecessor may be the caller's kernel - and at the latest before it
+// exits, so completion stays ordered along the chain; griddepcontrol.launch_dependents (one thread per
+// CTA suffices: the first arrival counts for the whole CTA) only lets the successor's CTAs be scheduled
+// early, it orders nothing, which is safe because every successor obeys the same rule.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
@@ -26,8 +29,7 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
-  static const bool no_pdl = getenv("WS_NO_PDL") != nullptr;   // debugging aid (A/B timing)
-  cfg.attrs = at; cfg.numAttrs = no_pdl ? 0 : 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
   return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
 
@@ -65,10 +67,12 @@ cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse
 struct Sm100Launch {
   AttnParams p;                      // p.meta == nullptr: use `inl`
   CUtensorMap tmap_q, tmap_k, tmap_v;
+  CUtensorMap tmap_kn, tmap_vn;      // fused step: k_new / v_new as [D, Hkv, tokens] (else copies of tmap_k / tmap_v)
   InlineAttnMetaLarge inl;
+  InlineAppendMeta app;              // fused step: the append descriptor (p.append_tokens > 0)
+  PeerPools peers;
   int32_t inl_words;                 // words of `inl` in use (selects the small / large parameter tier)
   int32_t num_ctas;
-  int32_t cta_group;                 // 1, or 2 (CTA pairs; needs an even team size)
   bool alt;                          // decode plan (plan.h): same Q tile, alternate KV tiles
 };
 cudaError_t sm100_attn_configure();    // one-time cudaFuncSetAttribute

@@ -49,9 +49,11 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
         int32_t last_tok = std::min(s.q_end, g.q_token0 + g.npairs * tok_per_pair) - 1;
         g.kv_len = vis_end[last_tok];
         g.vis_off = s.multi_block ? g.q_token0 : -1;
-        g.dep_tile = s.stable_tokens / kTileKeys;
+        const int32_t new_len = s.multi_block ? 0 : std::min(s.new_len, g.kv_len);
+        g.cache_len = g.kv_len - new_len;
+        g.new_tok0 = s.q_begin;
         plan.groups.push_back(g);
-        int32_t nt = (g.kv_len + kTileKeys - 1) / kTileKeys;
+        int32_t nt = (g.cache_len + kTileKeys - 1) / kTileKeys + (new_len + kTileKeys - 1) / kTileKeys;
         group_tiles.push_back(nt);
         plan.total_tiles += nt;
       }
@@ -156,7 +158,7 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
 
 std::vector<int32_t> serialise_plan(const Plan& plan, const std::vector<int32_t>& vis_end,
                                     bool has_vis) {
-  static_assert(sizeof(Group) == 32 && sizeof(Segment) == 16 && sizeof(CombineItem) == 16 &&
+  static_assert(sizeof(Group) == 40 && sizeof(Segment) == 16 && sizeof(CombineItem) == 16 &&
                 sizeof(AttnMeta) == 64, "blob layout");
   AttnMeta m{};
   m.num_teams = plan.num_teams;

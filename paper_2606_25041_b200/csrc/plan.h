@@ -14,7 +14,8 @@ struct PlanSession {
   int32_t q_begin;       // first global query token of this session in the call
   int32_t q_end;         // exclusive
   bool multi_block;      // queries span more than one block (per-token visible ends differ)
-  int32_t stable_tokens; // cache tokens that no in-flight predecessor kernel can still be writing
+  int32_t new_len;       // fused step: the last `new_len` visible keys are read from k_new / v_new (rows
+                         // q_begin ..) instead of the pool; 0 otherwise (and whenever multi_block)
 };
 
 struct PlanConfig {

@@ -19,7 +19,7 @@ constexpr int kMaxTeam = 8;       // max row-tile pairs of one (session, KV head
 // plans (MHA with 16+ heads, ragged multi-session batches) so that those steps, too, need no
 // host->device copy and stay CUDA-graph capturable.
 constexpr int kInlineAttnWords = 1000;
-constexpr int kInlineAttnWordsLarge = 7000;
+constexpr int kInlineAttnWordsLarge = 6800;
 constexpr int kInlineAppendWords = 960;
 template <int W> struct InlineMeta { int32_t w[W]; };
 using InlineAttnMeta = InlineMeta<kInlineAttnWords>;
@@ -53,9 +53,13 @@ struct Group {
   int32_t kv_len;        // keys visible to the LAST row of the group (= max visible end)
   int32_t npairs;        // row-tile pairs in this group (<= team size)
   int32_t vis_off;       // >= 0: per-token visible ends at vis_end[vis_off + (token - q_token0)]
-  int32_t dep_tile;      // KV tiles >= dep_tile (and their page-table entries) may have been written by
-                         // the kernel launched just before (the append of this step): the TMA producer
-                         // executes griddepcontrol.wait before touching them
+  // Key sources.  Keys [0, cache_len) are read from the paged pool: KV tiles [0, Tc), Tc =
+  // ceil(cache_len / 128).  Keys [cache_len, kv_len) - the block a fused step (ws_stream_step) is
+  // committing in the same launch - are read straight from the caller's k_new / v_new, rows new_tok0 ..:
+  // KV tiles [Tc, Tc + ceil((kv_len - cache_len) / 128)).  Outside fused steps cache_len == kv_len.
+  int32_t cache_len;
+  int32_t new_tok0;
+  int32_t pad;
 };
 
 // A contiguous KV-tile range of one group, processed by one team (CTA p handles pair p).
@@ -117,6 +121,12 @@ struct AttnParams {
   int32_t Hq, Hkv, D, G, P;
   int32_t total_q_tokens;
   float scale;
+  // fused step (ws_stream_step): warp 11 of every CTA commits its share of the new block (same code as
+  // kv_append_kernel, metadata in the `app` kernel parameter).  0: no append in this launch.
+  const void* k_new; const void* v_new;
+  void* k_pool_w; void* v_pool_w; int32_t* page_table_w;
+  int32_t append_tokens;
+  int32_t pad_a;
   // fused combine (a4 inside the attention kernel): arrival counters [max_part_slots] followed by
   // completion counters [max_part_slots], indexed by the first partial slot of a (combine item, pair);
   // all zero between launches (the last merging warp of an item resets them).  nullptr: the partials

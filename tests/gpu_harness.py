@@ -82,7 +82,9 @@ def preload_gpu(cache, w: Workload, dev_k: List, dev_v: List) -> List[int]:
 
 def run_workload_gpu(w: Workload, flags: int = 0, min_splits: int = 0, shuffle_seed: Optional[int] = None,
                      want_lse: bool = True, gather: bool = True, pool_fill: Optional[int] = None,
-                     decode_plan: Optional[bool] = None) -> Dict:
+                     decode_plan: Optional[bool] = None, fused_step: bool = False) -> Dict:
+    """fused_step: every step goes through ws_stream_step (one launch commits and attends the block, the
+    configuration bench.py times) instead of ws_kv_append followed by ws_block_causal_attn_fwd."""
     import torch
     sp = w.spec
     dev = torch.device("cuda", 0)
@@ -106,8 +108,11 @@ def run_workload_gpu(w: Workload, flags: int = 0, min_splits: int = 0, shuffle_s
         v = torch.cat([_torch_of(s.v[t], dev) for s in w.sessions])
         out = torch.full((S * n, sp.num_q_heads, sp.head_dim), float("nan"), dtype=tdt, device=dev)
         lse = torch.full((S * n, sp.num_q_heads), float("nan"), dtype=torch.float32, device=dev) if want_lse else None
-        cache.kv_append(ids, cu, k, v, modality=np.tile(w.modality, S))
-        cache.block_causal_attn_fwd(ids, cu, q, out, sp.scale, lse=lse)
+        if fused_step:
+            cache.stream_step(ids, cu, q, k, v, out, sp.scale, lse=lse)
+        else:
+            cache.kv_append(ids, cu, k, v, modality=np.tile(w.modality, S))
+            cache.block_causal_attn_fwd(ids, cu, q, out, sp.scale, lse=lse)
         torch.cuda.synchronize()
         plans.append(cache.last_plan_info())
         o = out.float().cpu().numpy().astype(np.float64).reshape(S, n, sp.num_q_heads, sp.head_dim)

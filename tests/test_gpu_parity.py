@@ -200,33 +200,13 @@ SMALL_TC = [
 ]
 
 
+@pytest.mark.parametrize("fused_step", [False, True], ids=["two_calls", "fused_step"])
 @pytest.mark.parametrize("label,ov", SMALL_TC, ids=[x[0] for x in SMALL_TC])
-def test_bf16_tensor_core_kernel_small(label, ov):
+def test_bf16_tensor_core_kernel_small(label, ov, fused_step):
     w = _small(2, **ov)
-    got = run_workload_gpu(w, pool_fill=0x7FC1)            # NaN canary in unused cache slots
+    got = run_workload_gpu(w, pool_fill=0x7FC1, fused_step=fused_step)   # NaN canary in unused cache slots
     assert got["tensor"]
     _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, label)
-
-
-@pytest.mark.parametrize("label,ov", [x for x in SMALL_TC if x[0] in ("gqa4_ragged_tail", "gqa8_tail_le_64", "mha_aligned")],
-                         ids=["gqa4_ragged_tail", "gqa8_tail_le_64", "mha_aligned"])
-def test_bf16_cta_pair_variant(label, ov):
-    """WS_FLAG_CTA_PAIRS: the same kernel on 2-CTA clusters (tcgen05 cta_group::2, each CTA stages half
-    of every K/V tile, cross-CTA barriers).  Opt-in; must match the oracle like the default path."""
-    from paper_2606_25041_b200 import WS_FLAG_CTA_PAIRS
-    w = _small(2, **ov)
-    got = run_workload_gpu(w, flags=WS_FLAG_CTA_PAIRS, pool_fill=0x7FC1)
-    even_team = got["plans"][-1]["team_size"] % 2 == 0
-    assert got["plans"][-1]["used_tensor_core_kernel"] == (2 if even_team else 1)
-    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, label + " (cta pairs)")
-
-
-def test_cta_pair_variant_config3_shape():
-    from paper_2606_25041_b200 import WS_FLAG_CTA_PAIRS
-    w = _small(3, cache_lens=(5000,), block_tokens=512)
-    got = run_workload_gpu(w, flags=WS_FLAG_CTA_PAIRS, min_splits=2)
-    assert got["plans"][-1]["used_tensor_core_kernel"] == 2 and got["plans"][-1]["team_size"] == 8
-    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "cfg3-like cta pairs")
 
 
 @pytest.mark.parametrize("splits", [1, 2, 3, 7, 12])
@@ -425,6 +405,9 @@ def test_next4_decode_plan_matches_oracle(label, ov):
     got = run_workload_gpu(w, pool_fill=0x7FC1)
     assert all(pl["used_tensor_core_kernel"] == 3 for pl in got["plans"]), got["plans"]
     _assert_close(compare(got, ref, "bf16"), BF16_TOL, label + " (decode plan)")
+    fus = run_workload_gpu(w, pool_fill=0x7FC1, fused_step=True)
+    assert all(pl["used_tensor_core_kernel"] == 3 for pl in fus["plans"]), fus["plans"]
+    _assert_close(compare(fus, ref, "bf16"), BF16_TOL, label + " (decode plan, fused step)")
     gen = run_workload_gpu(w, pool_fill=0x7FC1, decode_plan=False, gather=False)
     assert all(pl["used_tensor_core_kernel"] == 1 for pl in gen["plans"])
     _assert_close(compare(gen, ref, "bf16"), BF16_TOL, label + " (general plan)")
@@ -726,24 +709,28 @@ def _sample(n, Hq, k=24, seed=0):
 
 def test_config2_full_size():
     w = generate(spec_for_config(2))
-    got = run_workload_gpu(w)
-    assert got["tensor"]
-    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "cfg2")
+    ref = run_workload_oracle(w)
+    for fused_step in (True, False):                       # bench.py times the fused step
+        got = run_workload_gpu(w, fused_step=fused_step)
+        assert got["tensor"]
+        _assert_close(compare(got, ref, "bf16"), BF16_TOL, f"cfg2 fused_step={fused_step}")
 
 
 def test_config3_full_size_every_element():
     """Every output element (512 tokens x 32 heads x 128) against the oracle (reading A18)."""
     w = generate(spec_for_config(3))
-    got = run_workload_gpu(w)
-    assert got["tensor"]
-    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "cfg3 (all elements)")
+    ref = run_workload_oracle(w)
+    for fused_step in (True, False):                       # bench.py times the fused step
+        got = run_workload_gpu(w, fused_step=fused_step)
+        assert got["tensor"]
+        _assert_close(compare(got, ref, "bf16"), BF16_TOL, f"cfg3 (all elements) fused_step={fused_step}")
 
 
 def test_config4_long_session_20_steps():
     """Units 1 and 20 (cache 65,536 and 70,400 tokens): every output element; the 18 units in between:
     sampled rows x heads (the float64 oracle needs ~5 s per full unit on the test box)."""
     w = generate(spec_for_config(4))
-    got = run_workload_gpu(w)
+    got = run_workload_gpu(w, fused_step=True)              # the launch configuration bench.py times
     assert got["tensor"] and got["plans"][0]["num_ctas"] == 148
     full = run_workload_oracle(w, steps=(0, 19))
     _assert_close(compare(got, full, "bf16"), BF16_TOL, "cfg4 units 1 and 20 (all elements)")
@@ -761,9 +748,11 @@ def test_config4_long_session_20_steps():
 def test_config5_ragged_multi_session_every_element():
     """All 8 sessions x 256 tokens x 32 heads x 128 against the oracle (reading A18)."""
     w = generate(spec_for_config(5))
-    got = run_workload_gpu(w)
-    assert got["tensor"]
-    _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "cfg5 (all elements)")
+    ref = run_workload_oracle(w)
+    for fused_step in (True, False):                       # bench.py times the fused step
+        got = run_workload_gpu(w, fused_step=fused_step)
+        assert got["tensor"]
+        _assert_close(compare(got, ref, "bf16"), BF16_TOL, f"cfg5 (all elements) fused_step={fused_step}")
 
 
 def test_maximum_size_one_million_token_session_sampled():
@@ -872,38 +861,116 @@ def test_stream_step_host_end_to_end():
     assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3
 
 
-def test_stream_step_single_call_equals_two_calls():
-    """ws_stream_step (append + attend in one call, device buffers): bit-identical to ws_kv_append followed by
-    ws_block_causal_attn_fwd on a twin cache, matches the oracle, and rejects what the attention half would
-    reject before anything is committed."""
+@pytest.mark.parametrize("aligned", [True, False], ids=["aligned", "ragged"])
+def test_stream_step_fused_launch_equals_separate_kernels(aligned):
+    """ws_stream_step commits and attends in ONE launch (new keys read from k_new / v_new as KV tiles of
+    their own, warps 10-11 copy them into the pool).  Against a twin cache driven by ws_kv_append +
+    ws_block_causal_attn_fwd and a third one with WS_FLAG_SEPARATE_APPEND: the caches end bit-identical,
+    every path matches the oracle, and where the cache lengths are multiples of the 128-key tile (same
+    tiles, same plan) the outputs are bit-identical too.  Rejected arguments commit nothing."""
     import torch
-    from paper_2606_25041_b200 import WsError
-    w = _small(5, cache_len_range=(100, 1500), block_tokens=64, modality_split=(48, 12, 4), steps=2)
-    S, n, sp = w.spec.num_sessions, 64, w.spec
+    from paper_2606_25041_b200 import WS_FLAG_SEPARATE_APPEND, WsError
+    if aligned:
+        w = _small(5, num_sessions=3, cache_lens=(1024, 256, 2048), block_tokens=128, modality_split=(96, 24, 8), steps=3)
+    else:
+        w = _small(5, cache_len_range=(100, 1500), block_tokens=72, modality_split=(54, 12, 6), steps=3)
+    S, n, sp = w.spec.num_sessions, w.spec.block_tokens, w.spec
     dev = torch.device("cuda", 0)
     dk = [_torch_of(s.k_cache, dev) for s in w.sessions]; dv = [_torch_of(s.v_cache, dev) for s in w.sessions]
-    a, b = make_cache(w), make_cache(w)
-    ids_a, ids_b = preload_gpu(a, w, dk, dv), preload_gpu(b, w, dk, dv)
+    a, b, c3 = make_cache(w, pool_fill=0x7FC1), make_cache(w, pool_fill=0x7FC1), make_cache(w, flags=WS_FLAG_SEPARATE_APPEND, pool_fill=0x7FC1)
+    ids_a, ids_b, ids_c = preload_gpu(a, w, dk, dv), preload_gpu(b, w, dk, dv), preload_gpu(c3, w, dk, dv)
     cu = [i * n for i in range(S + 1)]
     ref = run_workload_oracle(w)
-    for t in range(2):
+    for t in range(sp.steps):
         q = torch.cat([_torch_of(s.q[t], dev) for s in w.sessions])
         k = torch.cat([_torch_of(s.k[t], dev) for s in w.sessions])
         v = torch.cat([_torch_of(s.v[t], dev) for s in w.sessions])
-        oa = torch.full((S * n, sp.num_q_heads, 128), float("nan"), dtype=torch.bfloat16, device=dev); ob = oa.clone()
-        la = torch.full((S * n, sp.num_q_heads), float("nan"), dtype=torch.float32, device=dev); lb = la.clone()
+        oa = torch.full((S * n, sp.num_q_heads, 128), float("nan"), dtype=torch.bfloat16, device=dev); ob = oa.clone(); oc = oa.clone()
+        la = torch.full((S * n, sp.num_q_heads), float("nan"), dtype=torch.float32, device=dev); lb = la.clone(); lc = la.clone()
+        launches0 = a.launch_count()
         a.stream_step(ids_a, cu, q, k, v, oa, sp.scale, lse=la)
+        assert a.launch_count() - launches0 == 1 + (a.last_plan_info()["num_combine_items"] > 0)   # no append launch
         b.kv_append(ids_b, cu, k, v); b.block_causal_attn_fwd(ids_b, cu, q, ob, sp.scale, lse=lb)
+        c3.stream_step(ids_c, cu, q, k, v, oc, sp.scale, lse=lc)
         torch.cuda.synchronize()
-        assert torch.equal(oa.view(torch.int16), ob.view(torch.int16)) and torch.equal(la, lb)
-        o = oa.float().cpu().numpy().reshape(S, n, sp.num_q_heads, 128)
-        for s in range(S):
-            d = np.abs(o[s] - ref["out"][t][s])
-            assert (d <= bf16_error_bound(ref["out"][t][s], o[s], ref["abs"][t][s])).all() and d.mean() <= 1e-3
+        assert torch.equal(ob.view(torch.int16), oc.view(torch.int16)) and torch.equal(lb, lc)
+        if aligned:
+            assert torch.equal(oa.view(torch.int16), ob.view(torch.int16)) and torch.equal(la, lb)
+        for o_t, l_t in ((oa, la), (ob, lb)):
+            o = o_t.float().cpu().numpy().astype(np.float64).reshape(S, n, sp.num_q_heads, 128)
+            l = l_t.cpu().numpy().astype(np.float64).reshape(S, n, sp.num_q_heads)
+            for s in range(S):
+                d = np.abs(o[s] - ref["out"][t][s])
+                assert (d <= bf16_error_bound(ref["out"][t][s], o[s], ref["abs"][t][s])).all() and d.mean() <= 1e-3
+                assert np.abs(l[s] - ref["lse"][t][s]).max() <= 1e-4
+    for s in range(S):                                     # the three caches hold the same bytes
+        tokens = a.session_info(ids_a[s])[0]
+        got = []
+        for cch, ids in ((a, ids_a), (b, ids_b), (c3, ids_c)):
+            kg = torch.empty((tokens, sp.num_kv_heads, 128), dtype=torch.bfloat16, device=dev); vg = torch.empty_like(kg)
+            cch.kv_gather(ids[s], 0, tokens, kg, vg)
+            torch.cuda.synchronize()
+            got.append((_numpy_of(kg).tobytes(), _numpy_of(vg).tobytes()))
+        kr, vr = ref["kv"][s]
+        assert got[0] == got[1] == got[2] == (np.ascontiguousarray(kr).tobytes(), np.ascontiguousarray(vr).tobytes())
     tokens_before = a.session_info(ids_a[0])[0]
     with pytest.raises(WsError):
         a.stream_step(ids_a, cu, q, k, v, oa, -1.0)          # bad scale: nothing may be committed
     assert a.session_info(ids_a[0])[0] == tokens_before
+
+
+@pytest.mark.parametrize("flags", ["default", "fused_combine", "separate_append"])
+def test_back_to_back_steps_without_host_sync_changing_data(flags):
+    """The PDL chain with CHANGING data and no host synchronisation between steps: solver-style
+    stage / attend / roll back / re-append at the SAME cache positions with different K/V every step (a
+    write-after-read hazard if a kernel could start before its predecessor's reads were done), each step's
+    q / k / v produced on the same stream immediately before the call by a deliberately slow kernel chain
+    (a read-after-write hazard if the library read its inputs before waiting for its stream predecessor).
+    Every step's output goes to its own buffer and is compared with the oracle afterwards."""
+    import torch
+    from oracle.block_causal import OracleSession, attend
+    from paper_2606_25041_b200 import WS_FLAG_FUSED_COMBINE, WS_FLAG_SEPARATE_APPEND
+    fl = {"default": 0, "fused_combine": WS_FLAG_FUSED_COMBINE, "separate_append": WS_FLAG_SEPARATE_APPEND}[flags]
+    w = _small(3, cache_lens=(2500,), block_tokens=128, modality_split=(96, 24, 8), steps=1)
+    si = w.sessions[0]
+    dev = torch.device("cuda", 0)
+    cache = make_cache(w, flags=fl)
+    cache.set_min_splits(3 if flags != "separate_append" else 0)
+    ids = preload_gpu(cache, w, [_torch_of(si.k_cache, dev)], [_torch_of(si.v_cache, dev)])
+    base_blocks = cache.session_info(ids[0])[1]
+    n, Hq, Hkv, steps = 128, 32, 8, 6
+    rng = np.random.default_rng(123)
+    src = [tuple(_torch_of(to_bf16(rng.standard_normal(sh, dtype=np.float32)), dev)
+                 for sh in ((n, Hq, 128), (n, Hkv, 128), (n, Hkv, 128))) for _ in range(steps)]
+    qb = torch.zeros((n, Hq, 128), dtype=torch.bfloat16, device=dev)
+    kb = torch.zeros((n, Hkv, 128), dtype=torch.bfloat16, device=dev); vb = torch.zeros_like(kb)
+    outs = [torch.full((n, Hq, 128), float("nan"), dtype=torch.bfloat16, device=dev) for _ in range(steps)]
+    big = torch.randn((4096, 4096), device=dev)
+    torch.cuda.synchronize()
+    for t in range(steps):
+        # slow producer chain on the same stream: the inputs of step t are complete only when it ends
+        z = big @ big
+        qb.copy_(src[t][0] + 0 * z[0, 0].to(torch.bfloat16)); kb.copy_(src[t][1]); vb.copy_(src[t][2])
+        if t % 2 == 0:
+            cache.stream_step(ids, [0, n], qb, kb, vb, outs[t], w.spec.scale)
+        else:
+            cache.kv_append(ids, [0, n], kb, vb)
+            cache.block_causal_attn_fwd(ids, [0, n], qb, outs[t], w.spec.scale)
+        cache.session_truncate(ids[0], base_blocks)            # roll the staged block back (host metadata)
+    torch.cuda.synchronize()
+    hist = OracleSession(Hkv, 128)
+    from tests.gpu_harness import preload_rounds
+    for _, rng_ in preload_rounds(w):
+        lo, hi = rng_[0]
+        hist.append(si.k_cache[lo:hi], si.v_cache[lo:hi])
+    for t in range(steps):
+        trial = OracleSession(Hkv, 128)
+        trial.k_slices, trial.v_slices, trial.block_ends = list(hist.k_slices), list(hist.v_slices), list(hist.block_ends)
+        trial.append(_numpy_of(src[t][1]), _numpy_of(src[t][2]))
+        o_ref, _, a_ref = attend(trial, _numpy_of(src[t][0]), w.spec.scale, want_abs=True)
+        o = outs[t].float().cpu().numpy().astype(np.float64)
+        d = np.abs(o - o_ref)
+        assert np.isfinite(o).all() and (d <= bf16_error_bound(o_ref, o, a_ref)).all() and d.max() <= 1e-2, (t, d.max())
 
 
 def test_fp32_generic_kernel_step_is_cuda_graph_capturable():
