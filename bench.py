@@ -3,9 +3,10 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
 
-A "step" is one streaming unit of the hot path: ws_kv_append (commit the unit's K/V block) followed by
-ws_block_causal_attn_fwd (the block attends to the full history; includes the split-KV combine), issued through
-ws_stream_step (the two in one C call: same kernels, one trip through the binding).
+A "step" is one streaming unit of the hot path: commit the unit's K/V block (a2) and let the block attend to
+the full history (a3, + the split-KV combine a4), issued through ws_stream_step: ONE launch commits and attends
+(the attention kernel reads the new keys from k_new / v_new and two of its warps copy them into the pool),
+followed by the combine launch when the plan splits the cache.
 Headline workload = BASELINE.json configs[3] ("bf16 long session": 32 q / 8 kv heads, D=128, block of
 256 tokens, cache 65536 growing over 20 consecutive units) - the configuration the north_star's 60 %
 target is quoted on.  After 20 units the session is rolled back (host metadata only) and replayed.
@@ -171,8 +172,7 @@ def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, r
     torch.cuda.synchronize()
     g = torch.cuda.CUDAGraph()
     with torch.cuda.graph(g):
-        cache.kv_append(ids, cu, k0, v0)
-        cache.block_causal_attn_fwd(ids, cu, q0, out, sp.scale)
+        cache.stream_step(ids, cu, q0, k0, v0, out, sp.scale)
     reps = 200
     for _ in range(5):
         g.replay()
@@ -182,7 +182,7 @@ def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, r
     fl = 4.0 * sp.head_dim * sp.num_q_heads * sp.block_tokens * sum(cache.session_info(i)[0] for i in ids)
     res["solver_step_cuda_graph"] = {"us_per_step": 1e3 * ms / reps, "tflops": fl / (ms / reps * 1e-3) / 1e12,
                                      "kv_tokens": L, "replays": reps,
-                                     "what": "append + attention + combine of one uncommitted block, graph replay"}
+                                     "what": "ws_stream_step (commit + attention in one launch, + combine) of one uncommitted block, graph replay"}
     reset()
     # --- NEXT-1: multi-block prefill
     Hq, Hkv, D, n, B = sp.num_q_heads, sp.num_kv_heads, sp.head_dim, 256, 32
@@ -215,14 +215,13 @@ def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, r
         kd, vd, qd = k0[:n_dec].contiguous(), v0[:n_dec].contiguous(), q0[:n_dec].contiguous()
         od = torch.empty_like(qd)
         cud = [0, n_dec]
-        cache.kv_append(ids, cud, kd, vd); cache.block_causal_attn_fwd(ids, cud, qd, od, sp.scale)
+        cache.stream_step(ids, cud, qd, kd, vd, od, sp.scale)
         plan = cache.last_plan_info()
         reset()
         torch.cuda.synchronize()
         gd = torch.cuda.CUDAGraph()
         with torch.cuda.graph(gd):
-            cache.kv_append(ids, cud, kd, vd)
-            cache.block_causal_attn_fwd(ids, cud, qd, od, sp.scale)
+            cache.stream_step(ids, cud, qd, kd, vd, od, sp.scale)
         for _ in range(5):
             gd.replay()
         reps = 200
@@ -238,7 +237,7 @@ def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, r
             "hbm_gbs": byts / us / 1e3, "hbm_peak_gbs": float(peaks["hbm_gbs"]),
             "frac_of_hbm_roofline": byts / us / 1e3 / float(peaks["hbm_gbs"]),
             "kernel": plan["used_tensor_core_kernel"],
-            "what": "append + attention (decode plan) + combine, CUDA-graph replay, history read from HBM"})
+            "what": "ws_stream_step (commit + attention on the decode plan in one launch, + combine), CUDA-graph replay, history read from HBM"})
     # --- NEXT-3: replica link (thinker -> performer KV-slice exchange).  The box has ONE GPU, so the
     # linked pool is a second pool on the same device: these numbers show the cost of the extra stores
     # and of the page push at HBM speed; over NVLink 5 the peer stores run at <= 900 GB/s per direction.
@@ -331,6 +330,45 @@ def run_reference(args, spec):
     print(json.dumps(line))
 
 
+def spawn_ranks(n: int) -> int:
+    """`python bench.py --gpus N` without a launcher: re-execute this command line under torch.distributed.run
+    with N ranks on this node (one process per GPU).  Returns the launcher's exit code."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    rc = subprocess.call(cmd)
+    if rc != 0:
+        raise SystemExit(rc)
+    return rc
+
+
+def selftest_cpu(args):
+    """The N > 1 plumbing without GPUs: gloo rendezvous, barrier, MAX-over-ranks time and SUM-over-ranks work
+    (aggregate_over_ranks), rank 0 prints one line.  Per-rank numbers are made up (rank r: 10 + r ms, 1e12 flops)."""
+    import torch
+    import torch.distributed as dist
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+        dist.barrier()
+    ms, fl = aggregate_over_ranks(10.0 + rank, 1e12, dist if world > 1 else None, torch.device("cpu"))
+    if rank == 0:
+        print(json.dumps({"selftest": True, "n_gpus": world, "ms_max_over_ranks": ms, "flops_sum_over_ranks": fl,
+                          "value": fl / (ms * 1e-3) / 1e12, "unit": "TFLOP/s (made-up timings: plumbing test only)"}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def region_stats(us_list):
+    a = np.asarray(us_list, dtype=np.float64)
+    return {"mean": float(a.mean()), "median": float(np.median(a)), "min": float(a.min()), "max": float(a.max()),
+            "regions": int(a.size)}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -345,10 +383,17 @@ def main():
     ap.add_argument("--no-next", action="store_true", help="skip the NEXT-1 / NEXT-2 side measurements")
     ap.add_argument("--fused-combine", action="store_true",
                     help="A/B: merge the split-KV partials inside the attention kernel (WS_FLAG_FUSED_COMBINE)")
+    ap.add_argument("--selftest-cpu", action="store_true",
+                    help="exercise the multi-rank entry path (spawn, rendezvous, max/sum over ranks) on CPU with "
+                         "the gloo backend and made-up per-rank timings; prints a line marked selftest, no metric")
     args = ap.parse_args()
     spec = CONFIG_SPECS[args.config]
     if args.impl == "reference":
         return run_reference(args, spec)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args.gpus)
+    if args.selftest_cpu:
+        return selftest_cpu(args)
 
     import torch
     import __graft_entry__ as entry
@@ -432,12 +477,57 @@ def main():
     def work(nsteps, fn):
         return sum(fn[(i // R) % steps_per_cycle] for i in range(nsteps))
 
+    def timed_chunks(nchunks, chunk, fn, first=0):
+        """nchunks regions of `chunk` steps back to back, an event at every region boundary (one boundary per
+        `chunk` steps: the kernels inside a region keep their programmatic overlap).  Returns per-region
+        us per step (max over ranks per region)."""
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(nchunks + 1)]
+        barrier()
+        evs[0].record(stream)
+        for cix in range(nchunks):
+            for i in range(first + cix * chunk, first + (cix + 1) * chunk):
+                fn(i)
+            evs[cix + 1].record(stream)
+        barrier()
+        per = [evs[cix].elapsed_time(evs[cix + 1]) for cix in range(nchunks)]
+        if dist is not None:
+            t = torch.tensor(per, dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            per = t.tolist()
+        return [1e3 * x / chunk for x in per]
+
     K, W = args.steps, max(args.warmup, 3)
-    for i in range(W):
+    cycle = steps_per_cycle * R                            # one pass over every cache / unit of the loop
+    for i in range(max(W, cycle)):
         step(i)
-    # a short burst (one cycle of units) before the long region: the kernel's capability before the
-    # 1 kW power cap pulls the SM clock down (reported beside the sustained headline, not instead of it)
-    ms_burst = timed(steps_per_cycle, step) if K > 4 * steps_per_cycle else None
+    # ---- burst: single cycles timed alone after a pause (clocks not yet pulled down by the 1 kW cap)
+    us_burst = []
+    for _ in range(5):
+        barrier()
+        time.sleep(0.15)
+        us_burst += timed_chunks(1, cycle, step)
+    # ---- sustained: >= 2 s of back-to-back cycles, one event per cycle (median / min / mean per unit)
+    est_us = float(np.median(us_burst))
+    n_sus = max(3, int(np.ceil(2.0e6 / (est_us * cycle))))
+    sus_sampler = ClockSampler(local)
+    sus_sampler.start()
+    t_wall = time.perf_counter()
+    us_sus = timed_chunks(n_sus, cycle, step)
+    t_wall = time.perf_counter() - t_wall
+    sus_sampler.stop_flag.set(); sus_sampler.join(timeout=2)
+    # ---- warm L2 beside cold L2 (configs whose history fits L2): one cache replayed
+    us_warm = None
+    if R > 1:
+        def step_warm(i):
+            if (i % steps_per_cycle) == 0:
+                reset(0)
+            caches[0].stream_step(ids_of[0], cu, q_d[i % steps_per_cycle], k_d[i % steps_per_cycle],
+                                  v_d[i % steps_per_cycle], out, sp.scale, stream=stream)
+        for i in range(3 * steps_per_cycle):
+            step_warm(i)
+        us_warm = timed_chunks(20, 10 * steps_per_cycle, step_warm)
+        barrier()
+        time.sleep(0.15)
     # ---- pass A: whole-step throughput (no per-kernel events), clocks sampled during the region
     sampler = ClockSampler(local)
     sampler.start()
@@ -467,7 +557,7 @@ def main():
     # Denominator (B200_PROFILING.md): the kernel is timed INSIDE a long step loop under the 1 kW power
     # cap, so its peer is the sustained cuBLAS figure; the short burst region below is paired with the
     # burst figure.  Both fractions are printed.
-    long_loop = ms_total >= 100.0
+    long_loop = True      # the K-step region directly follows the >= 2 s sustained loop: power-capped state
     peak_burst = float(peaks["bf16_tflops"])
     peak = float(peaks.get("bf16_tflops_sustained", peak_burst)) if long_loop else peak_burst
     kv_bytes_per_launch = work(K, bytes_cycle) / K
@@ -478,8 +568,7 @@ def main():
                 "kernel": "attn_sm100_kernel" if plan["used_tensor_core_kernel"] else "attn_simt_kernel (fp32 CUDA cores; launch-bound at this size)",
                 "achieved": achieved, "peak": peak,
                 "unit": "TFLOP/s", "frac": achieved / peak,
-                "peak_source": peak_src + (" bf16 sustained (kernel timed inside a %.0f ms loop)" % ms_total
-                                           if long_loop else " bf16 burst (short region)"),
+                "peak_source": peak_src + " bf16 sustained (the timed region directly follows a >= 2 s loop of the same steps)",
                 "frac_of_burst": achieved / peak_burst,
                 "traffic": read_traffic(args.config),
                 "frac_of_sustained": achieved / float(peaks.get("bf16_tflops_sustained", peak)),
@@ -493,11 +582,28 @@ def main():
                                              kv_bytes_per_launch / (float(peaks["hbm_gbs"]) * 1e9)),
                 "step_frac_of_roofline": max(flops_per_launch / (peak * 1e12),
                                              kv_bytes_per_launch / (float(peaks["hbm_gbs"]) * 1e9)) / (ms_per_step * 1e-3),
-                "ms_per_step_with_kernel_events": ms_total_b / K,
-                "burst": None if ms_burst is None else {
-                    "steps": steps_per_cycle, "us_per_unit": 1e3 * ms_burst / steps_per_cycle,
-                    "tflops": world * work(steps_per_cycle, flops_cycle) / (ms_burst * 1e-3) / 1e12,
-                    "frac_of_burst_peak": work(steps_per_cycle, flops_cycle) / (ms_burst * 1e-3) / 1e12 / peak_burst}}
+                "ms_per_step_with_kernel_events": ms_total_b / K}
+    flops_per_unit_cycle = work(cycle, flops_cycle) / cycle
+    bytes_per_unit_cycle = work(cycle, bytes_cycle) / cycle
+    peak_sus = float(peaks.get("bf16_tflops_sustained", peak_burst))
+
+    def regime(us_list, peak_tf):
+        st = region_stats(us_list)
+        roof_us = 1e6 * max(flops_per_unit_cycle / (peak_tf * 1e12), bytes_per_unit_cycle / (float(peaks["hbm_gbs"]) * 1e9))
+        return {"us_per_unit": st, "units_per_region": cycle,
+                "tflops_at_median": world * flops_per_unit_cycle / (st["median"] * 1e-6) / 1e12,
+                "hbm_gbs_at_median": world * bytes_per_unit_cycle / (st["median"] * 1e-6) / 1e9,
+                "step_roofline_us": roof_us, "step_frac_of_roofline_at_median": roof_us / st["median"],
+                "bf16_peak_tflops_used": peak_tf}
+    burst = regime(us_burst, peak_burst)
+    burst["what"] = "5 single cycles of the loop, each timed alone after a 0.15 s pause (burst cuBLAS peak as denominator)"
+    sustained = regime(us_sus, peak_sus)
+    sustained.update({"seconds": t_wall, "clocks": sus_sampler.result(),
+                      "what": ">= 2 s of back-to-back cycles, one CUDA event per cycle (sustained cuBLAS peak as denominator)"})
+    warm_l2 = None
+    if us_warm is not None:
+        warm_l2 = {"us_per_unit": region_stats(us_warm),
+                   "what": "one cache replayed (history served from L2) - the cold-L2 figures above cycle over %d caches" % R}
 
     if roofline["bound"] == "hbm":
         # cache-read-bound step: report the dominant kernel against the measured copy bandwidth
@@ -550,8 +656,7 @@ def main():
         gr = torch.cuda.CUDAGraph()
         with torch.cuda.graph(gr):
             for r in range(R):
-                caches[r].kv_append(ids_of[r], cu, k_d[0], v_d[0])
-                caches[r].block_causal_attn_fwd(ids_of[r], cu, q_d[0], out, sp.scale)
+                caches[r].stream_step(ids_of[r], cu, q_d[0], k_d[0], v_d[0], out, sp.scale)
         for _ in range(5):
             gr.replay()
         reps = max(20, 400 // R)
@@ -561,7 +666,7 @@ def main():
         nxt["step_cuda_graph"] = {"us_per_unit": us_g, "tflops": flops_cycle[0] / (us_g * 1e-6) / 1e12,
                                   "hbm_gbs": bytes_cycle[0] / (us_g * 1e-6) / 1e9,
                                   "frac_of_step_roofline": roofline["step_roofline_us"] / us_g,
-                                  "what": "append + attention + combine of %d caches captured once, replayed: "
+                                  "what": "ws_stream_step (+ combine) of %d caches captured once, replayed: "
                                           "no host planning or launch cost in the loop" % R}
         reset()
 
@@ -593,7 +698,8 @@ def main():
                                   % (R, bytes_cycle[0] / 1e6, R * bytes_cycle[0] / 1e6)),
                            "parallelism": f"dp{world} (independent sessions per GPU, no collective)",
                            "plan": plan},
-                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+                "roofline": roofline, "burst": burst, "sustained": sustained, "warm_l2": warm_l2,
+                "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
                 "next": nxt,
                 "clocks": sampler.result(),
                 "context": {"paper_model_side_latency_ms": 200, "paper_total_latency_ms": 550,

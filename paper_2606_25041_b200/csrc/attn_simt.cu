@@ -8,7 +8,9 @@
 // :47 Eq. (1): row r of block b sees keys j < e_b.
 //
 // One warp per (query token, q head).  Lane = key for the scores (online softmax, max/sum reduced
-// with warp shuffles), lane = output-dim slice for P.V.
+// with warp shuffles), lane = output-dim slice for P.V, eight V rows in flight per lane (the loop is
+// bound by load latency, not by arithmetic: walking the keys one dependent load at a time cost 19 us for
+// the 48 keys of the fp32 config).
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <math.h>
@@ -57,6 +59,10 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
   // per-token (session slot, visible end): device blob, or - small calls - the kernel parameter itself
   // (constant-bank reads; no host->device copy in the chain, so the call is CUDA-graph capturable)
   const MetaView<kInlineAppendWords> meta{tok_meta, inl};
+  // programmatic dependent launch (launch.h): q, the pool and the page table may come from the kernel
+  // just before (ws_kv_append of the same step)
+  pdl_wait();
+  pdl_launch_dependents();
   __shared__ float q_s[kSimtWarps][kMaxD];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const int64_t w = (int64_t)blockIdx.x * kSimtWarps + wib;
@@ -86,6 +92,7 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
       rowidx = (page_row[j / P] * Hkv + g) * P + (j % P);
       const T* kp = k_pool + (int64_t)rowidx * D;
       float a = 0.f;
+#pragma unroll 4
       for (int d = 0; d < D; d += VN) {
         float kv[VN];
         Vec16<T>::load(kp + d, kv);
@@ -107,14 +114,26 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
 #pragma unroll
     for (int i = 0; i < kMaxD / 32; ++i) acc[i] *= corr;
     const int nk = min(32, vis - base);
-    for (int kk = 0; kk < nk; ++kk) {
-      const float pk = __shfl_sync(0xffffffffu, p, kk);
-      const int32_t r = __shfl_sync(0xffffffffu, rowidx, kk);
-      const T* vp = v_pool + (int64_t)r * D;
+    constexpr int kBatch = 8;
+    for (int kk0 = 0; kk0 < nk; kk0 += kBatch) {
+      float pk[kBatch];
+      const T* vp[kBatch];
+#pragma unroll
+      for (int u = 0; u < kBatch; ++u) {
+        const int kk = (kk0 + u) & 31;
+        pk[u] = kk0 + u < nk ? __shfl_sync(0xffffffffu, p, kk) : 0.f;
+        vp[u] = v_pool + (int64_t)__shfl_sync(0xffffffffu, rowidx, kk) * D;
+      }
 #pragma unroll
       for (int i = 0; i < kMaxD / 32; ++i) {
-        int d = lane + 32 * i;
-        if (d < D) acc[i] = fmaf(pk, to_f32(vp[d]), acc[i]);
+        const int d = lane + 32 * i;
+        if (d < D) {
+          float vv[kBatch];
+#pragma unroll
+          for (int u = 0; u < kBatch; ++u) vv[u] = kk0 + u < nk ? to_f32(vp[u][d]) : 0.f;
+#pragma unroll
+          for (int u = 0; u < kBatch; ++u) acc[i] = fmaf(pk[u], vv[u], acc[i]);
+        }
       }
     }
     m = m_new;
@@ -137,17 +156,14 @@ cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse
   int64_t warps = (int64_t)total_q_tokens * Hq;
   int32_t grid = (int32_t)((warps + kSimtWarps - 1) / kSimtWarps);
   if (grid == 0) return cudaSuccess;
-  if (dtype == 1) {
-    attn_simt_kernel<float><<<grid, kSimtWarps * 32, 0, stream>>>(
-        (const float*)q, (float*)out, lse, (const float*)k_pool, (const float*)v_pool, page_table,
-        tok_meta, inl, q_to_kv, total_q_tokens, max_pages, Hq, Hkv, D, P, scale);
-  } else {
-    attn_simt_kernel<__nv_bfloat16><<<grid, kSimtWarps * 32, 0, stream>>>(
-        (const __nv_bfloat16*)q, (__nv_bfloat16*)out, lse, (const __nv_bfloat16*)k_pool,
-        (const __nv_bfloat16*)v_pool, page_table, tok_meta, inl, q_to_kv, total_q_tokens, max_pages, Hq,
-        Hkv, D, P, scale);
-  }
-  return cudaGetLastError();
+  if (dtype == 1)
+    return launch_pdl(attn_simt_kernel<float>, dim3(grid), dim3(kSimtWarps * 32), 0, stream,
+                      (const float*)q, (float*)out, lse, (const float*)k_pool, (const float*)v_pool, page_table,
+                      tok_meta, inl, q_to_kv, total_q_tokens, max_pages, Hq, Hkv, D, P, scale);
+  return launch_pdl(attn_simt_kernel<__nv_bfloat16>, dim3(grid), dim3(kSimtWarps * 32), 0, stream,
+                    (const __nv_bfloat16*)q, (__nv_bfloat16*)out, lse, (const __nv_bfloat16*)k_pool,
+                    (const __nv_bfloat16*)v_pool, page_table, tok_meta, inl, q_to_kv, total_q_tokens, max_pages,
+                    Hq, Hkv, D, P, scale);
 }
 
 }  // namespace ws

@@ -42,6 +42,8 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <type_traits>
+
 #include "kv_append.cuh"
 #include "launch.h"
 #include "sm100_ptx.cuh"
@@ -69,7 +71,8 @@ constexpr int kFirstPieceSteps = 6;                         // P is handed to th
 //    reference the x8-outlier config reached 1.2e-2 max-abs; with this rule it stays at the output's
 //    own rounding).
 constexpr float kFastSumLimit = 1024.0f;
-constexpr float kFastSumShare = 0.5f;
+constexpr float kFastSumShare = 1.0f;
+constexpr int kExactFirstTiles = 2;                         // tiles 0-1 of a segment go straight to the exact path
 // 2 of every 8 exponentials run as a polynomial on the FMA pipe (ex2_poly2); sweep: DESIGN.md section 8
 constexpr int kPolyPer8 = 2;
 
@@ -245,22 +248,45 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   // the first MMA.
   SegView sv_first;
   int32_t si_first = seg_hi, pre_pg0 = 0, pre_pg1 = 0;
+  // Q tiles of segment `sv` -> sQ (general plan: the pair's two tiles; decode plan: the one shared tile)
+  auto issue_q = [&](const SegView& sv) {
+    if constexpr (kAlt) {
+      mbar_arrive_expect_tx(bq_full, kQTileBytes);
+      for (int h = 0; h < 2; ++h)
+        tma_load_3d(sQ + h * kHalfBytes, &tmap_q, bq_full, h * 64, sv.g.kv_head * p.G, sv.g.q_token0);
+    } else {
+      mbar_arrive_expect_tx(bq_full, 2 * kQTileBytes);
+      const int32_t tok0 = sv.g.q_token0 + pair * tok_per_pair;
+      for (int q = 0; q < 2; ++q)
+        for (int h = 0; h < 2; ++h)
+          tma_load_3d(sQ + q * kQTileBytes + h * kHalfBytes, &tmap_q, bq_full, h * 64,
+                      sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
+    }
+  };
   if (warp == 8 && lane == 0) {
+    // the producer owns the Q barriers: initialised here so that the first Q load leaves before the
+    // CTA-wide set-up barrier (the MMA warp first looks at q_full after that barrier)
+    mbar_init(bq_full, 1); mbar_init(bq_empty, 1);
+    fence_mbar_init();
+    fence_proxy_async_smem();
     prefetch_tmap(&tmap_q); prefetch_tmap(&tmap_k); prefetch_tmap(&tmap_v);
     if (p.append_tokens > 0) { prefetch_tmap(&tmap_kn); prefetch_tmap(&tmap_vn); }
     pdl_wait();
     for (si_first = seg_lo; si_first < seg_hi; ++si_first)
       if (load_segment(meta, hdr, si_first, pair, tok_per_pair, sv_first) &&
           sv_first.tile_end > sv_first.tile_begin) break;
-    if (si_first < seg_hi && sv_first.tile_begin * kTileKeys < sv_first.g.cache_len) {
-      const int32_t* page_row = p.page_table + (int64_t)sv_first.g.slot * p.max_pages_per_session;
-      const int32_t last_page = (sv_first.g.cache_len - 1) / p.P;
-      pre_pg0 = page_row[min(2 * sv_first.tile_begin, last_page)];
-      pre_pg1 = page_row[min(2 * sv_first.tile_begin + 1, last_page)];
+    if (si_first < seg_hi) {
+      issue_q(sv_first);
+      if (sv_first.tile_begin * kTileKeys < sv_first.g.cache_len) {
+        const int32_t* page_row = p.page_table + (int64_t)sv_first.g.slot * p.max_pages_per_session;
+        const int32_t last_page = (sv_first.g.cache_len - 1) / p.P;
+        pre_pg0 = page_row[min(2 * sv_first.tile_begin, last_page)];
+        pre_pg1 = page_row[min(2 * sv_first.tile_begin + 1, last_page)];
+      }
     }
   }
   if (warp == 9 && lane == 0) {
-    mbar_init(bq_full, 1); mbar_init(bq_empty, 1); mbar_init(smem_u32(&bars->merge_full), 1);
+    mbar_init(smem_u32(&bars->merge_full), 1);
     bars->njobs = 0;
     for (int s = 0; s < kStages; ++s) { mbar_init(bkv_full(s), 1); mbar_init(bkv_empty(s), 1); }
     for (int q = 0; q < 2; ++q) {
@@ -320,11 +346,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         };
         auto page_of = [&](int32_t logical) { return logical <= 2 * Tc - 1 ? page_row[min(logical, last_page)] : 0; };
         if constexpr (kAlt) {
-          // one Q tile serves both accumulator sets
-          mbar_wait(bq_empty, (q_it & 1) ^ 1);
-          mbar_arrive_expect_tx(bq_full, kQTileBytes);
-          for (int h = 0; h < 2; ++h)
-            tma_load_3d(sQ + h * kHalfBytes, &tmap_q, bq_full, h * 64, sv.g.kv_head * p.G, sv.g.q_token0);
+          // one Q tile serves both accumulator sets (the first segment's was issued during set-up)
+          if (si != si_first) { mbar_wait(bq_empty, (q_it & 1) ^ 1); issue_q(sv); }
           ++q_it;
           auto load_alt = [&](bool is_v, int32_t j) {
             const bool pre = si == si_first && j == sv.tile_begin;   // ids fetched during set-up
@@ -339,14 +362,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           }
           continue;
         }
-        // Q pair (own rows); the page ids of the first tile are fetched while the Q loads are in flight
-        mbar_wait(bq_empty, (q_it & 1) ^ 1);
-        mbar_arrive_expect_tx(bq_full, 2 * kQTileBytes);
-        const int32_t tok0 = sv.g.q_token0 + pair * tok_per_pair;
-        for (int q = 0; q < 2; ++q)
-          for (int h = 0; h < 2; ++h)
-            tma_load_3d(sQ + q * kQTileBytes + h * kHalfBytes, &tmap_q, bq_full, h * 64,
-                        sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
+        // Q pair (own rows); the first segment's was issued during set-up, ahead of the page-id reads
+        if (si != si_first) { mbar_wait(bq_empty, (q_it & 1) ^ 1); issue_q(sv); }
         ++q_it;
         int32_t pg0, pg1;
         if (si == si_first) {
@@ -598,99 +615,140 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const int32_t vis_cache = min(vis, sv.g.cache_len);
       float m_used = -INFINITY, l = 0.f;
 
+      // O and l of this row scaled by alpha (after a change of reference).  Safe whenever the PV MMAs of
+      // the previous tile have completed: s_full of the current tile was committed after them on the same
+      // in-order tensor pipe.
+      auto rescale_o = [&](float alpha) {
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+          uint32_t o[32];
+          tmem_ld32(t_o + ch * 32, o);
+          tmem_wait_ld();
+#pragma unroll
+          for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+          tmem_st32(t_o + ch * 32, o);
+        }
+      };
+      // One unmasked tile exponentiated against the reference m_used while it streams out of TMEM in
+      // 32-column chunks; P is handed to the MMA warp in two pieces (keys 0-95, then 96-127) as soon as
+      // each is written: PV of the first piece (384 tensor cycles) overlaps the softmax of the last 32
+      // keys, and only 128 cycles of PV remain on the S -> softmax -> PV -> S chain.
+      // kCheck: the optimistic use - the reference may be stale, so each piece's row sum is tested against
+      // sum_lim (kFastSumLimit / kFastSumShare; a NaN/inf sum fails the test).  Returns false, with nothing
+      // handed off and S intact, if the first piece fails.
+      auto stream_tile = [&](auto check_tag, float sum_lim) -> bool {
+        constexpr bool kCheck = decltype(check_tag)::value;
+        const float neg_mc = -m_used;
+        uint32_t pk[64];                                    // P row, packed bf16x2
+        uint64_t l01 = 0, l23 = 0;                          // packed fp32x2 partial row sums
+        uint32_t sa[32], sb[32];
+        tmem_ld32(t_s + 0, sa);
+        tmem_wait_ld();
+        tmem_ld32(t_s + 32, sb);
+        softmax_chunk(sa, c, neg_mc, l01, l23, pk + 0);
+        tmem_wait_ld();
+        tmem_ld32(t_s + 64, sa);
+        softmax_chunk(sb, c, neg_mc, l01, l23, pk + 16);
+        tmem_wait_ld();
+        tmem_ld32(t_s + 96, sb);
+        softmax_chunk(sa, c, neg_mc, l01, l23, pk + 32);
+        float la, lb;
+        unpack_f32x2(add_f32x2(l01, l23), la, lb);
+        const float sum_a = la + lb;
+        if (kCheck && __any_sync(0xffffffffu, !(sum_a < sum_lim))) return false;
+        tmem_st32(t_s + 0, pk);
+        tmem_st16(t_s + 32, pk + 32);
+        tmem_wait_st();
+        tc_fence_before();
+        mbar_arrive(bp_full(q, 0));                         // first 96 keys of P handed off
+        tmem_wait_ld();
+        l01 = 0; l23 = 0;
+        softmax_chunk(sb, c, neg_mc, l01, l23, pk + 48);
+        unpack_f32x2(add_f32x2(l01, l23), la, lb);
+        const float sum_b = la + lb;
+        l += sum_a;
+        if (!kCheck || !__any_sync(0xffffffffu, !(sum_b < sum_lim))) {
+          l += sum_b;
+        } else {
+          // Rare: the last 32 keys fail the test after the first piece was handed off.  Wait until
+          // PV of the first piece has completed (O is then quiescent: the PV of the last piece needs
+          // our arrival), re-reference O and l to the exact maximum if it grew and redo the last 32
+          // keys exactly.
+          mbar_wait(bpv_h0(q), tile_it & 1);
+          tc_fence_after();
+          uint32_t sr[32];
+          tmem_ld32(t_s + 96, sr);
+          tmem_wait_ld();
+          float mx = __uint_as_float(sr[0]);
+#pragma unroll
+          for (int i = 1; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sr[i]));
+          const float tm = mx * c;
+          float alpha = 1.f;
+          if (tm > m_used) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
+          rescale_o(alpha);
+          float ls = 0.f;
+#pragma unroll
+          for (int i = 0; i < 32; i += 2) {
+            const float p0 = ex2_approx(fmaf(__uint_as_float(sr[i]), c, -m_used));
+            const float p1 = ex2_approx(fmaf(__uint_as_float(sr[i + 1]), c, -m_used));
+            ls += p0 + p1;
+            pk[48 + i / 2] = pack_bf16x2(p0, p1);
+          }
+          l += ls;
+        }
+        tmem_st16(t_s + 48, pk + 48);
+        tmem_wait_st();
+        tc_fence_before();
+        mbar_arrive(bp_full(q, 1));
+        return true;
+      };
+
       for (int32_t j = 0; j < nt; ++j) {
         const int32_t t = sv.tile_begin + (kAlt ? 2 * j + q : j);
         const int32_t key0 = t < Tc ? t * kTileKeys : sv.g.cache_len + (t - Tc) * kTileKeys;
         const int32_t lim = t < Tc ? vis_cache : vis;        // keys >= lim of this tile are masked
         mbar_wait(bs_full(q), tile_it & 1);
         tc_fence_after();
-        uint32_t pk[64];                                    // P row, packed bf16x2
         const bool need_mask = __any_sync(0xffffffffu, key0 + kTileKeys > lim);
         bool done = false;
-        // (rows whose reference is still -inf, i.e. nothing visible so far, also take the exact path)
-        if (j > 0 && !need_mask && !__any_sync(0xffffffffu, m_used == -INFINITY)) {
-          // ---- fast path (optimistic): exponentiate against the running reference m_used while
-          // the tile streams out of TMEM in 32-column chunks.  Each piece (keys 0-95, keys 96-127) is
-          // checked against the two limits described at kFastSumLimit / kFastSumShare (a NaN/inf sum
-          // fails the test) and handed to the MMA warp as soon as it is written: PV of the first piece
-          // (384 tensor cycles) overlaps the softmax of the last 32 keys, and only 128 cycles of PV
-          // remain on the S -> softmax -> PV -> S chain.
-          const float neg_mc = -m_used;
-          const float sum_lim = fminf(kFastSumLimit, kFastSumShare * l);
-          uint64_t l01 = 0, l23 = 0;                        // packed fp32x2 partial row sums
-          uint32_t sa[32], sb[32];
-          tmem_ld32(t_s + 0, sa);
-          tmem_wait_ld();
-          tmem_ld32(t_s + 32, sb);
-          softmax_chunk(sa, c, neg_mc, l01, l23, pk + 0);
-          tmem_wait_ld();
-          tmem_ld32(t_s + 64, sa);
-          softmax_chunk(sb, c, neg_mc, l01, l23, pk + 16);
-          tmem_wait_ld();
-          tmem_ld32(t_s + 96, sb);
-          softmax_chunk(sa, c, neg_mc, l01, l23, pk + 32);
-          float la, lb;
-          unpack_f32x2(add_f32x2(l01, l23), la, lb);
-          const float sum_a = la + lb;
-          if (!__any_sync(0xffffffffu, !(sum_a < sum_lim))) {
-            tmem_st32(t_s + 0, pk);
-            tmem_st16(t_s + 32, pk + 32);
-            tmem_wait_st();
-            tc_fence_before();
-            mbar_arrive(bp_full(q, 0));                     // first 96 keys of P handed off
+        // ---- optimistic path: no look at the tile's maximum.  Not tried on the first tiles of a segment
+        // (their sums are of the order of the accumulated l: the share test would refuse them anyway) nor
+        // while a row has seen nothing yet (reference still -inf).
+        if (j >= kExactFirstTiles && !need_mask && !__any_sync(0xffffffffu, m_used == -INFINITY))
+          done = stream_tile(std::true_type{}, fminf(kFastSumLimit, kFastSumShare * l));
+        if (!done && !need_mask) {
+          // ---- exact path, unmasked tile: one pass over S for the row maximum, the reference follows
+          // it whenever it grew (the row's largest weight so far is then p = 1, exactly representable in
+          // bf16), then the same streaming pass as above against the now exact reference.
+          float mx0, mx1, mx2, mx3;
+#pragma unroll
+          for (int ch = 0; ch < 4; ++ch) {
+            uint32_t sr[32];
+            tmem_ld32(t_s + ch * 32, sr);
             tmem_wait_ld();
-            l01 = 0; l23 = 0;
-            softmax_chunk(sb, c, neg_mc, l01, l23, pk + 48);
-            unpack_f32x2(add_f32x2(l01, l23), la, lb);
-            const float sum_b = la + lb;
-            l += sum_a;
-            if (!__any_sync(0xffffffffu, !(sum_b < sum_lim))) {
-              l += sum_b;
-            } else {
-              // Rare: the last 32 keys fail the test after the first piece was handed off.  Wait until
-              // PV of the first piece has completed (O is then quiescent: the PV of the last piece needs
-              // our arrival), re-reference O and l to the exact maximum if it grew and redo the last 32
-              // keys exactly.
-              mbar_wait(bpv_h0(q), tile_it & 1);
-              tc_fence_after();
-              uint32_t sr[32];
-              tmem_ld32(t_s + 96, sr);
-              tmem_wait_ld();
-              float mx = __uint_as_float(sr[0]);
+            if (ch == 0) { mx0 = __uint_as_float(sr[0]); mx1 = __uint_as_float(sr[1]); mx2 = __uint_as_float(sr[2]); mx3 = __uint_as_float(sr[3]); }
 #pragma unroll
-              for (int i = 1; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sr[i]));
-              const float tm = mx * c;
-              float alpha = 1.f;
-              if (tm > m_used) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
-#pragma unroll
-              for (int ch = 0; ch < 4; ++ch) {
-                uint32_t o[32];
-                tmem_ld32(t_o + ch * 32, o);
-                tmem_wait_ld();
-#pragma unroll
-                for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-                tmem_st32(t_o + ch * 32, o);
-              }
-              float ls = 0.f;
-#pragma unroll
-              for (int i = 0; i < 32; i += 2) {
-                const float p0 = ex2_approx(fmaf(__uint_as_float(sr[i]), c, -m_used));
-                const float p1 = ex2_approx(fmaf(__uint_as_float(sr[i + 1]), c, -m_used));
-                ls += p0 + p1;
-                pk[48 + i / 2] = pack_bf16x2(p0, p1);
-              }
-              l += ls;
+            for (int i = (ch == 0 ? 4 : 0); i < 32; i += 4) {
+              mx0 = fmaxf(mx0, __uint_as_float(sr[i])); mx1 = fmaxf(mx1, __uint_as_float(sr[i + 1]));
+              mx2 = fmaxf(mx2, __uint_as_float(sr[i + 2])); mx3 = fmaxf(mx3, __uint_as_float(sr[i + 3]));
             }
-            tmem_st16(t_s + 48, pk + 48);
-            tmem_wait_st();
-            tc_fence_before();
-            mbar_arrive(bp_full(q, 1));
-            done = true;
           }
+          const float tm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;
+          const bool grow = tm > m_used;
+          if (j == 0) {
+            m_used = tm;
+          } else if (__any_sync(0xffffffffu, grow)) {
+            float alpha = 1.f;
+            if (grow) { alpha = m_used == -INFINITY ? 0.f : ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
+            rescale_o(alpha);
+          }
+          stream_tile(std::false_type{}, 0.f);
+          done = true;
         }
         if (!done) {
-          // ---- exact path: first tile of a segment, masked tiles, tiles that may carry a large share of
-          // the row's weight (nothing has been handed off yet in that case)
+          // ---- exact path, masked tile (the last tile of the cache part or of the new block when their
+          // lengths are no multiples of 128; multi-block queries): whole S row in registers
+          uint32_t pk[64];
           uint32_t sr[128];                                 // one whole S row (fp32 bits)
           tmem_ld32(t_s + 0, sr + 0);
           tmem_ld32(t_s + 32, sr + 32);
@@ -698,11 +756,9 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           tmem_ld32(t_s + 96, sr + 96);
           tmem_wait_ld();
 #define S_(i) __uint_as_float(sr[i])
-          if (need_mask) {
 #pragma unroll
-            for (int i = 0; i < 128; ++i)
-              if (key0 + i >= lim) sr[i] = 0xff800000u;     // -inf
-          }
+          for (int i = 0; i < 128; ++i)
+            if (key0 + i >= lim) sr[i] = 0xff800000u;       // -inf
           float mx0 = S_(0), mx1 = S_(1), mx2 = S_(2), mx3 = S_(3);
 #pragma unroll
           for (int i = 4; i < 128; i += 4) {
@@ -710,25 +766,13 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             mx2 = fmaxf(mx2, S_(i + 2)); mx3 = fmaxf(mx3, S_(i + 3));
           }
           const float tm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;
-          // the reference follows the exact running maximum on this path: the row's largest weight so
-          // far is then p = 1, exactly representable in bf16
           const bool grow = tm > m_used;
           if (j == 0) {
             m_used = tm;
           } else if (__any_sync(0xffffffffu, grow)) {
-            // rescale O and l (PV of the previous tile has completed: s_full was committed after it on
-            // the same in-order tensor pipe)
             float alpha = 1.f;
-            if (grow) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
-#pragma unroll
-            for (int ch = 0; ch < 4; ++ch) {
-              uint32_t o[32];
-              tmem_ld32(t_o + ch * 32, o);
-              tmem_wait_ld();
-#pragma unroll
-              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-              tmem_st32(t_o + ch * 32, o);
-            }
+            if (grow) { alpha = m_used == -INFINITY ? 0.f : ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
+            rescale_o(alpha);
           }
           const float m_c = (m_used == -INFINITY) ? 0.f : m_used;
           float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;

@@ -56,3 +56,20 @@ def test_two_rank_replicas_gloo():
     assert ms0 == ms1 == 20.0                                      # MAX over ranks
     want = 4.0 * 128 * 32 * 256 * (t0 + t1)
     assert tot0 == tot1 == pytest.approx(want)                     # SUM over ranks
+
+
+def test_bench_gpus_n_spawns_its_own_ranks():
+    """`python bench.py --gpus 2` with no launcher (WORLD_SIZE unset) re-executes itself under
+    torch.distributed.run with 2 ranks; --selftest-cpu runs the rendezvous / barrier / max-and-sum-over-ranks
+    plumbing on gloo with made-up per-rank timings (rank r: 10 + r ms, 1e12 flops) and rank 0 prints one line."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--selftest-cpu"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    d = json.loads(lines[0])
+    assert d["selftest"] and d["n_gpus"] == 2
+    assert d["ms_max_over_ranks"] == 11.0 and d["flops_sum_over_ranks"] == 2e12
