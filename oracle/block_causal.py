@@ -28,6 +28,16 @@ attend(Q for the last m blocks):  for every query row r in block b and q-head h,
     O[r,h,:] = sum_j (p_j / Z) * Vc[j,g,:] ;  LSE[r,h] = m + log Z
 The matrix products use numpy's float64 matmul as the library primitive; there is no tiling, no
 online-softmax recurrence and no reordering beyond that.
+
+Mixed intra-block mask (NEXT-4, `text_causal=True`; reading A19).  The thinker "runs the short
+token-causal Transformer pass for language prediction and state update" / "token-causal
+decoding over the language and state slots" while audio/video stay block-wise.  Reading:
+with per-token modality tags (0 video, 1 audio, 2 text) the visible set becomes
+    V(r) = { j : j < e_b  and not ( tag(r) == text and tag(j) == text and j > pos(r) ) }
+i.e. text slots are token-causal AMONG THEMSELVES (a text query never sees a later text key, which by
+j < e_b can only be one of its own block), every other (query, key) pair keeps the block-causal rule:
+audio/video keys of the block are visible to every query of the block, text keys are visible to every
+audio/video query of the block.  A query always sees itself, so no row is empty.
 """
 from __future__ import annotations
 
@@ -44,19 +54,31 @@ class OracleSession:
         self.k_slices: List[np.ndarray] = []     # storage-dtype slices exactly as appended
         self.v_slices: List[np.ndarray] = []
         self.block_ends: List[int] = [0]
+        self.tags: List[np.ndarray] = []         # per-slice modality tags (uint8) or None
 
     @property
     def length(self) -> int:
         return self.block_ends[-1]
 
-    def append(self, k_new: np.ndarray, v_new: np.ndarray) -> None:
-        """Commit one block: history <- [history; slice]; records e_{B+1} = L + n."""
+    def append(self, k_new: np.ndarray, v_new: np.ndarray, modality: Optional[Sequence[int]] = None) -> None:
+        """Commit one block: history <- [history; slice]; records e_{B+1} = L + n.
+        modality: optional per-token tags (0 video, 1 audio, 2 text), metadata for `text_causal`."""
         assert k_new.shape == v_new.shape and k_new.ndim == 3
         n, Hkv, D = k_new.shape
         assert n > 0 and (Hkv, D) == (self.Hkv, self.D)
         self.k_slices.append(np.array(k_new, copy=True))
         self.v_slices.append(np.array(v_new, copy=True))
         self.block_ends.append(self.length + n)
+        if modality is not None:
+            modality = np.asarray(modality, dtype=np.uint8)
+            assert modality.shape == (n,)
+        self.tags.append(modality)
+
+    def text_mask(self) -> np.ndarray:
+        """is_text[j] for every committed token j (tokens appended without tags count as non-text)."""
+        parts = [np.zeros(len(k), dtype=bool) if t is None else (t == 2)
+                 for k, t in zip(self.k_slices, self.tags)]
+        return np.concatenate(parts) if parts else np.zeros(0, dtype=bool)
 
     def gather(self, start: int = 0, count: Optional[int] = None) -> Tuple[np.ndarray, np.ndarray]:
         """Logical tokens [start, start+count) of the committed history, storage dtype."""
@@ -77,7 +99,7 @@ def default_q_to_kv(num_q_heads: int, num_kv_heads: int) -> np.ndarray:
 def attend(sess: OracleSession, q: np.ndarray, scale: float, num_q_blocks: int = 1,
            q_to_kv: Optional[Sequence[int]] = None,
            rows: Optional[Sequence[int]] = None,
-           heads: Optional[Sequence[int]] = None, want_abs: bool = False):
+           heads: Optional[Sequence[int]] = None, want_abs: bool = False, text_causal: bool = False):
     """Block-causal attention of the LAST `num_q_blocks` committed blocks against the history.
 
     q: [n_q, Hq, D] (n_q = total tokens of those blocks, storage dtype, widened to float64 here).
@@ -87,6 +109,8 @@ def attend(sess: OracleSession, q: np.ndarray, scale: float, num_q_blocks: int =
     want_abs: additionally return A[r,h,:] = sum_j (p_j / Z) * |Vc[j,g,:]| (same weights, |V| instead
     of V): the condition number of the output w.r.t. relative perturbations of the weights, used by the
     tests to state the bf16 error bound of DESIGN.md reading A10 (|O| <= A, with equality for V >= 0).
+    text_causal: the mixed intra-block mask of the module docstring (reading A19): a text query does not
+    see text keys at later positions; everything else as above.
     """
     B = len(sess.block_ends) - 1
     assert 1 <= num_q_blocks <= B
@@ -107,6 +131,7 @@ def attend(sess: OracleSession, q: np.ndarray, scale: float, num_q_blocks: int =
     ends = np.asarray(sess.block_ends)
     blk = np.searchsorted(ends, abs_pos, side="right")        # e_{blk-1} <= pos < e_blk
     vis_end = ends[blk]
+    is_text = sess.text_mask() if text_causal else None
     for g in np.unique(g_of[heads]):
         Kg = Kc[:, g, :].astype(np.float64)
         Vg = Vc[:, g, :].astype(np.float64)
@@ -117,6 +142,11 @@ def attend(sess: OracleSession, q: np.ndarray, scale: float, num_q_blocks: int =
                 sel = np.nonzero(vis_end == e)[0]
                 Q = q[rows[sel], h, :].astype(np.float64)
                 S = scale * (Q @ Kg[:e].T)                      # s_j for all visible j < e_b
+                if text_causal:
+                    # text query at position pos: text keys j > pos are not visible (score -inf, weight 0)
+                    pos = abs_pos[sel]
+                    hidden = (is_text[pos][:, None] & is_text[None, :e]) & (np.arange(e)[None, :] > pos[:, None])
+                    S = np.where(hidden, -np.inf, S)
                 m = S.max(axis=1, keepdims=True)
                 P = np.exp(S - m)
                 Z = P.sum(axis=1, keepdims=True)

@@ -14,11 +14,14 @@ from typing import List, Sequence
 
 
 def dense_block_causal(q, k, v, block_sizes: Sequence[int], scale: float,
-                       q_to_kv: Sequence[int] = None, mask_kind: str = "block_causal"):
+                       q_to_kv: Sequence[int] = None, mask_kind: str = "block_causal",
+                       tags: Sequence[int] = None):
     """q: [T][Hq][D], k/v: [T][Hkv][D] nested sequences / arrays.  Returns (O [T][Hq][D], LSE [T][Hq]).
 
     mask_kind: "block_causal" (the method), or the two WRONG readings used by the pin tests to
-    show the hand example separates them: "token_causal" (j <= i) and "none" (all visible).
+    show the hand example separates them: "token_causal" (j <= i) and "none" (all visible);
+    "text_causal" = the mixed intra-block mask of NEXT-4 (reading A19): block-causal,
+    except that a text token (tags[i] == 2) does not see text tokens at later positions.
     """
     T = len(q); Hq = len(q[0]); D = len(q[0][0]); Hkv = len(k[0])
     assert sum(block_sizes) == T
@@ -30,6 +33,10 @@ def dense_block_causal(q, k, v, block_sizes: Sequence[int], scale: float,
     kv_of = [h // G for h in range(Hq)] if q_to_kv is None else list(q_to_kv)
     if mask_kind == "block_causal":
         M = [[blk[j] <= blk[i] for j in range(T)] for i in range(T)]
+    elif mask_kind == "text_causal":
+        assert tags is not None and len(tags) == T
+        M = [[blk[j] <= blk[i] and not (tags[i] == 2 and tags[j] == 2 and j > i) for j in range(T)]
+             for i in range(T)]
     elif mask_kind == "token_causal":
         M = [[j <= i for j in range(T)] for i in range(T)]
     elif mask_kind == "none":

@@ -377,3 +377,96 @@ def test_abs_weighted_output_pins():
     o0, _, a0 = attend(s0, Q, 1.0, want_abs=True)
     np.testing.assert_allclose(o0[:, 0], [[1 / 3, -2 / 3]] * 2, atol=1e-15)
     np.testing.assert_allclose(a0[:, 0], [[1 / 3, 2 / 3]] * 2, atol=1e-15)
+
+
+# ---------------------------------------------------------------- NEXT-4: text-causal mixed mask (reading A19)
+def _tc_run(q, k, v, block_sizes, tags, scale, one_shot, q_to_kv=None):
+    """Oracle with text_causal=True, either block by block (hot path) or all blocks in one query."""
+    sess = OracleSession(k.shape[1], k.shape[2])
+    tags = np.asarray(tags, dtype=np.uint8)
+    outs, lses, pos = [], [], 0
+    for sz in block_sizes:
+        sess.append(k[pos:pos + sz], v[pos:pos + sz], modality=tags[pos:pos + sz])
+        if not one_shot:
+            o, l = attend(sess, q[pos:pos + sz], scale, 1, q_to_kv, text_causal=True)
+            outs.append(o); lses.append(l)
+        pos += sz
+    if one_shot:
+        return attend(sess, q, scale, len(block_sizes), q_to_kv, text_causal=True)
+    return np.concatenate(outs), np.concatenate(lses)
+
+
+def _p7_inputs():
+    a = np.arange(1.0, 7.0)
+    q = np.tile(np.array([1.0, 0.0]), (6, 1, 1))
+    k = np.stack([np.log(a), np.zeros(6)], axis=1)[:, None, :]
+    v = np.array([[1.0, 0.0], [0.0, 1.0], [2.0, 0.0], [0.0, 2.0], [3.0, 0.0], [0.0, 3.0]])[:, None, :]
+    return q, k, v, [3, 3], [0, 2, 2, 2, 2, 1]
+
+
+def test_p7_text_causal_hand_example():
+    """tests/golden/p7_text_causal_hand_example.txt (hand-derived): oracle (incremental and one-shot) and the
+    brute-force dense mask agree with it; plain block-causal and token-causal do not."""
+    gold = _load("p7_text_causal_hand_example.txt")
+    q, k, v, blocks, tags = _p7_inputs()
+    for one_shot in (False, True):
+        o, lse = _tc_run(q, k, v, blocks, tags, 1.0, one_shot)
+        np.testing.assert_allclose(o[:, 0, :], gold[:, 1:3], rtol=0, atol=1e-15)
+        np.testing.assert_allclose(np.exp(lse[:, 0]), gold[:, 3], rtol=1e-14)
+    o_bf, lse_bf = dense_block_causal(q, k, v, blocks, 1.0, mask_kind="text_causal", tags=tags)
+    np.testing.assert_allclose(np.array(o_bf)[:, 0, :], gold[:, 1:3], atol=1e-15)
+    np.testing.assert_allclose(np.exp(np.array(lse_bf)[:, 0]), gold[:, 3], rtol=1e-14)
+    o_bc, _ = _one_shot(q, k, v, blocks, 1.0)
+    assert abs(o_bc[1, 0, 0] - gold[1, 1]) > 0.5 and abs(o_bc[3, 0, 0] - gold[3, 1]) > 0.5
+    o_tok, _ = dense_block_causal(q, k, v, blocks, 1.0, mask_kind="token_causal")
+    assert abs(o_tok[0][0][0] - gold[0, 1]) > 0.1
+
+
+@pytest.mark.parametrize("blocks,Hq,Hkv,D", [([5, 3, 7], 2, 1, 4), ([1, 6, 2, 4], 4, 2, 3), ([9], 1, 1, 5)])
+def test_text_causal_vs_brute_force_random_tiny(blocks, Hq, Hkv, D):
+    q, k, v = _stream(blocks, Hq, Hkv, D, seed=71)
+    rng = np.random.default_rng(72)
+    tags = rng.integers(0, 3, size=sum(blocks))
+    o_bf, lse_bf = dense_block_causal(q, k, v, blocks, 0.4, mask_kind="text_causal", tags=list(tags))
+    for one_shot in (False, True):
+        o, lse = _tc_run(q, k, v, blocks, tags, 0.4, one_shot)
+        np.testing.assert_allclose(o, np.array(o_bf), rtol=1e-12, atol=1e-13)
+        np.testing.assert_allclose(lse, np.array(lse_bf), rtol=1e-12, atol=1e-13)
+
+
+def test_text_causal_without_text_tokens_is_block_causal_bit_identical():
+    blocks = [4, 6, 3]
+    q, k, v = _stream(blocks, 2, 2, 8, seed=73)
+    tags = np.random.default_rng(74).integers(0, 2, size=sum(blocks))      # video / audio only
+    o, lse = _tc_run(q, k, v, blocks, tags, 0.3, True)
+    o_ref, lse_ref = _one_shot(q, k, v, blocks, 0.3)
+    assert o.tobytes() == o_ref.tobytes() and lse.tobytes() == lse_ref.tobytes()
+
+
+def test_text_causal_all_text_single_block_is_causal_sdpa():
+    """Library pin: one block whose tokens are all text = standard causal attention."""
+    q, k, v = _stream([23], 3, 3, 16, seed=75)
+    o, _ = _tc_run(q, k, v, [23], [2] * 23, 0.25, True)
+    np.testing.assert_allclose(o, _sdpa(q, k, v, 0.25, True), rtol=1e-10, atol=1e-12)
+    # ... and all-text blocks of any sizes are token-causal too (text never sees later text)
+    o2, _ = _tc_run(q, k, v, [5, 11, 7], [2] * 23, 0.25, False)
+    np.testing.assert_allclose(o2, _sdpa(q, k, v, 0.25, True), rtol=1e-10, atol=1e-12)
+
+
+def test_text_causal_dependence_structure():
+    """Perturbing a LATER text token of the block changes the A/V rows and the later text rows of that block,
+    and leaves earlier text rows bit-identical; perturbing a later A/V token changes every row of the block."""
+    blocks, tags = [8], [0, 2, 1, 2, 0, 2, 1, 2]
+    q, k, v = _stream(blocks, 2, 1, 8, seed=76)
+    o0, _ = _tc_run(q, k, v, blocks, tags, 0.5, True)
+    k2, v2 = k.copy(), v.copy()
+    k2[5] += 1.0; v2[5] -= 2.0                                  # text token at position 5
+    o1, _ = _tc_run(q, k2, v2, blocks, tags, 0.5, True)
+    for r in (1, 3):                                           # earlier text rows: unchanged
+        assert o1[r].tobytes() == o0[r].tobytes()
+    for r in (0, 2, 4, 5, 6, 7):                               # A/V rows, the token itself, later text
+        assert np.abs(o1[r] - o0[r]).max() > 1e-6
+    k3, v3 = k.copy(), v.copy()
+    k3[6] += 1.0; v3[6] -= 2.0                                  # audio token at position 6
+    o2, _ = _tc_run(q, k3, v3, blocks, tags, 0.5, True)
+    assert all(np.abs(o2[r] - o0[r]).max() > 1e-6 for r in range(8))
