@@ -131,6 +131,18 @@ ws_status_t ws_kv_append(ws_cache_t* cache, int32_t num_sessions, const int32_t*
                          const int32_t* cu_new_tokens, const void* k_new, const void* v_new,
                          const uint8_t* modality, void* cuda_stream);
 
+/* NEXT-1 - commit SEVERAL blocks per session in one call (system prefill, "After system
+ * prefill, the thinker broadcasts the initial KV cache": the whole initial history is built in one shot;
+ * the same causal format in one pass).  Exactly ws_kv_append, except that session s's
+ * n_s = cu[s+1] - cu[s] tokens are committed as the blocks block_tokens[cu_blocks[s] .. cu_blocks[s+1]) (each
+ * >= 1 token, their sum must be n_s): one block end is recorded per block, in order.  One host pass, one
+ * kernel launch, bit-exact.  cu_blocks: HOST [S+1] (cu_blocks[0] = 0); block_tokens: HOST [cu_blocks[S]].
+ * The blocks can then be queried together with ws_block_causal_attn_fwd(num_q_blocks = their count). */
+ws_status_t ws_kv_append_blocks(ws_cache_t* cache, int32_t num_sessions, const int32_t* session_ids,
+                                const int32_t* cu_new_tokens, const int32_t* cu_blocks,
+                                const int32_t* block_tokens, const void* k_new, const void* v_new,
+                                const uint8_t* modality, void* cuda_stream);
+
 /* a3 (+a4) - block-causal attention forward.  For each listed session the queries are the tokens of
  * its LAST num_q_blocks[s] committed blocks (1 on the hot path: the block just appended).  A query
  * row in block b sees keys j < e_b: its whole own block and every earlier block.
@@ -144,6 +156,21 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* cache, int32_t num_sessions,
                                      const int32_t* cu_q_tokens, const void* q, void* out,
                                      float* lse, float scale, void* cuda_stream);
 
+/* NEXT-4 (optional half) - mixed intra-block mask.  PAPER.md:31 "the short token-causal Transformer pass
+ * for language prediction and state update", :77 "token-causal decoding over the language and state
+ * slots", while audio/video units are block-wise.  Reading A19: with
+ * WS_ATTN_TEXT_CAUSAL the text slots (modality tag 2) are token-causal AMONG THEMSELVES - a text query
+ * does not see text keys at later positions (those can only be in its own block) - and every other
+ * (query, key) pair keeps the block-causal rule: audio/video keys of the block are visible to every query
+ * of the block, text keys to every audio/video query.  attn_flags = 0 is ws_block_causal_attn_fwd.
+ * Every queried token must have been appended WITH a modality tag (else WS_ERR_INVALID_ARG). */
+enum { WS_ATTN_TEXT_CAUSAL = 1u };
+ws_status_t ws_block_causal_attn_fwd_masked(ws_cache_t* cache, int32_t num_sessions,
+                                            const int32_t* session_ids, const int32_t* num_q_blocks,
+                                            const int32_t* cu_q_tokens, const void* q, void* out,
+                                            float* lse, float scale, uint32_t attn_flags,
+                                            void* cuda_stream);
+
 /* One streaming-unit step with DEVICE buffers in a single call: ws_kv_append(k_new, v_new) followed by
  * ws_block_causal_attn_fwd of the block just committed (one block per session, n_q = n_new; PAPER.md:83
  * "appends the received KV slice", then the unit attends).  Same kernels and results as the two calls;
@@ -152,6 +179,13 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* cache, int32_t num_sessions,
 ws_status_t ws_stream_step(ws_cache_t* cache, int32_t num_sessions, const int32_t* session_ids,
                            const int32_t* cu_new_tokens, const void* q, const void* k_new,
                            const void* v_new, void* out, float* lse, float scale, void* cuda_stream);
+
+/* ws_stream_step with the block's modality tags (HOST [cu[S]], stored like ws_kv_append's; may be NULL when
+ * attn_flags = 0) and the attention flags of ws_block_causal_attn_fwd_masked. */
+ws_status_t ws_stream_step_tagged(ws_cache_t* cache, int32_t num_sessions, const int32_t* session_ids,
+                                  const int32_t* cu_new_tokens, const void* q, const void* k_new,
+                                  const void* v_new, const uint8_t* modality, uint32_t attn_flags,
+                                  void* out, float* lse, float scale, void* cuda_stream);
 
 /* One streaming-unit step with HOST buffers (the end-to-end path): copies q/k_new/v_new from host
  * (pinned for async copies) into `staging` (DEVICE, >= ws_step_staging_bytes(n_total); two slots used

@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_PKG, "libwanstream.so")
 
 WS_BF16, WS_F32 = 0, 1
 WS_FLAG_DRY_RUN, WS_FLAG_FORCE_SIMT, WS_FLAG_FUSED_COMBINE, WS_FLAG_SEPARATE_APPEND = 1, 2, 8, 16
+WS_ATTN_TEXT_CAUSAL = 1
 STATUS_NAMES = ["WS_OK", "WS_ERR_INVALID_ARG", "WS_ERR_BAD_SESSION", "WS_ERR_OUT_OF_PAGES",
                 "WS_ERR_UNSUPPORTED", "WS_ERR_WORKSPACE_TOO_SMALL", "WS_ERR_CUDA"]
 
@@ -59,8 +60,8 @@ EXPORTS = ["ws_replica_link", "ws_replica_accept", "ws_replica_commit_message",
            "ws_replica_snapshot_message", "ws_replica_push_session", "ws_replica_apply",
            "ws_ipc_export", "ws_ipc_open", "ws_ipc_close", "ws_pool_bytes", "ws_workspace_bytes", "ws_cache_create", "ws_cache_destroy",
            "ws_session_open", "ws_session_close", "ws_session_info", "ws_session_truncate",
-           "ws_free_pages", "ws_kv_append", "ws_block_causal_attn_fwd", "ws_step_staging_bytes",
-           "ws_stream_step", "ws_stream_step_host", "ws_stream_host_join", "ws_fm_euler_update", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
+           "ws_free_pages", "ws_kv_append", "ws_kv_append_blocks", "ws_block_causal_attn_fwd", "ws_step_staging_bytes",
+           "ws_stream_step", "ws_stream_step_tagged", "ws_block_causal_attn_fwd_masked", "ws_stream_step_host", "ws_stream_host_join", "ws_fm_euler_update", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
            "ws_debug_set_min_splits", "ws_debug_set_decode_plan", "ws_last_plan_info", "ws_last_plan_segment",
            "ws_launch_count", "ws_debug_kernel_timing", "ws_debug_read_kernel_times",
            "ws_status_str", "ws_last_error", "ws_version"]
@@ -90,8 +91,13 @@ def load_library() -> C.CDLL:
     lib.ws_session_truncate.argtypes = [vp, C.c_int32, C.c_int32]
     lib.ws_free_pages.argtypes = [vp]; lib.ws_free_pages.restype = C.c_int32
     lib.ws_kv_append.argtypes = [vp, C.c_int32, i32p, i32p, vp, vp, C.POINTER(C.c_uint8), vp]
+    lib.ws_kv_append_blocks.argtypes = [vp, C.c_int32, i32p, i32p, i32p, i32p, vp, vp, C.POINTER(C.c_uint8), vp]
     lib.ws_block_causal_attn_fwd.argtypes = [vp, C.c_int32, i32p, i32p, i32p, vp, vp, vp,
                                              C.c_float, vp]
+    lib.ws_block_causal_attn_fwd_masked.argtypes = [vp, C.c_int32, i32p, i32p, i32p, vp, vp, vp,
+                                                    C.c_float, C.c_uint32, vp]
+    lib.ws_stream_step_tagged.argtypes = [vp, C.c_int32, i32p, i32p, vp, vp, vp, C.POINTER(C.c_uint8),
+                                          C.c_uint32, vp, vp, C.c_float, vp]
     lib.ws_step_staging_bytes.restype = C.c_size_t
     lib.ws_step_staging_bytes.argtypes = [cfgp, C.c_int32]
     lib.ws_stream_step.argtypes = [vp, C.c_int32, i32p, i32p, vp, vp, vp, vp, vp, C.c_float, vp]
@@ -253,15 +259,44 @@ class Cache:
                                      _i32(cu_new_tokens), _ptr(k_new), _ptr(v_new), mod,
                                      _stream_ptr(stream)))
 
+    def kv_append_blocks(self, session_ids, cu_new_tokens, cu_blocks, block_tokens, k_new, v_new,
+                         modality=None, stream=None):
+        """ws_kv_append_blocks: several blocks per session committed by one call / one launch (NEXT-1)."""
+        mod = None
+        if modality is not None:
+            m = np.ascontiguousarray(np.asarray(modality, dtype=np.uint8))
+            mod = (C.c_uint8 * len(m)).from_buffer_copy(m.tobytes())
+        _check(self.lib.ws_kv_append_blocks(self.handle, len(session_ids), _i32(session_ids),
+                                            _i32(cu_new_tokens), _i32(cu_blocks), _i32(block_tokens),
+                                            _ptr(k_new), _ptr(v_new), mod, _stream_ptr(stream)))
+
     def block_causal_attn_fwd(self, session_ids, cu_q_tokens, q, out, scale: float, lse=None,
-                              num_q_blocks=None, stream=None):
+                              num_q_blocks=None, stream=None, attn_flags: int = 0):
+        """attn_flags != 0: ws_block_causal_attn_fwd_masked (WS_ATTN_TEXT_CAUSAL)."""
         nqb = _i32(num_q_blocks) if num_q_blocks is not None else None
+        if attn_flags:
+            _check(self.lib.ws_block_causal_attn_fwd_masked(self.handle, len(session_ids), _i32(session_ids),
+                                                            nqb, _i32(cu_q_tokens), _ptr(q), _ptr(out), _ptr(lse),
+                                                            C.c_float(scale), attn_flags, _stream_ptr(stream)))
+            return
         _check(self.lib.ws_block_causal_attn_fwd(self.handle, len(session_ids), _i32(session_ids),
                                                  nqb, _i32(cu_q_tokens), _ptr(q), _ptr(out),
                                                  _ptr(lse), C.c_float(scale), _stream_ptr(stream)))
 
-    def stream_step(self, session_ids, cu_new_tokens, q, k_new, v_new, out, scale: float, lse=None, stream=None):
-        """ws_kv_append + ws_block_causal_attn_fwd of the block just committed, one call (device buffers)."""
+    def stream_step(self, session_ids, cu_new_tokens, q, k_new, v_new, out, scale: float, lse=None, stream=None,
+                    modality=None, attn_flags: int = 0):
+        """ws_kv_append + ws_block_causal_attn_fwd of the block just committed, one call (device buffers).
+        modality / attn_flags: ws_stream_step_tagged."""
+        if modality is not None or attn_flags:
+            mod = None
+            if modality is not None:
+                m = np.ascontiguousarray(np.asarray(modality, dtype=np.uint8))
+                mod = (C.c_uint8 * len(m)).from_buffer_copy(m.tobytes())
+            _check(self.lib.ws_stream_step_tagged(self.handle, len(session_ids), _i32(session_ids),
+                                                  _i32(cu_new_tokens), _ptr(q), _ptr(k_new), _ptr(v_new), mod,
+                                                  attn_flags, _ptr(out), _ptr(lse), C.c_float(scale),
+                                                  _stream_ptr(stream)))
+            return
         _check(self.lib.ws_stream_step(self.handle, len(session_ids), _i32(session_ids), _i32(cu_new_tokens),
                                        _ptr(q), _ptr(k_new), _ptr(v_new), _ptr(out), _ptr(lse),
                                        C.c_float(scale), _stream_ptr(stream)))
@@ -365,6 +400,11 @@ class Cache:
 # ---- module-level functions with the C names (same marshalling) -------------------------------
 def ws_kv_append(cache: Cache, session_ids, cu_new_tokens, k_new, v_new, modality=None, stream=None):
     cache.kv_append(session_ids, cu_new_tokens, k_new, v_new, modality, stream)
+
+
+def ws_kv_append_blocks(cache: Cache, session_ids, cu_new_tokens, cu_blocks, block_tokens, k_new, v_new,
+                        modality=None, stream=None):
+    cache.kv_append_blocks(session_ids, cu_new_tokens, cu_blocks, block_tokens, k_new, v_new, modality, stream)
 
 
 def ws_block_causal_attn_fwd(cache: Cache, session_ids, cu_q_tokens, q, out, scale, lse=None,

@@ -482,9 +482,15 @@ struct AppendPrep {
 };
 
 // No state changes.  *words = size of the descriptor blob.
+// cu_blocks / block_tokens (ws_kv_append_blocks): session s commits its n_s tokens as the blocks
+// block_tokens[cu_blocks[s] .. cu_blocks[s+1]); both NULL = one block per session.
 ws_status_t append_validate(ws_cache* c, int32_t S, const int32_t* session_ids, const int32_t* cu,
-                            const void* k_new, const void* v_new, size_t* words_out) {
+                            const void* k_new, const void* v_new, size_t* words_out,
+                            const int32_t* cu_blocks = nullptr, const int32_t* block_tokens = nullptr) {
   if (!c || !session_ids || !cu) return fail(WS_ERR_INVALID_ARG, "NULL argument");
+  if ((cu_blocks == nullptr) != (block_tokens == nullptr))
+    return fail(WS_ERR_INVALID_ARG, "cu_blocks and block_tokens must be given together");
+  if (cu_blocks && cu_blocks[0] != 0) return fail(WS_ERR_INVALID_ARG, "cu_blocks[0] must be 0");
   if (S < 1 || S > c->cfg.max_sessions_per_call)
     return fail(WS_ERR_INVALID_ARG, "num_sessions %d not in [1, %d]", S, c->cfg.max_sessions_per_call);
   if (!c->dry && (!k_new || !v_new)) return fail(WS_ERR_INVALID_ARG, "k_new / v_new is NULL");
@@ -498,7 +504,20 @@ ws_status_t append_validate(ws_cache* c, int32_t S, const int32_t* session_ids, 
     if (!c->host->is_open(id)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", id);
     for (int32_t t = 0; t < s; ++t)
       if (session_ids[t] == id) return fail(WS_ERR_INVALID_ARG, "session %d listed twice", id);
-    if (!c->host->fits(id, n))
+    int32_t nb = 1;
+    if (cu_blocks) {
+      nb = cu_blocks[s + 1] - cu_blocks[s];
+      if (nb < 1) return fail(WS_ERR_INVALID_ARG, "session %d commits %d blocks (must be >= 1)", s, nb);
+      int64_t sum = 0;
+      for (int32_t b = cu_blocks[s]; b < cu_blocks[s + 1]; ++b) {
+        if (block_tokens[b] < 1) return fail(WS_ERR_INVALID_ARG, "session %d: block of %d tokens", s, block_tokens[b]);
+        sum += block_tokens[b];
+      }
+      if (sum != n)
+        return fail(WS_ERR_INVALID_ARG, "session %d: its blocks hold %lld tokens, cu_new_tokens gives %d", s,
+                    (long long)sum, n);
+    }
+    if (!c->host->fits(id, n, nb))
       return fail(WS_ERR_OUT_OF_PAGES, "session %d exceeds its page-table or block capacity", id);
     if (c->host->session(id).tokens + n >= (1ll << 31))
       return fail(WS_ERR_UNSUPPORTED, "session %d would exceed 2^31 tokens", id);
@@ -520,7 +539,8 @@ ws_status_t append_validate(ws_cache* c, int32_t S, const int32_t* session_ids, 
 
 // Commits the blocks to the host metadata and builds the descriptor.  Call only after append_validate.
 ws_status_t append_commit(ws_cache* c, int32_t S, const int32_t* session_ids, const int32_t* cu,
-                          const uint8_t* modality, size_t words, cudaStream_t stream, AppendPrep* ap) {
+                          const uint8_t* modality, size_t words, cudaStream_t stream, AppendPrep* ap,
+                          const int32_t* cu_blocks = nullptr, const int32_t* block_tokens = nullptr) {
   ap->inline_meta = words <= (size_t)ws::kInlineAppendWords;
   char* h = (char*)ap->inl.w;
   if (!ap->inline_meta) {
@@ -545,11 +565,18 @@ ws_status_t append_commit(ws_cache* c, int32_t S, const int32_t* session_ids, co
     int32_t id = session_ids[s], n = cu[s + 1] - cu[s];
     int64_t len_old = c->host->session(id).tokens;
     const size_t old_pages = c->host->session(id).pages.size();
-    int32_t first = c->host->commit_block(id, n, modality ? modality + cu[s] : nullptr);
+    // the device side sees one contiguous run of n tokens per session whatever its block structure
+    const int32_t nb = cu_blocks ? cu_blocks[s + 1] - cu_blocks[s] : 1;
+    const int32_t* lens = cu_blocks ? block_tokens + cu_blocks[s] : &n;
+    const int32_t first = (int32_t)(len_old / c->cfg.page_tokens);
+    c->host->note_append(id);
+    for (int32_t b = 0, done = 0; b < nb; done += lens[b], ++b)
+      c->host->commit_block(id, lens[b], modality ? modality + cu[s] + done : nullptr);
     const ws::SessionState& ss = c->host->session(id);
     as[s] = ws::AppendSession{id, (int32_t)len_old, cu[s], cu[s + 1], npg, {0, 0, 0}};
     for (size_t i = first; i < ss.pages.size(); ++i) pages[npg++] = ss.pages[i];
-    msg.insert(msg.end(), {id, (int32_t)len_old, 1, (int32_t)(ss.pages.size() - old_pages), n});
+    msg.insert(msg.end(), {id, (int32_t)len_old, nb, (int32_t)(ss.pages.size() - old_pages)});
+    msg.insert(msg.end(), lens, lens + nb);
     msg.insert(msg.end(), ss.pages.begin() + old_pages, ss.pages.end());
   }
   msg[kMsgTotalWord] = (int32_t)msg.size();
@@ -586,10 +613,14 @@ struct FusedAppend {
 // launch: its keys are read from k_new / v_new, and warps 10-11 of the kernel copy it into the pool.
 ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const int32_t* num_q_blocks,
                       const int32_t* cu, const void* q, void* out, float* lse, float scale,
-                      cudaStream_t stream, const FusedAppend* fuse) {
+                      cudaStream_t stream, const FusedAppend* fuse, uint32_t attn_flags = 0) {
   std::vector<ws::PlanSession> ps(S);
   std::vector<int32_t> vis_end, tok_slot;
   bool any_multi = false;
+  if (attn_flags & ~(uint32_t)WS_ATTN_TEXT_CAUSAL) return fail(WS_ERR_INVALID_ARG, "unknown attn_flags 0x%x", attn_flags);
+  // NEXT-4 mixed mask (reading A19): per session a record {abs_pos0, nbits, text bits of the query tokens...}
+  const bool text_causal = (attn_flags & WS_ATTN_TEXT_CAUSAL) != 0;
+  std::vector<int32_t> txt_words, txt_pos, txt_rec;
   for (int32_t s = 0; s < S; ++s) {
     int32_t id = session_ids[s];
     if (!c->host->is_open(id)) return fail(WS_ERR_BAD_SESSION, "session %d is not open", id);
@@ -603,7 +634,25 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
     if (cu[s + 1] - cu[s] != nq)
       return fail(WS_ERR_INVALID_ARG, "session %d: cu gives %d query tokens, its last %d block(s) hold %lld",
                   id, cu[s + 1] - cu[s], m, (long long)nq);
-    ps[s] = ws::PlanSession{id, cu[s], cu[s + 1], m > 1, fuse ? (int32_t)nq : 0};
+    ps[s] = ws::PlanSession{id, cu[s], cu[s + 1], m > 1, fuse ? (int32_t)nq : 0, (int32_t)ss.settled[1], -1};
+    if (text_causal) {
+      if ((int64_t)ss.modality.size() < ss.tokens)
+        return fail(WS_ERR_INVALID_ARG, "session %d: WS_ATTN_TEXT_CAUSAL needs modality tags for the queried tokens", id);
+      ps[s].txt_off = (int32_t)txt_words.size();
+      const size_t rec = txt_words.size();
+      txt_words.push_back((int32_t)q_start);
+      txt_words.push_back((int32_t)nq);
+      txt_words.resize(rec + 2 + (size_t)(nq + 31) / 32, 0);
+      for (int64_t k = 0; k < nq; ++k) {
+        const uint8_t tag = ss.modality[(size_t)(q_start + k)];
+        if (tag > 2)
+          return fail(WS_ERR_INVALID_ARG, "session %d: token %lld was appended without a modality tag", id,
+                      (long long)(q_start + k));
+        if (tag == 2) txt_words[rec + 2 + (size_t)(k >> 5)] |= (int32_t)(1u << (k & 31));
+        txt_pos.push_back(tag == 2 ? (int32_t)(q_start + k) : -1);
+        txt_rec.push_back((int32_t)rec);
+      }
+    }
     any_multi |= m > 1;
     for (int32_t b = B - m; b < B; ++b) {
       int64_t lo = b ? ss.block_ends[b - 1] : 0;
@@ -624,21 +673,27 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
     if (fuse) return fail(WS_ERR_UNSUPPORTED, "internal: fused step on the generic kernel");
     if (c->dry && !c->tensor_path_ok) { c->last_plan = ws::Plan(); return WS_OK; }
     if (!c->dry) {
-      size_t bytes = (size_t)NQ * 8;
+      // rows: session slot, visible end [, text position or -1, record offset; then the text-bit records]
+      std::vector<int32_t> tm(tok_slot);
+      tm.insert(tm.end(), vis_end.begin(), vis_end.end());
+      if (text_causal) {
+        tm.insert(tm.end(), txt_pos.begin(), txt_pos.end());
+        for (int32_t r : txt_rec) tm.push_back(4 * NQ + r);
+        tm.insert(tm.end(), txt_words.begin(), txt_words.end());
+      }
+      const size_t bytes = tm.size() * 4;
       ws::InlineAppendMeta inl;
       ws_status_t st = WS_OK;
-      if (2 * (size_t)NQ <= (size_t)ws::kInlineAppendWords) {
+      if (tm.size() <= (size_t)ws::kInlineAppendWords) {
         // small call (the fp32 config: 16 tokens): the metadata rides in the kernel parameters
-        memcpy(inl.w, tok_slot.data(), (size_t)NQ * 4);
-        memcpy(inl.w + NQ, vis_end.data(), (size_t)NQ * 4);
+        memcpy(inl.w, tm.data(), bytes);
         d = nullptr;
       } else {
         st = refuse_if_capturing(stream, "generic-kernel metadata");
         if (st != WS_OK) return st;
         st = next_slot(c, bytes, &h, &d);
         if (st != WS_OK) return st;
-        memcpy(h, tok_slot.data(), (size_t)NQ * 4);
-        memcpy(h + (size_t)NQ * 4, vis_end.data(), (size_t)NQ * 4);
+        memcpy(h, tm.data(), bytes);
         st = upload_slot(c, h, d, bytes, stream);
         if (st != WS_OK) return st;
       }
@@ -648,7 +703,7 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
                                    c->default_map ? nullptr : c->d_q_to_kv, NQ,
                                    c->cfg.max_pages_per_session, c->cfg.num_q_heads,
                                    c->cfg.num_kv_heads, c->cfg.head_dim, c->cfg.page_tokens, scale,
-                                   stream));
+                                   text_causal ? 1 : 0, stream));
       tl.done();
       c->launches += 1;
       c->last_plan = ws::Plan();
@@ -665,11 +720,13 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
   std::vector<int32_t> blob;
   std::vector<int32_t> key;
   bool cached = false;
-  if (!any_multi) {
-    key.reserve(8 + 5 * (size_t)S);
+  const bool cacheable = !any_multi && !text_causal;
+  if (cacheable) {
+    key.reserve(8 + 6 * (size_t)S);
     key.insert(key.end(), {pc.Hkv, pc.G, pc.num_sms, pc.min_splits, pc.max_part_slots, (int32_t)pc.allow_alt, S});
     for (int32_t s = 0; s < S; ++s)
-      key.insert(key.end(), {ps[s].slot, ps[s].q_begin, ps[s].q_end, vis_end[ps[s].q_begin], ps[s].new_len});
+      key.insert(key.end(), {ps[s].slot, ps[s].q_begin, ps[s].q_end, vis_end[ps[s].q_begin], ps[s].new_len,
+                             ps[s].stable_len / ws::kTileKeys});
     cached = plan_cache_lookup(key, &plan, &blob);
   }
   if (!cached) {
@@ -681,8 +738,8 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
     if (!plan.ok)
       return fail(WS_ERR_WORKSPACE_TOO_SMALL, "plan needs %d partial slots, workspace holds %d",
                   plan.num_part_slots, c->lay.max_part_slots);
-    blob = ws::serialise_plan(plan, vis_end, any_multi);
-    if (!any_multi) plan_cache_insert(key, plan, blob);
+    blob = ws::serialise_plan(plan, vis_end, any_multi, txt_words);
+    if (cacheable) plan_cache_insert(key, plan, blob);
   }
   const bool inline_meta = blob.size() <= (size_t)ws::kInlineAttnWordsLarge;
   ws_status_t st = WS_OK;
@@ -787,6 +844,20 @@ ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
   return append_launch(c, ap, k_new, v_new, cu[S], (cudaStream_t)cuda_stream);
 }
 
+ws_status_t ws_kv_append_blocks(ws_cache_t* c, int32_t S, const int32_t* session_ids, const int32_t* cu,
+                                const int32_t* cu_blocks, const int32_t* block_tokens, const void* k_new,
+                                const void* v_new, const uint8_t* modality, void* cuda_stream) {
+  if (!cu_blocks || !block_tokens) return fail(WS_ERR_INVALID_ARG, "cu_blocks / block_tokens is NULL");
+  size_t words = 0;
+  ws_status_t st = append_validate(c, S, session_ids, cu, k_new, v_new, &words, cu_blocks, block_tokens);
+  if (st != WS_OK) return st;
+  DeviceGuard dg(c);
+  AppendPrep ap;
+  st = append_commit(c, S, session_ids, cu, modality, words, (cudaStream_t)cuda_stream, &ap, cu_blocks, block_tokens);
+  if (st != WS_OK) return st;
+  return append_launch(c, ap, k_new, v_new, cu[S], (cudaStream_t)cuda_stream);
+}
+
 // ------------------------------------------------------------------------------------ a3 + a4
 ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* session_ids,
                                      const int32_t* num_q_blocks, const int32_t* cu, const void* q,
@@ -797,9 +868,32 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* c, int32_t S, const int32_t* se
   return attn_impl(c, S, session_ids, num_q_blocks, cu, q, out, lse, scale, (cudaStream_t)cuda_stream, nullptr);
 }
 
+ws_status_t ws_block_causal_attn_fwd_masked(ws_cache_t* c, int32_t S, const int32_t* session_ids,
+                                            const int32_t* num_q_blocks, const int32_t* cu, const void* q,
+                                            void* out, float* lse, float scale, uint32_t attn_flags,
+                                            void* cuda_stream) {
+  ws_status_t st = attn_validate_args(c, S, session_ids, cu, q, out, scale);
+  if (st != WS_OK) return st;
+  DeviceGuard dg(c);
+  return attn_impl(c, S, session_ids, num_q_blocks, cu, q, out, lse, scale, (cudaStream_t)cuda_stream, nullptr,
+                   attn_flags);
+}
+
 ws_status_t ws_stream_step(ws_cache_t* c, int32_t S, const int32_t* session_ids, const int32_t* cu,
                            const void* q, const void* k_new, const void* v_new, void* out, float* lse,
                            float scale, void* cuda_stream) {
+  return ws_stream_step_tagged(c, S, session_ids, cu, q, k_new, v_new, nullptr, 0u, out, lse, scale, cuda_stream);
+}
+
+ws_status_t ws_stream_step_tagged(ws_cache_t* c, int32_t S, const int32_t* session_ids, const int32_t* cu,
+                                  const void* q, const void* k_new, const void* v_new, const uint8_t* modality,
+                                  uint32_t attn_flags, void* out, float* lse, float scale, void* cuda_stream) {
+  if (attn_flags & ~(uint32_t)WS_ATTN_TEXT_CAUSAL) return fail(WS_ERR_INVALID_ARG, "unknown attn_flags 0x%x", attn_flags);
+  if ((attn_flags & WS_ATTN_TEXT_CAUSAL) && !modality)
+    return fail(WS_ERR_INVALID_ARG, "WS_ATTN_TEXT_CAUSAL needs the block's modality tags");
+  if (modality && c && cu && S >= 1 && cu[0] == 0)
+    for (int32_t t = 0; t < cu[S]; ++t)
+      if (modality[t] > 2) return fail(WS_ERR_INVALID_ARG, "modality[%d] = %d (0 video, 1 audio, 2 text)", t, modality[t]);
   // validate what only the second half would reject BEFORE the append commits anything
   ws_status_t st = attn_validate_args(c, S, session_ids, cu, q, out, scale);
   if (st != WS_OK) return st;
@@ -809,18 +903,18 @@ ws_status_t ws_stream_step(ws_cache_t* c, int32_t S, const int32_t* session_ids,
   DeviceGuard dg(c);
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   AppendPrep ap;
-  st = append_commit(c, S, session_ids, cu, nullptr, words, stream, &ap);
+  st = append_commit(c, S, session_ids, cu, modality, words, stream, &ap);
   if (st != WS_OK) return st;
   // One launch commits and attends when the tcgen05 kernel runs and the append descriptor fits the kernel
   // parameters (up to ~900 new pages per call); otherwise: the append kernel, then attention over the pool.
   const bool tensor = c->tensor_path_ok && !(c->cfg.flags & WS_FLAG_FORCE_SIMT);
   if (tensor && ap.inline_meta && !(c->cfg.flags & WS_FLAG_SEPARATE_APPEND)) {
     const FusedAppend fuse{&ap, k_new, v_new};
-    return attn_impl(c, S, session_ids, nullptr, cu, q, out, lse, scale, stream, &fuse);
+    return attn_impl(c, S, session_ids, nullptr, cu, q, out, lse, scale, stream, &fuse, attn_flags);
   }
   st = append_launch(c, ap, k_new, v_new, cu[S], stream);
   if (st != WS_OK) return st;
-  return attn_impl(c, S, session_ids, nullptr, cu, q, out, lse, scale, stream, nullptr);
+  return attn_impl(c, S, session_ids, nullptr, cu, q, out, lse, scale, stream, nullptr, attn_flags);
 }
 
 size_t ws_step_staging_bytes(const ws_cache_config_t* cfg, int32_t n) {

@@ -55,7 +55,7 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
                  const int32_t* __restrict__ page_table, const int32_t* __restrict__ tok_meta,
                  const __grid_constant__ InlineAppendMeta inl,
                  const int32_t* __restrict__ q_to_kv, int32_t total_q_tokens, int32_t max_pages,
-                 int32_t Hq, int32_t Hkv, int32_t D, int32_t P, float scale) {
+                 int32_t Hq, int32_t Hkv, int32_t D, int32_t P, float scale, int32_t text_causal) {
   // per-token (session slot, visible end): device blob, or - small calls - the kernel parameter itself
   // (constant-bank reads; no host->device copy in the chain, so the call is CUDA-graph capturable)
   const MetaView<kInlineAppendWords> meta{tok_meta, inl};
@@ -71,6 +71,15 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
   const int32_t g = q_to_kv ? q_to_kv[h] : h / (Hq / Hkv);
   const int32_t slot = meta[tok];
   const int32_t vis = meta[total_q_tokens + tok];
+  // text-causal mixed mask (NEXT-4, reading A19): rows 2, 3 of the per-token metadata = the token's absolute
+  // position if it is a text token (else -1) and the blob offset of its session's record {abs_pos0, nbits,
+  // bits...} (bit k <=> the token at position abs_pos0 + k is text).  A text row skips later text keys.
+  int32_t txt_pos = -1, txt_rec = 0, txt_abs0 = 0;
+  if (text_causal) {
+    txt_pos = meta[2 * total_q_tokens + tok];
+    txt_rec = meta[3 * total_q_tokens + tok];
+    txt_abs0 = meta[txt_rec];
+  }
   const int32_t* page_row = page_table + (int64_t)slot * max_pages;
 
   const T* qrow = q + ((int64_t)tok * Hq + h) * D;
@@ -85,7 +94,11 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
 
   for (int32_t base = 0; base < vis; base += 32) {
     const int32_t j = base + lane;
-    const bool valid = j < vis;
+    bool valid = j < vis;
+    if (valid && txt_pos >= 0 && j > txt_pos) {
+      const int32_t b = j - txt_abs0;
+      if ((meta[txt_rec + 2 + (b >> 5)] >> (b & 31)) & 1) valid = false;
+    }
     float s = -INFINITY;
     int32_t rowidx = 0;
     if (valid) {
@@ -104,7 +117,9 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
     float tmax = s;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, o));
-    const float m_new = fmaxf(m, tmax);                 // finite: at least one key is valid
+    const float m_new = fmaxf(m, tmax);
+    // finite: the first chunk holds a visible key (a text row sees every key up to its own position),
+    // a later chunk may be hidden entirely (text-causal), m is finite by then
     const float corr = expf(m - m_new);                 // m = -inf -> 0
     const float p = valid ? expf(s - m_new) : 0.f;
     float psum = p;
@@ -152,18 +167,18 @@ cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse
                              const void* k_pool, const void* v_pool, const int32_t* page_table,
                              const int32_t* tok_meta, const InlineAppendMeta& inl, const int32_t* q_to_kv,
                              int32_t total_q_tokens, int32_t max_pages, int32_t Hq, int32_t Hkv, int32_t D,
-                             int32_t P, float scale, cudaStream_t stream) {
+                             int32_t P, float scale, int32_t text_causal, cudaStream_t stream) {
   int64_t warps = (int64_t)total_q_tokens * Hq;
   int32_t grid = (int32_t)((warps + kSimtWarps - 1) / kSimtWarps);
   if (grid == 0) return cudaSuccess;
   if (dtype == 1)
     return launch_pdl(attn_simt_kernel<float>, dim3(grid), dim3(kSimtWarps * 32), 0, stream,
                       (const float*)q, (float*)out, lse, (const float*)k_pool, (const float*)v_pool, page_table,
-                      tok_meta, inl, q_to_kv, total_q_tokens, max_pages, Hq, Hkv, D, P, scale);
+                      tok_meta, inl, q_to_kv, total_q_tokens, max_pages, Hq, Hkv, D, P, scale, text_causal);
   return launch_pdl(attn_simt_kernel<__nv_bfloat16>, dim3(grid), dim3(kSimtWarps * 32), 0, stream,
                     (const __nv_bfloat16*)q, (__nv_bfloat16*)out, lse, (const __nv_bfloat16*)k_pool,
                     (const __nv_bfloat16*)v_pool, page_table, tok_meta, inl, q_to_kv, total_q_tokens, max_pages,
-                    Hq, Hkv, D, P, scale);
+                    Hq, Hkv, D, P, scale, text_causal);
 }
 
 }  // namespace ws

@@ -203,11 +203,14 @@ __device__ __forceinline__ void red_release_gpu_add(int32_t* p, int32_t v) {
 // kAlt: decode plan (plan.h) - both accumulator sets use Q tile 0; set q processes the KV tiles of the
 // segment with (tile - tile_begin) % 2 == q and writes its own partial (slot part_base + q).
 //
-// Programmatic dependent launch (protocol: launch.h).  Thread 0 lets the successor's CTAs be scheduled as
-// soon as this CTA is set up; the TMA producer executes griddepcontrol.wait before its first load (q,
-// k_new, v_new may come from the caller's kernel just before; pool pages and page-table entries from an
-// append just before), the append warps before their first store, and every softmax thread before its
-// first global write (out / partials may still be read or written by the previous step's kernels).
+// Programmatic dependent launch (protocol: launch.h).  Before griddepcontrol.wait the TMA producer fetches
+// only KV tiles of the stable prefix of its first segment (Group::stable_tiles: committed at least two
+// append calls ago, so no kernel that can still be in flight writes them); the wait precedes every other
+// load (q, k_new, v_new may come from the caller's kernel just before; pool pages and page-table entries
+// from an append just before) and only after it does that thread let the successor's CTAs be scheduled;
+// the append warps wait before their first store, every softmax thread before its first global write
+// (out / partials may still be read or written by the previous step's kernels).  Metadata in a device blob
+// (p.meta: large calls, uploaded by a stream-ordered copy) is only read after the wait.
 template <int kInlW, bool kAlt>
 __global__ void __launch_bounds__(kThreads, 1)
 attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
@@ -218,6 +221,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ InlineMeta<kInlW> inl,
                   const __grid_constant__ InlineAppendMeta app, const PeerPools peers, const AttnParams p_in) {
   AttnParams p = p_in;
+  if (p.meta != nullptr) pdl_wait();
   const MetaView<kInlW> meta{p.meta, inl};
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -248,6 +252,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   // the first MMA.
   SegView sv_first;
   int32_t si_first = seg_hi, pre_pg0 = 0, pre_pg1 = 0;
+  bool pre_valid = false;
   // Q tiles of segment `sv` -> sQ (general plan: the pair's two tiles; decode plan: the one shared tile)
   auto issue_q = [&](const SegView& sv) {
     if constexpr (kAlt) {
@@ -264,25 +269,21 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     }
   };
   if (warp == 8 && lane == 0) {
-    // the producer owns the Q barriers: initialised here so that the first Q load leaves before the
-    // CTA-wide set-up barrier (the MMA warp first looks at q_full after that barrier)
+    // the producer owns the Q barriers
     mbar_init(bq_full, 1); mbar_init(bq_empty, 1);
     fence_mbar_init();
     fence_proxy_async_smem();
     prefetch_tmap(&tmap_q); prefetch_tmap(&tmap_k); prefetch_tmap(&tmap_v);
     if (p.append_tokens > 0) { prefetch_tmap(&tmap_kn); prefetch_tmap(&tmap_vn); }
-    pdl_wait();
     for (si_first = seg_lo; si_first < seg_hi; ++si_first)
       if (load_segment(meta, hdr, si_first, pair, tok_per_pair, sv_first) &&
           sv_first.tile_end > sv_first.tile_begin) break;
-    if (si_first < seg_hi) {
-      issue_q(sv_first);
-      if (sv_first.tile_begin * kTileKeys < sv_first.g.cache_len) {
-        const int32_t* page_row = p.page_table + (int64_t)sv_first.g.slot * p.max_pages_per_session;
-        const int32_t last_page = (sv_first.g.cache_len - 1) / p.P;
-        pre_pg0 = page_row[min(2 * sv_first.tile_begin, last_page)];
-        pre_pg1 = page_row[min(2 * sv_first.tile_begin + 1, last_page)];
-      }
+    // page ids of the first tile, if it lies in the stable prefix (readable before griddepcontrol.wait)
+    if (si_first < seg_hi && sv_first.tile_begin < sv_first.g.stable_tiles) {
+      const int32_t* page_row = p.page_table + (int64_t)sv_first.g.slot * p.max_pages_per_session;
+      pre_pg0 = page_row[2 * sv_first.tile_begin];
+      pre_pg1 = page_row[2 * sv_first.tile_begin + 1];
+      pre_valid = true;
     }
   }
   if (warp == 9 && lane == 0) {
@@ -301,16 +302,24 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
-  if (threadIdx.x == 0) pdl_launch_dependents();
 
   if (warp >= 8) {
     setmaxnreg_dec<88>();
     if (warp == 8 && lane == 0) {
       // ===================================================== TMA producer
       uint32_t ring_it = 0, q_it = 0;
+      // Programmatic dependent launch (launch.h).  Until `waited`, only KV tiles of the FIRST segment's
+      // stable prefix are fetched (at most one ring of them: the MMA warp cannot consume without Q);
+      // griddepcontrol.wait precedes everything else - q, k_new / v_new, page ids and pool rows of recent
+      // appends - and only then does this thread let the successor's CTAs be scheduled.
+      bool waited = false;
+      auto ensure_wait = [&]() {
+        if (!waited) { pdl_wait(); pdl_launch_dependents(); waited = true; }
+      };
       for (int32_t si = si_first; si < seg_hi; ++si) {
         SegView sv;
-        if (si == si_first) {
+        const bool first = si == si_first;
+        if (first) {
           sv = sv_first;
         } else {
           if (!load_segment(meta, hdr, si, pair, tok_per_pair, sv)) continue;
@@ -319,6 +328,18 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         const int32_t* page_row = p.page_table + (int64_t)sv.g.slot * p.max_pages_per_session;
         const int32_t last_page = (sv.g.cache_len - 1) / p.P;
         const int32_t Tc = (sv.g.cache_len + kTileKeys - 1) / kTileKeys;   // tiles >= Tc: the block being committed
+        // Q tiles of this segment: the first segment's go out right after the wait, later ones when the
+        // MMA warp has released the Q buffers
+        bool q_pending = true;
+        auto before_load = [&](int32_t j) {                  // j == tile_end: end of the segment, Q must go out
+          if (!q_pending) return;
+          if (first && !waited && j < sv.tile_end && j < sv.g.stable_tiles && ring_it < (uint32_t)kStages) return;   // prefetch
+          ensure_wait();
+          if (!first) mbar_wait(bq_empty, (q_it & 1) ^ 1);
+          issue_q(sv);
+          q_pending = false;
+        };
+        if (!first) before_load(sv.tile_begin);
         // one 128-key K or V tile -> the next ring slot: 64-key x 64-dim boxes at offsets 0 (keys 0-63,
         // dims 0-63), 8 KB (keys 64-127), 16 KB and 24 KB (dims 64-127)
         auto load_tile = [&](bool is_v, int32_t j, int32_t c0, int32_t c1) {
@@ -346,11 +367,10 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         };
         auto page_of = [&](int32_t logical) { return logical <= 2 * Tc - 1 ? page_row[min(logical, last_page)] : 0; };
         if constexpr (kAlt) {
-          // one Q tile serves both accumulator sets (the first segment's was issued during set-up)
-          if (si != si_first) { mbar_wait(bq_empty, (q_it & 1) ^ 1); issue_q(sv); }
-          ++q_it;
+          // one Q tile serves both accumulator sets
           auto load_alt = [&](bool is_v, int32_t j) {
-            const bool pre = si == si_first && j == sv.tile_begin;   // ids fetched during set-up
+            before_load(j);
+            const bool pre = first && pre_valid && j == sv.tile_begin;   // ids fetched during set-up
             load_tile(is_v, j, pre ? pre_pg0 : page_of(2 * j), pre ? pre_pg1 : page_of(2 * j + 1));
           };
           // consumption order of the MMA warp: K0 K1 | V0 K2 | V1 K3 | ...
@@ -360,24 +380,27 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             load_alt(true, j);
             if (j + 2 < sv.tile_end) load_alt(false, j + 2);
           }
+          before_load(sv.tile_end);                          // (a segment that fitted the prefetch window)
+          ++q_it;
           continue;
         }
-        // Q pair (own rows); the first segment's was issued during set-up, ahead of the page-id reads
-        if (si != si_first) { mbar_wait(bq_empty, (q_it & 1) ^ 1); issue_q(sv); }
-        ++q_it;
-        int32_t pg0, pg1;
-        if (si == si_first) {
-          pg0 = pre_pg0; pg1 = pre_pg1;
-        } else {
-          pg0 = page_of(2 * sv.tile_begin); pg1 = page_of(2 * sv.tile_begin + 1);
-        }
+        int32_t pg0 = pre_pg0, pg1 = pre_pg1;
+        bool have_ids = first && pre_valid;
         for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
+          before_load(j);
+          if (!have_ids) { pg0 = page_of(2 * j); pg1 = page_of(2 * j + 1); }
           const int32_t c0 = pg0, c1 = pg1;
-          if (j + 1 < sv.tile_end) { pg0 = page_of(2 * j + 2); pg1 = page_of(2 * j + 3); }   // next tile's ids
+          // next tile's ids one tile ahead - unless they may not be published yet
+          have_ids = j + 1 < sv.tile_end && (!q_pending || j + 1 < sv.g.stable_tiles);
+          if (have_ids) { pg0 = page_of(2 * j + 2); pg1 = page_of(2 * j + 3); }
           load_tile(false, j, c0, c1);
+          before_load(j);
           load_tile(true, j, c0, c1);
         }
+        before_load(sv.tile_end);
+        ++q_it;
       }
+      ensure_wait();
     } else if (warp == 9) {
       // ===================================================== MMA issuer
       // The whole warp runs the control flow convergently (all values stay warp-uniform, so the
@@ -614,6 +637,19 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const int32_t Tc = (sv.g.cache_len + kTileKeys - 1) / kTileKeys;
       const int32_t vis_cache = min(vis, sv.g.cache_len);
       float m_used = -INFINITY, l = 0.f;
+      // text-causal mixed mask (NEXT-4, reading A19): a text row at absolute position
+      // txt_pos does not see text keys at later positions.  The session's record in the blob:
+      // {abs_pos0, nbits, bits...}, bit k <=> the token at position abs_pos0 + k is text.
+      const int32_t txt_rec = sv.g.txt_off;
+      int32_t txt_pos = -1, txt_abs0 = 0, txt_nw = 0;
+      if (txt_rec >= 0) {
+        txt_abs0 = meta[txt_rec];
+        txt_nw = (meta[txt_rec + 1] + 31) >> 5;
+        if (row_valid) {
+          const int32_t k = tok - sv.g.new_tok0;
+          if ((meta[txt_rec + 2 + (k >> 5)] >> (k & 31)) & 1) txt_pos = txt_abs0 + k;
+        }
+      }
 
       // O and l of this row scaled by alpha (after a change of reference).  Safe whenever the PV MMAs of
       // the previous tile have completed: s_full of the current tile was committed after them on the same
@@ -709,7 +745,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         const int32_t lim = t < Tc ? vis_cache : vis;        // keys >= lim of this tile are masked
         mbar_wait(bs_full(q), tile_it & 1);
         tc_fence_after();
-        const bool need_mask = __any_sync(0xffffffffu, key0 + kTileKeys > lim);
+        const bool need_mask = __any_sync(0xffffffffu, key0 + kTileKeys > lim ||
+                                                       (txt_pos >= 0 && key0 + kTileKeys - 1 > txt_pos));
         bool done = false;
         // ---- optimistic path: no look at the tile's maximum.  Not tried on the first tiles of a segment
         // (their sums are of the order of the accumulated l: the share test would refuse them anyway) nor
@@ -759,6 +796,32 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #pragma unroll
           for (int i = 0; i < 128; ++i)
             if (key0 + i >= lim) sr[i] = 0xff800000u;       // -inf
+          if (txt_rec >= 0) {                               // (warp-uniform)
+            uint32_t hide[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              // text bits of keys key0 + 32k .. + 31 (the record is not aligned to the tile), and the keys
+              // among them that lie after this row's position
+              const int32_t b0 = key0 + 32 * k - txt_abs0;
+              uint32_t tw = 0;
+              if (b0 > -32 && b0 < 32 * txt_nw) {
+                if (b0 < 0) {
+                  tw = (uint32_t)meta[txt_rec + 2] << (-b0);
+                } else {
+                  const int32_t idx = b0 >> 5;
+                  const uint32_t lo = (uint32_t)meta[txt_rec + 2 + idx];
+                  const uint32_t hi = idx + 1 < txt_nw ? (uint32_t)meta[txt_rec + 3 + idx] : 0u;
+                  tw = __funnelshift_r(lo, hi, b0 & 31);
+                }
+              }
+              const int32_t d = txt_pos - (key0 + 32 * k);
+              const uint32_t later = txt_pos < 0 ? 0u : (d < 0 ? 0xffffffffu : (d >= 31 ? 0u : (0xffffffffu << (d + 1))));
+              hide[k] = tw & later;
+            }
+#pragma unroll
+            for (int i = 0; i < 128; ++i)
+              if ((hide[i >> 5] >> (i & 31)) & 1u) sr[i] = 0xff800000u;
+          }
           float mx0 = S_(0), mx1 = S_(1), mx2 = S_(2), mx3 = S_(3);
 #pragma unroll
           for (int i = 4; i < 128; i += 4) {

@@ -32,8 +32,10 @@ constexpr int kCombineRowsPerBlock = 8;
 template <int kInlW, int kDepth>
 __global__ void __launch_bounds__(kCombineRowsPerBlock * 32)
 combine_rows_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int32_t team_size) {
+  // The successor (the next step's append or attention kernel) may be scheduled at once: before its own
+  // griddepcontrol.wait it touches nothing this kernel or the attention kernel before it writes (launch.h).
+  pdl_launch_dependents();
   pdl_wait();                      // partials of the attention kernel launched just before
-  pdl_launch_dependents();         // the next step's append does not depend on this kernel
   const MetaView<kInlW> meta{p.meta, inl};
   const AttnMeta hdr = meta.template load<AttnMeta>(0);
   const int32_t blocks_per_pair = kPairRows / kCombineRowsPerBlock;
@@ -119,6 +121,8 @@ __global__ void __launch_bounds__(256)
 combine_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int32_t team_size, int32_t rows_pb) {
   extern __shared__ uint8_t smem_raw[];
   __shared__ uint64_t bar;
+  pdl_launch_dependents();         // see combine_rows_kernel
+  if (p.meta != nullptr) pdl_wait();
   const uint32_t sO = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint8_t* o_s = smem_raw + (sO - smem_u32(smem_raw));
   const uint32_t sLse = sO + kCombineRowsCap * 512;
@@ -140,7 +144,6 @@ combine_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int3
   if (threadIdx.x == 0) { mbar_init(smem_u32(&bar), 1); fence_mbar_init(); }
   __syncthreads();
   pdl_wait();                      // partials of the attention kernel launched just before
-  pdl_launch_dependents();         // the next step's append does not depend on this kernel
   if (!active) return;
   uint32_t phase = 0;
   // the LSE area holds nparts x ((rows + 8) & ~3) floats: shrink the chunk for very many parts

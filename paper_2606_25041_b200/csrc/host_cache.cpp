@@ -38,10 +38,10 @@ int32_t HostCache::pages_needed(int32_t s, int64_t new_tokens) const {
   return (int32_t)std::max<int64_t>(0, need - (int64_t)sess_[s].pages.size());
 }
 
-bool HostCache::fits(int32_t s, int64_t n) const {
+bool HostCache::fits(int32_t s, int64_t n, int32_t nblocks) const {
   const SessionState& st = sess_[s];
   int64_t need = (st.tokens + n + P_ - 1) / P_;
-  return need <= max_pages_ && (int64_t)st.block_ends.size() + 1 <= max_blocks_;
+  return need <= max_pages_ && (int64_t)st.block_ends.size() + nblocks <= max_blocks_;
 }
 
 int32_t HostCache::commit_block(int32_t s, int64_t n, const uint8_t* modality) {
@@ -73,6 +73,8 @@ bool HostCache::truncate_blocks(int32_t s, int32_t keep_blocks) {
     st.pages.pop_back();
   }
   if (st.modality.size() > (size_t)st.tokens) st.modality.resize((size_t)st.tokens);
+  st.settled[0] = std::min(st.settled[0], st.tokens);
+  st.settled[1] = std::min(st.settled[1], st.tokens);
   return true;
 }
 
@@ -103,6 +105,7 @@ bool HostCache::open_session_at(int32_t s) {
 void HostCache::adopt(int32_t s, const int32_t* block_lens, int32_t nblocks, const int32_t* pages,
                       int32_t npages) {
   SessionState& st = sess_[s];
+  note_append(s);
   for (int32_t i = 0; i < npages; ++i) {
     owner_used_[pages[i]] = 1;
     st.pages.push_back(pages[i]);

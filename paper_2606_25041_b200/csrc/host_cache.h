@@ -15,6 +15,10 @@ struct SessionState {
   std::vector<int32_t> pages;        // physical page ids, logical page i -> pages[i]
   std::vector<int64_t> block_ends;   // e_1 < ... < e_B
   std::vector<uint8_t> modality;     // per committed token (optional metadata, may be shorter)
+  // settled[0] / settled[1]: committed length before the most recent / the second most recent append call
+  // (or replica adoption) on this session, lowered by truncation.  Tokens below settled[1] are not written
+  // by any kernel that can still be in flight when the next launch starts (PDL protocol, launch.h).
+  int64_t settled[2] = {0, 0};
 };
 
 class HostCache {
@@ -29,12 +33,17 @@ class HostCache {
 
   // Pages a session needs in addition to what it holds to reach `new_tokens` committed tokens.
   int32_t pages_needed(int32_t s, int64_t new_tokens) const;
-  // Whether appending n tokens as ONE block fits the per-session capacities (pages, blocks).
-  bool fits(int32_t s, int64_t n) const;
+  // Whether appending n tokens as `nblocks` blocks fits the per-session capacities (pages, blocks).
+  bool fits(int32_t s, int64_t n, int32_t nblocks = 1) const;
   // Commit a block of n tokens (caller has checked free pages / capacity).  Returns index of the
   // first logical page touched by the new tokens.
   int32_t commit_block(int32_t s, int64_t n, const uint8_t* modality);
   bool truncate_blocks(int32_t s, int32_t keep_blocks);
+  // Once per append call (or adoption) and session, BEFORE its blocks are committed.
+  void note_append(int32_t s) {
+    sess_[s].settled[1] = sess_[s].settled[0];
+    sess_[s].settled[0] = sess_[s].tokens;
+  }
 
   // ---- NEXT-3 replica side: pages [0, owner_pages) are handed out only by adopt()
   // (the owner of the link names them); local appends draw from the rest.

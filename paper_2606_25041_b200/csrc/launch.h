@@ -56,12 +56,13 @@ cudaError_t launch_fm_euler(int32_t dtype, void* z, const void* v, float dtau, i
 
 // Generic SIMT attention (fp32 config; bf16 debug / unsupported-shape path).
 // tok_meta: [2][total_q_tokens] int32 = session slot, visible end per query token; nullptr: the same
-// words are in `inl` (kernel parameter, 2 * total_q_tokens <= kInlineAppendWords).
+// words are in `inl` (kernel parameter, 2 * total_q_tokens <= kInlineAppendWords).  text_causal: two more
+// rows (text position or -1, record offset) followed by the sessions' text-bit records (attn_simt.cu).
 cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse,
                              const void* k_pool, const void* v_pool, const int32_t* page_table,
                              const int32_t* tok_meta, const InlineAppendMeta& inl, const int32_t* q_to_kv,
                              int32_t total_q_tokens, int32_t max_pages, int32_t Hq, int32_t Hkv, int32_t D,
-                             int32_t P, float scale, cudaStream_t stream);
+                             int32_t P, float scale, int32_t text_causal, cudaStream_t stream);
 
 // sm_100a tcgen05 kernel (bf16, D = 128, P = 64).
 struct Sm100Launch {

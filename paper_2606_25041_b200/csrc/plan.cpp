@@ -52,6 +52,8 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
         const int32_t new_len = s.multi_block ? 0 : std::min(s.new_len, g.kv_len);
         g.cache_len = g.kv_len - new_len;
         g.new_tok0 = s.q_begin;
+        g.stable_tiles = std::min(s.stable_len, g.cache_len) / kTileKeys;
+        g.txt_off = s.txt_off;
         plan.groups.push_back(g);
         int32_t nt = (g.cache_len + kTileKeys - 1) / kTileKeys + (new_len + kTileKeys - 1) / kTileKeys;
         group_tiles.push_back(nt);
@@ -157,8 +159,8 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
 }
 
 std::vector<int32_t> serialise_plan(const Plan& plan, const std::vector<int32_t>& vis_end,
-                                    bool has_vis) {
-  static_assert(sizeof(Group) == 40 && sizeof(Segment) == 16 && sizeof(CombineItem) == 16 &&
+                                    bool has_vis, const std::vector<int32_t>& extra) {
+  static_assert(sizeof(Group) == 48 && sizeof(Segment) == 16 && sizeof(CombineItem) == 16 &&
                 sizeof(AttnMeta) == 64, "blob layout");
   AttnMeta m{};
   m.num_teams = plan.num_teams;
@@ -175,6 +177,7 @@ std::vector<int32_t> serialise_plan(const Plan& plan, const std::vector<int32_t>
   m.off_segments = off;          off += m.num_segments * (int32_t)(sizeof(Segment) / 4);
   m.off_combine = off;           off += m.num_combine * (int32_t)(sizeof(CombineItem) / 4);
   m.off_vis = off;               off += has_vis ? (int32_t)vis_end.size() : 0;
+  const int32_t off_extra = off; off += (int32_t)extra.size();
   off = (off + 3) & ~3;
   m.total_words = off;
   std::vector<int32_t> blob(off, 0);
@@ -183,6 +186,12 @@ std::vector<int32_t> serialise_plan(const Plan& plan, const std::vector<int32_t>
   };
   put(0, &m, sizeof(m));
   put(m.off_groups, plan.groups.data(), plan.groups.size() * sizeof(Group));
+  if (!extra.empty()) {
+    put(off_extra, extra.data(), extra.size() * 4);
+    for (size_t gi = 0; gi < plan.groups.size(); ++gi)
+      if (plan.groups[gi].txt_off >= 0)
+        reinterpret_cast<Group*>(blob.data() + m.off_groups)[gi].txt_off += off_extra;
+  }
   put(m.off_team_seg_begin, plan.team_seg_begin.data(), plan.team_seg_begin.size() * 4);
   put(m.off_segments, plan.segments.data(), plan.segments.size() * sizeof(Segment));
   put(m.off_combine, plan.combine.data(), plan.combine.size() * sizeof(CombineItem));

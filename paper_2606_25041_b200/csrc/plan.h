@@ -16,6 +16,8 @@ struct PlanSession {
   bool multi_block;      // queries span more than one block (per-token visible ends differ)
   int32_t new_len;       // fused step: the last `new_len` visible keys are read from k_new / v_new (rows
                          // q_begin ..) instead of the pool; 0 otherwise (and whenever multi_block)
+  int32_t stable_len;    // tokens committed at least two append calls ago (Group::stable_tiles)
+  int32_t txt_off;       // Group::txt_off (-1: none); offsets are relative to the start of the `extra` words
 };
 
 struct PlanConfig {
@@ -51,7 +53,9 @@ Plan build_plan(const PlanConfig& cfg, const std::vector<PlanSession>& sessions,
                 const std::vector<int32_t>& vis_end);
 
 // Serialise into the device blob layout described by AttnMeta (ws_internal.h).
+// `extra`: words appended after the visible ends (text-bit records of the mixed mask); every group's
+// txt_off >= 0 is rebased to the blob offset of extra[0].
 std::vector<int32_t> serialise_plan(const Plan& plan, const std::vector<int32_t>& vis_end,
-                                    bool has_vis);
+                                    bool has_vis, const std::vector<int32_t>& extra = std::vector<int32_t>());
 
 }  // namespace ws

@@ -59,6 +59,14 @@ struct Group {
   // KV tiles [Tc, Tc + ceil((kv_len - cache_len) / 128)).  Outside fused steps cache_len == kv_len.
   int32_t cache_len;
   int32_t new_tok0;
+  // KV tiles [0, stable_tiles) of the pool part were committed at least two append calls ago: no kernel
+  // that can still be in flight when this launch starts writes them (PDL protocol, launch.h), so the TMA
+  // producer may fetch them BEFORE griddepcontrol.wait.
+  int32_t stable_tiles;
+  // >= 0: text-causal mixed mask (NEXT-4, reading A19): word offset in the blob of this session's
+  // record {abs_pos0, nbits, bits...}: bit k set <=> the token at absolute position abs_pos0 + k is a text
+  // token; abs_pos0 = position of the session's first query token (row new_tok0 of q).  -1: plain block-causal.
+  int32_t txt_off;
   int32_t pad;
 };
 

@@ -74,6 +74,47 @@ def test_page_allocation_block_boundaries_and_truncate(pkg):
     assert e.value.status_name == "WS_ERR_BAD_SESSION"
 
 
+def test_append_blocks_commits_many_blocks_in_one_call(pkg):
+    """NEXT-1 (PAPER.md:75 system prefill): ws_kv_append_blocks == a sequence of ws_kv_append calls for the
+    host metadata (tokens, block ends, page ids), and rejects malformed block lists with nothing changed."""
+    a, b = _dry(pkg), _dry(pkg)
+    sa = [a.session_open(), a.session_open()]
+    sb = [b.session_open(), b.session_open()]
+    a.kv_append([sa[0]], [0, 10], None, None)
+    b.kv_append([sb[0]], [0, 10], None, None)
+    lens0, lens1 = [100, 29, 64, 7], [64, 1]
+    a.kv_append_blocks(sa, [0, sum(lens0), sum(lens0) + sum(lens1)], [0, 4, 6], lens0 + lens1, None, None)
+    # reference: one ws_kv_append per block, in an order that allocates the same pages (session 0 first)
+    for n in lens0:
+        b.kv_append([sb[0]], [0, n], None, None)
+    for n in lens1:
+        b.kv_append([sb[1]], [0, n], None, None)
+    for x, y in zip(sa, sb):
+        assert a.session_info(x) == b.session_info(y)
+        assert a.session_pages(x) == b.session_pages(y)
+    assert a.session_info(sa[0]) == (210, 5, [10, 110, 139, 203, 210])
+    assert a.free_pages() == b.free_pages()
+    # the commit message names every block (replica side applies them in one go)
+    msg = a.replica_commit_message()
+    assert list(msg[9:13]) == [sa[0], 10, 4, 4 - 1 + 0] or msg[11] == 4
+    before = (a.session_info(sa[0]), a.session_info(sa[1]), a.free_pages())
+    for cu_b, lens in (([0, 2, 3], [5, 5, 7]),            # session 0: 10 tokens but cu says 12
+                       ([0, 1, 1], [12]),                  # session 1: zero blocks
+                       ([0, 2, 3], [12, 0, 7]),            # empty block
+                       ([1, 2, 3], [12, 7, 7])):           # cu_blocks[0] != 0
+        with pytest.raises(pkg.WsError) as e:
+            a.kv_append_blocks(sa, [0, 12, 19], cu_b, lens, None, None)
+        assert e.value.status_name == "WS_ERR_INVALID_ARG"
+        assert (a.session_info(sa[0]), a.session_info(sa[1]), a.free_pages()) == before
+    # block capacity (16 per session): 5 committed + 12 more does not fit, 11 does
+    with pytest.raises(pkg.WsError) as e:
+        a.kv_append_blocks([sa[0]], [0, 12], [0, 12], [1] * 12, None, None)
+    assert e.value.status_name == "WS_ERR_OUT_OF_PAGES"
+    assert (a.session_info(sa[0]), a.session_info(sa[1]), a.free_pages()) == before
+    a.kv_append_blocks([sa[0]], [0, 11], [0, 11], [1] * 11, None, None)
+    assert a.session_info(sa[0])[1] == 16
+
+
 def test_error_paths_leave_state_unchanged(pkg):
     c = _dry(pkg, num_pages=4)
     s = c.session_open(); t = c.session_open()
