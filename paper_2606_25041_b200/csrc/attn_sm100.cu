@@ -53,9 +53,13 @@ namespace ws {
 
 using namespace ptx;
 
-constexpr int kStages = 5;                                 // K/V ring: 5 slots of one 128-key tile (32 KB)
+// K/V ring: slots of one 128-key tile (32 KB).  General plan: two Q tiles + 5 slots.  Decode plan: ONE Q tile,
+// so its ring starts where the second Q tile would be and has 6 slots - the decode step is bound by the
+// latency of the K/V stream (a slot is held from the issue of its load until the MMA that reads it has
+// completed, V slots until the softmax of their tile is through), every slot counts.
+constexpr int kStagesGen = 5, kStagesAlt = 6, kStagesMax = 6;
 constexpr uint32_t kSlotBytes = 32768;
-constexpr uint32_t kRingBytes = kStages * kSlotBytes;
+constexpr uint32_t kRingBytes = kStagesGen * kSlotBytes;   // capacity both plans have
 constexpr uint32_t kHalfBytes = 16384;                     // one 64-dim half of a 128-row tile: 128 rows x 128 B
 constexpr uint32_t kQTileBytes = kTileRows * 128 * 2;
 constexpr int kThreads = 384;
@@ -80,16 +84,20 @@ constexpr int kMaxJobs = 4;
 
 struct Barriers {
   uint64_t q_full, q_empty;
-  uint64_t kv_full[kStages], kv_empty[kStages];
+  uint64_t kv_full[kStagesMax], kv_empty[kStagesMax];
   uint64_t s_full[2], p_full[2][2], pv_h0_done[2], o_full[2], o_empty[2];
   uint64_t merge_full;
-  alignas(16) float lse_stage[kPairRows];
+  // staged epilogue: the pair's log2-LSEs on their way to part_lse ([0, 256); the decode plan uses [0, 128) and
+  // exchanges (LSE, 1/l) of its second accumulator set through the 1 KB that starts at float 128)
+  alignas(16) float lse_stage[kPairRows + kTileRows];
   MergeJob jobs[kMaxJobs];
   int32_t njobs, cur_slot0;          // staged epilogue: the pair's log2-LSEs on their way to part_lse
   uint32_t tmem_base;
   uint32_t pad;
 };
 constexpr uint32_t kSmemBytes = 2 * kQTileBytes + kRingBytes + sizeof(Barriers) + 1024;
+static_assert(kQTileBytes + kStagesAlt * kSlotBytes == 2 * kQTileBytes + kRingBytes, "both plans fill the same area");
+static_assert(kSmemBytes <= 232448, "227 KB of shared memory per CTA");
 
 struct SegView {
   Group g;
@@ -219,14 +227,16 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ CUtensorMap tmap_kn,
                   const __grid_constant__ CUtensorMap tmap_vn,
                   const __grid_constant__ InlineMeta<kInlW> inl,
-                  const __grid_constant__ InlineAppendMeta app, const PeerPools peers, const AttnParams p_in) {
+                  const __grid_constant__ InlineAppendMeta app, const __grid_constant__ PeerPools peers,
+                  const AttnParams p_in) {
   AttnParams p = p_in;
   if (p.meta != nullptr) pdl_wait();
   const MetaView<kInlW> meta{p.meta, inl};
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem_base;                           // 2 x 32 KB
-  const uint32_t sRing = smem_base + 2 * kQTileBytes;      // kStages x kSlotBytes
+  constexpr int kStages = kAlt ? kStagesAlt : kStagesGen;
+  const uint32_t sRing = smem_base + (kAlt ? 1 : 2) * kQTileBytes;   // kStages x kSlotBytes
   Barriers* bars = reinterpret_cast<Barriers*>(smem_raw + (smem_base - smem_u32(smem_raw)) +
                                                2 * kQTileBytes + kRingBytes);
   const uint32_t bq_full = smem_u32(&bars->q_full), bq_empty = smem_u32(&bars->q_empty);
@@ -328,21 +338,50 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         const int32_t* page_row = p.page_table + (int64_t)sv.g.slot * p.max_pages_per_session;
         const int32_t last_page = (sv.g.cache_len - 1) / p.P;
         const int32_t Tc = (sv.g.cache_len + kTileKeys - 1) / kTileKeys;   // tiles >= Tc: the block being committed
-        // Q tiles of this segment: the first segment's go out right after the wait, later ones when the
-        // MMA warp has released the Q buffers
-        bool q_pending = true;
-        auto before_load = [&](int32_t j) {                  // j == tile_end: end of the segment, Q must go out
-          if (!q_pending) return;
-          if (first && !waited && j < sv.tile_end && j < sv.g.stable_tiles && ring_it < (uint32_t)kStages) return;   // prefetch
-          ensure_wait();
-          if (!first) mbar_wait(bq_empty, (q_it & 1) ^ 1);
-          issue_q(sv);
-          q_pending = false;
-        };
-        if (!first) before_load(sv.tile_begin);
-        // one 128-key K or V tile -> the next ring slot: 64-key x 64-dim boxes at offsets 0 (keys 0-63,
-        // dims 0-63), 8 KB (keys 64-127), 16 KB and 24 KB (dims 64-127)
-        auto load_tile = [&](bool is_v, int32_t j, int32_t c0, int32_t c1) {
+        const int32_t nt = sv.tile_end - sv.tile_begin;
+        // ONE loop, ONE issue site for the K/V tiles of the segment (code size: the hot loops of the four warp
+        // roles have to stay inside the 32 KB instruction cache).  Order = consumption order of the MMA warp:
+        // general plan K0 V0 K1 V1 ..., decode plan K0 K1 | V0 K2 | V1 K3 | ... (K runs kAhead tiles ahead of V).
+        // The Q tiles go out once: the first segment's right after the wait (until then only tiles of its
+        // stable prefix are fetched, at most one ring of them), a later segment's when the MMA warp has
+        // released the Q buffers.
+        constexpr int32_t kAhead = kAlt ? 2 : 1;
+        int32_t nk = 0, nv = 0, pg0 = pre_pg0, pg1 = pre_pg1;
+        bool have_ids = first && pre_valid, q_pending = true;
+        for (;;) {
+          const bool is_v = !(nk < nt && nk < nv + kAhead);
+          const int32_t j = sv.tile_begin + (is_v ? nv : nk);
+          const bool at_end = nv >= nt;
+          if (q_pending && !(first && !waited && !at_end && j < sv.g.stable_tiles && ring_it < (uint32_t)kStages)) {
+            ensure_wait();
+            if (!first) mbar_wait(bq_empty, (q_it & 1) ^ 1);
+            issue_q(sv);
+            q_pending = false;
+          }
+          if (at_end) break;
+          // page ids of tile j (pool part): the general plan loads them with the K tile and keeps them for
+          // the V tile that follows (and fetches the next tile's one tile ahead when they are published)
+          int32_t c0, c1;
+          if constexpr (kAlt) {
+            const bool pre = have_ids && !is_v && nk == 0;
+            c0 = pre ? pre_pg0 : (j < Tc ? page_row[min(2 * j, last_page)] : 0);
+            c1 = pre ? pre_pg1 : (j < Tc ? page_row[min(2 * j + 1, last_page)] : 0);
+          } else {
+            if (!is_v) {
+              if (!have_ids) {
+                pg0 = j < Tc ? page_row[min(2 * j, last_page)] : 0;
+                pg1 = j < Tc ? page_row[min(2 * j + 1, last_page)] : 0;
+              }
+            }
+            c0 = pg0; c1 = pg1;
+            if (is_v) {
+              // next tile's ids one tile ahead - unless they may not be published yet
+              have_ids = j + 1 < sv.tile_end && j + 1 < Tc && (!q_pending || j + 1 < sv.g.stable_tiles);
+              if (have_ids) { pg0 = page_row[min(2 * j + 2, last_page)]; pg1 = page_row[min(2 * j + 3, last_page)]; }
+            }
+          }
+          // one 128-key K or V tile -> the next ring slot: 64-key x 64-dim boxes at offsets 0 (keys 0-63,
+          // dims 0-63), 8 KB (keys 64-127), 16 KB and 24 KB (dims 64-127)
           const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
           mbar_wait(bkv_empty(slot), par ^ 1);
           mbar_arrive_expect_tx(bkv_full(slot), kSlotBytes);
@@ -364,40 +403,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             tma_load_3d(dst + kHalfBytes + kHalfBytes / 2, tm, bkv_full(slot), 64, sv.g.kv_head, tok + 64);
           }
           ++ring_it;
-        };
-        auto page_of = [&](int32_t logical) { return logical <= 2 * Tc - 1 ? page_row[min(logical, last_page)] : 0; };
-        if constexpr (kAlt) {
-          // one Q tile serves both accumulator sets
-          auto load_alt = [&](bool is_v, int32_t j) {
-            before_load(j);
-            const bool pre = first && pre_valid && j == sv.tile_begin;   // ids fetched during set-up
-            load_tile(is_v, j, pre ? pre_pg0 : page_of(2 * j), pre ? pre_pg1 : page_of(2 * j + 1));
-          };
-          // consumption order of the MMA warp: K0 K1 | V0 K2 | V1 K3 | ...
-          load_alt(false, sv.tile_begin);
-          if (sv.tile_begin + 1 < sv.tile_end) load_alt(false, sv.tile_begin + 1);
-          for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
-            load_alt(true, j);
-            if (j + 2 < sv.tile_end) load_alt(false, j + 2);
-          }
-          before_load(sv.tile_end);                          // (a segment that fitted the prefetch window)
-          ++q_it;
-          continue;
+          if (is_v) ++nv; else ++nk;
         }
-        int32_t pg0 = pre_pg0, pg1 = pre_pg1;
-        bool have_ids = first && pre_valid;
-        for (int32_t j = sv.tile_begin; j < sv.tile_end; ++j) {
-          before_load(j);
-          if (!have_ids) { pg0 = page_of(2 * j); pg1 = page_of(2 * j + 1); }
-          const int32_t c0 = pg0, c1 = pg1;
-          // next tile's ids one tile ahead - unless they may not be published yet
-          have_ids = j + 1 < sv.tile_end && (!q_pending || j + 1 < sv.g.stable_tiles);
-          if (have_ids) { pg0 = page_of(2 * j + 2); pg1 = page_of(2 * j + 3); }
-          load_tile(false, j, c0, c1);
-          before_load(j);
-          load_tile(true, j, c0, c1);
-        }
-        before_load(sv.tile_end);
         ++q_it;
       }
       ensure_wait();
@@ -545,20 +552,6 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         ++q_it; ++seg_it;
       }
     }
-    if (warp >= 10 && p.append_tokens > 0) {
-      // ===================================================== a2 inside the fused step (kv_append.cuh)
-      // The pool rows and page-table entries written here are not read by this launch (its KV tiles over
-      // the new block come from k_new / v_new); at most the masked tail of a session's last cache page is
-      // overwritten while a tile holding it is in flight, which changes nothing: those keys carry P = 0
-      // and the bytes are finite before and after.
-      pdl_wait();
-      const AppendGeom geom{reinterpret_cast<const int4*>(p.k_new), reinterpret_cast<const int4*>(p.v_new),
-                            reinterpret_cast<int4*>(p.k_pool_w), reinterpret_cast<int4*>(p.v_pool_w),
-                            p.page_table_w, p.max_pages_per_session, p.P, p.Hkv, p.D * 2 / 16};
-      const MetaView<kInlineAppendWords> ameta{nullptr, app};
-      append_work(ameta, geom, peers, ((int64_t)blockIdx.x * 2 + (warp - 10)) * 32 + lane, (int64_t)gridDim.x * 64,
-                  (blockIdx.x == 0 && warp == 10) ? lane : -1, 32);
-    }
   } else {
     // ======================================================= softmax warpgroups (warps 0-7)
     setmaxnreg_inc<208>();
@@ -569,7 +562,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t t_s = tmem_base + (lane_base << 16) + q * 128;
     const uint32_t t_o = tmem_base + (lane_base << 16) + 256 + q * 128;
     const float c = p.scale * 1.4426950408889634f;
-    uint32_t tile_it = 0, seg_it = 0, alt_sync_it = 0;
+    uint32_t tile_it = 0, seg_it = 0;
     bool pdl_done = false;
     const bool fused = p.merge_ctr != nullptr;
     // publish this warpgroup's half of a partial: every thread's stores are fenced, the warpgroup
@@ -655,7 +648,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       // the previous tile have completed: s_full of the current tile was committed after them on the same
       // in-order tensor pipe.
       auto rescale_o = [&](float alpha) {
-#pragma unroll
+#pragma unroll 1                                            // rare path, inlined at three sites: keep it small
         for (int ch = 0; ch < 4; ++ch) {
           uint32_t o[32];
           tmem_ld32(t_o + ch * 32, o);
@@ -672,8 +665,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       // kCheck: the optimistic use - the reference may be stale, so each piece's row sum is tested against
       // sum_lim (kFastSumLimit / kFastSumShare; a NaN/inf sum fails the test).  Returns false, with nothing
       // handed off and S intact, if the first piece fails.
-      auto stream_tile = [&](auto check_tag, float sum_lim) -> bool {
-        constexpr bool kCheck = decltype(check_tag)::value;
+      auto stream_tile = [&](const bool kCheck, float sum_lim) -> bool {
         const float neg_mc = -m_used;
         uint32_t pk[64];                                    // P row, packed bf16x2
         uint64_t l01 = 0, l23 = 0;                          // packed fp32x2 partial row sums
@@ -751,36 +743,45 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         // ---- optimistic path: no look at the tile's maximum.  Not tried on the first tiles of a segment
         // (their sums are of the order of the accumulated l: the share test would refuse them anyway) nor
         // while a row has seen nothing yet (reference still -inf).
-        if (j >= kExactFirstTiles && !need_mask && !__any_sync(0xffffffffu, m_used == -INFINITY))
-          done = stream_tile(std::true_type{}, fminf(kFastSumLimit, kFastSumShare * l));
-        if (!done && !need_mask) {
-          // ---- exact path, unmasked tile: one pass over S for the row maximum, the reference follows
-          // it whenever it grew (the row's largest weight so far is then p = 1, exactly representable in
-          // bf16), then the same streaming pass as above against the now exact reference.
-          float mx0, mx1, mx2, mx3;
+        // ONE call site of stream_tile for both uses (attempt 0: optimistic, attempt 1: exact) - the loop is
+        // not unrolled: a second inlined copy of the streaming pass pushed the hot loops of the four warp
+        // roles out of the instruction cache (ncu: stall_no_inst x4 on the decode plan, 50 -> 66 us per step).
+        const bool try_fast = j >= kExactFirstTiles && !need_mask && !__any_sync(0xffffffffu, m_used == -INFINITY);
+        if (!need_mask) {
+#pragma unroll 1
+          for (int attempt = try_fast ? 0 : 1; attempt < 2 && !done; ++attempt) {
+            if (attempt == 1) {
+              // ---- exact path, unmasked tile: one pass over S for the row maximum, the reference follows
+              // it whenever it grew (the row's largest weight so far is then p = 1, exactly representable in
+              // bf16), then the same streaming pass against the now exact reference.
+              float mx0, mx1, mx2, mx3;
 #pragma unroll
-          for (int ch = 0; ch < 4; ++ch) {
-            uint32_t sr[32];
-            tmem_ld32(t_s + ch * 32, sr);
-            tmem_wait_ld();
-            if (ch == 0) { mx0 = __uint_as_float(sr[0]); mx1 = __uint_as_float(sr[1]); mx2 = __uint_as_float(sr[2]); mx3 = __uint_as_float(sr[3]); }
+              for (int ch = 0; ch < 4; ++ch) {
+                uint32_t sr[32];
+                tmem_ld32(t_s + ch * 32, sr);
+                tmem_wait_ld();
+                if (ch == 0) { mx0 = __uint_as_float(sr[0]); mx1 = __uint_as_float(sr[1]); mx2 = __uint_as_float(sr[2]); mx3 = __uint_as_float(sr[3]); }
 #pragma unroll
-            for (int i = (ch == 0 ? 4 : 0); i < 32; i += 4) {
-              mx0 = fmaxf(mx0, __uint_as_float(sr[i])); mx1 = fmaxf(mx1, __uint_as_float(sr[i + 1]));
-              mx2 = fmaxf(mx2, __uint_as_float(sr[i + 2])); mx3 = fmaxf(mx3, __uint_as_float(sr[i + 3]));
+                for (int i = (ch == 0 ? 4 : 0); i < 32; i += 4) {
+                  mx0 = fmaxf(mx0, __uint_as_float(sr[i])); mx1 = fmaxf(mx1, __uint_as_float(sr[i + 1]));
+                  mx2 = fmaxf(mx2, __uint_as_float(sr[i + 2])); mx3 = fmaxf(mx3, __uint_as_float(sr[i + 3]));
+                }
+              }
+              const float tm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;
+              const bool grow = tm > m_used;
+              if (j == 0) {
+                m_used = tm;
+              } else if (__any_sync(0xffffffffu, grow)) {
+                float alpha = 1.f;
+                if (grow) { alpha = m_used == -INFINITY ? 0.f : ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
+                rescale_o(alpha);
+              }
             }
+            // ---- attempt 0, optimistic: no look at the tile's maximum.  Not tried on the first tiles of a
+            // segment (their sums are of the order of the accumulated l: the share test would refuse them
+            // anyway) nor while a row has seen nothing yet (reference still -inf).
+            done = stream_tile(attempt == 0, attempt == 0 ? fminf(kFastSumLimit, kFastSumShare * l) : 0.f);
           }
-          const float tm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;
-          const bool grow = tm > m_used;
-          if (j == 0) {
-            m_used = tm;
-          } else if (__any_sync(0xffffffffu, grow)) {
-            float alpha = 1.f;
-            if (grow) { alpha = m_used == -INFINITY ? 0.f : ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
-            rescale_o(alpha);
-          }
-          stream_tile(std::false_type{}, 0.f);
-          done = true;
         }
         if (!done) {
           // ---- exact path, masked tile (the last tile of the cache part or of the new block when their
@@ -879,21 +880,21 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         // The two accumulator sets hold attention over the even / odd KV tiles of the segment for the
         // SAME rows: merge them here (LSE-weighted, exactly what the combine kernel does across
         // segments) so the segment yields one result.  Set 1 hands (lse2, 1/l) to warpgroup 0 through
-        // the shared memory of the unused second Q tile (double-buffered by segment parity);
+        // shared memory (Barriers::lse_stage, upper part; a second barrier keeps set 1 from overwriting it early);
         // warpgroup 0 reads O_1 straight from TMEM (same lanes) and releases it on set 1's behalf.
-        float2* xchg = reinterpret_cast<float2*>(smem_raw + (sQ - smem_u32(smem_raw)) + kQTileBytes) +
-                       (alt_sync_it & 1) * kTileRows;
-        ++alt_sync_it;
+        float2* xchg = reinterpret_cast<float2*>(&bars->lse_stage[kTileRows]);
         if (q == 1) {
           xchg[row_in_tile] = make_float2(lse2, inv_l);
           tc_fence_before();
           asm volatile("bar.sync 1, 256;" ::: "memory");
+          asm volatile("bar.sync 1, 256;" ::: "memory");    // warpgroup 0 has read the exchange area
           if (nt > 0) ++seg_it;
           continue;
         }
         asm volatile("bar.sync 1, 256;" ::: "memory");
         tc_fence_after();                                   // set 1's PV completion was observed by warpgroup 1
         const float2 peer = xchg[row_in_tile];
+        asm volatile("bar.sync 1, 256;" ::: "memory");
         use1 = sv.tile_end - sv.tile_begin >= 2;            // set 1 processed at least one tile
         const float mx = fmaxf(lse2, peer.x);
         if (mx == -INFINITY) {
@@ -1037,6 +1038,22 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         }
       }
     }
+  }
+
+  // (placed after the softmax code: the hot loops of producer, MMA issuer and softmax stay close together)
+  if (warp >= 10 && p.append_tokens > 0) {
+    // ===================================================== a2 inside the fused step (kv_append.cuh)
+    // The pool rows and page-table entries written here are not read by this launch (its KV tiles over
+    // the new block come from k_new / v_new); at most the masked tail of a session's last cache page is
+    // overwritten while a tile holding it is in flight, which changes nothing: those keys carry P = 0
+    // and the bytes are finite before and after.
+    pdl_wait();
+    const AppendGeom geom{reinterpret_cast<const int4*>(p.k_new), reinterpret_cast<const int4*>(p.v_new),
+                          reinterpret_cast<int4*>(p.k_pool_w), reinterpret_cast<int4*>(p.v_pool_w),
+                          p.page_table_w, p.max_pages_per_session, p.P, p.Hkv, p.D * 2 / 16};
+    const MetaView<kInlineAppendWords> ameta{nullptr, app};
+    append_work(ameta, geom, peers, ((int64_t)blockIdx.x * 2 + (warp - 10)) * 32 + lane, (int64_t)gridDim.x * 64,
+                (blockIdx.x == 0 && warp == 10) ? lane : -1, 32);
   }
 
   tc_fence_before();

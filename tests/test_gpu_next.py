@@ -238,7 +238,9 @@ def test_text_causal_split_kv_and_decode_plan(splits):
         o, l, o_ref, l_ref, a_ref, plans = _text_causal_case("bf16", Hq, Hkv, 128, 64, [256, 256, 130], [n, n], seed=40 + n,
                                                              mode="two_calls", min_splits=splits, p_text=0.6)
         assert plans[-1]["used_tensor_core_kernel"] == (3 if n == 16 else 1)
-        assert plans[-1]["num_segments"] >= Hkv * min(splits, (642 + 2 * n + 127) // 128)
+        nt = (642 + 2 * n + 127) // 128                               # KV tiles of the last step
+        per = -(-nt // splits)                                        # planner: tiles per forced piece
+        assert plans[-1]["num_segments"] >= Hkv * -(-nt // per)
         _gate_bf16(o, l, o_ref, l_ref, a_ref, f"n={n} splits={splits}")
 
 
