@@ -731,22 +731,32 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         return true;
       };
 
+      // Tiles that need the masked path, resolved ONCE per segment and warp (the tile loop itself stays free of
+      // votes and index arithmetic): in the pool part (t < Tc) tiles t >= mask_a, in the part read from k_new
+      // (t >= Tc) tiles t >= mask_b.  A tile needs a mask when it reaches beyond a row's visible end, or - mixed
+      // mask - beyond the position of a text row.
+      int32_t mask_a, mask_b;
+      {
+        const int32_t new_vis = max(vis - sv.g.cache_len, 0);
+        int32_t ma = vis_cache >> 7, mb = new_vis >> 7;
+        if (txt_pos >= 0) { ma = min(ma, (txt_pos + 1) >> 7); mb = min(mb, max(txt_pos + 1 - sv.g.cache_len, 0) >> 7); }
+        mask_a = __reduce_min_sync(0xffffffffu, ma);
+        mask_b = Tc + __reduce_min_sync(0xffffffffu, mb);
+      }
+      bool all_finite = false;                               // warp-uniform: every row's reference is finite
+
       for (int32_t j = 0; j < nt; ++j) {
         const int32_t t = sv.tile_begin + (kAlt ? 2 * j + q : j);
-        const int32_t key0 = t < Tc ? t * kTileKeys : sv.g.cache_len + (t - Tc) * kTileKeys;
-        const int32_t lim = t < Tc ? vis_cache : vis;        // keys >= lim of this tile are masked
         mbar_wait(bs_full(q), tile_it & 1);
         tc_fence_after();
-        const bool need_mask = __any_sync(0xffffffffu, key0 + kTileKeys > lim ||
-                                                       (txt_pos >= 0 && key0 + kTileKeys - 1 > txt_pos));
+        const bool need_mask = t >= (t < Tc ? mask_a : mask_b);
         bool done = false;
-        // ---- optimistic path: no look at the tile's maximum.  Not tried on the first tiles of a segment
-        // (their sums are of the order of the accumulated l: the share test would refuse them anyway) nor
-        // while a row has seen nothing yet (reference still -inf).
         // ONE call site of stream_tile for both uses (attempt 0: optimistic, attempt 1: exact) - the loop is
         // not unrolled: a second inlined copy of the streaming pass pushed the hot loops of the four warp
         // roles out of the instruction cache (ncu: stall_no_inst x4 on the decode plan, 50 -> 66 us per step).
-        const bool try_fast = j >= kExactFirstTiles && !need_mask && !__any_sync(0xffffffffu, m_used == -INFINITY);
+        // The optimistic pass is not tried on the first tiles of a segment (their sums are of the order of the
+        // accumulated l: the share test would refuse them anyway) nor while a row has seen nothing yet.
+        const bool try_fast = j >= kExactFirstTiles && all_finite;
         if (!need_mask) {
 #pragma unroll 1
           for (int attempt = try_fast ? 0 : 1; attempt < 2 && !done; ++attempt) {
@@ -776,16 +786,17 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 if (grow) { alpha = m_used == -INFINITY ? 0.f : ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
                 rescale_o(alpha);
               }
+              all_finite = !__any_sync(0xffffffffu, m_used == -INFINITY);
             }
-            // ---- attempt 0, optimistic: no look at the tile's maximum.  Not tried on the first tiles of a
-            // segment (their sums are of the order of the accumulated l: the share test would refuse them
-            // anyway) nor while a row has seen nothing yet (reference still -inf).
+            // ---- attempt 0, optimistic: no look at the tile's maximum
             done = stream_tile(attempt == 0, attempt == 0 ? fminf(kFastSumLimit, kFastSumShare * l) : 0.f);
           }
         }
         if (!done) {
           // ---- exact path, masked tile (the last tile of the cache part or of the new block when their
           // lengths are no multiples of 128; multi-block queries): whole S row in registers
+          const int32_t key0 = t < Tc ? t * kTileKeys : sv.g.cache_len + (t - Tc) * kTileKeys;
+          const int32_t lim = t < Tc ? vis_cache : vis;      // keys >= lim of this tile are masked
           uint32_t pk[64];
           uint32_t sr[128];                                 // one whole S row (fp32 bits)
           tmem_ld32(t_s + 0, sr + 0);
@@ -839,6 +850,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             rescale_o(alpha);
           }
           const float m_c = (m_used == -INFINITY) ? 0.f : m_used;
+          all_finite = !__any_sync(0xffffffffu, m_used == -INFINITY);
           float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
 #pragma unroll
           for (int i = 0; i < 128; i += 4) {
