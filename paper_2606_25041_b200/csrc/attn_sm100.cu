@@ -750,49 +750,49 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         mbar_wait(bs_full(q), tile_it & 1);
         tc_fence_after();
         const bool need_mask = t >= (t < Tc ? mask_a : mask_b);
-        bool done = false;
-        // ONE call site of stream_tile for both uses (attempt 0: optimistic, attempt 1: exact) - the loop is
-        // not unrolled: a second inlined copy of the streaming pass pushed the hot loops of the four warp
-        // roles out of the instruction cache (ncu: stall_no_inst x4 on the decode plan, 50 -> 66 us per step).
-        // The optimistic pass is not tried on the first tiles of a segment (their sums are of the order of the
-        // accumulated l: the share test would refuse them anyway) nor while a row has seen nothing yet.
-        const bool try_fast = j >= kExactFirstTiles && all_finite;
+        // ---- exact reference for an unmasked tile: one pass over S for the row maximum, the reference
+        // follows it whenever it grew (the row's largest weight so far is then p = 1, exactly representable
+        // in bf16).  Rare (first tiles of a segment, refused optimistic passes): kept out of the hot path.
+        auto exact_reference = [&]() {
+          float mx0, mx1, mx2, mx3;
+#pragma unroll
+          for (int ch = 0; ch < 4; ++ch) {
+            uint32_t sr[32];
+            tmem_ld32(t_s + ch * 32, sr);
+            tmem_wait_ld();
+            if (ch == 0) { mx0 = __uint_as_float(sr[0]); mx1 = __uint_as_float(sr[1]); mx2 = __uint_as_float(sr[2]); mx3 = __uint_as_float(sr[3]); }
+#pragma unroll
+            for (int i = (ch == 0 ? 4 : 0); i < 32; i += 4) {
+              mx0 = fmaxf(mx0, __uint_as_float(sr[i])); mx1 = fmaxf(mx1, __uint_as_float(sr[i + 1]));
+              mx2 = fmaxf(mx2, __uint_as_float(sr[i + 2])); mx3 = fmaxf(mx3, __uint_as_float(sr[i + 3]));
+            }
+          }
+          const float tm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;
+          const bool grow = tm > m_used;
+          if (j == 0) {
+            m_used = tm;
+          } else if (__any_sync(0xffffffffu, grow)) {
+            float alpha = 1.f;
+            if (grow) { alpha = m_used == -INFINITY ? 0.f : ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
+            rescale_o(alpha);
+          }
+          all_finite = !__any_sync(0xffffffffu, m_used == -INFINITY);
+        };
+        // ONE call site of stream_tile (a second inlined copy of the streaming pass pushed the hot loops of the
+        // four warp roles out of the instruction cache: ncu stall_no_inst x4 on the decode plan, 50 -> 66 us per
+        // step), reached by falling through in the common case: optimistic pass, accepted.  The optimistic pass
+        // is not tried on the first tiles of a segment (their sums are of the order of the accumulated l: the
+        // share test would refuse them anyway) nor while a row has seen nothing yet.
+        bool fast = j >= kExactFirstTiles && all_finite;
         if (!need_mask) {
 #pragma unroll 1
-          for (int attempt = try_fast ? 0 : 1; attempt < 2 && !done; ++attempt) {
-            if (attempt == 1) {
-              // ---- exact path, unmasked tile: one pass over S for the row maximum, the reference follows
-              // it whenever it grew (the row's largest weight so far is then p = 1, exactly representable in
-              // bf16), then the same streaming pass against the now exact reference.
-              float mx0, mx1, mx2, mx3;
-#pragma unroll
-              for (int ch = 0; ch < 4; ++ch) {
-                uint32_t sr[32];
-                tmem_ld32(t_s + ch * 32, sr);
-                tmem_wait_ld();
-                if (ch == 0) { mx0 = __uint_as_float(sr[0]); mx1 = __uint_as_float(sr[1]); mx2 = __uint_as_float(sr[2]); mx3 = __uint_as_float(sr[3]); }
-#pragma unroll
-                for (int i = (ch == 0 ? 4 : 0); i < 32; i += 4) {
-                  mx0 = fmaxf(mx0, __uint_as_float(sr[i])); mx1 = fmaxf(mx1, __uint_as_float(sr[i + 1]));
-                  mx2 = fmaxf(mx2, __uint_as_float(sr[i + 2])); mx3 = fmaxf(mx3, __uint_as_float(sr[i + 3]));
-                }
-              }
-              const float tm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;
-              const bool grow = tm > m_used;
-              if (j == 0) {
-                m_used = tm;
-              } else if (__any_sync(0xffffffffu, grow)) {
-                float alpha = 1.f;
-                if (grow) { alpha = m_used == -INFINITY ? 0.f : ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
-                rescale_o(alpha);
-              }
-              all_finite = !__any_sync(0xffffffffu, m_used == -INFINITY);
-            }
-            // ---- attempt 0, optimistic: no look at the tile's maximum
-            done = stream_tile(attempt == 0, attempt == 0 ? fminf(kFastSumLimit, kFastSumShare * l) : 0.f);
+          for (;;) {
+            if (!fast) exact_reference();
+            if (stream_tile(fast, fast ? fminf(kFastSumLimit, kFastSumShare * l) : 0.f)) break;
+            fast = false;
           }
         }
-        if (!done) {
+        if (need_mask) {
           // ---- exact path, masked tile (the last tile of the cache part or of the new block when their
           // lengths are no multiples of 128; multi-block queries): whole S row in registers
           const int32_t key0 = t < Tc ? t * kTileKeys : sv.g.cache_len + (t - Tc) * kTileKeys;
