@@ -192,18 +192,47 @@ def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, r
     gen = torch.Generator(device=dev); gen.manual_seed(2606)
     mk = lambda h: torch.randn((T, h, D), device=dev, dtype=torch.float32, generator=gen).bfloat16()
     q, k, v = mk(Hq), mk(Hkv), mk(Hkv)
-    for b in range(B):
-        c2.kv_append([sid], [0, n], k[b * n:(b + 1) * n], v[b * n:(b + 1) * n])
     o2 = torch.empty_like(q)
-    call = lambda i: c2.block_causal_attn_fwd([sid], [0, T], q, o2, 1.0 / math.sqrt(D), num_q_blocks=[B])
+    base2 = 0
+
+    def prefill(i):
+        # the whole prompt committed by ONE ws_kv_append_blocks call (32 block ends, one launch), then queried
+        # by ONE multi-block attention call
+        c2.session_truncate(sid, base2)
+        c2.kv_append_blocks([sid], [0, T], [0, B], [n] * B, k, v)
+        c2.block_causal_attn_fwd([sid], [0, T], q, o2, 1.0 / math.sqrt(D), num_q_blocks=[B])
     for i in range(3):
-        call(i)
+        prefill(i)
     reps = 30
-    ms = timed(reps, call)
+    ms = timed(reps, prefill)
+    call = lambda i: c2.block_causal_attn_fwd([sid], [0, T], q, o2, 1.0 / math.sqrt(D), num_q_blocks=[B])
+    ms_attn = timed(reps, call)
     fl = 4.0 * D * Hq * sum(n * n * (b + 1) for b in range(B))
-    res["prefill_multi_block"] = {"tokens": T, "blocks": B, "us": 1e3 * ms / reps,
+    res["prefill_multi_block"] = {"tokens": T, "blocks": B, "us": 1e3 * ms / reps, "us_attention_only": 1e3 * ms_attn / reps,
                                   "tflops": fl / (ms / reps * 1e-3) / 1e12,
-                                  "what": "32 committed blocks of 256 tokens queried in one call (block-causal FLOPs)"}
+                                  "what": "system prefill: 32 blocks of 256 tokens committed by one ws_kv_append_blocks call "
+                                          "and queried in one multi-block call (commit + attention timed together; "
+                                          "block-causal FLOPs)"}
+    # --- NEXT-4 (optional half): one unit of the headline shape with the text-causal mixed mask
+    # (192 video / 48 audio / 16 text slots interleaved per frame), fused step
+    from paper_2606_25041_b200 import WS_ATTN_TEXT_CAUSAL
+    tags = ([0] * 48 + [1] * 12 + [2] * 4) * (sp.block_tokens // 64) if sp.block_tokens % 64 == 0 else None
+    if tags is not None and len(ids) == 1:
+        import numpy as np
+        tg = np.asarray(tags * len(ids), dtype=np.uint8)
+
+        def tc_step(i):
+            reset()
+            cache.stream_step(ids, cu, q0, k0, v0, out, sp.scale, modality=tg, attn_flags=WS_ATTN_TEXT_CAUSAL)
+        for i in range(5):
+            tc_step(i)
+        reps = 100
+        ms_tc = timed(reps, tc_step)
+        reset()
+        res["text_causal_step"] = {"us_per_step": 1e3 * ms_tc / reps, "text_slots": int((tg == 2).sum()),
+                                   "what": "ws_stream_step_tagged with WS_ATTN_TEXT_CAUSAL on the headline shape "
+                                           "(text slots token-causal among themselves; only the tiles of the new "
+                                           "block take the masked path)"}
     c2.close()
     # --- NEXT-4: decode steps (n * G <= 128 packed rows: cache-read bound, decode plan) on the headline
     # session: n new tokens appended + attended against the 65,536-token history.  History (269 MB)

@@ -79,7 +79,11 @@ typedef struct {
   int32_t dtype;                  /* ws_dtype_t                                                    */
   int32_t num_q_heads;            /* Hq                                                            */
   int32_t num_kv_heads;           /* Hkv, Hq % Hkv == 0                                            */
-  int32_t head_dim;               /* D: bf16 tensor-core path D = 128; generic path D <= 256, D%8==0 */
+  int32_t head_dim;               /* D: bf16 tensor-core path D = 128; generic path D <= 256, D%8==0.
+                                   * A bf16 cache whose shape the tcgen05 kernel does not cover (D != 128, page != 64,
+                                   * Hq/Hkv not in {1,2,4,8,16}, explicit q_to_kv_head) is served by the generic
+                                   * CUDA-core kernel - same results, no tensor cores; ws_last_plan_info reports
+                                   * which kernel ran.  WS_ERR_UNSUPPORTED is returned only for shapes neither covers. */
   const int32_t* q_to_kv_head;    /* HOST [Hq] or NULL = grouped default                           */
   int32_t page_tokens;            /* P: tokens per page (64 for the bf16 tensor-core path)         */
   int32_t num_pages;              /* pages in each pool                                            */

@@ -24,7 +24,7 @@ __global__ void __launch_bounds__(256)
 kv_append_kernel(const int4* __restrict__ k_new, const int4* __restrict__ v_new,
                  int4* __restrict__ k_pool, int4* __restrict__ v_pool,
                  int32_t* __restrict__ page_table, const int32_t* __restrict__ meta_g,
-                 const __grid_constant__ InlineAppendMeta inl, const PeerPools peers,
+                 const __grid_constant__ InlineAppendMeta inl, const __grid_constant__ PeerPools peers,
                  int32_t max_pages, int32_t P, int32_t Hkv, int32_t chunks_per_head) {
   pdl_wait();
   pdl_launch_dependents();
@@ -68,7 +68,7 @@ page_table_publish_kernel(int32_t* __restrict__ page_table, const __grid_constan
 // all KV heads (one page = Hkv * P * D * eb contiguous bytes), local pool -> linked pools.
 __global__ void __launch_bounds__(256)
 kv_push_pages_kernel(const int4* __restrict__ k_pool, const int4* __restrict__ v_pool,
-                     const PeerPools peers, const int32_t* __restrict__ page_row, int32_t npages,
+                     const __grid_constant__ PeerPools peers, const int32_t* __restrict__ page_row, int32_t npages,
                      int32_t chunks_per_page) {
   const int64_t total = (int64_t)npages * chunks_per_page;
   for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
