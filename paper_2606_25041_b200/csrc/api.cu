@@ -670,7 +670,6 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
   char *h = nullptr, *d = nullptr;
 
   if (!tensor) {
-    if (fuse) return fail(WS_ERR_UNSUPPORTED, "internal: fused step on the generic kernel");
     if (c->dry && !c->tensor_path_ok) { c->last_plan = ws::Plan(); return WS_OK; }
     if (!c->dry) {
       // rows: session slot, visible end [, text position or -1, record offset; then the text-bit records]
@@ -678,7 +677,15 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
       tm.insert(tm.end(), vis_end.begin(), vis_end.end());
       if (text_causal) {
         tm.insert(tm.end(), txt_pos.begin(), txt_pos.end());
-        for (int32_t r : txt_rec) tm.push_back(4 * NQ + r);
+        tm.insert(tm.end(), txt_rec.begin(), txt_rec.end());      // (rebased below, once the row count is known)
+      }
+      if (fuse) {                      // committed length before this step's append, first row in k_new
+        for (int32_t s2 = 0; s2 < S; ++s2) tm.insert(tm.end(), (size_t)(cu[s2 + 1] - cu[s2]), vis_end[cu[s2]] - (cu[s2 + 1] - cu[s2]));
+        for (int32_t s2 = 0; s2 < S; ++s2) tm.insert(tm.end(), (size_t)(cu[s2 + 1] - cu[s2]), cu[s2]);
+      }
+      if (text_causal) {
+        for (int32_t& r : txt_rec) r += (int32_t)tm.size();
+        for (size_t t2 = 0; t2 < txt_rec.size(); ++t2) tm[3 * (size_t)NQ + t2] = txt_rec[t2];
         tm.insert(tm.end(), txt_words.begin(), txt_words.end());
       }
       const size_t bytes = tm.size() * 4;
@@ -697,13 +704,15 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
         st = upload_slot(c, h, d, bytes, stream);
         if (st != WS_OK) return st;
       }
+      ws::SimtFused sf{};
+      if (fuse) sf = ws::SimtFused{fuse->k_new, fuse->v_new, c->cfg.k_pool, c->cfg.v_pool, c->d_page_table, &fuse->ap->inl, NQ};
       TimedLaunch tl(c, &c->t_attn, stream);
       WS_CUDA(ws::launch_attn_simt(c->cfg.dtype, q, out, lse, c->cfg.k_pool, c->cfg.v_pool,
                                    c->d_page_table, (const int32_t*)d, inl,
                                    c->default_map ? nullptr : c->d_q_to_kv, NQ,
                                    c->cfg.max_pages_per_session, c->cfg.num_q_heads,
                                    c->cfg.num_kv_heads, c->cfg.head_dim, c->cfg.page_tokens, scale,
-                                   text_causal ? 1 : 0, stream));
+                                   text_causal ? 1 : 0, fuse ? &sf : nullptr, stream));
       tl.done();
       c->launches += 1;
       c->last_plan = ws::Plan();
@@ -908,7 +917,11 @@ ws_status_t ws_stream_step_tagged(ws_cache_t* c, int32_t S, const int32_t* sessi
   // One launch commits and attends when the tcgen05 kernel runs and the append descriptor fits the kernel
   // parameters (up to ~900 new pages per call); otherwise: the append kernel, then attention over the pool.
   const bool tensor = c->tensor_path_ok && !(c->cfg.flags & WS_FLAG_FORCE_SIMT);
-  if (tensor && ap.inline_meta && !(c->cfg.flags & WS_FLAG_SEPARATE_APPEND)) {
+  // (generic kernel: also one launch, when its per-token metadata fits the kernel parameters too and no replica
+  // is linked - the generic path does not mirror)
+  const bool simt_fusable = !tensor && !c->dry && c->peers.n == 0 &&
+                            (size_t)cu[S] * ((attn_flags & WS_ATTN_TEXT_CAUSAL) ? 7 : 4) + 64 <= (size_t)ws::kInlineAppendWords;
+  if ((tensor || simt_fusable) && ap.inline_meta && !(c->cfg.flags & WS_FLAG_SEPARATE_APPEND)) {
     const FusedAppend fuse{&ap, k_new, v_new};
     return attn_impl(c, S, session_ids, nullptr, cu, q, out, lse, scale, stream, &fuse, attn_flags);
   }

@@ -15,6 +15,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 
+#include "kv_append.cuh"
 #include "launch.h"
 
 namespace ws {
@@ -55,7 +56,9 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
                  const int32_t* __restrict__ page_table, const int32_t* __restrict__ tok_meta,
                  const __grid_constant__ InlineAppendMeta inl,
                  const int32_t* __restrict__ q_to_kv, int32_t total_q_tokens, int32_t max_pages,
-                 int32_t Hq, int32_t Hkv, int32_t D, int32_t P, float scale, int32_t text_causal) {
+                 int32_t Hq, int32_t Hkv, int32_t D, int32_t P, float scale, int32_t text_causal,
+                 const T* __restrict__ k_new, const T* __restrict__ v_new, T* k_pool_w, T* v_pool_w,
+                 int32_t* page_table_w, const __grid_constant__ InlineAppendMeta app, int32_t attn_blocks) {
   // per-token (session slot, visible end): device blob, or - small calls - the kernel parameter itself
   // (constant-bank reads; no host->device copy in the chain, so the call is CUDA-graph capturable)
   const MetaView<kInlineAppendWords> meta{tok_meta, inl};
@@ -63,6 +66,19 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
   // just before (ws_kv_append of the same step)
   pdl_wait();
   pdl_launch_dependents();
+  if ((int32_t)blockIdx.x >= attn_blocks) {
+    // fused step (ws_stream_step on the generic path): the blocks behind the attention blocks commit the new
+    // block to the pool (a2, kv_append.cuh) while the attention blocks read its keys straight from k_new / v_new
+    const AppendGeom geom{reinterpret_cast<const int4*>(k_new), reinterpret_cast<const int4*>(v_new),
+                          reinterpret_cast<int4*>(k_pool_w), reinterpret_cast<int4*>(v_pool_w), page_table_w,
+                          max_pages, P, Hkv, D * (int32_t)sizeof(T) / 16};
+    const MetaView<kInlineAppendWords> ameta{nullptr, app};
+    const PeerPools none{};
+    const int32_t b = (int32_t)blockIdx.x - attn_blocks, nb = (int32_t)gridDim.x - attn_blocks;
+    append_work(ameta, geom, none, (int64_t)b * blockDim.x + threadIdx.x, (int64_t)nb * blockDim.x,
+                b == 0 ? (int32_t)threadIdx.x : -1, (int32_t)blockDim.x);
+    return;
+  }
   __shared__ float q_s[kSimtWarps][kMaxD];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const int64_t w = (int64_t)blockIdx.x * kSimtWarps + wib;
@@ -79,6 +95,14 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
     txt_pos = meta[2 * total_q_tokens + tok];
     txt_rec = meta[3 * total_q_tokens + tok];
     txt_abs0 = meta[txt_rec];
+  }
+  // fused step: keys >= cache_len are rows new_row0 .. of k_new / v_new (two more metadata rows, after the
+  // text rows if present); otherwise every key comes from the pool
+  int32_t cache_len = vis, new_row0 = 0;
+  if (k_new != nullptr) {
+    const int32_t base = (text_causal ? 4 : 2) * total_q_tokens;
+    cache_len = meta[base + tok];
+    new_row0 = meta[base + total_q_tokens + tok];
   }
   const int32_t* page_row = page_table + (int64_t)slot * max_pages;
 
@@ -102,8 +126,9 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
     float s = -INFINITY;
     int32_t rowidx = 0;
     if (valid) {
-      rowidx = (page_row[j / P] * Hkv + g) * P + (j % P);
-      const T* kp = k_pool + (int64_t)rowidx * D;
+      // rowidx >= 0: row of the pool; < 0: row -(rowidx + 1) of k_new / v_new
+      rowidx = j < cache_len ? (page_row[j / P] * Hkv + g) * P + (j % P) : -1 - ((new_row0 + j - cache_len) * Hkv + g);
+      const T* kp = rowidx >= 0 ? k_pool + (int64_t)rowidx * D : k_new + (int64_t)(-1 - rowidx) * D;
       float a = 0.f;
 #pragma unroll 4
       for (int d = 0; d < D; d += VN) {
@@ -137,7 +162,8 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
       for (int u = 0; u < kBatch; ++u) {
         const int kk = (kk0 + u) & 31;
         pk[u] = kk0 + u < nk ? __shfl_sync(0xffffffffu, p, kk) : 0.f;
-        vp[u] = v_pool + (int64_t)__shfl_sync(0xffffffffu, rowidx, kk) * D;
+        const int32_t ri = __shfl_sync(0xffffffffu, rowidx, kk);
+        vp[u] = ri >= 0 ? v_pool + (int64_t)ri * D : v_new + (int64_t)(-1 - ri) * D;
       }
 #pragma unroll
       for (int i = 0; i < kMaxD / 32; ++i) {
@@ -167,18 +193,34 @@ cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse
                              const void* k_pool, const void* v_pool, const int32_t* page_table,
                              const int32_t* tok_meta, const InlineAppendMeta& inl, const int32_t* q_to_kv,
                              int32_t total_q_tokens, int32_t max_pages, int32_t Hq, int32_t Hkv, int32_t D,
-                             int32_t P, float scale, int32_t text_causal, cudaStream_t stream) {
+                             int32_t P, float scale, int32_t text_causal, const SimtFused* fused, cudaStream_t stream) {
   int64_t warps = (int64_t)total_q_tokens * Hq;
   int32_t grid = (int32_t)((warps + kSimtWarps - 1) / kSimtWarps);
   if (grid == 0) return cudaSuccess;
+  const int32_t attn_blocks = grid;
+  const void *k_new = nullptr, *v_new = nullptr;
+  void *kw = nullptr, *vw = nullptr;
+  int32_t* ptw = nullptr;
+  InlineAppendMeta app_none;
+  const InlineAppendMeta* app = &app_none;
+  if (fused) {
+    k_new = fused->k_new; v_new = fused->v_new; kw = fused->k_pool_w; vw = fused->v_pool_w; ptw = fused->page_table_w;
+    app = fused->app;
+    const int64_t chunks = (int64_t)std::max(fused->append_tokens, P - 1) * Hkv * (D * (dtype == 1 ? 4 : 2) / 16);
+    grid += (int32_t)std::min<int64_t>(std::max<int64_t>((chunks + kSimtWarps * 32 - 1) / (kSimtWarps * 32), 1), 148 * 4);
+  } else {
+    app_none.w[0] = 0;
+  }
   if (dtype == 1)
     return launch_pdl(attn_simt_kernel<float>, dim3(grid), dim3(kSimtWarps * 32), 0, stream,
                       (const float*)q, (float*)out, lse, (const float*)k_pool, (const float*)v_pool, page_table,
-                      tok_meta, inl, q_to_kv, total_q_tokens, max_pages, Hq, Hkv, D, P, scale, text_causal);
+                      tok_meta, inl, q_to_kv, total_q_tokens, max_pages, Hq, Hkv, D, P, scale, text_causal,
+                      (const float*)k_new, (const float*)v_new, (float*)kw, (float*)vw, ptw, *app, attn_blocks);
   return launch_pdl(attn_simt_kernel<__nv_bfloat16>, dim3(grid), dim3(kSimtWarps * 32), 0, stream,
                     (const __nv_bfloat16*)q, (__nv_bfloat16*)out, lse, (const __nv_bfloat16*)k_pool,
                     (const __nv_bfloat16*)v_pool, page_table, tok_meta, inl, q_to_kv, total_q_tokens, max_pages,
-                    Hq, Hkv, D, P, scale, text_causal);
+                    Hq, Hkv, D, P, scale, text_causal, (const __nv_bfloat16*)k_new, (const __nv_bfloat16*)v_new,
+                    (__nv_bfloat16*)kw, (__nv_bfloat16*)vw, ptw, *app, attn_blocks);
 }
 
 }  // namespace ws

@@ -58,11 +58,20 @@ cudaError_t launch_fm_euler(int32_t dtype, void* z, const void* v, float dtau, i
 // tok_meta: [2][total_q_tokens] int32 = session slot, visible end per query token; nullptr: the same
 // words are in `inl` (kernel parameter, 2 * total_q_tokens <= kInlineAppendWords).  text_causal: two more
 // rows (text position or -1, record offset) followed by the sessions' text-bit records (attn_simt.cu).
+// fused != nullptr: ws_stream_step on the generic path - the launch also commits the block (extra thread blocks run
+// the append) and reads its keys from k_new / v_new; tok_meta then carries two more rows per token (committed
+// length before the append, first row of the session's block in k_new).
+struct SimtFused {
+  const void* k_new; const void* v_new;
+  void* k_pool_w; void* v_pool_w; int32_t* page_table_w;
+  const InlineAppendMeta* app;
+  int32_t append_tokens;
+};
 cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse,
                              const void* k_pool, const void* v_pool, const int32_t* page_table,
                              const int32_t* tok_meta, const InlineAppendMeta& inl, const int32_t* q_to_kv,
                              int32_t total_q_tokens, int32_t max_pages, int32_t Hq, int32_t Hkv, int32_t D,
-                             int32_t P, float scale, int32_t text_causal, cudaStream_t stream);
+                             int32_t P, float scale, int32_t text_causal, const SimtFused* fused, cudaStream_t stream);
 
 // sm_100a tcgen05 kernel (bf16, D = 128, P = 64).
 struct Sm100Launch {

@@ -270,3 +270,36 @@ def test_text_causal_bf16_generic_kernel():
                                                          flags=WS_FLAG_FORCE_SIMT)
     assert all(p["used_tensor_core_kernel"] == 0 for p in plans)
     _gate_bf16(o, l, o_ref, l_ref, a_ref, "bf16 generic kernel")
+
+
+# ------------------------------------------------------------------------------------------ generic kernel, fused step
+def test_generic_kernel_fused_step_config1_and_bf16():
+    """ws_stream_step on the generic (CUDA-core) path is ONE launch as well: the attention blocks read the new
+    block's keys from k_new / v_new, extra blocks of the same grid commit it.  Config 1 (fp32, 1e-5) and a bf16
+    case forced onto the generic kernel; append bit-exact; one launch per step."""
+    from paper_2606_25041_b200 import WS_FLAG_FORCE_SIMT
+    from synth_inputs import generate, spec_for_config
+    from tests.gpu_harness import compare, run_workload_gpu, run_workload_oracle
+    w = generate(spec_for_config(1))
+    ref = run_workload_oracle(w)
+    got = run_workload_gpu(w, fused_step=True, pool_fill=0x7FC00001)
+    err = compare(got, ref, "fp32")
+    print("[parity] config 1, fused generic step:", {k: v for k, v in err.items()})
+    assert err["finite"] and err["max_abs"] <= 1e-5 and err["lse_max"] <= 1e-5 and err["kv_bit_exact"]
+    two = run_workload_gpu(w, fused_step=False)
+    assert got["launches"] == two["launches"] - w.spec.steps            # one launch fewer per step
+    wb = generate(spec_for_config(2, cache_lens=(333,), num_q_heads=4, num_kv_heads=2, block_tokens=40,
+                                  modality_split=(30, 8, 2), steps=3))
+    refb = run_workload_oracle(wb)
+    gotb = run_workload_gpu(wb, flags=WS_FLAG_FORCE_SIMT, fused_step=True, pool_fill=0x7FC1)
+    errb = compare(gotb, refb, "bf16")
+    print("[parity] bf16 generic kernel, fused step:", {k: v for k, v in errb.items()})
+    assert not gotb["tensor"]
+    assert errb["finite"] and errb["max_abs"] <= 1e-2 and errb["mean_abs"] <= 1e-3 and errb["bound_viol"] <= 0
+    assert errb["lse_max"] <= 1e-4 and errb["kv_bit_exact"]
+
+
+def test_text_causal_generic_fp32_fused_step():
+    o, l, o_ref, l_ref, _, plans = _text_causal_case("fp32", 2, 2, 64, 16, [16], [16, 16, 40], seed=4, mode="fused", p_text=0.4)
+    assert all(p["used_tensor_core_kernel"] == 0 for p in plans)
+    assert np.abs(o - o_ref).max() <= 1e-5 and np.abs(l - l_ref).max() <= 1e-5
