@@ -154,7 +154,7 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
 #pragma unroll
     for (int i = 0; i < kMaxD / 32; ++i) acc[i] *= corr;
     const int nk = min(32, vis - base);
-    constexpr int kBatch = 8;
+    constexpr int kBatch = 16;                          // V rows in flight per lane (the loop is bound by load latency)
     for (int kk0 = 0; kk0 < nk; kk0 += kBatch) {
       float pk[kBatch];
       const T* vp[kBatch];
