@@ -18,7 +18,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 OUT = os.path.join(PKG, "libwanstream.so")
 OBJ = os.path.join(PKG, "build")
-SOURCES = ["api.cu", "kv_append.cu", "attn_simt.cu", "attn_sm100.cu", "combine.cu", "fm_euler.cu",
+SOURCES = ["api.cu", "kv_append.cu", "attn_simt.cu", "attn_sm100.cu", "attn_dec_sm100.cu", "combine.cu", "fm_euler.cu",
            "host_cache.cpp", "plan.cpp"]
 NVCC = "/usr/local/cuda/bin/nvcc"
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -87,6 +87,10 @@ struct Sm100Launch {
 };
 cudaError_t sm100_attn_configure();    // one-time cudaFuncSetAttribute
 cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream);
+// decode kernel (attn_dec_sm100.cu): decode plans (at most 128 packed query rows per (session, KV head)), both
+// softmax warpgroups on every KV tile; no in-kernel merge phase
+cudaError_t dec_sm100_configure();
+cudaError_t launch_attn_dec_sm100(const Sm100Launch& l, cudaStream_t stream);
 cudaError_t combine_configure();        // one-time cudaFuncSetAttribute
 cudaError_t launch_combine(const AttnParams& p, const InlineAttnMetaLarge& inl, int32_t inl_words,
                            int32_t num_combine, int32_t team_size, int32_t max_parts, cudaStream_t stream);

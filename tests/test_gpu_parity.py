@@ -263,7 +263,8 @@ def test_fused_combine_decode_plan_and_ragged_batch():
     from paper_2606_25041_b200 import WS_FLAG_FUSED_COMBINE
     w = _small(3, cache_lens=(6000,), block_tokens=16, modality_split=(12, 3, 1), steps=2)
     got = run_workload_gpu(w, flags=WS_FLAG_FUSED_COMBINE, min_splits=5, gather=False)
-    assert got["plans"][-1]["used_tensor_core_kernel"] == 3 and got["plans"][-1]["num_combine_items"] > 0
+    # (the decode kernel has no merge phase: WS_FLAG_FUSED_COMBINE runs the decode plan on the general kernel, 4)
+    assert got["plans"][-1]["used_tensor_core_kernel"] == 4 and got["plans"][-1]["num_combine_items"] > 0
     _assert_close(compare(got, run_workload_oracle(w), "bf16"), BF16_TOL, "fused combine, decode plan")
     w = _small(5, cache_len_range=(100, 1500), block_tokens=64, modality_split=(48, 12, 4))
     got = run_workload_gpu(w, flags=WS_FLAG_FUSED_COMBINE, gather=False)
@@ -411,6 +412,9 @@ def test_next4_decode_plan_matches_oracle(label, ov):
     gen = run_workload_gpu(w, pool_fill=0x7FC1, decode_plan=False, gather=False)
     assert all(pl["used_tensor_core_kernel"] == 1 for pl in gen["plans"])
     _assert_close(compare(gen, ref, "bf16"), BF16_TOL, label + " (general plan)")
+    old = run_workload_gpu(w, pool_fill=0x7FC1, decode_plan=2, fused_step=True, gather=False)
+    assert all(pl["used_tensor_core_kernel"] == 4 for pl in old["plans"])
+    _assert_close(compare(old, ref, "bf16"), BF16_TOL, label + " (decode plan on the general kernel)")
 
 
 @pytest.mark.parametrize("splits", [1, 2, 5, 40])
