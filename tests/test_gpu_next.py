@@ -303,3 +303,41 @@ def test_text_causal_generic_fp32_fused_step():
     o, l, o_ref, l_ref, _, plans = _text_causal_case("fp32", 2, 2, 64, 16, [16], [16, 16, 40], seed=4, mode="fused", p_text=0.4)
     assert all(p["used_tensor_core_kernel"] == 0 for p in plans)
     assert np.abs(o - o_ref).max() <= 1e-5 and np.abs(l - l_ref).max() <= 1e-5
+
+
+@pytest.mark.parametrize("n", [4, 64], ids=["decode_kernel", "general_plan"])
+def test_text_causal_ragged_multi_session_batch(n):
+    """Three sessions with different history lengths in ONE fused call, text-causal mixed mask, each session's
+    block with its own tag pattern (the text-bit records are per session); vs the oracle."""
+    import torch
+    from oracle.block_causal import OracleSession, attend
+    from paper_2606_25041_b200 import WS_ATTN_TEXT_CAUSAL
+    rng = np.random.default_rng(90 + n)
+    dev = torch.device("cuda", 0)
+    Hq, Hkv, D = 8, 2, 128
+    lens = [300, 1000, 77]
+    c = _cache("bf16", Hq, Hkv, D, 64, max(lens) + 4 * n + 64, sessions=3, max_q=max(512, 3 * n))
+    ids = [c.session_open() for _ in lens]
+    sess = [OracleSession(Hkv, D) for _ in lens]
+    for s, L in enumerate(lens):
+        kk, vv, tg = _mk(rng, "bf16", L, Hkv, D), _mk(rng, "bf16", L, Hkv, D), _tags(rng, L)
+        c.kv_append([ids[s]], [0, L], _torch_of(kk, dev), _torch_of(vv, dev), modality=tg)
+        sess[s].append(kk, vv, modality=tg)
+    scale = 1.0 / math.sqrt(D)
+    for step in range(2):
+        qs, ks, vs, tgs = [], [], [], []
+        for s in range(3):
+            qs.append(_mk(rng, "bf16", n, Hq, D)); ks.append(_mk(rng, "bf16", n, Hkv, D)); vs.append(_mk(rng, "bf16", n, Hkv, D))
+            tgs.append(_tags(rng, n, 0.5))
+            sess[s].append(ks[-1], vs[-1], modality=tgs[-1])
+        out = torch.full((3 * n, Hq, D), float("nan"), dtype=torch.bfloat16, device=dev)
+        lse = torch.full((3 * n, Hq), float("nan"), dtype=torch.float32, device=dev)
+        c.stream_step(ids, [0, n, 2 * n, 3 * n], _torch_of(np.concatenate(qs), dev), _torch_of(np.concatenate(ks), dev),
+                      _torch_of(np.concatenate(vs), dev), out, scale, lse=lse, modality=np.concatenate(tgs),
+                      attn_flags=WS_ATTN_TEXT_CAUSAL)
+        torch.cuda.synchronize()
+        assert c.last_plan_info()["used_tensor_core_kernel"] == (3 if n == 4 else 1)
+        o = out.float().cpu().numpy().astype(np.float64); l = lse.cpu().numpy().astype(np.float64)
+        refs = [attend(sess[s], qs[s], scale, 1, want_abs=True, text_causal=True) for s in range(3)]
+        o_ref, l_ref, a_ref = (np.concatenate([r[i] for r in refs]) for i in range(3))
+        _gate_bf16(o, l, o_ref, l_ref, a_ref, f"ragged 3-session batch n={n} step {step}")
