@@ -316,7 +316,7 @@ def test_text_causal_ragged_multi_session_batch(n):
     dev = torch.device("cuda", 0)
     Hq, Hkv, D = 8, 2, 128
     lens = [300, 1000, 77]
-    c = _cache("bf16", Hq, Hkv, D, 64, max(lens) + 4 * n + 64, sessions=3, max_q=max(512, 3 * n))
+    c = _cache("bf16", Hq, Hkv, D, 64, max(lens) + 4 * n + 64, sessions=3, max_q=max(lens))
     ids = [c.session_open() for _ in lens]
     sess = [OracleSession(Hkv, D) for _ in lens]
     for s, L in enumerate(lens):
