@@ -64,7 +64,7 @@ enum {
    * until all splits of its (session, KV head) group are there and merges its share of the rows; the
    * kernel is then launched cooperatively so that all CTAs are co-resident while they wait on each
    * other.  Correct and one launch fewer, but measured no faster than the separate kernel on B200
-   * (DESIGN.md section 8), so it is opt-in.                                                         */
+   * (DESIGN.md section 8), so it is opt-in.  Decode plans ignore it (the decode kernel has no merge phase). */
   WS_FLAG_FUSED_COMBINE = 8u,
   /* ws_stream_step normally commits and attends a block in ONE launch (the attention kernel reads the
    * new keys from k_new / v_new and two of its warps copy them into the pool).  With this flag it
@@ -290,16 +290,15 @@ ws_status_t ws_debug_set_min_splits(ws_cache_t* cache, int32_t min_splits);
 /* NEXT-4 (token-causal text decode: "short token-causal Transformer pass ... over
  * the language and state slots"): when every session of a call has at most 128 packed query rows
  * (n_q * Hq/Hkv <= 128) the step is cache-read bound and the scheduler switches the tcgen05 kernel to
- * the decode plan, run by the decode kernel: one Q tile per CTA, BOTH softmax warpgroups on every KV tile (64 of
- * its 128 keys each), S double-buffered by tile parity.  enable = 1 (default): automatic; 0: always the general
- * plan; 2: the decode plan on the general kernel (two accumulator sets on alternate KV tiles - what
- * WS_FLAG_FUSED_COMBINE uses as well).  For A/B measurements and tests. */
+ * the decode plan, run by the decode kernel (attn_dec_sm100.cu): one Q tile per CTA, BOTH softmax warpgroups on
+ * every KV tile (64 of its 128 keys each), S double-buffered by tile parity.  Enabled by default; this switch
+ * forces the general plan (A/B measurements and tests). */
 ws_status_t ws_debug_set_decode_plan(ws_cache_t* cache, int32_t enable);
 
 /* Description of the last attention plan built on this cache (a1): CTAs launched, team size,
  * number of (session,KV-head) groups, KV segments, split partial slots, combine items, and whether
- * the tcgen05 kernel (1; 3 = decode plan on the decode kernel; 4 = decode plan on the general kernel) or the
- * generic SIMT kernel (0) was selected. */
+ * the tcgen05 kernel (1 = general kernel; 3 = decode plan on the decode kernel) or the generic SIMT kernel (0)
+ * was selected. */
 typedef struct {
   int32_t num_ctas, team_size, num_groups, num_segments, num_partial_slots, num_combine_items;
   int32_t used_tensor_core_kernel, total_kv_tiles;

@@ -367,8 +367,7 @@ class Cache:
     def set_min_splits(self, n: int) -> None:
         _check(self.lib.ws_debug_set_min_splits(self.handle, n))
 
-    def set_decode_plan(self, enable) -> None:
-        """True / 1: automatic (default); False / 0: general plan only; 2: decode plan on the general kernel."""
+    def set_decode_plan(self, enable: bool) -> None:
         _check(self.lib.ws_debug_set_decode_plan(self.handle, int(enable)))
 
     def last_plan_info(self) -> dict:

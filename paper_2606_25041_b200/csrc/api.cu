@@ -149,8 +149,6 @@ struct ws_cache {
   CUtensorMap tmap_k{}, tmap_v{};
   int32_t min_splits = 0;
   bool decode_plan_enabled = true;
-  bool decode_kernel_enabled = true;       // decode plans run attn_dec_sm100.cu (else attn_sm100.cu's alternate-tile plan)
-  bool last_dec_kernel = false;
   int64_t launches = 0;
   ws::Plan last_plan;
   bool last_tensor = false;
@@ -460,7 +458,6 @@ ws_status_t ws_debug_shuffle_free_pages(ws_cache_t* c, uint64_t seed) {
 ws_status_t ws_debug_set_decode_plan(ws_cache_t* c, int32_t enable) {
   if (!c) return fail(WS_ERR_INVALID_ARG, "cache is NULL");
   c->decode_plan_enabled = enable != 0;
-  c->decode_kernel_enabled = enable == 1;
   return WS_OK;
 }
 
@@ -766,10 +763,6 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
     memcpy(h, blob.data(), blob.size() * 4);
   }
   c->last_plan = std::move(plan);
-  // decode plans run the decode kernel (both softmax warpgroups on every KV tile); it has no in-kernel merge
-  // phase, so WS_FLAG_FUSED_COMBINE keeps attn_sm100.cu's alternate-tile decode plan
-  c->last_dec_kernel = c->last_plan.alt && c->decode_kernel_enabled &&
-                       !((c->cfg.flags & WS_FLAG_FUSED_COMBINE) && !c->last_plan.combine.empty());
   if (c->dry) return WS_OK;
 
   ws::Sm100Launch L{};
@@ -777,7 +770,8 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
   L.p.k_pool = c->cfg.k_pool; L.p.v_pool = c->cfg.v_pool;
   L.p.page_table = c->d_page_table;
   L.p.part_o = c->d_part_o; L.p.part_lse = c->d_part_lse;
-  const bool fused_combine = (c->cfg.flags & WS_FLAG_FUSED_COMBINE) && !c->last_plan.combine.empty();
+  // (decode plans run on the decode kernel, which has no in-kernel merge phase: they keep the combine kernel)
+  const bool fused_combine = (c->cfg.flags & WS_FLAG_FUSED_COMBINE) && !c->last_plan.combine.empty() && !c->last_plan.alt;
   L.p.merge_ctr = fused_combine ? c->d_merge_ctr : nullptr;
   L.p.max_part_slots = c->lay.max_part_slots;
   L.p.max_pages_per_session = c->cfg.max_pages_per_session;
@@ -819,7 +813,7 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
   L.num_ctas = c->last_plan.num_teams * c->last_plan.team_size;
   L.alt = c->last_plan.alt;
   TimedLaunch tl(c, &c->t_attn, stream);
-  if (c->last_dec_kernel) WS_CUDA(ws::launch_attn_dec_sm100(L, stream));
+  if (L.alt) WS_CUDA(ws::launch_attn_dec_sm100(L, stream));
   else WS_CUDA(ws::launch_attn_sm100(L, stream));
   tl.done();
   c->launches += 1;
@@ -1223,7 +1217,7 @@ ws_status_t ws_last_plan_info(const ws_cache_t* c, ws_plan_info_t* out) {
   out->num_segments = (int32_t)p.segments.size();
   out->num_partial_slots = p.num_part_slots;
   out->num_combine_items = (int32_t)p.combine.size();
-  out->used_tensor_core_kernel = c->last_tensor ? (p.alt ? (c->last_dec_kernel ? 3 : 4) : 1) : 0;
+  out->used_tensor_core_kernel = c->last_tensor ? (p.alt ? 3 : 1) : 0;
   out->total_kv_tiles = p.total_tiles;
   return WS_OK;
 }

@@ -3,7 +3,7 @@
 // token-causal Transformer pass", :77 "token-causal decoding over the language and state slots").
 //
 // Such a step is cache-read bound (HBM needs ~1400 cycles per 128-key tile and SM).  With one softmax warpgroup
-// per tile (attn_sm100.cu's decode plan: two accumulator sets on alternate tiles) a tile costs ~2300 cycles: the
+// per tile (round 1: two accumulator sets of the general kernel on alternate tiles) a tile costs ~2300 cycles: the
 // chain S -> softmax (~1500 cycles, 128 keys per thread) -> PV -> next S of a set is pure latency, and two sets
 // do not hide it.  Here BOTH warpgroups work on EVERY tile, 64 of its 128 keys each
 // (thread = row, as before): softmax latency per tile halves, S is double-buffered by tile parity, and there is

@@ -54,13 +54,9 @@ namespace ws {
 
 using namespace ptx;
 
-// K/V ring: slots of one 128-key tile (32 KB).  General plan: two Q tiles + 5 slots.  Decode plan: ONE Q tile,
-// so its ring starts where the second Q tile would be and has 6 slots - the decode step is bound by the
-// latency of the K/V stream (a slot is held from the issue of its load until the MMA that reads it has
-// completed, V slots until the softmax of their tile is through), every slot counts.
-constexpr int kStagesGen = 5, kStagesAlt = 6, kStagesMax = 6;
+constexpr int kStages = 5;                                 // K/V ring: 5 slots of one 128-key tile (32 KB)
 constexpr uint32_t kSlotBytes = 32768;
-constexpr uint32_t kRingBytes = kStagesGen * kSlotBytes;   // capacity both plans have
+constexpr uint32_t kRingBytes = kStages * kSlotBytes;
 constexpr uint32_t kHalfBytes = 16384;                     // one 64-dim half of a 128-row tile: 128 rows x 128 B
 constexpr uint32_t kQTileBytes = kTileRows * 128 * 2;
 constexpr int kThreads = 384;
@@ -83,19 +79,16 @@ constexpr int kMaxJobs = 4;
 
 struct Barriers {
   uint64_t q_full, q_empty;
-  uint64_t kv_full[kStagesMax], kv_empty[kStagesMax];
+  uint64_t kv_full[kStages], kv_empty[kStages];
   uint64_t s_full[2], p_full[2][2], pv_h0_done[2], o_full[2], o_empty[2];
   uint64_t merge_full;
-  // staged epilogue: the pair's log2-LSEs on their way to part_lse ([0, 256); the decode plan uses [0, 128) and
-  // exchanges (LSE, 1/l) of its second accumulator set through the 1 KB that starts at float 128)
-  alignas(16) float lse_stage[kPairRows + kTileRows];
+  alignas(16) float lse_stage[kPairRows];                  // staged epilogue: the pair's log2-LSEs on their way to part_lse
   MergeJob jobs[kMaxJobs];
-  int32_t njobs, cur_slot0;          // staged epilogue: the pair's log2-LSEs on their way to part_lse
+  int32_t njobs, cur_slot0;          // fused combine: parked merge jobs, first partial slot of the current (item, pair)
   uint32_t tmem_base;
   uint32_t pad;
 };
 constexpr uint32_t kSmemBytes = 2 * kQTileBytes + kRingBytes + sizeof(Barriers) + 1024;
-static_assert(kQTileBytes + kStagesAlt * kSlotBytes == 2 * kQTileBytes + kRingBytes, "both plans fill the same area");
 static_assert(kSmemBytes <= 232448, "227 KB of shared memory per CTA");
 
 struct SegView {
@@ -151,8 +144,7 @@ __device__ __forceinline__ void red_release_gpu_add(int32_t* p, int32_t v) {
   asm volatile("red.release.gpu.global.add.s32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
 }
 
-// kAlt: decode plan (plan.h) - both accumulator sets use Q tile 0; set q processes the KV tiles of the
-// segment with (tile - tile_begin) % 2 == q and writes its own partial (slot part_base + q).
+// (Decode plans - at most 128 packed rows per group - run on attn_dec_sm100.cu.)
 //
 // Programmatic dependent launch (protocol: launch.h).  Before griddepcontrol.wait the TMA producer fetches
 // only KV tiles of the stable prefix of its first segment (Group::stable_tiles: committed at least two
@@ -162,7 +154,7 @@ __device__ __forceinline__ void red_release_gpu_add(int32_t* p, int32_t v) {
 // the append warps wait before their first store, every softmax thread before its first global write
 // (out / partials may still be read or written by the previous step's kernels).  Metadata in a device blob
 // (p.meta: large calls, uploaded by a stream-ordered copy) is only read after the wait.
-template <int kInlW, bool kAlt>
+template <int kInlW>
 __global__ void __launch_bounds__(kThreads, 1)
 attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ CUtensorMap tmap_k,
@@ -178,8 +170,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem_base;                           // 2 x 32 KB
-  constexpr int kStages = kAlt ? kStagesAlt : kStagesGen;
-  const uint32_t sRing = smem_base + (kAlt ? 1 : 2) * kQTileBytes;   // kStages x kSlotBytes
+  const uint32_t sRing = smem_base + 2 * kQTileBytes;      // kStages x kSlotBytes
   Barriers* bars = reinterpret_cast<Barriers*>(smem_raw + (smem_base - smem_u32(smem_raw)) +
                                                2 * kQTileBytes + kRingBytes);
   const uint32_t bq_full = smem_u32(&bars->q_full), bq_empty = smem_u32(&bars->q_empty);
@@ -206,20 +197,14 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   SegView sv_first;
   int32_t si_first = seg_hi, pre_pg0 = 0, pre_pg1 = 0;
   bool pre_valid = false;
-  // Q tiles of segment `sv` -> sQ (general plan: the pair's two tiles; decode plan: the one shared tile)
+  // Q tiles of segment `sv` (the pair's two tiles) -> sQ
   auto issue_q = [&](const SegView& sv) {
-    if constexpr (kAlt) {
-      mbar_arrive_expect_tx(bq_full, kQTileBytes);
+    mbar_arrive_expect_tx(bq_full, 2 * kQTileBytes);
+    const int32_t tok0 = sv.g.q_token0 + pair * tok_per_pair;
+    for (int q = 0; q < 2; ++q)
       for (int h = 0; h < 2; ++h)
-        tma_load_3d(sQ + h * kHalfBytes, &tmap_q, bq_full, h * 64, sv.g.kv_head * p.G, sv.g.q_token0);
-    } else {
-      mbar_arrive_expect_tx(bq_full, 2 * kQTileBytes);
-      const int32_t tok0 = sv.g.q_token0 + pair * tok_per_pair;
-      for (int q = 0; q < 2; ++q)
-        for (int h = 0; h < 2; ++h)
-          tma_load_3d(sQ + q * kQTileBytes + h * kHalfBytes, &tmap_q, bq_full, h * 64,
-                      sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
-    }
+        tma_load_3d(sQ + q * kQTileBytes + h * kHalfBytes, &tmap_q, bq_full, h * 64,
+                    sv.g.kv_head * p.G, tok0 + q * tok_per_tile);
   };
   if (warp == 8 && lane == 0) {
     // the producer owns the Q barriers
@@ -284,11 +269,11 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         const int32_t nt = sv.tile_end - sv.tile_begin;
         // ONE loop, ONE issue site for the K/V tiles of the segment (code size: the hot loops of the four warp
         // roles have to stay inside the 32 KB instruction cache).  Order = consumption order of the MMA warp:
-        // general plan K0 V0 K1 V1 ..., decode plan K0 K1 | V0 K2 | V1 K3 | ... (K runs kAhead tiles ahead of V).
+        // K0 V0 K1 V1 ... (K runs kAhead tiles ahead of V; the decode kernel uses the same loop with 2).
         // The Q tiles go out once: the first segment's right after the wait (until then only tiles of its
         // stable prefix are fetched, at most one ring of them), a later segment's when the MMA warp has
         // released the Q buffers.
-        constexpr int32_t kAhead = kAlt ? 2 : 1;
+        constexpr int32_t kAhead = 1;
         int32_t nk = 0, nv = 0, pg0 = pre_pg0, pg1 = pre_pg1;
         bool have_ids = first && pre_valid, q_pending = true;
         for (;;) {
@@ -304,24 +289,15 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           if (at_end) break;
           // page ids of tile j (pool part): the general plan loads them with the K tile and keeps them for
           // the V tile that follows (and fetches the next tile's one tile ahead when they are published)
-          int32_t c0, c1;
-          if constexpr (kAlt) {
-            const bool pre = have_ids && !is_v && nk == 0;
-            c0 = pre ? pre_pg0 : (j < Tc ? page_row[min(2 * j, last_page)] : 0);
-            c1 = pre ? pre_pg1 : (j < Tc ? page_row[min(2 * j + 1, last_page)] : 0);
-          } else {
-            if (!is_v) {
-              if (!have_ids) {
-                pg0 = j < Tc ? page_row[min(2 * j, last_page)] : 0;
-                pg1 = j < Tc ? page_row[min(2 * j + 1, last_page)] : 0;
-              }
-            }
-            c0 = pg0; c1 = pg1;
-            if (is_v) {
-              // next tile's ids one tile ahead - unless they may not be published yet
-              have_ids = j + 1 < sv.tile_end && j + 1 < Tc && (!q_pending || j + 1 < sv.g.stable_tiles);
-              if (have_ids) { pg0 = page_row[min(2 * j + 2, last_page)]; pg1 = page_row[min(2 * j + 3, last_page)]; }
-            }
+          if (!is_v && !have_ids) {
+            pg0 = j < Tc ? page_row[min(2 * j, last_page)] : 0;
+            pg1 = j < Tc ? page_row[min(2 * j + 1, last_page)] : 0;
+          }
+          const int32_t c0 = pg0, c1 = pg1;
+          if (is_v) {
+            // next tile's ids one tile ahead - unless they may not be published yet
+            have_ids = j + 1 < sv.tile_end && j + 1 < Tc && (!q_pending || j + 1 < sv.g.stable_tiles);
+            if (have_ids) { pg0 = page_row[min(2 * j + 2, last_page)]; pg1 = page_row[min(2 * j + 3, last_page)]; }
           }
           // one 128-key K or V tile -> the next ring slot: 64-key x 64-dim boxes at offsets 0 (keys 0-63,
           // dims 0-63), 8 KB (keys 64-127), 16 KB and 24 KB (dims 64-127)
@@ -361,9 +337,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const uint64_t desc_k = make_smem_desc_sw128(0, 16, 1024);          // K-major operands (Q, K)
       const uint64_t desc_v = make_smem_desc_sw128(0, kHalfBytes, 1024);  // MN-major operand (V)
       uint32_t ring_it = 0, q_it = 0, tile_it = 0, seg_it = 0;
-      uint32_t alt_tiles0 = 0, alt_tiles1 = 0, alt_segs0 = 0, alt_segs1 = 0;   // kAlt: per accumulator set
       auto issue_S = [&](int q, uint32_t slot) {
-        const uint64_t da = desc_k + ((sQ + (kAlt ? 0 : q) * kQTileBytes) >> 4);
+        const uint64_t da = desc_k + ((sQ + q * kQTileBytes) >> 4);
         const uint64_t db = desc_k + ((sRing + slot * kSlotBytes) >> 4);
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {
@@ -387,57 +362,6 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         if (sv.tile_end <= sv.tile_begin) continue;          // clipped away for this pair
         const int32_t nt = sv.tile_end - sv.tile_begin;
         mbar_wait(bq_full, q_it & 1);
-        if constexpr (kAlt) {
-          // S_q <- Q K(tile q) for q = 0, 1; then per tile j (set q = j & 1): O_q += P V(j), S_q <- Q K(j+2)
-          for (int q = 0; q < 2 && q < nt; ++q) {
-            const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
-            mbar_wait(bkv_full(slot), par);
-            tc_fence_after();
-            if (leader) {
-              issue_S(q, slot); mma_commit(bs_full(q)); mma_commit(bkv_empty(slot));
-              if (q + 1 == nt || (q == 1 && nt == 2)) mma_commit(bq_empty);
-            }
-            __syncwarp();
-            ++ring_it;
-          }
-          for (int32_t j = 0; j < nt; ++j) {
-            const int q = j & 1;
-            const uint32_t tq = q ? alt_tiles1 : alt_tiles0, sq = q ? alt_segs1 : alt_segs0;
-            const uint32_t slot_v = ring_it % kStages, par_v = (ring_it / kStages) & 1;
-            ++ring_it;
-            const bool have_next = j + 2 < nt;
-            uint32_t slot_k = 0, par_k = 0;
-            if (have_next) { slot_k = ring_it % kStages; par_k = (ring_it / kStages) & 1; ++ring_it; }
-            mbar_wait(bkv_full(slot_v), par_v);
-            mbar_wait(bp_full(q, 0), tq & 1);
-            if (j < 2) mbar_wait(bo_empty(q), (sq & 1) ^ 1);
-            tc_fence_after();
-            if (leader) { issue_PV(q, slot_v, 0, j >= 2); mma_commit(bpv_h0(q)); }
-            __syncwarp();
-            mbar_wait(bp_full(q, 1), tq & 1);
-            tc_fence_after();
-            if (leader) {
-              issue_PV(q, slot_v, 1, true);
-              if (!have_next) mma_commit(bo_full(q));
-              mma_commit(bkv_empty(slot_v));
-            }
-            __syncwarp();
-            if (have_next) {
-              mbar_wait(bkv_full(slot_k), par_k);
-              tc_fence_after();
-              if (leader) {
-                issue_S(q, slot_k); mma_commit(bs_full(q)); mma_commit(bkv_empty(slot_k));
-                if (j + 3 == nt) mma_commit(bq_empty);
-              }
-              __syncwarp();
-            }
-            if (q) ++alt_tiles1; else ++alt_tiles0;
-          }
-          ++alt_segs0;
-          if (nt > 1) ++alt_segs1;
-          ++q_it;
-          continue;
-        }
         {
           const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
           mbar_wait(bkv_full(slot), par);
@@ -501,7 +425,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const int q = warp >> 2;
     const uint32_t lane_base = (uint32_t)(warp & 3) * 32;
     const int32_t row_in_tile = (int32_t)lane_base + lane;
-    const int32_t R = kAlt ? row_in_tile : q * kTileRows + row_in_tile;   // packed row inside the pair
+    const int32_t R = q * kTileRows + row_in_tile;          // packed row inside the pair
     const uint32_t t_s = tmem_base + (lane_base << 16) + q * 128;
     const uint32_t t_o = tmem_base + (lane_base << 16) + 256 + q * 128;
     const float c = p.scale * 1.4426950408889634f;
@@ -522,9 +446,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       // whose completion lane 0 of each warp has already waited for; the barrier below orders them
       // before the (cumulative) release of the counter update.
       if (fence_all) __threadfence();
-      // one release per CTA and partial: both warpgroups meet (decode plan: warpgroup 0 alone)
-      if constexpr (kAlt) asm volatile("bar.sync 2, 128;" ::: "memory");
-      else asm volatile("bar.sync 3, 256;" ::: "memory");
+      // one release per CTA and partial: both warpgroups meet
+      asm volatile("bar.sync 3, 256;" ::: "memory");
       if (threadIdx.x == 0) red_release_gpu_add(p.merge_ctr + bars->cur_slot0, 2);
     };
     // resolve the merge duty that comes with a partial segment (thread 0, while the first tile loads)
@@ -533,7 +456,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const int32_t part = (sv.part_base - ci.part_base) / sv.g.npairs;
       job.slot0 = ci.part_base + pair; job.nparts = ci.nparts; job.npairs = sv.g.npairs; job.kv_head = sv.g.kv_head;
       job.tok0 = sv.g.q_token0 + pair * tok_per_pair;
-      const int32_t nv = min(kAlt ? kTileRows : kPairRows, (min(sv.g.q_token_end, job.tok0 + tok_per_pair) - job.tok0) * p.G);
+      const int32_t nv = min(kPairRows, (min(sv.g.q_token_end, job.tok0 + tok_per_pair) - job.tok0) * p.G);
       job.r_lo = (int32_t)((int64_t)part * nv / ci.nparts);
       job.r_hi = (int32_t)((int64_t)(part + 1) * nv / ci.nparts);
       job.pad = 0;
@@ -542,9 +465,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     for (int32_t si = seg_lo; si < seg_hi; ++si) {
       SegView sv;
       if (!load_segment(meta, hdr, si, pair, tok_per_pair, sv)) continue;
-      // kAlt: this warpgroup takes tiles tile_begin + q, + q + 2, ...
-      const int32_t nt = kAlt ? (sv.tile_end > sv.tile_begin ? (sv.tile_end - sv.tile_begin + 1 - q) / 2 : 0)
-                              : sv.tile_end - sv.tile_begin;
+      const int32_t nt = sv.tile_end - sv.tile_begin;
       const int32_t part_slot = sv.part_base + pair;
       if (fused && sv.part_base >= 0 && threadIdx.x == 0) {
         MergeJob job;
@@ -560,9 +481,9 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         // every tile of this segment lies beyond what the pair can see: publish an empty partial
         // (the segment is one of several splits, otherwise it would start at tile 0)
         if (!pdl_done) { pdl_wait(); pdl_done = true; }
-        if (row_valid && sv.part_base >= 0 && (!kAlt || q == 0))
+        if (row_valid && sv.part_base >= 0)
           p.part_lse[(int64_t)part_slot * kPairRows + R] = -INFINITY;
-        if (sv.part_base >= 0 && (!kAlt || q == 0)) publish(true);
+        if (sv.part_base >= 0) publish(true);
         continue;
       }
       const int32_t head = sv.g.kv_head * p.G + R % p.G;
@@ -689,7 +610,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       bool all_finite = false;                               // warp-uniform: every row's reference is finite
 
       for (int32_t j = 0; j < nt; ++j) {
-        const int32_t t = sv.tile_begin + (kAlt ? 2 * j + q : j);
+        const int32_t t = sv.tile_begin + j;
         mbar_wait(bs_full(q), tile_it & 1);
         tc_fence_after();
         const bool need_mask = t >= (t < Tc ? mask_a : mask_b);
@@ -829,40 +750,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       }
       float inv_l = l > 0.f ? 1.f / l : 0.f;                // coefficient of this set's accumulator
       float lse2 = l > 0.f ? m_used + log2f(l) : -INFINITY;
-      float inv_l1 = 0.f;                                   // kAlt: coefficient of accumulator set 1
-      bool use1 = false;
-      if constexpr (kAlt) {
-        // The two accumulator sets hold attention over the even / odd KV tiles of the segment for the
-        // SAME rows: merge them here (LSE-weighted, exactly what the combine kernel does across
-        // segments) so the segment yields one result.  Set 1 hands (lse2, 1/l) to warpgroup 0 through
-        // shared memory (Barriers::lse_stage, upper part; a second barrier keeps set 1 from overwriting it early);
-        // warpgroup 0 reads O_1 straight from TMEM (same lanes) and releases it on set 1's behalf.
-        float2* xchg = reinterpret_cast<float2*>(&bars->lse_stage[kTileRows]);
-        if (q == 1) {
-          xchg[row_in_tile] = make_float2(lse2, inv_l);
-          tc_fence_before();
-          asm volatile("bar.sync 1, 256;" ::: "memory");
-          asm volatile("bar.sync 1, 256;" ::: "memory");    // warpgroup 0 has read the exchange area
-          if (nt > 0) ++seg_it;
-          continue;
-        }
-        asm volatile("bar.sync 1, 256;" ::: "memory");
-        tc_fence_after();                                   // set 1's PV completion was observed by warpgroup 1
-        const float2 peer = xchg[row_in_tile];
-        asm volatile("bar.sync 1, 256;" ::: "memory");
-        use1 = sv.tile_end - sv.tile_begin >= 2;            // set 1 processed at least one tile
-        const float mx = fmaxf(lse2, peer.x);
-        if (mx == -INFINITY) {
-          inv_l = 0.f;
-        } else {
-          const float w0 = ex2_approx(lse2 - mx), w1 = use1 ? ex2_approx(peer.x - mx) : 0.f;
-          const float inv_w = 1.f / (w0 + w1);
-          inv_l = w0 * inv_w * inv_l;
-          inv_l1 = w1 * inv_w * peer.y;
-          lse2 = mx + log2f(w0 + w1);
-        }
-      }
-      const float osc = kAlt ? 1.f : inv_l;                 // kAlt: already applied by the merge above
+      const float osc = inv_l;
       bool pub = false, pub_fence = false;
       if (sv.part_base < 0) {
         __nv_bfloat16* orow = reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)tok * p.Hq + head) * p.D;
@@ -871,19 +759,6 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           uint32_t o[32];
           tmem_ld32(t_o + ch * 32, o);
           tmem_wait_ld();
-          if constexpr (kAlt) {
-            if (use1) {
-              uint32_t o1[32];
-              tmem_ld32(t_o + 128 + ch * 32, o1);
-              tmem_wait_ld();
-#pragma unroll
-              for (int i = 0; i < 32; ++i)
-                o[i] = __float_as_uint(fmaf(__uint_as_float(o1[i]), inv_l1, __uint_as_float(o[i]) * inv_l));
-            } else {
-#pragma unroll
-              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * inv_l);
-            }
-          }
           if (row_valid) {
 #pragma unroll
             for (int i = 0; i < 32; i += 8) {
@@ -905,28 +780,14 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         // warp stages its 32 rows x 512 B there and writes them with ONE 16 KB bulk store; rows are
         // contiguous in the partial buffer.  Otherwise: direct 16-byte stores (same chunk positions).
         const bool staged = si + 1 == seg_hi && __all_sync(0xffffffffu, row_valid);   // (few valid rows, e.g. decode steps: store just those)
-        const uint32_t stage = ((kAlt || q == 1) ? sRing : sQ) + (uint32_t)(warp & 3) * 16384u + (uint32_t)lane * 512u;
+        const uint32_t stage = (q == 1 ? sRing : sQ) + (uint32_t)(warp & 3) * 16384u + (uint32_t)lane * 512u;
 #pragma unroll
         for (int ch = 0; ch < 4; ++ch) {
           uint32_t o[32];
           tmem_ld32(t_o + ch * 32, o);
           tmem_wait_ld();
-          if constexpr (kAlt) {
-            if (use1) {
-              uint32_t o1[32];
-              tmem_ld32(t_o + 128 + ch * 32, o1);
-              tmem_wait_ld();
 #pragma unroll
-              for (int i = 0; i < 32; ++i)
-                o[i] = __float_as_uint(fmaf(__uint_as_float(o1[i]), inv_l1, __uint_as_float(o[i]) * inv_l));
-            } else {
-#pragma unroll
-              for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * inv_l);
-            }
-          } else {
-#pragma unroll
-            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * osc);
-          }
+          for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * osc);
           if (staged) {
 #pragma unroll
             for (int i = 0; i < 32; i += 4)
@@ -954,7 +815,6 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       }
       tc_fence_before();
       mbar_arrive(bo_empty(q));
-      if constexpr (kAlt) { if (use1) mbar_arrive(bo_empty(1)); }
       if (pub) publish(pub_fence);
       ++seg_it;
     }
@@ -1020,10 +880,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 }
 
 cudaError_t sm100_attn_configure() {
-  const void* fns[4] = {(const void*)attn_sm100_kernel<kInlineAttnWords, false>,
-                        (const void*)attn_sm100_kernel<kInlineAttnWordsLarge, false>,
-                        (const void*)attn_sm100_kernel<kInlineAttnWords, true>,
-                        (const void*)attn_sm100_kernel<kInlineAttnWordsLarge, true>};
+  const void* fns[2] = {(const void*)attn_sm100_kernel<kInlineAttnWords>,
+                        (const void*)attn_sm100_kernel<kInlineAttnWordsLarge>};
   for (const void* f : fns) {
     cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
     if (e != cudaSuccess) return e;
@@ -1050,16 +908,10 @@ cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream) {
   if (l.inl_words <= kInlineAttnWords) {
     InlineAttnMeta small;
     memcpy(small.w, l.inl.w, sizeof(small.w));
-    if (l.alt)
-      return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<kInlineAttnWords, true>, l.tmap_q, l.tmap_k, l.tmap_v,
-                                l.tmap_kn, l.tmap_vn, small, l.app, l.peers, l.p);
-    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<kInlineAttnWords, false>, l.tmap_q, l.tmap_k, l.tmap_v,
+    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<kInlineAttnWords>, l.tmap_q, l.tmap_k, l.tmap_v,
                               l.tmap_kn, l.tmap_vn, small, l.app, l.peers, l.p);
   }
-  if (l.alt)
-    return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<kInlineAttnWordsLarge, true>, l.tmap_q, l.tmap_k, l.tmap_v,
-                              l.tmap_kn, l.tmap_vn, l.inl, l.app, l.peers, l.p);
-  return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<kInlineAttnWordsLarge, false>, l.tmap_q, l.tmap_k, l.tmap_v,
+  return cudaLaunchKernelEx(&cfg, attn_sm100_kernel<kInlineAttnWordsLarge>, l.tmap_q, l.tmap_k, l.tmap_v,
                             l.tmap_kn, l.tmap_vn, l.inl, l.app, l.peers, l.p);
 }
 

@@ -83,7 +83,7 @@ struct Sm100Launch {
   PeerPools peers;
   int32_t inl_words;                 // words of `inl` in use (selects the small / large parameter tier)
   int32_t num_ctas;
-  bool alt;                          // decode plan (plan.h): same Q tile, alternate KV tiles
+  bool alt;                          // decode plan (plan.h): runs on attn_dec_sm100_kernel
 };
 cudaError_t sm100_attn_configure();    // one-time cudaFuncSetAttribute
 cudaError_t launch_attn_sm100(const Sm100Launch& l, cudaStream_t stream);
