@@ -8,9 +8,11 @@
 // :47 Eq. (1): row r of block b sees keys j < e_b.
 //
 // One warp per (query token, q head).  Lane = key for the scores (online softmax, max/sum reduced
-// with warp shuffles), lane = output-dim slice for P.V, eight V rows in flight per lane (the loop is
-// bound by load latency, not by arithmetic: walking the keys one dependent load at a time cost 19 us for
-// the 48 keys of the fp32 config).
+// with warp shuffles), lane = output-dim slice for P.V.  The loop is bound by load latency, not by
+// arithmetic (walking the keys one dependent load at a time cost 19 us for the 48 keys of the fp32 config):
+// a chunk's K rows are read with every 16-byte load of a row in flight at once, and the V rows of its first
+// 64 / kDV keys (kDV = 32-wide slices of D) are requested BEFORE the scores - their addresses need only the
+// page ids - so they arrive under the K round and the softmax.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <math.h>
@@ -49,7 +51,7 @@ __device__ __forceinline__ void store_out(__nv_bfloat16* p, float x) { *p = __fl
 constexpr int kSimtWarps = 4;
 constexpr int kMaxD = 256;
 
-template <typename T>
+template <typename T, int kDV>
 __global__ void __launch_bounds__(kSimtWarps * 32)
 attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict__ lse,
                  const T* __restrict__ k_pool, const T* __restrict__ v_pool,
@@ -111,10 +113,32 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
   __syncwarp();
 
   constexpr int VN = Vec16<T>::N;
-  float acc[kMaxD / 32];
+  constexpr int kBatch = 64 / kDV;                      // V rows in flight per lane
+  float acc[kDV];
 #pragma unroll
-  for (int i = 0; i < kMaxD / 32; ++i) acc[i] = 0.f;
+  for (int i = 0; i < kDV; ++i) acc[i] = 0.f;
   float m = -INFINITY, l = 0.f;
+  // V values of keys kk0 .. kk0 + kBatch - 1 of the current chunk for this lane's output dims
+  auto load_v = [&](int32_t rowidx, int kk0, int nk, float (&vv)[kBatch][kDV]) {
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const int32_t ri = __shfl_sync(0xffffffffu, rowidx, (kk0 + u) & 31);
+      const T* vp = ri >= 0 ? v_pool + (int64_t)ri * D : v_new + (int64_t)(-1 - ri) * D;
+#pragma unroll
+      for (int i = 0; i < kDV; ++i) {
+        const int d = lane + 32 * i;
+        vv[u][i] = (kk0 + u < nk && d < D) ? to_f32(vp[d]) : 0.f;
+      }
+    }
+  };
+  auto fma_v = [&](float p, int kk0, int nk, const float (&vv)[kBatch][kDV]) {
+#pragma unroll
+    for (int u = 0; u < kBatch; ++u) {
+      const float pu = __shfl_sync(0xffffffffu, p, (kk0 + u) & 31);   // (keys >= nk: vv = 0)
+#pragma unroll
+      for (int i = 0; i < kDV; ++i) acc[i] = fmaf(pu, vv[u][i], acc[i]);
+    }
+  };
 
   for (int32_t base = 0; base < vis; base += 32) {
     const int32_t j = base + lane;
@@ -125,12 +149,16 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
     }
     float s = -INFINITY;
     int32_t rowidx = 0;
-    if (valid) {
-      // rowidx >= 0: row of the pool; < 0: row -(rowidx + 1) of k_new / v_new
+    // rowidx >= 0: row of the pool; < 0: row -(rowidx + 1) of k_new / v_new (hidden keys: pool row 0, p = 0)
+    if (valid)
       rowidx = j < cache_len ? (page_row[j / P] * Hkv + g) * P + (j % P) : -1 - ((new_row0 + j - cache_len) * Hkv + g);
+    const int nk = min(32, vis - base);
+    float vv[kBatch][kDV];
+    load_v(rowidx, 0, nk, vv);
+    if (valid) {
       const T* kp = rowidx >= 0 ? k_pool + (int64_t)rowidx * D : k_new + (int64_t)(-1 - rowidx) * D;
       float a = 0.f;
-#pragma unroll 4
+#pragma unroll 16
       for (int d = 0; d < D; d += VN) {
         float kv[VN];
         Vec16<T>::load(kp + d, kv);
@@ -152,37 +180,19 @@ attn_simt_kernel(const T* __restrict__ q, T* __restrict__ out, float* __restrict
     for (int o = 16; o > 0; o >>= 1) psum += __shfl_xor_sync(0xffffffffu, psum, o);
     l = l * corr + psum;
 #pragma unroll
-    for (int i = 0; i < kMaxD / 32; ++i) acc[i] *= corr;
-    const int nk = min(32, vis - base);
-    constexpr int kBatch = 16;                          // V rows in flight per lane (the loop is bound by load latency)
-    for (int kk0 = 0; kk0 < nk; kk0 += kBatch) {
-      float pk[kBatch];
-      const T* vp[kBatch];
-#pragma unroll
-      for (int u = 0; u < kBatch; ++u) {
-        const int kk = (kk0 + u) & 31;
-        pk[u] = kk0 + u < nk ? __shfl_sync(0xffffffffu, p, kk) : 0.f;
-        const int32_t ri = __shfl_sync(0xffffffffu, rowidx, kk);
-        vp[u] = ri >= 0 ? v_pool + (int64_t)ri * D : v_new + (int64_t)(-1 - ri) * D;
-      }
-#pragma unroll
-      for (int i = 0; i < kMaxD / 32; ++i) {
-        const int d = lane + 32 * i;
-        if (d < D) {
-          float vv[kBatch];
-#pragma unroll
-          for (int u = 0; u < kBatch; ++u) vv[u] = kk0 + u < nk ? to_f32(vp[u][d]) : 0.f;
-#pragma unroll
-          for (int u = 0; u < kBatch; ++u) acc[i] = fmaf(pk[u], vv[u], acc[i]);
-        }
-      }
+    for (int i = 0; i < kDV; ++i) acc[i] *= corr;
+    fma_v(p, 0, nk, vv);
+#pragma unroll 1
+    for (int kk0 = kBatch; kk0 < nk; kk0 += kBatch) {
+      load_v(rowidx, kk0, nk, vv);
+      fma_v(p, kk0, nk, vv);
     }
     m = m_new;
   }
   const float inv = 1.f / l;
   T* orow = out + ((int64_t)tok * Hq + h) * D;
 #pragma unroll
-  for (int i = 0; i < kMaxD / 32; ++i) {
+  for (int i = 0; i < kDV; ++i) {
     int d = lane + 32 * i;
     if (d < D) store_out(orow + d, acc[i] * inv);
   }
@@ -211,16 +221,22 @@ cudaError_t launch_attn_simt(int32_t dtype, const void* q, void* out, float* lse
   } else {
     app_none.w[0] = 0;
   }
-  if (dtype == 1)
-    return launch_pdl(attn_simt_kernel<float>, dim3(grid), dim3(kSimtWarps * 32), 0, stream,
-                      (const float*)q, (float*)out, lse, (const float*)k_pool, (const float*)v_pool, page_table,
-                      tok_meta, inl, q_to_kv, total_q_tokens, max_pages, Hq, Hkv, D, P, scale, text_causal,
-                      (const float*)k_new, (const float*)v_new, (float*)kw, (float*)vw, ptw, *app, attn_blocks);
-  return launch_pdl(attn_simt_kernel<__nv_bfloat16>, dim3(grid), dim3(kSimtWarps * 32), 0, stream,
-                    (const __nv_bfloat16*)q, (__nv_bfloat16*)out, lse, (const __nv_bfloat16*)k_pool,
-                    (const __nv_bfloat16*)v_pool, page_table, tok_meta, inl, q_to_kv, total_q_tokens, max_pages,
-                    Hq, Hkv, D, P, scale, text_causal, (const __nv_bfloat16*)k_new, (const __nv_bfloat16*)v_new,
-                    (__nv_bfloat16*)kw, (__nv_bfloat16*)vw, ptw, *app, attn_blocks);
+  auto go = [&](auto kern_f32, auto kern_bf16) {
+    if (dtype == 1)
+      return launch_pdl(kern_f32, dim3(grid), dim3(kSimtWarps * 32), 0, stream,
+                        (const float*)q, (float*)out, lse, (const float*)k_pool, (const float*)v_pool, page_table,
+                        tok_meta, inl, q_to_kv, total_q_tokens, max_pages, Hq, Hkv, D, P, scale, text_causal,
+                        (const float*)k_new, (const float*)v_new, (float*)kw, (float*)vw, ptw, *app, attn_blocks);
+    return launch_pdl(kern_bf16, dim3(grid), dim3(kSimtWarps * 32), 0, stream,
+                      (const __nv_bfloat16*)q, (__nv_bfloat16*)out, lse, (const __nv_bfloat16*)k_pool,
+                      (const __nv_bfloat16*)v_pool, page_table, tok_meta, inl, q_to_kv, total_q_tokens, max_pages,
+                      Hq, Hkv, D, P, scale, text_causal, (const __nv_bfloat16*)k_new, (const __nv_bfloat16*)v_new,
+                      (__nv_bfloat16*)kw, (__nv_bfloat16*)vw, ptw, *app, attn_blocks);
+  };
+  // kDV = 32-wide slices of D held per lane
+  if (D <= 64) return go(attn_simt_kernel<float, 2>, attn_simt_kernel<__nv_bfloat16, 2>);
+  if (D <= 128) return go(attn_simt_kernel<float, 4>, attn_simt_kernel<__nv_bfloat16, 4>);
+  return go(attn_simt_kernel<float, 8>, attn_simt_kernel<__nv_bfloat16, 8>);
 }
 
 }  // namespace ws
