@@ -31,12 +31,10 @@ struct PlanConfig {
 };
 
 // Decode plan ("alt", NEXT-4: n*G <= 128 packed rows per (session, KV head), e.g. token-causal text
-// decode).  Such a step is cache-read bound (n*G FLOP/B << ridge), so the CTA's two
-// S/O accumulator sets are not given two Q tiles but the SAME Q tile and ALTERNATE KV tiles: set 0
-// takes the even tiles of the segment, set 1 the odd ones, each with its own running max / sum.  The
-// tensor pipe and the two softmax warpgroups then consume K/V twice as fast per CTA (HBM-bound instead
-// of bound by the S -> softmax -> PV chain).  The two sets are merged inside the CTA at the end of the
-// segment (LSE-weighted), so a segment still yields one result and the plan is otherwise unchanged.
+// decode).  Such a step is cache-read bound (n*G FLOP/B << ridge): one 128-row Q tile per
+// CTA, run by attn_dec_sm100_kernel (both softmax warpgroups on every KV tile, one O accumulator, six ring
+// slots).  Groups, segments, partial slots and the combine are those of the general plan; a partial has
+// 128 rows in use.
 struct Plan {
   bool alt = false;
   int32_t team_size = 1, num_teams = 0, total_tiles = 0, num_part_slots = 0;

@@ -341,3 +341,27 @@ def test_text_causal_ragged_multi_session_batch(n):
         refs = [attend(sess[s], qs[s], scale, 1, want_abs=True, text_causal=True) for s in range(3)]
         o_ref, l_ref, a_ref = (np.concatenate([r[i] for r in refs]) for i in range(3))
         _gate_bf16(o, l, o_ref, l_ref, a_ref, f"ragged 3-session batch n={n} step {step}")
+
+
+def _tc_fuzz_cases():
+    rng = np.random.default_rng([2606, 25041, 4])
+    out = []
+    for i in range(16):
+        Hkv = int(rng.choice([1, 2, 4]))
+        G = int(rng.choice([1, 2, 4, 8]))
+        hist = [int(x) for x in rng.integers(1, 400, size=int(rng.integers(0, 4)))]
+        qb = [int(x) for x in rng.choice([1, 2, 7, 16, 33, 64, 100, 130, 257], size=int(rng.integers(1, 4)))]
+        out.append(dict(idx=i, Hq=Hkv * G, Hkv=Hkv, hist=hist, qb=qb, mode=["two_calls", "fused", "one_shot"][i % 3],
+                        splits=int(rng.choice([0, 0, 2, 4])), p_text=float(rng.choice([0.1, 0.3, 0.6, 1.0]))))
+    return out
+
+
+@pytest.mark.parametrize("case", _tc_fuzz_cases(), ids=lambda c: f"{c['idx']}_{c['mode']}_h{c['Hkv']}x{c['Hq'] // c['Hkv']}")
+def test_text_causal_random_shapes(case):
+    """Seeded random shapes of the mixed mask (block sizes from one token to more than a Q tile pair, histories that
+    end mid-page and mid-tile, text share 10 % - 100 %, forced splits, the three call modes) against the oracle."""
+    o, l, o_ref, l_ref, a_ref, plans = _text_causal_case("bf16", case["Hq"], case["Hkv"], 128, 64, case["hist"], case["qb"],
+                                                         seed=1000 + case["idx"], mode=case["mode"],
+                                                         min_splits=case["splits"], p_text=case["p_text"])
+    assert all(p["used_tensor_core_kernel"] in (1, 3) for p in plans), plans
+    _gate_bf16(o, l, o_ref, l_ref, a_ref, f"fuzz {case}")
