@@ -80,7 +80,7 @@ constexpr int kMaxJobs = 4;
 struct Barriers {
   uint64_t q_full, q_empty;
   uint64_t kv_full[kStages], kv_empty[kStages];
-  uint64_t s_full[2], s_free[2], p_full[2][2], pv_h0_done[2], pv_done[2], o_full[2], o_empty[2];
+  uint64_t s_full[2], p_full[2][2], pv_h0_done[2], o_full[2], o_empty[2];
   uint64_t merge_full;
   alignas(16) float lse_stage[kPairRows];                  // staged epilogue: the pair's log2-LSEs on their way to part_lse
   MergeJob jobs[kMaxJobs];
@@ -178,9 +178,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
   auto bkv_empty = [&](int s) { return smem_u32(&bars->kv_empty[s]); };
   auto bs_full = [&](int q) { return smem_u32(&bars->s_full[q]); };
   auto bp_full = [&](int q, int half) { return smem_u32(&bars->p_full[q][half]); };
-  auto bs_free = [&](int q) { return smem_u32(&bars->s_free[q]); };
   auto bpv_h0 = [&](int q) { return smem_u32(&bars->pv_h0_done[q]); };
-  auto bpv_done = [&](int q) { return smem_u32(&bars->pv_done[q]); };
   auto bo_full = [&](int q) { return smem_u32(&bars->o_full[q]); };
   auto bo_empty = [&](int q) { return smem_u32(&bars->o_empty[q]); };
 
@@ -232,7 +230,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     for (int s = 0; s < kStages; ++s) { mbar_init(bkv_full(s), 1); mbar_init(bkv_empty(s), 1); }
     for (int q = 0; q < 2; ++q) {
       mbar_init(bs_full(q), 1); mbar_init(bp_full(q, 0), 128); mbar_init(bp_full(q, 1), 128);
-      mbar_init(bpv_h0(q), 1); mbar_init(bpv_done(q), 1); mbar_init(bs_free(q), 128);
+      mbar_init(bpv_h0(q), 1);
       mbar_init(bo_full(q), 1); mbar_init(bo_empty(q), 128);
     }
     fence_mbar_init();
@@ -271,13 +269,12 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         const int32_t nt = sv.tile_end - sv.tile_begin;
         // ONE loop, ONE issue site for the K/V tiles of the segment (code size: the hot loops of the four warp
         // roles have to stay inside the 32 KB instruction cache).  Order = consumption order of the MMA warp:
-        // K0 K1 V0 K2 V1 ... (K runs kAhead = 2 tiles ahead of V: S of tile j + 1 is issued before PV of tile j).
+        // K0 V0 K1 V1 ... (K runs kAhead tiles ahead of V; the decode kernel uses the same loop with 2).
         // The Q tiles go out once: the first segment's right after the wait (until then only tiles of its
         // stable prefix are fetched, at most one ring of them), a later segment's when the MMA warp has
         // released the Q buffers.
-        constexpr int32_t kAhead = 2;
+        constexpr int32_t kAhead = 1;
         int32_t nk = 0, nv = 0, pg0 = pre_pg0, pg1 = pre_pg1;
-        int32_t ha0 = 0, ha1 = 0, hb0 = 0, hb1 = 0;          // page ids of the last two K tiles (for their V tiles)
         bool have_ids = first && pre_valid, q_pending = true;
         for (;;) {
           const bool is_v = !(nk < nt && nk < nv + kAhead);
@@ -290,21 +287,17 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             q_pending = false;
           }
           if (at_end) break;
-          // page ids of tile j (pool part): read (or prefetched one tile ahead) for the K tile and kept for the
-          // V tile of the same keys, which follows one K tile later
-          int32_t c0, c1;
-          if (!is_v) {
-            if (!have_ids) {
-              pg0 = j < Tc ? page_row[min(2 * j, last_page)] : 0;
-              pg1 = j < Tc ? page_row[min(2 * j + 1, last_page)] : 0;
-            }
-            c0 = pg0; c1 = pg1;
-            if (nk & 1) { hb0 = c0; hb1 = c1; } else { ha0 = c0; ha1 = c1; }
-            // the next K tile's ids one tile ahead - unless they may not be published yet
+          // page ids of tile j (pool part): the general plan loads them with the K tile and keeps them for
+          // the V tile that follows (and fetches the next tile's one tile ahead when they are published)
+          if (!is_v && !have_ids) {
+            pg0 = j < Tc ? page_row[min(2 * j, last_page)] : 0;
+            pg1 = j < Tc ? page_row[min(2 * j + 1, last_page)] : 0;
+          }
+          const int32_t c0 = pg0, c1 = pg1;
+          if (is_v) {
+            // next tile's ids one tile ahead - unless they may not be published yet
             have_ids = j + 1 < sv.tile_end && j + 1 < Tc && (!q_pending || j + 1 < sv.g.stable_tiles);
             if (have_ids) { pg0 = page_row[min(2 * j + 2, last_page)]; pg1 = page_row[min(2 * j + 3, last_page)]; }
-          } else {
-            c0 = (nv & 1) ? hb0 : ha0; c1 = (nv & 1) ? hb1 : ha1;
           }
           // one 128-key K or V tile -> the next ring slot: 64-key x 64-dim boxes at offsets 0 (keys 0-63,
           // dims 0-63), 8 KB (keys 64-127), 16 KB and 24 KB (dims 64-127)
@@ -343,33 +336,23 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       constexpr uint32_t idesc_pv = make_idesc_bf16(128, 128, 0, 1);
       const uint64_t desc_k = make_smem_desc_sw128(0, 16, 1024);          // K-major operands (Q, K)
       const uint64_t desc_v = make_smem_desc_sw128(0, kHalfBytes, 1024);  // MN-major operand (V)
-      uint32_t ring_it = 0, q_it = 0, tile_it = 0, seg_it = 0, s_it = 0;
-      // S = Q_q K^T into the ONE S buffer (TMEM columns 0-127).  The buffer is free again as soon as the softmax
-      // warpgroup of the previous S has copied its rows into registers (s_free), so the S of a Q tile's next KV
-      // tile is computed while that Q tile's softmax is still running: S(q, j + 1) does not wait for PV(q, j).
+      uint32_t ring_it = 0, q_it = 0, tile_it = 0, seg_it = 0;
       auto issue_S = [&](int q, uint32_t slot) {
-        if (s_it > 0) { mbar_wait(bs_free(q ^ 1), ((s_it - 1) >> 1) & 1); tc_fence_after(); }
-        if (leader) {
-          const uint64_t da = desc_k + ((sQ + q * kQTileBytes) >> 4);
-          const uint64_t db = desc_k + ((sRing + slot * kSlotBytes) >> 4);
+        const uint64_t da = desc_k + ((sQ + q * kQTileBytes) >> 4);
+        const uint64_t db = desc_k + ((sRing + slot * kSlotBytes) >> 4);
 #pragma unroll
-          for (int ks = 0; ks < 8; ++ks) {
-            const uint32_t off = ((ks >> 2) * kHalfBytes + (ks & 3) * 32) >> 4;
-            mma_ss(tmem_base, da + off, db + off, idesc_qk, ks > 0);
-          }
-          mma_commit(bs_full(q));
+        for (int ks = 0; ks < 8; ++ks) {
+          const uint32_t off = ((ks >> 2) * kHalfBytes + (ks & 3) * 32) >> 4;
+          mma_ss(tmem_base + q * 128, da + off, db + off, idesc_qk, ks > 0);
         }
-        __syncwarp();
-        ++s_it;
       };
-      // PV for one of the two pieces in which the softmax hands P over (k-steps of 16 keys); P_q: columns
-      // 128 + 64 q .. + 63 (bf16 pairs), O_q: columns 256 + 128 q
+      // PV for one of the two pieces in which the softmax hands P over (k-steps of 16 keys)
       auto issue_PV = [&](int q, uint32_t slot, int half, bool accumulate) {
         const uint64_t db = desc_v + ((sRing + slot * kSlotBytes) >> 4);
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {
           if ((ks < kFirstPieceSteps) != (half == 0)) continue;   // piece 0: keys 0-95, piece 1: keys 96-127
-          mma_ts(tmem_base + 256 + q * 128, tmem_base + 128 + q * 64 + ks * 8, db + ks * (2048 >> 4),
+          mma_ts(tmem_base + 256 + q * 128, tmem_base + q * 128 + ks * 8, db + ks * (2048 >> 4),
                  idesc_pv, (accumulate || ks > 0) ? 1u : 0u);
         }
       };
@@ -383,28 +366,22 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           const uint32_t slot = ring_it % kStages, par = (ring_it / kStages) & 1;
           mbar_wait(bkv_full(slot), par);
           tc_fence_after();
-          issue_S(0, slot);
-          issue_S(1, slot);
           if (leader) {
+            for (int q = 0; q < 2; ++q) { issue_S(q, slot); mma_commit(bs_full(q)); }
             mma_commit(bkv_empty(slot));
             if (nt == 1) mma_commit(bq_empty);
           }
           __syncwarp();
           ++ring_it;
         }
-        // ring order (producer): K0 K1 V0 K2 V1 ... ; issue order: S(0,j+1) PV(0,j) S(1,j+1) PV(1,j)
         for (int32_t j = 0; j < nt; ++j) {
+          const uint32_t slot_v = ring_it % kStages, par_v = (ring_it / kStages) & 1;
+          ++ring_it;
           const bool have_next = j + 1 < nt;
           uint32_t slot_k = 0, par_k = 0;
           if (have_next) { slot_k = ring_it % kStages; par_k = (ring_it / kStages) & 1; ++ring_it; }
-          const uint32_t slot_v = ring_it % kStages, par_v = (ring_it / kStages) & 1;
-          ++ring_it;
+          mbar_wait(bkv_full(slot_v), par_v);
           for (int q = 0; q < 2; ++q) {
-            if (have_next) {
-              if (q == 0) { mbar_wait(bkv_full(slot_k), par_k); tc_fence_after(); }
-              issue_S(q, slot_k);
-            }
-            if (q == 0) mbar_wait(bkv_full(slot_v), par_v);
             mbar_wait(bp_full(q, 0), tile_it & 1);
             if (j == 0) mbar_wait(bo_empty(q), (seg_it & 1) ^ 1);
             tc_fence_after();
@@ -417,10 +394,17 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
             tc_fence_after();
             if (leader) {
               issue_PV(q, slot_v, 1, true);
-              mma_commit(bpv_done(q));
               if (!have_next) mma_commit(bo_full(q));
             }
             __syncwarp();
+            if (have_next) {
+              if (q == 0) { mbar_wait(bkv_full(slot_k), par_k); tc_fence_after(); }
+              if (leader) {
+                issue_S(q, slot_k);
+                mma_commit(bs_full(q));
+              }
+              __syncwarp();
+            }
           }
           if (leader) {
             mma_commit(bkv_empty(slot_v));
@@ -442,8 +426,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t lane_base = (uint32_t)(warp & 3) * 32;
     const int32_t row_in_tile = (int32_t)lane_base + lane;
     const int32_t R = q * kTileRows + row_in_tile;          // packed row inside the pair
-    const uint32_t t_s = tmem_base + (lane_base << 16);                 // the one S buffer (both Q tiles in turn)
-    const uint32_t t_p = tmem_base + (lane_base << 16) + 128 + q * 64;  // P of this Q tile (bf16 pairs)
+    const uint32_t t_s = tmem_base + (lane_base << 16) + q * 128;
     const uint32_t t_o = tmem_base + (lane_base << 16) + 256 + q * 128;
     const float c = p.scale * 1.4426950408889634f;
     uint32_t tile_it = 0, seg_it = 0;
@@ -525,8 +508,9 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         }
       }
 
-      // O and l of this row scaled by alpha (after a change of reference).  O must be quiescent: the caller has
-      // waited for the PV MMAs of the previous tile (wait_prev_pv); those of this tile need our P.
+      // O and l of this row scaled by alpha (after a change of reference).  Safe whenever the PV MMAs of
+      // the previous tile have completed: s_full of the current tile was committed after them on the same
+      // in-order tensor pipe.
       auto rescale_o = [&](float alpha) {
 #pragma unroll 1                                            // rare path, inlined at three sites: keep it small
         for (int ch = 0; ch < 4; ++ch) {
@@ -538,35 +522,40 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           tmem_st32(t_o + ch * 32, o);
         }
       };
-      // PV of this Q tile's previous KV tile has completed: P may be overwritten, O may be rescaled.  (S of the
-      // current tile was issued BEFORE that PV, so s_full alone does not imply it.)
-      auto wait_prev_pv = [&]() {
-        if (tile_it > 0) { mbar_wait(bpv_done(q), (tile_it - 1) & 1); tc_fence_after(); }
-      };
-      // One unmasked tile (its S row in registers, `sr`) exponentiated against the reference m_used; P is handed
-      // to the MMA warp in two pieces (keys 0-95, then 96-127) as soon as each is written.
+      // One unmasked tile exponentiated against the reference m_used while it streams out of TMEM in
+      // 32-column chunks; P is handed to the MMA warp in two pieces (keys 0-95, then 96-127) as soon as
+      // each is written: PV of the first piece (384 tensor cycles) overlaps the softmax of the last 32
+      // keys, and only 128 cycles of PV remain on the S -> softmax -> PV -> S chain.
       // kCheck: the optimistic use - the reference may be stale, so each piece's row sum is tested against
       // sum_lim (kFastSumLimit / kFastSumShare; a NaN/inf sum fails the test).  Returns false, with nothing
-      // handed off, if the first piece fails.
-      auto stream_tile = [&](const uint32_t* sr, const bool kCheck, float sum_lim) -> bool {
+      // handed off and S intact, if the first piece fails.
+      auto stream_tile = [&](const bool kCheck, float sum_lim) -> bool {
         const float neg_mc = -m_used;
         uint32_t pk[64];                                    // P row, packed bf16x2
         uint64_t l01 = 0, l23 = 0;                          // packed fp32x2 partial row sums
-        softmax_chunk(sr + 0, c, neg_mc, l01, l23, pk + 0);
-        softmax_chunk(sr + 32, c, neg_mc, l01, l23, pk + 16);
-        softmax_chunk(sr + 64, c, neg_mc, l01, l23, pk + 32);
+        uint32_t sa[32], sb[32];
+        tmem_ld32(t_s + 0, sa);
+        tmem_wait_ld();
+        tmem_ld32(t_s + 32, sb);
+        softmax_chunk(sa, c, neg_mc, l01, l23, pk + 0);
+        tmem_wait_ld();
+        tmem_ld32(t_s + 64, sa);
+        softmax_chunk(sb, c, neg_mc, l01, l23, pk + 16);
+        tmem_wait_ld();
+        tmem_ld32(t_s + 96, sb);
+        softmax_chunk(sa, c, neg_mc, l01, l23, pk + 32);
         float la, lb;
         unpack_f32x2(add_f32x2(l01, l23), la, lb);
         const float sum_a = la + lb;
         if (kCheck && __any_sync(0xffffffffu, !(sum_a < sum_lim))) return false;
-        wait_prev_pv();
-        tmem_st32(t_p + 0, pk);
-        tmem_st16(t_p + 32, pk + 32);
+        tmem_st32(t_s + 0, pk);
+        tmem_st16(t_s + 32, pk + 32);
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(bp_full(q, 0));                         // first 96 keys of P handed off
+        tmem_wait_ld();
         l01 = 0; l23 = 0;
-        softmax_chunk(sr + 96, c, neg_mc, l01, l23, pk + 48);
+        softmax_chunk(sb, c, neg_mc, l01, l23, pk + 48);
         unpack_f32x2(add_f32x2(l01, l23), la, lb);
         const float sum_b = la + lb;
         l += sum_a;
@@ -579,9 +568,12 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           // keys exactly.
           mbar_wait(bpv_h0(q), tile_it & 1);
           tc_fence_after();
-          float mx = __uint_as_float(sr[96]);
+          uint32_t sr[32];
+          tmem_ld32(t_s + 96, sr);
+          tmem_wait_ld();
+          float mx = __uint_as_float(sr[0]);
 #pragma unroll
-          for (int i = 1; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sr[96 + i]));
+          for (int i = 1; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sr[i]));
           const float tm = mx * c;
           float alpha = 1.f;
           if (tm > m_used) { alpha = ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
@@ -589,14 +581,14 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           float ls = 0.f;
 #pragma unroll
           for (int i = 0; i < 32; i += 2) {
-            const float p0 = ex2_approx(fmaf(__uint_as_float(sr[96 + i]), c, -m_used));
-            const float p1 = ex2_approx(fmaf(__uint_as_float(sr[96 + i + 1]), c, -m_used));
+            const float p0 = ex2_approx(fmaf(__uint_as_float(sr[i]), c, -m_used));
+            const float p1 = ex2_approx(fmaf(__uint_as_float(sr[i + 1]), c, -m_used));
             ls += p0 + p1;
             pk[48 + i / 2] = pack_bf16x2(p0, p1);
           }
           l += ls;
         }
-        tmem_st16(t_p + 48, pk + 48);
+        tmem_st16(t_s + 48, pk + 48);
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(bp_full(q, 1));
@@ -621,38 +613,31 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
         const int32_t t = sv.tile_begin + j;
         mbar_wait(bs_full(q), tile_it & 1);
         tc_fence_after();
-        // The whole S row goes to registers at once and the S buffer is handed back (the MMA warp writes the
-        // other Q tile's S into it, then this Q tile's next one, while this softmax runs).
-        uint32_t sr[128];                                   // one whole S row (fp32 bits)
-        tmem_ld32(t_s + 0, sr + 0);
-        tmem_ld32(t_s + 32, sr + 32);
-        tmem_ld32(t_s + 64, sr + 64);
-        tmem_ld32(t_s + 96, sr + 96);
-        tmem_wait_ld();
-        tc_fence_before();
-        mbar_arrive(bs_free(q));
         const bool need_mask = t >= (t < Tc ? mask_a : mask_b);
-        // ---- exact reference for an unmasked tile: the row maximum, the reference follows it whenever it grew
-        // (the row's largest weight so far is then p = 1, exactly representable in bf16).  Rare (first tiles of
-        // a segment, refused optimistic passes): kept out of the hot path.
+        // ---- exact reference for an unmasked tile: one pass over S for the row maximum, the reference
+        // follows it whenever it grew (the row's largest weight so far is then p = 1, exactly representable
+        // in bf16).  Rare (first tiles of a segment, refused optimistic passes): kept out of the hot path.
         auto exact_reference = [&]() {
-          // (volatile: the maximum must stay inside this rarely taken branch - as plain fmaxf over registers the
-          // compiler computed it speculatively on every tile, 62 FMNMX3 of the ~550 instructions per tile)
-          float mx0 = max3_volatile(__uint_as_float(sr[0]), __uint_as_float(sr[1]), __uint_as_float(sr[2]));
-          float mx1 = max3_volatile(__uint_as_float(sr[3]), __uint_as_float(sr[4]), __uint_as_float(sr[5]));
+          float mx0, mx1, mx2, mx3;
 #pragma unroll
-          for (int i = 6; i < 126; i += 4) {
-            mx0 = max3_volatile(mx0, __uint_as_float(sr[i]), __uint_as_float(sr[i + 1]));
-            mx1 = max3_volatile(mx1, __uint_as_float(sr[i + 2]), __uint_as_float(sr[i + 3]));
+          for (int ch = 0; ch < 4; ++ch) {
+            uint32_t sr[32];
+            tmem_ld32(t_s + ch * 32, sr);
+            tmem_wait_ld();
+            if (ch == 0) { mx0 = __uint_as_float(sr[0]); mx1 = __uint_as_float(sr[1]); mx2 = __uint_as_float(sr[2]); mx3 = __uint_as_float(sr[3]); }
+#pragma unroll
+            for (int i = (ch == 0 ? 4 : 0); i < 32; i += 4) {
+              mx0 = fmaxf(mx0, __uint_as_float(sr[i])); mx1 = fmaxf(mx1, __uint_as_float(sr[i + 1]));
+              mx2 = fmaxf(mx2, __uint_as_float(sr[i + 2])); mx3 = fmaxf(mx3, __uint_as_float(sr[i + 3]));
+            }
           }
-          const float tm = fmaxf(max3_volatile(mx0, __uint_as_float(sr[126]), __uint_as_float(sr[127])), mx1) * c;
+          const float tm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c;
           const bool grow = tm > m_used;
           if (j == 0) {
             m_used = tm;
           } else if (__any_sync(0xffffffffu, grow)) {
             float alpha = 1.f;
             if (grow) { alpha = m_used == -INFINITY ? 0.f : ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
-            wait_prev_pv();
             rescale_o(alpha);
           }
           all_finite = !__any_sync(0xffffffffu, m_used == -INFINITY);
@@ -667,16 +652,22 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #pragma unroll 1
           for (;;) {
             if (!fast) exact_reference();
-            if (stream_tile(sr, fast, fast ? fminf(kFastSumLimit, kFastSumShare * l) : 0.f)) break;
+            if (stream_tile(fast, fast ? fminf(kFastSumLimit, kFastSumShare * l) : 0.f)) break;
             fast = false;
           }
         }
         if (need_mask) {
           // ---- exact path, masked tile (the last tile of the cache part or of the new block when their
-          // lengths are no multiples of 128; multi-block queries)
+          // lengths are no multiples of 128; multi-block queries): whole S row in registers
           const int32_t key0 = t < Tc ? t * kTileKeys : sv.g.cache_len + (t - Tc) * kTileKeys;
           const int32_t lim = t < Tc ? vis_cache : vis;      // keys >= lim of this tile are masked
           uint32_t pk[64];
+          uint32_t sr[128];                                 // one whole S row (fp32 bits)
+          tmem_ld32(t_s + 0, sr + 0);
+          tmem_ld32(t_s + 32, sr + 32);
+          tmem_ld32(t_s + 64, sr + 64);
+          tmem_ld32(t_s + 96, sr + 96);
+          tmem_wait_ld();
 #define S_(i) __uint_as_float(sr[i])
 #pragma unroll
           for (int i = 0; i < 128; ++i)
@@ -720,7 +711,6 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           } else if (__any_sync(0xffffffffu, grow)) {
             float alpha = 1.f;
             if (grow) { alpha = m_used == -INFINITY ? 0.f : ex2_approx(m_used - tm); m_used = tm; l *= alpha; }
-            wait_prev_pv();
             rescale_o(alpha);
           }
           const float m_c = (m_used == -INFINITY) ? 0.f : m_used;
@@ -738,9 +728,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
           }
           l += (l0 + l1) + (l2 + l3);
 #undef S_
-          wait_prev_pv();
-          tmem_st32(t_p + 0, pk);
-          tmem_st32(t_p + 32, pk + 32);
+          tmem_st32(t_s + 0, pk);
+          tmem_st32(t_s + 32, pk + 32);
           // (masked keys: P is exactly 0 there and the bytes behind them are finite - the append keeps the
           // unused tail of a session's last page zeroed, rows past the end of k_new are zero-filled - so
           // 0 x V stays 0)

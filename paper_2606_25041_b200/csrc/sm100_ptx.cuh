@@ -207,12 +207,6 @@ __device__ __forceinline__ float ex2_approx(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-// max(a, b, c) that the compiler may neither speculate nor hoist out of its branch
-__device__ __forceinline__ float max3_volatile(float a, float b, float c) {
-  float y;
-  asm volatile("max.f32 %0, %1, %2, %3;" : "=f"(y) : "f"(a), "f"(b), "f"(c));
-  return y;
-}
 // two fp32 -> packed bf16x2 (lo = first argument), round-to-nearest-even
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   uint32_t r;

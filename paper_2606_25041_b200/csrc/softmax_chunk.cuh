@@ -13,10 +13,7 @@ namespace ws {
 using namespace ptx;
 
 // 2 of every 8 exponentials run as a polynomial on the FMA pipe (ex2_poly2); sweep: DESIGN.md section 8
-#ifndef WS_POLY_PER8
-#define WS_POLY_PER8 0
-#endif
-constexpr int kPolyPer8 = WS_POLY_PER8;
+constexpr int kPolyPer8 = 2;
 
 // 2^x for a PAIR of values on the FMA/ALU pipes (no MUFU): round-to-nearest split x = r + f with
 // f in [-0.5, 0.5], a degree-3 minimax polynomial for 2^f (max relative error 7.5e-5, well inside
