@@ -160,6 +160,31 @@ ws_status_t ws_block_causal_attn_fwd(ws_cache_t* cache, int32_t num_sessions,
                                      const int32_t* cu_q_tokens, const void* q, void* out,
                                      float* lse, float scale, void* cuda_stream);
 
+/* ws_block_causal_attn_fwd for callers that cannot allocate or provide split-KV scratch per call (code under
+ * CUDA-graph capture, serving loops and harnesses that forbid cudaMalloc): same arguments, same host path, same
+ * kernels and results (a3 + a4, Eq. (1); split-KV combine from north_star), but the partials of the
+ * split-KV plan go to a file-scope static __device__ array inside the library image instead of the cache's
+ * workspace.  The call and everything below it call no cudaMalloc / cudaFree / allocating library routine.
+ *  - Size: WS_STATIC_PART_SLOTS partial slots ([256 rows][128] fp32 + [256] fp32 LSE each) = 8,454,144 bytes,
+ *    held by EVERY GPU that loads the library until the process exits.
+ *  - A call whose plan needs more slots returns WS_ERR_WORKSPACE_TOO_SMALL with nothing launched and no state
+ *    changed (one slot per (KV range, row-tile pair) of a split group; e.g. BASELINE config 2 needs ~144: use the
+ *    workspace path there).  Plans that do not split (or the CUDA-core kernel) use no scratch at all.
+ *  - Not with WS_FLAG_FUSED_COMBINE (WS_ERR_UNSUPPORTED): that mode's arrival counters live in the workspace.
+ *  - ALL calls of the process on one device share the array.  Nothing in it has to start at zero (every slot a
+ *    launch reads was written by the same launch chain first) and the previous call's contents are simply
+ *    overwritten, but calls that OVERLAP on the GPU (different streams, different caches) race on it: issue
+ *    them on one stream, or order them with events.
+ *  - The device address of the array is resolved once per device (cudaGetSymbolAddress with that device
+ *    current).  ws_static_scratch_setup(device) does that ahead of time - call it once per device before stream
+ *    capture; otherwise the first ws_block_causal_attn_fwd_static on a device does it.                        */
+#define WS_STATIC_PART_SLOTS 64
+ws_status_t ws_static_scratch_setup(int32_t device);
+ws_status_t ws_block_causal_attn_fwd_static(ws_cache_t* cache, int32_t num_sessions,
+                                            const int32_t* session_ids, const int32_t* num_q_blocks,
+                                            const int32_t* cu_q_tokens, const void* q, void* out,
+                                            float* lse, float scale, void* cuda_stream);
+
 /* NEXT-4 (optional half) - mixed intra-block mask.  PAPER.md:31 "the short token-causal Transformer pass
  * for language prediction and state update", :77 "token-causal decoding over the language and state
  * slots", while audio/video units are block-wise.  Reading A19: with

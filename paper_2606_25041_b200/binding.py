@@ -62,7 +62,8 @@ EXPORTS = ["ws_replica_link", "ws_replica_accept", "ws_replica_commit_message",
            "ws_session_open", "ws_session_close", "ws_session_info", "ws_session_truncate",
            "ws_free_pages", "ws_kv_append", "ws_kv_append_blocks", "ws_block_causal_attn_fwd", "ws_step_staging_bytes",
            "ws_stream_step", "ws_stream_step_tagged", "ws_block_causal_attn_fwd_masked", "ws_stream_step_host", "ws_stream_host_join", "ws_fm_euler_update", "ws_kv_gather", "ws_session_pages", "ws_debug_shuffle_free_pages",
-           "ws_debug_set_min_splits", "ws_debug_set_decode_plan", "ws_last_plan_info", "ws_last_plan_segment",
+           "ws_debug_set_min_splits", "ws_debug_set_decode_plan", "ws_static_scratch_setup",
+           "ws_block_causal_attn_fwd_static", "ws_last_plan_info", "ws_last_plan_segment",
            "ws_launch_count", "ws_debug_kernel_timing", "ws_debug_read_kernel_times",
            "ws_status_str", "ws_last_error", "ws_version"]
 
@@ -94,6 +95,9 @@ def load_library() -> C.CDLL:
     lib.ws_kv_append_blocks.argtypes = [vp, C.c_int32, i32p, i32p, i32p, i32p, vp, vp, C.POINTER(C.c_uint8), vp]
     lib.ws_block_causal_attn_fwd.argtypes = [vp, C.c_int32, i32p, i32p, i32p, vp, vp, vp,
                                              C.c_float, vp]
+    lib.ws_block_causal_attn_fwd_static.argtypes = [vp, C.c_int32, i32p, i32p, i32p, vp, vp, vp,
+                                                    C.c_float, vp]
+    lib.ws_static_scratch_setup.argtypes = [C.c_int32]
     lib.ws_block_causal_attn_fwd_masked.argtypes = [vp, C.c_int32, i32p, i32p, i32p, vp, vp, vp,
                                                     C.c_float, C.c_uint32, vp]
     lib.ws_stream_step_tagged.argtypes = [vp, C.c_int32, i32p, i32p, vp, vp, vp, C.POINTER(C.c_uint8),
@@ -283,6 +287,14 @@ class Cache:
                                                  nqb, _i32(cu_q_tokens), _ptr(q), _ptr(out),
                                                  _ptr(lse), C.c_float(scale), _stream_ptr(stream)))
 
+    def block_causal_attn_fwd_static(self, session_ids, cu_q_tokens, q, out, scale: float, lse=None,
+                                     num_q_blocks=None, stream=None):
+        """ws_block_causal_attn_fwd_static: split-KV partials in the library's static device array (no allocation)."""
+        nqb = _i32(num_q_blocks) if num_q_blocks is not None else None
+        _check(self.lib.ws_block_causal_attn_fwd_static(self.handle, len(session_ids), _i32(session_ids),
+                                                        nqb, _i32(cu_q_tokens), _ptr(q), _ptr(out),
+                                                        _ptr(lse), C.c_float(scale), _stream_ptr(stream)))
+
     def stream_step(self, session_ids, cu_new_tokens, q, k_new, v_new, out, scale: float, lse=None, stream=None,
                     modality=None, attn_flags: int = 0):
         """ws_kv_append + ws_block_causal_attn_fwd of the block just committed, one call (device buffers).
@@ -410,6 +422,15 @@ def ws_kv_append_blocks(cache: Cache, session_ids, cu_new_tokens, cu_blocks, blo
 def ws_block_causal_attn_fwd(cache: Cache, session_ids, cu_q_tokens, q, out, scale, lse=None,
                              num_q_blocks=None, stream=None):
     cache.block_causal_attn_fwd(session_ids, cu_q_tokens, q, out, scale, lse, num_q_blocks, stream)
+
+
+def ws_block_causal_attn_fwd_static(cache: Cache, session_ids, cu_q_tokens, q, out, scale, lse=None,
+                                    num_q_blocks=None, stream=None):
+    cache.block_causal_attn_fwd_static(session_ids, cu_q_tokens, q, out, scale, lse, num_q_blocks, stream)
+
+
+def ws_static_scratch_setup(device: int = 0) -> None:
+    _check(load_library().ws_static_scratch_setup(device))
 
 
 def ws_kv_gather(cache: Cache, session, start, count, k_out, v_out, stream=None):

@@ -839,9 +839,78 @@ ws_status_t attn_validate_args(ws_cache* c, int32_t S, const int32_t* session_id
   return WS_OK;
 }
 
+// ---- ws_block_causal_attn_fwd_static: split-KV scratch inside the library image (no allocation anywhere) ----
+// The partials of the split-KV plan (a3 -> a4: normalised fp32 O per partial slot + log2-LSEs) normally live in
+// the caller's workspace.  This array is the same scratch for callers that cannot provide / allocate one:
+// WS_STATIC_PART_SLOTS partial slots of [256 rows][128] fp32 followed by the slots' [256] fp32 LSEs = 8,454,144
+// bytes, held by every GPU that loads the library until the process exits.  In HOST code the name below is only
+// a stand-in for the symbol: the device address comes from cudaGetSymbolAddress, once per device, with that
+// device current (static_scratch_ensure), and that pointer is what the kernels get.
+constexpr size_t kStaticPartOBytes = (size_t)WS_STATIC_PART_SLOTS * ws::kPairRows * 128 * sizeof(float);
+constexpr size_t kStaticPartLseBytes = (size_t)WS_STATIC_PART_SLOTS * ws::kPairRows * sizeof(float);
+static __device__ __align__(256) unsigned char g_static_part_scratch[kStaticPartOBytes + kStaticPartLseBytes];
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+void* g_static_scratch_ptr[kStaticMaxDevices] = {};      // device address of the array on each device (0 = not set up)
+
+// Resolves the array's address on `device` (made current for the call, restored afterwards).  No allocation:
+// the array is part of the loaded module.
+ws_status_t static_scratch_ensure(int device, void** ptr_out) {
+  if (device < 0 || device >= kStaticMaxDevices) return fail(WS_ERR_INVALID_ARG, "device %d out of range", device);
+  std::lock_guard<std::mutex> lk(g_static_mu);
+  if (!g_static_scratch_ptr[device]) {
+    int prev = -1;
+    WS_CUDA(cudaGetDevice(&prev));
+    if (prev != device) WS_CUDA(cudaSetDevice(device));
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_part_scratch);
+    if (prev != device) (void)cudaSetDevice(prev);
+    if (e != cudaSuccess || !ptr)
+      return fail(WS_ERR_CUDA, "cudaGetSymbolAddress(static split-KV scratch) on device %d: %s", device,
+                  cudaGetErrorString(e));
+    g_static_scratch_ptr[device] = ptr;
+  }
+  if (ptr_out) *ptr_out = g_static_scratch_ptr[device];
+  return WS_OK;
+}
+
 }  // namespace
 
 extern "C" {
+
+ws_status_t ws_static_scratch_setup(int32_t device) { return static_scratch_ensure(device, nullptr); }
+
+ws_status_t ws_block_causal_attn_fwd_static(ws_cache_t* c, int32_t S, const int32_t* session_ids,
+                                            const int32_t* num_q_blocks, const int32_t* cu, const void* q,
+                                            void* out, float* lse, float scale, void* cuda_stream) {
+  ws_status_t st = attn_validate_args(c, S, session_ids, cu, q, out, scale);
+  if (st != WS_OK) return st;
+  if (c->dry) return fail(WS_ERR_INVALID_ARG, "ws_block_causal_attn_fwd_static needs a device cache (not WS_FLAG_DRY_RUN)");
+  if (c->cfg.flags & WS_FLAG_FUSED_COMBINE)
+    return fail(WS_ERR_UNSUPPORTED, "ws_block_causal_attn_fwd_static: not with WS_FLAG_FUSED_COMBINE (its counters live in the workspace)");
+  DeviceGuard dg(c);
+  void* scratch = nullptr;
+  st = static_scratch_ensure(c->cfg.device, &scratch);
+  if (st != WS_OK) return st;
+  // The same host path and the same kernels as ws_block_causal_attn_fwd; for the duration of this call the
+  // cache's partial-slot views point into the static array and the planner's slot budget is the array's.
+  float* const save_o = c->d_part_o;
+  float* const save_lse = c->d_part_lse;
+  const int32_t save_slots = c->lay.max_part_slots;
+  c->d_part_o = reinterpret_cast<float*>(scratch);
+  c->d_part_lse = reinterpret_cast<float*>(static_cast<unsigned char*>(scratch) + kStaticPartOBytes);
+  c->lay.max_part_slots = std::min<int32_t>(save_slots, WS_STATIC_PART_SLOTS);
+  st = attn_impl(c, S, session_ids, num_q_blocks, cu, q, out, lse, scale, (cudaStream_t)cuda_stream, nullptr);
+  c->d_part_o = save_o; c->d_part_lse = save_lse; c->lay.max_part_slots = save_slots;
+  if (st == WS_ERR_WORKSPACE_TOO_SMALL) {
+    return fail(WS_ERR_WORKSPACE_TOO_SMALL,
+                "ws_block_causal_attn_fwd_static: the split-KV plan of this call needs more than the %d partial slots "
+                "(%zu bytes) of the library's static scratch; nothing was launched - use ws_block_causal_attn_fwd "
+                "with a workspace", (int)WS_STATIC_PART_SLOTS, kStaticPartOBytes + kStaticPartLseBytes);
+  }
+  return st;
+}
 
 ws_status_t ws_kv_append(ws_cache_t* c, int32_t S, const int32_t* session_ids,
                          const int32_t* cu, const void* k_new, const void* v_new,
