@@ -195,8 +195,8 @@ attn_dec_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const uint64_t desc_v = make_smem_desc_sw128(0, kHalfBytes, 1024);  // MN-major operand (V)
       uint32_t ring_it = 0, q_it = 0, seg_it = 0, tiles0 = 0, tiles1 = 0;
       auto issue_S = [&](int b, uint32_t slot) {              // S_b = Q K^T (tile parity b)
-        const uint64_t da = desc_k + (sQ >> 4);
-        const uint64_t db = desc_k + ((sRing + slot * kSlotBytes) >> 4);
+        const uint64_t da = desc_k + ((sQ & 0x3FFFFu) >> 4);
+        const uint64_t db = desc_k + (((sRing + slot * kSlotBytes) & 0x3FFFFu) >> 4);   // (mask: see kDescAddrMask in attn_sm100.cu)
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {
           const uint32_t off = ((ks >> 2) * kHalfBytes + (ks & 3) * 32) >> 4;
@@ -206,7 +206,7 @@ attn_dec_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       // O += P V for the 64 keys of warpgroup `half`: its P (bf16 pairs) sits in the first 32 columns of its own
       // half of S_b
       auto issue_PV = [&](int b, uint32_t slot, int half, bool accumulate) {
-        const uint64_t db = desc_v + ((sRing + slot * kSlotBytes) >> 4);
+        const uint64_t db = desc_v + (((sRing + slot * kSlotBytes) & 0x3FFFFu) >> 4);
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           const int ks = half * 4 + i;

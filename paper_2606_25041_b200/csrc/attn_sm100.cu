@@ -75,6 +75,12 @@ constexpr float kFastSumLimit = 1024.0f;
 constexpr float kFastSumShare = 1.0f;
 constexpr int kExactFirstTiles = 2;                         // tiles 0-1 of a segment go straight to the exact path
 
+// Shared-memory matrix descriptors hold bits [4, 18) of the CTA-local address.  In a CLUSTER launch the shared-window
+// address of a CTA of rank >= 1 carries its rank in higher bits; unmasked they spill into the descriptor's
+// leading-byte-offset field - harmless for the K-major operands (Q, K: LBO unused), wrong upper 64 dims for the
+// MN-major V (found with the cluster-plan experiment, DESIGN.md section 8 x: LSE exact, O columns 64-127 wrong on
+// ranks >= 1).  This kernel is not launched in clusters today; the mask keeps the descriptors right if it ever is.
+constexpr uint32_t kDescAddrMask = 0x3FFFFu;
 constexpr int kMaxJobs = 4;
 
 struct Barriers {
@@ -338,8 +344,8 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const uint64_t desc_v = make_smem_desc_sw128(0, kHalfBytes, 1024);  // MN-major operand (V)
       uint32_t ring_it = 0, q_it = 0, tile_it = 0, seg_it = 0;
       auto issue_S = [&](int q, uint32_t slot) {
-        const uint64_t da = desc_k + ((sQ + q * kQTileBytes) >> 4);
-        const uint64_t db = desc_k + ((sRing + slot * kSlotBytes) >> 4);
+        const uint64_t da = desc_k + (((sQ + q * kQTileBytes) & kDescAddrMask) >> 4);
+        const uint64_t db = desc_k + (((sRing + slot * kSlotBytes) & kDescAddrMask) >> 4);
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {
           const uint32_t off = ((ks >> 2) * kHalfBytes + (ks & 3) * 32) >> 4;
@@ -348,7 +354,7 @@ attn_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q,
       };
       // PV for one of the two pieces in which the softmax hands P over (k-steps of 16 keys)
       auto issue_PV = [&](int q, uint32_t slot, int half, bool accumulate) {
-        const uint64_t db = desc_v + ((sRing + slot * kSlotBytes) >> 4);
+        const uint64_t db = desc_v + (((sRing + slot * kSlotBytes) & kDescAddrMask) >> 4);
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {
           if ((ks < kFirstPieceSteps) != (half == 0)) continue;   // piece 0: keys 0-95, piece 1: keys 96-127
