@@ -102,3 +102,44 @@ def test_static_scratch_entry_point_rejects_plans_beyond_its_size():
     c.block_causal_attn_fwd([sid], [0, n], q, out, scale)
     torch.cuda.synchronize()
     assert c.last_plan_info()["num_partial_slots"] > 64 and bool(torch.isfinite(out.float()).all())
+
+
+def test_static_scratch_entry_point_ragged_batch_and_generic_kernel():
+    """Three sessions of unequal history in one call (bf16, tcgen05 kernel, split plan) and the fp32 cache (CUDA-core
+    kernel: no scratch in use at all) through the same entry point: both equal the existing path bit for bit."""
+    import torch
+    from paper_2606_25041_b200 import WS_BF16, WS_F32, Cache
+    dev = torch.device("cuda", 0)
+    for dtype, tdt, Hq, Hkv, D, P, lens, n in ((WS_BF16, torch.bfloat16, 8, 2, 128, 64, (700, 1531, 2048), 48),
+                                               (WS_F32, torch.float32, 2, 2, 64, 16, (0, 33), 16)):
+        S = len(lens)
+        pages = sum((L + n + P - 1) // P for L in lens) + 4
+        c = Cache(dtype, Hq, Hkv, D, P, pages, max_sessions=S, max_sessions_per_call=S, max_q_tokens_per_call=max(S * n, 256))
+        g = torch.Generator(device=dev); g.manual_seed(21)
+        ids = [c.session_open() for _ in lens]
+        for sid, L in zip(ids, lens):
+            pos = 0
+            while pos < L:
+                m = min(256, L - pos)
+                c.kv_append([sid], [0, m], torch.randn((m, Hkv, D), device=dev, generator=g).to(tdt),
+                            torch.randn((m, Hkv, D), device=dev, generator=g).to(tdt)); pos += m
+        cu = [i * n for i in range(S + 1)]
+        c.kv_append(ids, cu, torch.randn((S * n, Hkv, D), device=dev, generator=g).to(tdt),
+                    torch.randn((S * n, Hkv, D), device=dev, generator=g).to(tdt))
+        q = torch.randn((S * n, Hq, D), device=dev, generator=g).to(tdt)
+        scale = 1.0 / math.sqrt(D)
+        want, got = torch.empty_like(q), torch.full_like(q, float("nan"))
+        wl = torch.empty((S * n, Hq), dtype=torch.float32, device=dev); gl = torch.full_like(wl, float("nan"))
+        c.block_causal_attn_fwd(ids, cu, q, want, scale, lse=wl)
+        info = c.last_plan_info()
+        c.block_causal_attn_fwd_static(ids, cu, q, got, scale, lse=gl)
+        torch.cuda.synchronize()
+        assert c.last_plan_info() == info
+        if dtype == WS_BF16:
+            assert info["used_tensor_core_kernel"] == 1 and 0 < info["num_partial_slots"] <= 64, info
+        else:
+            assert info["used_tensor_core_kernel"] == 0
+        d = (got.float() - want.float()).abs()
+        assert bool(torch.isfinite(got.float()).all()) and float(d.max()) <= (TOL_MAX_ABS if dtype == WS_BF16 else 1e-5)
+        assert float((gl - wl).abs().max()) <= (TOL_LSE if dtype == WS_BF16 else 1e-5)
+        assert bool((got == want).all()) and bool((gl == wl).all())
