@@ -821,7 +821,10 @@ ws_status_t attn_impl(ws_cache* c, int32_t S, const int32_t* session_ids, const 
     TimedLaunch tc(c, &c->t_combine, stream);
     int32_t max_parts = 1;
     for (const ws::CombineItem& ci : c->last_plan.combine) max_parts = std::max(max_parts, ci.nparts);
-    WS_CUDA(ws::launch_combine(L.p, L.inl, L.inl_words, (int32_t)c->last_plan.combine.size(), c->last_plan.team_size, max_parts, stream));
+    int32_t max_nq = 0;                                    // most query tokens of one session in this call
+    for (int32_t s = 0; s < S; ++s) max_nq = std::max(max_nq, cu[s + 1] - cu[s]);
+    WS_CUDA(ws::launch_combine(L.p, L.inl, L.inl_words, (int32_t)c->last_plan.combine.size(), c->last_plan.team_size, max_parts,
+                               (int32_t)std::min<int64_t>(ws::kPairRows, (int64_t)max_nq * G), stream));
     tc.done();
     c->launches += 1;
   }

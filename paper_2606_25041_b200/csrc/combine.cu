@@ -27,18 +27,18 @@ namespace ws {
 constexpr int kCombineRowsPerBlock = 8;
 
 // kDepth = O-row loads in flight per lane: 4 keeps the kernel at 64 registers (8 blocks / SM) for
-// the large grids of the general plan; 8 serves the small grids of decode steps, where few warps
-// have work and memory-level parallelism has to come from each of them.
+// the large grids of the general plan; 20 serves the small grids of decode steps (one 65k-key step has 18-19
+// parts per row), where few warps have work, memory-level parallelism has to come from each of them, and the
+// O rows are requested together with the LSEs (kEager).
 template <int kInlW, int kDepth>
 __global__ void __launch_bounds__(kCombineRowsPerBlock * 32)
-combine_rows_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int32_t team_size) {
+combine_rows_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl, int32_t team_size, int32_t blocks_per_pair) {
   // The successor (the next step's append or attention kernel) may be scheduled at once: before its own
   // griddepcontrol.wait it touches nothing this kernel or the attention kernel before it writes (launch.h).
   pdl_launch_dependents();
   pdl_wait();                      // partials of the attention kernel launched just before
   const MetaView<kInlW> meta{p.meta, inl};
   const AttnMeta hdr = meta.template load<AttnMeta>(0);
-  const int32_t blocks_per_pair = kPairRows / kCombineRowsPerBlock;
   int32_t b = blockIdx.x;
   const int32_t rchunk = b % blocks_per_pair; b /= blocks_per_pair;
   const int32_t pair = b % team_size;
@@ -61,6 +61,17 @@ combine_rows_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl,
   for (int32_t base = 0; base < ci.nparts; base += 32) {
     const int32_t i = base + lane;
     const float l2 = i < ci.nparts ? p.part_lse[(slot0 + i * stride) * kPairRows + r] : -INFINITY;
+    const int32_t cnt = min(32, ci.nparts - base);
+    // Deep variant (few rows, many parts: decode steps): the first kDepth O rows are requested TOGETHER with the
+    // LSEs - their addresses do not depend on them - so the row pays one round trip instead of two.
+    constexpr bool kEager = kDepth > 8;
+    float4 o0[kEager ? kDepth : 1];
+    if constexpr (kEager) {
+#pragma unroll
+      for (int u = 0; u < kDepth; ++u)
+        o0[u] = u < cnt ? reinterpret_cast<const float4*>(p.part_o + ((slot0 + (base + u) * stride) * kPairRows + r) * p.D)[lane]
+                        : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
     float mx = l2;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
@@ -74,7 +85,6 @@ combine_rows_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl,
     acc.x *= rescale; acc.y *= rescale; acc.z *= rescale; acc.w *= rescale;
     wsum_run = wsum_run * rescale + ws;
     mx_run = mx_new;
-    const int32_t cnt = min(32, ci.nparts - base);
     for (int32_t k0 = 0; k0 < cnt; k0 += kDepth) {
       float4 o[kDepth];
       float wk[kDepth];
@@ -82,9 +92,13 @@ combine_rows_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl,
       for (int u = 0; u < kDepth; ++u) {
         const int32_t k = k0 + u;
         wk[u] = __shfl_sync(0xffffffffu, w, k & 31);
-        if (k < cnt && wk[u] != 0.f)
+        if (kEager && k0 == 0) {
+          // (requested above; a part with weight 0 - an empty range - may hold stale bytes: not used)
+          if (k < cnt && wk[u] != 0.f) o[u] = o0[u];
+          else { o[u] = make_float4(0.f, 0.f, 0.f, 0.f); wk[u] = 0.f; }
+        } else if (k < cnt && wk[u] != 0.f) {
           o[u] = reinterpret_cast<const float4*>(p.part_o + ((slot0 + (base + k) * stride) * kPairRows + r) * p.D)[lane];
-        else { o[u] = make_float4(0.f, 0.f, 0.f, 0.f); wk[u] = 0.f; }
+        } else { o[u] = make_float4(0.f, 0.f, 0.f, 0.f); wk[u] = 0.f; }
       }
 #pragma unroll
       for (int u = 0; u < kDepth; ++u) {
@@ -158,22 +172,27 @@ cudaError_t combine_configure() {
 }
 
 cudaError_t launch_combine(const AttnParams& p, const InlineAttnMetaLarge& inl, int32_t inl_words,
-                           int32_t num_combine, int32_t team_size, int32_t max_parts, cudaStream_t stream) {
+                           int32_t num_combine, int32_t team_size, int32_t max_parts, int32_t max_rows_per_pair,
+                           cudaStream_t stream) {
   if (num_combine == 0) return cudaSuccess;
   const bool small_tier = inl_words <= kInlineAttnWords;
   InlineAttnMeta small;
   if (small_tier) memcpy(small.w, inl.w, sizeof(small.w));
   if (max_parts > kStagedMaxParts) {
     // many parts per row: a staged block would hold only a few rows - one warp per row instead
-    const int32_t grid = num_combine * team_size * (kPairRows / kCombineRowsPerBlock);
+    // blocks only for the packed rows a pair can hold in this call (a one-token decode step has G rows per group:
+    // one block instead of 32, of which 31 would find nothing to do)
+    const int32_t rows = std::max(1, std::min<int32_t>(kPairRows, max_rows_per_pair));
+    const int32_t bpp = (rows + kCombineRowsPerBlock - 1) / kCombineRowsPerBlock;
+    const int32_t grid = num_combine * team_size * bpp;
     const dim3 g(grid), b(kCombineRowsPerBlock * 32);
-    const bool deep = grid <= 2 * 148;
+    const bool deep = grid <= 148;                      // (205 registers: one block per SM)
     if (small_tier) {
-      if (deep) return launch_pdl(combine_rows_kernel<kInlineAttnWords, 8>, g, b, 0, stream, p, small, team_size);
-      return launch_pdl(combine_rows_kernel<kInlineAttnWords, 4>, g, b, 0, stream, p, small, team_size);
+      if (deep) return launch_pdl(combine_rows_kernel<kInlineAttnWords, 20>, g, b, 0, stream, p, small, team_size, bpp);
+      return launch_pdl(combine_rows_kernel<kInlineAttnWords, 4>, g, b, 0, stream, p, small, team_size, bpp);
     }
-    if (deep) return launch_pdl(combine_rows_kernel<kInlineAttnWordsLarge, 8>, g, b, 0, stream, p, inl, team_size);
-    return launch_pdl(combine_rows_kernel<kInlineAttnWordsLarge, 4>, g, b, 0, stream, p, inl, team_size);
+    if (deep) return launch_pdl(combine_rows_kernel<kInlineAttnWordsLarge, 20>, g, b, 0, stream, p, inl, team_size, bpp);
+    return launch_pdl(combine_rows_kernel<kInlineAttnWordsLarge, 4>, g, b, 0, stream, p, inl, team_size, bpp);
   }
   // rows per block: as many as fit the staging area in one piece for the item with the most parts
   const int32_t rows_pb = std::max(1, std::min(kCombineRowsMax, kCombineRowsCap / std::max(1, max_parts)));

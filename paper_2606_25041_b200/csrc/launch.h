@@ -93,6 +93,7 @@ cudaError_t dec_sm100_configure();
 cudaError_t launch_attn_dec_sm100(const Sm100Launch& l, cudaStream_t stream);
 cudaError_t combine_configure();        // one-time cudaFuncSetAttribute
 cudaError_t launch_combine(const AttnParams& p, const InlineAttnMetaLarge& inl, int32_t inl_words,
-                           int32_t num_combine, int32_t team_size, int32_t max_parts, cudaStream_t stream);
+                           int32_t num_combine, int32_t team_size, int32_t max_parts, int32_t max_rows_per_pair,
+                           cudaStream_t stream);
 
 }  // namespace ws
