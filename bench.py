@@ -256,6 +256,22 @@ def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, r
         reps = 200
         ms = timed(reps, lambda i: gd.replay())
         reset()
+        # the same step 8 times in ONE graph (the block is rolled back on the host after every captured step, so
+        # each one attends the same 65,536-token history): the chain a multi-layer decode pass or a solver loop
+        # enqueues - the kernels keep their programmatic dependent launch edges, which separate graph launches lose
+        chain = 8
+        torch.cuda.synchronize()
+        gc = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(gc):
+            for _ in range(chain):
+                cache.stream_step(ids, cud, qd, kd, vd, od, sp.scale)
+                reset()
+        for _ in range(3):
+            gc.replay()
+        creps = 40
+        ms_chain = timed(creps, lambda i: gc.replay())
+        reset()
+        us_chain = 1e3 * ms_chain / creps / chain
         Lk = w_cache_len + n_dec
         eb = 2
         byts = 2 * eb * sp.num_kv_heads * sp.head_dim * Lk + 2 * eb * sp.num_q_heads * sp.head_dim * n_dec \
@@ -266,6 +282,10 @@ def measure_next(cache, ids, base_blocks, sp, cu, q0, k0, v0, out, dev, timed, r
             "hbm_gbs": byts / us / 1e3, "hbm_peak_gbs": float(peaks["hbm_gbs"]),
             "frac_of_hbm_roofline": byts / us / 1e3 / float(peaks["hbm_gbs"]),
             "kernel": plan["used_tensor_core_kernel"],
+            "chained": {"steps_per_graph": chain, "us_per_step": us_chain, "hbm_gbs": byts / us_chain / 1e3,
+                        "frac_of_hbm_roofline": byts / us_chain / 1e3 / float(peaks["hbm_gbs"]),
+                        "what": "8 such steps captured in one graph (programmatic dependent launch between them), "
+                                "each over the same history, rolled back on the host during capture"},
             "what": "ws_stream_step (commit + attention on the decode plan in one launch, + combine), CUDA-graph replay, history read from HBM"})
     # --- NEXT-3: replica link (thinker -> performer KV-slice exchange).  The box has ONE GPU, so the
     # linked pool is a second pool on the same device: these numbers show the cost of the extra stores
