@@ -122,7 +122,7 @@ combine_rows_kernel(AttnParams p, const __grid_constant__ InlineMeta<kInlW> inl,
 
 // ---- staged variant ----
 constexpr int kStagedMaxParts = 8;                     // more parts per row than this: row-per-warp variant (12 measured the same)
-constexpr int kCombineRowsMax = 32;                    // rows per block (fewer when a row has many parts)
+constexpr int kCombineRowsMax = 64;                    // rows per block (fewer when a row has many parts)
 constexpr int kCombineRowsCap = 192;                   // staged rows x parts per chunk: 96 KB -> 2 blocks / SM
 constexpr uint32_t kCombineLseBytes = 8192;            // nparts x (rows + 8) fp32, nparts <= 148
 constexpr uint32_t kCombineSmem = kCombineRowsCap * 512 + kCombineLseBytes + 1024;
