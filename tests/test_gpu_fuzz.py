@@ -51,3 +51,53 @@ def test_random_shapes_match_oracle(case):
     assert err["bound_viol"] <= 0 and err["mean_abs"] <= 1e-3 and err["rel_rms"] <= 1e-2 and err["lse_max"] <= 1e-4
     if max(np.abs(o).max() for step in ref["out"] for o in step) < 1.0:
         assert err["max_abs"] <= 1e-2
+
+
+def _wide_cases():
+    """A second, wider draw: odd KV head counts, up to five ragged sessions, cache lengths up to 9000 and around every
+    page / tile boundary, x8 outlier channels (reading A15), the decode plan forced on or off, shuffled free pages, and
+    G in {3, 6} - group sizes the tcgen05 kernel does not cover, which the generic CUDA-core kernel serves (ws.h,
+    `head_dim`).  Forced split counts are kept within the workspace's partial slots."""
+    rng = np.random.default_rng([2606, 25041, 1905])
+    out = []
+    for i in range(48):
+        Hkv = int(rng.choice([1, 2, 3, 4, 8]))
+        G = int(rng.choice([3, 6])) if i % 6 == 5 else int(rng.choice([1, 2, 4, 8, 16]))
+        n = int(rng.choice([1, 2, 3, 4, 7, 8, 15, 16, 17, 31, 32, 33, 63, 64, 65, 96, 127, 128, 129, 200, 255, 256, 257,
+                            300, 384, 513]))
+        S = int(rng.choice([1, 1, 2, 3, 5]))
+        lens = tuple(int(x) for x in rng.integers(0, int(rng.choice([300, 2600, 9000])), size=S))
+        if i % 5 == 0:
+            lens = tuple(int(rng.choice([0, 1, 63, 64, 65, 127, 128, 129, 191, 192, 193, 1023, 1024, 1025, 4095, 4096,
+                                         4097])) for _ in range(S))
+        splits = int(rng.choice([0, 0, 2, 3, 5, 9]))
+        groups = S * Hkv * (-(-n * G // 256))
+        if groups * max(splits, 1) > 400:
+            splits = 0
+        out.append(dict(idx=i, Hkv=Hkv, G=G, n=n, lens=lens, steps=int(rng.choice([1, 2, 3])), splits=splits,
+                        fused=bool(rng.integers(0, 2)), seed_cfg=2 if S == 1 else 5, outl=bool(rng.integers(0, 4) == 0),
+                        decode=[None, True, False][int(rng.integers(0, 3))], shuffle=int(rng.integers(0, 1000))))
+    return out
+
+
+@pytest.mark.parametrize("case", _wide_cases(),
+                         ids=lambda c: f"w{c['idx']}_S{len(c['lens'])}_h{c['Hkv']}x{c['G']}_n{c['n']}")
+def test_random_shapes_wide_match_oracle(case):
+    n = case["n"]
+    text = max(0, n // 16)
+    spec = spec_for_config(case["seed_cfg"], num_sessions=len(case["lens"]), cache_lens=case["lens"], cache_len_range=None,
+                           num_q_heads=case["Hkv"] * case["G"], num_kv_heads=case["Hkv"], block_tokens=n,
+                           modality_split=(n - text - min(n - text, n // 4), min(n - text, n // 4), text),
+                           steps=case["steps"], outlier_frac=0.05 if case["outl"] else 0.0,
+                           outlier_scale=8.0 if case["outl"] else 1.0)
+    w = generate(spec)
+    ref = run_workload_oracle(w)
+    got = run_workload_gpu(w, min_splits=case["splits"], fused_step=case["fused"], pool_fill=0x7FC1,
+                           decode_plan=case["decode"], shuffle_seed=case["shuffle"])
+    assert got["tensor"] == (case["G"] in (1, 2, 4, 8, 16))
+    err = compare(got, ref, "bf16")
+    print(f"[parity] fuzz-wide {case}: " + " ".join(f"{k}={v:.3e}" if isinstance(v, float) else f"{k}={v}" for k, v in err.items()))
+    assert err["finite"] and err["kv_bit_exact"]
+    assert err["bound_viol"] <= 0 and err["mean_abs"] <= 1e-3 and err["rel_rms"] <= 1e-2 and err["lse_max"] <= 1e-4
+    if max(np.abs(o).max() for step in ref["out"] for o in step) < 1.0:
+        assert err["max_abs"] <= 1e-2
