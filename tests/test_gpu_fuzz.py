@@ -101,3 +101,32 @@ def test_random_shapes_wide_match_oracle(case):
     assert err["bound_viol"] <= 0 and err["mean_abs"] <= 1e-3 and err["rel_rms"] <= 1e-2 and err["lse_max"] <= 1e-4
     if max(np.abs(o).max() for step in ref["out"] for o in step) < 1.0:
         assert err["max_abs"] <= 1e-2
+
+
+@pytest.mark.parametrize("S,Hkv,G,n,hi,fused,decode", [
+    (32, 2, 4, 1, 2000, True, None),        # batched one-token decode, 32 sessions
+    (64, 1, 4, 1, 1500, False, None),       # 64 sessions, separate append / attend calls
+    (32, 8, 4, 4, 1500, True, None),        # 256 (session, KV head) groups on 148 CTAs
+    (24, 2, 8, 64, 1200, True, None),       # general plan, teams of two
+    (48, 1, 16, 8, 800, True, True),        # 128 packed rows per group on the decode kernel
+    (20, 8, 4, 33, 600, True, False),       # more groups than CTAs, decode plan off
+], ids=lambda v: str(v))
+def test_many_session_batches_match_oracle(S, Hkv, G, n, hi, fused, decode):
+    """Serving-sized batches: BASELINE config 5's ragged multi-session shape widened to tens of sessions in ONE call,
+    more (session, KV head) groups than CTAs; vs the oracle at every element, append bit-exact."""
+    rng = np.random.default_rng([S, Hkv, G, n])
+    lens = tuple(int(x) for x in rng.integers(0, hi, size=S))
+    text = n // 16
+    spec = spec_for_config(5, num_sessions=S, cache_lens=lens, cache_len_range=None, num_q_heads=Hkv * G, num_kv_heads=Hkv,
+                           block_tokens=n, modality_split=(n - text - min(n - text, n // 4), min(n - text, n // 4), text),
+                           steps=2, outlier_frac=0.0, outlier_scale=1.0)
+    w = generate(spec)
+    ref = run_workload_oracle(w)
+    got = run_workload_gpu(w, fused_step=fused, pool_fill=0x7FC1, decode_plan=decode)
+    assert got["tensor"]
+    err = compare(got, ref, "bf16")
+    print(f"[parity] batch S={S} Hkv={Hkv} G={G} n={n} plan={got['plans'][-1]}: "
+          + " ".join(f"{k}={v:.3e}" if isinstance(v, float) else f"{k}={v}" for k, v in err.items()))
+    assert err["finite"] and err["kv_bit_exact"]
+    assert err["bound_viol"] <= 0 and err["max_abs"] <= 1e-2 and err["mean_abs"] <= 1e-3 and err["rel_rms"] <= 1e-2
+    assert err["lse_max"] <= 1e-4
