@@ -365,3 +365,53 @@ def test_text_causal_random_shapes(case):
                                                          min_splits=case["splits"], p_text=case["p_text"])
     assert all(p["used_tensor_core_kernel"] in (1, 3) for p in plans), plans
     _gate_bf16(o, l, o_ref, l_ref, a_ref, f"fuzz {case}")
+
+
+# ------------------------------------------------------------------------------------------ host-buffer step, ragged units
+def test_stream_step_host_ragged_units_back_to_back():
+    """ws_stream_step_host with units of DIFFERENT sizes enqueued back to back (no host sync, copies of step t
+    overlap the kernels of its neighbours through the two staging slots): every step's host result matches the
+    oracle and the cache ends bit-exact.  The slot stride is fixed by the staging buffer, not by a step's token
+    count, so a small step after a large one cannot land inside the region the large one still uses."""
+    import torch
+    from oracle.block_causal import OracleSession, attend
+    rng = np.random.default_rng(2025)
+    dev = torch.device("cuda", 0)
+    Hq, Hkv, D = 8, 2, 128
+    units = [256, 40, 200, 7, 256, 1, 130, 64]
+    L0 = 700
+    c = _cache("bf16", Hq, Hkv, D, 64, L0 + sum(units), max_q=1024)
+    sid = c.session_open()
+    sess = OracleSession(Hkv, D)
+    k0, v0 = _mk(rng, "bf16", L0, Hkv, D), _mk(rng, "bf16", L0, Hkv, D)
+    c.kv_append([sid], [0, L0], _torch_of(k0, dev), _torch_of(v0, dev))
+    sess.append(k0, v0)
+    pin = lambda a: torch.from_numpy(a.view(np.uint16).copy()).view(torch.bfloat16).pin_memory()
+    staging = torch.empty(c.step_staging_bytes(max(units)), dtype=torch.uint8, device=dev)
+    scale = 1.0 / math.sqrt(D)
+    host, refs = [], []
+    for n in units:
+        q, k, v = _mk(rng, "bf16", n, Hq, D), _mk(rng, "bf16", n, Hkv, D), _mk(rng, "bf16", n, Hkv, D)
+        sess.append(k, v)
+        refs.append(attend(sess, q, scale, 1, want_abs=True))
+        host.append((pin(q), pin(k), pin(v), torch.full((n, Hq, D), float("nan"), dtype=torch.bfloat16).pin_memory()))
+    torch.cuda.synchronize()
+    for n, (qh, kh, vh, oh) in zip(units, host):
+        c.stream_step_host([sid], [0, n], qh, kh, vh, oh, staging, scale)       # no sync between steps
+    c.stream_host_join()
+    torch.cuda.synchronize()
+    for i, (n, (qh, kh, vh, oh), (o_ref, l_ref, a_ref)) in enumerate(zip(units, host, refs)):
+        o = oh.float().numpy().astype(np.float64)
+        d = o - o_ref
+        viol = (np.abs(d) - bf16_error_bound(o_ref, o, a_ref)).max()
+        print(f"[parity] host step {i} n={n}: max_abs={np.abs(d).max():.3e} mean_abs={np.abs(d).mean():.3e} bound_viol={viol:.3e}")
+        assert np.isfinite(o).all()
+        assert np.abs(d).max() <= 1e-2 and np.abs(d).mean() <= 1e-3 and viol <= 0
+    T = c.session_info(sid)[0]
+    assert T == L0 + sum(units)
+    kg = torch.empty((T, Hkv, D), dtype=torch.bfloat16, device=dev); vg = torch.empty_like(kg)
+    c.kv_gather(sid, 0, T, kg, vg)
+    torch.cuda.synchronize()
+    k_all = np.concatenate([k0] + [_numpy_of(h[1]) for h in host]); v_all = np.concatenate([v0] + [_numpy_of(h[2]) for h in host])
+    assert np.array_equal(_numpy_of(kg).view(np.uint16), k_all.view(np.uint16))
+    assert np.array_equal(_numpy_of(vg).view(np.uint16), v_all.view(np.uint16))
