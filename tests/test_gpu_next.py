@@ -415,3 +415,34 @@ def test_stream_step_host_ragged_units_back_to_back():
     k_all = np.concatenate([k0] + [_numpy_of(h[1]) for h in host]); v_all = np.concatenate([v0] + [_numpy_of(h[2]) for h in host])
     assert np.array_equal(_numpy_of(kg).view(np.uint16), k_all.view(np.uint16))
     assert np.array_equal(_numpy_of(vg).view(np.uint16), v_all.view(np.uint16))
+
+
+# ------------------------------------------------------------------------------------------ generic kernel, shape space
+def _generic_cases():
+    rng = np.random.default_rng([2606, 25041, 31])
+    out = []
+    for i in range(32):
+        Hkv = int(rng.choice([1, 2, 3, 4])); G = int(rng.choice([1, 2, 3, 4, 8]))
+        D = int(rng.choice([8, 16, 24, 32, 40, 64, 72, 96, 128, 160, 192, 256])); P = int(rng.choice([1, 4, 16, 32, 64, 128]))
+        hist = [int(x) for x in rng.integers(1, 300, size=int(rng.integers(1, 4)))]
+        qb = [int(x) for x in rng.choice([1, 2, 3, 7, 16, 33, 64, 100], size=int(rng.integers(1, 4)))]
+        out.append(dict(idx=i, dt="fp32" if i % 3 else "bf16", Hq=Hkv * G, Hkv=Hkv, D=D, P=P, hist=hist, qb=qb,
+                        mode=["two_calls", "fused", "one_shot"][i % 3 if i % 2 else (i // 2) % 3],
+                        p_text=float(rng.choice([0.0, 0.3, 1.0]))))
+    return out
+
+
+@pytest.mark.parametrize("case", _generic_cases(), ids=lambda c: f"{c['idx']}_{c['dt']}_D{c['D']}_P{c['P']}_{c['mode']}")
+def test_generic_kernel_shape_space(case):
+    """The CUDA-core kernel over its own shape space (head_dim 8-256, pages of 1-128 tokens, group sizes incl. 3, both
+    dtypes, the three call modes, text share 0-100 %): fp32 within the 1e-5 contract, bf16 within the bf16 gates."""
+    from paper_2606_25041_b200 import WS_FLAG_FORCE_SIMT
+    o, l, o_ref, l_ref, a_ref, plans = _text_causal_case(case["dt"], case["Hq"], case["Hkv"], case["D"], case["P"], case["hist"],
+                                                         case["qb"], seed=3000 + case["idx"], mode=case["mode"],
+                                                         p_text=case["p_text"], flags=WS_FLAG_FORCE_SIMT)
+    assert all(p["used_tensor_core_kernel"] == 0 for p in plans)
+    if case["dt"] == "fp32":
+        print(f"[parity] generic fp32 {case}: max_abs={np.abs(o - o_ref).max():.3e} lse_max={np.abs(l - l_ref).max():.3e}")
+        assert np.isfinite(o).all() and np.abs(o - o_ref).max() <= 1e-5 and np.abs(l - l_ref).max() <= 1e-5
+    else:
+        _gate_bf16(o, l, o_ref, l_ref, a_ref, f"generic bf16 {case}")
